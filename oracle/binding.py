@@ -1,0 +1,201 @@
+"""ctypes binding of the CPU oracle (oracle/qmc_oracle.c).
+
+TEST INFRASTRUCTURE.  Only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this.  It imports nothing from
+the CUDA package; it takes any object with the attribute names of
+`workloads.SystemDesc` (plain numpy arrays).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import threading
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libqmc_oracle.so")
+_SRC = os.path.join(_HERE, "qmc_oracle.c")
+_lock = threading.Lock()
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc -O2 (no fast-math, no contraction)."""
+    hdr = os.path.join(_HERE, "qmc_oracle.h")
+    stale = (not os.path.exists(_SO)) or any(os.path.getmtime(f) > os.path.getmtime(_SO) for f in (_SRC, hdr))
+    if force or stale:
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fPIC", "-shared",
+                               "-o", _SO, _SRC, "-lm"])
+    return _SO
+
+
+class _Desc(C.Structure):
+    _fields_ = [
+        ("n_atoms", C.c_int32), ("atom_xyz", C.c_void_p), ("atom_Z", C.c_void_p),
+        ("n_up", C.c_int32), ("n_dn", C.c_int32),
+        ("n_ao", C.c_int32), ("ao_atom", C.c_void_p), ("ao_n", C.c_void_p), ("ao_l", C.c_void_p),
+        ("ao_m", C.c_void_p), ("ao_zeta", C.c_void_p), ("ao_norm", C.c_void_p),
+        ("n_mo", C.c_int32), ("mo_coeff", C.c_void_p),
+        ("n_det", C.c_int32), ("det_up", C.c_void_p), ("det_dn", C.c_void_p), ("ci_coeff", C.c_void_p),
+        ("jastrow_a_par", C.c_double), ("jastrow_a_anti", C.c_double), ("jastrow_b", C.c_double),
+    ]
+
+
+def lib():
+    global _lib
+    with _lock:
+        if _lib is None:
+            build()
+            L = C.CDLL(_SO)
+            L.oracle_sto_norm.restype = C.c_double
+            L.oracle_sto_norm.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double]
+            L.oracle_det_inv.restype = C.c_double
+            L.oracle_det_inv.argtypes = [C.c_int, C.c_void_p, C.c_void_p]
+            L.oracle_psi_plain.restype = C.c_double
+            L.oracle_psi_plain.argtypes = [C.c_void_p, C.c_void_p]
+            L.oracle_ao_eval.restype = None
+            L.oracle_ao_eval.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+            L.oracle_local_energy.restype = C.c_int
+            L.oracle_local_energy.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64,
+                                              C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+            L.oracle_philox4x32_10.restype = None
+            L.oracle_philox4x32_10.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+            L.oracle_walker_draws.restype = None
+            L.oracle_walker_draws.argtypes = [C.c_uint64, C.c_int64, C.c_uint64, C.c_int, C.c_void_p, C.c_void_p]
+            L.oracle_metropolis.restype = C.c_int
+            L.oracle_metropolis.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64,
+                                            C.c_double, C.c_int32, C.c_uint64, C.c_uint64,
+                                            C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+            L.oracle_batch_stats.restype = None
+            L.oracle_batch_stats.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+            _lib = L
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data
+
+
+class OracleSystem:
+    """Holds contiguous copies of the description arrays + the C struct."""
+
+    def __init__(self, d):
+        f64 = lambda a: np.ascontiguousarray(a, np.float64)
+        i32 = lambda a: np.ascontiguousarray(a, np.int32)
+        self.n_up, self.n_dn = int(d.n_up), int(d.n_dn)
+        self.n_e = self.n_up + self.n_dn
+        self._keep = dict(
+            atom_xyz=f64(d.atom_xyz), atom_Z=f64(d.atom_Z), ao_atom=i32(d.ao_atom), ao_n=i32(d.ao_n),
+            ao_l=i32(d.ao_l), ao_m=i32(d.ao_m), ao_zeta=f64(d.ao_zeta),
+            ao_norm=None if d.ao_norm is None else f64(d.ao_norm), mo_coeff=f64(d.mo_coeff),
+            det_up=i32(d.det_up), det_dn=i32(d.det_dn), ci_coeff=f64(d.ci_coeff))
+        k = self._keep
+        self.n_ao = int(k["ao_atom"].shape[0])
+        self.c = _Desc(int(k["atom_xyz"].shape[0]), _p(k["atom_xyz"]), _p(k["atom_Z"]), self.n_up, self.n_dn,
+                       self.n_ao, _p(k["ao_atom"]), _p(k["ao_n"]), _p(k["ao_l"]), _p(k["ao_m"]),
+                       _p(k["ao_zeta"]), _p(k["ao_norm"]), int(k["mo_coeff"].shape[1]), _p(k["mo_coeff"]),
+                       int(k["ci_coeff"].shape[0]), _p(k["det_up"]), _p(k["det_dn"]), _p(k["ci_coeff"]),
+                       float(d.jastrow_a_par), float(d.jastrow_a_anti), float(d.jastrow_b))
+        self.ref = C.addressof(self.c)
+
+
+def _ranges(M, n):
+    n = max(1, min(n, M))
+    edges = np.linspace(0, M, n + 1).astype(np.int64)
+    return [(int(edges[i]), int(edges[i + 1])) for i in range(n) if edges[i + 1] > edges[i]]
+
+
+def sto_norm(n, l, m, zeta):
+    return lib().oracle_sto_norm(n, l, m, zeta)
+
+
+def det_inv(A):
+    A = np.ascontiguousarray(A, np.float64)
+    n = A.shape[0]
+    inv = np.empty_like(A)
+    d = lib().oracle_det_inv(n, _p(A), _p(inv))
+    return d, inv
+
+
+def ao_eval(sysd: OracleSystem, ao: int, xyz):
+    xyz = np.ascontiguousarray(xyz, np.float64)
+    out = np.empty(5)
+    lib().oracle_ao_eval(sysd.ref, ao, _p(xyz), _p(out))
+    return out
+
+
+def psi_plain(sysd: OracleSystem, r_aos):
+    """r_aos: [n_e,3] one walker."""
+    r = np.ascontiguousarray(r_aos, np.float64)
+    return lib().oracle_psi_plain(sysd.ref, _p(r))
+
+
+def local_energy(sysd: OracleSystem, r_soa, threads: int = 1, parts: bool = False):
+    """r_soa: float64 [n_e,3,M].  Returns logpsi, sign, eloc[, parts[M,4]]."""
+    r = np.ascontiguousarray(r_soa, np.float64)
+    M = r.shape[2]
+    lp, sg, el = np.empty(M), np.empty(M), np.empty(M)
+    pt = np.empty((M, 4)) if parts else None
+    L = lib()
+
+    def run(rng):
+        rc = L.oracle_local_energy(sysd.ref, _p(r), M, rng[0], rng[1], _p(lp), _p(sg), _p(el), _p(pt))
+        assert rc == 0
+
+    rs = _ranges(M, threads)
+    if len(rs) == 1:
+        run(rs[0])
+    else:
+        with ThreadPoolExecutor(len(rs)) as ex:
+            list(ex.map(run, rs))
+    return (lp, sg, el, pt) if parts else (lp, sg, el)
+
+
+def philox(ctr, key):
+    c = np.ascontiguousarray(ctr, np.uint32)
+    k = np.ascontiguousarray(key, np.uint32)
+    out = np.empty(4, np.uint32)
+    lib().oracle_philox4x32_10(_p(c), _p(k), _p(out))
+    return out
+
+
+def walker_draws(seed, w, sweep, n_coord):
+    z = np.empty(n_coord + 1)
+    u = C.c_double()
+    lib().oracle_walker_draws(seed, w, sweep, n_coord, _p(z), C.addressof(u))
+    return z[:n_coord].copy(), u.value
+
+
+def metropolis(sysd: OracleSystem, r_soa, step, n_sweeps, seed, sweep_offset=0, threads: int = 1,
+               want_eloc_acc: bool = False):
+    """Returns dict(r, logpsi, sign, accept[n_sweeps,M], margin[n_sweeps,M], eloc_acc)."""
+    r = np.array(r_soa, np.float64, order="C", copy=True)
+    M = r.shape[2]
+    lp, sg = np.empty(M), np.empty(M)
+    acc = np.zeros((n_sweeps, M), np.uint8)
+    mg = np.zeros((n_sweeps, M))
+    ea = np.zeros(M) if want_eloc_acc else None
+    L = lib()
+
+    def run(rng):
+        rc = L.oracle_metropolis(sysd.ref, _p(r), M, rng[0], rng[1], step, n_sweeps, seed, sweep_offset,
+                                 _p(lp), _p(sg), _p(acc), _p(mg), _p(ea))
+        assert rc == 0
+
+    rs = _ranges(M, threads)
+    if len(rs) == 1:
+        run(rs[0])
+    else:
+        with ThreadPoolExecutor(len(rs)) as ex:
+            list(ex.map(run, rs))
+    return dict(r=r, logpsi=lp, sign=sg, accept=acc, margin=mg, eloc_acc=ea)
+
+
+def batch_stats(x):
+    x = np.ascontiguousarray(x, np.float64)
+    m, s = C.c_double(), C.c_double()
+    lib().oracle_batch_stats(_p(x), x.shape[0], C.addressof(m), C.addressof(s))
+    return m.value, s.value

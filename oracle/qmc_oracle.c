@@ -1,0 +1,506 @@
+/* qmc_oracle.c -- plain float64 CPU oracle (see qmc_oracle.h: test
+ * infrastructure only; shares nothing with the CUDA path).
+ *
+ * Build: gcc -O2 -std=c11 -fPIC -shared -o libqmc_oracle.so qmc_oracle.c -lm
+ * (no -ffast-math).  Citations: PAPER.md:<line> of /root/reference/PAPER.md.
+ */
+#include "qmc_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORACLE_PI 3.14159265358979323846
+
+/* ------------------------------------------------------------------ */
+/* Atomic orbitals: phi = N * S_lm(d) * r^k * exp(-zeta r), */
+/* k = n-1-l (reading Q3), S_lm real solid harmonics in the order       */
+/* l=0:{1}; l=1:{x,y,z}; l=2:{xy,yz,zx,x^2-y^2,2z^2-x^2-y^2}.           */
+/* ------------------------------------------------------------------ */
+
+static double factorial(int n) {
+  double f = 1.0;
+  for (int i = 2; i <= n; ++i) f *= (double)i;
+  return f;
+}
+
+double oracle_sto_norm(int n, int l, int m, double zeta) {
+  /* radial: (2 zeta)^(n+1/2) / sqrt((2n)!) ; angular: real spherical harmonic constant */
+  double radial = pow(2.0 * zeta, (double)n + 0.5) / sqrt(factorial(2 * n));
+  double ang = 0.0;
+  if (l == 0) ang = 1.0 / (2.0 * sqrt(ORACLE_PI));
+  else if (l == 1) ang = sqrt(3.0 / (4.0 * ORACLE_PI));
+  else if (l == 2) {
+    if (m <= 2) ang = 0.5 * sqrt(15.0 / ORACLE_PI);
+    else if (m == 3) ang = 0.25 * sqrt(15.0 / ORACLE_PI);
+    else ang = 0.25 * sqrt(5.0 / ORACLE_PI);
+  }
+  return radial * ang;
+}
+
+/* S, its gradient and its three pure second derivatives, written out. */
+static void solid_harmonic(int l, int m, double x, double y, double z, double *S, double g[3],
+                           double h[3]) {
+  *S = 0.0;
+  g[0] = g[1] = g[2] = 0.0;
+  h[0] = h[1] = h[2] = 0.0;
+  if (l == 0) {
+    *S = 1.0;
+  } else if (l == 1) {
+    if (m == 0) { *S = x; g[0] = 1.0; }
+    if (m == 1) { *S = y; g[1] = 1.0; }
+    if (m == 2) { *S = z; g[2] = 1.0; }
+  } else if (l == 2) {
+    if (m == 0) { *S = x * y; g[0] = y; g[1] = x; }
+    if (m == 1) { *S = y * z; g[1] = z; g[2] = y; }
+    if (m == 2) { *S = z * x; g[0] = z; g[2] = x; }
+    if (m == 3) { *S = x * x - y * y; g[0] = 2.0 * x; g[1] = -2.0 * y; h[0] = 2.0; h[1] = -2.0; }
+    if (m == 4) {
+      *S = 2.0 * z * z - x * x - y * y;
+      g[0] = -2.0 * x; g[1] = -2.0 * y; g[2] = 4.0 * z;
+      h[0] = -2.0; h[1] = -2.0; h[2] = 4.0;
+    }
+  }
+}
+
+void oracle_ao_eval(const oracle_system_desc_t *s, int ao, const double *xyz, double *out5) {
+  int a = s->ao_atom[ao], n = s->ao_n[ao], l = s->ao_l[ao], m = s->ao_m[ao];
+  double zeta = s->ao_zeta[ao];
+  double N = s->ao_norm ? s->ao_norm[ao] : oracle_sto_norm(n, l, m, zeta);
+  double d[3];
+  for (int c = 0; c < 3; ++c) d[c] = xyz[c] - s->atom_xyz[3 * a + c];
+  double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+  int k = n - 1 - l;
+
+  double S, gS[3], hS[3];
+  solid_harmonic(l, m, d[0], d[1], d[2], &S, gS, hS);
+
+  /* radial factor f(r) = r^k e^{-zeta r} and its first two derivatives, term by term */
+  double e = exp(-zeta * r);
+  double rk = pow(r, (double)k);                         /* r^k       */
+  double rk1 = (k >= 1) ? pow(r, (double)(k - 1)) : 0.0; /* r^(k-1)   */
+  double rk2 = (k >= 2) ? pow(r, (double)(k - 2)) : 0.0; /* r^(k-2)   */
+  double f = rk * e;
+  double f1 = ((double)k * rk1 - zeta * rk) * e;
+  double f2 = ((double)(k * (k - 1)) * rk2 - 2.0 * (double)k * zeta * rk1 + zeta * zeta * rk) * e;
+
+  /* grad f = f' d/r ; lap f = f'' + 2 f'/r */
+  double gf[3];
+  for (int c = 0; c < 3; ++c) gf[c] = f1 * d[c] / r;
+  double lapf = f2 + 2.0 * f1 / r;
+
+  /* product rule: grad(S f) = gS f + S gf ; lap(S f) = lapS f + 2 gS.gf + S lapf */
+  double lapS = hS[0] + hS[1] + hS[2];
+  double dot = gS[0] * gf[0] + gS[1] * gf[1] + gS[2] * gf[2];
+  out5[0] = N * S * f;
+  for (int c = 0; c < 3; ++c) out5[1 + c] = N * (gS[c] * f + S * gf[c]);
+  out5[4] = N * (lapS * f + 2.0 * dot + S * lapf);
+}
+
+/* ------------------------------------------------------------------ */
+/* Partial-pivot LU: determinant and inverse   */
+/* ------------------------------------------------------------------ */
+
+double oracle_det_inv(int n, const double *A, double *inv) {
+  if (n <= 0) return 1.0;
+  double *lu = (double *)malloc(sizeof(double) * (size_t)n * (size_t)n);
+  int *perm = (int *)malloc(sizeof(int) * (size_t)n);
+  memcpy(lu, A, sizeof(double) * (size_t)n * (size_t)n);
+  for (int i = 0; i < n; ++i) perm[i] = i;
+  double det = 1.0;
+  for (int k = 0; k < n; ++k) {
+    int p = k;
+    double best = fabs(lu[k * n + k]);
+    for (int i = k + 1; i < n; ++i)
+      if (fabs(lu[i * n + k]) > best) { best = fabs(lu[i * n + k]); p = i; }
+    if (p != k) {
+      for (int j = 0; j < n; ++j) { double t = lu[k * n + j]; lu[k * n + j] = lu[p * n + j]; lu[p * n + j] = t; }
+      int t = perm[k]; perm[k] = perm[p]; perm[p] = t;
+      det = -det;
+    }
+    double piv = lu[k * n + k];
+    det *= piv;
+    if (piv == 0.0) continue; /* singular: det = 0, inverse undefined (inf/nan follow) */
+    for (int i = k + 1; i < n; ++i) {
+      lu[i * n + k] /= piv;
+      double lik = lu[i * n + k];
+      for (int j = k + 1; j < n; ++j) lu[i * n + j] -= lik * lu[k * n + j];
+    }
+  }
+  if (inv) {
+    /* solve A x = e_c for every unit vector: P A = L U */
+    double *y = (double *)malloc(sizeof(double) * (size_t)n);
+    for (int c = 0; c < n; ++c) {
+      for (int i = 0; i < n; ++i) {
+        double v = (perm[i] == c) ? 1.0 : 0.0;
+        for (int j = 0; j < i; ++j) v -= lu[i * n + j] * y[j];
+        y[i] = v;
+      }
+      for (int i = n - 1; i >= 0; --i) {
+        double v = y[i];
+        for (int j = i + 1; j < n; ++j) v -= lu[i * n + j] * inv[j * n + c];
+        inv[i * n + c] = v / lu[i * n + i];
+      }
+    }
+    free(y);
+  }
+  free(lu);
+  free(perm);
+  return det;
+}
+
+/* ------------------------------------------------------------------ */
+/* Pade e-e Jastrow (D.1; cusps C.1):       */
+/* K(r) = w0 r / (1 + w r), w0 = a_par (same spin), a_anti (opposite).  */
+/* ------------------------------------------------------------------ */
+
+static int spin_of(const oracle_system_desc_t *s, int i) { return i < s->n_up ? 0 : 1; }
+
+/* J, grad_i J [n_e][3], lap J (sum over all electrons), pair loop. r is AoS [n_e][3]. */
+static void jastrow_all(const oracle_system_desc_t *s, const double *r, double *J, double *gJ,
+                        double *lapJ) {
+  int ne = s->n_up + s->n_dn;
+  *J = 0.0;
+  *lapJ = 0.0;
+  for (int i = 0; i < 3 * ne; ++i) gJ[i] = 0.0;
+  for (int i = 0; i < ne; ++i)
+    for (int j = i + 1; j < ne; ++j) {
+      double a = (spin_of(s, i) == spin_of(s, j)) ? s->jastrow_a_par : s->jastrow_a_anti;
+      double b = s->jastrow_b;
+      double d[3];
+      for (int c = 0; c < 3; ++c) d[c] = r[3 * i + c] - r[3 * j + c];
+      double rij = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+      double den = 1.0 + b * rij;
+      double u = a * rij / den;
+      double u1 = a / (den * den);
+      double u2 = -2.0 * a * b / (den * den * den);
+      *J += u;
+      for (int c = 0; c < 3; ++c) {
+        gJ[3 * i + c] += u1 * d[c] / rij;
+        gJ[3 * j + c] -= u1 * d[c] / rij;
+      }
+      /* lap_i K + lap_j K = 2 (u'' + 2 u'/r) */
+      *lapJ += 2.0 * (u2 + 2.0 * u1 / rij);
+    }
+}
+
+/* ------------------------------------------------------------------ */
+/* AO -> MO: phi_alpha = sum_beta C[beta][alpha] ao_beta  */
+/* mo[i][alpha][q], q = value, d/dx, d/dy, d/dz, laplacian              */
+/* ------------------------------------------------------------------ */
+
+static void mo_all(const oracle_system_desc_t *s, const double *r, double *mo) {
+  int ne = s->n_up + s->n_dn;
+  double ao[5];
+  for (int i = 0; i < ne * s->n_mo * 5; ++i) mo[i] = 0.0;
+  for (int i = 0; i < ne; ++i)
+    for (int beta = 0; beta < s->n_ao; ++beta) {
+      oracle_ao_eval(s, beta, r + 3 * i, ao);
+      for (int alpha = 0; alpha < s->n_mo; ++alpha)
+        for (int q = 0; q < 5; ++q)
+          mo[(i * s->n_mo + alpha) * 5 + q] += s->mo_coeff[beta * s->n_mo + alpha] * ao[q];
+    }
+}
+
+double oracle_psi_plain(const oracle_system_desc_t *s, const double *r) {
+  int ne = s->n_up + s->n_dn, nmo = s->n_mo;
+  double *mo = (double *)malloc(sizeof(double) * (size_t)(ne * nmo * 5 + 1));
+  double *gJ = (double *)malloc(sizeof(double) * (size_t)(3 * ne + 1));
+  double *A = (double *)malloc(sizeof(double) * (size_t)(ne * ne + 1));
+  mo_all(s, r, mo);
+  double J, lapJ;
+  jastrow_all(s, r, &J, gJ, &lapJ);
+  double sigma = 0.0;
+  for (int n = 0; n < s->n_det; ++n) {
+    double D[2];
+    for (int sp = 0; sp < 2; ++sp) {
+      int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
+      const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
+      for (int i = 0; i < ns; ++i)
+        for (int j = 0; j < ns; ++j) A[i * ns + j] = mo[((e0 + i) * nmo + lst[j]) * 5 + 0];
+      D[sp] = oracle_det_inv(ns, A, NULL);
+    }
+    sigma += s->ci_coeff[n] * D[0] * D[1];
+  }
+  free(mo); free(gJ); free(A);
+  return exp(J) * sigma;
+}
+
+/* ------------------------------------------------------------------ */
+/* Local energy of one walker (AoS r[n_e][3]).                          */
+/* F.1, F.2 (:295), F.3 (:300), F.4 (:304), G.7 (:386),  */
+/* eq. 1 (:21).                                                         */
+/* ------------------------------------------------------------------ */
+
+static void local_energy_one(const oracle_system_desc_t *s, const double *r, double *work,
+                             double *logpsi, double *sign, double *eloc, double *parts) {
+  int ne = s->n_up + s->n_dn, nmo = s->n_mo;
+  double *mo = work;                 /* ne*nmo*5 */
+  double *gJ = mo + ne * nmo * 5;    /* 3 ne */
+  double *gS = gJ + 3 * ne;          /* 3 ne: grad_i Sigma */
+  double *A = gS + 3 * ne;           /* ne*ne */
+  double *Ai = A + ne * ne;          /* ne*ne */
+  double *gdet = Ai + ne * ne;       /* 3 ne: grad_i D / D of the current determinant */
+
+  mo_all(s, r, mo);
+  double J, lapJ;
+  jastrow_all(s, r, &J, gJ, &lapJ);
+
+  double sigma = 0.0, lapS = 0.0;
+  for (int i = 0; i < 3 * ne; ++i) gS[i] = 0.0;
+  for (int n = 0; n < s->n_det; ++n) {
+    double D[2], t[2];
+    for (int sp = 0; sp < 2; ++sp) {
+      int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
+      const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
+      /* rows = electrons, columns = orbitals (reading Q7) */
+      for (int i = 0; i < ns; ++i)
+        for (int j = 0; j < ns; ++j) A[i * ns + j] = mo[((e0 + i) * nmo + lst[j]) * 5 + 0];
+      D[sp] = oracle_det_inv(ns, A, Ai);
+      t[sp] = 0.0;
+      for (int i = 0; i < ns; ++i) {
+        /* G.2: Tr(A^-1 dA/dx_i) = sum_k A^-1[k][i] d phi_k(r_i)/dx_i ; G.7 likewise with lap */
+        for (int c = 0; c < 3; ++c) {
+          double g = 0.0;
+          for (int k = 0; k < ns; ++k) g += Ai[k * ns + i] * mo[((e0 + i) * nmo + lst[k]) * 5 + 1 + c];
+          gdet[3 * (e0 + i) + c] = g;
+        }
+        for (int k = 0; k < ns; ++k) t[sp] += Ai[k * ns + i] * mo[((e0 + i) * nmo + lst[k]) * 5 + 4];
+      }
+    }
+    double w = s->ci_coeff[n] * D[0] * D[1];
+    sigma += w;
+    for (int i = 0; i < 3 * ne; ++i) gS[i] += w * gdet[i];   /* F.2 */
+    lapS += w * (t[0] + t[1]);                               /* F.4; cross term vanishes (no coordinate in both spins) */
+  }
+
+  /* F.1 with script-J = e^J (reading Q5): lap Psi / Psi = lapJ + |gJ|^2 + 2 gJ.gS/S + lapS/S */
+  double gJ2 = 0.0, cross = 0.0;
+  for (int i = 0; i < 3 * ne; ++i) { gJ2 += gJ[i] * gJ[i]; cross += gJ[i] * gS[i]; }
+  double lap_over_psi = lapJ + gJ2 + 2.0 * cross / sigma + lapS / sigma;
+  double kinetic = -0.5 * lap_over_psi;
+
+  /* potential, eq. 1 */
+  double vee = 0.0, ven = 0.0, vnn = 0.0;
+  for (int i = 0; i < ne; ++i)
+    for (int j = i + 1; j < ne; ++j) {
+      double dx = r[3 * i] - r[3 * j], dy = r[3 * i + 1] - r[3 * j + 1], dz = r[3 * i + 2] - r[3 * j + 2];
+      vee += 1.0 / sqrt(dx * dx + dy * dy + dz * dz);
+    }
+  for (int i = 0; i < ne; ++i)
+    for (int a = 0; a < s->n_atoms; ++a) {
+      double dx = r[3 * i] - s->atom_xyz[3 * a], dy = r[3 * i + 1] - s->atom_xyz[3 * a + 1],
+             dz = r[3 * i + 2] - s->atom_xyz[3 * a + 2];
+      ven -= s->atom_Z[a] / sqrt(dx * dx + dy * dy + dz * dz);
+    }
+  for (int a = 0; a < s->n_atoms; ++a)
+    for (int b = a + 1; b < s->n_atoms; ++b) {
+      double dx = s->atom_xyz[3 * a] - s->atom_xyz[3 * b], dy = s->atom_xyz[3 * a + 1] - s->atom_xyz[3 * b + 1],
+             dz = s->atom_xyz[3 * a + 2] - s->atom_xyz[3 * b + 2];
+      vnn += s->atom_Z[a] * s->atom_Z[b] / sqrt(dx * dx + dy * dy + dz * dz);
+    }
+
+  *logpsi = J + log(fabs(sigma));
+  *sign = (sigma > 0.0) ? 1.0 : ((sigma < 0.0) ? -1.0 : 0.0);
+  *eloc = kinetic + vee + ven + vnn;
+  if (parts) { parts[0] = kinetic; parts[1] = vee; parts[2] = ven; parts[3] = vnn; }
+}
+
+static size_t work_doubles(const oracle_system_desc_t *s) {
+  size_t ne = (size_t)(s->n_up + s->n_dn);
+  return ne * (size_t)s->n_mo * 5 + 9 * ne + 2 * ne * ne + 16;
+}
+
+static void gather_walker(const double *r, int64_t M, int64_t w, int ne, double *aos) {
+  for (int i = 0; i < ne; ++i)
+    for (int c = 0; c < 3; ++c) aos[3 * i + c] = r[((size_t)i * 3 + (size_t)c) * (size_t)M + (size_t)w];
+}
+
+int oracle_local_energy(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
+                        int64_t w1, double *logpsi, double *sign, double *eloc, double *parts) {
+  int ne = s->n_up + s->n_dn;
+  double *work = (double *)malloc(sizeof(double) * work_doubles(s));
+  double *pos = (double *)malloc(sizeof(double) * (size_t)(3 * ne + 1));
+  if (!work || !pos) return -1;
+  for (int64_t w = w0; w < w1; ++w) {
+    gather_walker(r, M, w, ne, pos);
+    double lp, sg, el;
+    local_energy_one(s, pos, work, &lp, &sg, &el, parts ? parts + 4 * w : NULL);
+    if (logpsi) logpsi[w] = lp;
+    if (sign) sign[w] = sg;
+    if (eloc) eloc[w] = el;
+  }
+  free(work); free(pos);
+  return 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* Philox4x32-10 counter-based generator (reading Q9)                   */
+/* ------------------------------------------------------------------ */
+
+void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+  uint32_t k0 = key[0], k1 = key[1];
+  for (int round = 0; round < 10; ++round) {
+    uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c0;
+    uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c2;
+    uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    uint32_t n0 = hi1 ^ c1 ^ k0;
+    uint32_t n1 = lo1;
+    uint32_t n2 = hi0 ^ c3 ^ k1;
+    uint32_t n3 = lo0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* two words -> u in (0,1): ((hi*2^32 + lo) >> 11 + 1/2) * 2^-53 */
+static double uniform53(uint32_t hi, uint32_t lo) {
+  uint64_t v = (((uint64_t)hi << 32) | (uint64_t)lo) >> 11;
+  return ((double)v + 0.5) * (1.0 / 9007199254740992.0);
+}
+
+void oracle_walker_draws(uint64_t seed, int64_t w, uint64_t sweep, int n_coord, double *z,
+                         double *u_accept) {
+  uint32_t key[2] = {(uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32)};
+  uint32_t ctr[4], out[4];
+  ctr[0] = (uint32_t)((uint64_t)w & 0xFFFFFFFFu);
+  ctr[1] = (uint32_t)(sweep & 0xFFFFFFFFu);
+  ctr[3] = (uint32_t)((uint64_t)w >> 32);
+  int n_pairs = (n_coord + 1) / 2;
+  for (int j = 0; j < n_pairs; ++j) {
+    ctr[2] = (uint32_t)j;
+    oracle_philox4x32_10(ctr, key, out);
+    double u1 = uniform53(out[0], out[1]);
+    double u2 = uniform53(out[2], out[3]);
+    /* Box-Muller */
+    double rho = sqrt(-2.0 * log(u1));
+    double theta = 2.0 * ORACLE_PI * u2;
+    if (z) {
+      z[2 * j] = rho * cos(theta);
+      if (2 * j + 1 < n_coord) z[2 * j + 1] = rho * sin(theta);
+    }
+  }
+  if (u_accept) {
+    ctr[2] = 0xFFFFFFFFu;
+    oracle_philox4x32_10(ctr, key, out);
+    *u_accept = uniform53(out[0], out[1]);
+  }
+}
+
+/* ------------------------------------------------------------------ */
+/* log|Psi| and sign from the plain definition (eq. 4)     */
+/* ------------------------------------------------------------------ */
+
+static void logpsi_one(const oracle_system_desc_t *s, const double *r, double *work, double *logpsi,
+                       double *sign) {
+  int ne = s->n_up + s->n_dn, nmo = s->n_mo;
+  double *mo = work;              /* ne*nmo (values only) */
+  double *A = mo + ne * nmo * 5;  /* ne*ne, same offsets as local_energy_one's layout */
+  double ao[5];
+  for (int i = 0; i < ne * nmo; ++i) mo[i] = 0.0;
+  for (int i = 0; i < ne; ++i)
+    for (int beta = 0; beta < s->n_ao; ++beta) {
+      oracle_ao_eval(s, beta, r + 3 * i, ao);
+      for (int alpha = 0; alpha < nmo; ++alpha) mo[i * nmo + alpha] += s->mo_coeff[beta * nmo + alpha] * ao[0];
+    }
+  double J = 0.0;
+  for (int i = 0; i < ne; ++i)
+    for (int j = i + 1; j < ne; ++j) {
+      double a = (spin_of(s, i) == spin_of(s, j)) ? s->jastrow_a_par : s->jastrow_a_anti;
+      double dx = r[3 * i] - r[3 * j], dy = r[3 * i + 1] - r[3 * j + 1], dz = r[3 * i + 2] - r[3 * j + 2];
+      double rij = sqrt(dx * dx + dy * dy + dz * dz);
+      J += a * rij / (1.0 + s->jastrow_b * rij);
+    }
+  double sigma = 0.0;
+  for (int n = 0; n < s->n_det; ++n) {
+    double D[2];
+    for (int sp = 0; sp < 2; ++sp) {
+      int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
+      const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
+      for (int i = 0; i < ns; ++i)
+        for (int j = 0; j < ns; ++j) A[i * ns + j] = mo[(e0 + i) * nmo + lst[j]];
+      D[sp] = oracle_det_inv(ns, A, NULL);
+    }
+    sigma += s->ci_coeff[n] * D[0] * D[1];
+  }
+  *logpsi = J + log(fabs(sigma));
+  *sign = (sigma > 0.0) ? 1.0 : ((sigma < 0.0) ? -1.0 : 0.0);
+}
+
+/* ------------------------------------------------------------------ */
+/* All-electron Metropolis (readings Q9, Q10)             */
+/* ------------------------------------------------------------------ */
+
+int oracle_metropolis(const oracle_system_desc_t *s, double *r, int64_t M, int64_t w0, int64_t w1,
+                      double step, int32_t n_sweeps, uint64_t seed, uint64_t sweep_offset,
+                      double *logpsi, double *sign, uint8_t *accept, double *margin,
+                      double *eloc_acc) {
+  int ne = s->n_up + s->n_dn, nc = 3 * ne;
+  double *work = (double *)malloc(sizeof(double) * work_doubles(s));
+  double *pos = (double *)malloc(sizeof(double) * (size_t)(nc + 1));
+  double *prop = (double *)malloc(sizeof(double) * (size_t)(nc + 1));
+  double *z = (double *)malloc(sizeof(double) * (size_t)(nc + 2));
+  if (!work || !pos || !prop || !z) return -1;
+  for (int64_t w = w0; w < w1; ++w) {
+    gather_walker(r, M, w, ne, pos);
+    double lp, sg;
+    logpsi_one(s, pos, work, &lp, &sg);
+    double acc_e = 0.0;
+    for (int32_t sw = 0; sw < n_sweeps; ++sw) {
+      double u;
+      oracle_walker_draws(seed, w, sweep_offset + (uint64_t)sw, nc, z, &u);
+      for (int q = 0; q < nc; ++q) prop[q] = pos[q] + step * z[q];
+      double lp2, sg2;
+      logpsi_one(s, prop, work, &lp2, &sg2);
+      double mg = 2.0 * (lp2 - lp) - log(u);
+      int ok = (log(u) < 2.0 * (lp2 - lp)) ? 1 : 0; /* false for NaN and for Psi' = 0 */
+      if (ok) {
+        for (int q = 0; q < nc; ++q) pos[q] = prop[q];
+        lp = lp2;
+        sg = sg2;
+      }
+      if (accept) accept[(size_t)sw * (size_t)M + (size_t)w] = (uint8_t)ok;
+      if (margin) margin[(size_t)sw * (size_t)M + (size_t)w] = mg;
+      if (eloc_acc) {
+        double l3, s3, el;
+        local_energy_one(s, pos, work, &l3, &s3, &el, NULL);
+        acc_e += el;
+      }
+    }
+    for (int i = 0; i < ne; ++i)
+      for (int c = 0; c < 3; ++c) r[((size_t)i * 3 + (size_t)c) * (size_t)M + (size_t)w] = pos[3 * i + c];
+    if (logpsi) logpsi[w] = lp;
+    if (sign) sign[w] = sg;
+    if (eloc_acc) eloc_acc[w] = acc_e;
+  }
+  free(work); free(pos); free(prop); free(z);
+  return 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* Batch statistics (eq. 3), Kahan-compensated             */
+/* ------------------------------------------------------------------ */
+
+void oracle_batch_stats(const double *x, int64_t M, double *mean, double *stderr_out) {
+  double sum = 0.0, comp = 0.0;
+  for (int64_t i = 0; i < M; ++i) {
+    double y = x[i] - comp, t = sum + y;
+    comp = (t - sum) - y;
+    sum = t;
+  }
+  double mu = sum / (double)M;
+  double s2 = 0.0;
+  comp = 0.0;
+  for (int64_t i = 0; i < M; ++i) {
+    double dlt = x[i] - mu;
+    double y = dlt * dlt - comp, t = s2 + y;
+    comp = (t - s2) - y;
+    s2 = t;
+  }
+  if (mean) *mean = mu;
+  if (stderr_out) *stderr_out = (M > 1) ? sqrt(s2 / (double)(M - 1) / (double)M) : 0.0;
+}

@@ -1,0 +1,92 @@
+/* qmc_oracle.h -- CPU oracle for the Slater-Jastrow Psi / E_L / Metropolis path.
+ *
+ * TEST INFRASTRUCTURE, NOT PRODUCT.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may load this library.  It
+ * shares no code, header, table or helper with the CUDA path
+ * (paper_2506_09743_b200/csrc, include/qmc.h); the struct below is declared
+ * here on its own.
+ *
+ * Everything is float64, long-hand loops, every determinant factored
+ * explicitly; no excitation tables, no combined one-body operator, no BLAS.
+ * Citations are PAPER.md:<line> (+ equation) of /root/reference/PAPER.md.
+ *
+ * Parity pins (tests/test_oracle_pins.py): hydrogenic closed forms for every
+ * harmonic (1s, 2s, 2p x3, 3d x5), He-like closed form with the Pade Jastrow,
+ * n-electron hydrogenic determinants (exact sum of orbital energies), central
+ * finite differences of the plain Psi, antisymmetry, Leibniz determinants,
+ * nuclear repulsion, cusp finiteness, Philox known answers, sampler moments.
+ * Unpinned by anything but those: absolute energies of the random-MO
+ * synthetic LiH / Li2 / CO configs (no physical reference exists for them).
+ */
+#ifndef QMC_ORACLE_H
+#define QMC_ORACLE_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct {
+  int32_t n_atoms;
+  const double *atom_xyz; /* [n_atoms][3] bohr */
+  const double *atom_Z;   /* [n_atoms] */
+  int32_t n_up, n_dn;     /* electrons 0..n_up-1 are spin-up */
+  int32_t n_ao;
+  const int32_t *ao_atom, *ao_n, *ao_l, *ao_m; /* per AO: centre, n, l, harmonic index */
+  const double *ao_zeta;  /* [n_ao] */
+  const double *ao_norm;  /* [n_ao] or NULL = standard normalisation */
+  int32_t n_mo;
+  const double *mo_coeff; /* [n_ao][n_mo] */
+  int32_t n_det;
+  const int32_t *det_up, *det_dn; /* [n_det][n_up], [n_det][n_dn] ordered MO columns */
+  const double *ci_coeff;         /* [n_det] */
+  double jastrow_a_par, jastrow_a_anti, jastrow_b;
+} oracle_system_desc_t;
+
+/* All pointers are HOST pointers.  Walker arrays are SoA [n_e][3][M]; the
+ * functions below process walkers w0 <= w < w1 only (so a caller can split a
+ * batch over threads) and index every per-walker array with the GLOBAL w. */
+
+/* STO normalisation, reading Q2 (PAPER.md:55 leaves N unspecified). */
+double oracle_sto_norm(int n, int l, int m, double zeta);
+
+/* One AO at one point: out = {phi, dphi/dx, dphi/dy, dphi/dz, lap phi}.  PAPER.md:55. */
+void oracle_ao_eval(const oracle_system_desc_t *s, int ao, const double *xyz, double *out5);
+
+/* Partial-pivot LU determinant and inverse of a row-major n x n matrix.
+ * inv may be NULL.  Returns det. */
+double oracle_det_inv(int n, const double *A, double *inv);
+
+/* Plain definition of eq. 4: e^J * sum_n d_n det(A_n^up) det(A_n^dn)
+ * for ONE walker given as AoS r[n_e][3].  Used for finite differences. */
+double oracle_psi_plain(const oracle_system_desc_t *s, const double *r);
+
+/* log|Psi|, sign, E_L = H Psi / Psi (eq. 1; F.1-F.4, G.7).
+ * parts, if non-NULL, receives [M][4] = {kinetic, V_ee, V_en, V_nn}. */
+int oracle_local_energy(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
+                        int64_t w1, double *logpsi, double *sign, double *eloc, double *parts);
+
+/* Philox4x32-10 (reading Q9). */
+void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+
+/* The proposal normals of walker w at absolute sweep index `sweep`:
+ * z[0..n_coord-1] (reading Q9), and the accept uniform. */
+void oracle_walker_draws(uint64_t seed, int64_t w, uint64_t sweep, int n_coord, double *z,
+                         double *u_accept);
+
+/* All-electron Metropolis (readings Q9, Q10).  r is updated in
+ * place.  accept [n_sweeps][M] (uint8) and margin [n_sweeps][M]
+ * (= 2*dlog|Psi| - log u, the quantity whose sign is the decision) may be
+ * NULL; eloc_acc [M] (sum over sweeps of E_L after each sweep) may be NULL. */
+int oracle_metropolis(const oracle_system_desc_t *s, double *r, int64_t M, int64_t w0, int64_t w1,
+                      double step, int32_t n_sweeps, uint64_t seed, uint64_t sweep_offset,
+                      double *logpsi, double *sign, uint8_t *accept, double *margin,
+                      double *eloc_acc);
+
+/* Mean and standard error of the mean (eq. 3), Kahan sums. */
+void oracle_batch_stats(const double *x, int64_t M, double *mean, double *stderr_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

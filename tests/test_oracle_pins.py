@@ -1,0 +1,552 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix
+(SURVEY.md 8(c) P1-P17).  CPU only."""
+import itertools
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import binding as ob
+from paper_2506_09743_b200 import workloads as wl
+from tests.helpers import atom_system, hydrogenic_set, soa
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+rng0 = np.random.default_rng(12345)
+
+
+def _rand_pos(M, n_e, scale=1.0, rmin=0.0, seed=0):
+    rng = np.random.default_rng(seed)
+    r = rng.standard_normal((M, n_e, 3)) * scale
+    if rmin > 0:
+        nrm = np.linalg.norm(r, axis=2, keepdims=True)
+        r = r * np.maximum(nrm, rmin) / nrm
+    return r
+
+
+# ---------------------------------------------------------------- P1, P2
+def test_P1_hydrogen_1s_exact():
+    d = atom_system(1, [(1, 0, 0, 1.0)], [[1.0]], 1, 0)
+    r = _rand_pos(200, 1, 2.0)
+    lp, sg, el = ob.local_energy(ob.OracleSystem(d), soa(r))
+    assert np.max(np.abs(el + 0.5)) < 1e-12
+    # normalised 1s: psi = e^{-r}/sqrt(pi)
+    rr = np.linalg.norm(r[:, 0], axis=1)
+    assert np.max(np.abs(lp - (-rr - 0.5 * math.log(math.pi)))) < 1e-13
+    assert np.all(sg == 1.0)
+
+
+@pytest.mark.parametrize("Z,zeta", [(1, 0.8), (2, 1.7), (3, 3.4)])
+def test_P2_hydrogenlike_wrong_zeta(Z, zeta):
+    d = atom_system(Z, [(1, 0, 0, zeta)], [[1.0]], 1, 0, xyz=(0.3, -0.2, 0.5))
+    r = _rand_pos(100, 1, 1.5, seed=1) + np.array([0.3, -0.2, 0.5])
+    lp, sg, el = ob.local_energy(ob.OracleSystem(d), soa(r))
+    rr = np.linalg.norm(r[:, 0] - np.array([0.3, -0.2, 0.5]), axis=1)
+    ref = -zeta ** 2 / 2 + (zeta - Z) / rr
+    assert np.max(np.abs(el - ref) / np.maximum(1, np.abs(ref))) < 1e-12
+
+
+# ---------------------------------------------------------------- P3, P4
+@pytest.mark.parametrize("Z", [1, 3])
+def test_P3_hydrogenic_2p_3d_every_harmonic(Z):
+    r = _rand_pos(50, 1, 3.0, rmin=0.05, seed=2)
+    for m in range(3):
+        d = atom_system(Z, [(2, 1, m, Z / 2)], [[1.0]], 1, 0)
+        _, _, el = ob.local_energy(ob.OracleSystem(d), soa(r))
+        assert np.max(np.abs(el + Z * Z / 8)) < 1e-11 * Z * Z
+    for m in range(5):
+        d = atom_system(Z, [(3, 2, m, Z / 3)], [[1.0]], 1, 0)
+        _, _, el = ob.local_energy(ob.OracleSystem(d), soa(r))
+        assert np.max(np.abs(el + Z * Z / 18)) < 1e-11 * Z * Z
+
+
+@pytest.mark.parametrize("Z", [1, 2])
+def test_P4_hydrogenic_2s_as_mo(Z):
+    # psi_2s ~ (2 - Z r) e^{-Z r/2} = 2*[1s-type, zeta Z/2] - Z*[2s-type r e^{-Z r /2}]
+    d = atom_system(Z, [(1, 0, 0, Z / 2), (2, 0, 0, Z / 2)], [[2.0], [-float(Z)]], 1, 0, norm=[1.0, 1.0])
+    r = _rand_pos(100, 1, 3.0, rmin=0.05, seed=3)
+    rr = np.linalg.norm(r[:, 0], axis=1)
+    keep = np.abs(2 - Z * rr) > 1e-2  # away from the radial node
+    _, _, el = ob.local_energy(ob.OracleSystem(d), soa(r))
+    assert np.max(np.abs(el[keep] + Z * Z / 8)) < 1e-10
+
+
+def test_3s_type_radial_power_two():
+    # k = 2 radial factor (3s-type AO r^2 e^{-zeta r}): E_L = -zeta^2/2 + (3 zeta - Z)/r - 3/r^2 ... closed form
+    # lap(r^2 e^{-z r}) / (r^2 e^{-z r}) = z^2 - 2 z (k+1)/r + k(k+1)/r^2 with k=2
+    Z, z = 1.0, 0.7
+    d = atom_system(Z, [(3, 0, 0, z)], [[1.0]], 1, 0)
+    r = _rand_pos(50, 1, 3.0, rmin=0.2, seed=4)
+    rr = np.linalg.norm(r[:, 0], axis=1)
+    ref = -0.5 * (z * z - 6 * z / rr + 6 / rr ** 2) - Z / rr
+    _, _, el = ob.local_energy(ob.OracleSystem(d), soa(r))
+    assert np.max(np.abs(el - ref) / np.maximum(1, np.abs(ref))) < 1e-12
+
+
+# ---------------------------------------------------------------- normalisation (Q2) by quadrature
+@pytest.mark.parametrize("n,l,m,zeta", [(1, 0, 0, 1.24), (2, 0, 0, 0.9), (2, 1, 0, 1.3), (2, 1, 2, 2.0),
+                                        (3, 2, 0, 1.1), (3, 2, 3, 0.8), (3, 2, 4, 1.7), (3, 2, 1, 1.0)])
+def test_sto_normalisation_integrates_to_one(n, l, m, zeta):
+    d = atom_system(1, [(n, l, m, zeta)], [[1.0]], 1, 0)
+    o = ob.OracleSystem(d)
+    # Gauss-Laguerre in r (weight e^{-2 zeta r} absorbed numerically), Gauss-Legendre x uniform in angles
+    xr, wr = np.polynomial.laguerre.laggauss(40)
+    rr = xr / (2 * zeta)
+    wrr = wr * np.exp(xr) / (2 * zeta)
+    ct, wct = np.polynomial.legendre.leggauss(16)
+    nphi = 16
+    ph = (np.arange(nphi) + 0.5) * 2 * math.pi / nphi
+    tot = 0.0
+    for ri, wi in zip(rr, wrr):
+        for c, wc in zip(ct, wct):
+            s = math.sqrt(1 - c * c)
+            for p in ph:
+                v = ob.ao_eval(o, 0, [ri * s * math.cos(p), ri * s * math.sin(p), ri * c])[0]
+                tot += wi * wc * (2 * math.pi / nphi) * ri * ri * v * v
+    assert abs(tot - 1.0) < 1e-9
+
+
+def test_P15_h2_overlap_and_mo_coefficient():
+    d, _ = wl.h2(M=4)
+    o = ob.OracleSystem(d)
+    # overlap of the two normalised 1s STOs by quadrature in prolate spheroidal coordinates
+    R, zeta = 1.4, 1.24
+    xm, wm = np.polynomial.laguerre.laggauss(40)  # mu = 1 + x/(zeta R)
+    nu, wn = np.polynomial.legendre.leggauss(24)
+    S = 0.0
+    for x, w in zip(xm, wm):
+        mu = 1 + x / (zeta * R)
+        for v, wv in zip(nu, wn):
+            rho = (R / 2) * math.sqrt((mu * mu - 1) * (1 - v * v))
+            z = (R / 2) * mu * v
+            fa = ob.ao_eval(o, 0, [rho, 0.0, z])[0]
+            fb = ob.ao_eval(o, 1, [rho, 0.0, z])[0]
+            jac = (R / 2) ** 3 * (mu * mu - v * v) * 2 * math.pi
+            S += w * math.exp(x) / (zeta * R) * wv * jac * fa * fb
+    assert abs(S - 0.65917696731845) < 1e-9
+    assert abs(d.mo_coeff[0, 0] - 0.54895740413533) < 1e-12
+    assert abs(d.extra["overlap"] - S) < 1e-9
+
+
+# ---------------------------------------------------------------- P5, P6
+@pytest.mark.parametrize("n", [2, 3, 4, 5, 6, 7])
+def test_P5_same_spin_hydrogenic_determinant(n):
+    Z = 2.0
+    aos, C, e = hydrogenic_set(Z)
+    d = atom_system(Z, aos, C[:, :n], n, 0, norm=np.ones(len(aos)))
+    r = _rand_pos(40, n, 2.5, rmin=0.1, seed=10 + n)
+    lp, sg, el, parts = ob.local_energy(ob.OracleSystem(d), soa(r), parts=True)
+    vee = np.zeros(len(r))
+    for i, j in itertools.combinations(range(n), 2):
+        vee += 1 / np.linalg.norm(r[:, i] - r[:, j], axis=1)
+    ref = e[:n].sum() + vee
+    ok = lp > np.max(lp) - 25  # drop walkers sitting on a node
+    assert ok.sum() > 20
+    assert np.max(np.abs(el[ok] - ref[ok]) / np.maximum(1, np.abs(ref[ok]))) < 1e-9
+    assert np.allclose(parts[:, 1], vee, rtol=1e-13)
+
+
+def test_P5_both_spins():
+    Z = 3.0
+    aos, C, e = hydrogenic_set(Z)
+    d = atom_system(Z, aos, C[:, :5], 3, 2, norm=np.ones(len(aos)),
+                    det_up=[[0, 2, 4]], det_dn=[[1, 3]])
+    r = _rand_pos(40, 5, 1.5, rmin=0.1, seed=20)
+    lp, sg, el = ob.local_energy(ob.OracleSystem(d), soa(r))
+    vee = sum(1 / np.linalg.norm(r[:, i] - r[:, j], axis=1) for i, j in itertools.combinations(range(5), 2))
+    ref = e[[0, 2, 4]].sum() + e[[1, 3]].sum() + vee
+    ok = lp > np.max(lp) - 25
+    assert np.max(np.abs(el[ok] - ref[ok]) / np.maximum(1, np.abs(ref[ok]))) < 1e-9
+
+
+def test_P6_ci_degenerate_and_nondegenerate():
+    Z = 2.0
+    aos, C, e = hydrogenic_set(Z)
+    # MOs: 0 1s, 1 2s, 2 2px, 3 2py, 4 2pz, 5 3dxy, 6 3dz2 ...
+    # reference up = (1s, 2px), dn = (1s); substitutions 2px->2py, 2px->2pz (degenerate), weights arbitrary
+    det_up = [[0, 2], [0, 3], [0, 4]]
+    det_dn = [[0], [0], [0]]
+    ci = [0.7, -0.4, 0.55]
+    d = atom_system(Z, aos, C[:, :7], 2, 1, det_up=det_up, det_dn=det_dn, ci=ci, norm=np.ones(len(aos)))
+    r = _rand_pos(60, 3, 1.5, rmin=0.1, seed=21)
+    lp, sg, el = ob.local_energy(ob.OracleSystem(d), soa(r))
+    vee = sum(1 / np.linalg.norm(r[:, i] - r[:, j], axis=1) for i, j in itertools.combinations(range(3), 2))
+    ref = (e[0] + e[2] + e[0]) + vee
+    ok = lp > np.max(lp) - 25
+    assert np.max(np.abs(el[ok] - ref[ok]) / np.maximum(1, np.abs(ref[ok]))) < 1e-9
+    # non-degenerate: E_L = sum d_n D_n E_n / sum d_n D_n + V_ee with D_n from single-determinant runs
+    det_up = [[0, 2], [1, 2], [0, 5], [5, 6]]
+    det_dn = [[0], [0], [1], [0]]
+    ci = [0.8, 0.3, -0.5, 0.25]
+    En = [e[0] + e[2] + e[0], e[1] + e[2] + e[0], e[0] + e[5] + e[1], e[5] + e[6] + e[0]]
+    d = atom_system(Z, aos, C[:, :7], 2, 1, det_up=det_up, det_dn=det_dn, ci=ci, norm=np.ones(len(aos)))
+    lp, sg, el = ob.local_energy(ob.OracleSystem(d), soa(r))
+    num = np.zeros(len(r)); den = np.zeros(len(r))
+    for k in range(4):
+        dk = atom_system(Z, aos, C[:, :7], 2, 1, det_up=[det_up[k]], det_dn=[det_dn[k]], norm=np.ones(len(aos)))
+        lpk, sgk, _ = ob.local_energy(ob.OracleSystem(dk), soa(r))
+        Dk = sgk * np.exp(lpk)
+        num += ci[k] * Dk * En[k]; den += ci[k] * Dk
+    ref = num / den + vee
+    ok = np.abs(den) > 1e-3 * np.max(np.abs(den))
+    assert np.max(np.abs(el[ok] - ref[ok]) / np.maximum(1, np.abs(ref[ok]))) < 1e-8
+
+
+# ---------------------------------------------------------------- P7
+@pytest.mark.parametrize("a,b", [(0.5, 1.0), (0.37, 0.6)])
+def test_P7_helium_like_with_pade_closed_form(a, b):
+    Z, zeta = 2.0, 1.6875
+    d = atom_system(Z, [(1, 0, 0, zeta)], [[1.0]], 1, 1, a_par=0.25, a_anti=a, b=b)
+    r = _rand_pos(200, 2, 1.0, rmin=0.05, seed=30)
+    lp, sg, el = ob.local_energy(ob.OracleSystem(d), soa(r))
+    r1, r2 = r[:, 0], r[:, 1]
+    n1, n2 = np.linalg.norm(r1, axis=1), np.linalg.norm(r2, axis=1)
+    d12 = r1 - r2
+    r12 = np.linalg.norm(d12, axis=1)
+    den = 1 + b * r12
+    u = a * r12 / den; u1 = a / den ** 2; u2 = -2 * a * b / den ** 3
+    hat = np.einsum("ij,ij->i", d12 / r12[:, None], r1 / n1[:, None] - r2 / n2[:, None])
+    ref = -zeta ** 2 + (zeta - Z) * (1 / n1 + 1 / n2) + 1 / r12 - (u2 + 2 * u1 / r12) - u1 ** 2 + zeta * u1 * hat
+    assert np.max(np.abs(el - ref) / np.maximum(1, np.abs(ref))) < 1e-12
+    # log psi = 2 log N - zeta (r1+r2) + u
+    N = zeta ** 1.5 / math.sqrt(math.pi)
+    assert np.max(np.abs(lp - (2 * math.log(N) - zeta * (n1 + n2) + u))) < 1e-12
+
+
+def test_parallel_spin_jastrow_uses_a_par():
+    # two same-spin electrons in 1s / 2pz hydrogenic orbitals; changing a_anti must not matter, a_par must
+    Z = 1.0
+    aos, C, e = hydrogenic_set(Z)
+    r = _rand_pos(10, 2, 2.0, rmin=0.2, seed=31)
+    out = []
+    for ap, aa in [(0.25, 0.5), (0.25, 0.9), (0.4, 0.5)]:
+        d = atom_system(Z, aos, C[:, [0, 4]], 2, 0, norm=np.ones(len(aos)), a_par=ap, a_anti=aa)
+        out.append(ob.local_energy(ob.OracleSystem(d), soa(r))[2])
+    assert np.allclose(out[0], out[1], rtol=0, atol=0)
+    assert np.max(np.abs(out[0] - out[2])) > 1e-3
+
+
+# ---------------------------------------------------------------- P8 finite differences
+def _fd_check(d, r_soa, h=1e-4, nwalk=6, tol=1e-6):
+    o = ob.OracleSystem(d)
+    lp, sg, el, parts = ob.local_energy(o, r_soa, parts=True)
+    n_e = d.n_e
+    worst = 0.0
+    for w in range(nwalk):
+        r = r_soa[:, :, w].copy()  # [n_e,3]
+        psi0 = ob.psi_plain(o, r)
+        assert abs(math.log(abs(psi0)) - lp[w]) < 1e-11 and np.sign(psi0) == sg[w]
+
+        def lap(hh):
+            tot, scale = 0.0, 0.0
+            for i in range(n_e):
+                acc = 0.0
+                for c in range(3):
+                    rp = r.copy(); rp[i, c] += hh
+                    rm = r.copy(); rm[i, c] -= hh
+                    acc += (ob.psi_plain(o, rp) - 2 * psi0 + ob.psi_plain(o, rm)) / (hh * hh)
+                tot += acc / psi0
+                scale += abs(acc / psi0)
+            return tot, scale
+        l1, scale = lap(h)
+        l2, _ = lap(h / 2)
+        rich = (4 * l2 - l1) / 3  # Richardson: removes the h^2 truncation term
+        kin_fd = -0.5 * rich
+        err = abs(kin_fd - parts[w, 0]) / max(1.0, scale)
+        worst = max(worst, err)
+    assert worst < tol, worst
+
+
+def _keep_away(d, r_soa, rmin=0.3):
+    """walkers whose electrons are all >= rmin from every nucleus (Q17)"""
+    r = r_soa.transpose(2, 0, 1)  # [M,n_e,3]
+    dist = np.linalg.norm(r[:, :, None, :] - d.atom_xyz[None, None], axis=3)
+    return np.where(dist.min(axis=(1, 2)) > rmin)[0]
+
+
+@pytest.mark.parametrize("name", ["H2", "LiH", "Li2", "CO"])
+def test_P8_finite_differences_configs(name):
+    d, r = wl.CONFIGS[name](M=64)
+    o = ob.OracleSystem(d)
+    lp, _, _ = ob.local_energy(o, r)
+    idx = _keep_away(d, r)
+    idx = idx[np.argsort(-lp[idx])][:4]  # well away from nodes
+    _fd_check(d, np.ascontiguousarray(r[:, :, idx]), nwalk=len(idx), tol=2e-6)
+
+
+def test_P8_ao_derivatives_vs_fd():
+    d, _ = wl.co(M=2)
+    o = ob.OracleSystem(d)
+    rng = np.random.default_rng(5)
+    h = 1e-4
+    for ao in range(d.n_ao):
+        a = d.ao_atom[ao]
+        x = d.atom_xyz[a] + rng.standard_normal(3) * 0.6 + 0.35
+        v = ob.ao_eval(o, ao, x)
+        g = np.zeros(3); lap = 0.0
+        for c in range(3):
+            e = np.zeros(3); e[c] = h
+            p, m = ob.ao_eval(o, ao, x + e)[0], ob.ao_eval(o, ao, x - e)[0]
+            p2, m2 = ob.ao_eval(o, ao, x + e / 2)[0], ob.ao_eval(o, ao, x - e / 2)[0]
+            g1, g2 = (p - m) / (2 * h), (p2 - m2) / h
+            g[c] = (4 * g2 - g1) / 3
+            l1, l2 = (p - 2 * v[0] + m) / h ** 2, (p2 - 2 * v[0] + m2) / (h / 2) ** 2
+            lap += (4 * l2 - l1) / 3
+        sc = max(1.0, abs(v[0]) * d.ao_zeta[ao] ** 2)
+        assert np.max(np.abs(g - v[1:4])) < 1e-7 * sc, (ao, g, v)
+        assert abs(lap - v[4]) < 2e-6 * sc, (ao, lap, v[4])
+
+
+# ---------------------------------------------------------------- P9 antisymmetry
+@pytest.mark.parametrize("name", ["LiH", "Li2", "CO"])
+def test_P9_same_spin_exchange(name):
+    d, r = wl.CONFIGS[name](M=32)
+    o = ob.OracleSystem(d)
+    lp, sg, el = ob.local_energy(o, r)
+    for (i, j) in [(0, 1), (d.n_up, d.n_up + 1)]:
+        r2 = r.copy()
+        r2[[i, j]] = r2[[j, i]]
+        lp2, sg2, el2 = ob.local_energy(o, r2)
+        assert np.all(sg2 == -sg)
+        assert np.max(np.abs(lp2 - lp)) < 1e-11
+        assert np.max(np.abs(el2 - el) / np.maximum(1, np.abs(el))) < 1e-9
+    # opposite-spin exchange is NOT a symmetry of the spin-assigned function
+    r3 = r.copy(); r3[[0, d.n_up]] = r3[[d.n_up, 0]]
+    lp3, _, _ = ob.local_energy(o, r3)
+    assert np.max(np.abs(lp3 - lp)) > 1e-3
+
+
+def test_pauli_zero_at_same_spin_coalescence():
+    # the wave function vanishes when two same-spin electrons coincide
+    d, r = wl.li2(M=4)
+    o = ob.OracleSystem(d)
+    base = ob.local_energy(o, r)[0]
+    r2 = r.copy(); r2[1] = r2[0] + 1e-9
+    lp2 = ob.local_energy(o, r2)[0]
+    assert np.all(lp2 < base - 12)
+
+
+# ---------------------------------------------------------------- P10 Leibniz
+def _leibniz(A):
+    n = A.shape[0]
+    tot = 0.0
+    for perm in itertools.permutations(range(n)):
+        sgn = 1
+        for i in range(n):
+            for j in range(i + 1, n):
+                if perm[i] > perm[j]:
+                    sgn = -sgn
+        p = 1.0
+        for i in range(n):
+            p *= A[i, perm[i]]
+        tot += sgn * p
+    return tot
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5])
+def test_P10_determinant_vs_permutation_sum(n):
+    rng = np.random.default_rng(n)
+    for _ in range(10):
+        A = rng.standard_normal((n, n))
+        dd, inv = ob.det_inv(A)
+        ref = _leibniz(A)
+        assert abs(dd - ref) < 1e-13 * max(1.0, abs(ref))
+        assert np.max(np.abs(inv @ A - np.eye(n))) < 1e-11
+    # a matrix that needs pivoting (zero leading element)
+    A = rng.standard_normal((n, n)); A[0, 0] = 0.0
+    if n > 1:
+        assert abs(ob.det_inv(A)[0] - _leibniz(A)) < 1e-13
+
+
+# ---------------------------------------------------------------- P11 nuclear repulsion
+def test_P11_nuclear_repulsion():
+    for fn, ref in [(wl.h2, 1 / 1.4), (wl.lih, 3 / 3.015), (wl.li2, 9 / 5.051), (wl.co, 48 / 2.132)]:
+        d, r = fn(M=2)
+        parts = ob.local_energy(ob.OracleSystem(d), r, parts=True)[3]
+        assert np.max(np.abs(parts[:, 3] - ref)) < 1e-14 * max(1, ref)
+    assert abs(1 / 1.4 - 0.7142857142857143) < 1e-15
+
+
+def test_potential_terms_brute_force():
+    d, r = wl.co(M=8)
+    parts = ob.local_energy(ob.OracleSystem(d), r, parts=True)[3]
+    rr = r.transpose(2, 0, 1)
+    for w in range(8):
+        ven = -sum(d.atom_Z[a] / np.linalg.norm(rr[w, i] - d.atom_xyz[a]) for i in range(14) for a in range(2))
+        vee = sum(1 / np.linalg.norm(rr[w, i] - rr[w, j]) for i in range(14) for j in range(i))
+        assert abs(parts[w, 2] - ven) < 1e-12 * abs(ven) and abs(parts[w, 1] - vee) < 1e-12 * abs(vee)
+
+
+# ---------------------------------------------------------------- P12 cusps
+def test_P12_electron_electron_cusp_finite():
+    Z, zeta = 2.0, 1.7
+    out = {}
+    for label, a in [("exact", 0.5), ("off", 0.4)]:
+        d = atom_system(Z, [(1, 0, 0, zeta)], [[1.0]], 1, 1, a_anti=a, b=1.0)
+        o = ob.OracleSystem(d)
+        vals = []
+        for eps in [1e-2, 1e-3, 1e-4, 1e-5, 1e-6]:
+            r = np.array([[[0.4, 0.3, 0.2], [0.4 + eps, 0.3, 0.2]]])
+            vals.append(ob.local_energy(o, soa(r))[2][0])
+        out[label] = np.array(vals)
+    assert np.all(np.abs(out["exact"]) < 50)
+    assert abs(out["exact"][-1] - out["exact"][-2]) < 1e-3  # converges
+    # perturbed cusp diverges like (1 - 2a)/r
+    assert abs(out["off"][-1] - (1 - 2 * 0.4) / 1e-6) < 0.01 * (0.2 / 1e-6)
+    # parallel spins (a = 1/4): antisymmetric pair 1s/2pz
+    aos, C, e = hydrogenic_set(1.0)
+    for a, finite in [(0.25, True), (0.15, False)]:
+        d = atom_system(1.0, aos, C[:, [0, 4]], 2, 0, norm=np.ones(len(aos)), a_par=a)
+        o = ob.OracleSystem(d)
+        vals = [ob.local_energy(o, soa(np.array([[[0.4, 0.3, 0.2], [0.4, 0.3, 0.2 + eps]]])))[2][0]
+                for eps in [1e-3, 1e-4, 1e-5]]
+        if finite:
+            assert max(abs(v) for v in vals) < 50 and abs(vals[-1] - vals[-2]) < 1e-2
+        else:
+            assert abs(vals[-1] - (1 - 4 * a) / 1e-5) < 0.02 * (1 - 4 * a) / 1e-5
+
+
+def test_electron_nucleus_cusp_finite_energy():
+    # STOs give finite E_L at electron-nucleus coalescence when zeta = Z (1s)
+    d = atom_system(3.0, [(1, 0, 0, 3.0)], [[1.0]], 1, 0)
+    o = ob.OracleSystem(d)
+    vals = [ob.local_energy(o, soa(np.array([[[eps, 0, 0]]])))[2][0] for eps in [1e-2, 1e-4, 1e-6]]
+    assert np.max(np.abs(np.array(vals) + 4.5)) < 1e-9
+
+
+# ---------------------------------------------------------------- P13 SD enumerator
+def test_P13_sd_counts_match_paper():
+    rows = [l.split() for l in open(os.path.join(GOLD, "sd_counts.txt")) if l.strip() and not l.startswith("#")]
+    assert len(rows) == 5
+    for n_el, n_orb, n_det in rows:
+        assert wl.sd_count(int(n_el), int(n_orb)) == int(n_det)
+
+
+def test_selected_determinants_structure():
+    for fn, nd in [(wl.li2, 20), (wl.co, 100)]:
+        d, _ = fn(M=2)
+        assert d.det_up.shape == (nd, d.n_up)
+        ref = np.arange(d.n_up)
+        seen = set()
+        ks = set()
+        for n in range(nd):
+            key = (tuple(d.det_up[n]), tuple(d.det_dn[n]))
+            assert key not in seen
+            seen.add(key)
+            for lst in key:
+                assert len(set(lst)) == len(lst) and max(lst) < d.n_mo
+            ks.add((int((d.det_up[n] != ref).sum()), int((d.det_dn[n] != ref).sum())))
+        assert ks == {(0, 0), (1, 0), (0, 1), (1, 1), (2, 0), (0, 2)}
+
+
+# ---------------------------------------------------------------- P14 identities behind the fast path
+def test_P14_trace_identities_random_matrices():
+    rng = np.random.default_rng(7)
+    n, nv = 6, 5
+    for trial in range(20):
+        A0 = rng.standard_normal((n, n)); Av = rng.standard_normal((n, nv))
+        B0 = rng.standard_normal((n, n)); Bv = rng.standard_normal((n, nv))
+        k = 1 + trial % 3
+        p = rng.choice(n, k, replace=False); q = rng.choice(nv, k, replace=False)
+        AX, BX = A0.copy(), B0.copy()
+        AX[:, p] = Av[:, q]; BX[:, p] = Bv[:, q]
+        d0, A0i = ob.det_inv(A0)
+        dX, AXi = ob.det_inv(AX)
+        T = A0i @ Av
+        Mtab = A0i @ Bv - (A0i @ B0) @ T
+        Tpq = T[np.ix_(p, q)]
+        # reading Q8: D_X / D_0 = det T[p,q]
+        assert abs(dX / d0 - np.linalg.det(Tpq)) < 1e-10 * max(1, abs(dX / d0))
+        # F.6 / F.7 in table form
+        lhs = np.trace(AXi @ BX)
+        rhs = np.trace(A0i @ B0) + np.trace(np.linalg.inv(Tpq) @ Mtab[np.ix_(p, q)])
+        assert abs(lhs - rhs) < 1e-9 * max(1, abs(lhs))
+        # H.10
+        P = np.zeros((n, n)); P[p, p] = 1
+        W = A0i @ AX
+        Tm = np.zeros((n, n)); Tm[np.ix_(p, p)] = np.linalg.inv(W[np.ix_(p, p)])
+        assert np.max(np.abs(AXi - (A0i - (W - np.eye(n)) @ Tm @ A0i))) < 1e-8
+    # G.5 / G.6: row-local derivative => (Tr)^2 = Tr(()^2)
+    A = rng.standard_normal((n, n)); Ai = np.linalg.inv(A)
+    dA = np.zeros((n, n)); dA[2] = rng.standard_normal(n)
+    X = Ai @ dA
+    assert abs(np.trace(X) ** 2 - np.trace(X @ X)) < 1e-12
+
+
+# ---------------------------------------------------------------- P16 Philox + normals
+def test_P16_philox_known_answers():
+    rows = [l.split() for l in open(os.path.join(GOLD, "philox4x32_10_kat.txt")) if l.strip() and not l.startswith("#")]
+    for row in rows:
+        v = [int(x, 16) for x in row]
+        out = ob.philox(v[0:4], v[4:6])
+        assert [int(x) for x in out] == v[6:10]
+
+
+def test_P16_uniform_mapping_and_counter_layout():
+    # walker_draws must be Philox(ctr=(w, sweep, j, 0), key=(seed lo, seed hi)) + the stated 53-bit mapping
+    seed, w, sweep = 0x123456789ABCDEF0, 77, 5
+    z, u = ob.walker_draws(seed, w, sweep, 6)
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    for j in range(3):
+        x = [int(t) for t in ob.philox([w, sweep, j, 0], key)]
+        u1 = (((x[0] << 32 | x[1]) >> 11) + 0.5) * 2.0 ** -53
+        u2 = (((x[2] << 32 | x[3]) >> 11) + 0.5) * 2.0 ** -53
+        rho = math.sqrt(-2 * math.log(u1))
+        assert abs(z[2 * j] - rho * math.cos(2 * math.pi * u2)) < 1e-15 * max(1, rho)
+        assert abs(z[2 * j + 1] - rho * math.sin(2 * math.pi * u2)) < 1e-15 * max(1, rho)
+    x = [int(t) for t in ob.philox([w, sweep, 0xFFFFFFFF, 0], key)]
+    assert u == (((x[0] << 32 | x[1]) >> 11) + 0.5) * 2.0 ** -53
+    assert 0.0 < u < 1.0
+
+
+def test_P16_normal_moments_and_ks():
+    from scipy import stats
+    zs = np.concatenate([ob.walker_draws(42, w, s, 42)[0] for w in range(400) for s in range(3)])
+    assert abs(zs.mean()) < 4 / math.sqrt(len(zs))
+    assert abs(zs.var() - 1) < 0.03
+    assert stats.kstest(zs, "norm").pvalue > 1e-3
+    us = np.array([ob.walker_draws(42, w, 0, 2)[1] for w in range(4000)])
+    assert stats.kstest(us, "uniform").pvalue > 1e-3
+
+
+# ---------------------------------------------------------------- P17 sampler sanity
+def test_P17_metropolis_hydrogen_atom():
+    d = atom_system(1, [(1, 0, 0, 1.0)], [[1.0]], 1, 0)
+    o = ob.OracleSystem(d)
+    M = 6000
+    r0 = soa(np.random.default_rng(3).standard_normal((M, 1, 3)))
+    out = ob.metropolis(o, r0, 0.5, 150, seed=9, threads=8)
+    rr = np.linalg.norm(out["r"][0], axis=0)
+    assert abs(rr.mean() - 1.5) < 0.05          # <r> of the 1s density
+    assert abs((rr ** 2).mean() - 3.0) < 0.2    # <r^2> = 3
+    acc = out["accept"].mean()
+    assert 0.3 < acc < 0.95
+    # decisions are exactly the sign of the margin
+    assert np.array_equal(out["accept"] == 1, out["margin"] > 0)
+    lp, sg, el = ob.local_energy(o, out["r"])
+    assert np.max(np.abs(el + 0.5)) < 1e-12 and np.max(np.abs(lp - out["logpsi"])) < 1e-13
+
+
+def test_metropolis_resumable_and_partition_independent():
+    d, r = wl.lih(M=64)
+    o = ob.OracleSystem(d)
+    a = ob.metropolis(o, r, 0.3, 6, seed=11)
+    b1 = ob.metropolis(o, r, 0.3, 2, seed=11, sweep_offset=0)
+    b2 = ob.metropolis(o, b1["r"], 0.3, 4, seed=11, sweep_offset=2, threads=3)
+    assert np.array_equal(a["r"], b2["r"]) and np.array_equal(a["accept"][2:], b2["accept"])
+    assert np.array_equal(a["logpsi"], b2["logpsi"])
+
+
+def test_metropolis_eloc_acc():
+    d, r = wl.lih(M=16)
+    o = ob.OracleSystem(d)
+    out1 = ob.metropolis(o, r, 0.3, 1, seed=5, want_eloc_acc=True)
+    el = ob.local_energy(o, out1["r"])[2]
+    assert np.allclose(out1["eloc_acc"], el, rtol=1e-14)
+
+
+def test_batch_stats():
+    x = np.random.default_rng(1).standard_normal(10001) * 3 + 1e6
+    m, s = ob.batch_stats(x)
+    assert abs(m - math.fsum(x) / len(x)) < 1e-9
+    assert abs(s - x.std(ddof=1) / math.sqrt(len(x))) < 1e-12
