@@ -1,0 +1,158 @@
+/* qmc.h -- C ABI of libqmcb200: batched Slater-Jastrow Psi, local energy and
+ * all-electron Metropolis sampling in FP64 on one B200 (sm_100a).
+ *
+ * The calls follow the paper's statement of the problem
+ * (/root/reference/PAPER.md, cited as PAPER.md:<line>):
+ *   Psi(r) = e^{J(r)} * sum_n d_n D_n^up(r^up) D_n^dn(r^dn)           eq. 4
+ *   E_L(r) = H Psi / Psi with the molecular Hamiltonian of eq. 1
+ *   walkers sampled from |Psi|^2 by Metropolis-Hastings, all electrons
+ *   moved at once with a normal proposal
+ *
+ * Conventions
+ *  - "host" / "device" is stated for every pointer.  The caller owns every
+ *    walker / output buffer; a qmc_system_t owns only device copies of the
+ *    constants given to qmc_setup and is immutable afterwards (so it may be
+ *    used from several streams concurrently).
+ *  - Walker coordinates are SoA: double r[n_e][3][M], walker index fastest,
+ *    electrons 0..n_up-1 spin-up, the rest spin-down, units bohr.
+ *  - Every call returns QMC_OK (0) or a negative status; nothing aborts or
+ *    prints.  qmc_status_string(status) describes it; for QMC_ECUDA it carries
+ *    the CUDA error text of the failing call on this thread.
+ *  - Calls are asynchronous on `cuda_stream` (a cudaStream_t passed as void*)
+ *    unless a host out-pointer is given, in which case the call synchronises
+ *    that stream before returning.
+ *  - There is no CPU fallback: without a CUDA device every call fails with
+ *    QMC_ECUDA.
+ */
+#ifndef QMC_B200_H
+#define QMC_B200_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define QMC_OK 0
+#define QMC_EINVAL (-1)       /* bad argument (null pointer, M <= 0, bad AO quantum numbers, ...) */
+#define QMC_EUNSUPPORTED (-2) /* valid problem outside the compiled limits (see qmc_setup) */
+#define QMC_ECUDA (-3)        /* a CUDA runtime call failed */
+#define QMC_ENOMEM (-4)       /* host allocation failed */
+
+typedef struct qmc_system qmc_system_t; /* opaque */
+
+/* Inputs of eq. 4.  All pointers are HOST pointers; the
+ * arrays are copied during qmc_setup and may be freed afterwards. */
+typedef struct {
+  int32_t n_atoms;
+  const double *atom_xyz; /* [n_atoms][3] nuclear positions R_alpha, bohr          (eq. 1) */
+  const double *atom_Z;   /* [n_atoms] nuclear charges Z_alpha                      (eq. 1) */
+  int32_t n_up, n_dn;     /* electrons per spin; n_up + n_dn >= 1 */
+  /* Slater-type atomic orbitals:
+   *   phi = N * S_lm(d) * r^(n-1-l) * exp(-zeta r),  d = r_i - R_atom, r = |d|,
+   * S_lm real solid harmonics, m index:  l=0: {1};  l=1: {x, y, z};
+   *   l=2: {xy, yz, zx, x^2-y^2, 2z^2-x^2-y^2}.   Requires 1 <= n <= 4, 0 <= l <= 2, l < n. */
+  int32_t n_ao;
+  const int32_t *ao_atom; /* [n_ao] centre index */
+  const int32_t *ao_n;    /* [n_ao] principal quantum number */
+  const int32_t *ao_l;    /* [n_ao] */
+  const int32_t *ao_m;    /* [n_ao] harmonic index within l (see above) */
+  const double *ao_zeta;  /* [n_ao] exponents, > 0 */
+  const double *ao_norm;  /* [n_ao] normalisation N, or NULL for the standard one:
+                             (2 zeta)^(n+1/2)/sqrt((2n)!) times the real-spherical-harmonic constant */
+  /* Molecular orbitals: phi_alpha = sum_beta C[beta][alpha] ao_beta,
+   * C = c * mu already multiplied by the caller. */
+  int32_t n_mo;
+  const double *mo_coeff; /* [n_ao][n_mo] row-major */
+  /* CI expansion: determinant n uses, for each spin, the ORDERED list of
+   * MO columns det_x[n][0..n_x-1]:  A_n[i][j] = phi_{det[n][j]}(r_i)  (rows = electrons).
+   * Determinant 0 is the reference; the others are usually in-place substitutions of
+   * its columns, any number of substitutions is accepted. */
+  int32_t n_det;
+  const int32_t *det_up; /* [n_det][n_up] (ignored when n_up == 0) */
+  const int32_t *det_dn; /* [n_det][n_dn] (ignored when n_dn == 0) */
+  const double *ci_coeff; /* [n_det] d_n */
+  /* Pade electron-electron Jastrow (D.1): K(r) = w0 r / (1 + w r) */
+  double jastrow_a_par;  /* w0 for parallel spins      (cusp value 1/4) */
+  double jastrow_a_anti; /* w0 for anti-parallel spins (cusp value 1/2) */
+  double jastrow_b;      /* w */
+} qmc_system_desc_t;
+
+/* Validate `desc`, preprocess it (shell grouping, excitation tables relative to
+ * determinant 0) and upload the constants to `device`.
+ * Limits (QMC_EUNSUPPORTED beyond them): n_up, n_dn <= 8; at most 8 distinct
+ * virtual (non-reference) orbitals per spin; n_up + n_dn <= 16; n_atoms <= 16;
+ * n_ao <= 256; at most 16 distinct orbitals referenced overall; determinants
+ * differing from determinant 0 in more than 2 columns of one spin are unsupported.
+ * QMC_EINVAL: null pointers, n_up + n_dn == 0, n_det < 1, bad (n,l,m), zeta <= 0,
+ * atom / MO index out of range, a determinant list repeating a column.
+ * On success *out receives a handle to be released with qmc_destroy. */
+int qmc_setup(const qmc_system_desc_t *desc, int device, qmc_system_t **out);
+
+/* Release a handle (device and host memory).  NULL is ignored. */
+void qmc_destroy(qmc_system_t *s);
+
+/* Local energy of M walkers (eq. 1-3; trace formulas F.1-F.7, G.7,
+ * PAPER.md:290-343, 386).
+ *   d_r      device, in : double [n_e][3][M]
+ *   d_logpsi device, out: double [M]  log|Psi|                 (may be NULL)
+ *   d_sign   device, out: double [M]  sign of Psi: +1, -1 or 0 (may be NULL)
+ *   d_eloc   device, out: double [M]  E_L in hartree            (may be NULL)
+ * NaN/Inf in the inputs propagate to the outputs.  Asynchronous on cuda_stream. */
+int qmc_local_energy(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign,
+                     double *d_eloc, void *cuda_stream);
+
+/* log|Psi| and sign only (the part of the path the sampler needs). Same arguments. */
+int qmc_log_psi(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign,
+                void *cuda_stream);
+
+/* n_sweeps all-electron Metropolis sweeps.  One sweep = one move attempt
+ * of every walker: r' = r + step * z, z ~ N(0,1)^(3 n_e); accepted iff
+ *   log u < 2 (log|Psi(r')| - log|Psi(r)|),  u uniform on (0,1);
+ * a proposal with Psi' = 0 or NaN is rejected.  Random numbers: Philox4x32-10,
+ * key = (seed lo32, seed hi32), counter = (w lo32, sweep lo32, j, w hi32) where w is
+ * walker_offset + the walker's index in this call and sweep = sweep_offset + s;
+ * block j < ceil(3 n_e / 2) gives Box-Muller normals for coordinates 2j, 2j+1
+ * (coordinate = 3*electron + xyz), block j = 0xFFFFFFFF gives u.  Two 32-bit words
+ * (hi, lo) map to ((hi*2^32 + lo) >> 11 + 1/2) * 2^-53.  Hence a trajectory depends
+ * only on (seed, w, sweep), not on batching, and is resumable through sweep_offset.
+ *   d_r        device, in/out: double [n_e][3][M]
+ *   step       > 0, standard deviation of the proposal per Cartesian coordinate, bohr
+ *   d_logpsi   device, out: [M] log|Psi| of the final positions   (may be NULL)
+ *   d_sign     device, out: [M]                                    (may be NULL)
+ *   d_accept   device, out: uint8 [n_sweeps][M] accept mask        (may be NULL)
+ *   d_eloc_acc device, out: [M] sum over the sweeps of E_L evaluated after each sweep
+ *              (BASELINE config 5: "E_L on every sweep")           (may be NULL)
+ *   h_n_accepted host, out: total number of accepted moves; if non-NULL the call
+ *              synchronises cuda_stream                              (may be NULL)
+ * sweep_offset + n_sweeps must be < 2^32. */
+int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t n_sweeps, uint64_t seed,
+                   uint64_t sweep_offset, int64_t walker_offset, double *d_logpsi, double *d_sign,
+                   uint8_t *d_accept, double *d_eloc_acc, int64_t *h_n_accepted, void *cuda_stream);
+
+/* Mean and standard error of the mean of M doubles (eq. 3):
+ *   d_x device in [M]; h_mean, h_stderr host out (either may be NULL).
+ * Deterministic (fixed reduction tree, compensated).  Synchronises cuda_stream. */
+int qmc_batch_stats(const double *d_x, int64_t M, double *h_mean, double *h_stderr, void *cuda_stream);
+
+/* Measured FP64 throughput of the current device, the roofline denominator of this
+ * path (BASELINE.json north_star: "the chip's FP64 peak, measured by a DFMA
+ * microbenchmark in the same run").  kind 0: dependent-chain DFMA kernel, 1: DMMA
+ * m8n8k4 kernel, 2: both interleaved in one kernel.  h_tflops host out: best of
+ * `reps` launches, counting 2 flops per FMA.  Synchronous. */
+int qmc_fp64_peak(int device, int kind, int reps, double *h_tflops);
+
+/* Model FP64 work per walker of this system for one E_L evaluation (which = 0) or one
+ * Metropolis walker-step (which = 1), in flop-equivalents, by the cost table of
+ * DESIGN.md "Roofline" (an FMA counts 2; exp, divide, sqrt, log, sincos by table). */
+double qmc_model_flops(const qmc_system_t *s, int which);
+
+/* Number of kernel launches issued by this library on the calling thread since the
+ * last call with reset != 0 (bench.py's gpu_launches). */
+int64_t qmc_launch_count(int reset);
+
+const char *qmc_status_string(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

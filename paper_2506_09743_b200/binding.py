@@ -1,0 +1,193 @@
+"""Thin ctypes binding of libqmcb200 (include/qmc.h).  Argument marshalling only:
+every step of the path runs in the CUDA kernels.  PyTorch supplies device memory and
+streams.  There is no CPU fallback: a missing library raises."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+QMC_OK, QMC_EINVAL, QMC_EUNSUPPORTED, QMC_ECUDA, QMC_ENOMEM = 0, -1, -2, -3, -4
+_lib = None
+
+EXPORTS = ["qmc_setup", "qmc_destroy", "qmc_local_energy", "qmc_log_psi", "qmc_metropolis", "qmc_batch_stats",
+           "qmc_fp64_peak", "qmc_model_flops", "qmc_launch_count", "qmc_status_string"]
+
+
+class QmcError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"libqmcb200 status {status}: {msg}")
+        self.status = status
+
+
+class _Desc(C.Structure):
+    _fields_ = [
+        ("n_atoms", C.c_int32), ("atom_xyz", C.c_void_p), ("atom_Z", C.c_void_p),
+        ("n_up", C.c_int32), ("n_dn", C.c_int32),
+        ("n_ao", C.c_int32), ("ao_atom", C.c_void_p), ("ao_n", C.c_void_p), ("ao_l", C.c_void_p),
+        ("ao_m", C.c_void_p), ("ao_zeta", C.c_void_p), ("ao_norm", C.c_void_p),
+        ("n_mo", C.c_int32), ("mo_coeff", C.c_void_p),
+        ("n_det", C.c_int32), ("det_up", C.c_void_p), ("det_dn", C.c_void_p), ("ci_coeff", C.c_void_p),
+        ("jastrow_a_par", C.c_double), ("jastrow_a_anti", C.c_double), ("jastrow_b", C.c_double),
+    ]
+
+
+def lib():
+    """Load libqmcb200.so (building it with nvcc if the sources are newer)."""
+    global _lib
+    if _lib is None:
+        so = _build.SO
+        if _build.needs_build():
+            so = _build.build()
+        if not os.path.exists(so):
+            raise ImportError("libqmcb200.so is missing and could not be built; there is no CPU fallback")
+        L = C.CDLL(so)
+        vp, i64, dbl = C.c_void_p, C.c_int64, C.c_double
+        L.qmc_setup.restype = C.c_int
+        L.qmc_setup.argtypes = [vp, C.c_int, C.POINTER(vp)]
+        L.qmc_destroy.restype = None
+        L.qmc_destroy.argtypes = [vp]
+        L.qmc_local_energy.restype = C.c_int
+        L.qmc_local_energy.argtypes = [vp, vp, i64, vp, vp, vp, vp]
+        L.qmc_log_psi.restype = C.c_int
+        L.qmc_log_psi.argtypes = [vp, vp, i64, vp, vp, vp]
+        L.qmc_metropolis.restype = C.c_int
+        L.qmc_metropolis.argtypes = [vp, vp, i64, dbl, C.c_int32, C.c_uint64, C.c_uint64, i64, vp, vp, vp, vp, vp, vp]
+        L.qmc_batch_stats.restype = C.c_int
+        L.qmc_batch_stats.argtypes = [vp, i64, vp, vp, vp]
+        L.qmc_fp64_peak.restype = C.c_int
+        L.qmc_fp64_peak.argtypes = [C.c_int, C.c_int, C.c_int, vp]
+        L.qmc_model_flops.restype = dbl
+        L.qmc_model_flops.argtypes = [vp, C.c_int]
+        L.qmc_launch_count.restype = i64
+        L.qmc_launch_count.argtypes = [C.c_int]
+        L.qmc_status_string.restype = C.c_char_p
+        L.qmc_status_string.argtypes = [C.c_int]
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != QMC_OK:
+        raise QmcError(rc, lib().qmc_status_string(rc).decode())
+
+
+def _np(a):
+    return None if a is None else a.ctypes.data
+
+
+def _dp(t):
+    return None if t is None else t.data_ptr()
+
+
+def _stream(stream=None):
+    st = stream if stream is not None else torch.cuda.current_stream()
+    return st.cuda_stream
+
+
+def make_desc(d):
+    """SystemDesc-like object -> (ctypes struct, keep-alive dict of contiguous arrays)."""
+    f64 = lambda a: np.ascontiguousarray(a, np.float64)
+    i32 = lambda a: np.ascontiguousarray(a, np.int32)
+    k = dict(atom_xyz=f64(d.atom_xyz), atom_Z=f64(d.atom_Z), ao_atom=i32(d.ao_atom), ao_n=i32(d.ao_n),
+             ao_l=i32(d.ao_l), ao_m=i32(d.ao_m), ao_zeta=f64(d.ao_zeta),
+             ao_norm=None if d.ao_norm is None else f64(d.ao_norm), mo_coeff=f64(d.mo_coeff),
+             det_up=i32(d.det_up), det_dn=i32(d.det_dn), ci_coeff=f64(d.ci_coeff))
+    desc = _Desc(int(k["atom_xyz"].shape[0]), _np(k["atom_xyz"]), _np(k["atom_Z"]), int(d.n_up), int(d.n_dn),
+                 int(k["ao_atom"].shape[0]), _np(k["ao_atom"]), _np(k["ao_n"]), _np(k["ao_l"]), _np(k["ao_m"]),
+                 _np(k["ao_zeta"]), _np(k["ao_norm"]), int(k["mo_coeff"].shape[1]), _np(k["mo_coeff"]),
+                 int(k["ci_coeff"].shape[0]), _np(k["det_up"]), _np(k["det_dn"]), _np(k["ci_coeff"]),
+                 float(d.jastrow_a_par), float(d.jastrow_a_anti), float(d.jastrow_b))
+    return desc, k
+
+
+class QmcSystem:
+    """Handle returned by qmc_setup; methods mirror the C calls."""
+
+    def __init__(self, d, device: int = 0):
+        self.n_up, self.n_dn = int(d.n_up), int(d.n_dn)
+        self.n_e = self.n_up + self.n_dn
+        self.device = device
+        desc, keep = make_desc(d)
+        h = C.c_void_p()
+        _check(lib().qmc_setup(C.addressof(desc), device, C.byref(h)))
+        del keep
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().qmc_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _chk_r(self, r):
+        assert r.is_cuda and r.dtype == torch.float64 and r.is_contiguous()
+        assert r.dim() == 3 and r.shape[0] == self.n_e and r.shape[1] == 3, "walkers must be [n_e,3,M]"
+        return int(r.shape[2])
+
+    def local_energy(self, r, logpsi=None, sign=None, eloc=None, stream=None):
+        """qmc_local_energy: r float64 cuda [n_e,3,M] -> (logpsi, sign, eloc) each [M]."""
+        M = self._chk_r(r)
+        new = lambda: torch.empty(M, dtype=torch.float64, device=r.device)
+        logpsi = new() if logpsi is None else logpsi
+        sign = new() if sign is None else sign
+        eloc = new() if eloc is None else eloc
+        _check(lib().qmc_local_energy(self._h, _dp(r), M, _dp(logpsi), _dp(sign), _dp(eloc), _stream(stream)))
+        return logpsi, sign, eloc
+
+    def log_psi(self, r, logpsi=None, sign=None, stream=None):
+        M = self._chk_r(r)
+        new = lambda: torch.empty(M, dtype=torch.float64, device=r.device)
+        logpsi = new() if logpsi is None else logpsi
+        sign = new() if sign is None else sign
+        _check(lib().qmc_log_psi(self._h, _dp(r), M, _dp(logpsi), _dp(sign), _stream(stream)))
+        return logpsi, sign
+
+    def metropolis(self, r, step, n_sweeps, seed, sweep_offset=0, walker_offset=0, logpsi=None, sign=None,
+                   accept=None, eloc_acc=None, want_accept=False, want_eloc_acc=False, count=False, stream=None):
+        """qmc_metropolis: r is updated in place.  Returns dict(logpsi, sign, accept, eloc_acc, n_accepted)."""
+        M = self._chk_r(r)
+        new = lambda: torch.empty(M, dtype=torch.float64, device=r.device)
+        logpsi = new() if logpsi is None else logpsi
+        sign = new() if sign is None else sign
+        if want_accept and accept is None:
+            accept = torch.empty((n_sweeps, M), dtype=torch.uint8, device=r.device)
+        if want_eloc_acc and eloc_acc is None:
+            eloc_acc = new()
+        nacc = C.c_int64(-1)
+        _check(lib().qmc_metropolis(self._h, _dp(r), M, float(step), int(n_sweeps), int(seed), int(sweep_offset),
+                                    int(walker_offset), _dp(logpsi), _dp(sign), _dp(accept), _dp(eloc_acc),
+                                    C.addressof(nacc) if count else None, _stream(stream)))
+        return dict(logpsi=logpsi, sign=sign, accept=accept, eloc_acc=eloc_acc,
+                    n_accepted=nacc.value if count else None)
+
+    def model_flops(self, which: int) -> float:
+        return lib().qmc_model_flops(self._h, which)
+
+
+def batch_stats(x, stream=None):
+    """qmc_batch_stats: mean and standard error of a float64 cuda vector."""
+    assert x.is_cuda and x.dtype == torch.float64 and x.is_contiguous()
+    m, s = C.c_double(), C.c_double()
+    _check(lib().qmc_batch_stats(_dp(x), x.numel(), C.addressof(m), C.addressof(s), _stream(stream)))
+    return m.value, s.value
+
+
+def fp64_peak(kind: int = 0, reps: int = 5, device: int = 0) -> float:
+    """qmc_fp64_peak: measured TFLOP/s of the DFMA (0) / DMMA (1) / mixed (2) microbenchmark."""
+    v = C.c_double()
+    _check(lib().qmc_fp64_peak(device, kind, reps, C.addressof(v)))
+    return v.value
+
+
+def launch_count(reset: bool = False) -> int:
+    return lib().qmc_launch_count(1 if reset else 0)

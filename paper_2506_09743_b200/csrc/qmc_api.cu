@@ -1,0 +1,459 @@
+// qmc_api.cu -- host side of libqmcb200: the C ABI of include/qmc.h.
+// Setup preprocessing (shell grouping, excitation descriptors relative to determinant 0:
+// PAPER.md:325 "A_X is constructed by replacing some columns of A_0"), dispatch to the
+// compiled (NS, NMO) instantiations, launch geometry, error reporting.
+#include "../../include/qmc.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "qmc_kernels.cuh"
+
+using namespace qmc;
+
+namespace {
+
+thread_local std::string g_cuda_err;
+thread_local int64_t g_launches = 0;
+
+int cuda_fail(cudaError_t e, const char *what) {
+  g_cuda_err = std::string(what) + ": " + cudaGetErrorString(e);
+  return QMC_ECUDA;
+}
+#define CK(call)                                   \
+  do {                                             \
+    cudaError_t e__ = (call);                      \
+    if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
+  } while (0)
+
+struct Variant {
+  int NS, NMO, LP, ws_doubles;
+  const void *k_el, *k_psi, *k_metro;
+};
+
+template <int NS, int NMO>
+Variant make_variant() {
+  Variant v;
+  v.NS = NS;
+  v.NMO = NMO;
+  v.LP = Geo<NS, NMO>::LP;
+  v.ws_doubles = Geo<NS, NMO>::total;
+  v.k_el = (const void *)local_energy_kernel<NS, NMO, true>;
+  v.k_psi = (const void *)local_energy_kernel<NS, NMO, false>;
+  v.k_metro = (const void *)metropolis_kernel<NS, NMO>;
+  return v;
+}
+
+const std::vector<Variant> &variants() {
+  static const std::vector<Variant> v = {
+      make_variant<1, 2>(),  // H2-like
+      make_variant<2, 2>(),  // LiH-like single determinant
+      make_variant<3, 8>(),  // Li2-like
+      make_variant<4, 8>(),
+      make_variant<7, 14>(),  // CO-like (headline)
+      make_variant<8, 16>(),  // generic upper bound
+  };
+  return v;
+}
+
+double sto_norm(int n, int l, int m, double zeta) {
+  double fact = 1.0;
+  for (int i = 2; i <= 2 * n; ++i) fact *= i;
+  const double radial = std::pow(2.0 * zeta, n + 0.5) / std::sqrt(fact);
+  const double pi = 3.14159265358979323846;
+  double ang = 1.0 / (2.0 * std::sqrt(pi));
+  if (l == 1) ang = std::sqrt(3.0 / (4.0 * pi));
+  if (l == 2) ang = (m <= 2) ? 0.5 * std::sqrt(15.0 / pi) : ((m == 3) ? 0.25 * std::sqrt(15.0 / pi) : 0.25 * std::sqrt(5.0 / pi));
+  return radial * ang;
+}
+
+}  // namespace
+
+struct qmc_system {
+  int device = 0;
+  SysParams P{};
+  Variant var{};
+  int smem_bytes = 0;
+  int blocks_el = 0, blocks_psi = 0, blocks_metro = 0;
+  void *d_shells = nullptr, *d_C = nullptr, *d_dets = nullptr;
+  double *d_stats = nullptr;
+  unsigned long long *d_counter = nullptr;
+  double flops_el = 0, flops_step = 0;
+};
+
+extern "C" {
+
+const char *qmc_status_string(int status) {
+  switch (status) {
+    case QMC_OK: return "ok";
+    case QMC_EINVAL: return "invalid argument";
+    case QMC_EUNSUPPORTED: return "problem outside the compiled limits";
+    case QMC_ENOMEM: return "host allocation failed";
+    case QMC_ECUDA: return g_cuda_err.empty() ? "CUDA error" : g_cuda_err.c_str();
+    default: return "unknown status";
+  }
+}
+
+int64_t qmc_launch_count(int reset) {
+  int64_t v = g_launches;
+  if (reset) g_launches = 0;
+  return v;
+}
+
+void qmc_destroy(qmc_system_t *s) {
+  if (!s) return;
+  cudaSetDevice(s->device);
+  cudaFree(s->d_shells);
+  cudaFree(s->d_C);
+  cudaFree(s->d_dets);
+  cudaFree(s->d_stats);
+  cudaFree(s->d_counter);
+  delete s;
+}
+
+int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
+  if (!d || !out) return QMC_EINVAL;
+  *out = nullptr;
+  if (d->n_atoms < 1 || !d->atom_xyz || !d->atom_Z) return QMC_EINVAL;
+  if (d->n_up < 0 || d->n_dn < 0 || d->n_up + d->n_dn < 1) return QMC_EINVAL;
+  if (d->n_ao < 1 || !d->ao_atom || !d->ao_n || !d->ao_l || !d->ao_m || !d->ao_zeta) return QMC_EINVAL;
+  if (d->n_mo < 1 || !d->mo_coeff) return QMC_EINVAL;
+  if (d->n_det < 1 || !d->ci_coeff) return QMC_EINVAL;
+  if ((d->n_up > 0 && !d->det_up) || (d->n_dn > 0 && !d->det_dn)) return QMC_EINVAL;
+  for (int b = 0; b < d->n_ao; ++b) {
+    const int n = d->ao_n[b], l = d->ao_l[b], m = d->ao_m[b];
+    if (n < 1 || n > 4 || l < 0 || l > 2 || l >= n || m < 0 || m > 2 * l) return QMC_EINVAL;
+    if (!(d->ao_zeta[b] > 0.0)) return QMC_EINVAL;
+    if (d->ao_atom[b] < 0 || d->ao_atom[b] >= d->n_atoms) return QMC_EINVAL;
+  }
+  const int nsp[2] = {d->n_up, d->n_dn};
+  const int32_t *lists[2] = {d->det_up, d->det_dn};
+  for (int sp = 0; sp < 2; ++sp)
+    for (int n = 0; n < d->n_det; ++n)
+      for (int j = 0; j < nsp[sp]; ++j) {
+        const int c = lists[sp][(size_t)n * nsp[sp] + j];
+        if (c < 0 || c >= d->n_mo) return QMC_EINVAL;
+        for (int j2 = 0; j2 < j; ++j2)
+          if (lists[sp][(size_t)n * nsp[sp] + j2] == c) return QMC_EINVAL;
+      }
+  if (d->n_atoms > kMaxAtoms || d->n_up > kMaxSpin || d->n_dn > kMaxSpin || d->n_ao > 256) return QMC_EUNSUPPORTED;
+
+  qmc_system *s = new (std::nothrow) qmc_system;
+  if (!s) return QMC_ENOMEM;
+  s->device = device;
+  SysParams &P = s->P;
+  P.n_atoms = d->n_atoms;
+  P.n_up = d->n_up;
+  P.n_dn = d->n_dn;
+  P.n_e = d->n_up + d->n_dn;
+  P.n_det = d->n_det;
+  P.a_par = d->jastrow_a_par;
+  P.a_anti = d->jastrow_a_anti;
+  P.b = d->jastrow_b;
+  for (int a = 0; a < d->n_atoms; ++a) {
+    for (int c = 0; c < 3; ++c) P.atom[a][c] = d->atom_xyz[3 * a + c];
+    P.atom[a][3] = d->atom_Z[a];
+  }
+  // nuclear repulsion, last term of eq. 1
+  P.vnn = 0.0;
+  for (int a = 0; a < d->n_atoms; ++a)
+    for (int b = a + 1; b < d->n_atoms; ++b) {
+      const double dx = P.atom[a][0] - P.atom[b][0], dy = P.atom[a][1] - P.atom[b][1], dz = P.atom[a][2] - P.atom[b][2];
+      P.vnn += P.atom[a][3] * P.atom[b][3] / std::sqrt(dx * dx + dy * dy + dz * dz);
+    }
+
+  // ---- orbitals actually referenced; excitation descriptors relative to determinant 0
+  std::vector<int> used;  // kernel column -> caller MO index
+  auto col_of = [&](int mo) {
+    for (size_t i = 0; i < used.size(); ++i)
+      if (used[i] == mo) return (int)i;
+    used.push_back(mo);
+    return (int)used.size() - 1;
+  };
+  std::vector<int> virt[2];  // caller MO index of virtual q
+  std::vector<DetRec> dets(d->n_det);
+  bool unsupported = false;
+  for (int sp = 0; sp < 2; ++sp)
+    for (int j = 0; j < nsp[sp]; ++j) P.ref_col[sp][j] = (int8_t)col_of(lists[sp][j]);
+  for (int n = 0; n < d->n_det; ++n) {
+    dets[n].d = d->ci_coeff[n];
+    uint32_t code[2] = {0, 0};
+    for (int sp = 0; sp < 2; ++sp) {
+      int k = 0;
+      uint32_t c = 0;
+      for (int j = 0; j < nsp[sp]; ++j) {
+        const int mo = lists[sp][(size_t)n * nsp[sp] + j];
+        if (mo == lists[sp][j]) continue;
+        int q = -1;
+        for (size_t t = 0; t < virt[sp].size(); ++t)
+          if (virt[sp][t] == mo) q = (int)t;
+        if (q < 0) {
+          virt[sp].push_back(mo);
+          q = (int)virt[sp].size() - 1;
+        }
+        if (k < 2 && q < 16) c |= ((uint32_t)j << (4 + 8 * k)) | ((uint32_t)q << (8 + 8 * k));
+        ++k;
+      }
+      if (k > 2) unsupported = true;
+      code[sp] = c | (uint32_t)std::min(k, 15);
+    }
+    dets[n].up = code[0];
+    dets[n].dn = code[1];
+  }
+  for (int sp = 0; sp < 2; ++sp) {
+    if ((int)virt[sp].size() > kMaxVirt) unsupported = true;
+    P.nv[sp] = (int)virt[sp].size();
+    if (!unsupported)
+      for (int q = 0; q < P.nv[sp]; ++q) P.virt_col[sp][q] = (int8_t)col_of(virt[sp][q]);
+  }
+  if (unsupported || used.size() > 16) {
+    delete s;
+    return QMC_EUNSUPPORTED;
+  }
+  P.n_mo = (int)used.size();
+
+  // ---- pick the instantiation
+  const int ns_max = std::max(d->n_up, d->n_dn), nv_max = std::max(P.nv[0], P.nv[1]);
+  const Variant *var = nullptr;
+  for (const Variant &v : variants())
+    if (v.NS >= ns_max && v.NMO >= P.n_mo && v.LP >= nv_max && v.LP >= ns_max) {
+      var = &v;
+      break;
+    }
+  if (!var) {
+    delete s;
+    return QMC_EUNSUPPORTED;
+  }
+  s->var = *var;
+  const int NMO = var->NMO;
+  P.G = std::max(1, std::min(32 / P.n_e, 16 / var->NS));
+
+  // ---- shell grouping: AOs that share a centre, n, l and zeta share one radial factor
+  struct Rec { ShellRec r; std::vector<int> aos; int atom; };
+  std::vector<Rec> recs;
+  for (int b = 0; b < d->n_ao;) {
+    const int at = d->ao_atom[b], n = d->ao_n[b], l = d->ao_l[b];
+    const double z = d->ao_zeta[b];
+    const int nfun = 2 * l + 1;
+    bool full = (b + nfun <= d->n_ao);
+    for (int t = 0; full && t < nfun; ++t)
+      full = d->ao_atom[b + t] == at && d->ao_n[b + t] == n && d->ao_l[b + t] == l && d->ao_zeta[b + t] == z && d->ao_m[b + t] == t;
+    Rec rc;
+    rc.atom = at;
+    const int k = n - 1 - l;
+    rc.r.zeta = z;
+    rc.r.c1 = 2.0 * z * (k + l + 1);
+    rc.r.c2 = (float)(k * (k + 2 * l + 1));
+    rc.r.k = (int16_t)k;
+    rc.r.m = (int16_t)d->ao_m[b];
+    rc.r.pad = 0;
+    if (l == 0) { rc.r.kind = SH_S; rc.aos = {b}; b += 1; }
+    else if (full) { rc.r.kind = (l == 1) ? SH_P : SH_D; for (int t = 0; t < nfun; ++t) rc.aos.push_back(b + t); b += nfun; }
+    else { rc.r.kind = (l == 1) ? SH_P1 : SH_D1; rc.aos = {b}; b += 1; }
+    recs.push_back(rc);
+  }
+  std::stable_sort(recs.begin(), recs.end(), [](const Rec &a, const Rec &b) { return a.atom < b.atom; });
+  std::vector<ShellRec> shells;
+  std::vector<double> C((size_t)d->n_ao * NMO, 0.0);
+  int row = 0, at_cur = 0;
+  P.shell_begin[0] = 0;
+  for (size_t i = 0; i < recs.size(); ++i) {
+    while (at_cur < recs[i].atom) P.shell_begin[++at_cur] = (int)i;
+    recs[i].r.ao0 = (int16_t)row;
+    for (int b : recs[i].aos) {
+      const double nrm = d->ao_norm ? d->ao_norm[b] : sto_norm(d->ao_n[b], d->ao_l[b], d->ao_m[b], d->ao_zeta[b]);
+      for (int a = 0; a < P.n_mo; ++a) C[(size_t)row * NMO + a] = nrm * d->mo_coeff[(size_t)b * d->n_mo + used[a]];
+      ++row;
+    }
+    shells.push_back(recs[i].r);
+  }
+  while (at_cur < d->n_atoms) P.shell_begin[++at_cur] = (int)recs.size();
+  P.n_shell = (int)shells.size();
+  P.n_ao = d->n_ao;
+
+  // ---- model FP64 work per walker
+  {
+    const double cexp = 40, cdiv = 20, csqrt = 20, clog = 50, csincos = 80;
+    const double ne = P.n_e, nat = P.n_atoms, nsh = P.n_shell, nao = P.n_ao, nmo = P.n_mo, nd = P.n_det;
+    const double npair = ne * (ne - 1) / 2;
+    double lu_el = 0, lu_st = 0;
+    for (int sp = 0; sp < 2; ++sp) {
+      const double n = nsp[sp], v = P.nv[sp];
+      lu_el += 2 * n * n * n + 3 * 2 * n * n * v + 2 * n * n * n + n + n * cdiv;
+      lu_st += 2.0 / 3.0 * n * n * n + 2 * n * n * v + n * cdiv;
+    }
+    s->flops_el = ne * nat * (8 + csqrt + cdiv) + ne * nsh * (8 + cexp) + ne * nao * 21 + 2 * ne * nao * nmo * 2 +
+                  npair * (35 + csqrt + 2 * cdiv) + lu_el + 15 * nd + 100;
+    const double npr = std::ceil(3 * ne / 2);
+    s->flops_step = ne * nat * (8 + csqrt + cdiv) + ne * nsh * (2 + cexp) + ne * nao * 3 + 2 * ne * nao * nmo +
+                    npair * (12 + csqrt + cdiv) + lu_st + 3 * nd + 3 * ne * 2 + npr * (10 + clog + csqrt + csincos) + clog;
+  }
+
+  // ---- upload
+  cudaError_t e = cudaSetDevice(device);
+  if (e != cudaSuccess) { delete s; return cuda_fail(e, "cudaSetDevice"); }
+  const size_t szC = C.size() * sizeof(double), szS = shells.size() * sizeof(ShellRec), szD = dets.size() * sizeof(DetRec);
+  if ((e = cudaMalloc(&s->d_C, szC)) != cudaSuccess || (e = cudaMalloc(&s->d_shells, szS)) != cudaSuccess ||
+      (e = cudaMalloc(&s->d_dets, szD)) != cudaSuccess || (e = cudaMalloc(&s->d_stats, 2 * sizeof(double))) != cudaSuccess ||
+      (e = cudaMalloc(&s->d_counter, sizeof(unsigned long long))) != cudaSuccess ||
+      (e = cudaMemcpy(s->d_C, C.data(), szC, cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMemcpy(s->d_shells, shells.data(), szS, cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMemcpy(s->d_dets, dets.data(), szD, cudaMemcpyHostToDevice)) != cudaSuccess) {
+    int rc = cuda_fail(e, "qmc_setup upload");
+    qmc_destroy(s);
+    return rc;
+  }
+  P.shells = (const ShellRec *)s->d_shells;
+  P.C = (const double *)s->d_C;
+  P.dets = (const DetRec *)s->d_dets;
+  P.smem_const_bytes = (int)((szC + szS + szD + 15) / 16 * 16);
+  s->smem_bytes = P.smem_const_bytes + kWarpsPerBlock * var->ws_doubles * (int)sizeof(double);
+
+  int dev_smem = 0, n_sm = 0;
+  cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+  cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device);
+  if (s->smem_bytes > dev_smem) {
+    qmc_destroy(s);
+    return QMC_EUNSUPPORTED;
+  }
+  const void *ks[3] = {var->k_el, var->k_psi, var->k_metro};
+  int *nb[3] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro};
+  for (int i = 0; i < 3; ++i) {
+    if ((e = cudaFuncSetAttribute(ks[i], cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_bytes)) != cudaSuccess) {
+      int rc = cuda_fail(e, "cudaFuncSetAttribute");
+      qmc_destroy(s);
+      return rc;
+    }
+    int per_sm = 0;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ks[i], kWarpsPerBlock * 32, s->smem_bytes)) != cudaSuccess || per_sm < 1) {
+      int rc = (e != cudaSuccess) ? cuda_fail(e, "occupancy") : QMC_EUNSUPPORTED;
+      qmc_destroy(s);
+      return rc;
+    }
+    *nb[i] = per_sm * n_sm;
+  }
+  *out = s;
+  return QMC_OK;
+}
+
+static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, double *d_eloc,
+                       void *stream, bool el) {
+  if (!s || !d_r || M <= 0) return QMC_EINVAL;
+  CK(cudaSetDevice(s->device));
+  WalkerIO io{d_r, nullptr, d_logpsi, d_sign, d_eloc, M};
+  const int64_t groups = (M + s->P.G - 1) / s->P.G;
+  const int64_t need = (groups + kWarpsPerBlock - 1) / kWarpsPerBlock;
+  const int grid = (int)std::min<int64_t>(need, el ? s->blocks_el : s->blocks_psi);
+  void *args[2] = {(void *)&s->P, (void *)&io};
+  CK(cudaLaunchKernel(el ? s->var.k_el : s->var.k_psi, dim3(grid), dim3(kWarpsPerBlock * 32), args, s->smem_bytes,
+                      (cudaStream_t)stream));
+  ++g_launches;
+  return QMC_OK;
+}
+
+int qmc_local_energy(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, double *d_eloc,
+                     void *cuda_stream) {
+  return launch_eval(s, d_r, M, d_logpsi, d_sign, d_eloc, cuda_stream, true);
+}
+
+int qmc_log_psi(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, void *cuda_stream) {
+  return launch_eval(s, d_r, M, d_logpsi, d_sign, nullptr, cuda_stream, false);
+}
+
+int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t n_sweeps, uint64_t seed,
+                   uint64_t sweep_offset, int64_t walker_offset, double *d_logpsi, double *d_sign, uint8_t *d_accept,
+                   double *d_eloc_acc, int64_t *h_n_accepted, void *cuda_stream) {
+  if (!s || !d_r || M <= 0 || !(step > 0.0) || n_sweeps < 0 || walker_offset < 0) return QMC_EINVAL;
+  if (sweep_offset + (uint64_t)n_sweeps >= (1ull << 32)) return QMC_EINVAL;
+  CK(cudaSetDevice(s->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  WalkerIO io{d_r, d_r, d_logpsi, d_sign, nullptr, M};
+  MetroParams mp{};
+  mp.step = step;
+  mp.n_sweeps = n_sweeps;
+  mp.key0 = (uint32_t)(seed & 0xFFFFFFFFu);
+  mp.key1 = (uint32_t)(seed >> 32);
+  mp.sweep0 = (uint32_t)sweep_offset;
+  mp.walker_offset = walker_offset;
+  mp.accept = d_accept;
+  mp.eloc_acc = d_eloc_acc;
+  mp.n_accepted = h_n_accepted ? s->d_counter : nullptr;
+  if (h_n_accepted) CK(cudaMemsetAsync(s->d_counter, 0, sizeof(unsigned long long), st));
+  const int64_t groups = (M + s->P.G - 1) / s->P.G;
+  const int64_t need = (groups + kWarpsPerBlock - 1) / kWarpsPerBlock;
+  const int grid = (int)std::min<int64_t>(need, s->blocks_metro);
+  void *args[3] = {(void *)&s->P, (void *)&io, (void *)&mp};
+  CK(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPerBlock * 32), args, s->smem_bytes, st));
+  ++g_launches;
+  if (h_n_accepted) {
+    unsigned long long v = 0;
+    CK(cudaMemcpyAsync(&v, s->d_counter, sizeof(v), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    *h_n_accepted = (int64_t)v;
+  }
+  return QMC_OK;
+}
+
+int qmc_batch_stats(const double *d_x, int64_t M, double *h_mean, double *h_stderr, void *cuda_stream) {
+  if (!d_x || M <= 0) return QMC_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  double *d_out = nullptr;
+  CK(cudaMallocAsync(&d_out, 2 * sizeof(double), st));
+  batch_stats_kernel<<<1, 1024, 0, st>>>(d_x, M, d_out);
+  ++g_launches;
+  double h[2] = {0, 0};
+  cudaError_t e = cudaMemcpyAsync(h, d_out, sizeof(h), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaFreeAsync(d_out, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return cuda_fail(e, "qmc_batch_stats");
+  if (h_mean) *h_mean = h[0];
+  if (h_stderr) *h_stderr = h[1];
+  return QMC_OK;
+}
+
+int qmc_fp64_peak(int device, int kind, int reps, double *h_tflops) {
+  if (!h_tflops || kind < 0 || kind > 2 || reps < 1) return QMC_EINVAL;
+  CK(cudaSetDevice(device));
+  int n_sm = 0;
+  CK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device));
+  double *d_out = nullptr;
+  CK(cudaMalloc(&d_out, sizeof(double)));
+  cudaEvent_t e0, e1;
+  CK(cudaEventCreate(&e0));
+  CK(cudaEventCreate(&e1));
+  const int iters = 4096, blocks = n_sm * 8, threads = 256;
+  double best = 0.0;
+  for (int r = 0; r < reps + 1; ++r) {
+    CK(cudaEventRecord(e0, 0));
+    if (kind == 0) fp64_peak_kernel<0><<<blocks, threads>>>(d_out, iters, 1.0);
+    if (kind == 1) fp64_peak_kernel<1><<<blocks, threads>>>(d_out, iters, 1.0);
+    if (kind == 2) fp64_peak_kernel<2><<<blocks, threads>>>(d_out, iters, 1.0);
+    ++g_launches;
+    CK(cudaEventRecord(e1, 0));
+    CK(cudaEventSynchronize(e1));
+    float ms = 0;
+    CK(cudaEventElapsedTime(&ms, e0, e1));
+    double flops_thread = 0;
+    if (kind == 0 || kind == 2) flops_thread += (double)iters * 32 * 2;
+    if (kind == 1 || kind == 2) flops_thread += (double)iters * 4 * 512 / 32;
+    const double tf = flops_thread * blocks * threads / (ms * 1e-3) / 1e12;
+    if (r > 0 && tf > best) best = tf;  // first launch is warm-up
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(d_out);
+  *h_tflops = best;
+  return QMC_OK;
+}
+
+double qmc_model_flops(const qmc_system_t *s, int which) {
+  if (!s) return 0.0;
+  return which == 0 ? s->flops_el : s->flops_step;
+}
+
+}  // extern "C"

@@ -1,0 +1,352 @@
+// qmc_eval.cuh -- the fused per-walker evaluator: STO atomic orbitals -> MO contraction
+// -> Pade Jastrow -> per-spin Gauss-Jordan (A0^-1 [Av | B0 | Bv]) -> excitation tables
+// -> CI sum -> E_L assembly.  Citations are /root/reference/PAPER.md lines.
+#pragma once
+#include "qmc_device.cuh"
+
+namespace qmc {
+
+// ---------------------------------------------------------------------------------
+// stage a4: rank-1 update of the MO accumulators with one AO.
+// crow points at C[beta][0..NMO) in shared memory (same address in every lane: broadcast).
+// ---------------------------------------------------------------------------------
+template <int NMO, bool EL>
+__device__ __forceinline__ void contract(const double *__restrict__ crow, double phi, double bop,
+                                         double (&accP)[NMO], double (&accB)[EL ? NMO : 1]) {
+  const double2 *c2 = reinterpret_cast<const double2 *>(crow);
+#pragma unroll
+  for (int a = 0; a < NMO / 2; ++a) {
+    double2 c = c2[a];
+    accP[2 * a] = fma(phi, c.x, accP[2 * a]);
+    accP[2 * a + 1] = fma(phi, c.y, accP[2 * a + 1]);
+    if (EL) {
+      accB[2 * a] = fma(bop, c.x, accB[2 * a]);
+      accB[2 * a + 1] = fma(bop, c.y, accB[2 * a + 1]);
+    }
+  }
+}
+
+// excitation factor of one spin of one determinant relative to the reference:
+//   R  = det T[p,q]                     = D_X / D_0           (reading Q8; H.1)
+//   Rd = Tr(adj(T[p,q]) Mtab[p,q])      = R * Tr((P A0^-1 A_X P)^-1 P M P)   (F.6)
+template <int LP, bool EL>
+__device__ __forceinline__ void excite(uint32_t e, const double *__restrict__ T, const double *__restrict__ Mt,
+                                       double &R, double &Rd) {
+  int k = e & 15;
+  R = 1.0;
+  Rd = 0.0;
+  if (k == 0) return;
+  int p1 = (e >> 4) & 15, q1 = (e >> 8) & 15;
+  if (k == 1) {
+    R = T[p1 * LP + q1];
+    if (EL) Rd = Mt[p1 * LP + q1];
+    return;
+  }
+  int p2 = (e >> 12) & 15, q2 = (e >> 16) & 15;
+  double t11 = T[p1 * LP + q1], t12 = T[p1 * LP + q2], t21 = T[p2 * LP + q1], t22 = T[p2 * LP + q2];
+  R = t11 * t22 - t12 * t21;
+  if (EL) {
+    double m11 = Mt[p1 * LP + q1], m12 = Mt[p1 * LP + q2], m21 = Mt[p2 * LP + q1], m22 = Mt[p2 * LP + q2];
+    Rd = t22 * m11 - t12 * m21 - t21 * m12 + t11 * m22;
+  }
+}
+
+// ---------------------------------------------------------------------------------
+// Evaluate the G walkers of this warp.  Lane = g * n_e + e holds electron e of walker g
+// at (x, y, z).  Results for walker g are left in ws[oRes + 3 g + {0,1,2}] =
+// {log|Psi|, sign, E_L} (E_L only if EL).  All 32 lanes must call.
+// ---------------------------------------------------------------------------------
+template <int NS, int NMO, bool EL>
+__device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sShell,
+                             const double *__restrict__ sC, const DetRec *__restrict__ sDet,
+                             double *__restrict__ ws, double x, double y, double z, int lane) {
+  using GE = Geo<NS, NMO>;
+  constexpr int LP = GE::LP, PP = GE::PP;
+  const int ne = P.n_e, G = P.G;
+  const int g = lane / ne, e = lane - g * ne;
+  const bool active = lane < G * ne;
+  double *sPhi = ws + GE::oPhi, *sB = ws + GE::oB, *sXYZ = ws + GE::oXYZ, *sPart = ws + GE::oPart;
+  double *sG = ws + GE::oG, *sT = ws + GE::oT, *sM = ws + GE::oM, *sProb = ws + GE::oProb;
+  double *sRes = ws + GE::oRes;
+
+  // ---- publish coordinates for the pair loop
+  sXYZ[lane * 3 + 0] = x;
+  sXYZ[lane * 3 + 1] = y;
+  sXYZ[lane * 3 + 2] = z;
+  __syncwarp();
+
+  // ---- stage a5: Pade Jastrow (D.1) and e-e repulsion (eq. 1)
+  double J2 = 0.0, gJx = 0.0, gJy = 0.0, gJz = 0.0, lapJ = 0.0, vee2 = 0.0;
+  {
+    const bool up = e < P.n_up;
+    const int base = (active ? g : 0) * ne;
+    for (int j = 0; j < ne; ++j) {
+      double dx = x - sXYZ[(base + j) * 3 + 0];
+      double dy = y - sXYZ[(base + j) * 3 + 1];
+      double dz = z - sXYZ[(base + j) * 3 + 2];
+      if (j == e) continue;
+      double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+      double r = sqrt(r2);
+      double ri = 1.0 / r;
+      double a = ((j < P.n_up) == up) ? P.a_par : P.a_anti;
+      double di = 1.0 / fma(P.b, r, 1.0);
+      double adi = a * di;
+      J2 = fma(adi, r, J2);  // u = a r / (1 + b r)
+      if (EL) {
+        double u1 = adi * di;                  // u'  = a / (1 + b r)^2
+        double u2 = -2.0 * P.b * u1 * di;      // u'' = -2 a b / (1 + b r)^3
+        double s = u1 * ri;
+        gJx = fma(s, dx, gJx);
+        gJy = fma(s, dy, gJy);
+        gJz = fma(s, dz, gJz);
+        lapJ += fma(2.0, s, u2);               // lap_i K(r_ij) = u'' + 2 u'/r
+        vee2 += ri;
+      }
+    }
+  }
+
+  // ---- stages a1-a4: STO shells and AO -> MO contraction.
+  // For E_L the gradient and Laplacian are folded into ONE operator per AO (stage a6):
+  //   b = -1/2 lap(phi) - grad_i J . grad(phi)      (middle and last terms of F.1)
+  double accP[NMO];
+  double accB[EL ? NMO : 1];
+#pragma unroll
+  for (int a = 0; a < NMO; ++a) accP[a] = 0.0;
+#pragma unroll
+  for (int a = 0; a < (EL ? NMO : 1); ++a) accB[a] = 0.0;
+  double ven = 0.0;
+  for (int at = 0; at < P.n_atoms; ++at) {
+    const double dx = x - P.atom[at][0], dy = y - P.atom[at][1], dz = z - P.atom[at][2];
+    const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+    const double r = sqrt(r2);
+    const double ri = 1.0 / r;
+    if (EL) ven = fma(-P.atom[at][3], ri, ven);
+    const double gd = EL ? fma(gJx, dx, fma(gJy, dy, gJz * dz)) * ri : 0.0;  // grad J . d / r
+    for (int s = P.shell_begin[at]; s < P.shell_begin[at + 1]; ++s) {
+      const ShellRec sh = sShell[s];
+      const double ex = exp(-sh.zeta * r);
+      const int k = sh.k;
+      const double gr = (k == 0) ? ex : ((k == 1) ? ex * r : ((k == 2) ? ex * r2 : ex * r2 * r));
+      double h = 0.0;
+      if (EL) {
+        // lap(S r^k e^{-zeta r}) = phi * [zeta^2 - 2 zeta (k+l+1)/r + k (k+2l+1)/r^2]
+        const double lapfac = fma(fma((double)sh.c2, ri, -sh.c1), ri, sh.zeta * sh.zeta);
+        const double radlog = fma((double)k, ri, -sh.zeta);  // g'/g
+        h = fma(-0.5, lapfac, -radlog * gd);
+      }
+      const double *crow = sC + sh.ao0 * NMO;
+      switch (sh.kind) {
+        case SH_S: {
+          contract<NMO, EL>(crow, gr, gr * h, accP, accB);
+        } break;
+        case SH_P: {
+          contract<NMO, EL>(crow, gr * dx, gr * fma(dx, h, -gJx), accP, accB);
+          contract<NMO, EL>(crow + NMO, gr * dy, gr * fma(dy, h, -gJy), accP, accB);
+          contract<NMO, EL>(crow + 2 * NMO, gr * dz, gr * fma(dz, h, -gJz), accP, accB);
+        } break;
+        case SH_D: {
+          double S, gs;
+          S = dx * dy; gs = fma(gJx, dy, gJy * dx);
+          contract<NMO, EL>(crow, gr * S, gr * fma(S, h, -gs), accP, accB);
+          S = dy * dz; gs = fma(gJy, dz, gJz * dy);
+          contract<NMO, EL>(crow + NMO, gr * S, gr * fma(S, h, -gs), accP, accB);
+          S = dz * dx; gs = fma(gJz, dx, gJx * dz);
+          contract<NMO, EL>(crow + 2 * NMO, gr * S, gr * fma(S, h, -gs), accP, accB);
+          S = fma(dx, dx, -dy * dy); gs = 2.0 * fma(gJx, dx, -gJy * dy);
+          contract<NMO, EL>(crow + 3 * NMO, gr * S, gr * fma(S, h, -gs), accP, accB);
+          S = fma(2.0 * dz, dz, -fma(dx, dx, dy * dy));
+          gs = 2.0 * fma(2.0 * gJz, dz, -fma(gJx, dx, gJy * dy));
+          contract<NMO, EL>(crow + 4 * NMO, gr * S, gr * fma(S, h, -gs), accP, accB);
+        } break;
+        case SH_P1: {
+          const int m = sh.m;
+          const double S = (m == 0) ? dx : ((m == 1) ? dy : dz);
+          const double gs = (m == 0) ? gJx : ((m == 1) ? gJy : gJz);
+          contract<NMO, EL>(crow, gr * S, gr * fma(S, h, -gs), accP, accB);
+        } break;
+        default: {  // SH_D1
+          const int m = sh.m;
+          double S, gs;
+          if (m == 0) { S = dx * dy; gs = fma(gJx, dy, gJy * dx); }
+          else if (m == 1) { S = dy * dz; gs = fma(gJy, dz, gJz * dy); }
+          else if (m == 2) { S = dz * dx; gs = fma(gJz, dx, gJx * dz); }
+          else if (m == 3) { S = fma(dx, dx, -dy * dy); gs = 2.0 * fma(gJx, dx, -gJy * dy); }
+          else { S = fma(2.0 * dz, dz, -fma(dx, dx, dy * dy)); gs = 2.0 * fma(2.0 * gJz, dz, -fma(gJx, dx, gJy * dy)); }
+          contract<NMO, EL>(crow, gr * S, gr * fma(S, h, -gs), accP, accB);
+        } break;
+      }
+    }
+  }
+  // hand the MO rows over
+  {
+    double2 *dst = reinterpret_cast<double2 *>(sPhi + lane * NMO);
+#pragma unroll
+    for (int a = 0; a < NMO / 2; ++a) dst[a] = make_double2(accP[2 * a], accP[2 * a + 1]);
+    if (EL) {
+      double2 *dstb = reinterpret_cast<double2 *>(sB + lane * NMO);
+#pragma unroll
+      for (int a = 0; a < NMO / 2; ++a) dstb[a] = make_double2(accB[2 * a], accB[2 * a + 1]);
+    }
+    // per-electron scalars: J/2-sum and the electron's share of the energy
+    sPart[lane * 2 + 0] = 0.5 * J2;
+    sPart[lane * 2 + 1] =
+        EL ? (fma(-0.5, lapJ + fma(gJx, gJx, fma(gJy, gJy, gJz * gJz)), fma(0.5, vee2, ven))) : 0.0;
+  }
+  __syncwarp();
+
+  // ---- stages a7-a8: per (walker, spin) Gauss-Jordan with partial pivoting on the augmented
+  // matrix [A0 | Av | B0 | Bv]; lane c of a group of LP lanes owns column c of every block.
+  // Result: T = A0^-1 Av, Gm = A0^-1 B0, H = A0^-1 Bv, det A0.  (F.6/F.7)
+  {
+    const int c = lane % LP, slot = lane / LP, gbase = lane - c;
+    const int nprob = 2 * G;
+    for (int pass = 0; pass * PP < nprob; ++pass) {
+      const int pr = pass * PP + slot;
+      const bool pvalid = pr < nprob;
+      const int pg = pvalid ? (pr >> 1) : 0, sp = pr & 1;
+      const int ns = sp ? P.n_dn : P.n_up, nv = P.nv[sp], e0 = sp ? P.n_up : 0;
+      double a0[NS], av[NS], b0[EL ? NS : 1], bv[EL ? NS : 1];
+      {
+        const bool cA = c < ns, cV = c < nv;
+        const int colA = cA ? P.ref_col[sp][c < kMaxSpin ? c : 0] : 0;
+        const int colV = cV ? P.virt_col[sp][c < kMaxVirt ? c : 0] : 0;
+#pragma unroll
+        for (int i = 0; i < NS; ++i) {
+          const int row = (pg * ne + e0 + (i < ns ? i : 0)) * NMO;
+          const bool ri = i < ns;
+          a0[i] = (ri && cA) ? sPhi[row + colA] : ((i == c) ? 1.0 : 0.0);  // identity padding
+          av[i] = (ri && cV) ? sPhi[row + colV] : 0.0;
+          if (EL) {
+            b0[i] = (ri && cA) ? sB[row + colA] : 0.0;
+            bv[i] = (ri && cV) ? sB[row + colV] : 0.0;
+          }
+        }
+      }
+      double det = 1.0;
+#pragma unroll
+      for (int k = 0; k < NS; ++k) {
+        int p = k;
+        double best = fabs(a0[k]);
+#pragma unroll
+        for (int i = k + 1; i < NS; ++i) {
+          double v = fabs(a0[i]);
+          if (v > best) { best = v; p = i; }
+        }
+        p = __shfl_sync(0xffffffffu, p, gbase + k);
+#pragma unroll
+        for (int i = k + 1; i < NS; ++i) {
+          if (p == i) {
+            double t;
+            t = a0[k]; a0[k] = a0[i]; a0[i] = t;
+            t = av[k]; av[k] = av[i]; av[i] = t;
+            if (EL) {
+              t = b0[k]; b0[k] = b0[i]; b0[i] = t;
+              t = bv[k]; bv[k] = bv[i]; bv[i] = t;
+            }
+          }
+        }
+        double f[NS];
+#pragma unroll
+        for (int i = 0; i < NS; ++i) f[i] = __shfl_sync(0xffffffffu, a0[i], gbase + k);
+        const double piv = f[k];
+        const double inv = 1.0 / piv;
+        det *= (p != k) ? -piv : piv;
+        {
+          double t = a0[k] * inv;
+          a0[k] = t;
+#pragma unroll
+          for (int i = 0; i < NS; ++i) if (i != k) a0[i] = fma(-f[i], t, a0[i]);
+          t = av[k] * inv;
+          av[k] = t;
+#pragma unroll
+          for (int i = 0; i < NS; ++i) if (i != k) av[i] = fma(-f[i], t, av[i]);
+          if (EL) {
+            t = b0[k] * inv;
+            b0[k] = t;
+#pragma unroll
+            for (int i = 0; i < NS; ++i) if (i != k) b0[i] = fma(-f[i], t, b0[i]);
+            t = bv[k] * inv;
+            bv[k] = t;
+#pragma unroll
+            for (int i = 0; i < NS; ++i) if (i != k) bv[i] = fma(-f[i], t, bv[i]);
+          }
+        }
+      }
+      // t0 = Tr(A0^-1 B0)   (G.7, applied to the combined operator)
+      double t0 = 0.0;
+      if (EL) {
+#pragma unroll
+        for (int i = 0; i < NS; ++i) if (i == c) t0 = b0[i];
+#pragma unroll
+        for (int m = 1; m < LP; m <<= 1) t0 += shfl_xor_d(t0, m);
+        // Mtab = A0^-1 Bv - (A0^-1 B0) T   (F.7), column c in this lane
+        double *gs = sG + slot * NS * NS;
+        if (c < NS) {
+#pragma unroll
+          for (int i = 0; i < NS; ++i) gs[c * NS + i] = b0[i];  // gs[j][i] = Gm[i][j]
+        }
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < NS; ++j) {
+          const double tj = av[j];
+#pragma unroll
+          for (int i = 0; i < NS; ++i) bv[i] = fma(-gs[j * NS + i], tj, bv[i]);
+        }
+        __syncwarp();
+      }
+      if (pvalid) {
+#pragma unroll
+        for (int i = 0; i < NS; ++i) {
+          sT[(pr * NS + i) * LP + c] = av[i];
+          if (EL) sM[(pr * NS + i) * LP + c] = bv[i];
+        }
+        if (c == 0) {
+          sProb[pr * 4 + 0] = log(fabs(det));
+          sProb[pr * 4 + 1] = (det > 0.0) ? 1.0 : ((det < 0.0) ? -1.0 : 0.0);
+          sProb[pr * 4 + 2] = t0;
+        }
+      }
+    }
+  }
+  __syncwarp();
+
+  // ---- stage a9: CI sum over determinants (eq. 4; F.2/F.4)
+  // ---- stage a10: assembly (eq. 1; F.1)
+  {
+    const int LW = pow2floor(32 / G);
+    const int wg = lane / LW, sub = lane - wg * LW;
+    const bool wvalid = wg < G;
+    const int pu = 2 * (wvalid ? wg : 0), pd = pu + 1;
+    const double *Tu = sT + pu * NS * LP, *Td = sT + pd * NS * LP;
+    const double *Mu = sM + pu * NS * LP, *Md = sM + pd * NS * LP;
+    double den = 0.0, num = 0.0;
+    for (int n = sub; n < P.n_det; n += LW) {
+      const DetRec dr = sDet[n];
+      double Ru, Du, Rd, Dd;
+      excite<LP, EL>(dr.up, Tu, Mu, Ru, Du);
+      excite<LP, EL>(dr.dn, Td, Md, Rd, Dd);
+      const double w = dr.d * Ru;
+      den = fma(w, Rd, den);
+      if (EL) num = fma(dr.d, Du * Rd, fma(w, Dd, num));
+    }
+    for (int m = 1; m < LW; m <<= 1) {
+      den += shfl_xor_d(den, m);
+      if (EL) num += shfl_xor_d(num, m);
+    }
+    if (wvalid && sub == 0) {
+      double Jsum = 0.0, esum = 0.0;
+      for (int j = 0; j < ne; ++j) {
+        Jsum += sPart[(wg * ne + j) * 2 + 0];
+        esum += sPart[(wg * ne + j) * 2 + 1];
+      }
+      const double lu = sProb[pu * 4 + 0], ld = sProb[pd * 4 + 0];
+      const double sgn = sProb[pu * 4 + 1] * sProb[pd * 4 + 1];
+      sRes[wg * 3 + 0] = Jsum + lu + ld + log(fabs(den));
+      sRes[wg * 3 + 1] = sgn * ((den > 0.0) ? 1.0 : ((den < 0.0) ? -1.0 : 0.0));
+      if (EL) sRes[wg * 3 + 2] = esum + (sProb[pu * 4 + 2] + sProb[pd * 4 + 2]) + num / den + P.vnn;
+    }
+  }
+  __syncwarp();
+}
+
+}  // namespace qmc

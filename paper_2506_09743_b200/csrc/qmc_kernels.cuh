@@ -1,0 +1,264 @@
+// qmc_kernels.cuh -- __global__ entry points: local energy / log psi, persistent
+// Metropolis, batch statistics.  One warp = G walkers per pass, grid-stride over groups.
+#pragma once
+#include "qmc_eval.cuh"
+
+namespace qmc {
+
+// copy the constants into shared memory; returns pointers.  Layout: C | shells | dets.
+template <int NMO>
+__device__ __forceinline__ void load_constants(const SysParams &P, unsigned char *smem, const double *&sC,
+                                               const ShellRec *&sShell, const DetRec *&sDet, double *&wsBase) {
+  double *c = reinterpret_cast<double *>(smem);
+  const int nC = P.n_ao * NMO;
+  for (int i = threadIdx.x; i < nC; i += blockDim.x) c[i] = P.C[i];
+  ShellRec *sh = reinterpret_cast<ShellRec *>(c + nC);
+  {
+    const double *src = reinterpret_cast<const double *>(P.shells);
+    double *dst = reinterpret_cast<double *>(sh);
+    for (int i = threadIdx.x; i < P.n_shell * 4; i += blockDim.x) dst[i] = src[i];
+  }
+  DetRec *dt = reinterpret_cast<DetRec *>(sh + P.n_shell);
+  {
+    const double *src = reinterpret_cast<const double *>(P.dets);
+    double *dst = reinterpret_cast<double *>(dt);
+    for (int i = threadIdx.x; i < P.n_det * 2; i += blockDim.x) dst[i] = src[i];
+  }
+  sC = c;
+  sShell = sh;
+  sDet = dt;
+  wsBase = reinterpret_cast<double *>(smem + P.smem_const_bytes);
+  __syncthreads();
+}
+
+// benign coordinates for lanes that own no electron (results are discarded)
+__device__ __forceinline__ void dummy_xyz(int lane, double &x, double &y, double &z) {
+  x = 0.37 + 0.11 * lane;
+  y = -0.21 + 0.07 * lane;
+  z = 0.53 - 0.05 * lane;
+}
+
+template <int NS, int NMO, bool EL>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+    local_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const double *sC;
+  const ShellRec *sShell;
+  const DetRec *sDet;
+  double *wsBase;
+  load_constants<NMO>(P, smem, sC, sShell, sDet, wsBase);
+  using GE = Geo<NS, NMO>;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  double *ws = wsBase + warp * GE::total;
+  const int ne = P.n_e, G = P.G;
+  const int g = lane / ne, e = lane - g * ne;
+  const int64_t n_groups = (io.M + G - 1) / G;
+  const int64_t stride = (int64_t)gridDim.x * kWarpsPerBlock;
+  for (int64_t grp = (int64_t)blockIdx.x * kWarpsPerBlock + warp; grp < n_groups; grp += stride) {
+    const int64_t w = grp * G + g;
+    const bool own = (g < G) && (w < io.M);
+    double x, y, z;
+    if (own) {
+      x = io.r_in[((int64_t)e * 3 + 0) * io.M + w];
+      y = io.r_in[((int64_t)e * 3 + 1) * io.M + w];
+      z = io.r_in[((int64_t)e * 3 + 2) * io.M + w];
+    } else {
+      dummy_xyz(lane, x, y, z);
+    }
+    eval_walkers<NS, NMO, EL>(P, sShell, sC, sDet, ws, x, y, z, lane);
+    if (lane < G) {
+      const int64_t wo = grp * G + lane;
+      if (wo < io.M) {
+        const double *res = ws + GE::oRes + lane * 3;
+        if (io.logpsi) io.logpsi[wo] = res[0];
+        if (io.sign) io.sign[wo] = res[1];
+        if (EL && io.eloc) io.eloc[wo] = res[2];
+      }
+    }
+    __syncwarp();
+  }
+}
+
+// ---------------------------------------------------------------------------------
+// Persistent all-electron Metropolis (readings Q9, Q10).
+// Walker coordinates and log|Psi| stay in registers for all sweeps.
+// ---------------------------------------------------------------------------------
+template <int NS, int NMO>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+    metropolis_kernel(const __grid_constant__ SysParams P, const WalkerIO io, const MetroParams mp) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const double *sC;
+  const ShellRec *sShell;
+  const DetRec *sDet;
+  double *wsBase;
+  load_constants<NMO>(P, smem, sC, sShell, sDet, wsBase);
+  using GE = Geo<NS, NMO>;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  double *ws = wsBase + warp * GE::total;
+  double *sProp = ws + GE::oProp;       // [G][3 ne] normals
+  double *sLogU = sProp + 96;           // [G]
+  const double *sRes = ws + GE::oRes;
+  const int ne = P.n_e, G = P.G, nc = 3 * ne, npair = (nc + 1) / 2;
+  const int g = lane / ne, e = lane - g * ne;
+  const int64_t n_groups = (io.M + G - 1) / G;
+  const int64_t stride = (int64_t)gridDim.x * kWarpsPerBlock;
+  unsigned long long acc_count = 0;
+  for (int64_t grp = (int64_t)blockIdx.x * kWarpsPerBlock + warp; grp < n_groups; grp += stride) {
+    const int64_t w = grp * G + g;
+    const bool own = (g < G) && (w < io.M);
+    double x, y, z;
+    if (own) {
+      x = io.r_out[((int64_t)e * 3 + 0) * io.M + w];
+      y = io.r_out[((int64_t)e * 3 + 1) * io.M + w];
+      z = io.r_out[((int64_t)e * 3 + 2) * io.M + w];
+    } else {
+      dummy_xyz(lane, x, y, z);
+    }
+    eval_walkers<NS, NMO, false>(P, sShell, sC, sDet, ws, x, y, z, lane);
+    double lp = sRes[(own ? g : 0) * 3 + 0], sg = sRes[(own ? g : 0) * 3 + 1];
+    double eacc = 0.0;
+    __syncwarp();
+    for (int sw = 0; sw < mp.n_sweeps; ++sw) {
+      // --- draws: lanes share the (walker, pair) blocks of the G walkers
+      for (int idx = lane; idx < G * (npair + 1); idx += 32) {
+        const int dg = idx / (npair + 1), j = idx - dg * (npair + 1);
+        const uint64_t gw = (uint64_t)(mp.walker_offset + grp * G + dg);
+        uint32_t o[4];
+        philox4x32_10((uint32_t)gw, mp.sweep0 + (uint32_t)sw, (j == npair) ? 0xFFFFFFFFu : (uint32_t)j,
+                      (uint32_t)(gw >> 32), mp.key0, mp.key1, o);
+        const double u1 = u53(o[0], o[1]);
+        if (j == npair) {
+          sLogU[dg] = log(u1);
+        } else {
+          const double u2 = u53(o[2], o[3]);
+          const double rho = sqrt(-2.0 * log(u1));
+          double sn, cs;
+          sincos(6.283185307179586 * u2, &sn, &cs);
+          sProp[dg * nc + 2 * j] = rho * cs;
+          if (2 * j + 1 < nc) sProp[dg * nc + 2 * j + 1] = rho * sn;
+        }
+      }
+      __syncwarp();
+      double xp = x, yp = y, zp = z;
+      if (own) {
+        xp = fma(mp.step, sProp[g * nc + 3 * e + 0], x);
+        yp = fma(mp.step, sProp[g * nc + 3 * e + 1], y);
+        zp = fma(mp.step, sProp[g * nc + 3 * e + 2], z);
+      }
+      const double logu = sLogU[own ? g : 0];
+      __syncwarp();
+      eval_walkers<NS, NMO, false>(P, sShell, sC, sDet, ws, xp, yp, zp, lane);
+      const double lp2 = sRes[(own ? g : 0) * 3 + 0], sg2 = sRes[(own ? g : 0) * 3 + 1];
+      const bool ok = own && (logu < 2.0 * (lp2 - lp));  // false for NaN and for Psi' = 0
+      if (ok) { x = xp; y = yp; z = zp; lp = lp2; sg = sg2; }
+      if (own && e == 0) {
+        if (mp.accept) mp.accept[(int64_t)sw * io.M + w] = ok ? 1 : 0;
+        acc_count += ok ? 1 : 0;
+      }
+      __syncwarp();
+      if (mp.eloc_acc) {
+        eval_walkers<NS, NMO, true>(P, sShell, sC, sDet, ws, x, y, z, lane);
+        eacc += sRes[(own ? g : 0) * 3 + 2];
+        __syncwarp();
+      }
+    }
+    if (own) {
+      io.r_out[((int64_t)e * 3 + 0) * io.M + w] = x;
+      io.r_out[((int64_t)e * 3 + 1) * io.M + w] = y;
+      io.r_out[((int64_t)e * 3 + 2) * io.M + w] = z;
+      if (e == 0) {
+        if (io.logpsi) io.logpsi[w] = lp;
+        if (io.sign) io.sign[w] = sg;
+        if (mp.eloc_acc) mp.eloc_acc[w] = eacc;
+      }
+    }
+    __syncwarp();
+  }
+  if (mp.n_accepted) {
+    for (int m = 16; m > 0; m >>= 1) acc_count += __shfl_xor_sync(0xffffffffu, acc_count, m);
+    if (lane == 0 && acc_count) atomicAdd(mp.n_accepted, acc_count);
+  }
+}
+
+// ---------------------------------------------------------------------------------
+// batch mean and standard error (eq. 3): one block, fixed tree, two passes
+// out[0] = mean, out[1] = stderr
+// ---------------------------------------------------------------------------------
+__device__ __forceinline__ double block_sum_1024(double v, double *sh) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int m = 16; m > 0; m >>= 1) v += shfl_xor_d(v, m);
+  __syncthreads();
+  if (lane == 0) sh[warp] = v;
+  __syncthreads();
+  double t = (threadIdx.x < (blockDim.x >> 5)) ? sh[threadIdx.x] : 0.0;
+  if (warp == 0) {
+    for (int m = 16; m > 0; m >>= 1) t += shfl_xor_d(t, m);
+    if (lane == 0) sh[32] = t;
+  }
+  __syncthreads();
+  return sh[32];
+}
+
+__global__ void __launch_bounds__(1024) batch_stats_kernel(const double *__restrict__ x, int64_t M, double *out) {
+  __shared__ double sh[33];
+  // pass 1: Kahan partial sums per thread
+  double s = 0.0, c = 0.0;
+  for (int64_t i = threadIdx.x; i < M; i += blockDim.x) {
+    double y = x[i] - c, t = s + y;
+    c = (t - s) - y;
+    s = t;
+  }
+  const double mean = block_sum_1024(s, sh) / (double)M;
+  s = 0.0;
+  c = 0.0;
+  for (int64_t i = threadIdx.x; i < M; i += blockDim.x) {
+    double d = x[i] - mean;
+    double y = d * d - c, t = s + y;
+    c = (t - s) - y;
+    s = t;
+  }
+  const double ss = block_sum_1024(s, sh);
+  if (threadIdx.x == 0) {
+    out[0] = mean;
+    out[1] = (M > 1) ? sqrt(ss / (double)(M - 1) / (double)M) : 0.0;
+  }
+}
+
+// ---------------------------------------------------------------------------------
+// FP64 peak microbenchmarks (roofline denominator; BASELINE.json north_star)
+// ---------------------------------------------------------------------------------
+__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(d0), "+d"(d1)
+               : "d"(a), "d"(b));
+}
+
+template <int KIND>
+__global__ void __launch_bounds__(256) fp64_peak_kernel(double *out, int iters, double seed) {
+  double a[8], m0[4], m1[4];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) a[i] = seed + threadIdx.x * 1e-3 + i;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { m0[i] = 0.0; m1[i] = 0.0; }
+  const double x = 1.0 + seed * 1e-9, y = seed * 1e-7;
+  for (int it = 0; it < iters; ++it) {
+    if (KIND == 0 || KIND == 2) {
+#pragma unroll
+      for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int i = 0; i < 8; ++i) a[i] = fma(a[i], x, y);
+    }
+    if (KIND == 1 || KIND == 2) {
+#pragma unroll
+      for (int i = 0; i < 4; ++i) dmma884(m0[i], m1[i], x, y);
+    }
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += a[i];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) s += m0[i] + m1[i];
+  if (s == 123.456) out[0] = s;  // keep the work alive
+}
+
+}  // namespace qmc
