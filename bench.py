@@ -1,0 +1,285 @@
+#!/usr/bin/env python
+"""bench.py -- the driver's benchmark contract for the QMC hot path.
+
+A "step" is one pass of the whole hot path over one batch of synthetic walkers of
+BASELINE.json configs[3] (CO, 14 electrons, 30 STOs, 100 determinants, 131072 walkers
+per GPU): 20 all-electron Metropolis sweeps (qmc_metropolis) + the local energy of the
+resulting walkers (qmc_local_energy) + the batch mean / standard error (qmc_batch_stats).
+
+value   = walker*E_L evaluations per second (M / device time of qmc_local_energy), inputs
+          resident in HBM; the Metropolis walker-steps/s of the same steps is reported
+          beside it ("metropolis").
+e2e     = the same metric through the C ABI with HOST buffers: pinned host walkers -> H2D ->
+          qmc_local_energy -> D2H of log|Psi|, sign, E_L, copies inside the timed region.
+roofline= model FP64 flop-equivalents of the E_L kernel / its mean launch time, against the
+          DFMA peak measured in this same process (qmc_fp64_peak).
+cpu_baseline = the CPU oracle, as it stands, on the host cores, on a bounded sample.
+
+N > 1 (torchrun): walkers are sharded, M per GPU fixed (weak scaling), no data-path
+collective; Philox counters use the global walker index.  --impl reference times the oracle.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+WORKLOAD = "BASELINE configs[3]: CO 14e, 30 STOs, 14 MOs, 100 determinants, 131072 walkers/GPU, " \
+           "20 Metropolis sweeps (step 0.2) + E_L + batch stats"
+METRIC = "walker*E_L evals/sec (CO 14e, FP64); Metropolis walker-steps/sec reported beside it"
+UNIT = "walker*E_L evals/s"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                 "-lms", "50"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for row in self.rows:
+            p = [x.strip() for x in row.split(",")]
+            if len(p) < 7:
+                continue
+            try:
+                sm.append(float(p[0])); mx.append(float(p[1])); pw.append(float(p[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, p[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(d, r, n_sample, threads):
+    """Time the CPU oracle's E_L on the first n_sample walkers; returns walkers/s."""
+    from oracle import binding as ob
+    o = ob.OracleSystem(d)
+    rs = np.ascontiguousarray(r[:, :, :n_sample])
+    ob.local_energy(o, rs[:, :, :64], threads=1)  # load + warm
+    t0 = time.perf_counter()
+    ob.local_energy(o, rs, threads=threads)
+    dt = time.perf_counter() - t0
+    return n_sample / dt, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same config / metric."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2506_09743_b200 import workloads as wl
+    cores = os.cpu_count() or 1
+    n_sample = 4096
+    d, r = wl.co(M=n_sample)
+    times = []
+    for i in range(args.warmup + args.steps):
+        v, dt = oracle_sample(d, r, n_sample, cores)
+        if i >= args.warmup:
+            times.append(dt)
+    ms = 1e3 * float(np.mean(times))
+    val = n_sample / (ms * 1e-3)
+    sample = f"E_L of {n_sample} CO walkers per step (the oracle's explicit per-determinant path), {cores} threads"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": {"workload": WORKLOAD, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--walkers", type=int, default=131072, help="walkers per GPU")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2506_09743_b200 import binding as qb
+    from paper_2506_09743_b200 import workloads as wl
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dev = torch.device("cuda", local_rank)
+
+    M = args.walkers
+    n_sweeps, step_size, seed = 20, 0.2, 20250609
+    d, r_host = wl.co(M=M)
+    if world > 1:  # every rank gets its own walkers; constants are replicated
+        r_host = wl.make_walkers(np.random.default_rng([3, 100 + rank]), d.atom_xyz, d.n_e, M)
+    sysh = qb.QmcSystem(d, device=local_rank)
+    st = torch.cuda.current_stream()
+
+    peak_dfma = qb.fp64_peak(0, reps=5, device=local_rank)
+    peak_dmma = qb.fp64_peak(1, reps=5, device=local_rank)
+
+    r0 = torch.from_numpy(r_host).to(dev)
+    r = r0.clone()
+    lp = torch.empty(M, dtype=torch.float64, device=dev)
+    sg = torch.empty_like(lp)
+    el = torch.empty_like(lp)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)  # > 126 MB L2
+    r_pin = torch.from_numpy(r_host).pin_memory()
+    out_pin = torch.empty((3, M), dtype=torch.float64).pin_memory()
+    r_e2e = torch.empty_like(r0)
+    out_dev = torch.empty((3, M), dtype=torch.float64, device=dev)
+
+    def ev():
+        return torch.cuda.Event(enable_timing=True)
+
+    def one_step(k, timed):
+        """Metropolis (20 sweeps) -> E_L -> batch stats; returns event triple."""
+        flush.fill_(k & 0xFF)
+        a, b, c, e = ev(), ev(), ev(), ev()
+        a.record(st)
+        sysh.metropolis(r, step_size, n_sweeps, seed, sweep_offset=k * n_sweeps, walker_offset=rank * M,
+                        logpsi=lp, sign=sg)
+        b.record(st)
+        sysh.local_energy(r, lp, sg, el)
+        c.record(st)
+        mean, err = qb.batch_stats(el)
+        e.record(st)
+        return (a, b, c, e, mean, err)
+
+    for k in range(args.warmup):
+        one_step(k, False)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    qb.launch_count(reset=True)
+    torch.cuda.synchronize()
+    recs = [one_step(args.warmup + k, True) for k in range(args.steps)]
+    torch.cuda.synchronize()
+    launches = qb.launch_count()
+    if world > 1:
+        dist.barrier()
+    t_met = sum(a.elapsed_time(b) for a, b, c, e, _, _ in recs) * 1e-3
+    t_el = sum(b.elapsed_time(c) for a, b, c, e, _, _ in recs) * 1e-3
+    t_all = sum(a.elapsed_time(e) for a, b, c, e, _, _ in recs) * 1e-3
+
+    # ---- end to end through the C ABI with host buffers
+    def e2e_step():
+        r_e2e.copy_(r_pin, non_blocking=True)
+        sysh.local_energy(r_e2e, out_dev[0], out_dev[1], out_dev[2])
+        out_pin.copy_(out_dev, non_blocking=True)
+    for _ in range(3):
+        e2e_step()
+    torch.cuda.synchronize()
+    a, b = ev(), ev()
+    a.record(st)
+    for _ in range(args.steps):
+        e2e_step()
+    b.record(st)
+    torch.cuda.synchronize()
+    t_e2e = a.elapsed_time(b) * 1e-3
+    clocks = sampler.stop()
+
+    times = torch.tensor([t_met, t_el, t_all, t_e2e], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    t_met, t_el, t_all, t_e2e = (float(x) for x in times.cpu())
+
+    K = args.steps
+    el_rate = world * M * K / t_el
+    met_rate = world * M * n_sweeps * K / t_met
+    e2e_rate = world * M * K / t_e2e
+    flops_el, flops_st = sysh.model_flops(0), sysh.model_flops(1)
+    achieved = flops_el * M * K / t_el / 1e12  # per GPU
+    achieved_met = flops_st * M * n_sweeps * K / t_met / 1e12
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        n_sample = min(M, 8192 * cores)  # ~20-30 core-seconds of CPU work
+        v, dt = oracle_sample(d, r_host, n_sample, cores)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"E_L of the first {n_sample} walkers of the same batch, {cores} threads, {dt:.1f} s"}
+
+    if rank == 0:
+        mean, err = recs[-1][4], recs[-1][5]
+        line = {
+            "metric": METRIC, "value": el_rate, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+            "ms_per_step": 1e3 * t_all / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "walkers_per_gpu": M, "n_sweeps": n_sweeps, "step_bohr": step_size,
+                       "l2": "flushed between steps (256 MB write, outside the event-timed regions)",
+                       "timing": "CUDA events on torch's current stream around each call; sums over the K steps; max over ranks"},
+            "metropolis": {"value": met_rate, "unit": "walker-steps/s", "ms_per_call": 1e3 * t_met / K,
+                           "model_tflops": achieved_met, "frac_of_dfma_peak": achieved_met / peak_dfma},
+            "local_energy_ms": 1e3 * t_el / K,
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_dfma, "unit": "TFLOP/s",
+                         "frac": achieved / peak_dfma, "traffic": None,
+                         "kernel": "local_energy_kernel<7,14,true>",
+                         "peak_source": "qmc_fp64_peak DFMA microbenchmark in this process (no FP64 entry in MEASURED_PEAKS.json)",
+                         "dmma_peak": peak_dmma, "model_flop_eq_per_walker": flops_el},
+            "cpu_baseline": cpu,
+            "e2e": {"value": e2e_rate, "unit": UNIT, "h2d_bytes_per_step": int(r_pin.numel() * 8),
+                    "d2h_bytes_per_step": int(out_pin.numel() * 8)},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+            "last_step": {"mean_E_L": mean, "stderr": err},
+        }
+        print(json.dumps(line))
+    sysh.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
