@@ -33,7 +33,7 @@ int cuda_fail(cudaError_t e, const char *what) {
 
 struct Variant {
   int NS, NMO, LP, ws_doubles;
-  const void *k_el, *k_psi, *k_metro;
+  const void *k_el, *k_psi, *k_metro, *k_metro_el;
 };
 
 template <int NS, int NMO>
@@ -45,7 +45,8 @@ Variant make_variant() {
   v.ws_doubles = Geo<NS, NMO>::total;
   v.k_el = (const void *)local_energy_kernel<NS, NMO, true>;
   v.k_psi = (const void *)local_energy_kernel<NS, NMO, false>;
-  v.k_metro = (const void *)metropolis_kernel<NS, NMO>;
+  v.k_metro = (const void *)metropolis_kernel<NS, NMO, false>;
+  v.k_metro_el = (const void *)metropolis_kernel<NS, NMO, true>;
   return v;
 }
 
@@ -79,7 +80,7 @@ struct qmc_system {
   SysParams P{};
   Variant var{};
   int smem_bytes = 0;
-  int blocks_el = 0, blocks_psi = 0, blocks_metro = 0;
+  int blocks_el = 0, blocks_psi = 0, blocks_metro = 0, blocks_metro_el = 0;
   void *d_shells = nullptr, *d_C = nullptr, *d_dets = nullptr;
   double *d_stats = nullptr;
   unsigned long long *d_counter = nullptr;
@@ -176,16 +177,16 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     return (int)used.size() - 1;
   };
   std::vector<int> virt[2];  // caller MO index of virtual q
-  std::vector<DetRec> dets(d->n_det);
+  struct Exc { int k[2]; int p[2][2]; int q[2][2]; double d; };
+  std::vector<Exc> excs(d->n_det);
   bool unsupported = false;
   for (int sp = 0; sp < 2; ++sp)
     for (int j = 0; j < nsp[sp]; ++j) P.ref_col[sp][j] = (int8_t)col_of(lists[sp][j]);
   for (int n = 0; n < d->n_det; ++n) {
-    dets[n].d = d->ci_coeff[n];
-    uint32_t code[2] = {0, 0};
+    Exc &x = excs[n];
+    x.d = d->ci_coeff[n];
     for (int sp = 0; sp < 2; ++sp) {
       int k = 0;
-      uint32_t c = 0;
       for (int j = 0; j < nsp[sp]; ++j) {
         const int mo = lists[sp][(size_t)n * nsp[sp] + j];
         if (mo == lists[sp][j]) continue;
@@ -196,15 +197,20 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
           virt[sp].push_back(mo);
           q = (int)virt[sp].size() - 1;
         }
-        if (k < 2 && q < 16) c |= ((uint32_t)j << (4 + 8 * k)) | ((uint32_t)q << (8 + 8 * k));
+        if (k < 2) { x.p[sp][k] = j; x.q[sp][k] = q; }
         ++k;
       }
       if (k > 2) unsupported = true;
-      code[sp] = c | (uint32_t)std::min(k, 15);
+      x.k[sp] = k;
     }
-    dets[n].up = code[0];
-    dets[n].dn = code[1];
   }
+  // determinants with at most one substitution per spin first: the lanes of a warp, which take
+  // consecutive determinants, then run the same code
+  std::stable_sort(excs.begin(), excs.end(), [](const Exc &a, const Exc &b) {
+    return std::max(a.k[0], a.k[1]) / 2 < std::max(b.k[0], b.k[1]) / 2;
+  });
+  P.n_det_single = 0;
+  for (const Exc &x : excs) P.n_det_single += (std::max(x.k[0], x.k[1]) < 2) ? 1 : 0;
   for (int sp = 0; sp < 2; ++sp) {
     if ((int)virt[sp].size() > kMaxVirt) unsupported = true;
     P.nv[sp] = (int)virt[sp].size();
@@ -231,6 +237,27 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   }
   s->var = *var;
   const int NMO = var->NMO;
+  std::vector<DetRec> dets(d->n_det);
+  {
+    const uint32_t one = (uint32_t)(var->NS * var->LP), zero = one + 1;  // constant table entries (Geo::TS)
+    for (int n = 0; n < d->n_det; ++n) {
+      const Exc &x = excs[n];
+      uint32_t code[2];
+      for (int sp = 0; sp < 2; ++sp) {
+        uint32_t i11 = one, i12 = zero, i21 = zero, i22 = one;
+        if (x.k[sp] >= 1) i11 = (uint32_t)(x.p[sp][0] * var->LP + x.q[sp][0]);
+        if (x.k[sp] == 2) {
+          i12 = (uint32_t)(x.p[sp][0] * var->LP + x.q[sp][1]);
+          i21 = (uint32_t)(x.p[sp][1] * var->LP + x.q[sp][0]);
+          i22 = (uint32_t)(x.p[sp][1] * var->LP + x.q[sp][1]);
+        }
+        code[sp] = i11 | (i12 << 8) | (i21 << 16) | (i22 << 24);
+      }
+      dets[n].up = code[0];
+      dets[n].dn = code[1];
+      dets[n].d = x.d;
+    }
+  }
   P.G = std::max(1, std::min(32 / P.n_e, 16 / var->NS));
 
   // ---- shell grouping: AOs that share a centre, n, l and zeta share one radial factor
@@ -321,9 +348,9 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     qmc_destroy(s);
     return QMC_EUNSUPPORTED;
   }
-  const void *ks[3] = {var->k_el, var->k_psi, var->k_metro};
-  int *nb[3] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro};
-  for (int i = 0; i < 3; ++i) {
+  const void *ks[4] = {var->k_el, var->k_psi, var->k_metro, var->k_metro_el};
+  int *nb[4] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro, &s->blocks_metro_el};
+  for (int i = 0; i < 4; ++i) {
     if ((e = cudaFuncSetAttribute(ks[i], cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_bytes)) != cudaSuccess) {
       int rc = cuda_fail(e, "cudaFuncSetAttribute");
       qmc_destroy(s);
@@ -386,9 +413,9 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
   if (h_n_accepted) CK(cudaMemsetAsync(s->d_counter, 0, sizeof(unsigned long long), st));
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
   const int64_t need = (groups + kWarpsPerBlock - 1) / kWarpsPerBlock;
-  const int grid = (int)std::min<int64_t>(need, s->blocks_metro);
+  const int grid = (int)std::min<int64_t>(need, d_eloc_acc ? s->blocks_metro_el : s->blocks_metro);
   void *args[3] = {(void *)&s->P, (void *)&io, (void *)&mp};
-  CK(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPerBlock * 32), args, s->smem_bytes, st));
+  CK(cudaLaunchKernel(d_eloc_acc ? s->var.k_metro_el : s->var.k_metro, dim3(grid), dim3(kWarpsPerBlock * 32), args, s->smem_bytes, st));
   ++g_launches;
   if (h_n_accepted) {
     unsigned long long v = 0;

@@ -15,7 +15,7 @@ namespace qmc {
 constexpr int kMaxAtoms = 16;
 constexpr int kMaxSpin = 8;   // electrons per spin
 constexpr int kMaxVirt = 8;   // distinct virtual orbitals per spin
-constexpr int kWarpsPerBlock = 4;
+constexpr int kWarpsPerBlock = 8;
 
 // shell record kinds
 enum : int { SH_S = 0, SH_P = 1, SH_D = 2, SH_P1 = 3, SH_D1 = 4 };
@@ -31,14 +31,18 @@ struct ShellRec {  // 32 bytes
   int32_t pad;
 };
 
-struct DetRec {  // 16 bytes.  exc: bits 0-3 k, 4-7 p1, 8-11 q1, 12-15 p2, 16-19 q2
-  uint32_t up, dn;
+// One determinant relative to the reference, per spin four table indices (p*LP+q) of the 2x2
+// sub-block {11, 12, 21, 22}; unused slots point at the constant entries TS-2 (= 1.0 in T, 0 in M)
+// and TS-1 (= 0.0), so k = 0, 1, 2 substitutions share one formula.  16 bytes.
+struct DetRec {
+  uint32_t up, dn;  // 4 x uint8 each
   double d;
 };
 
 struct SysParams {  // passed by value to every kernel
   int n_atoms, n_up, n_dn, n_e;
   int n_shell, n_ao, n_mo, n_det;  // n_mo = orbitals referenced (kernel order)
+  int n_det_single;                // determinants [0, n_det_single) have at most one substitution per spin
   int nv[2];                       // virtual orbitals per spin
   int G;                           // walkers per warp pass
   int smem_const_bytes;
@@ -88,18 +92,22 @@ struct Geo {
   static constexpr int NV = (NMO - NS) > 0 ? ((NMO - NS) < kMaxVirt ? (NMO - NS) : kMaxVirt) : 0;
   static constexpr int LP = pow2ceil(cmax(cmax(NS, NV), 1));  // lanes per Gauss-Jordan problem
   static constexpr int PP = 32 / LP;                          // problems per pass
-  // per-warp scratch, in doubles
+  static constexpr int GMAX = 16 / NS;                        // walkers per warp pass (host: G <= GMAX)
+  static constexpr int ROWS = (2 * GMAX * NS) < 32 ? (2 * GMAX * NS) : 32;  // electron rows of a pass
+  static constexpr int TS = NS * LP + 2;  // table stride per problem: T[p][q] entries + {1.0, 0.0}
+  static constexpr int even(int x) { return (x + 1) & ~1; }
+  // per-warp scratch, in doubles (all offsets even: 16-byte aligned)
   static constexpr int oPhi = 0;
-  static constexpr int oB = oPhi + 32 * NMO;
-  static constexpr int oXYZ = oB + 32 * NMO;
-  static constexpr int oPart = oXYZ + 96;
-  static constexpr int oG = oPart + 64;
-  static constexpr int oT = oG + PP * NS * NS;
-  static constexpr int oM = oT + 32 * LP;   // 2G*NS <= 32 rows of LP entries
-  static constexpr int oProb = oM + 32 * LP;
-  static constexpr int oProp = oProb + 32 * 4;  // Metropolis: proposals z [G][3 n_e] + log u [G]
-  static constexpr int oRes = oProp + 96 + 32;   // per walker {log|Psi|, sign, E_L}
-  static constexpr int total = oRes + 96;
+  static constexpr int oB = oPhi + even(ROWS * NMO);
+  static constexpr int oPart = oB + even(ROWS * NMO);
+  static constexpr int oXYZ = oPart + 64;                     // coordinates (pair loop) ...
+  static constexpr int oG = oXYZ;                             // ... later reused by the Gm staging
+  static constexpr int oT = oG + even(cmax(PP * NS * NS, 96));
+  static constexpr int oProp = oT;                            // Metropolis draws are consumed before T is written
+  static constexpr int oM = oT + even(cmax(2 * GMAX * TS, 96 + 32));
+  static constexpr int oProb = oM + even(2 * GMAX * TS);
+  static constexpr int oRes = oProb + 2 * GMAX * 4;           // per walker {log|Psi|, sign, E_L, -}
+  static constexpr int total = oRes + GMAX * 4;
 };
 
 // ---------------------------------------------------------------------------------
@@ -121,6 +129,51 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 __device__ __forceinline__ double u53(uint32_t hi, uint32_t lo) {
   unsigned long long v = (((unsigned long long)hi << 32) | lo) >> 11;
   return ((double)v + 0.5) * (1.0 / 9007199254740992.0);
+}
+
+// Fast FP64 reciprocal / reciprocal square root: MUFU seed (about 20 bits) + two Newton steps
+// (relative error ~1e-16; inputs here are distances and pivots, never subnormal).
+__device__ __forceinline__ double rcp_fast(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-x, y, 1.0);
+  return fma(y, e, y);
+}
+__device__ __forceinline__ double rsqrt_fast(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double h = 0.5 * x;
+  double e = fma(-h * y, y, 0.5);
+  y = fma(y, e, y);
+  e = fma(-h * y, y, 0.5);
+  return fma(y, e, y);
+}
+
+// exp(x) for x <= 0 (STO radial factors e^{-zeta r}): x = n ln2 + f, |f| <= ln2/2, degree-13 Taylor
+// polynomial in Estrin form (truncation 4e-18 relative), 2^n applied to the exponent field.
+// Arguments below -700 are clamped (value ~1e-304, i.e. zero for every use here).
+__device__ __forceinline__ double exp_neg(double x) {
+  x = fmax(x, -700.0);
+  const double magic = 6755399441055744.0;  // 1.5 * 2^52
+  const double t = fma(x, 1.4426950408889634, magic);
+  const int n = __double2loint(t);
+  const double nd = t - magic;
+  double f = fma(nd, -6.93147180369123816490e-01, x);
+  f = fma(nd, -1.90821492927058770002e-10, f);
+  const double f2 = f * f, f4 = f2 * f2, f8 = f4 * f4;
+  const double p01 = 1.0 + f;
+  const double p23 = fma(f, 1.0 / 6.0, 0.5);
+  const double p45 = fma(f, 1.0 / 120.0, 1.0 / 24.0);
+  const double p67 = fma(f, 1.0 / 5040.0, 1.0 / 720.0);
+  const double p89 = fma(f, 1.0 / 362880.0, 1.0 / 40320.0);
+  const double pab = fma(f, 1.0 / 39916800.0, 1.0 / 3628800.0);
+  const double pcd = fma(f, 1.0 / 6227020800.0, 1.0 / 479001600.0);
+  const double q0 = fma(p23, f2, p01), q1 = fma(p67, f2, p45), q2 = fma(pab, f2, p89);
+  const double r0 = fma(q1, f4, q0), r1 = fma(pcd, f4, q2);
+  const double p = fma(r1, f8, r0);
+  return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
 }
 
 __device__ __forceinline__ double shfl_d(double v, int src, int width) {

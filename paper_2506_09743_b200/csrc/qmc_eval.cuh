@@ -26,34 +26,34 @@ __device__ __forceinline__ void contract(const double *__restrict__ crow, double
   }
 }
 
-// excitation factor of one spin of one determinant relative to the reference:
-//   R  = det T[p,q]                     = D_X / D_0           (reading Q8; H.1)
-//   Rd = Tr(adj(T[p,q]) Mtab[p,q])      = R * Tr((P A0^-1 A_X P)^-1 P M P)   (F.6)
-template <int LP, bool EL>
-__device__ __forceinline__ void excite(uint32_t e, const double *__restrict__ T, const double *__restrict__ Mt,
-                                       double &R, double &Rd) {
-  int k = e & 15;
-  R = 1.0;
+// Excitation factors of one spin of one determinant relative to the reference, from the tables
+//   T = A0^-1 Av,  Mt = A0^-1 Bv - A0^-1 B0 T                      (F.6/F.7)
+//   R  = det T[p,q] = D_X / D_0                                     (reading Q8; H.1)
+//   Rd = Tr(adj(T[p,q]) Mt[p,q]) = R * Tr((P A0^-1 A_X P)^-1 P M P) (F.6)
+// idx packs four uint8 table indices {11, 12, 21, 22}.
+template <bool EL>
+__device__ __forceinline__ void excite_single(uint32_t idx, const double *__restrict__ T,
+                                              const double *__restrict__ Mt, double &R, double &Rd) {
+  const int i = idx & 255;
+  R = T[i];
+  Rd = EL ? Mt[i] : 0.0;
+}
+template <bool EL>
+__device__ __forceinline__ void excite_double(uint32_t idx, const double *__restrict__ T,
+                                              const double *__restrict__ Mt, double &R, double &Rd) {
+  const int i11 = idx & 255, i12 = (idx >> 8) & 255, i21 = (idx >> 16) & 255, i22 = idx >> 24;
+  const double t11 = T[i11], t12 = T[i12], t21 = T[i21], t22 = T[i22];
+  R = fma(t11, t22, -t12 * t21);
   Rd = 0.0;
-  if (k == 0) return;
-  int p1 = (e >> 4) & 15, q1 = (e >> 8) & 15;
-  if (k == 1) {
-    R = T[p1 * LP + q1];
-    if (EL) Rd = Mt[p1 * LP + q1];
-    return;
-  }
-  int p2 = (e >> 12) & 15, q2 = (e >> 16) & 15;
-  double t11 = T[p1 * LP + q1], t12 = T[p1 * LP + q2], t21 = T[p2 * LP + q1], t22 = T[p2 * LP + q2];
-  R = t11 * t22 - t12 * t21;
   if (EL) {
-    double m11 = Mt[p1 * LP + q1], m12 = Mt[p1 * LP + q2], m21 = Mt[p2 * LP + q1], m22 = Mt[p2 * LP + q2];
-    Rd = t22 * m11 - t12 * m21 - t21 * m12 + t11 * m22;
+    const double m11 = Mt[i11], m12 = Mt[i12], m21 = Mt[i21], m22 = Mt[i22];
+    Rd = fma(t22, m11, fma(t11, m22, -fma(t12, m21, t21 * m12)));
   }
 }
 
 // ---------------------------------------------------------------------------------
 // Evaluate the G walkers of this warp.  Lane = g * n_e + e holds electron e of walker g
-// at (x, y, z).  Results for walker g are left in ws[oRes + 3 g + {0,1,2}] =
+// at (x, y, z).  Results for walker g are left in ws[oRes + 4 g + {0,1,2}] =
 // {log|Psi|, sign, E_L} (E_L only if EL).  All 32 lanes must call.
 // ---------------------------------------------------------------------------------
 template <int NS, int NMO, bool EL>
@@ -61,7 +61,7 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
                              const double *__restrict__ sC, const DetRec *__restrict__ sDet,
                              double *__restrict__ ws, double x, double y, double z, int lane) {
   using GE = Geo<NS, NMO>;
-  constexpr int LP = GE::LP, PP = GE::PP;
+  constexpr int LP = GE::LP, PP = GE::PP, TS = GE::TS;
   const int ne = P.n_e, G = P.G;
   const int g = lane / ne, e = lane - g * ne;
   const bool active = lane < G * ne;
@@ -86,10 +86,10 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
       double dz = z - sXYZ[(base + j) * 3 + 2];
       if (j == e) continue;
       double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-      double r = sqrt(r2);
-      double ri = 1.0 / r;
+      double ri = rsqrt_fast(r2);
+      double r = r2 * ri;
       double a = ((j < P.n_up) == up) ? P.a_par : P.a_anti;
-      double di = 1.0 / fma(P.b, r, 1.0);
+      double di = rcp_fast(fma(P.b, r, 1.0));
       double adi = a * di;
       J2 = fma(adi, r, J2);  // u = a r / (1 + b r)
       if (EL) {
@@ -118,13 +118,13 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
   for (int at = 0; at < P.n_atoms; ++at) {
     const double dx = x - P.atom[at][0], dy = y - P.atom[at][1], dz = z - P.atom[at][2];
     const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-    const double r = sqrt(r2);
-    const double ri = 1.0 / r;
+    const double ri = rsqrt_fast(r2);
+    const double r = r2 * ri;
     if (EL) ven = fma(-P.atom[at][3], ri, ven);
     const double gd = EL ? fma(gJx, dx, fma(gJy, dy, gJz * dz)) * ri : 0.0;  // grad J . d / r
     for (int s = P.shell_begin[at]; s < P.shell_begin[at + 1]; ++s) {
       const ShellRec sh = sShell[s];
-      const double ex = exp(-sh.zeta * r);
+      const double ex = exp_neg(-sh.zeta * r);
       const int k = sh.k;
       const double gr = (k == 0) ? ex : ((k == 1) ? ex * r : ((k == 2) ? ex * r2 : ex * r2 * r));
       double h = 0.0;
@@ -178,7 +178,7 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
     }
   }
   // hand the MO rows over
-  {
+  if (active) {
     double2 *dst = reinterpret_cast<double2 *>(sPhi + lane * NMO);
 #pragma unroll
     for (int a = 0; a < NMO / 2; ++a) dst[a] = make_double2(accP[2 * a], accP[2 * a + 1]);
@@ -187,6 +187,8 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
 #pragma unroll
       for (int a = 0; a < NMO / 2; ++a) dstb[a] = make_double2(accB[2 * a], accB[2 * a + 1]);
     }
+  }
+  {
     // per-electron scalars: J/2-sum and the electron's share of the energy
     sPart[lane * 2 + 0] = 0.5 * J2;
     sPart[lane * 2 + 1] =
@@ -222,35 +224,28 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
           }
         }
       }
+      // Pivoting is by COLUMN: at step k the not-yet-used A0 column with the largest |entry| in row k
+      // becomes the pivot; columns live in lanes, so nothing moves.  Row k of the reduced right-hand
+      // sides then belongs to reference position perm[k] (the pivot lane).
       double det = 1.0;
+      int perm[NS];
+      int myrow = 0;
+      bool used = !(c < NS);
 #pragma unroll
       for (int k = 0; k < NS; ++k) {
-        int p = k;
-        double best = fabs(a0[k]);
+        // 32-bit monotone key of |a0[k]| with the lane index in the low bits: unique arg-max
+        unsigned key = used ? 0u : (((unsigned)(__double2hiint(a0[k]) & 0x7fffffff) & ~(unsigned)(LP - 1)) | (unsigned)c);
 #pragma unroll
-        for (int i = k + 1; i < NS; ++i) {
-          double v = fabs(a0[i]);
-          if (v > best) { best = v; p = i; }
-        }
-        p = __shfl_sync(0xffffffffu, p, gbase + k);
-#pragma unroll
-        for (int i = k + 1; i < NS; ++i) {
-          if (p == i) {
-            double t;
-            t = a0[k]; a0[k] = a0[i]; a0[i] = t;
-            t = av[k]; av[k] = av[i]; av[i] = t;
-            if (EL) {
-              t = b0[k]; b0[k] = b0[i]; b0[i] = t;
-              t = bv[k]; bv[k] = bv[i]; bv[i] = t;
-            }
-          }
-        }
+        for (int m = 1; m < LP; m <<= 1) key = max(key, __shfl_xor_sync(0xffffffffu, key, m));
+        const int pl = (int)(key & (unsigned)(LP - 1));
+        perm[k] = pl;
+        if (c == pl) { used = true; myrow = k; }
         double f[NS];
 #pragma unroll
-        for (int i = 0; i < NS; ++i) f[i] = __shfl_sync(0xffffffffu, a0[i], gbase + k);
+        for (int i = 0; i < NS; ++i) f[i] = __shfl_sync(0xffffffffu, a0[i], gbase + pl);
         const double piv = f[k];
-        const double inv = 1.0 / piv;
-        det *= (p != k) ? -piv : piv;
+        const double inv = rcp_fast(piv);
+        det *= piv;
         {
           double t = a0[k] * inv;
           a0[k] = t;
@@ -272,35 +267,51 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
           }
         }
       }
+      {  // sign of the permutation k -> perm[k]
+        int inversions = 0;
+#pragma unroll
+        for (int k = 0; k < NS; ++k)
+#pragma unroll
+          for (int k2 = k + 1; k2 < NS; ++k2) inversions += (perm[k] > perm[k2]) ? 1 : 0;
+        if (inversions & 1) det = -det;
+      }
       // t0 = Tr(A0^-1 B0)   (G.7, applied to the combined operator)
       double t0 = 0.0;
       if (EL) {
 #pragma unroll
-        for (int i = 0; i < NS; ++i) if (i == c) t0 = b0[i];
+        for (int i = 0; i < NS; ++i) if (i == myrow && c < NS) t0 = b0[i];
 #pragma unroll
         for (int m = 1; m < LP; m <<= 1) t0 += shfl_xor_d(t0, m);
-        // Mtab = A0^-1 Bv - (A0^-1 B0) T   (F.7), column c in this lane
+        // Mtab = A0^-1 Bv - (A0^-1 B0) T   (F.7), column c in this lane;
+        // rows stay in elimination order (row k <-> position perm[k]) on both sides.
         double *gs = sG + slot * NS * NS;
         if (c < NS) {
 #pragma unroll
-          for (int i = 0; i < NS; ++i) gs[c * NS + i] = b0[i];  // gs[j][i] = Gm[i][j]
+          for (int i = 0; i < NS; ++i) gs[c * NS + i] = b0[i];  // gs[j][k] = Gm[perm[k]][j]
         }
         __syncwarp();
 #pragma unroll
-        for (int j = 0; j < NS; ++j) {
-          const double tj = av[j];
+        for (int k = 0; k < NS; ++k) {
+          const double tj = av[k];  // T[perm[k]][c]
+          const double *gcol = gs + perm[k] * NS;
 #pragma unroll
-          for (int i = 0; i < NS; ++i) bv[i] = fma(-gs[j * NS + i], tj, bv[i]);
+          for (int i = 0; i < NS; ++i) bv[i] = fma(-gcol[i], tj, bv[i]);
         }
         __syncwarp();
       }
       if (pvalid) {
 #pragma unroll
-        for (int i = 0; i < NS; ++i) {
-          sT[(pr * NS + i) * LP + c] = av[i];
-          if (EL) sM[(pr * NS + i) * LP + c] = bv[i];
+        for (int k = 0; k < NS; ++k) {
+          sT[pr * TS + perm[k] * LP + c] = av[k];
+          if (EL) sM[pr * TS + perm[k] * LP + c] = bv[k];
         }
         if (c == 0) {
+          sT[pr * TS + NS * LP] = 1.0;
+          sT[pr * TS + NS * LP + 1] = 0.0;
+          if (EL) {
+            sM[pr * TS + NS * LP] = 0.0;
+            sM[pr * TS + NS * LP + 1] = 0.0;
+          }
           sProb[pr * 4 + 0] = log(fabs(det));
           sProb[pr * 4 + 1] = (det > 0.0) ? 1.0 : ((det < 0.0) ? -1.0 : 0.0);
           sProb[pr * 4 + 2] = t0;
@@ -317,14 +328,25 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
     const int wg = lane / LW, sub = lane - wg * LW;
     const bool wvalid = wg < G;
     const int pu = 2 * (wvalid ? wg : 0), pd = pu + 1;
-    const double *Tu = sT + pu * NS * LP, *Td = sT + pd * NS * LP;
-    const double *Mu = sM + pu * NS * LP, *Md = sM + pd * NS * LP;
+    const double *Tu = sT + pu * TS, *Td = sT + pd * TS;
+    const double *Mu = sM + pu * TS, *Md = sM + pd * TS;
     double den = 0.0, num = 0.0;
-    for (int n = sub; n < P.n_det; n += LW) {
+    // determinants with at most one substitution per spin: one table entry per spin
+    for (int n = sub; n < P.n_det_single; n += LW) {
       const DetRec dr = sDet[n];
       double Ru, Du, Rd, Dd;
-      excite<LP, EL>(dr.up, Tu, Mu, Ru, Du);
-      excite<LP, EL>(dr.dn, Td, Md, Rd, Dd);
+      excite_single<EL>(dr.up, Tu, Mu, Ru, Du);
+      excite_single<EL>(dr.dn, Td, Md, Rd, Dd);
+      const double w = dr.d * Ru;
+      den = fma(w, Rd, den);
+      if (EL) num = fma(dr.d, Du * Rd, fma(w, Dd, num));
+    }
+    // the rest: 2x2 sub-determinants
+    for (int n = P.n_det_single + sub; n < P.n_det; n += LW) {
+      const DetRec dr = sDet[n];
+      double Ru, Du, Rd, Dd;
+      excite_double<EL>(dr.up, Tu, Mu, Ru, Du);
+      excite_double<EL>(dr.dn, Td, Md, Rd, Dd);
       const double w = dr.d * Ru;
       den = fma(w, Rd, den);
       if (EL) num = fma(dr.d, Du * Rd, fma(w, Dd, num));
@@ -341,9 +363,9 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
       }
       const double lu = sProb[pu * 4 + 0], ld = sProb[pd * 4 + 0];
       const double sgn = sProb[pu * 4 + 1] * sProb[pd * 4 + 1];
-      sRes[wg * 3 + 0] = Jsum + lu + ld + log(fabs(den));
-      sRes[wg * 3 + 1] = sgn * ((den > 0.0) ? 1.0 : ((den < 0.0) ? -1.0 : 0.0));
-      if (EL) sRes[wg * 3 + 2] = esum + (sProb[pu * 4 + 2] + sProb[pd * 4 + 2]) + num / den + P.vnn;
+      sRes[wg * 4 + 0] = Jsum + lu + ld + log(fabs(den));
+      sRes[wg * 4 + 1] = sgn * ((den > 0.0) ? 1.0 : ((den < 0.0) ? -1.0 : 0.0));
+      if (EL) sRes[wg * 4 + 2] = esum + (sProb[pu * 4 + 2] + sProb[pd * 4 + 2]) + num / den + P.vnn;
     }
   }
   __syncwarp();

@@ -39,7 +39,7 @@ __device__ __forceinline__ void dummy_xyz(int lane, double &x, double &y, double
 }
 
 template <int NS, int NMO, bool EL>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 2)
     local_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
   const double *sC;
@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32)
     if (lane < G) {
       const int64_t wo = grp * G + lane;
       if (wo < io.M) {
-        const double *res = ws + GE::oRes + lane * 3;
+        const double *res = ws + GE::oRes + lane * 4;
         if (io.logpsi) io.logpsi[wo] = res[0];
         if (io.sign) io.sign[wo] = res[1];
         if (EL && io.eloc) io.eloc[wo] = res[2];
@@ -83,8 +83,8 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32)
 // Persistent all-electron Metropolis (readings Q9, Q10).
 // Walker coordinates and log|Psi| stay in registers for all sweeps.
 // ---------------------------------------------------------------------------------
-template <int NS, int NMO>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32)
+template <int NS, int NMO, bool WITH_EL>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, 2)
     metropolis_kernel(const __grid_constant__ SysParams P, const WalkerIO io, const MetroParams mp) {
   extern __shared__ __align__(16) unsigned char smem[];
   const double *sC;
@@ -106,6 +106,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32)
   for (int64_t grp = (int64_t)blockIdx.x * kWarpsPerBlock + warp; grp < n_groups; grp += stride) {
     const int64_t w = grp * G + g;
     const bool own = (g < G) && (w < io.M);
+    const int rg = (own ? g : 0) * 4;
     double x, y, z;
     if (own) {
       x = io.r_out[((int64_t)e * 3 + 0) * io.M + w];
@@ -114,51 +115,52 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32)
     } else {
       dummy_xyz(lane, x, y, z);
     }
-    eval_walkers<NS, NMO, false>(P, sShell, sC, sDet, ws, x, y, z, lane);
-    double lp = sRes[(own ? g : 0) * 3 + 0], sg = sRes[(own ? g : 0) * 3 + 1];
-    double eacc = 0.0;
-    __syncwarp();
-    for (int sw = 0; sw < mp.n_sweeps; ++sw) {
-      // --- draws: lanes share the (walker, pair) blocks of the G walkers
-      for (int idx = lane; idx < G * (npair + 1); idx += 32) {
-        const int dg = idx / (npair + 1), j = idx - dg * (npair + 1);
-        const uint64_t gw = (uint64_t)(mp.walker_offset + grp * G + dg);
-        uint32_t o[4];
-        philox4x32_10((uint32_t)gw, mp.sweep0 + (uint32_t)sw, (j == npair) ? 0xFFFFFFFFu : (uint32_t)j,
-                      (uint32_t)(gw >> 32), mp.key0, mp.key1, o);
-        const double u1 = u53(o[0], o[1]);
-        if (j == npair) {
-          sLogU[dg] = log(u1);
-        } else {
-          const double u2 = u53(o[2], o[3]);
-          const double rho = sqrt(-2.0 * log(u1));
-          double sn, cs;
-          sincos(6.283185307179586 * u2, &sn, &cs);
-          sProp[dg * nc + 2 * j] = rho * cs;
-          if (2 * j + 1 < nc) sProp[dg * nc + 2 * j + 1] = rho * sn;
+    double lp = 0.0, sg = 0.0, eacc = 0.0;
+    // sweep -1 evaluates the starting point (always "accepted", no draws)
+    for (int sw = -1; sw < mp.n_sweeps; ++sw) {
+      double xp = x, yp = y, zp = z, logu = 0.0;
+      if (sw >= 0) {
+        // --- draws: lanes share the (walker, pair) Philox blocks of the G walkers
+        for (int idx = lane; idx < G * (npair + 1); idx += 32) {
+          const int dg = idx / (npair + 1), j = idx - dg * (npair + 1);
+          const uint64_t gw = (uint64_t)(mp.walker_offset + grp * G + dg);
+          uint32_t o[4];
+          philox4x32_10((uint32_t)gw, mp.sweep0 + (uint32_t)sw, (j == npair) ? 0xFFFFFFFFu : (uint32_t)j,
+                        (uint32_t)(gw >> 32), mp.key0, mp.key1, o);
+          const double u1 = u53(o[0], o[1]);
+          if (j == npair) {
+            sLogU[dg] = log(u1);
+          } else {
+            const double u2 = u53(o[2], o[3]);
+            const double rho = sqrt(-2.0 * log(u1));
+            double sn, cs;
+            sincos(6.283185307179586 * u2, &sn, &cs);
+            sProp[dg * nc + 2 * j] = rho * cs;
+            if (2 * j + 1 < nc) sProp[dg * nc + 2 * j + 1] = rho * sn;
+          }
         }
+        __syncwarp();
+        if (own) {
+          xp = fma(mp.step, sProp[g * nc + 3 * e + 0], x);
+          yp = fma(mp.step, sProp[g * nc + 3 * e + 1], y);
+          zp = fma(mp.step, sProp[g * nc + 3 * e + 2], z);
+        }
+        logu = sLogU[own ? g : 0];
+        __syncwarp();
       }
-      __syncwarp();
-      double xp = x, yp = y, zp = z;
-      if (own) {
-        xp = fma(mp.step, sProp[g * nc + 3 * e + 0], x);
-        yp = fma(mp.step, sProp[g * nc + 3 * e + 1], y);
-        zp = fma(mp.step, sProp[g * nc + 3 * e + 2], z);
-      }
-      const double logu = sLogU[own ? g : 0];
-      __syncwarp();
       eval_walkers<NS, NMO, false>(P, sShell, sC, sDet, ws, xp, yp, zp, lane);
-      const double lp2 = sRes[(own ? g : 0) * 3 + 0], sg2 = sRes[(own ? g : 0) * 3 + 1];
-      const bool ok = own && (logu < 2.0 * (lp2 - lp));  // false for NaN and for Psi' = 0
+      const double lp2 = sRes[rg + 0], sg2 = sRes[rg + 1];
+      // accept iff log u < 2 (log|Psi'| - log|Psi|): false for NaN and for Psi' = 0
+      const bool ok = (sw < 0) || (own && (logu < 2.0 * (lp2 - lp)));
       if (ok) { x = xp; y = yp; z = zp; lp = lp2; sg = sg2; }
-      if (own && e == 0) {
+      if (sw >= 0 && own && e == 0) {
         if (mp.accept) mp.accept[(int64_t)sw * io.M + w] = ok ? 1 : 0;
         acc_count += ok ? 1 : 0;
       }
       __syncwarp();
-      if (mp.eloc_acc) {
+      if (WITH_EL && sw >= 0) {
         eval_walkers<NS, NMO, true>(P, sShell, sC, sDet, ws, x, y, z, lane);
-        eacc += sRes[(own ? g : 0) * 3 + 2];
+        eacc += sRes[rg + 2];
         __syncwarp();
       }
     }
@@ -169,7 +171,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32)
       if (e == 0) {
         if (io.logpsi) io.logpsi[w] = lp;
         if (io.sign) io.sign[w] = sg;
-        if (mp.eloc_acc) mp.eloc_acc[w] = eacc;
+        if (WITH_EL) mp.eloc_acc[w] = eacc;
       }
     }
     __syncwarp();
