@@ -278,30 +278,55 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     rc.r.c2 = (float)(k * (k + 2 * l + 1));
     rc.r.k = (int16_t)k;
     rc.r.m = (int16_t)d->ao_m[b];
-    rc.r.pad = 0;
+    rc.r.atom = (int16_t)at; rc.r.flush = 0;
     if (l == 0) { rc.r.kind = SH_S; rc.aos = {b}; b += 1; }
     else if (full) { rc.r.kind = (l == 1) ? SH_P : SH_D; for (int t = 0; t < nfun; ++t) rc.aos.push_back(b + t); b += nfun; }
     else { rc.r.kind = (l == 1) ? SH_P1 : SH_D1; rc.aos = {b}; b += 1; }
     recs.push_back(rc);
   }
   std::stable_sort(recs.begin(), recs.end(), [](const Rec &a, const Rec &b) { return a.atom < b.atom; });
+  // AO rows are laid out in chunks of 16 (one DMMA pass each); a record never straddles a chunk
   std::vector<ShellRec> shells;
-  std::vector<double> C((size_t)d->n_ao * NMO, 0.0);
-  int row = 0, at_cur = 0;
-  P.shell_begin[0] = 0;
-  for (size_t i = 0; i < recs.size(); ++i) {
-    while (at_cur < recs[i].atom) P.shell_begin[++at_cur] = (int)i;
-    recs[i].r.ao0 = (int16_t)row;
-    for (int b : recs[i].aos) {
-      const double nrm = d->ao_norm ? d->ao_norm[b] : sto_norm(d->ao_n[b], d->ao_l[b], d->ao_m[b], d->ao_zeta[b]);
-      for (int a = 0; a < P.n_mo; ++a) C[(size_t)row * NMO + a] = nrm * d->mo_coeff[(size_t)b * d->n_mo + used[a]];
-      ++row;
+  std::vector<std::vector<double>> crow;  // kernel AO row -> coefficients of the referenced MOs (or empty = pad)
+  {
+    int row = 0;
+    for (size_t i = 0; i < recs.size(); ++i) {
+      const int nf = (int)recs[i].aos.size();
+      if (row % kChunk + nf > kChunk) {
+        shells.back().flush = (int16_t)(row % kChunk);
+        while (row % kChunk) { crow.emplace_back(); ++row; }
+      }
+      recs[i].r.ao0 = (int16_t)row;
+      recs[i].r.atom = (int16_t)recs[i].atom;
+      recs[i].r.flush = 0;
+      for (int b : recs[i].aos) {
+        const double nrm = d->ao_norm ? d->ao_norm[b] : sto_norm(d->ao_n[b], d->ao_l[b], d->ao_m[b], d->ao_zeta[b]);
+        std::vector<double> c(P.n_mo);
+        for (int a = 0; a < P.n_mo; ++a) c[a] = nrm * d->mo_coeff[(size_t)b * d->n_mo + used[a]];
+        crow.push_back(c);
+        ++row;
+      }
+      shells.push_back(recs[i].r);
+      if (row % kChunk == 0) shells.back().flush = (int16_t)kChunk;
     }
-    shells.push_back(recs[i].r);
+    if (row % kChunk) {
+      shells.back().flush = (int16_t)(row % kChunk);
+      while (row % kChunk) { crow.emplace_back(); ++row; }
+    }
   }
-  while (at_cur < d->n_atoms) P.shell_begin[++at_cur] = (int)recs.size();
+  const int n_chunks = (int)crow.size() / kChunk, NT = (NMO + 7) / 8;
+  // B fragments of mma.m8n8k4 (col-major B[k][n] held by lane 4 n + k)
+  std::vector<double> C((size_t)n_chunks * 4 * NT * 32, 0.0);
+  for (int ch = 0; ch < n_chunks; ++ch)
+    for (int ks = 0; ks < 4; ++ks)
+      for (int t = 0; t < NT; ++t)
+        for (int lane = 0; lane < 32; ++lane) {
+          const int k = ch * kChunk + 4 * ks + (lane & 3), n = 8 * t + (lane >> 2);
+          if (!crow[k].empty() && n < P.n_mo) C[(((size_t)ch * 4 + ks) * NT + t) * 32 + lane] = crow[k][n];
+        }
   P.n_shell = (int)shells.size();
   P.n_ao = d->n_ao;
+  P.c_doubles = (int)C.size();
 
   // ---- model FP64 work per walker
   {

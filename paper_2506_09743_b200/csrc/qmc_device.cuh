@@ -27,9 +27,12 @@ struct ShellRec {  // 32 bytes
   int16_t kind;  // SH_*
   int16_t k;     // radial power n-1-l
   int16_t m;     // harmonic index for the single-function kinds
-  int16_t ao0;   // first AO row (kernel order) of this record
-  int32_t pad;
+  int16_t ao0;   // first AO row of this record in kernel order (chunk * 16 + row in chunk)
+  int16_t atom;  // centre
+  int16_t flush; // 0, or on the last record of a 16-row AO chunk: the number of rows the chunk uses
 };
+
+constexpr int kChunk = 16;  // AO rows per DMMA chunk (4 k-steps of the m8n8k4 shape)
 
 // One determinant relative to the reference, per spin four table indices (p*LP+q) of the 2x2
 // sub-block {11, 12, 21, 22}; unused slots point at the constant entries TS-2 (= 1.0 in T, 0 in M)
@@ -46,13 +49,15 @@ struct SysParams {  // passed by value to every kernel
   int nv[2];                       // virtual orbitals per spin
   int G;                           // walkers per warp pass
   int smem_const_bytes;
+  int c_doubles;                   // size of the C fragment table
   double a_par, a_anti, b, vnn;
   double atom[kMaxAtoms][4];       // x, y, z, Z
   int shell_begin[kMaxAtoms + 1];  // shells of atom a: [shell_begin[a], shell_begin[a+1])
   int8_t ref_col[2][kMaxSpin];     // kernel MO column of reference position j, per spin
   int8_t virt_col[2][kMaxVirt];    // kernel MO column of virtual q, per spin
   const ShellRec *shells;          // device [n_shell]
-  const double *C;                 // device [n_ao][NMO]  (normalisation folded in, zero padded)
+  const double *C;                 // device [chunk][k-step 4][MO tile NT][lane 32]: DMMA B fragments of
+                                   // N_ao * C (normalisation folded in, zero padded), see qmc_setup
   const DetRec *dets;              // device [n_det]
 };
 
@@ -95,7 +100,7 @@ struct Geo {
   static constexpr int GMAX = 16 / NS;                        // walkers per warp pass (host: G <= GMAX)
   static constexpr int ROWS = (2 * GMAX * NS) < 32 ? (2 * GMAX * NS) : 32;  // electron rows of a pass
   static constexpr int TS = NS * LP + 2;  // table stride per problem: T[p][q] entries + {1.0, 0.0}
-  static constexpr int even(int x) { return (x + 1) & ~1; }
+  __host__ __device__ static constexpr int even(int x) { return (x + 1) & ~1; }
   // per-warp scratch, in doubles (all offsets even: 16-byte aligned)
   static constexpr int oPhi = 0;
   static constexpr int oB = oPhi + even(ROWS * NMO);
@@ -107,7 +112,16 @@ struct Geo {
   static constexpr int oM = oT + even(cmax(2 * GMAX * TS, 96 + 32));
   static constexpr int oProb = oM + even(2 * GMAX * TS);
   static constexpr int oRes = oProb + 2 * GMAX * 4;           // per walker {log|Psi|, sign, E_L, -}
-  static constexpr int total = oRes + GMAX * 4;
+  static constexpr int layout_total = oRes + GMAX * 4;
+  // AO tile of the DMMA contraction, [kChunk][S] doubles from offset 0 (everything it overlays is
+  // dead while it is live).  Rows: [0, ROWS) values, [ROWS, 2 ROWS) the combined operator (E_L only).
+  // S = 8 (mod 16) makes the A-fragment loads (4 k-rows x 8 rows per instruction) conflict-free.
+  __host__ __device__ static constexpr int aoStride(int ncomp) {
+    int m8 = ((ncomp * ROWS + 7) / 8) * 8;
+    return (m8 % 16 == 0) ? m8 + 8 : m8;
+  }
+  static constexpr int total = cmax(layout_total, kChunk * aoStride(2));
+  static constexpr int NT = (NMO + 7) / 8;                    // 8-column MO tiles
 };
 
 // ---------------------------------------------------------------------------------
@@ -174,6 +188,14 @@ __device__ __forceinline__ double exp_neg(double x) {
   const double r0 = fma(q1, f4, q0), r1 = fma(pcd, f4, q2);
   const double p = fma(r1, f8, r0);
   return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
+}
+
+// FP64 tensor-core MMA, D(8x8) += A(8x4) B(4x8).  Fragments (lane = 4 r + k):
+//   A[r][k] in lane 4r+k;  B[k][n] in lane 4n+k;  D[r][2k], D[r][2k+1] in lane 4r+k.
+__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+               : "+d"(d0), "+d"(d1)
+               : "d"(a), "d"(b));
 }
 
 __device__ __forceinline__ double shfl_d(double v, int src, int width) {

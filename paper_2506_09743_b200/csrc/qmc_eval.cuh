@@ -6,26 +6,6 @@
 
 namespace qmc {
 
-// ---------------------------------------------------------------------------------
-// stage a4: rank-1 update of the MO accumulators with one AO.
-// crow points at C[beta][0..NMO) in shared memory (same address in every lane: broadcast).
-// ---------------------------------------------------------------------------------
-template <int NMO, bool EL>
-__device__ __forceinline__ void contract(const double *__restrict__ crow, double phi, double bop,
-                                         double (&accP)[NMO], double (&accB)[EL ? NMO : 1]) {
-  const double2 *c2 = reinterpret_cast<const double2 *>(crow);
-#pragma unroll
-  for (int a = 0; a < NMO / 2; ++a) {
-    double2 c = c2[a];
-    accP[2 * a] = fma(phi, c.x, accP[2 * a]);
-    accP[2 * a + 1] = fma(phi, c.y, accP[2 * a + 1]);
-    if (EL) {
-      accB[2 * a] = fma(bop, c.x, accB[2 * a]);
-      accB[2 * a + 1] = fma(bop, c.y, accB[2 * a + 1]);
-    }
-  }
-}
-
 // Excitation factors of one spin of one determinant relative to the reference, from the tables
 //   T = A0^-1 Av,  Mt = A0^-1 Bv - A0^-1 B0 T                      (F.6/F.7)
 //   R  = det T[p,q] = D_X / D_0                                     (reading Q8; H.1)
@@ -108,22 +88,46 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
   // ---- stages a1-a4: STO shells and AO -> MO contraction.
   // For E_L the gradient and Laplacian are folded into ONE operator per AO (stage a6):
   //   b = -1/2 lap(phi) - grad_i J . grad(phi)      (middle and last terms of F.1)
-  double accP[NMO];
-  double accB[EL ? NMO : 1];
+  // The lane evaluates the AOs of its electron and writes them into a [16 AO rows][S] tile; every
+  // 16 rows the warp multiplies the tile into the MO accumulators with DMMA m8n8k4
+  // (D[row][mo] += A[row][ao] C[ao][mo]; rows = electrons x {value, operator}).
+  constexpr int NT = GE::NT;
+  constexpr int NCOMP = EL ? 2 : 1;
+  constexpr int MT = (NCOMP * GE::ROWS + 7) / 8;
+  constexpr int S = GE::aoStride(NCOMP);
+  double acc[MT][NT][2];
 #pragma unroll
-  for (int a = 0; a < NMO; ++a) accP[a] = 0.0;
+  for (int m = 0; m < MT; ++m)
 #pragma unroll
-  for (int a = 0; a < (EL ? NMO : 1); ++a) accB[a] = 0.0;
+    for (int t = 0; t < NT; ++t) acc[m][t][0] = acc[m][t][1] = 0.0;
   double ven = 0.0;
-  for (int at = 0; at < P.n_atoms; ++at) {
-    const double dx = x - P.atom[at][0], dy = y - P.atom[at][1], dz = z - P.atom[at][2];
-    const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-    const double ri = rsqrt_fast(r2);
-    const double r = r2 * ri;
-    if (EL) ven = fma(-P.atom[at][3], ri, ven);
-    const double gd = EL ? fma(gJx, dx, fma(gJy, dy, gJz * dz)) * ri : 0.0;  // grad J . d / r
-    for (int s = P.shell_begin[at]; s < P.shell_begin[at + 1]; ++s) {
+  {
+    double *tile = ws;  // overlays the scratch from offset 0 (all dead here except sXYZ, read above)
+    __syncwarp();       // every lane is done with sXYZ
+    const int fr = lane >> 2, fk = lane & 3;  // fragment row / k of this lane
+    int cur_atom = -1, chunk = 0;
+    double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1.0, r = 1.0, ri = 1.0, gd = 0.0;
+    auto put = [&](int row, double phi, double bop) {
+      if (active) {
+        tile[row * S + lane] = phi;
+        if (EL) tile[row * S + GE::ROWS + lane] = bop;
+      }
+    };
+    for (int s = 0; s < P.n_shell; ++s) {
       const ShellRec sh = sShell[s];
+      if (sh.atom != cur_atom) {
+        cur_atom = sh.atom;
+        dx = x - P.atom[cur_atom][0];
+        dy = y - P.atom[cur_atom][1];
+        dz = z - P.atom[cur_atom][2];
+        r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+        ri = rsqrt_fast(r2);
+        r = r2 * ri;
+        if (EL) {
+          ven = fma(-P.atom[cur_atom][3], ri, ven);
+          gd = fma(gJx, dx, fma(gJy, dy, gJz * dz)) * ri;  // grad J . d / r
+        }
+      }
       const double ex = exp_neg(-sh.zeta * r);
       const int k = sh.k;
       const double gr = (k == 0) ? ex : ((k == 1) ? ex * r : ((k == 2) ? ex * r2 : ex * r2 * r));
@@ -134,58 +138,83 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
         const double radlog = fma((double)k, ri, -sh.zeta);  // g'/g
         h = fma(-0.5, lapfac, -radlog * gd);
       }
-      const double *crow = sC + sh.ao0 * NMO;
+      const int row = sh.ao0 & (kChunk - 1);
       switch (sh.kind) {
         case SH_S: {
-          contract<NMO, EL>(crow, gr, gr * h, accP, accB);
+          put(row, gr, gr * h);
         } break;
         case SH_P: {
-          contract<NMO, EL>(crow, gr * dx, gr * fma(dx, h, -gJx), accP, accB);
-          contract<NMO, EL>(crow + NMO, gr * dy, gr * fma(dy, h, -gJy), accP, accB);
-          contract<NMO, EL>(crow + 2 * NMO, gr * dz, gr * fma(dz, h, -gJz), accP, accB);
+          put(row, gr * dx, gr * fma(dx, h, -gJx));
+          put(row + 1, gr * dy, gr * fma(dy, h, -gJy));
+          put(row + 2, gr * dz, gr * fma(dz, h, -gJz));
         } break;
         case SH_D: {
-          double S, gs;
-          S = dx * dy; gs = fma(gJx, dy, gJy * dx);
-          contract<NMO, EL>(crow, gr * S, gr * fma(S, h, -gs), accP, accB);
-          S = dy * dz; gs = fma(gJy, dz, gJz * dy);
-          contract<NMO, EL>(crow + NMO, gr * S, gr * fma(S, h, -gs), accP, accB);
-          S = dz * dx; gs = fma(gJz, dx, gJx * dz);
-          contract<NMO, EL>(crow + 2 * NMO, gr * S, gr * fma(S, h, -gs), accP, accB);
-          S = fma(dx, dx, -dy * dy); gs = 2.0 * fma(gJx, dx, -gJy * dy);
-          contract<NMO, EL>(crow + 3 * NMO, gr * S, gr * fma(S, h, -gs), accP, accB);
-          S = fma(2.0 * dz, dz, -fma(dx, dx, dy * dy));
+          double Sh, gs;
+          Sh = dx * dy; gs = fma(gJx, dy, gJy * dx);
+          put(row, gr * Sh, gr * fma(Sh, h, -gs));
+          Sh = dy * dz; gs = fma(gJy, dz, gJz * dy);
+          put(row + 1, gr * Sh, gr * fma(Sh, h, -gs));
+          Sh = dz * dx; gs = fma(gJz, dx, gJx * dz);
+          put(row + 2, gr * Sh, gr * fma(Sh, h, -gs));
+          Sh = fma(dx, dx, -dy * dy); gs = 2.0 * fma(gJx, dx, -gJy * dy);
+          put(row + 3, gr * Sh, gr * fma(Sh, h, -gs));
+          Sh = fma(2.0 * dz, dz, -fma(dx, dx, dy * dy));
           gs = 2.0 * fma(2.0 * gJz, dz, -fma(gJx, dx, gJy * dy));
-          contract<NMO, EL>(crow + 4 * NMO, gr * S, gr * fma(S, h, -gs), accP, accB);
+          put(row + 4, gr * Sh, gr * fma(Sh, h, -gs));
         } break;
         case SH_P1: {
           const int m = sh.m;
-          const double S = (m == 0) ? dx : ((m == 1) ? dy : dz);
+          const double Sh = (m == 0) ? dx : ((m == 1) ? dy : dz);
           const double gs = (m == 0) ? gJx : ((m == 1) ? gJy : gJz);
-          contract<NMO, EL>(crow, gr * S, gr * fma(S, h, -gs), accP, accB);
+          put(row, gr * Sh, gr * fma(Sh, h, -gs));
         } break;
         default: {  // SH_D1
           const int m = sh.m;
-          double S, gs;
-          if (m == 0) { S = dx * dy; gs = fma(gJx, dy, gJy * dx); }
-          else if (m == 1) { S = dy * dz; gs = fma(gJy, dz, gJz * dy); }
-          else if (m == 2) { S = dz * dx; gs = fma(gJz, dx, gJx * dz); }
-          else if (m == 3) { S = fma(dx, dx, -dy * dy); gs = 2.0 * fma(gJx, dx, -gJy * dy); }
-          else { S = fma(2.0 * dz, dz, -fma(dx, dx, dy * dy)); gs = 2.0 * fma(2.0 * gJz, dz, -fma(gJx, dx, gJy * dy)); }
-          contract<NMO, EL>(crow, gr * S, gr * fma(S, h, -gs), accP, accB);
+          double Sh, gs;
+          if (m == 0) { Sh = dx * dy; gs = fma(gJx, dy, gJy * dx); }
+          else if (m == 1) { Sh = dy * dz; gs = fma(gJy, dz, gJz * dy); }
+          else if (m == 2) { Sh = dz * dx; gs = fma(gJz, dx, gJx * dz); }
+          else if (m == 3) { Sh = fma(dx, dx, -dy * dy); gs = 2.0 * fma(gJx, dx, -gJy * dy); }
+          else { Sh = fma(2.0 * dz, dz, -fma(dx, dx, dy * dy)); gs = 2.0 * fma(2.0 * gJz, dz, -fma(gJx, dx, gJy * dy)); }
+          put(row, gr * Sh, gr * fma(Sh, h, -gs));
         } break;
       }
+      if (sh.flush) {
+        // unused rows of the chunk meet zero rows of C, but must themselves be finite
+        for (int pr = sh.flush; pr < kChunk; ++pr) put(pr, 0.0, 0.0);
+        __syncwarp();
+        const double *cf = sC + chunk * (4 * NT * 32) + lane;
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks) {
+          double bf[NT];
+#pragma unroll
+          for (int t = 0; t < NT; ++t) bf[t] = cf[(ks * NT + t) * 32];
+          const double *arow = tile + (4 * ks + fk) * S + fr;
+#pragma unroll
+          for (int m = 0; m < MT; ++m) {
+            const double a = arow[8 * m];
+#pragma unroll
+            for (int t = 0; t < NT; ++t) dmma884(acc[m][t][0], acc[m][t][1], a, bf[t]);
+          }
+        }
+        __syncwarp();
+        ++chunk;
+      }
     }
-  }
-  // hand the MO rows over
-  if (active) {
-    double2 *dst = reinterpret_cast<double2 *>(sPhi + lane * NMO);
+    // D fragments -> MO rows: lane holds D[8 m + fr][8 t + 2 fk + {0,1}]
 #pragma unroll
-    for (int a = 0; a < NMO / 2; ++a) dst[a] = make_double2(accP[2 * a], accP[2 * a + 1]);
-    if (EL) {
-      double2 *dstb = reinterpret_cast<double2 *>(sB + lane * NMO);
+    for (int m = 0; m < MT; ++m) {
+      const int R = 8 * m + fr;
+      const bool isB = EL && (R >= GE::ROWS);
+      const int el = isB ? R - GE::ROWS : R;
+      double *dst = (isB ? sB : sPhi) + el * NMO;
+      if (el < G * ne && R < NCOMP * GE::ROWS) {
 #pragma unroll
-      for (int a = 0; a < NMO / 2; ++a) dstb[a] = make_double2(accB[2 * a], accB[2 * a + 1]);
+        for (int t = 0; t < NT; ++t) {
+          const int col = 8 * t + 2 * fk;
+          if (col < NMO) *reinterpret_cast<double2 *>(dst + col) = make_double2(acc[m][t][0], acc[m][t][1]);
+        }
+      }
     }
   }
   {

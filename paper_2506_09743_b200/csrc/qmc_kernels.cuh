@@ -10,7 +10,7 @@ template <int NMO>
 __device__ __forceinline__ void load_constants(const SysParams &P, unsigned char *smem, const double *&sC,
                                                const ShellRec *&sShell, const DetRec *&sDet, double *&wsBase) {
   double *c = reinterpret_cast<double *>(smem);
-  const int nC = P.n_ao * NMO;
+  const int nC = P.c_doubles;
   for (int i = threadIdx.x; i < nC; i += blockDim.x) c[i] = P.C[i];
   ShellRec *sh = reinterpret_cast<ShellRec *>(c + nC);
   {
@@ -229,12 +229,6 @@ __global__ void __launch_bounds__(1024) batch_stats_kernel(const double *__restr
 // ---------------------------------------------------------------------------------
 // FP64 peak microbenchmarks (roofline denominator; BASELINE.json north_star)
 // ---------------------------------------------------------------------------------
-__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
-  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
-               : "+d"(d0), "+d"(d1)
-               : "d"(a), "d"(b));
-}
-
 template <int KIND>
 __global__ void __launch_bounds__(256) fp64_peak_kernel(double *out, int iters, double seed) {
   double a[8], m0[4], m1[4];
