@@ -325,6 +325,8 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
           if (!crow[k].empty() && n < P.n_mo) C[(((size_t)ch * 4 + ks) * NT + t) * 32 + lane] = crow[k][n];
         }
   P.n_shell = (int)shells.size();
+  shells.push_back(shells.back());  // padding record: the kernel prefetches one ahead
+  shells.back().flush = 0;
   P.n_ao = d->n_ao;
   P.c_doubles = (int)C.size();
 

@@ -55,32 +55,44 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
   sXYZ[lane * 3 + 2] = z;
   __syncwarp();
 
-  // ---- stage a5: Pade Jastrow (D.1) and e-e repulsion (eq. 1)
-  double J2 = 0.0, gJx = 0.0, gJy = 0.0, gJz = 0.0, lapJ = 0.0, vee2 = 0.0;
+  // ---- stage a5: Pade Jastrow (D.1) and e-e repulsion (eq. 1).
+  // Every unordered pair is evaluated once: electron e takes the partners e+1 .. e+(ne-1)/2 (cyclic),
+  // and for even ne the lower half also takes e+ne/2; the partner's share of the gradient (the
+  // opposite vector) travels by shuffle from the lane that computed the pair.
+  double Jp = 0.0, gJx = 0.0, gJy = 0.0, gJz = 0.0, lapJ = 0.0, vee = 0.0;
   {
     const bool up = e < P.n_up;
     const int base = (active ? g : 0) * ne;
-    for (int j = 0; j < ne; ++j) {
-      double dx = x - sXYZ[(base + j) * 3 + 0];
-      double dy = y - sXYZ[(base + j) * 3 + 1];
-      double dz = z - sXYZ[(base + j) * 3 + 2];
-      if (j == e) continue;
-      double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-      double ri = rsqrt_fast(r2);
-      double r = r2 * ri;
+    const int nfull = (ne - 1) >> 1, nofs = ne >> 1, half = ne >> 1;
+#pragma unroll 2
+    for (int o = 1; o <= nofs; ++o) {
+      int j = e + o;
+      j -= (j >= ne) ? ne : 0;
+      const bool take = (o <= nfull) || (e < half);
+      const double dx = x - sXYZ[(base + j) * 3 + 0];
+      const double dy = y - sXYZ[(base + j) * 3 + 1];
+      const double dz = z - sXYZ[(base + j) * 3 + 2];
+      const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+      const double ri = rsqrt_fast(r2);
+      const double r = r2 * ri;
       double a = ((j < P.n_up) == up) ? P.a_par : P.a_anti;
-      double di = rcp_fast(fma(P.b, r, 1.0));
-      double adi = a * di;
-      J2 = fma(adi, r, J2);  // u = a r / (1 + b r)
+      a = take ? a : 0.0;
+      const double di = rcp_fast(fma(P.b, r, 1.0));
+      const double adi = a * di;
+      Jp = fma(adi, r, Jp);  // u = a r / (1 + b r)
       if (EL) {
-        double u1 = adi * di;                  // u'  = a / (1 + b r)^2
-        double u2 = -2.0 * P.b * u1 * di;      // u'' = -2 a b / (1 + b r)^3
-        double s = u1 * ri;
-        gJx = fma(s, dx, gJx);
-        gJy = fma(s, dy, gJy);
-        gJz = fma(s, dz, gJz);
-        lapJ += fma(2.0, s, u2);               // lap_i K(r_ij) = u'' + 2 u'/r
-        vee2 += ri;
+        const double u1 = adi * di;              // u'  = a / (1 + b r)^2
+        const double u2 = -2.0 * P.b * u1 * di;  // u'' = -2 a b / (1 + b r)^3
+        const double sc = u1 * ri;
+        const double cx = sc * dx, cy = sc * dy, cz = sc * dz;
+        lapJ += 2.0 * fma(2.0, sc, u2);          // lap_i K + lap_j K = 2 (u'' + 2 u'/r)
+        vee += take ? ri : 0.0;
+        int src = e - o;
+        src += (src < 0) ? ne : 0;
+        const int sl = (lane - e + src) & 31;    // lane that computed the pair (src, e)
+        gJx += cx - shfl_d(cx, sl, 32);
+        gJy += cy - shfl_d(cy, sl, 32);
+        gJz += cz - shfl_d(cz, sl, 32);
       }
     }
   }
@@ -113,8 +125,10 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
         if (EL) tile[row * S + GE::ROWS + lane] = bop;
       }
     };
+    ShellRec nxt = sShell[0];
     for (int s = 0; s < P.n_shell; ++s) {
-      const ShellRec sh = sShell[s];
+      const ShellRec sh = nxt;
+      nxt = sShell[s + 1];  // one padding record follows the table
       if (sh.atom != cur_atom) {
         cur_atom = sh.atom;
         dx = x - P.atom[cur_atom][0];
@@ -219,9 +233,8 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
   }
   {
     // per-electron scalars: J/2-sum and the electron's share of the energy
-    sPart[lane * 2 + 0] = 0.5 * J2;
-    sPart[lane * 2 + 1] =
-        EL ? (fma(-0.5, lapJ + fma(gJx, gJx, fma(gJy, gJy, gJz * gJz)), fma(0.5, vee2, ven))) : 0.0;
+    sPart[lane * 2 + 0] = Jp;
+    sPart[lane * 2 + 1] = EL ? (fma(-0.5, lapJ + fma(gJx, gJx, fma(gJy, gJy, gJz * gJz)), vee + ven)) : 0.0;
   }
   __syncwarp();
 
@@ -380,16 +393,21 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
       den = fma(w, Rd, den);
       if (EL) num = fma(dr.d, Du * Rd, fma(w, Dd, num));
     }
+    double Jsum = 0.0, esum = 0.0;
+    if (wvalid)
+      for (int j = sub; j < ne; j += LW) {
+        Jsum += sPart[(wg * ne + j) * 2 + 0];
+        if (EL) esum += sPart[(wg * ne + j) * 2 + 1];
+      }
     for (int m = 1; m < LW; m <<= 1) {
       den += shfl_xor_d(den, m);
-      if (EL) num += shfl_xor_d(num, m);
+      Jsum += shfl_xor_d(Jsum, m);
+      if (EL) {
+        num += shfl_xor_d(num, m);
+        esum += shfl_xor_d(esum, m);
+      }
     }
     if (wvalid && sub == 0) {
-      double Jsum = 0.0, esum = 0.0;
-      for (int j = 0; j < ne; ++j) {
-        Jsum += sPart[(wg * ne + j) * 2 + 0];
-        esum += sPart[(wg * ne + j) * 2 + 1];
-      }
       const double lu = sProb[pu * 4 + 0], ld = sProb[pd * 4 + 0];
       const double sgn = sProb[pu * 4 + 1] * sProb[pd * 4 + 1];
       sRes[wg * 4 + 0] = Jsum + lu + ld + log(fabs(den));

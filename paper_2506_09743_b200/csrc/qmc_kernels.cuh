@@ -16,9 +16,9 @@ __device__ __forceinline__ void load_constants(const SysParams &P, unsigned char
   {
     const double *src = reinterpret_cast<const double *>(P.shells);
     double *dst = reinterpret_cast<double *>(sh);
-    for (int i = threadIdx.x; i < P.n_shell * 4; i += blockDim.x) dst[i] = src[i];
+    for (int i = threadIdx.x; i < (P.n_shell + 1) * 4; i += blockDim.x) dst[i] = src[i];
   }
-  DetRec *dt = reinterpret_cast<DetRec *>(sh + P.n_shell);
+  DetRec *dt = reinterpret_cast<DetRec *>(sh + P.n_shell + 1);
   {
     const double *src = reinterpret_cast<const double *>(P.dets);
     double *dst = reinterpret_cast<double *>(dt);
@@ -54,17 +54,23 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, 2)
   const int g = lane / ne, e = lane - g * ne;
   const int64_t n_groups = (io.M + G - 1) / G;
   const int64_t stride = (int64_t)gridDim.x * kWarpsPerBlock;
-  for (int64_t grp = (int64_t)blockIdx.x * kWarpsPerBlock + warp; grp < n_groups; grp += stride) {
+  // the coordinates of the next group are fetched while the current one is evaluated
+  auto fetch = [&](int64_t grp, double &x, double &y, double &z) {
     const int64_t w = grp * G + g;
-    const bool own = (g < G) && (w < io.M);
-    double x, y, z;
-    if (own) {
-      x = io.r_in[((int64_t)e * 3 + 0) * io.M + w];
-      y = io.r_in[((int64_t)e * 3 + 1) * io.M + w];
-      z = io.r_in[((int64_t)e * 3 + 2) * io.M + w];
+    if ((g < G) && (w < io.M)) {
+      x = __ldg(io.r_in + ((int64_t)e * 3 + 0) * io.M + w);
+      y = __ldg(io.r_in + ((int64_t)e * 3 + 1) * io.M + w);
+      z = __ldg(io.r_in + ((int64_t)e * 3 + 2) * io.M + w);
     } else {
       dummy_xyz(lane, x, y, z);
     }
+  };
+  int64_t grp = (int64_t)blockIdx.x * kWarpsPerBlock + warp;
+  double nx, ny, nz;
+  fetch(grp, nx, ny, nz);
+  for (; grp < n_groups; grp += stride) {
+    const double x = nx, y = ny, z = nz;
+    fetch(grp + stride, nx, ny, nz);
     eval_walkers<NS, NMO, EL>(P, sShell, sC, sDet, ws, x, y, z, lane);
     if (lane < G) {
       const int64_t wo = grp * G + lane;
