@@ -33,31 +33,37 @@ int cuda_fail(cudaError_t e, const char *what) {
 
 struct Variant {
   int NS, NMO, LP, ws_doubles;
+  bool exact;  // compiled for n_up = n_dn = NS
   const void *k_el, *k_psi, *k_metro, *k_metro_el;
 };
 
-template <int NS, int NMO>
+template <int NS, int NMO, bool X>
 Variant make_variant() {
   Variant v;
   v.NS = NS;
   v.NMO = NMO;
   v.LP = Geo<NS, NMO>::LP;
+  v.exact = X;
   v.ws_doubles = Geo<NS, NMO>::total;
-  v.k_el = (const void *)local_energy_kernel<NS, NMO, true>;
-  v.k_psi = (const void *)local_energy_kernel<NS, NMO, false>;
-  v.k_metro = (const void *)metropolis_kernel<NS, NMO, false>;
-  v.k_metro_el = (const void *)metropolis_kernel<NS, NMO, true>;
+  v.k_el = (const void *)local_energy_kernel<NS, NMO, true, X>;
+  v.k_psi = (const void *)local_energy_kernel<NS, NMO, false, X>;
+  v.k_metro = (const void *)metropolis_kernel<NS, NMO, false, X>;
+  v.k_metro_el = (const void *)metropolis_kernel<NS, NMO, true, X>;
   return v;
 }
 
 const std::vector<Variant> &variants() {
   static const std::vector<Variant> v = {
-      make_variant<1, 2>(),  // H2-like
-      make_variant<2, 2>(),  // LiH-like single determinant
-      make_variant<3, 8>(),  // Li2-like
-      make_variant<4, 8>(),
-      make_variant<7, 14>(),  // CO-like (headline)
-      make_variant<8, 16>(),  // generic upper bound
+#ifndef QMC_ONLY_CO  // (experiments: build the headline instantiation only)
+      make_variant<1, 2, true>(),   // H2-like
+      make_variant<2, 2, true>(),   // LiH-like single determinant
+      make_variant<3, 8, true>(),   // Li2-like
+#endif
+      make_variant<7, 14, true>(),  // CO-like (headline)
+#ifndef QMC_ONLY_CO
+      make_variant<4, 8, false>(),  // generic, runtime electron counts
+      make_variant<8, 16, false>(), // generic upper bound
+#endif
   };
   return v;
 }
@@ -227,7 +233,8 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   const int ns_max = std::max(d->n_up, d->n_dn), nv_max = std::max(P.nv[0], P.nv[1]);
   const Variant *var = nullptr;
   for (const Variant &v : variants())
-    if (v.NS >= ns_max && v.NMO >= P.n_mo && v.LP >= nv_max && v.LP >= ns_max) {
+    if (v.NS >= ns_max && v.NMO >= P.n_mo && v.LP >= nv_max && v.LP >= ns_max &&
+        (!v.exact || (d->n_up == v.NS && d->n_dn == v.NS))) {
       var = &v;
       break;
     }
@@ -285,15 +292,31 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     recs.push_back(rc);
   }
   std::stable_sort(recs.begin(), recs.end(), [](const Rec &a, const Rec &b) { return a.atom < b.atom; });
-  // AO rows are laid out in chunks of 16 (one DMMA pass each); a record never straddles a chunk
+  // AO rows are laid out in chunks of kChunk (one DMMA pass each); a record never straddles a chunk.
+  // Records are grouped in fours that share a centre (padded with SH_NULL) for the kernel's quad loop.
   std::vector<ShellRec> shells;
   std::vector<std::vector<double>> crow;  // kernel AO row -> coefficients of the referenced MOs (or empty = pad)
+  int n_real_shells = 0;
   {
     int row = 0;
+    auto last_real = [&]() -> ShellRec & {
+      size_t i = shells.size();
+      while (shells[i - 1].kind == SH_NULL) --i;
+      return shells[i - 1];
+    };
+    auto pad_quad = [&]() {
+      while (shells.size() % 4) {
+        ShellRec nul = shells.back();
+        nul.kind = SH_NULL;
+        nul.flush = 0;
+        shells.push_back(nul);
+      }
+    };
     for (size_t i = 0; i < recs.size(); ++i) {
       const int nf = (int)recs[i].aos.size();
+      if (i > 0 && recs[i].atom != recs[i - 1].atom) pad_quad();
       if (row % kChunk + nf > kChunk) {
-        shells.back().flush = (int16_t)(row % kChunk);
+        last_real().flush = (int16_t)(row % kChunk);
         while (row % kChunk) { crow.emplace_back(); ++row; }
       }
       recs[i].r.ao0 = (int16_t)row;
@@ -307,33 +330,34 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
         ++row;
       }
       shells.push_back(recs[i].r);
+      ++n_real_shells;
       if (row % kChunk == 0) shells.back().flush = (int16_t)kChunk;
     }
     if (row % kChunk) {
-      shells.back().flush = (int16_t)(row % kChunk);
+      last_real().flush = (int16_t)(row % kChunk);
       while (row % kChunk) { crow.emplace_back(); ++row; }
     }
+    pad_quad();
   }
-  const int n_chunks = (int)crow.size() / kChunk, NT = (NMO + 7) / 8;
+  const int n_chunks = (int)crow.size() / kChunk, NT = (NMO + 7) / 8, KS = kChunk / 4;
+  P.n_chunks = n_chunks;
   // B fragments of mma.m8n8k4 (col-major B[k][n] held by lane 4 n + k)
-  std::vector<double> C((size_t)n_chunks * 4 * NT * 32, 0.0);
+  std::vector<double> C((size_t)n_chunks * KS * NT * 32, 0.0);
   for (int ch = 0; ch < n_chunks; ++ch)
-    for (int ks = 0; ks < 4; ++ks)
+    for (int ks = 0; ks < KS; ++ks)
       for (int t = 0; t < NT; ++t)
         for (int lane = 0; lane < 32; ++lane) {
           const int k = ch * kChunk + 4 * ks + (lane & 3), n = 8 * t + (lane >> 2);
-          if (!crow[k].empty() && n < P.n_mo) C[(((size_t)ch * 4 + ks) * NT + t) * 32 + lane] = crow[k][n];
+          if (!crow[k].empty() && n < P.n_mo) C[(((size_t)ch * KS + ks) * NT + t) * 32 + lane] = crow[k][n];
         }
-  P.n_shell = (int)shells.size();
-  shells.push_back(shells.back());  // padding record: the kernel prefetches one ahead
-  shells.back().flush = 0;
+  P.n_shell = (int)shells.size();  // multiple of 4, SH_NULL padding included
   P.n_ao = d->n_ao;
   P.c_doubles = (int)C.size();
 
   // ---- model FP64 work per walker
   {
     const double cexp = 40, cdiv = 20, csqrt = 20, clog = 50, csincos = 80;
-    const double ne = P.n_e, nat = P.n_atoms, nsh = P.n_shell, nao = P.n_ao, nmo = P.n_mo, nd = P.n_det;
+    const double ne = P.n_e, nat = P.n_atoms, nsh = n_real_shells, nao = P.n_ao, nmo = P.n_mo, nd = P.n_det;
     const double npair = ne * (ne - 1) / 2;
     double lu_el = 0, lu_st = 0;
     for (int sp = 0; sp < 2; ++sp) {

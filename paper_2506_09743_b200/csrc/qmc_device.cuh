@@ -15,10 +15,26 @@ namespace qmc {
 constexpr int kMaxAtoms = 16;
 constexpr int kMaxSpin = 8;   // electrons per spin
 constexpr int kMaxVirt = 8;   // distinct virtual orbitals per spin
-constexpr int kWarpsPerBlock = 8;
+// tuning knobs (defaults are the measured best on B200)
+#ifndef QMC_WARPS
+#define QMC_WARPS 8          // warps per block
+#endif
+#ifndef QMC_MINBLOCKS
+#define QMC_MINBLOCKS 2      // blocks per SM the register allocation must allow
+#endif
+#ifndef QMC_SHELL_UNROLL
+#define QMC_SHELL_UNROLL 1   // shell records whose exponentials are evaluated together (1, 2 or 4)
+#endif
+#ifndef QMC_PAIR_UNROLL
+#define QMC_PAIR_UNROLL 2    // unroll factor of the electron-pair loop
+#endif
+#ifndef QMC_EARLY_INV
+#define QMC_EARLY_INV 0      // Gauss-Jordan: invert every pivot candidate before the arg-max is known
+#endif
+constexpr int kWarpsPerBlock = QMC_WARPS;
 
 // shell record kinds
-enum : int { SH_S = 0, SH_P = 1, SH_D = 2, SH_P1 = 3, SH_D1 = 4 };
+enum : int { SH_S = 0, SH_P = 1, SH_D = 2, SH_P1 = 3, SH_D1 = 4, SH_NULL = 5 };
 
 struct ShellRec {  // 32 bytes
   double zeta;
@@ -32,7 +48,14 @@ struct ShellRec {  // 32 bytes
   int16_t flush; // 0, or on the last record of a 16-row AO chunk: the number of rows the chunk uses
 };
 
-constexpr int kChunk = 16;  // AO rows per DMMA chunk (4 k-steps of the m8n8k4 shape)
+#ifndef QMC_CHUNK
+#define QMC_CHUNK 16         // AO rows per DMMA chunk (8 or 16: 2 or 4 k-steps of the m8n8k4 shape)
+#endif
+#ifndef QMC_PARK_ACC
+#define QMC_PARK_ACC 0       // 1: park the MO accumulators in shared memory between chunks (frees registers
+                             // during the AO evaluation, costs ~20% more shared-memory wavefronts)
+#endif
+constexpr int kChunk = QMC_CHUNK;
 
 // One determinant relative to the reference, per spin four table indices (p*LP+q) of the 2x2
 // sub-block {11, 12, 21, 22}; unused slots point at the constant entries TS-2 (= 1.0 in T, 0 in M)
@@ -50,6 +73,7 @@ struct SysParams {  // passed by value to every kernel
   int G;                           // walkers per warp pass
   int smem_const_bytes;
   int c_doubles;                   // size of the C fragment table
+  int n_chunks;                    // AO chunks of kChunk rows
   double a_par, a_anti, b, vnn;
   double atom[kMaxAtoms][4];       // x, y, z, Z
   int shell_begin[kMaxAtoms + 1];  // shells of atom a: [shell_begin[a], shell_begin[a+1])
@@ -101,26 +125,38 @@ struct Geo {
   static constexpr int ROWS = (2 * GMAX * NS) < 32 ? (2 * GMAX * NS) : 32;  // electron rows of a pass
   static constexpr int TS = NS * LP + 2;  // table stride per problem: T[p][q] entries + {1.0, 0.0}
   __host__ __device__ static constexpr int even(int x) { return (x + 1) & ~1; }
-  // per-warp scratch, in doubles (all offsets even: 16-byte aligned)
+  // per-warp scratch, in doubles (all offsets even: 16-byte aligned).
+  // When one Gauss-Jordan pass covers all 2 GMAX problems (SINGLE), the MO rows are in registers
+  // before the first table entry is written, so G, T and M reuse the space of Phi and B.
+  static constexpr int szPhi = even(ROWS * NMO);
+  static constexpr int szG = even(cmax(PP * NS * NS, 2));
+  static constexpr int szT = even(cmax(2 * GMAX * TS, 96 + 32));  // also hosts the Metropolis draws
+  static constexpr int szM = even(2 * GMAX * TS);
+  static constexpr bool SINGLE = (2 * GMAX <= PP) && (2 * szPhi >= szG + szT + szM);
   static constexpr int oPhi = 0;
-  static constexpr int oB = oPhi + even(ROWS * NMO);
-  static constexpr int oPart = oB + even(ROWS * NMO);
-  static constexpr int oXYZ = oPart + 64;                     // coordinates (pair loop) ...
-  static constexpr int oG = oXYZ;                             // ... later reused by the Gm staging
-  static constexpr int oT = oG + even(cmax(PP * NS * NS, 96));
+  static constexpr int oB = oPhi + szPhi;
+  static constexpr int oG = SINGLE ? 0 : oB + szPhi;
+  static constexpr int oT = oG + szG;
   static constexpr int oProp = oT;                            // Metropolis draws are consumed before T is written
-  static constexpr int oM = oT + even(cmax(2 * GMAX * TS, 96 + 32));
-  static constexpr int oProb = oM + even(2 * GMAX * TS);
+  static constexpr int oM = oT + szT;
+  static constexpr int oPart = SINGLE ? oB + szPhi : oM + szM;
+  static constexpr int oXYZ = oPart + 64;                     // coordinates (pair loop)
+  static constexpr int oProb = oXYZ + 96;
   static constexpr int oRes = oProb + 2 * GMAX * 4;           // per walker {log|Psi|, sign, E_L, -}
   static constexpr int layout_total = oRes + GMAX * 4;
-  // AO tile of the DMMA contraction, [kChunk][S] doubles from offset 0 (everything it overlays is
-  // dead while it is live).  Rows: [0, ROWS) values, [ROWS, 2 ROWS) the combined operator (E_L only).
-  // S = 8 (mod 16) makes the A-fragment loads (4 k-rows x 8 rows per instruction) conflict-free.
+  // DMMA contraction scratch, from offset 0 (everything it overlays is dead while it is live):
+  // the MO accumulators in D-fragment order [m-tile][n-tile][lane][2] (parked here between AO chunks
+  // so that they occupy no registers while the AOs are evaluated), then the AO tile [kChunk][S].
+  // Tile rows: [0, ROWS) values, [ROWS, 2 ROWS) the combined operator (E_L only).  S = 8 (mod 16)
+  // makes the A-fragment loads (4 k-rows x 8 rows per instruction) conflict-free.
   __host__ __device__ static constexpr int aoStride(int ncomp) {
     int m8 = ((ncomp * ROWS + 7) / 8) * 8;
     return (m8 % 16 == 0) ? m8 + 8 : m8;
   }
-  static constexpr int total = cmax(layout_total, kChunk * aoStride(2));
+  __host__ __device__ static constexpr int accDoubles(int ncomp) {
+    return ((ncomp * ROWS + 7) / 8) * ((NMO + 7) / 8) * 64;
+  }
+  static constexpr int total = cmax(layout_total, (QMC_PARK_ACC ? accDoubles(2) : 0) + kChunk * aoStride(2));
   static constexpr int NT = (NMO + 7) / 8;                    // 8-column MO tiles
 };
 
@@ -166,27 +202,35 @@ __device__ __forceinline__ double rsqrt_fast(double x) {
 }
 
 // exp(x) for x <= 0 (STO radial factors e^{-zeta r}): x = n ln2 + f, |f| <= ln2/2, degree-13 Taylor
-// polynomial in Estrin form (truncation 4e-18 relative), 2^n applied to the exponent field.
-// Arguments below -700 are clamped (value ~1e-304, i.e. zero for every use here).
+// polynomial (truncation 4e-18 relative) as two Horner chains in f^2 whose coefficients come straight
+// from the constant bank (no registers), 2^n applied to the exponent field.  Arguments below -700
+// are clamped (value ~1e-304, i.e. zero for every use here).
+__constant__ double kExpC[14] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040,
+                                 1.0 / 40320, 1.0 / 362880, 1.0 / 3628800, 1.0 / 39916800,
+                                 1.0 / 479001600, 1.0 / 6227020800.0};
+__constant__ double kExpR[4] = {1.4426950408889634, 6755399441055744.0, -6.93147180369123816490e-01,
+                                -1.90821492927058770002e-10};
 __device__ __forceinline__ double exp_neg(double x) {
   x = fmax(x, -700.0);
-  const double magic = 6755399441055744.0;  // 1.5 * 2^52
-  const double t = fma(x, 1.4426950408889634, magic);
+  const double t = fma(x, kExpR[0], kExpR[1]);  // round(x / ln2) in the low mantissa bits
   const int n = __double2loint(t);
-  const double nd = t - magic;
-  double f = fma(nd, -6.93147180369123816490e-01, x);
-  f = fma(nd, -1.90821492927058770002e-10, f);
-  const double f2 = f * f, f4 = f2 * f2, f8 = f4 * f4;
-  const double p01 = 1.0 + f;
-  const double p23 = fma(f, 1.0 / 6.0, 0.5);
-  const double p45 = fma(f, 1.0 / 120.0, 1.0 / 24.0);
-  const double p67 = fma(f, 1.0 / 5040.0, 1.0 / 720.0);
-  const double p89 = fma(f, 1.0 / 362880.0, 1.0 / 40320.0);
-  const double pab = fma(f, 1.0 / 39916800.0, 1.0 / 3628800.0);
-  const double pcd = fma(f, 1.0 / 6227020800.0, 1.0 / 479001600.0);
-  const double q0 = fma(p23, f2, p01), q1 = fma(p67, f2, p45), q2 = fma(pab, f2, p89);
-  const double r0 = fma(q1, f4, q0), r1 = fma(pcd, f4, q2);
-  const double p = fma(r1, f8, r0);
+  const double nd = t - kExpR[1];
+  double f = fma(nd, kExpR[2], x);
+  f = fma(nd, kExpR[3], f);
+  const double f2 = f * f;
+  double pe = fma(f2, kExpC[12], kExpC[10]);
+  double po = fma(f2, kExpC[13], kExpC[11]);
+  pe = fma(pe, f2, kExpC[8]);
+  po = fma(po, f2, kExpC[9]);
+  pe = fma(pe, f2, kExpC[6]);
+  po = fma(po, f2, kExpC[7]);
+  pe = fma(pe, f2, kExpC[4]);
+  po = fma(po, f2, kExpC[5]);
+  pe = fma(pe, f2, kExpC[2]);
+  po = fma(po, f2, kExpC[3]);
+  pe = fma(pe, f2, kExpC[0]);
+  po = fma(po, f2, kExpC[1]);
+  const double p = fma(po, f, pe);
   return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
 }
 

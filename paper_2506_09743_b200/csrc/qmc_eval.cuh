@@ -11,23 +11,30 @@ namespace qmc {
 //   R  = det T[p,q] = D_X / D_0                                     (reading Q8; H.1)
 //   Rd = Tr(adj(T[p,q]) Mt[p,q]) = R * Tr((P A0^-1 A_X P)^-1 P M P) (F.6)
 // idx packs four uint8 table indices {11, 12, 21, 22}.
+// For E_L the two tables are interleaved, entry = {T, Mt} (one 16-byte load per entry).
 template <bool EL>
-__device__ __forceinline__ void excite_single(uint32_t idx, const double *__restrict__ T,
-                                              const double *__restrict__ Mt, double &R, double &Rd) {
+__device__ __forceinline__ void excite_single(uint32_t idx, const double *__restrict__ T, double &R, double &Rd) {
   const int i = idx & 255;
-  R = T[i];
-  Rd = EL ? Mt[i] : 0.0;
+  if (EL) {
+    const double2 v = reinterpret_cast<const double2 *>(T)[i];
+    R = v.x;
+    Rd = v.y;
+  } else {
+    R = T[i];
+    Rd = 0.0;
+  }
 }
 template <bool EL>
-__device__ __forceinline__ void excite_double(uint32_t idx, const double *__restrict__ T,
-                                              const double *__restrict__ Mt, double &R, double &Rd) {
+__device__ __forceinline__ void excite_double(uint32_t idx, const double *__restrict__ T, double &R, double &Rd) {
   const int i11 = idx & 255, i12 = (idx >> 8) & 255, i21 = (idx >> 16) & 255, i22 = idx >> 24;
-  const double t11 = T[i11], t12 = T[i12], t21 = T[i21], t22 = T[i22];
-  R = fma(t11, t22, -t12 * t21);
-  Rd = 0.0;
   if (EL) {
-    const double m11 = Mt[i11], m12 = Mt[i12], m21 = Mt[i21], m22 = Mt[i22];
-    Rd = fma(t22, m11, fma(t11, m22, -fma(t12, m21, t21 * m12)));
+    const double2 *TM = reinterpret_cast<const double2 *>(T);
+    const double2 a = TM[i11], b = TM[i12], c = TM[i21], d = TM[i22];
+    R = fma(a.x, d.x, -b.x * c.x);
+    Rd = fma(d.x, a.y, fma(a.x, d.y, -fma(b.x, c.y, c.x * b.y)));
+  } else {
+    R = fma(T[i11], T[i22], -T[i12] * T[i21]);
+    Rd = 0.0;
   }
 }
 
@@ -36,23 +43,24 @@ __device__ __forceinline__ void excite_double(uint32_t idx, const double *__rest
 // at (x, y, z).  Results for walker g are left in ws[oRes + 4 g + {0,1,2}] =
 // {log|Psi|, sign, E_L} (E_L only if EL).  All 32 lanes must call.
 // ---------------------------------------------------------------------------------
-template <int NS, int NMO, bool EL>
+template <int NS, int NMO, bool EL, bool X>
 __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sShell,
                              const double *__restrict__ sC, const DetRec *__restrict__ sDet,
                              double *__restrict__ ws, double x, double y, double z, int lane) {
   using GE = Geo<NS, NMO>;
   constexpr int LP = GE::LP, PP = GE::PP, TS = GE::TS;
-  const int ne = P.n_e, G = P.G;
+  // X: closed-shell system that matches the instantiation exactly (n_up = n_dn = NS): sizes fold
+  const int n_up = X ? NS : P.n_up, n_dn = X ? NS : P.n_dn, ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
   const int g = lane / ne, e = lane - g * ne;
   const bool active = lane < G * ne;
   double *sPhi = ws + GE::oPhi, *sB = ws + GE::oB, *sXYZ = ws + GE::oXYZ, *sPart = ws + GE::oPart;
-  double *sG = ws + GE::oG, *sT = ws + GE::oT, *sM = ws + GE::oM, *sProb = ws + GE::oProb;
+  double *sG = ws + GE::oG, *sT = ws + GE::oT, *sProb = ws + GE::oProb;
   double *sRes = ws + GE::oRes;
 
   // ---- publish coordinates for the pair loop
-  sXYZ[lane * 3 + 0] = x;
-  sXYZ[lane * 3 + 1] = y;
-  sXYZ[lane * 3 + 2] = z;
+  sXYZ[lane] = x;  // [xyz][lane]: the pair loop reads consecutive lanes
+  sXYZ[32 + lane] = y;
+  sXYZ[64 + lane] = z;
   __syncwarp();
 
   // ---- stage a5: Pade Jastrow (D.1) and e-e repulsion (eq. 1).
@@ -61,21 +69,22 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
   // opposite vector) travels by shuffle from the lane that computed the pair.
   double Jp = 0.0, gJx = 0.0, gJy = 0.0, gJz = 0.0, lapJ = 0.0, vee = 0.0;
   {
-    const bool up = e < P.n_up;
+    const bool up = e < n_up;
     const int base = (active ? g : 0) * ne;
     const int nfull = (ne - 1) >> 1, nofs = ne >> 1, half = ne >> 1;
-#pragma unroll 2
+    constexpr int kPairUnroll = QMC_PAIR_UNROLL;
+#pragma unroll kPairUnroll
     for (int o = 1; o <= nofs; ++o) {
       int j = e + o;
       j -= (j >= ne) ? ne : 0;
       const bool take = (o <= nfull) || (e < half);
-      const double dx = x - sXYZ[(base + j) * 3 + 0];
-      const double dy = y - sXYZ[(base + j) * 3 + 1];
-      const double dz = z - sXYZ[(base + j) * 3 + 2];
+      const double dx = x - sXYZ[base + j];
+      const double dy = y - sXYZ[32 + base + j];
+      const double dz = z - sXYZ[64 + base + j];
       const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
       const double ri = rsqrt_fast(r2);
       const double r = r2 * ri;
-      double a = ((j < P.n_up) == up) ? P.a_par : P.a_anti;
+      double a = ((j < n_up) == up) ? P.a_par : P.a_anti;
       a = take ? a : 0.0;
       const double di = rcp_fast(fma(P.b, r, 1.0));
       const double adi = a * di;
@@ -107,42 +116,32 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
   constexpr int NCOMP = EL ? 2 : 1;
   constexpr int MT = (NCOMP * GE::ROWS + 7) / 8;
   constexpr int S = GE::aoStride(NCOMP);
-  double acc[MT][NT][2];
-#pragma unroll
-  for (int m = 0; m < MT; ++m)
-#pragma unroll
-    for (int t = 0; t < NT; ++t) acc[m][t][0] = acc[m][t][1] = 0.0;
   double ven = 0.0;
   {
-    double *tile = ws;  // overlays the scratch from offset 0 (all dead here except sXYZ, read above)
+#if !QMC_PARK_ACC
+    double acc[MT][NT][2];
+#pragma unroll
+    for (int m = 0; m < MT; ++m)
+#pragma unroll
+      for (int t = 0; t < NT; ++t) acc[m][t][0] = acc[m][t][1] = 0.0;
+#endif
+    double *accst = ws;  // overlays the scratch from offset 0 (all dead here except sXYZ, read above)
+    double *tile = ws + (QMC_PARK_ACC ? GE::accDoubles(NCOMP) : 0);
     __syncwarp();       // every lane is done with sXYZ
     const int fr = lane >> 2, fk = lane & 3;  // fragment row / k of this lane
     int cur_atom = -1, chunk = 0;
     double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1.0, r = 1.0, ri = 1.0, gd = 0.0;
-    auto put = [&](int row, double phi, double bop) {
+    double *const tl = tile + lane;  // this lane's column of the tile
+    auto put = [&](double *trow, int t, double phi, double bop) {
       if (active) {
-        tile[row * S + lane] = phi;
-        if (EL) tile[row * S + GE::ROWS + lane] = bop;
+        trow[t * S] = phi;
+        if (EL) trow[t * S + GE::ROWS] = bop;
       }
     };
-    ShellRec nxt = sShell[0];
-    for (int s = 0; s < P.n_shell; ++s) {
-      const ShellRec sh = nxt;
-      nxt = sShell[s + 1];  // one padding record follows the table
-      if (sh.atom != cur_atom) {
-        cur_atom = sh.atom;
-        dx = x - P.atom[cur_atom][0];
-        dy = y - P.atom[cur_atom][1];
-        dz = z - P.atom[cur_atom][2];
-        r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-        ri = rsqrt_fast(r2);
-        r = r2 * ri;
-        if (EL) {
-          ven = fma(-P.atom[cur_atom][3], ri, ven);
-          gd = fma(gJx, dx, fma(gJy, dy, gJz * dz)) * ri;  // grad J . d / r
-        }
-      }
-      const double ex = exp_neg(-sh.zeta * r);
+    // one record: angular factors, the combined operator, stores into the tile, and -- on the last
+    // record of a chunk -- the DMMA pass over the chunk
+    auto process = [&](const ShellRec &sh, const double ex) {
+      if (sh.kind == SH_NULL) return;
       const int k = sh.k;
       const double gr = (k == 0) ? ex : ((k == 1) ? ex * r : ((k == 2) ? ex * r2 : ex * r2 * r));
       double h = 0.0;
@@ -152,35 +151,35 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
         const double radlog = fma((double)k, ri, -sh.zeta);  // g'/g
         h = fma(-0.5, lapfac, -radlog * gd);
       }
-      const int row = sh.ao0 & (kChunk - 1);
+      double *const tr = tl + (sh.ao0 & (kChunk - 1)) * S;
       switch (sh.kind) {
         case SH_S: {
-          put(row, gr, gr * h);
+          put(tr, 0, gr, gr * h);
         } break;
         case SH_P: {
-          put(row, gr * dx, gr * fma(dx, h, -gJx));
-          put(row + 1, gr * dy, gr * fma(dy, h, -gJy));
-          put(row + 2, gr * dz, gr * fma(dz, h, -gJz));
+          put(tr, 0, gr * dx, gr * fma(dx, h, -gJx));
+          put(tr, 1, gr * dy, gr * fma(dy, h, -gJy));
+          put(tr, 2, gr * dz, gr * fma(dz, h, -gJz));
         } break;
         case SH_D: {
           double Sh, gs;
           Sh = dx * dy; gs = fma(gJx, dy, gJy * dx);
-          put(row, gr * Sh, gr * fma(Sh, h, -gs));
+          put(tr, 0, gr * Sh, gr * fma(Sh, h, -gs));
           Sh = dy * dz; gs = fma(gJy, dz, gJz * dy);
-          put(row + 1, gr * Sh, gr * fma(Sh, h, -gs));
+          put(tr, 1, gr * Sh, gr * fma(Sh, h, -gs));
           Sh = dz * dx; gs = fma(gJz, dx, gJx * dz);
-          put(row + 2, gr * Sh, gr * fma(Sh, h, -gs));
+          put(tr, 2, gr * Sh, gr * fma(Sh, h, -gs));
           Sh = fma(dx, dx, -dy * dy); gs = 2.0 * fma(gJx, dx, -gJy * dy);
-          put(row + 3, gr * Sh, gr * fma(Sh, h, -gs));
+          put(tr, 3, gr * Sh, gr * fma(Sh, h, -gs));
           Sh = fma(2.0 * dz, dz, -fma(dx, dx, dy * dy));
           gs = 2.0 * fma(2.0 * gJz, dz, -fma(gJx, dx, gJy * dy));
-          put(row + 4, gr * Sh, gr * fma(Sh, h, -gs));
+          put(tr, 4, gr * Sh, gr * fma(Sh, h, -gs));
         } break;
         case SH_P1: {
           const int m = sh.m;
           const double Sh = (m == 0) ? dx : ((m == 1) ? dy : dz);
           const double gs = (m == 0) ? gJx : ((m == 1) ? gJy : gJz);
-          put(row, gr * Sh, gr * fma(Sh, h, -gs));
+          put(tr, 0, gr * Sh, gr * fma(Sh, h, -gs));
         } break;
         default: {  // SH_D1
           const int m = sh.m;
@@ -190,16 +189,35 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
           else if (m == 2) { Sh = dz * dx; gs = fma(gJz, dx, gJx * dz); }
           else if (m == 3) { Sh = fma(dx, dx, -dy * dy); gs = 2.0 * fma(gJx, dx, -gJy * dy); }
           else { Sh = fma(2.0 * dz, dz, -fma(dx, dx, dy * dy)); gs = 2.0 * fma(2.0 * gJz, dz, -fma(gJx, dx, gJy * dy)); }
-          put(row, gr * Sh, gr * fma(Sh, h, -gs));
+          put(tr, 0, gr * Sh, gr * fma(Sh, h, -gs));
         } break;
       }
       if (sh.flush) {
         // unused rows of the chunk meet zero rows of C, but must themselves be finite
-        for (int pr = sh.flush; pr < kChunk; ++pr) put(pr, 0.0, 0.0);
+        for (int pr = sh.flush; pr < kChunk; ++pr) put(tl + pr * S, 0, 0.0, 0.0);
         __syncwarp();
-        const double *cf = sC + chunk * (4 * NT * 32) + lane;
+#if QMC_PARK_ACC
+        double acc[MT][NT][2];
+        double2 *ast = reinterpret_cast<double2 *>(accst) + lane;
+        if (chunk == 0) {
 #pragma unroll
-        for (int ks = 0; ks < 4; ++ks) {
+          for (int m = 0; m < MT; ++m)
+#pragma unroll
+            for (int t = 0; t < NT; ++t) acc[m][t][0] = acc[m][t][1] = 0.0;
+        } else {
+#pragma unroll
+          for (int m = 0; m < MT; ++m)
+#pragma unroll
+            for (int t = 0; t < NT; ++t) {
+              const double2 v = ast[(m * NT + t) * 32];
+              acc[m][t][0] = v.x;
+              acc[m][t][1] = v.y;
+            }
+        }
+#endif
+        const double *cf = sC + chunk * ((kChunk / 4) * NT * 32) + lane;
+#pragma unroll
+        for (int ks = 0; ks < kChunk / 4; ++ks) {
           double bf[NT];
 #pragma unroll
           for (int t = 0; t < NT; ++t) bf[t] = cf[(ks * NT + t) * 32];
@@ -211,24 +229,60 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
             for (int t = 0; t < NT; ++t) dmma884(acc[m][t][0], acc[m][t][1], a, bf[t]);
           }
         }
-        __syncwarp();
         ++chunk;
+        if (chunk < P.n_chunks) {
+#if QMC_PARK_ACC
+#pragma unroll
+          for (int m = 0; m < MT; ++m)
+#pragma unroll
+            for (int t = 0; t < NT; ++t) ast[(m * NT + t) * 32] = make_double2(acc[m][t][0], acc[m][t][1]);
+#endif
+        } else {
+          __syncwarp();  // the tile and the parked accumulators are dead: the MO rows overlay them
+          // D fragments -> MO rows: lane holds D[8 m + fr][8 t + 2 fk + {0,1}]
+#pragma unroll
+          for (int m = 0; m < MT; ++m) {
+            const int R = 8 * m + fr;
+            const bool isB = EL && (R >= GE::ROWS);
+            const int el = isB ? R - GE::ROWS : R;
+            double *dst = (isB ? sB : sPhi) + el * NMO;
+            if (el < G * ne && R < NCOMP * GE::ROWS) {
+#pragma unroll
+              for (int t = 0; t < NT; ++t) {
+                const int col = 8 * t + 2 * fk;
+                if (col < NMO) *reinterpret_cast<double2 *>(dst + col) = make_double2(acc[m][t][0], acc[m][t][1]);
+              }
+            }
+          }
+        }
+        __syncwarp();
       }
-    }
-    // D fragments -> MO rows: lane holds D[8 m + fr][8 t + 2 fk + {0,1}]
+    };
+    // Records come in groups of four that share a centre (the host pads with SH_NULL records): the four
+    // exponentials are independent chains the scheduler can interleave.
+    for (int s = 0; s < P.n_shell; s += QMC_SHELL_UNROLL) {
+      ShellRec q[QMC_SHELL_UNROLL];
 #pragma unroll
-    for (int m = 0; m < MT; ++m) {
-      const int R = 8 * m + fr;
-      const bool isB = EL && (R >= GE::ROWS);
-      const int el = isB ? R - GE::ROWS : R;
-      double *dst = (isB ? sB : sPhi) + el * NMO;
-      if (el < G * ne && R < NCOMP * GE::ROWS) {
-#pragma unroll
-        for (int t = 0; t < NT; ++t) {
-          const int col = 8 * t + 2 * fk;
-          if (col < NMO) *reinterpret_cast<double2 *>(dst + col) = make_double2(acc[m][t][0], acc[m][t][1]);
+      for (int u = 0; u < QMC_SHELL_UNROLL; ++u) q[u] = sShell[s + u];
+      const ShellRec &q0 = q[0];
+      if (q0.atom != cur_atom) {
+        cur_atom = q0.atom;
+        dx = x - P.atom[cur_atom][0];
+        dy = y - P.atom[cur_atom][1];
+        dz = z - P.atom[cur_atom][2];
+        r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+        ri = rsqrt_fast(r2);
+        r = r2 * ri;
+        if (EL) {
+          ven = fma(-P.atom[cur_atom][3], ri, ven);
+          gd = fma(gJx, dx, fma(gJy, dy, gJz * dz)) * ri;  // grad J . d / r
         }
       }
+      double ex[QMC_SHELL_UNROLL];
+#pragma unroll
+      for (int u = 0; u < QMC_SHELL_UNROLL; ++u) ex[u] = exp_neg(-q[u].zeta * r);
+#pragma unroll
+      for (int u = 0; u < QMC_SHELL_UNROLL; ++u) process(q[u], ex[u]);
     }
   }
   {
@@ -248,7 +302,7 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
       const int pr = pass * PP + slot;
       const bool pvalid = pr < nprob;
       const int pg = pvalid ? (pr >> 1) : 0, sp = pr & 1;
-      const int ns = sp ? P.n_dn : P.n_up, nv = P.nv[sp], e0 = sp ? P.n_up : 0;
+      const int ns = sp ? n_dn : n_up, nv = P.nv[sp], e0 = sp ? n_up : 0;
       double a0[NS], av[NS], b0[EL ? NS : 1], bv[EL ? NS : 1];
       {
         const bool cA = c < ns, cV = c < nv;
@@ -276,6 +330,9 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
 #pragma unroll
       for (int k = 0; k < NS; ++k) {
         // 32-bit monotone key of |a0[k]| with the lane index in the low bits: unique arg-max
+#if QMC_EARLY_INV
+        const double myinv = rcp_fast(a0[k]);  // off the critical path: overlaps the arg-max shuffles
+#endif
         unsigned key = used ? 0u : (((unsigned)(__double2hiint(a0[k]) & 0x7fffffff) & ~(unsigned)(LP - 1)) | (unsigned)c);
 #pragma unroll
         for (int m = 1; m < LP; m <<= 1) key = max(key, __shfl_xor_sync(0xffffffffu, key, m));
@@ -286,7 +343,11 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
 #pragma unroll
         for (int i = 0; i < NS; ++i) f[i] = __shfl_sync(0xffffffffu, a0[i], gbase + pl);
         const double piv = f[k];
+#if QMC_EARLY_INV
+        const double inv = shfl_d(myinv, gbase + pl, 32);
+#else
         const double inv = rcp_fast(piv);
+#endif
         det *= piv;
         {
           double t = a0[k] * inv;
@@ -344,15 +405,16 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
       if (pvalid) {
 #pragma unroll
         for (int k = 0; k < NS; ++k) {
-          sT[pr * TS + perm[k] * LP + c] = av[k];
-          if (EL) sM[pr * TS + perm[k] * LP + c] = bv[k];
+          if (EL) reinterpret_cast<double2 *>(sT)[pr * TS + perm[k] * LP + c] = make_double2(av[k], bv[EL ? k : 0]);
+          else sT[pr * TS + perm[k] * LP + c] = av[k];
         }
         if (c == 0) {
-          sT[pr * TS + NS * LP] = 1.0;
-          sT[pr * TS + NS * LP + 1] = 0.0;
           if (EL) {
-            sM[pr * TS + NS * LP] = 0.0;
-            sM[pr * TS + NS * LP + 1] = 0.0;
+            reinterpret_cast<double2 *>(sT)[pr * TS + NS * LP] = make_double2(1.0, 0.0);
+            reinterpret_cast<double2 *>(sT)[pr * TS + NS * LP + 1] = make_double2(0.0, 0.0);
+          } else {
+            sT[pr * TS + NS * LP] = 1.0;
+            sT[pr * TS + NS * LP + 1] = 0.0;
           }
           sProb[pr * 4 + 0] = log(fabs(det));
           sProb[pr * 4 + 1] = (det > 0.0) ? 1.0 : ((det < 0.0) ? -1.0 : 0.0);
@@ -370,15 +432,14 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
     const int wg = lane / LW, sub = lane - wg * LW;
     const bool wvalid = wg < G;
     const int pu = 2 * (wvalid ? wg : 0), pd = pu + 1;
-    const double *Tu = sT + pu * TS, *Td = sT + pd * TS;
-    const double *Mu = sM + pu * TS, *Md = sM + pd * TS;
+    const double *Tu = sT + (EL ? 2 : 1) * pu * TS, *Td = sT + (EL ? 2 : 1) * pd * TS;
     double den = 0.0, num = 0.0;
     // determinants with at most one substitution per spin: one table entry per spin
     for (int n = sub; n < P.n_det_single; n += LW) {
       const DetRec dr = sDet[n];
       double Ru, Du, Rd, Dd;
-      excite_single<EL>(dr.up, Tu, Mu, Ru, Du);
-      excite_single<EL>(dr.dn, Td, Md, Rd, Dd);
+      excite_single<EL>(dr.up, Tu, Ru, Du);
+      excite_single<EL>(dr.dn, Td, Rd, Dd);
       const double w = dr.d * Ru;
       den = fma(w, Rd, den);
       if (EL) num = fma(dr.d, Du * Rd, fma(w, Dd, num));
@@ -387,8 +448,8 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
     for (int n = P.n_det_single + sub; n < P.n_det; n += LW) {
       const DetRec dr = sDet[n];
       double Ru, Du, Rd, Dd;
-      excite_double<EL>(dr.up, Tu, Mu, Ru, Du);
-      excite_double<EL>(dr.dn, Td, Md, Rd, Dd);
+      excite_double<EL>(dr.up, Tu, Ru, Du);
+      excite_double<EL>(dr.dn, Td, Rd, Dd);
       const double w = dr.d * Ru;
       den = fma(w, Rd, den);
       if (EL) num = fma(dr.d, Du * Rd, fma(w, Dd, num));

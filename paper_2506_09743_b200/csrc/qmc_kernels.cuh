@@ -16,9 +16,9 @@ __device__ __forceinline__ void load_constants(const SysParams &P, unsigned char
   {
     const double *src = reinterpret_cast<const double *>(P.shells);
     double *dst = reinterpret_cast<double *>(sh);
-    for (int i = threadIdx.x; i < (P.n_shell + 1) * 4; i += blockDim.x) dst[i] = src[i];
+    for (int i = threadIdx.x; i < P.n_shell * 4; i += blockDim.x) dst[i] = src[i];
   }
-  DetRec *dt = reinterpret_cast<DetRec *>(sh + P.n_shell + 1);
+  DetRec *dt = reinterpret_cast<DetRec *>(sh + P.n_shell);
   {
     const double *src = reinterpret_cast<const double *>(P.dets);
     double *dst = reinterpret_cast<double *>(dt);
@@ -38,8 +38,8 @@ __device__ __forceinline__ void dummy_xyz(int lane, double &x, double &y, double
   z = 0.53 - 0.05 * lane;
 }
 
-template <int NS, int NMO, bool EL>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32, 2)
+template <int NS, int NMO, bool EL, bool X>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
     local_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
   const double *sC;
@@ -50,11 +50,10 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, 2)
   using GE = Geo<NS, NMO>;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   double *ws = wsBase + warp * GE::total;
-  const int ne = P.n_e, G = P.G;
+  const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
   const int g = lane / ne, e = lane - g * ne;
   const int64_t n_groups = (io.M + G - 1) / G;
   const int64_t stride = (int64_t)gridDim.x * kWarpsPerBlock;
-  // the coordinates of the next group are fetched while the current one is evaluated
   auto fetch = [&](int64_t grp, double &x, double &y, double &z) {
     const int64_t w = grp * G + g;
     if ((g < G) && (w < io.M)) {
@@ -65,13 +64,10 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, 2)
       dummy_xyz(lane, x, y, z);
     }
   };
-  int64_t grp = (int64_t)blockIdx.x * kWarpsPerBlock + warp;
-  double nx, ny, nz;
-  fetch(grp, nx, ny, nz);
-  for (; grp < n_groups; grp += stride) {
-    const double x = nx, y = ny, z = nz;
-    fetch(grp + stride, nx, ny, nz);
-    eval_walkers<NS, NMO, EL>(P, sShell, sC, sDet, ws, x, y, z, lane);
+  for (int64_t grp = (int64_t)blockIdx.x * kWarpsPerBlock + warp; grp < n_groups; grp += stride) {
+    double x, y, z;
+    fetch(grp, x, y, z);
+    eval_walkers<NS, NMO, EL, X>(P, sShell, sC, sDet, ws, x, y, z, lane);
     if (lane < G) {
       const int64_t wo = grp * G + lane;
       if (wo < io.M) {
@@ -89,8 +85,8 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, 2)
 // Persistent all-electron Metropolis (readings Q9, Q10).
 // Walker coordinates and log|Psi| stay in registers for all sweeps.
 // ---------------------------------------------------------------------------------
-template <int NS, int NMO, bool WITH_EL>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32, 2)
+template <int NS, int NMO, bool WITH_EL, bool X>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
     metropolis_kernel(const __grid_constant__ SysParams P, const WalkerIO io, const MetroParams mp) {
   extern __shared__ __align__(16) unsigned char smem[];
   const double *sC;
@@ -104,7 +100,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, 2)
   double *sProp = ws + GE::oProp;       // [G][3 ne] normals
   double *sLogU = sProp + 96;           // [G]
   const double *sRes = ws + GE::oRes;
-  const int ne = P.n_e, G = P.G, nc = 3 * ne, npair = (nc + 1) / 2;
+  const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G, nc = 3 * ne, npair = (nc + 1) / 2;
   const int g = lane / ne, e = lane - g * ne;
   const int64_t n_groups = (io.M + G - 1) / G;
   const int64_t stride = (int64_t)gridDim.x * kWarpsPerBlock;
@@ -154,7 +150,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, 2)
         logu = sLogU[own ? g : 0];
         __syncwarp();
       }
-      eval_walkers<NS, NMO, false>(P, sShell, sC, sDet, ws, xp, yp, zp, lane);
+      eval_walkers<NS, NMO, false, X>(P, sShell, sC, sDet, ws, xp, yp, zp, lane);
       const double lp2 = sRes[rg + 0], sg2 = sRes[rg + 1];
       // accept iff log u < 2 (log|Psi'| - log|Psi|): false for NaN and for Psi' = 0
       const bool ok = (sw < 0) || (own && (logu < 2.0 * (lp2 - lp)));
@@ -165,7 +161,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, 2)
       }
       __syncwarp();
       if (WITH_EL && sw >= 0) {
-        eval_walkers<NS, NMO, true>(P, sShell, sC, sDet, ws, x, y, z, lane);
+        eval_walkers<NS, NMO, true, X>(P, sShell, sC, sDet, ws, x, y, z, lane);
         eacc += sRes[rg + 2];
         __syncwarp();
       }
