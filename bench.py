@@ -145,6 +145,7 @@ def main():
     import torch.distributed as dist
     from paper_2506_09743_b200 import binding as qb
     from paper_2506_09743_b200 import workloads as wl
+    from paper_2506_09743_b200.sharding import max_over_ranks
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -230,10 +231,7 @@ def main():
     t_e2e = a.elapsed_time(b) * 1e-3
     clocks = sampler.stop()
 
-    times = torch.tensor([t_met, t_el, t_all, t_e2e], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    t_met, t_el, t_all, t_e2e = (float(x) for x in times.cpu())
+    t_met, t_el, t_all, t_e2e = max_over_ranks([t_met, t_el, t_all, t_e2e], device=dev)
 
     K = args.steps
     el_rate = world * M * K / t_el
