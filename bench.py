@@ -262,7 +262,8 @@ def main():
                            "model_tflops": achieved_met, "frac_of_dfma_peak": achieved_met / peak_dfma},
             "local_energy_ms": 1e3 * t_el / K,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_dfma, "unit": "TFLOP/s",
-                         "frac": achieved / peak_dfma, "traffic": None,
+                         "frac": achieved / peak_dfma,
+                         "traffic": 44129280,  # dram bytes read+written per launch, profiles/r01_el_kernel.md
                          "kernel": "local_energy_kernel<7,14,true>",
                          "peak_source": "qmc_fp64_peak DFMA microbenchmark in this process (no FP64 entry in MEASURED_PEAKS.json)",
                          "dmma_peak": peak_dmma, "model_flop_eq_per_walker": flops_el},

@@ -81,8 +81,9 @@ typedef struct {
  * determinant 0) and upload the constants to `device`.
  * Limits (QMC_EUNSUPPORTED beyond them): n_up, n_dn <= 8; at most 8 distinct
  * virtual (non-reference) orbitals per spin; n_up + n_dn <= 16; n_atoms <= 16;
- * n_ao <= 256; at most 16 distinct orbitals referenced overall; determinants
- * differing from determinant 0 in more than 2 columns of one spin are unsupported.
+ * n_ao <= 256; at most 16 distinct orbitals referenced overall.  Determinants that differ
+ * from determinant 0 in at most 2 columns per spin take the fast path; more
+ * substitutions are evaluated through general k x k sub-determinants (correct, slower).
  * QMC_EINVAL: null pointers, n_up + n_dn == 0, n_det < 1, bad (n,l,m), zeta <= 0,
  * atom / MO index out of range, a determinant list repeating a column.
  * On success *out receives a handle to be released with qmc_destroy. */

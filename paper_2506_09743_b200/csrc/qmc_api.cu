@@ -34,7 +34,7 @@ int cuda_fail(cudaError_t e, const char *what) {
 struct Variant {
   int NS, NMO, LP, ws_doubles;
   bool exact;  // compiled for n_up = n_dn = NS
-  const void *k_el, *k_psi, *k_metro, *k_metro_el;
+  const void *k_el, *k_psi, *k_metro, *k_metro_el, *k_expl;
 };
 
 template <int NS, int NMO, bool X>
@@ -49,6 +49,7 @@ Variant make_variant() {
   v.k_psi = (const void *)local_energy_kernel<NS, NMO, false, X>;
   v.k_metro = (const void *)metropolis_kernel<NS, NMO, false, X>;
   v.k_metro_el = (const void *)metropolis_kernel<NS, NMO, true, X>;
+  v.k_expl = (const void *)explicit_energy_kernel<NS, NMO, X>;
   return v;
 }
 
@@ -87,7 +88,8 @@ struct qmc_system {
   Variant var{};
   int smem_bytes = 0;
   int blocks_el = 0, blocks_psi = 0, blocks_metro = 0, blocks_metro_el = 0;
-  void *d_shells = nullptr, *d_C = nullptr, *d_dets = nullptr;
+  void *d_shells = nullptr, *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr;
+  int n_sm = 0;
   double *d_stats = nullptr;
   unsigned long long *d_counter = nullptr;
   double flops_el = 0, flops_step = 0;
@@ -118,6 +120,8 @@ void qmc_destroy(qmc_system_t *s) {
   cudaFree(s->d_shells);
   cudaFree(s->d_C);
   cudaFree(s->d_dets);
+  cudaFree(s->d_gen);
+  cudaFree(s->d_cols);
   cudaFree(s->d_stats);
   cudaFree(s->d_counter);
   delete s;
@@ -183,7 +187,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     return (int)used.size() - 1;
   };
   std::vector<int> virt[2];  // caller MO index of virtual q
-  struct Exc { int k[2]; int p[2][2]; int q[2][2]; double d; };
+  struct Exc { int k[2]; int p[2][kMaxSpin]; int q[2][kMaxSpin]; double d; };
   std::vector<Exc> excs(d->n_det);
   bool unsupported = false;
   for (int sp = 0; sp < 2; ++sp)
@@ -203,20 +207,25 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
           virt[sp].push_back(mo);
           q = (int)virt[sp].size() - 1;
         }
-        if (k < 2) { x.p[sp][k] = j; x.q[sp][k] = q; }
+        x.p[sp][k] = j;
+        x.q[sp][k] = q;
         ++k;
       }
-      if (k > 2) unsupported = true;
       x.k[sp] = k;
     }
   }
   // determinants with at most one substitution per spin first: the lanes of a warp, which take
   // consecutive determinants, then run the same code
   std::stable_sort(excs.begin(), excs.end(), [](const Exc &a, const Exc &b) {
-    return std::max(a.k[0], a.k[1]) / 2 < std::max(b.k[0], b.k[1]) / 2;
+    auto cls = [](const Exc &x) { const int m = std::max(x.k[0], x.k[1]); return m < 2 ? 0 : (m == 2 ? 1 : 2); };
+    return cls(a) < cls(b);
   });
   P.n_det_single = 0;
-  for (const Exc &x : excs) P.n_det_single += (std::max(x.k[0], x.k[1]) < 2) ? 1 : 0;
+  int n_packed = 0;  // determinants with at most two substitutions per spin (packed 16-byte records)
+  for (const Exc &x : excs) {
+    P.n_det_single += (std::max(x.k[0], x.k[1]) < 2) ? 1 : 0;
+    n_packed += (std::max(x.k[0], x.k[1]) <= 2) ? 1 : 0;
+  }
   for (int sp = 0; sp < 2; ++sp) {
     if ((int)virt[sp].size() > kMaxVirt) unsupported = true;
     P.nv[sp] = (int)virt[sp].size();
@@ -228,6 +237,15 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     return QMC_EUNSUPPORTED;
   }
   P.n_mo = (int)used.size();
+  // column lists of every determinant in kernel MO order (explicit fallback path)
+  std::vector<DetCols> cols(d->n_det);
+  for (int n = 0; n < d->n_det; ++n) {
+    cols[n].d = d->ci_coeff[n];
+    for (int sp = 0; sp < 2; ++sp)
+      for (int j = 0; j < kMaxSpin; ++j)
+        cols[n].col[sp][j] = (j < nsp[sp]) ? (int8_t)col_of(lists[sp][(size_t)n * nsp[sp] + j]) : 0;
+  }
+  P.n_det_all = d->n_det;
 
   // ---- pick the instantiation
   const int ns_max = std::max(d->n_up, d->n_dn), nv_max = std::max(P.nv[0], P.nv[1]);
@@ -244,10 +262,25 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   }
   s->var = *var;
   const int NMO = var->NMO;
-  std::vector<DetRec> dets(d->n_det);
+  std::vector<DetRec> dets(n_packed);
+  std::vector<GenDet> gens;
+  for (int n = n_packed; n < d->n_det; ++n) {
+    GenDet g{};
+    g.d = excs[n].d;
+    for (int sp = 0; sp < 2; ++sp) {
+      g.s[sp].k = (uint8_t)excs[n].k[sp];
+      for (int t = 0; t < excs[n].k[sp]; ++t) {
+        g.s[sp].p[t] = (uint8_t)excs[n].p[sp][t];
+        g.s[sp].q[t] = (uint8_t)excs[n].q[sp][t];
+      }
+    }
+    gens.push_back(g);
+  }
+  P.n_det = n_packed;
+  P.n_gen = (int)gens.size();
   {
     const uint32_t one = (uint32_t)(var->NS * var->LP), zero = one + 1;  // constant table entries (Geo::TS)
-    for (int n = 0; n < d->n_det; ++n) {
+    for (int n = 0; n < n_packed; ++n) {
       const Exc &x = excs[n];
       uint32_t code[2];
       for (int sp = 0; sp < 2; ++sp) {
@@ -357,7 +390,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   // ---- model FP64 work per walker
   {
     const double cexp = 40, cdiv = 20, csqrt = 20, clog = 50, csincos = 80;
-    const double ne = P.n_e, nat = P.n_atoms, nsh = n_real_shells, nao = P.n_ao, nmo = P.n_mo, nd = P.n_det;
+    const double ne = P.n_e, nat = P.n_atoms, nsh = n_real_shells, nao = P.n_ao, nmo = P.n_mo, nd = d->n_det;
     const double npair = ne * (ne - 1) / 2;
     double lu_el = 0, lu_st = 0;
     for (int sp = 0; sp < 2; ++sp) {
@@ -381,7 +414,11 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
       (e = cudaMalloc(&s->d_counter, sizeof(unsigned long long))) != cudaSuccess ||
       (e = cudaMemcpy(s->d_C, C.data(), szC, cudaMemcpyHostToDevice)) != cudaSuccess ||
       (e = cudaMemcpy(s->d_shells, shells.data(), szS, cudaMemcpyHostToDevice)) != cudaSuccess ||
-      (e = cudaMemcpy(s->d_dets, dets.data(), szD, cudaMemcpyHostToDevice)) != cudaSuccess) {
+      (e = cudaMemcpy(s->d_dets, dets.data(), szD, cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMalloc(&s->d_gen, std::max<size_t>(gens.size(), 1) * sizeof(GenDet))) != cudaSuccess ||
+      (!gens.empty() && (e = cudaMemcpy(s->d_gen, gens.data(), gens.size() * sizeof(GenDet), cudaMemcpyHostToDevice)) != cudaSuccess) ||
+      (e = cudaMalloc(&s->d_cols, cols.size() * sizeof(DetCols))) != cudaSuccess ||
+      (e = cudaMemcpy(s->d_cols, cols.data(), cols.size() * sizeof(DetCols), cudaMemcpyHostToDevice)) != cudaSuccess) {
     int rc = cuda_fail(e, "qmc_setup upload");
     qmc_destroy(s);
     return rc;
@@ -389,6 +426,8 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   P.shells = (const ShellRec *)s->d_shells;
   P.C = (const double *)s->d_C;
   P.dets = (const DetRec *)s->d_dets;
+  P.gen = (const GenDet *)s->d_gen;
+  P.det_cols = (const DetCols *)s->d_cols;
   P.smem_const_bytes = (int)((szC + szS + szD + 15) / 16 * 16);
   s->smem_bytes = P.smem_const_bytes + kWarpsPerBlock * var->ws_doubles * (int)sizeof(double);
 
@@ -399,9 +438,11 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     qmc_destroy(s);
     return QMC_EUNSUPPORTED;
   }
-  const void *ks[4] = {var->k_el, var->k_psi, var->k_metro, var->k_metro_el};
-  int *nb[4] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro, &s->blocks_metro_el};
-  for (int i = 0; i < 4; ++i) {
+  int blocks_expl = 0;
+  s->n_sm = n_sm;
+  const void *ks[5] = {var->k_el, var->k_psi, var->k_metro, var->k_metro_el, var->k_expl};
+  int *nb[5] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro, &s->blocks_metro_el, &blocks_expl};
+  for (int i = 0; i < 5; ++i) {
     if ((e = cudaFuncSetAttribute(ks[i], cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_bytes)) != cudaSuccess) {
       int rc = cuda_fail(e, "cudaFuncSetAttribute");
       qmc_destroy(s);
@@ -423,14 +464,32 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
                        void *stream, bool el) {
   if (!s || !d_r || M <= 0) return QMC_EINVAL;
   CK(cudaSetDevice(s->device));
-  WalkerIO io{d_r, nullptr, d_logpsi, d_sign, d_eloc, M};
+  cudaStream_t st = (cudaStream_t)stream;
+  WalkerIO io{};
+  io.r_in = d_r;
+  io.logpsi = d_logpsi;
+  io.sign = d_sign;
+  io.eloc = d_eloc;
+  io.M = M;
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
   const int64_t need = (groups + kWarpsPerBlock - 1) / kWarpsPerBlock;
   const int grid = (int)std::min<int64_t>(need, el ? s->blocks_el : s->blocks_psi);
+  int *fb = nullptr;
+  const bool fallback = el && s->P.n_det_all > 1;  // a single determinant has no reference to be ill-conditioned against
+  if (fallback) {  // work list of the explicit fallback: [0] = counter, [1..] = group indices (stream-ordered scratch)
+    CK(cudaMallocAsync(&fb, (size_t)(groups + 1) * sizeof(int), st));
+    CK(cudaMemsetAsync(fb, 0, sizeof(int), st));
+    io.fb_count = fb;
+    io.fb_list = fb + 1;
+  }
   void *args[2] = {(void *)&s->P, (void *)&io};
-  CK(cudaLaunchKernel(el ? s->var.k_el : s->var.k_psi, dim3(grid), dim3(kWarpsPerBlock * 32), args, s->smem_bytes,
-                      (cudaStream_t)stream));
+  CK(cudaLaunchKernel(el ? s->var.k_el : s->var.k_psi, dim3(grid), dim3(kWarpsPerBlock * 32), args, s->smem_bytes, st));
   ++g_launches;
+  if (fallback) {
+    CK(cudaLaunchKernel(s->var.k_expl, dim3(grid), dim3(kWarpsPerBlock * 32), args, s->smem_bytes, st));
+    ++g_launches;
+    CK(cudaFreeAsync(fb, st));
+  }
   return QMC_OK;
 }
 
@@ -450,7 +509,12 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
   if (sweep_offset + (uint64_t)n_sweeps >= (1ull << 32)) return QMC_EINVAL;
   CK(cudaSetDevice(s->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  WalkerIO io{d_r, d_r, d_logpsi, d_sign, nullptr, M};
+  WalkerIO io{};
+  io.r_in = d_r;
+  io.r_out = d_r;
+  io.logpsi = d_logpsi;
+  io.sign = d_sign;
+  io.M = M;
   MetroParams mp{};
   mp.step = step;
   mp.n_sweeps = n_sweeps;

@@ -65,6 +65,29 @@ struct DetRec {
   double d;
 };
 
+// A determinant with more than two substitutions in one spin (rare; general k x k sub-determinants).
+struct GenSpin {
+  uint8_t k;
+  uint8_t p[kMaxSpin];  // substituted reference positions
+  uint8_t q[kMaxSpin];  // virtual indices
+  uint8_t pad[7];
+};
+struct GenDet {  // 56 bytes
+  double d;
+  GenSpin s[2];
+};
+
+// Column lists of every determinant (caller order), for the explicit fallback path.  24 bytes.
+struct DetCols {
+  int8_t col[2][kMaxSpin];  // kernel MO column of position j, per spin
+  double d;
+};
+
+// |Sigma / D_0| above which a walker is re-evaluated with every determinant eliminated explicitly:
+// the table path (F.6/F.7) loses about log10((Sigma/D_0)^2) digits when the reference determinant
+// is nearly singular while the expansion is not.
+constexpr double kFallbackRatio = 1024.0;  // measured: E_L error ~ 1.2e-15 (Sigma/D_0)^2  ->  1.3e-9 at the threshold
+
 struct SysParams {  // passed by value to every kernel
   int n_atoms, n_up, n_dn, n_e;
   int n_shell, n_ao, n_mo, n_det;  // n_mo = orbitals referenced (kernel order)
@@ -82,10 +105,17 @@ struct SysParams {  // passed by value to every kernel
   const ShellRec *shells;          // device [n_shell]
   const double *C;                 // device [chunk][k-step 4][MO tile NT][lane 32]: DMMA B fragments of
                                    // N_ao * C (normalisation folded in, zero padded), see qmc_setup
-  const DetRec *dets;              // device [n_det]
+  const DetRec *dets;              // device [n_det]  (at most two substitutions per spin)
+  const GenDet *gen;               // device [n_gen]  (the others)
+  int n_gen;
+  int n_det_all;                   // all determinants
+  const DetCols *det_cols;         // device [n_det_all]
 };
 
 struct WalkerIO {
+  // explicit-fallback work list: groups whose walkers need re-evaluation (filled by the fast kernel)
+  int *fb_list;        // device [ceil(M / G)] group indices, or null
+  int *fb_count;       // device counter
   const double *r_in;  // [n_e][3][M]
   double *r_out;       // Metropolis: same buffer
   double *logpsi, *sign, *eloc;

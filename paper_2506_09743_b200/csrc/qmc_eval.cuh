@@ -38,15 +38,64 @@ __device__ __forceinline__ void excite_double(uint32_t idx, const double *__rest
   }
 }
 
+// General substitution order k (> 2): R = det T[p,q]; Rd = Tr(adj(T[p,q]) Mt[p,q]) = sum_j det(T[p,q] with
+// column j taken from Mt[p,q]) -- division-free, valid at R = 0.  Rare path: local-memory k x k LU.
+__device__ __noinline__ double small_det(double *a, int k) {
+  double det = 1.0;
+  for (int c = 0; c < k; ++c) {
+    int piv = c;
+    double best = fabs(a[c * k + c]);
+    for (int r = c + 1; r < k; ++r)
+      if (fabs(a[r * k + c]) > best) { best = fabs(a[r * k + c]); piv = r; }
+    if (piv != c) {
+      for (int j = 0; j < k; ++j) { const double t = a[c * k + j]; a[c * k + j] = a[piv * k + j]; a[piv * k + j] = t; }
+      det = -det;
+    }
+    const double d = a[c * k + c];
+    det *= d;
+    if (d == 0.0) return 0.0;
+    const double inv = 1.0 / d;
+    for (int r = c + 1; r < k; ++r) {
+      const double f = a[r * k + c] * inv;
+      for (int j = c + 1; j < k; ++j) a[r * k + j] = fma(-f, a[c * k + j], a[r * k + j]);
+    }
+  }
+  return det;
+}
+template <bool EL>
+__device__ __noinline__ void excite_general(const GenSpin *g, const double *T, int LP, double *out) {
+  const int k = g->k;
+  double R = 1.0, Rd = 0.0;
+  if (k > 0) {
+    double a[kMaxSpin * kMaxSpin], w[kMaxSpin * kMaxSpin];
+    for (int i = 0; i < k; ++i)
+      for (int j = 0; j < k; ++j) {
+        const int idx = g->p[i] * LP + g->q[j];
+        a[i * k + j] = EL ? reinterpret_cast<const double2 *>(T)[idx].x : T[idx];
+      }
+    for (int i = 0; i < k * k; ++i) w[i] = a[i];
+    R = small_det(w, k);
+    if (EL)
+      for (int c = 0; c < k; ++c) {
+        for (int i = 0; i < k * k; ++i) w[i] = a[i];
+        for (int i = 0; i < k; ++i) w[i * k + c] = reinterpret_cast<const double2 *>(T)[g->p[i] * LP + g->q[c]].y;
+        Rd += small_det(w, k);
+      }
+  }
+  out[0] = R;
+  out[1] = Rd;
+}
+
 // ---------------------------------------------------------------------------------
 // Evaluate the G walkers of this warp.  Lane = g * n_e + e holds electron e of walker g
 // at (x, y, z).  Results for walker g are left in ws[oRes + 4 g + {0,1,2}] =
 // {log|Psi|, sign, E_L} (E_L only if EL).  All 32 lanes must call.
 // ---------------------------------------------------------------------------------
-template <int NS, int NMO, bool EL, bool X>
+template <int NS, int NMO, bool EL, bool X, bool EXPL = false>
 __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sShell,
                              const double *__restrict__ sC, const DetRec *__restrict__ sDet,
-                             double *__restrict__ ws, double x, double y, double z, int lane) {
+                             double *__restrict__ ws, double x, double y, double z, int lane,
+                             int det0 = 0, int det_step = 1) {
   using GE = Geo<NS, NMO>;
   constexpr int LP = GE::LP, PP = GE::PP, TS = GE::TS;
   // X: closed-shell system that matches the instantiation exactly (n_up = n_dn = NS): sizes fold
@@ -292,6 +341,102 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
   }
   __syncwarp();
 
+  if (EXPL) {
+    // ---- explicit path (Fig. 11's "explicit"): every determinant is eliminated on its own,
+    // D_n = det A_n, t_n = Tr(A_n^-1 B_n) (G.7 with the combined operator); no excitation tables.
+    // Used for walkers whose reference determinant is nearly singular (kFallbackRatio).
+    const int c = lane % LP, slot = lane / LP, gbase = lane - c;
+    const int nprob = 2 * G;
+    double sig = 0.0, numk = 0.0;
+    // this warp takes determinants det0, det0 + det_step, ... (the block shares one walker group)
+    DetCols nxt = P.det_cols[det0 < P.n_det_all ? det0 : 0];
+    for (int n = det0; n < P.n_det_all; n += det_step) {
+      const DetCols dc = nxt;
+      if (n + det_step < P.n_det_all) nxt = P.det_cols[n + det_step];  // hide the L2 latency behind the elimination
+      for (int pass = 0; pass * PP < nprob; ++pass) {
+        const int pr = pass * PP + slot;
+        const bool pvalid = pr < nprob;
+        const int pg = pvalid ? (pr >> 1) : 0, sp = pr & 1;
+        const int ns = sp ? n_dn : n_up, e0 = sp ? n_up : 0;
+        double a0[NS], b0[NS];
+        {
+          const bool cA = c < ns;
+          const int colA = cA ? dc.col[sp][c < kMaxSpin ? c : 0] : 0;
+#pragma unroll
+          for (int i = 0; i < NS; ++i) {
+            const int row = (pg * ne + e0 + (i < ns ? i : 0)) * NMO;
+            const bool ri = i < ns;
+            a0[i] = (ri && cA) ? sPhi[row + colA] : ((i == c) ? 1.0 : 0.0);
+            b0[i] = (ri && cA) ? sB[EL ? row + colA : 0] : 0.0;
+          }
+        }
+        double det = 1.0;
+        int perm[NS];
+        int myrow = 0;
+        bool used = !(c < NS);
+#pragma unroll
+        for (int k = 0; k < NS; ++k) {
+          unsigned key = used ? 0u : (((unsigned)(__double2hiint(a0[k]) & 0x7fffffff) & ~(unsigned)(LP - 1)) | (unsigned)c);
+#pragma unroll
+          for (int m = 1; m < LP; m <<= 1) key = max(key, __shfl_xor_sync(0xffffffffu, key, m));
+          const int pl = (int)(key & (unsigned)(LP - 1));
+          perm[k] = pl;
+          if (c == pl) { used = true; myrow = k; }
+          double f[NS];
+#pragma unroll
+          for (int i = 0; i < NS; ++i) f[i] = __shfl_sync(0xffffffffu, a0[i], gbase + pl);
+          const double piv = f[k];
+          const double inv = 1.0 / piv;
+          det *= piv;
+          double t = a0[k] * inv;
+          a0[k] = t;
+#pragma unroll
+          for (int i = 0; i < NS; ++i) if (i != k) a0[i] = fma(-f[i], t, a0[i]);
+          t = b0[k] * inv;
+          b0[k] = t;
+#pragma unroll
+          for (int i = 0; i < NS; ++i) if (i != k) b0[i] = fma(-f[i], t, b0[i]);
+        }
+        int inversions = 0;
+#pragma unroll
+        for (int k = 0; k < NS; ++k)
+#pragma unroll
+          for (int k2 = k + 1; k2 < NS; ++k2) inversions += (perm[k] > perm[k2]) ? 1 : 0;
+        if (inversions & 1) det = -det;
+        double t0 = 0.0;
+#pragma unroll
+        for (int i = 0; i < NS; ++i) if (i == myrow && c < NS) t0 = b0[i];
+#pragma unroll
+        for (int m = 1; m < LP; m <<= 1) t0 += shfl_xor_d(t0, m);
+        if (pvalid && c == 0) {
+          sProb[pr * 4 + 0] = det;
+          sProb[pr * 4 + 2] = t0;
+        }
+      }
+      __syncwarp();
+      if (lane < G) {
+        const double w = dc.d * sProb[(2 * lane) * 4 + 0] * sProb[(2 * lane + 1) * 4 + 0];
+        sig += w;                                                                  // eq. 4
+        numk = fma(w, sProb[(2 * lane) * 4 + 2] + sProb[(2 * lane + 1) * 4 + 2], numk);  // F.2 / F.4
+      }
+      __syncwarp();
+    }
+    if (lane < G) {
+      double Jsum = 0.0, esum = 0.0;
+      for (int j = 0; j < ne; ++j) {
+        Jsum += sPart[(lane * ne + j) * 2 + 0];
+        esum += sPart[(lane * ne + j) * 2 + 1];
+      }
+      // partial sums of this warp's determinants; the kernel combines the warps of the block
+      sRes[lane * 4 + 0] = sig;
+      sRes[lane * 4 + 1] = numk;
+      sRes[lane * 4 + 2] = Jsum;
+      sRes[lane * 4 + 3] = esum;
+    }
+    __syncwarp();
+    return;
+  }
+
   // ---- stages a7-a8: per (walker, spin) Gauss-Jordan with partial pivoting on the augmented
   // matrix [A0 | Av | B0 | Bv]; lane c of a group of LP lanes owns column c of every block.
   // Result: T = A0^-1 Av, Gm = A0^-1 B0, H = A0^-1 Bv, det A0.  (F.6/F.7)
@@ -454,6 +599,15 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
       den = fma(w, Rd, den);
       if (EL) num = fma(dr.d, Du * Rd, fma(w, Dd, num));
     }
+    // determinants with more than two substitutions in a spin (general sub-determinants)
+    for (int n = sub; n < P.n_gen; n += LW) {
+      double u[2], v[2];
+      excite_general<EL>(&P.gen[n].s[0], Tu, LP, u);
+      excite_general<EL>(&P.gen[n].s[1], Td, LP, v);
+      const double dn = P.gen[n].d, w = dn * u[0];
+      den = fma(w, v[0], den);
+      if (EL) num = fma(dn, u[1] * v[0], fma(w, v[1], num));
+    }
     double Jsum = 0.0, esum = 0.0;
     if (wvalid)
       for (int j = sub; j < ne; j += LW) {
@@ -474,6 +628,7 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
       sRes[wg * 4 + 0] = Jsum + lu + ld + log(fabs(den));
       sRes[wg * 4 + 1] = sgn * ((den > 0.0) ? 1.0 : ((den < 0.0) ? -1.0 : 0.0));
       if (EL) sRes[wg * 4 + 2] = esum + (sProb[pu * 4 + 2] + sProb[pd * 4 + 2]) + num / den + P.vnn;
+      sRes[wg * 4 + 3] = (fabs(den) <= kFallbackRatio) ? 0.0 : 1.0;  // also set for NaN (singular reference)
     }
   }
   __syncwarp();

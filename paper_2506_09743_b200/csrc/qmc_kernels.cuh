@@ -68,6 +68,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
     double x, y, z;
     fetch(grp, x, y, z);
     eval_walkers<NS, NMO, EL, X>(P, sShell, sC, sDet, ws, x, y, z, lane);
+    bool flagged = false;
     if (lane < G) {
       const int64_t wo = grp * G + lane;
       if (wo < io.M) {
@@ -75,9 +76,65 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
         if (io.logpsi) io.logpsi[wo] = res[0];
         if (io.sign) io.sign[wo] = res[1];
         if (EL && io.eloc) io.eloc[wo] = res[2];
+        flagged = res[3] != 0.0;
       }
     }
+    // walkers whose reference determinant is nearly singular go to the explicit kernel
+    if (EL && io.fb_list) {
+      const unsigned any = __ballot_sync(0xffffffffu, flagged);
+      if (any && lane == 0) io.fb_list[atomicAdd(io.fb_count, 1)] = (int)grp;
+    }
     __syncwarp();
+  }
+}
+
+// Explicit re-evaluation of the groups listed by the fast kernel (rare; see kFallbackRatio).
+template <int NS, int NMO, bool X>
+__global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
+    explicit_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const int n_list = *io.fb_count;
+  if (n_list == 0) return;
+  const double *sC;
+  const ShellRec *sShell;
+  const DetRec *sDet;
+  double *wsBase;
+  load_constants<NMO>(P, smem, sC, sShell, sDet, wsBase);
+  using GE = Geo<NS, NMO>;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  double *ws = wsBase + warp * GE::total;
+  const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
+  const int g = lane / ne, e = lane - g * ne;
+  // one block per listed group: every warp rebuilds the MO rows, the determinants are dealt over the warps
+  for (int it = blockIdx.x; it < n_list; it += gridDim.x) {
+    const int64_t grp = io.fb_list[it];
+    const int64_t w = grp * G + g;
+    double x, y, z;
+    if ((g < G) && (w < io.M)) {
+      x = io.r_in[((int64_t)e * 3 + 0) * io.M + w];
+      y = io.r_in[((int64_t)e * 3 + 1) * io.M + w];
+      z = io.r_in[((int64_t)e * 3 + 2) * io.M + w];
+    } else {
+      dummy_xyz(lane, x, y, z);
+    }
+    eval_walkers<NS, NMO, true, X, true>(P, sShell, sC, sDet, ws, x, y, z, lane, warp, kWarpsPerBlock);
+    __syncthreads();
+    if (warp == 0 && lane < G) {
+      const int64_t wo = grp * G + lane;
+      double sig = 0.0, numk = 0.0;
+      for (int ww = 0; ww < kWarpsPerBlock; ++ww) {
+        const double *res = wsBase + ww * GE::total + GE::oRes + lane * 4;
+        sig += res[0];      // eq. 4
+        numk += res[1];     // F.2 / F.4 with G.7
+      }
+      const double *mine = ws + GE::oRes + lane * 4;
+      if (wo < io.M) {
+        if (io.logpsi) io.logpsi[wo] = mine[2] + log(fabs(sig));
+        if (io.sign) io.sign[wo] = (sig > 0.0) ? 1.0 : ((sig < 0.0) ? -1.0 : 0.0);
+        if (io.eloc) io.eloc[wo] = mine[3] + numk / sig + P.vnn;
+      }
+    }
+    __syncthreads();
   }
 }
 

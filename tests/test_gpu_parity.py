@@ -4,6 +4,7 @@ Tolerances are BASELINE.json north_star's: sign exact; log|Psi| 1e-10 absolute; 
 E_L 1e-8*max(1,|E_L|) for walkers with |Psi|/max|Psi| > 1e-6; batch mean E_L 1e-10 relative;
 Metropolis accept masks bit-exact except inside the 1e-12 tie window."""
 import math
+import os
 
 import numpy as np
 import pytest
@@ -234,3 +235,83 @@ def test_fp64_peak_and_model_flops(env):
     s = qb.QmcSystem(d)
     assert 5.5e4 < s.model_flops(0) < 6.5e4 and 2.5e4 < s.model_flops(1) < 4e4
     s.close()
+
+
+# ----------------------------------------------------------------------------- full BASELINE sizes
+@pytest.mark.parametrize("name", ["H2", "LiH", "Li2"])
+def test_full_size_small_configs(env, name):
+    """BASELINE configs[0..2] at their stated walker counts, every walker compared."""
+    d, r = wl.CONFIGS[name]()
+    check_local_energy(env, d, r, threads=os.cpu_count() or 8)
+
+
+def test_full_size_co_sampled(env):
+    """BASELINE configs[3] at 131072 walkers in the launch configuration bench.py times; the oracle
+    evaluates a sample of walkers (E_L of a walker does not depend on the others)."""
+    torch, ob, qb = env
+    d, r = wl.co()
+    M = r.shape[2]
+    s = qb.QmcSystem(d)
+    lp, sg, el = (t.cpu().numpy() for t in s.local_energy(_to_gpu(torch, r)))
+    idx = np.unique(np.concatenate([np.arange(0, 64), np.arange(M - 65, M),
+                                    np.random.default_rng(0).integers(0, M, 2048)]))
+    o = ob.OracleSystem(d)
+    lp0, sg0, el0 = ob.local_energy(o, np.ascontiguousarray(r[:, :, idx]), threads=os.cpu_count() or 8)
+    assert np.array_equal(sg[idx], sg0)
+    assert np.max(np.abs(lp[idx] - lp0)) < 1e-10
+    keep = lp0 - lp.max() > math.log(1e-6)
+    err = np.abs(el[idx] - el0) / np.maximum(1.0, np.abs(el0))
+    assert np.max(err[keep]) < 1e-8
+    # properties that hold at any size: finite outputs, sign is +-1, mean agrees with the device reduction
+    assert np.isfinite(lp).all() and np.isin(sg, (-1.0, 1.0)).all()
+    m, e = qb.batch_stats(torch.from_numpy(el).cuda())
+    m0, e0 = ob.batch_stats(el)
+    assert abs(m - m0) < 1e-11 * abs(m0) and abs(e - e0) < 1e-8 * e0
+    # Metropolis at full size: contiguous sample ranges, global walker indices
+    rg = _to_gpu(torch, r)
+    out = s.metropolis(rg, 0.2, 5, seed=4242, want_accept=True)
+    acc = out["accept"].cpu().numpy()
+    rf = rg.cpu().numpy()
+    L = ob.lib()
+    for w0 in (0, 40001, M - 96):
+        w1 = w0 + 96
+        rr = np.array(r, order="C", copy=True)
+        a0 = np.zeros((5, M), np.uint8); mg = np.zeros((5, M)); l0 = np.zeros(M); s0 = np.zeros(M)
+        assert L.oracle_metropolis(o.ref, rr.ctypes.data, M, w0, w1, 0.2, 5, 4242, 0, l0.ctypes.data, s0.ctypes.data,
+                                   a0.ctypes.data, mg.ctypes.data, None) == 0
+        bad = (acc[:, w0:w1] != a0[:, w0:w1]) & (np.abs(mg[:, w0:w1]) >= 1e-12)
+        assert not bad.any()
+        same = (acc[:, w0:w1] == a0[:, w0:w1]).all(axis=0)
+        assert np.max(np.abs(rf[:, :, w0:w1][:, :, same] - rr[:, :, w0:w1][:, :, same])) < 1e-12
+    s.close()
+
+
+def test_co_scan_geometries_sampled(env):
+    """BASELINE configs[4] shape: 500 determinants, several bond lengths, E_L accumulated every sweep."""
+    torch, ob, qb = env
+    for k, (d, r) in enumerate(wl.co_scan(M=96, n_geom=16)):
+        if k not in (0, 7, 15):
+            continue
+        check_local_energy(env, d, r, threads=os.cpu_count() or 8, mean_rtol=1e-9)
+
+
+def test_triple_and_quadruple_substitutions(env):
+    """Determinants with more than two substitutions in a spin (general k x k path)."""
+    rng = np.random.default_rng(11)
+    d, r = wl.li2(M=130)
+    import copy
+    d = copy.copy(d)
+    # reference (0,1,2); virtuals 3..7
+    d.det_up = np.array([[0, 1, 2], [3, 4, 5], [0, 6, 2], [7, 3, 6], [3, 1, 4], [5, 7, 4]], np.int32)
+    d.det_dn = np.array([[0, 1, 2], [0, 1, 2], [4, 5, 6], [0, 1, 7], [5, 3, 6], [7, 6, 3]], np.int32)
+    d.ci_coeff = np.array([0.9, 0.2, -0.15, 0.1, 0.25, -0.12])
+    check_local_energy(env, d, r, threads=4)
+    check_metropolis(env, d, r, 0.3, 4, seed=3)
+    # CO-sized: quadruple in one spin, triple in the other
+    d, r = wl.co(M=66)
+    d = copy.copy(d)
+    up = d.det_up.copy(); dn = d.det_dn.copy()
+    up[5] = [7, 8, 9, 10, 4, 5, 6]; dn[5] = [0, 11, 2, 12, 4, 13, 6]
+    up[9] = [0, 1, 2, 13, 12, 11, 6]
+    d.det_up, d.det_dn = up, dn
+    check_local_energy(env, d, r, threads=8)
