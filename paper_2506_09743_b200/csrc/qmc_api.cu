@@ -88,7 +88,7 @@ struct qmc_system {
   Variant var{};
   int smem_bytes = 0;
   int blocks_el = 0, blocks_psi = 0, blocks_metro = 0, blocks_metro_el = 0;
-  void *d_shells = nullptr, *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr;
+  void *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr;
   int n_sm = 0;
   double *d_stats = nullptr;
   unsigned long long *d_counter = nullptr;
@@ -117,7 +117,6 @@ int64_t qmc_launch_count(int reset) {
 void qmc_destroy(qmc_system_t *s) {
   if (!s) return;
   cudaSetDevice(s->device);
-  cudaFree(s->d_shells);
   cudaFree(s->d_C);
   cudaFree(s->d_dets);
   cudaFree(s->d_gen);
@@ -315,63 +314,71 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     const int k = n - 1 - l;
     rc.r.zeta = z;
     rc.r.c1 = 2.0 * z * (k + l + 1);
-    rc.r.c2 = (float)(k * (k + 2 * l + 1));
-    rc.r.k = (int16_t)k;
-    rc.r.m = (int16_t)d->ao_m[b];
-    rc.r.atom = (int16_t)at; rc.r.flush = 0;
-    if (l == 0) { rc.r.kind = SH_S; rc.aos = {b}; b += 1; }
-    else if (full) { rc.r.kind = (l == 1) ? SH_P : SH_D; for (int t = 0; t < nfun; ++t) rc.aos.push_back(b + t); b += nfun; }
-    else { rc.r.kind = (l == 1) ? SH_P1 : SH_D1; rc.aos = {b}; b += 1; }
+    rc.r.c2 = (double)(k * (k + 2 * l + 1));
+    rc.r.kd = (double)k;
+    rc.r.pad = 0;
+    int kind;
+    if (l == 0) { kind = SH_S; rc.aos = {b}; b += 1; }
+    else if (full) { kind = (l == 1) ? SH_P : SH_D; for (int t = 0; t < nfun; ++t) rc.aos.push_back(b + t); b += nfun; }
+    else { kind = (l == 1) ? SH_P1 : SH_D1; rc.aos = {b}; b += 1; }
+    rc.r.meta = kind | (k << 4) | ((l == 0 || full ? 0 : d->ao_m[rc.aos[0]]) << 8);
     recs.push_back(rc);
   }
   std::stable_sort(recs.begin(), recs.end(), [](const Rec &a, const Rec &b) { return a.atom < b.atom; });
+  if (recs.size() + (size_t)d->n_atoms > (size_t)kMaxShells) {
+    delete s;
+    return QMC_EUNSUPPORTED;
+  }
   // AO rows are laid out in chunks of kChunk (one DMMA pass each); a record never straddles a chunk.
-  // Records are grouped in fours that share a centre (padded with SH_NULL) for the kernel's quad loop.
+  // The last record of a chunk carries the number of rows the chunk uses (meta >> 20).
   std::vector<ShellRec> shells;
-  std::vector<std::vector<double>> crow;  // kernel AO row -> coefficients of the referenced MOs (or empty = pad)
   int n_real_shells = 0;
+  std::vector<std::vector<double>> crow;  // kernel AO row -> coefficients of the referenced MOs (or empty = pad)
   {
     int row = 0;
-    auto last_real = [&]() -> ShellRec & {
-      size_t i = shells.size();
-      while (shells[i - 1].kind == SH_NULL) --i;
-      return shells[i - 1];
+    int n_real = 0;
+    auto last_shell = [&]() -> ShellRec & {  // the last shell record (an atom record cannot carry the flush)
+      size_t j = shells.size();
+      while ((shells[j - 1].meta & 15) == SH_ATOM) --j;
+      return shells[j - 1];
     };
-    auto pad_quad = [&]() {
-      while (shells.size() % 4) {
-        ShellRec nul = shells.back();
-        nul.kind = SH_NULL;
-        nul.flush = 0;
-        shells.push_back(nul);
+    size_t i = 0;
+    for (int a = 0; a < d->n_atoms; ++a) {
+      {  // atom record: {zeta, c1, c2, kd} = {X, Y, Z, charge} (also for a centre without basis functions: V_en)
+        ShellRec ar{};
+        ar.zeta = d->atom_xyz[3 * a + 0];
+        ar.c1 = d->atom_xyz[3 * a + 1];
+        ar.c2 = d->atom_xyz[3 * a + 2];
+        ar.kd = d->atom_Z[a];
+        ar.meta = SH_ATOM;
+        shells.push_back(ar);
       }
-    };
-    for (size_t i = 0; i < recs.size(); ++i) {
+      for (; i < recs.size() && recs[i].atom == a; ++i) {
       const int nf = (int)recs[i].aos.size();
-      if (i > 0 && recs[i].atom != recs[i - 1].atom) pad_quad();
+      ++n_real;
       if (row % kChunk + nf > kChunk) {
-        last_real().flush = (int16_t)(row % kChunk);
+        last_shell().meta |= (row % kChunk) << 20;
         while (row % kChunk) { crow.emplace_back(); ++row; }
       }
-      recs[i].r.ao0 = (int16_t)row;
-      recs[i].r.atom = (int16_t)recs[i].atom;
-      recs[i].r.flush = 0;
+      recs[i].r.meta |= (row % kChunk) << 12;
       for (int b : recs[i].aos) {
         const double nrm = d->ao_norm ? d->ao_norm[b] : sto_norm(d->ao_n[b], d->ao_l[b], d->ao_m[b], d->ao_zeta[b]);
         std::vector<double> c(P.n_mo);
-        for (int a = 0; a < P.n_mo; ++a) c[a] = nrm * d->mo_coeff[(size_t)b * d->n_mo + used[a]];
+        for (int mo = 0; mo < P.n_mo; ++mo) c[mo] = nrm * d->mo_coeff[(size_t)b * d->n_mo + used[mo]];
         crow.push_back(c);
         ++row;
       }
       shells.push_back(recs[i].r);
-      ++n_real_shells;
-      if (row % kChunk == 0) shells.back().flush = (int16_t)kChunk;
+      if (row % kChunk == 0) shells.back().meta |= kChunk << 20;
+      }
     }
     if (row % kChunk) {
-      last_real().flush = (int16_t)(row % kChunk);
+      last_shell().meta |= (row % kChunk) << 20;
       while (row % kChunk) { crow.emplace_back(); ++row; }
     }
-    pad_quad();
+    n_real_shells = n_real;
   }
+  for (size_t i = 0; i < shells.size(); ++i) P.shells[i] = shells[i];
   const int n_chunks = (int)crow.size() / kChunk, NT = (NMO + 7) / 8, KS = kChunk / 4;
   P.n_chunks = n_chunks;
   // B fragments of mma.m8n8k4 (col-major B[k][n] held by lane 4 n + k)
@@ -383,9 +390,10 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
           const int k = ch * kChunk + 4 * ks + (lane & 3), n = 8 * t + (lane >> 2);
           if (!crow[k].empty() && n < P.n_mo) C[(((size_t)ch * KS + ks) * NT + t) * 32 + lane] = crow[k][n];
         }
-  P.n_shell = (int)shells.size();  // multiple of 4, SH_NULL padding included
+  P.n_shell = (int)shells.size();
   P.n_ao = d->n_ao;
   P.c_doubles = (int)C.size();
+  for (int j = 0; j < kExpTab; ++j) C.push_back((double)exp2l((long double)j / kExpTab));  // exp_neg's 2^(j/64)
 
   // ---- model FP64 work per walker
   {
@@ -408,12 +416,11 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   // ---- upload
   cudaError_t e = cudaSetDevice(device);
   if (e != cudaSuccess) { delete s; return cuda_fail(e, "cudaSetDevice"); }
-  const size_t szC = C.size() * sizeof(double), szS = shells.size() * sizeof(ShellRec), szD = dets.size() * sizeof(DetRec);
-  if ((e = cudaMalloc(&s->d_C, szC)) != cudaSuccess || (e = cudaMalloc(&s->d_shells, szS)) != cudaSuccess ||
+  const size_t szC = C.size() * sizeof(double), szD = dets.size() * sizeof(DetRec);
+  if ((e = cudaMalloc(&s->d_C, szC)) != cudaSuccess ||
       (e = cudaMalloc(&s->d_dets, szD)) != cudaSuccess || (e = cudaMalloc(&s->d_stats, 2 * sizeof(double))) != cudaSuccess ||
       (e = cudaMalloc(&s->d_counter, sizeof(unsigned long long))) != cudaSuccess ||
       (e = cudaMemcpy(s->d_C, C.data(), szC, cudaMemcpyHostToDevice)) != cudaSuccess ||
-      (e = cudaMemcpy(s->d_shells, shells.data(), szS, cudaMemcpyHostToDevice)) != cudaSuccess ||
       (e = cudaMemcpy(s->d_dets, dets.data(), szD, cudaMemcpyHostToDevice)) != cudaSuccess ||
       (e = cudaMalloc(&s->d_gen, std::max<size_t>(gens.size(), 1) * sizeof(GenDet))) != cudaSuccess ||
       (!gens.empty() && (e = cudaMemcpy(s->d_gen, gens.data(), gens.size() * sizeof(GenDet), cudaMemcpyHostToDevice)) != cudaSuccess) ||
@@ -423,12 +430,12 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     qmc_destroy(s);
     return rc;
   }
-  P.shells = (const ShellRec *)s->d_shells;
+  P.exp_tab = (const double *)s->d_C + P.c_doubles;
   P.C = (const double *)s->d_C;
   P.dets = (const DetRec *)s->d_dets;
   P.gen = (const GenDet *)s->d_gen;
   P.det_cols = (const DetCols *)s->d_cols;
-  P.smem_const_bytes = (int)((szC + szS + szD + 15) / 16 * 16);
+  P.smem_const_bytes = (int)((szC + szD + 15) / 16 * 16);
   s->smem_bytes = P.smem_const_bytes + kWarpsPerBlock * var->ws_doubles * (int)sizeof(double);
 
   int dev_smem = 0, n_sm = 0;

@@ -22,9 +22,6 @@ constexpr int kMaxVirt = 8;   // distinct virtual orbitals per spin
 #ifndef QMC_MINBLOCKS
 #define QMC_MINBLOCKS 2      // blocks per SM the register allocation must allow
 #endif
-#ifndef QMC_SHELL_UNROLL
-#define QMC_SHELL_UNROLL 1   // shell records whose exponentials are evaluated together (1, 2 or 4)
-#endif
 #ifndef QMC_PAIR_UNROLL
 #define QMC_PAIR_UNROLL 2    // unroll factor of the electron-pair loop
 #endif
@@ -34,28 +31,29 @@ constexpr int kMaxVirt = 8;   // distinct virtual orbitals per spin
 constexpr int kWarpsPerBlock = QMC_WARPS;
 
 // shell record kinds
-enum : int { SH_S = 0, SH_P = 1, SH_D = 2, SH_P1 = 3, SH_D1 = 4, SH_NULL = 5 };
+enum : int { SH_S = 0, SH_P = 1, SH_D = 2, SH_P1 = 3, SH_D1 = 4, SH_ATOM = 5 };
+constexpr int kMaxShells = 208;  // shell + atom records; they live in the kernel parameter block (constant bank, uniform data path)
 
-struct ShellRec {  // 32 bytes
+// One shell = the AOs that share a centre, n, l and zeta (one radial factor).  Every lane reads the same
+// record, so the records sit in the kernel parameters: the loads go through the uniform data path
+// and the constants stay in uniform registers.  48 bytes.
+struct ShellRec {
   double zeta;
   double c1;     // 2 zeta (k + l + 1)
-  float c2;      // k (k + 2l + 1)
-  int16_t kind;  // SH_*
-  int16_t k;     // radial power n-1-l
-  int16_t m;     // harmonic index for the single-function kinds
-  int16_t ao0;   // first AO row of this record in kernel order (chunk * 16 + row in chunk)
-  int16_t atom;  // centre
-  int16_t flush; // 0, or on the last record of a 16-row AO chunk: the number of rows the chunk uses
+  double c2;     // k (k + 2l + 1)
+  double kd;     // (double) k,  k = n - 1 - l the radial power
+  int32_t meta;  // kind | k << 4 | m << 8 | row in chunk << 12 | flush << 20
+  int32_t pad;
 };
+// meta fields: kind = SH_*; m = harmonic index of the single-function kinds; row = first AO row of the record
+// inside its chunk; flush = 0, or on the last record of a chunk the number of rows the chunk uses
+constexpr int kMetaK1 = 1 << 4, kMetaK2 = 2 << 4;
 
 #ifndef QMC_CHUNK
 #define QMC_CHUNK 16         // AO rows per DMMA chunk (8 or 16: 2 or 4 k-steps of the m8n8k4 shape)
 #endif
-#ifndef QMC_PARK_ACC
-#define QMC_PARK_ACC 0       // 1: park the MO accumulators in shared memory between chunks (frees registers
-                             // during the AO evaluation, costs ~20% more shared-memory wavefronts)
-#endif
 constexpr int kChunk = QMC_CHUNK;
+constexpr int kExpTab = 64;  // entries of the 2^(j/64) table of exp_neg
 
 // One determinant relative to the reference, per spin four table indices (p*LP+q) of the 2x2
 // sub-block {11, 12, 21, 22}; unused slots point at the constant entries TS-2 (= 1.0 in T, 0 in M)
@@ -102,7 +100,8 @@ struct SysParams {  // passed by value to every kernel
   int shell_begin[kMaxAtoms + 1];  // shells of atom a: [shell_begin[a], shell_begin[a+1])
   int8_t ref_col[2][kMaxSpin];     // kernel MO column of reference position j, per spin
   int8_t virt_col[2][kMaxVirt];    // kernel MO column of virtual q, per spin
-  const ShellRec *shells;          // device [n_shell]
+  ShellRec shells[kMaxShells];     // [n_shell] record stream: {SH_ATOM a, shells of a} per atom (n_shell counts both)
+  const double *exp_tab;           // device [kExpTab]: 2^(j/64), correctly rounded (qmc_setup)
   const double *C;                 // device [chunk][k-step 4][MO tile NT][lane 32]: DMMA B fragments of
                                    // N_ao * C (normalisation folded in, zero padded), see qmc_setup
   const DetRec *dets;              // device [n_det]  (at most two substitutions per spin)
@@ -174,19 +173,24 @@ struct Geo {
   static constexpr int oProb = oXYZ + 96;
   static constexpr int oRes = oProb + 2 * GMAX * 4;           // per walker {log|Psi|, sign, E_L, -}
   static constexpr int layout_total = oRes + GMAX * 4;
-  // DMMA contraction scratch, from offset 0 (everything it overlays is dead while it is live):
-  // the MO accumulators in D-fragment order [m-tile][n-tile][lane][2] (parked here between AO chunks
-  // so that they occupy no registers while the AOs are evaluated), then the AO tile [kChunk][S].
-  // Tile rows: [0, ROWS) values, [ROWS, 2 ROWS) the combined operator (E_L only).  S = 8 (mod 16)
-  // makes the A-fragment loads (4 k-rows x 8 rows per instruction) conflict-free.
-  __host__ __device__ static constexpr int aoStride(int ncomp) {
-    int m8 = ((ncomp * ROWS + 7) / 8) * 8;
-    return (m8 % 16 == 0) ? m8 + 8 : m8;
+  // DMMA contraction scratch, from offset 0 (everything it overlays is dead while it is live): the AO
+  // tile [kChunk AO rows][S].  Column = lane for the AO values; for E_L the combined operator of the
+  // lane sits in column opCol(lane) >= 32, so every lane (also one that owns no electron) stores
+  // unconditionally.  The m8n8k4 A fragments read 8 columns per M-tile: VT full tiles of values, then --
+  // when ROWS = 8 VT + 4 -- one MERGED tile {4 value columns, 4 operator columns}, then the operator
+  // tiles.  S = 8 (mod 16) keeps the fragment loads (4 k-rows x 8 columns) conflict-free.
+  static constexpr int S1 = 40, S2 = 72;                      // tile row stride: values only / with operator
+  static constexpr int VT = ROWS / 8;                         // full value tiles
+  static constexpr bool MERGE = (ROWS % 8) == 4;
+  static constexpr int VTc = (ROWS + 7) / 8;
+  __host__ __device__ static constexpr int mTiles(bool el) { return el ? (MERGE ? 2 * VT + 1 : 2 * VTc) : VTc; }
+  __host__ __device__ static constexpr int opCol(int lane) { return 32 + lane + ((MERGE && lane >= 8 * VT) ? 4 : 0); }
+  // first tile column of M-tile m minus the fragment row (the merged tile adds mergeShift(fr))
+  __host__ __device__ static constexpr int tileCol(bool el, int m) {
+    return !el ? 8 * m : (MERGE ? (m <= VT ? 8 * m : 32 + 8 * (m - VT - 1)) : (m < VTc ? 8 * m : 32 + 8 * (m - VTc)));
   }
-  __host__ __device__ static constexpr int accDoubles(int ncomp) {
-    return ((ncomp * ROWS + 7) / 8) * ((NMO + 7) / 8) * 64;
-  }
-  static constexpr int total = cmax(layout_total, (QMC_PARK_ACC ? accDoubles(2) : 0) + kChunk * aoStride(2));
+  __host__ __device__ static constexpr int mergeShift(int fr) { return (fr & 4) << 3; }  // rows 4..7: + 32
+  static constexpr int total = cmax(layout_total, kChunk * S2);
   static constexpr int NT = (NMO + 7) / 8;                    // 8-column MO tiles
 };
 
@@ -231,37 +235,27 @@ __device__ __forceinline__ double rsqrt_fast(double x) {
   return fma(y, e, y);
 }
 
-// exp(x) for x <= 0 (STO radial factors e^{-zeta r}): x = n ln2 + f, |f| <= ln2/2, degree-13 Taylor
-// polynomial (truncation 4e-18 relative) as two Horner chains in f^2 whose coefficients come straight
-// from the constant bank (no registers), 2^n applied to the exponent field.  Arguments below -700
-// are clamped (value ~1e-304, i.e. zero for every use here).
-__constant__ double kExpC[14] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040,
-                                 1.0 / 40320, 1.0 / 362880, 1.0 / 3628800, 1.0 / 39916800,
-                                 1.0 / 479001600, 1.0 / 6227020800.0};
-__constant__ double kExpR[4] = {1.4426950408889634, 6755399441055744.0, -6.93147180369123816490e-01,
-                                -1.90821492927058770002e-10};
-__device__ __forceinline__ double exp_neg(double x) {
-  x = fmax(x, -700.0);
-  const double t = fma(x, kExpR[0], kExpR[1]);  // round(x / ln2) in the low mantissa bits
+// exp(x) for x <= 0 (STO radial factors e^{-zeta r}): x = (64 n + j) ln2/64 + f, |f| <= ln2/128,
+//   e^x = 2^n * 2^(j/64) * (1 + q(f)),  q = f + f^2 (1/2 + f/6 + f^2 (1/24 + f/120))   (truncation 3.5e-17)
+// with 2^(j/64) from a 64-entry shared-memory table (correctly rounded doubles, built by qmc_setup) and
+// 2^n applied to the exponent field.  Arguments below -690 are clamped (value ~1e-300, zero for every
+// use here); NaN stays NaN.
+__constant__ double kExpR[4] = {92.33248261689366, 6755399441055744.0, -6.93147180369123816490e-01 / 64,
+                                -1.90821492927058770002e-10 / 64};
+__constant__ double kExpC[4] = {1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120};
+__device__ __forceinline__ double exp_neg(double x, const double *__restrict__ tab) {
+  x = (x < -690.0) ? -690.0 : x;
+  const double t = fma(x, kExpR[0], kExpR[1]);  // round(64 x / ln2) in the low mantissa bits
   const int n = __double2loint(t);
   const double nd = t - kExpR[1];
   double f = fma(nd, kExpR[2], x);
   f = fma(nd, kExpR[3], f);
   const double f2 = f * f;
-  double pe = fma(f2, kExpC[12], kExpC[10]);
-  double po = fma(f2, kExpC[13], kExpC[11]);
-  pe = fma(pe, f2, kExpC[8]);
-  po = fma(po, f2, kExpC[9]);
-  pe = fma(pe, f2, kExpC[6]);
-  po = fma(po, f2, kExpC[7]);
-  pe = fma(pe, f2, kExpC[4]);
-  po = fma(po, f2, kExpC[5]);
-  pe = fma(pe, f2, kExpC[2]);
-  po = fma(po, f2, kExpC[3]);
-  pe = fma(pe, f2, kExpC[0]);
-  po = fma(po, f2, kExpC[1]);
-  const double p = fma(po, f, pe);
-  return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
+  const double a = fma(f, kExpC[3], kExpC[2]), b = fma(f, kExpC[1], kExpC[0]);
+  const double q = fma(f2, fma(f2, a, b), f);
+  const double T = tab[n & (kExpTab - 1)];
+  const double p = fma(T, q, T);
+  return __hiloint2double(__double2hiint(p) + ((n >> 6) << 20), __double2loint(p));
 }
 
 // FP64 tensor-core MMA, D(8x8) += A(8x4) B(4x8).  Fragments (lane = 4 r + k):

@@ -92,7 +92,7 @@ __device__ __noinline__ void excite_general(const GenSpin *g, const double *T, i
 // {log|Psi|, sign, E_L} (E_L only if EL).  All 32 lanes must call.
 // ---------------------------------------------------------------------------------
 template <int NS, int NMO, bool EL, bool X, bool EXPL = false>
-__device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sShell,
+__device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp,
                              const double *__restrict__ sC, const DetRec *__restrict__ sDet,
                              double *__restrict__ ws, double x, double y, double z, int lane,
                              int det0 = 0, int det_step = 1) {
@@ -162,177 +162,140 @@ __device__ void eval_walkers(const SysParams &P, const ShellRec *__restrict__ sS
   // 16 rows the warp multiplies the tile into the MO accumulators with DMMA m8n8k4
   // (D[row][mo] += A[row][ao] C[ao][mo]; rows = electrons x {value, operator}).
   constexpr int NT = GE::NT;
-  constexpr int NCOMP = EL ? 2 : 1;
-  constexpr int MT = (NCOMP * GE::ROWS + 7) / 8;
-  constexpr int S = GE::aoStride(NCOMP);
+  constexpr int MT = GE::mTiles(EL);
+  constexpr int S = EL ? GE::S2 : GE::S1;
   double ven = 0.0;
   {
-#if !QMC_PARK_ACC
     double acc[MT][NT][2];
 #pragma unroll
     for (int m = 0; m < MT; ++m)
 #pragma unroll
       for (int t = 0; t < NT; ++t) acc[m][t][0] = acc[m][t][1] = 0.0;
-#endif
-    double *accst = ws;  // overlays the scratch from offset 0 (all dead here except sXYZ, read above)
-    double *tile = ws + (QMC_PARK_ACC ? GE::accDoubles(NCOMP) : 0);
-    __syncwarp();       // every lane is done with sXYZ
+    double *const tile = ws;  // overlays the scratch from offset 0 (all dead here except sXYZ, read above)
+    __syncwarp();             // every lane is done with sXYZ
     const int fr = lane >> 2, fk = lane & 3;  // fragment row / k of this lane
-    int cur_atom = -1, chunk = 0;
+    const int oo = GE::opCol(lane) - lane;                         // operator column relative to the value column (32 or 36)
+    const int mshift = GE::mergeShift(fr);
+    double *const tl = tile + lane;                                // this lane's value column of the tile
+    const double *const afrag = tile + fk * S + fr;                // A fragments: + 4 ks S + tile column
+    int chunk = 0;
     double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1.0, r = 1.0, ri = 1.0, gd = 0.0;
-    double *const tl = tile + lane;  // this lane's column of the tile
-    auto put = [&](double *trow, int t, double phi, double bop) {
-      if (active) {
-        trow[t * S] = phi;
-        if (EL) trow[t * S + GE::ROWS] = bop;
-      }
-    };
-    // one record: angular factors, the combined operator, stores into the tile, and -- on the last
-    // record of a chunk -- the DMMA pass over the chunk
-    auto process = [&](const ShellRec &sh, const double ex) {
-      if (sh.kind == SH_NULL) return;
-      const int k = sh.k;
-      const double gr = (k == 0) ? ex : ((k == 1) ? ex * r : ((k == 2) ? ex * r2 : ex * r2 * r));
-      double h = 0.0;
-      if (EL) {
-        // lap(S r^k e^{-zeta r}) = phi * [zeta^2 - 2 zeta (k+l+1)/r + k (k+2l+1)/r^2]
-        const double lapfac = fma(fma((double)sh.c2, ri, -sh.c1), ri, sh.zeta * sh.zeta);
-        const double radlog = fma((double)k, ri, -sh.zeta);  // g'/g
-        h = fma(-0.5, lapfac, -radlog * gd);
-      }
-      double *const tr = tl + (sh.ao0 & (kChunk - 1)) * S;
-      switch (sh.kind) {
-        case SH_S: {
-          put(tr, 0, gr, gr * h);
-        } break;
-        case SH_P: {
-          put(tr, 0, gr * dx, gr * fma(dx, h, -gJx));
-          put(tr, 1, gr * dy, gr * fma(dy, h, -gJy));
-          put(tr, 2, gr * dz, gr * fma(dz, h, -gJz));
-        } break;
-        case SH_D: {
+    // one uniform loop over the record stream [ATOM a][shells of a] ... (every lane reads the same record)
+    {
+      for (int s = 0; s < P.n_shell; ++s) {
+        const ShellRec &sh = P.shells[s];
+        const int meta = sh.meta;
+        if ((meta & 15) == SH_ATOM) {  // new centre: {zeta, c1, c2, kd} = {X, Y, Z, charge}
+          dx = x - sh.zeta;
+          dy = y - sh.c1;
+          dz = z - sh.c2;
+          r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+          ri = rsqrt_fast(r2);
+          r = r2 * ri;
+          if (EL) {
+            ven = fma(-sh.kd, ri, ven);
+            gd = fma(gJx, dx, fma(gJy, dy, gJz * dz)) * ri;  // grad J . d / r
+          }
+          continue;
+        }
+        double gr = exp_neg(-sh.zeta * r, sExp);          // r^k e^{-zeta r}
+        if (meta & kMetaK1) gr *= r;
+        if (meta & kMetaK2) gr *= r2;
+        double h = 0.0;
+        if (EL) {
+          // lap(S r^k e^{-zeta r}) = phi * [zeta^2 - 2 zeta (k+l+1)/r + k (k+2l+1)/r^2]
+          const double lapfac = fma(fma(sh.c2, ri, -sh.c1), ri, sh.zeta * sh.zeta);
+          const double radlog = fma(sh.kd, ri, -sh.zeta);  // g'/g
+          h = fma(-0.5, lapfac, -radlog * gd);
+        }
+        double *const tr = tl + ((meta >> 12) & 15) * S;
+        // value into column lane, combined operator into column opCol(lane): every lane stores
+        auto put = [&](int t, double phi, double bop) {
+          tr[t * S] = phi;
+          if (EL) tr[t * S + oo] = bop;
+        };
+        const int kind = meta & 15;
+        if (kind == SH_S) {
+          put(0, gr, gr * h);
+        } else if (kind == SH_P) {
+          put(0, gr * dx, gr * fma(dx, h, -gJx));
+          put(1, gr * dy, gr * fma(dy, h, -gJy));
+          put(2, gr * dz, gr * fma(dz, h, -gJz));
+        } else if (kind == SH_D) {
           double Sh, gs;
           Sh = dx * dy; gs = fma(gJx, dy, gJy * dx);
-          put(tr, 0, gr * Sh, gr * fma(Sh, h, -gs));
+          put(0, gr * Sh, gr * fma(Sh, h, -gs));
           Sh = dy * dz; gs = fma(gJy, dz, gJz * dy);
-          put(tr, 1, gr * Sh, gr * fma(Sh, h, -gs));
+          put(1, gr * Sh, gr * fma(Sh, h, -gs));
           Sh = dz * dx; gs = fma(gJz, dx, gJx * dz);
-          put(tr, 2, gr * Sh, gr * fma(Sh, h, -gs));
+          put(2, gr * Sh, gr * fma(Sh, h, -gs));
           Sh = fma(dx, dx, -dy * dy); gs = 2.0 * fma(gJx, dx, -gJy * dy);
-          put(tr, 3, gr * Sh, gr * fma(Sh, h, -gs));
+          put(3, gr * Sh, gr * fma(Sh, h, -gs));
           Sh = fma(2.0 * dz, dz, -fma(dx, dx, dy * dy));
           gs = 2.0 * fma(2.0 * gJz, dz, -fma(gJx, dx, gJy * dy));
-          put(tr, 4, gr * Sh, gr * fma(Sh, h, -gs));
-        } break;
-        case SH_P1: {
-          const int m = sh.m;
-          const double Sh = (m == 0) ? dx : ((m == 1) ? dy : dz);
-          const double gs = (m == 0) ? gJx : ((m == 1) ? gJy : gJz);
-          put(tr, 0, gr * Sh, gr * fma(Sh, h, -gs));
-        } break;
-        default: {  // SH_D1
-          const int m = sh.m;
+          put(4, gr * Sh, gr * fma(Sh, h, -gs));
+        } else {  // a lone p or d function (SH_P1, SH_D1)
+          const int m = (meta >> 8) & 15;
           double Sh, gs;
-          if (m == 0) { Sh = dx * dy; gs = fma(gJx, dy, gJy * dx); }
+          if (kind == SH_P1) {
+            Sh = (m == 0) ? dx : ((m == 1) ? dy : dz);
+            gs = (m == 0) ? gJx : ((m == 1) ? gJy : gJz);
+          } else if (m == 0) { Sh = dx * dy; gs = fma(gJx, dy, gJy * dx); }
           else if (m == 1) { Sh = dy * dz; gs = fma(gJy, dz, gJz * dy); }
           else if (m == 2) { Sh = dz * dx; gs = fma(gJz, dx, gJx * dz); }
           else if (m == 3) { Sh = fma(dx, dx, -dy * dy); gs = 2.0 * fma(gJx, dx, -gJy * dy); }
           else { Sh = fma(2.0 * dz, dz, -fma(dx, dx, dy * dy)); gs = 2.0 * fma(2.0 * gJz, dz, -fma(gJx, dx, gJy * dy)); }
-          put(tr, 0, gr * Sh, gr * fma(Sh, h, -gs));
-        } break;
-      }
-      if (sh.flush) {
-        // unused rows of the chunk meet zero rows of C, but must themselves be finite
-        for (int pr = sh.flush; pr < kChunk; ++pr) put(tl + pr * S, 0, 0.0, 0.0);
-        __syncwarp();
-#if QMC_PARK_ACC
-        double acc[MT][NT][2];
-        double2 *ast = reinterpret_cast<double2 *>(accst) + lane;
-        if (chunk == 0) {
-#pragma unroll
-          for (int m = 0; m < MT; ++m)
-#pragma unroll
-            for (int t = 0; t < NT; ++t) acc[m][t][0] = acc[m][t][1] = 0.0;
-        } else {
-#pragma unroll
-          for (int m = 0; m < MT; ++m)
-#pragma unroll
-            for (int t = 0; t < NT; ++t) {
-              const double2 v = ast[(m * NT + t) * 32];
-              acc[m][t][0] = v.x;
-              acc[m][t][1] = v.y;
-            }
+          put(0, gr * Sh, gr * fma(Sh, h, -gs));
         }
-#endif
-        const double *cf = sC + chunk * ((kChunk / 4) * NT * 32) + lane;
-#pragma unroll
-        for (int ks = 0; ks < kChunk / 4; ++ks) {
-          double bf[NT];
-#pragma unroll
-          for (int t = 0; t < NT; ++t) bf[t] = cf[(ks * NT + t) * 32];
-          const double *arow = tile + (4 * ks + fk) * S + fr;
-#pragma unroll
-          for (int m = 0; m < MT; ++m) {
-            const double a = arow[8 * m];
-#pragma unroll
-            for (int t = 0; t < NT; ++t) dmma884(acc[m][t][0], acc[m][t][1], a, bf[t]);
+        const int flush = meta >> 20;
+        if (flush) {
+          // unused rows of the chunk meet zero rows of C, but must themselves be finite
+          for (int pr = flush; pr < kChunk; ++pr) {
+            tl[pr * S] = 0.0;
+            if (EL) tl[pr * S + oo] = 0.0;
           }
-        }
-        ++chunk;
-        if (chunk < P.n_chunks) {
-#if QMC_PARK_ACC
+          __syncwarp();
+          const double *cf = sC + chunk * ((kChunk / 4) * NT * 32) + lane;
 #pragma unroll
-          for (int m = 0; m < MT; ++m)
+          for (int ks = 0; ks < kChunk / 4; ++ks) {
+            double bf[NT];
 #pragma unroll
-            for (int t = 0; t < NT; ++t) ast[(m * NT + t) * 32] = make_double2(acc[m][t][0], acc[m][t][1]);
-#endif
-        } else {
-          __syncwarp();  // the tile and the parked accumulators are dead: the MO rows overlay them
-          // D fragments -> MO rows: lane holds D[8 m + fr][8 t + 2 fk + {0,1}]
+            for (int t = 0; t < NT; ++t) bf[t] = cf[(ks * NT + t) * 32];
+            const double *arow = afrag + 4 * ks * S;
 #pragma unroll
-          for (int m = 0; m < MT; ++m) {
-            const int R = 8 * m + fr;
-            const bool isB = EL && (R >= GE::ROWS);
-            const int el = isB ? R - GE::ROWS : R;
-            double *dst = (isB ? sB : sPhi) + el * NMO;
-            if (el < G * ne && R < NCOMP * GE::ROWS) {
+            for (int m = 0; m < MT; ++m) {
+              const double a = arow[GE::tileCol(EL, m) + ((EL && GE::MERGE && m == GE::VT) ? mshift : 0)];
 #pragma unroll
-              for (int t = 0; t < NT; ++t) {
-                const int col = 8 * t + 2 * fk;
-                if (col < NMO) *reinterpret_cast<double2 *>(dst + col) = make_double2(acc[m][t][0], acc[m][t][1]);
-              }
+              for (int t = 0; t < NT; ++t) dmma884(acc[m][t][0], acc[m][t][1], a, bf[t]);
             }
           }
-        }
-        __syncwarp();
-      }
-    };
-    // Records come in groups of four that share a centre (the host pads with SH_NULL records): the four
-    // exponentials are independent chains the scheduler can interleave.
-    for (int s = 0; s < P.n_shell; s += QMC_SHELL_UNROLL) {
-      ShellRec q[QMC_SHELL_UNROLL];
-#pragma unroll
-      for (int u = 0; u < QMC_SHELL_UNROLL; ++u) q[u] = sShell[s + u];
-      const ShellRec &q0 = q[0];
-      if (q0.atom != cur_atom) {
-        cur_atom = q0.atom;
-        dx = x - P.atom[cur_atom][0];
-        dy = y - P.atom[cur_atom][1];
-        dz = z - P.atom[cur_atom][2];
-        r2 = fma(dx, dx, fma(dy, dy, dz * dz));
-        ri = rsqrt_fast(r2);
-        r = r2 * ri;
-        if (EL) {
-          ven = fma(-P.atom[cur_atom][3], ri, ven);
-          gd = fma(gJx, dx, fma(gJy, dy, gJz * dz)) * ri;  // grad J . d / r
+          ++chunk;
+          __syncwarp();
         }
       }
-      double ex[QMC_SHELL_UNROLL];
-#pragma unroll
-      for (int u = 0; u < QMC_SHELL_UNROLL; ++u) ex[u] = exp_neg(-q[u].zeta * r);
-#pragma unroll
-      for (int u = 0; u < QMC_SHELL_UNROLL; ++u) process(q[u], ex[u]);
     }
+    // the tile is dead: the MO rows overlay it.  D fragments -> MO rows: the lane holds rows fr of every
+    // M-tile, columns 8 t + 2 fk + {0,1}
+#pragma unroll
+    for (int m = 0; m < MT; ++m) {
+      bool isB = false;
+      int el = 8 * m + fr;
+      if (EL) {
+        if (GE::MERGE) {
+          if (m == GE::VT) { isB = fr >= 4; el = 8 * GE::VT + (fr & 3); }
+          else if (m > GE::VT) { isB = true; el = 8 * (m - GE::VT - 1) + fr; }
+        } else if (m >= GE::VTc) { isB = true; el = 8 * (m - GE::VTc) + fr; }
+      }
+      double *dst = (isB ? sB : sPhi) + el * NMO;
+      if (el < G * ne) {
+#pragma unroll
+        for (int t = 0; t < NT; ++t) {
+          const int col = 8 * t + 2 * fk;
+          if (col < NMO) *reinterpret_cast<double2 *>(dst + col) = make_double2(acc[m][t][0], acc[m][t][1]);
+        }
+      }
+    }
+    __syncwarp();
   }
   {
     // per-electron scalars: J/2-sum and the electron's share of the energy

@@ -5,27 +5,23 @@
 
 namespace qmc {
 
-// copy the constants into shared memory; returns pointers.  Layout: C | shells | dets.
+// copy the constants into shared memory; returns pointers.  Layout: C | exp table | dets.
 template <int NMO>
 __device__ __forceinline__ void load_constants(const SysParams &P, unsigned char *smem, const double *&sC,
-                                               const ShellRec *&sShell, const DetRec *&sDet, double *&wsBase) {
+                                               const double *&sExp, const DetRec *&sDet, double *&wsBase) {
   double *c = reinterpret_cast<double *>(smem);
   const int nC = P.c_doubles;
   for (int i = threadIdx.x; i < nC; i += blockDim.x) c[i] = P.C[i];
-  ShellRec *sh = reinterpret_cast<ShellRec *>(c + nC);
-  {
-    const double *src = reinterpret_cast<const double *>(P.shells);
-    double *dst = reinterpret_cast<double *>(sh);
-    for (int i = threadIdx.x; i < P.n_shell * 4; i += blockDim.x) dst[i] = src[i];
-  }
-  DetRec *dt = reinterpret_cast<DetRec *>(sh + P.n_shell);
+  double *et = c + nC;
+  for (int i = threadIdx.x; i < kExpTab; i += blockDim.x) et[i] = P.exp_tab[i];
+  DetRec *dt = reinterpret_cast<DetRec *>(et + kExpTab);
   {
     const double *src = reinterpret_cast<const double *>(P.dets);
     double *dst = reinterpret_cast<double *>(dt);
     for (int i = threadIdx.x; i < P.n_det * 2; i += blockDim.x) dst[i] = src[i];
   }
   sC = c;
-  sShell = sh;
+  sExp = et;
   sDet = dt;
   wsBase = reinterpret_cast<double *>(smem + P.smem_const_bytes);
   __syncthreads();
@@ -43,12 +39,12 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
     local_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
   const double *sC;
-  const ShellRec *sShell;
+  const double *sExp;
   const DetRec *sDet;
   double *wsBase;
-  load_constants<NMO>(P, smem, sC, sShell, sDet, wsBase);
+  load_constants<NMO>(P, smem, sC, sExp, sDet, wsBase);
   using GE = Geo<NS, NMO>;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;  // shfl: tells the compiler it is warp-uniform
   double *ws = wsBase + warp * GE::total;
   const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
   const int g = lane / ne, e = lane - g * ne;
@@ -67,7 +63,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
   for (int64_t grp = (int64_t)blockIdx.x * kWarpsPerBlock + warp; grp < n_groups; grp += stride) {
     double x, y, z;
     fetch(grp, x, y, z);
-    eval_walkers<NS, NMO, EL, X>(P, sShell, sC, sDet, ws, x, y, z, lane);
+    eval_walkers<NS, NMO, EL, X>(P, sExp, sC, sDet, ws, x, y, z, lane);
     bool flagged = false;
     if (lane < G) {
       const int64_t wo = grp * G + lane;
@@ -96,12 +92,12 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
   const int n_list = *io.fb_count;
   if (n_list == 0) return;
   const double *sC;
-  const ShellRec *sShell;
+  const double *sExp;
   const DetRec *sDet;
   double *wsBase;
-  load_constants<NMO>(P, smem, sC, sShell, sDet, wsBase);
+  load_constants<NMO>(P, smem, sC, sExp, sDet, wsBase);
   using GE = Geo<NS, NMO>;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;  // shfl: tells the compiler it is warp-uniform
   double *ws = wsBase + warp * GE::total;
   const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
   const int g = lane / ne, e = lane - g * ne;
@@ -117,7 +113,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
     } else {
       dummy_xyz(lane, x, y, z);
     }
-    eval_walkers<NS, NMO, true, X, true>(P, sShell, sC, sDet, ws, x, y, z, lane, warp, kWarpsPerBlock);
+    eval_walkers<NS, NMO, true, X, true>(P, sExp, sC, sDet, ws, x, y, z, lane, warp, kWarpsPerBlock);
     __syncthreads();
     if (warp == 0 && lane < G) {
       const int64_t wo = grp * G + lane;
@@ -147,12 +143,12 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
     metropolis_kernel(const __grid_constant__ SysParams P, const WalkerIO io, const MetroParams mp) {
   extern __shared__ __align__(16) unsigned char smem[];
   const double *sC;
-  const ShellRec *sShell;
+  const double *sExp;
   const DetRec *sDet;
   double *wsBase;
-  load_constants<NMO>(P, smem, sC, sShell, sDet, wsBase);
+  load_constants<NMO>(P, smem, sC, sExp, sDet, wsBase);
   using GE = Geo<NS, NMO>;
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;  // shfl: tells the compiler it is warp-uniform
   double *ws = wsBase + warp * GE::total;
   double *sProp = ws + GE::oProp;       // [G][3 ne] normals
   double *sLogU = sProp + 96;           // [G]
@@ -207,7 +203,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
         logu = sLogU[own ? g : 0];
         __syncwarp();
       }
-      eval_walkers<NS, NMO, false, X>(P, sShell, sC, sDet, ws, xp, yp, zp, lane);
+      eval_walkers<NS, NMO, false, X>(P, sExp, sC, sDet, ws, xp, yp, zp, lane);
       const double lp2 = sRes[rg + 0], sg2 = sRes[rg + 1];
       // accept iff log u < 2 (log|Psi'| - log|Psi|): false for NaN and for Psi' = 0
       const bool ok = (sw < 0) || (own && (logu < 2.0 * (lp2 - lp)));
@@ -218,7 +214,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
       }
       __syncwarp();
       if (WITH_EL && sw >= 0) {
-        eval_walkers<NS, NMO, true, X>(P, sShell, sC, sDet, ws, x, y, z, lane);
+        eval_walkers<NS, NMO, true, X>(P, sExp, sC, sDet, ws, x, y, z, lane);
         eacc += sRes[rg + 2];
         __syncwarp();
       }
