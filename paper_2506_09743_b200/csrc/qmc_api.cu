@@ -394,6 +394,23 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   P.n_ao = d->n_ao;
   P.c_doubles = (int)C.size();
   for (int j = 0; j < kExpTab; ++j) C.push_back((double)exp2l((long double)j / kExpTab));  // exp_neg's 2^(j/64)
+  {  // Box-Muller tables (qmc_device.cuh: log_pos, sincos_2pi)
+    for (int j = 0; j < 64; ++j) {  // piece j of [sqrt(1/2), sqrt(2)): high words 0x3fe6a09e + [j, j+1) * 2^14
+      const uint64_t lo = ((uint64_t)(0x3fe6a09eu + ((uint32_t)j << 14))) << 32;
+      const uint64_t hi = (((uint64_t)(0x3fe6a09eu + ((uint32_t)(j + 1) << 14))) << 32) - 1;
+      double mlo, mhi;
+      std::memcpy(&mlo, &lo, 8);
+      std::memcpy(&mhi, &hi, 8);
+      const double inv = (double)(1.0L / (0.5L * ((long double)mlo + (long double)mhi)));
+      C.push_back(inv);
+      C.push_back((double)(-logl((long double)inv)));
+    }
+    const long double two_pi = 6.283185307179586476925286766559L;
+    for (int j = 0; j < 64; ++j) {
+      C.push_back((double)cosl(two_pi * j / 64));
+      C.push_back((double)sinl(two_pi * j / 64));
+    }
+  }
 
   // ---- model FP64 work per walker
   {
@@ -431,6 +448,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     return rc;
   }
   P.exp_tab = (const double *)s->d_C + P.c_doubles;
+  P.rng_tab = P.exp_tab + kExpTab;
   P.C = (const double *)s->d_C;
   P.dets = (const DetRec *)s->d_dets;
   P.gen = (const GenDet *)s->d_gen;

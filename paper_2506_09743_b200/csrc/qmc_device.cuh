@@ -102,6 +102,7 @@ struct SysParams {  // passed by value to every kernel
   int8_t virt_col[2][kMaxVirt];    // kernel MO column of virtual q, per spin
   ShellRec shells[kMaxShells];     // [n_shell] record stream: {SH_ATOM a, shells of a} per atom (n_shell counts both)
   const double *exp_tab;           // device [kExpTab]: 2^(j/64), correctly rounded (qmc_setup)
+  const double *rng_tab;           // device [kRngTab]: log and sincos tables of the Box-Muller transform
   const double *C;                 // device [chunk][k-step 4][MO tile NT][lane 32]: DMMA B fragments of
                                    // N_ao * C (normalisation folded in, zero padded), see qmc_setup
   const DetRec *dets;              // device [n_det]  (at most two substitutions per spin)
@@ -256,6 +257,55 @@ __device__ __forceinline__ double exp_neg(double x, const double *__restrict__ t
   const double T = tab[n & (kExpTab - 1)];
   const double p = fma(T, q, T);
   return __hiloint2double(__double2hiint(p) + ((n >> 6) << 20), __double2loint(p));
+}
+
+// ---------------------------------------------------------------------------------
+// Elementary functions of the Box-Muller transform (reading Q9), table-driven so that one
+// normal pair costs ~40 FP64 instructions.  Tables are built in long double by qmc_setup (kRngTab
+// doubles: 64 {1/c_j, -log(1/c_j)} pairs, then 64 {cos, sin}(2 pi j / 64) pairs) and sit in shared memory.
+// ---------------------------------------------------------------------------------
+constexpr int kRngTab = 256;
+__constant__ double kLogC[8] = {6.93147180369123816490e-01, 1.90821492927058770002e-10,  // ln2 hi, lo
+                                1.0 / 7, -1.0 / 6, 1.0 / 5, -1.0 / 4, 1.0 / 3, -1.0 / 2};
+// log(u) for a positive normal u (here u in (0,1)): u = 2^e m, m in [sqrt(1/2), sqrt(2)); the top six bits
+// of m's offset in that range select c_j; r = m / c_j - 1, |r| <= 0.0079;
+// log u = e ln2 - log(1/c_j) + (r - r^2/2 + ... + r^7/7)      (truncation r^8/8 < 2e-18)
+__device__ __forceinline__ double log_pos(double u, const double2 *__restrict__ tab) {
+  int hx = __double2hiint(u) + (0x3ff00000 - 0x3fe6a09e);
+  const int e = (hx >> 20) - 1023;
+  hx &= 0xfffff;
+  const double m = __hiloint2double(hx + 0x3fe6a09e, __double2loint(u));
+  const double2 t = tab[hx >> 14];
+  const double r = fma(m, t.x, -1.0);
+  double p = fma(r, kLogC[2], kLogC[3]);
+  p = fma(p, r, kLogC[4]);
+  p = fma(p, r, kLogC[5]);
+  p = fma(p, r, kLogC[6]);
+  p = fma(p, r, kLogC[7]);
+  const double lg = fma(r * r, p, r);
+  const double ed = (double)e;
+  return fma(ed, kLogC[0], t.y) + fma(ed, kLogC[1], lg);
+}
+// sqrt(x), x > 0 normal: x * rsqrt(x) with one correction step (error < 1 ulp)
+__device__ __forceinline__ double sqrt_pos(double x) {
+  const double y = rsqrt_fast(x);
+  const double s = x * y;
+  return fma(fma(-s, s, x), 0.5 * y, s);
+}
+// sin and cos of 2 pi u, u in [0,1): u = j/64 + f, |f| <= 1/128 (exact), a = 2 pi f, |a| <= 0.0491;
+// short Taylor polynomials in a (truncation < 5e-18) rotated by the tabulated {cos, sin}(2 pi j/64).
+__constant__ double kSinC[8] = {6.283185307179586, 6755399441055744.0, -1.0 / 6, 1.0 / 120, -1.0 / 5040,
+                                1.0 / 24, -1.0 / 720, 1.0 / 40320};
+__device__ __forceinline__ void sincos_2pi(double u, const double2 *__restrict__ tab, double &sn, double &cs) {
+  const double t = fma(u, 64.0, kSinC[1]);  // round(64 u) in the low mantissa bits
+  const double f = fma(t - kSinC[1], -1.0 / 64, u);
+  const double2 w = tab[__double2loint(t) & 63];
+  const double a = f * kSinC[0];
+  const double a2 = a * a;
+  const double sa = fma(a * a2, fma(a2, fma(a2, kSinC[4], kSinC[3]), kSinC[2]), a);          // sin a
+  const double qc = a2 * fma(a2, fma(a2, fma(a2, kSinC[7], kSinC[6]), kSinC[5]), -0.5);      // cos a - 1
+  cs = fma(-w.y, sa, fma(w.x, qc, w.x));
+  sn = fma(w.x, sa, fma(w.y, qc, w.y));
 }
 
 // FP64 tensor-core MMA, D(8x8) += A(8x4) B(4x8).  Fragments (lane = 4 r + k):

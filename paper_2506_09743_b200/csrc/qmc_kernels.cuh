@@ -5,7 +5,7 @@
 
 namespace qmc {
 
-// copy the constants into shared memory; returns pointers.  Layout: C | exp table | dets.
+// copy the constants into shared memory; returns pointers.  Layout: C | exp table | rng tables | dets.
 template <int NMO>
 __device__ __forceinline__ void load_constants(const SysParams &P, unsigned char *smem, const double *&sC,
                                                const double *&sExp, const DetRec *&sDet, double *&wsBase) {
@@ -14,7 +14,8 @@ __device__ __forceinline__ void load_constants(const SysParams &P, unsigned char
   for (int i = threadIdx.x; i < nC; i += blockDim.x) c[i] = P.C[i];
   double *et = c + nC;
   for (int i = threadIdx.x; i < kExpTab; i += blockDim.x) et[i] = P.exp_tab[i];
-  DetRec *dt = reinterpret_cast<DetRec *>(et + kExpTab);
+  for (int i = threadIdx.x; i < kRngTab; i += blockDim.x) et[kExpTab + i] = P.rng_tab[i];
+  DetRec *dt = reinterpret_cast<DetRec *>(et + kExpTab + kRngTab);
   {
     const double *src = reinterpret_cast<const double *>(P.dets);
     double *dst = reinterpret_cast<double *>(dt);
@@ -150,6 +151,8 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
   using GE = Geo<NS, NMO>;
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;  // shfl: tells the compiler it is warp-uniform
   double *ws = wsBase + warp * GE::total;
+  const double2 *sLogT = reinterpret_cast<const double2 *>(sExp + kExpTab);  // log_pos table
+  const double2 *sSinT = sLogT + 64;                                         // sincos_2pi table
   double *sProp = ws + GE::oProp;       // [G][3 ne] normals
   double *sLogU = sProp + 96;           // [G]
   const double *sRes = ws + GE::oRes;
@@ -182,14 +185,13 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
           uint32_t o[4];
           philox4x32_10((uint32_t)gw, mp.sweep0 + (uint32_t)sw, (j == npair) ? 0xFFFFFFFFu : (uint32_t)j,
                         (uint32_t)(gw >> 32), mp.key0, mp.key1, o);
-          const double u1 = u53(o[0], o[1]);
+          const double lu = log_pos(u53(o[0], o[1]), sLogT);
           if (j == npair) {
-            sLogU[dg] = log(u1);
+            sLogU[dg] = lu;
           } else {
-            const double u2 = u53(o[2], o[3]);
-            const double rho = sqrt(-2.0 * log(u1));
+            const double rho = sqrt_pos(-2.0 * lu);
             double sn, cs;
-            sincos(6.283185307179586 * u2, &sn, &cs);
+            sincos_2pi(u53(o[2], o[3]), sSinT, sn, cs);
             sProp[dg * nc + 2 * j] = rho * cs;
             if (2 * j + 1 < nc) sProp[dg * nc + 2 * j + 1] = rho * sn;
           }
