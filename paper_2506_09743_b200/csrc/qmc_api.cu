@@ -45,11 +45,11 @@ Variant make_variant() {
   v.LP = Geo<NS, NMO>::LP;
   v.exact = X;
   v.ws_doubles = Geo<NS, NMO>::total;
-  v.k_el = (const void *)local_energy_kernel<NS, NMO, true, X>;
-  v.k_psi = (const void *)local_energy_kernel<NS, NMO, false, X>;
-  v.k_metro = (const void *)metropolis_kernel<NS, NMO, false, X>;
-  v.k_metro_el = (const void *)metropolis_kernel<NS, NMO, true, X>;
-  v.k_expl = (const void *)explicit_energy_kernel<NS, NMO, X>;
+  v.k_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl>;
+  v.k_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi>;
+  v.k_metro = (const void *)metropolis_kernel<NS, NMO, false, X, kWarpsPsi>;
+  v.k_metro_el = (const void *)metropolis_kernel<NS, NMO, true, X, kWarpsEl>;
+  v.k_expl = (const void *)explicit_energy_kernel<NS, NMO, X, kWarpsEl>;
   return v;
 }
 
@@ -86,7 +86,7 @@ struct qmc_system {
   int device = 0;
   SysParams P{};
   Variant var{};
-  int smem_bytes = 0;
+  int smem_el = 0, smem_psi = 0;  // dynamic shared memory of the E_L kernels (kWarpsEl warps) / values-only kernels
   int blocks_el = 0, blocks_psi = 0, blocks_metro = 0, blocks_metro_el = 0;
   void *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr;
   int n_sm = 0;
@@ -454,12 +454,13 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   P.gen = (const GenDet *)s->d_gen;
   P.det_cols = (const DetCols *)s->d_cols;
   P.smem_const_bytes = (int)((szC + szD + 15) / 16 * 16);
-  s->smem_bytes = P.smem_const_bytes + kWarpsPerBlock * var->ws_doubles * (int)sizeof(double);
+  s->smem_el = P.smem_const_bytes + kWarpsEl * var->ws_doubles * (int)sizeof(double);
+  s->smem_psi = P.smem_const_bytes + kWarpsPsi * var->ws_doubles * (int)sizeof(double);
 
   int dev_smem = 0, n_sm = 0;
   cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
   cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device);
-  if (s->smem_bytes > dev_smem) {
+  if (std::max(s->smem_el, s->smem_psi) > dev_smem) {
     qmc_destroy(s);
     return QMC_EUNSUPPORTED;
   }
@@ -467,14 +468,16 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   s->n_sm = n_sm;
   const void *ks[5] = {var->k_el, var->k_psi, var->k_metro, var->k_metro_el, var->k_expl};
   int *nb[5] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro, &s->blocks_metro_el, &blocks_expl};
+  const int kw[5] = {kWarpsEl, kWarpsPsi, kWarpsPsi, kWarpsEl, kWarpsEl};
+  const int ksm[5] = {s->smem_el, s->smem_psi, s->smem_psi, s->smem_el, s->smem_el};
   for (int i = 0; i < 5; ++i) {
-    if ((e = cudaFuncSetAttribute(ks[i], cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_bytes)) != cudaSuccess) {
+    if ((e = cudaFuncSetAttribute(ks[i], cudaFuncAttributeMaxDynamicSharedMemorySize, ksm[i])) != cudaSuccess) {
       int rc = cuda_fail(e, "cudaFuncSetAttribute");
       qmc_destroy(s);
       return rc;
     }
     int per_sm = 0;
-    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ks[i], kWarpsPerBlock * 32, s->smem_bytes)) != cudaSuccess || per_sm < 1) {
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ks[i], kw[i] * 32, ksm[i])) != cudaSuccess || per_sm < 1) {
       int rc = (e != cudaSuccess) ? cuda_fail(e, "occupancy") : QMC_EUNSUPPORTED;
       qmc_destroy(s);
       return rc;
@@ -497,7 +500,8 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
   io.eloc = d_eloc;
   io.M = M;
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
-  const int64_t need = (groups + kWarpsPerBlock - 1) / kWarpsPerBlock;
+  const int wpb = el ? kWarpsEl : kWarpsPsi, smem = el ? s->smem_el : s->smem_psi;
+  const int64_t need = (groups + wpb - 1) / wpb;
   const int grid = (int)std::min<int64_t>(need, el ? s->blocks_el : s->blocks_psi);
   int *fb = nullptr;
   const bool fallback = el && s->P.n_det_all > 1;  // a single determinant has no reference to be ill-conditioned against
@@ -508,10 +512,10 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
     io.fb_list = fb + 1;
   }
   void *args[2] = {(void *)&s->P, (void *)&io};
-  CK(cudaLaunchKernel(el ? s->var.k_el : s->var.k_psi, dim3(grid), dim3(kWarpsPerBlock * 32), args, s->smem_bytes, st));
+  CK(cudaLaunchKernel(el ? s->var.k_el : s->var.k_psi, dim3(grid), dim3(wpb * 32), args, smem, st));
   ++g_launches;
   if (fallback) {
-    CK(cudaLaunchKernel(s->var.k_expl, dim3(grid), dim3(kWarpsPerBlock * 32), args, s->smem_bytes, st));
+    CK(cudaLaunchKernel(s->var.k_expl, dim3(grid), dim3(kWarpsEl * 32), args, s->smem_el, st));
     ++g_launches;
     CK(cudaFreeAsync(fb, st));
   }
@@ -552,10 +556,11 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
   mp.n_accepted = h_n_accepted ? s->d_counter : nullptr;
   if (h_n_accepted) CK(cudaMemsetAsync(s->d_counter, 0, sizeof(unsigned long long), st));
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
-  const int64_t need = (groups + kWarpsPerBlock - 1) / kWarpsPerBlock;
+  const int wpb = d_eloc_acc ? kWarpsEl : kWarpsPsi, smem = d_eloc_acc ? s->smem_el : s->smem_psi;
+  const int64_t need = (groups + wpb - 1) / wpb;
   const int grid = (int)std::min<int64_t>(need, d_eloc_acc ? s->blocks_metro_el : s->blocks_metro);
   void *args[3] = {(void *)&s->P, (void *)&io, (void *)&mp};
-  CK(cudaLaunchKernel(d_eloc_acc ? s->var.k_metro_el : s->var.k_metro, dim3(grid), dim3(kWarpsPerBlock * 32), args, s->smem_bytes, st));
+  CK(cudaLaunchKernel(d_eloc_acc ? s->var.k_metro_el : s->var.k_metro, dim3(grid), dim3(wpb * 32), args, smem, st));
   ++g_launches;
   if (h_n_accepted) {
     unsigned long long v = 0;

@@ -28,7 +28,11 @@ constexpr int kMaxVirt = 8;   // distinct virtual orbitals per spin
 #ifndef QMC_EARLY_INV
 #define QMC_EARLY_INV 0      // Gauss-Jordan: invert every pivot candidate before the arg-max is known
 #endif
-constexpr int kWarpsPerBlock = QMC_WARPS;
+#ifndef QMC_WARPS_PSI
+#define QMC_WARPS_PSI 10     // warps per block of the values-only kernels (log|Psi|, Metropolis): they fit 96 registers
+#endif
+constexpr int kWarpsEl = QMC_WARPS, kWarpsPsi = QMC_WARPS_PSI;
+constexpr int kWarpsMax = kWarpsEl > kWarpsPsi ? kWarpsEl : kWarpsPsi;
 
 // shell record kinds
 enum : int { SH_S = 0, SH_P = 1, SH_D = 2, SH_P1 = 3, SH_D1 = 4, SH_ATOM = 5 };
@@ -58,7 +62,7 @@ constexpr int kExpTab = 64;  // entries of the 2^(j/64) table of exp_neg
 // One determinant relative to the reference, per spin four table indices (p*LP+q) of the 2x2
 // sub-block {11, 12, 21, 22}; unused slots point at the constant entries TS-2 (= 1.0 in T, 0 in M)
 // and TS-1 (= 0.0), so k = 0, 1, 2 substitutions share one formula.  16 bytes.
-struct DetRec {
+struct __align__(16) DetRec {
   uint32_t up, dn;  // 4 x uint8 each
   double d;
 };
@@ -179,13 +183,19 @@ struct Geo {
   // lane sits in column opCol(lane) >= 32, so every lane (also one that owns no electron) stores
   // unconditionally.  The m8n8k4 A fragments read 8 columns per M-tile: VT full tiles of values, then --
   // when ROWS = 8 VT + 4 -- one MERGED tile {4 value columns, 4 operator columns}, then the operator
-  // tiles.  S = 8 (mod 16) keeps the fragment loads (4 k-rows x 8 columns) conflict-free.
-  static constexpr int S1 = 40, S2 = 72;                      // tile row stride: values only / with operator
+  // tiles.  S = 4 (mod 16): a half-warp of a fragment load (4 k-rows x 4 columns of doubles) then covers
+  // all 32 banks once (measured with S = 8 (mod 16): 2-way conflicts, 4 wavefronts per load instead of 2).
+  static constexpr int S1 = 36, S2 = 68;                      // tile row stride: values only / with operator
   static constexpr int VT = ROWS / 8;                         // full value tiles
   static constexpr bool MERGE = (ROWS % 8) == 4;
   static constexpr int VTc = (ROWS + 7) / 8;
   __host__ __device__ static constexpr int mTiles(bool el) { return el ? (MERGE ? 2 * VT + 1 : 2 * VTc) : VTc; }
-  __host__ __device__ static constexpr int opCol(int lane) { return 32 + lane + ((MERGE && lane >= 8 * VT) ? 4 : 0); }
+  // operator column of a lane: 32 + lane; behind the merged tile the real rows move up by 4 (columns
+  // 60..63 for ROWS = 28) and the lanes that own no row park in the free columns 56..59, which no fragment
+  // reads and whose banks no other lane of their half-warp touches
+  __host__ __device__ static constexpr int opCol(int lane) {
+    return !MERGE ? 32 + lane : (lane < 8 * VT ? 32 + lane : (lane < ROWS ? 36 + lane : 28 + lane));
+  }
   // first tile column of M-tile m minus the fragment row (the merged tile adds mergeShift(fr))
   __host__ __device__ static constexpr int tileCol(bool el, int m) {
     return !el ? 8 * m : (MERGE ? (m <= VT ? 8 * m : 32 + 8 * (m - VT - 1)) : (m < VTc ? 8 * m : 32 + 8 * (m - VTc)));
@@ -241,18 +251,19 @@ __device__ __forceinline__ double rsqrt_fast(double x) {
 // with 2^(j/64) from a 64-entry shared-memory table (correctly rounded doubles, built by qmc_setup) and
 // 2^n applied to the exponent field.  Arguments below -690 are clamped (value ~1e-300, zero for every
 // use here); NaN stays NaN.
-__constant__ double kExpR[4] = {92.33248261689366, 6755399441055744.0, -6.93147180369123816490e-01 / 64,
-                                -1.90821492927058770002e-10 / 64};
-__constant__ double kExpC[4] = {1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120};
+// Constants are literals: one constant per FMA comes straight from the compiler's constant bank or, when
+// its low word is zero (the rounding magic, 1/2), as an immediate -- no load instructions.
 __device__ __forceinline__ double exp_neg(double x, const double *__restrict__ tab) {
+  constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52
   x = (x < -690.0) ? -690.0 : x;
-  const double t = fma(x, kExpR[0], kExpR[1]);  // round(64 x / ln2) in the low mantissa bits
+  const double t = fma(x, 92.33248261689366, kMagic);  // round(64 x / ln2) in the low mantissa bits
   const int n = __double2loint(t);
-  const double nd = t - kExpR[1];
-  double f = fma(nd, kExpR[2], x);
-  f = fma(nd, kExpR[3], f);
+  const double nd = t - kMagic;
+  double f = fma(nd, -6.93147180369123816490e-01 / 64, x);
+  f = fma(nd, -1.90821492927058770002e-10 / 64, f);
   const double f2 = f * f;
-  const double a = fma(f, kExpC[3], kExpC[2]), b = fma(f, kExpC[1], kExpC[0]);
+  const double c4 = 1.0 / 24, c5 = 1.0 / 120;
+  const double a = fma(f, c5, c4), b = fma(f, 1.0 / 6, 0.5);
   const double q = fma(f2, fma(f2, a, b), f);
   const double T = tab[n & (kExpTab - 1)];
   const double p = fma(T, q, T);
@@ -265,8 +276,6 @@ __device__ __forceinline__ double exp_neg(double x, const double *__restrict__ t
 // doubles: 64 {1/c_j, -log(1/c_j)} pairs, then 64 {cos, sin}(2 pi j / 64) pairs) and sit in shared memory.
 // ---------------------------------------------------------------------------------
 constexpr int kRngTab = 256;
-__constant__ double kLogC[8] = {6.93147180369123816490e-01, 1.90821492927058770002e-10,  // ln2 hi, lo
-                                1.0 / 7, -1.0 / 6, 1.0 / 5, -1.0 / 4, 1.0 / 3, -1.0 / 2};
 // log(u) for a positive normal u (here u in (0,1)): u = 2^e m, m in [sqrt(1/2), sqrt(2)); the top six bits
 // of m's offset in that range select c_j; r = m / c_j - 1, |r| <= 0.0079;
 // log u = e ln2 - log(1/c_j) + (r - r^2/2 + ... + r^7/7)      (truncation r^8/8 < 2e-18)
@@ -277,14 +286,14 @@ __device__ __forceinline__ double log_pos(double u, const double2 *__restrict__ 
   const double m = __hiloint2double(hx + 0x3fe6a09e, __double2loint(u));
   const double2 t = tab[hx >> 14];
   const double r = fma(m, t.x, -1.0);
-  double p = fma(r, kLogC[2], kLogC[3]);
-  p = fma(p, r, kLogC[4]);
-  p = fma(p, r, kLogC[5]);
-  p = fma(p, r, kLogC[6]);
-  p = fma(p, r, kLogC[7]);
+  double p = fma(r, 1.0 / 7, -1.0 / 6);
+  p = fma(p, r, 1.0 / 5);
+  p = fma(p, r, -0.25);
+  p = fma(p, r, 1.0 / 3);
+  p = fma(p, r, -0.5);
   const double lg = fma(r * r, p, r);
   const double ed = (double)e;
-  return fma(ed, kLogC[0], t.y) + fma(ed, kLogC[1], lg);
+  return fma(ed, 6.93147180369123816490e-01, t.y) + fma(ed, 1.90821492927058770002e-10, lg);  // ln2 hi, lo
 }
 // sqrt(x), x > 0 normal: x * rsqrt(x) with one correction step (error < 1 ulp)
 __device__ __forceinline__ double sqrt_pos(double x) {
@@ -294,16 +303,15 @@ __device__ __forceinline__ double sqrt_pos(double x) {
 }
 // sin and cos of 2 pi u, u in [0,1): u = j/64 + f, |f| <= 1/128 (exact), a = 2 pi f, |a| <= 0.0491;
 // short Taylor polynomials in a (truncation < 5e-18) rotated by the tabulated {cos, sin}(2 pi j/64).
-__constant__ double kSinC[8] = {6.283185307179586, 6755399441055744.0, -1.0 / 6, 1.0 / 120, -1.0 / 5040,
-                                1.0 / 24, -1.0 / 720, 1.0 / 40320};
 __device__ __forceinline__ void sincos_2pi(double u, const double2 *__restrict__ tab, double &sn, double &cs) {
-  const double t = fma(u, 64.0, kSinC[1]);  // round(64 u) in the low mantissa bits
-  const double f = fma(t - kSinC[1], -1.0 / 64, u);
+  constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52
+  const double t = fma(u, 64.0, kMagic);  // round(64 u) in the low mantissa bits
+  const double f = fma(t - kMagic, -1.0 / 64, u);
   const double2 w = tab[__double2loint(t) & 63];
-  const double a = f * kSinC[0];
+  const double a = f * 6.283185307179586;
   const double a2 = a * a;
-  const double sa = fma(a * a2, fma(a2, fma(a2, kSinC[4], kSinC[3]), kSinC[2]), a);          // sin a
-  const double qc = a2 * fma(a2, fma(a2, fma(a2, kSinC[7], kSinC[6]), kSinC[5]), -0.5);      // cos a - 1
+  const double sa = fma(a * a2, fma(a2, fma(a2, -1.0 / 5040, 1.0 / 120), -1.0 / 6), a);           // sin a
+  const double qc = a2 * fma(a2, fma(a2, fma(a2, 1.0 / 40320, -1.0 / 720), 1.0 / 24), -0.5);      // cos a - 1
   cs = fma(-w.y, sa, fma(w.x, qc, w.x));
   sn = fma(w.x, sa, fma(w.y, qc, w.y));
 }
@@ -314,6 +322,17 @@ __device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double
   asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                : "+d"(d0), "+d"(d1)
                : "d"(a), "d"(b));
+}
+
+// Shared-memory stores through an explicit 32-bit shared address that the compiler cannot rematerialise
+// (opaque_u32): keeps one address register live instead of recomputing lane offsets at every store.
+__device__ __forceinline__ uint32_t opaque_u32(uint32_t v) {
+  asm volatile("" : "+r"(v));
+  return v;
+}
+template <int BYTE_OFF>
+__device__ __forceinline__ void sts_f64(uint32_t addr, double v) {
+  asm volatile("st.shared.f64 [%0+%1], %2;" ::"r"(addr), "n"(BYTE_OFF), "d"(v) : "memory");
 }
 
 __device__ __forceinline__ double shfl_d(double v, int src, int width) {

@@ -177,6 +177,9 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
     const int oo = GE::opCol(lane) - lane;                         // operator column relative to the value column (32 or 36)
     const int mshift = GE::mergeShift(fr);
     double *const tl = tile + lane;                                // this lane's value column of the tile
+    // 32-bit shared addresses of the lane's value / operator columns, kept live in registers
+    const uint32_t tl32 = opaque_u32((uint32_t)__cvta_generic_to_shared(tl));
+    const uint32_t to32 = EL ? opaque_u32(tl32 + 8u * (uint32_t)oo) : 0u;
     const double *const afrag = tile + fk * S + fr;                // A fragments: + 4 ks S + tile column
     int chunk = 0;
     double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1.0, r = 1.0, ri = 1.0, gd = 0.0;
@@ -208,12 +211,14 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           const double radlog = fma(sh.kd, ri, -sh.zeta);  // g'/g
           h = fma(-0.5, lapfac, -radlog * gd);
         }
-        double *const tr = tl + ((meta >> 12) & 15) * S;
+        const uint32_t rofs = (uint32_t)(((meta >> 12) & 15) * (S * 8));
+        const uint32_t tr = tl32 + rofs, tro = to32 + rofs;
         // value into column lane, combined operator into column opCol(lane): every lane stores
-        auto put = [&](int t, double phi, double bop) {
-          tr[t * S] = phi;
-          if (EL) tr[t * S + oo] = bop;
-        };
+#define put(t, phi, bop)                          \
+  do {                                            \
+    sts_f64<(t) * S * 8>(tr, (phi));              \
+    if (EL) sts_f64<(t) * S * 8>(tro, (bop));     \
+  } while (0)
         const int kind = meta & 15;
         if (kind == SH_S) {
           put(0, gr, gr * h);
@@ -247,6 +252,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           else { Sh = fma(2.0 * dz, dz, -fma(dx, dx, dy * dy)); gs = 2.0 * fma(2.0 * gJz, dz, -fma(gJx, dx, gJy * dy)); }
           put(0, gr * Sh, gr * fma(Sh, h, -gs));
         }
+#undef put
         const int flush = meta >> 20;
         if (flush) {
           // unused rows of the chunk meet zero rows of C, but must themselves be finite

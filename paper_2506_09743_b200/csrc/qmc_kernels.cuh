@@ -35,8 +35,8 @@ __device__ __forceinline__ void dummy_xyz(int lane, double &x, double &y, double
   z = 0.53 - 0.05 * lane;
 }
 
-template <int NS, int NMO, bool EL, bool X>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
+template <int NS, int NMO, bool EL, bool X, int WPB>
+__global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     local_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
   const double *sC;
@@ -50,7 +50,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
   const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
   const int g = lane / ne, e = lane - g * ne;
   const int64_t n_groups = (io.M + G - 1) / G;
-  const int64_t stride = (int64_t)gridDim.x * kWarpsPerBlock;
+  const int64_t stride = (int64_t)gridDim.x * WPB;
   auto fetch = [&](int64_t grp, double &x, double &y, double &z) {
     const int64_t w = grp * G + g;
     if ((g < G) && (w < io.M)) {
@@ -61,7 +61,7 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
       dummy_xyz(lane, x, y, z);
     }
   };
-  for (int64_t grp = (int64_t)blockIdx.x * kWarpsPerBlock + warp; grp < n_groups; grp += stride) {
+  for (int64_t grp = (int64_t)blockIdx.x * WPB + warp; grp < n_groups; grp += stride) {
     double x, y, z;
     fetch(grp, x, y, z);
     eval_walkers<NS, NMO, EL, X>(P, sExp, sC, sDet, ws, x, y, z, lane);
@@ -86,8 +86,8 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
 }
 
 // Explicit re-evaluation of the groups listed by the fast kernel (rare; see kFallbackRatio).
-template <int NS, int NMO, bool X>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
+template <int NS, int NMO, bool X, int WPB>
+__global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     explicit_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
   const int n_list = *io.fb_count;
@@ -114,12 +114,12 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
     } else {
       dummy_xyz(lane, x, y, z);
     }
-    eval_walkers<NS, NMO, true, X, true>(P, sExp, sC, sDet, ws, x, y, z, lane, warp, kWarpsPerBlock);
+    eval_walkers<NS, NMO, true, X, true>(P, sExp, sC, sDet, ws, x, y, z, lane, warp, WPB);
     __syncthreads();
     if (warp == 0 && lane < G) {
       const int64_t wo = grp * G + lane;
       double sig = 0.0, numk = 0.0;
-      for (int ww = 0; ww < kWarpsPerBlock; ++ww) {
+      for (int ww = 0; ww < WPB; ++ww) {
         const double *res = wsBase + ww * GE::total + GE::oRes + lane * 4;
         sig += res[0];      // eq. 4
         numk += res[1];     // F.2 / F.4 with G.7
@@ -139,8 +139,8 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
 // Persistent all-electron Metropolis (readings Q9, Q10).
 // Walker coordinates and log|Psi| stay in registers for all sweeps.
 // ---------------------------------------------------------------------------------
-template <int NS, int NMO, bool WITH_EL, bool X>
-__global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
+template <int NS, int NMO, bool WITH_EL, bool X, int WPB>
+__global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     metropolis_kernel(const __grid_constant__ SysParams P, const WalkerIO io, const MetroParams mp) {
   extern __shared__ __align__(16) unsigned char smem[];
   const double *sC;
@@ -159,9 +159,9 @@ __global__ void __launch_bounds__(kWarpsPerBlock * 32, QMC_MINBLOCKS)
   const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G, nc = 3 * ne, npair = (nc + 1) / 2;
   const int g = lane / ne, e = lane - g * ne;
   const int64_t n_groups = (io.M + G - 1) / G;
-  const int64_t stride = (int64_t)gridDim.x * kWarpsPerBlock;
+  const int64_t stride = (int64_t)gridDim.x * WPB;
   unsigned long long acc_count = 0;
-  for (int64_t grp = (int64_t)blockIdx.x * kWarpsPerBlock + warp; grp < n_groups; grp += stride) {
+  for (int64_t grp = (int64_t)blockIdx.x * WPB + warp; grp < n_groups; grp += stride) {
     const int64_t w = grp * G + g;
     const bool own = (g < G) && (w < io.M);
     const int rg = (own ? g : 0) * 4;
