@@ -34,7 +34,7 @@ int cuda_fail(cudaError_t e, const char *what) {
 struct Variant {
   int NS, NMO, LP, ws_doubles;
   bool exact;  // compiled for n_up = n_dn = NS
-  const void *k_el, *k_psi, *k_metro, *k_metro_el, *k_expl;
+  const void *k_el, *k_psi, *k_metro, *k_expl;
 };
 
 template <int NS, int NMO, bool X>
@@ -47,8 +47,7 @@ Variant make_variant() {
   v.ws_doubles = Geo<NS, NMO>::total;
   v.k_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl>;
   v.k_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi>;
-  v.k_metro = (const void *)metropolis_kernel<NS, NMO, false, X, kWarpsPsi>;
-  v.k_metro_el = (const void *)metropolis_kernel<NS, NMO, true, X, kWarpsEl>;
+  v.k_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi>;
   v.k_expl = (const void *)explicit_energy_kernel<NS, NMO, X, kWarpsEl>;
   return v;
 }
@@ -87,7 +86,7 @@ struct qmc_system {
   SysParams P{};
   Variant var{};
   int smem_el = 0, smem_psi = 0;  // dynamic shared memory of the E_L kernels (kWarpsEl warps) / values-only kernels
-  int blocks_el = 0, blocks_psi = 0, blocks_metro = 0, blocks_metro_el = 0;
+  int blocks_el = 0, blocks_psi = 0, blocks_metro = 0;
   void *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr;
   int n_sm = 0;
   double *d_stats = nullptr;
@@ -213,18 +212,30 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
       x.k[sp] = k;
     }
   }
-  // determinants with at most one substitution per spin first: the lanes of a warp, which take
-  // consecutive determinants, then run the same code
-  std::stable_sort(excs.begin(), excs.end(), [](const Exc &a, const Exc &b) {
-    auto cls = [](const Exc &x) { const int m = std::max(x.k[0], x.k[1]); return m < 2 ? 0 : (m == 2 ? 1 : 2); };
-    return cls(a) < cls(b);
-  });
-  P.n_det_single = 0;
-  int n_packed = 0;  // determinants with at most two substitutions per spin (packed 16-byte records)
-  for (const Exc &x : excs) {
-    P.n_det_single += (std::max(x.k[0], x.k[1]) < 2) ? 1 : 0;
-    n_packed += (std::max(x.k[0], x.k[1]) <= 2) ? 1 : 0;
-  }
+  // Determinant classes (the lanes of a warp take consecutive determinants of one class and run the same code):
+  //   0  equal to the reference                      -> their coefficients are summed into P.d_ref
+  //   1  one substitution in one spin                 -> one table entry
+  //   2  one substitution in each spin                -> two table entries
+  //   3  two substitutions in one spin, none in the other -> one 2x2 sub-determinant
+  //   4  anything else with at most two per spin      -> two 2x2 sub-determinants (padded with constant entries)
+  //   5  more than two substitutions in a spin        -> general sub-determinants (GenDet)
+  auto det_class = [](const Exc &x) {
+    const int lo = std::min(x.k[0], x.k[1]), hi = std::max(x.k[0], x.k[1]);
+    if (hi > 2) return 5;
+    if (hi == 0) return 0;
+    if (hi == 1) return lo == 0 ? 1 : 2;
+    return lo == 0 ? 3 : 4;
+  };
+  std::stable_sort(excs.begin(), excs.end(), [&](const Exc &a, const Exc &b) { return det_class(a) < det_class(b); });
+  int n_cls[6] = {0, 0, 0, 0, 0, 0};
+  for (const Exc &x : excs) ++n_cls[det_class(x)];
+  const int n_ref = n_cls[0];
+  const int n_packed = n_cls[1] + n_cls[2] + n_cls[3] + n_cls[4];  // packed 16-byte records (classes 1-4)
+  P.d_ref = 0.0;
+  for (int n = 0; n < n_ref; ++n) P.d_ref += excs[n].d;
+  P.n_a1 = n_cls[1];
+  P.n_a2 = P.n_a1 + n_cls[2];
+  P.n_b = P.n_a2 + n_cls[3];
   for (int sp = 0; sp < 2; ++sp) {
     if ((int)virt[sp].size() > kMaxVirt) unsupported = true;
     P.nv[sp] = (int)virt[sp].size();
@@ -263,7 +274,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   const int NMO = var->NMO;
   std::vector<DetRec> dets(n_packed);
   std::vector<GenDet> gens;
-  for (int n = n_packed; n < d->n_det; ++n) {
+  for (int n = n_ref + n_packed; n < d->n_det; ++n) {
     GenDet g{};
     g.d = excs[n].d;
     for (int sp = 0; sp < 2; ++sp) {
@@ -278,23 +289,42 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   P.n_det = n_packed;
   P.n_gen = (int)gens.size();
   {
-    const uint32_t one = (uint32_t)(var->NS * var->LP), zero = one + 1;  // constant table entries (Geo::TS)
+    const int LPv = var->LP, TSv = var->NS * var->LP + 2;       // Geo::TS: table stride per (walker, spin)
+    const uint32_t one = (uint32_t)(var->NS * LPv), zero = one + 1;  // constant table entries {1,0}, {0,0}
+    // byte offset (for 8-byte entries; the E_L tables hold 16-byte {T, M} entries and double it) of entry
+    // (p, q) of spin sp relative to the walker's up-spin table
+    auto off8 = [&](int sp, int p, int q) { return (uint32_t)(8 * (sp * TSv + p * LPv + q)); };
     for (int n = 0; n < n_packed; ++n) {
-      const Exc &x = excs[n];
-      uint32_t code[2];
-      for (int sp = 0; sp < 2; ++sp) {
-        uint32_t i11 = one, i12 = zero, i21 = zero, i22 = one;
-        if (x.k[sp] >= 1) i11 = (uint32_t)(x.p[sp][0] * var->LP + x.q[sp][0]);
-        if (x.k[sp] == 2) {
-          i12 = (uint32_t)(x.p[sp][0] * var->LP + x.q[sp][1]);
-          i21 = (uint32_t)(x.p[sp][1] * var->LP + x.q[sp][0]);
-          i22 = (uint32_t)(x.p[sp][1] * var->LP + x.q[sp][1]);
+      const Exc &x = excs[n_ref + n];
+      const int cls = det_class(x);
+      DetRec &r = dets[n];
+      r.d = x.d;
+      if (cls == 1) {
+        const int sp = x.k[0] ? 0 : 1;
+        r.up = off8(sp, x.p[sp][0], x.q[sp][0]);
+        r.dn = 0;
+      } else if (cls == 2) {
+        r.up = off8(0, x.p[0][0], x.q[0][0]);
+        r.dn = off8(1, x.p[1][0], x.q[1][0]);
+      } else if (cls == 3) {
+        const int sp = x.k[0] ? 0 : 1;
+        r.up = off8(sp, x.p[sp][0], x.q[sp][0]) | (off8(sp, x.p[sp][0], x.q[sp][1]) << 16);  // 11, 12
+        r.dn = off8(sp, x.p[sp][1], x.q[sp][0]) | (off8(sp, x.p[sp][1], x.q[sp][1]) << 16);  // 21, 22
+      } else {
+        uint32_t code[2];
+        for (int sp = 0; sp < 2; ++sp) {
+          uint32_t i11 = one, i12 = zero, i21 = zero, i22 = one;
+          if (x.k[sp] >= 1) i11 = (uint32_t)(x.p[sp][0] * LPv + x.q[sp][0]);
+          if (x.k[sp] == 2) {
+            i12 = (uint32_t)(x.p[sp][0] * LPv + x.q[sp][1]);
+            i21 = (uint32_t)(x.p[sp][1] * LPv + x.q[sp][0]);
+            i22 = (uint32_t)(x.p[sp][1] * LPv + x.q[sp][1]);
+          }
+          code[sp] = i11 | (i12 << 8) | (i21 << 16) | (i22 << 24);
         }
-        code[sp] = i11 | (i12 << 8) | (i21 << 16) | (i22 << 24);
+        r.up = code[0];
+        r.dn = code[1];
       }
-      dets[n].up = code[0];
-      dets[n].dn = code[1];
-      dets[n].d = x.d;
     }
   }
   P.G = std::max(1, std::min(32 / P.n_e, 16 / var->NS));
@@ -466,11 +496,11 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   }
   int blocks_expl = 0;
   s->n_sm = n_sm;
-  const void *ks[5] = {var->k_el, var->k_psi, var->k_metro, var->k_metro_el, var->k_expl};
-  int *nb[5] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro, &s->blocks_metro_el, &blocks_expl};
-  const int kw[5] = {kWarpsEl, kWarpsPsi, kWarpsPsi, kWarpsEl, kWarpsEl};
-  const int ksm[5] = {s->smem_el, s->smem_psi, s->smem_psi, s->smem_el, s->smem_el};
-  for (int i = 0; i < 5; ++i) {
+  const void *ks[4] = {var->k_el, var->k_psi, var->k_metro, var->k_expl};
+  int *nb[4] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro, &blocks_expl};
+  const int kw[4] = {kWarpsEl, kWarpsPsi, kWarpsPsi, kWarpsEl};
+  const int ksm[4] = {s->smem_el, s->smem_psi, s->smem_psi, s->smem_el};
+  for (int i = 0; i < 4; ++i) {
     if ((e = cudaFuncSetAttribute(ks[i], cudaFuncAttributeMaxDynamicSharedMemorySize, ksm[i])) != cudaSuccess) {
       int rc = cuda_fail(e, "cudaFuncSetAttribute");
       qmc_destroy(s);
@@ -552,16 +582,50 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
   mp.sweep0 = (uint32_t)sweep_offset;
   mp.walker_offset = walker_offset;
   mp.accept = d_accept;
-  mp.eloc_acc = d_eloc_acc;
+  mp.resume = 0;
   mp.n_accepted = h_n_accepted ? s->d_counter : nullptr;
   if (h_n_accepted) CK(cudaMemsetAsync(s->d_counter, 0, sizeof(unsigned long long), st));
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
-  const int wpb = d_eloc_acc ? kWarpsEl : kWarpsPsi, smem = d_eloc_acc ? s->smem_el : s->smem_psi;
-  const int64_t need = (groups + wpb - 1) / wpb;
-  const int grid = (int)std::min<int64_t>(need, d_eloc_acc ? s->blocks_metro_el : s->blocks_metro);
+  const int64_t need = (groups + kWarpsPsi - 1) / kWarpsPsi;
+  const int grid = (int)std::min<int64_t>(need, s->blocks_metro);
   void *args[3] = {(void *)&s->P, (void *)&io, (void *)&mp};
-  CK(cudaLaunchKernel(d_eloc_acc ? s->var.k_metro_el : s->var.k_metro, dim3(grid), dim3(wpb * 32), args, smem, st));
-  ++g_launches;
+  if (!d_eloc_acc) {
+    // one persistent launch for all sweeps: coordinates and log|Psi| stay in registers
+    CK(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_psi, st));
+    ++g_launches;
+  } else {
+    // E_L after every sweep (BASELINE config 5): one-sweep launches of the sampler alternate with the
+    // local-energy call (fast kernel + explicit fallback), whose result is added to d_eloc_acc.  The
+    // sampler resumes from the log|Psi| / sign the previous launch stored, so no evaluation is repeated.
+    double *scratch = nullptr;  // [M] E_L of one sweep, then [M] log|Psi|, [M] sign if the caller gave none
+    const size_t n_scr = (size_t)M * (1 + (d_logpsi ? 0 : 1) + (d_sign ? 0 : 1));
+    CK(cudaMallocAsync(&scratch, n_scr * sizeof(double), st));
+    double *nxt = scratch + M;
+    if (!d_logpsi) { io.logpsi = nxt; nxt += M; }
+    if (!d_sign) io.sign = nxt;
+    CK(cudaMemsetAsync(d_eloc_acc, 0, (size_t)M * sizeof(double), st));
+    mp.n_sweeps = 1;
+    if (n_sweeps == 0) {  // nothing to accumulate; still report log|Psi| of the starting positions
+      mp.n_sweeps = 0;
+      CK(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_psi, st));
+      ++g_launches;
+    }
+    for (int32_t sw = 0; sw < n_sweeps; ++sw) {
+      mp.sweep0 = (uint32_t)(sweep_offset + (uint64_t)sw);
+      mp.accept = d_accept ? d_accept + (size_t)sw * (size_t)M : nullptr;
+      mp.resume = sw > 0 ? 1 : 0;
+      CK(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_psi, st));
+      ++g_launches;
+      int rc = launch_eval(s, d_r, M, nullptr, nullptr, scratch, st, true);
+      if (rc != QMC_OK) {
+        cudaFreeAsync(scratch, st);
+        return rc;
+      }
+      accumulate_kernel<<<(unsigned)std::min<int64_t>((M + 255) / 256, 4 * s->n_sm), 256, 0, st>>>(d_eloc_acc, scratch, M);
+      ++g_launches;
+    }
+    CK(cudaFreeAsync(scratch, st));
+  }
   if (h_n_accepted) {
     unsigned long long v = 0;
     CK(cudaMemcpyAsync(&v, s->d_counter, sizeof(v), cudaMemcpyDeviceToHost, st));

@@ -59,9 +59,10 @@ constexpr int kMetaK1 = 1 << 4, kMetaK2 = 2 << 4;
 constexpr int kChunk = QMC_CHUNK;
 constexpr int kExpTab = 64;  // entries of the 2^(j/64) table of exp_neg
 
-// One determinant relative to the reference, per spin four table indices (p*LP+q) of the 2x2
-// sub-block {11, 12, 21, 22}; unused slots point at the constant entries TS-2 (= 1.0 in T, 0 in M)
-// and TS-1 (= 0.0), so k = 0, 1, 2 substitutions share one formula.  16 bytes.
+// One determinant relative to the reference; the meaning of the two words depends on the class (qmc_setup):
+// one or two byte offsets of table entries (class 1, 2), four 16-bit byte offsets {11,12 | 21,22} of a 2x2
+// block (class 3), or per spin four 8-bit entry indices {11,12,21,22} where unused slots point at the
+// constant entries TS-2 (= 1.0 in T, 0 in M) and TS-1 (= 0.0) (class 4).  16 bytes.
 struct __align__(16) DetRec {
   uint32_t up, dn;  // 4 x uint8 each
   double d;
@@ -93,7 +94,9 @@ constexpr double kFallbackRatio = 1024.0;  // measured: E_L error ~ 1.2e-15 (Sig
 struct SysParams {  // passed by value to every kernel
   int n_atoms, n_up, n_dn, n_e;
   int n_shell, n_ao, n_mo, n_det;  // n_mo = orbitals referenced (kernel order)
-  int n_det_single;                // determinants [0, n_det_single) have at most one substitution per spin
+  int n_a1, n_a2, n_b;             // class boundaries in dets[]: [0,n_a1) one entry, [n_a1,n_a2) two entries,
+                                   // [n_a2,n_b) one 2x2 block, [n_b,n_det) two 2x2 blocks (qmc_setup)
+  double d_ref;                    // summed coefficients of the determinants equal to the reference
   int nv[2];                       // virtual orbitals per spin
   int G;                           // walkers per warp pass
   int smem_const_bytes;
@@ -133,7 +136,8 @@ struct MetroParams {
   uint32_t sweep0;
   int64_t walker_offset;
   uint8_t *accept;       // [n_sweeps][M] or null
-  double *eloc_acc;      // [M] or null
+  int resume;            // 1: log|Psi| and sign of the starting positions are in io.logpsi / io.sign (as a
+                         // previous launch left them) instead of being evaluated
   unsigned long long *n_accepted;  // device counter or null
 };
 

@@ -13,18 +13,6 @@ namespace qmc {
 // idx packs four uint8 table indices {11, 12, 21, 22}.
 // For E_L the two tables are interleaved, entry = {T, Mt} (one 16-byte load per entry).
 template <bool EL>
-__device__ __forceinline__ void excite_single(uint32_t idx, const double *__restrict__ T, double &R, double &Rd) {
-  const int i = idx & 255;
-  if (EL) {
-    const double2 v = reinterpret_cast<const double2 *>(T)[i];
-    R = v.x;
-    Rd = v.y;
-  } else {
-    R = T[i];
-    Rd = 0.0;
-  }
-}
-template <bool EL>
 __device__ __forceinline__ void excite_double(uint32_t idx, const double *__restrict__ T, double &R, double &Rd) {
   const int i11 = idx & 255, i12 = (idx >> 8) & 255, i21 = (idx >> 16) & 255, i22 = idx >> 24;
   if (EL) {
@@ -547,19 +535,50 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
     const bool wvalid = wg < G;
     const int pu = 2 * (wvalid ? wg : 0), pd = pu + 1;
     const double *Tu = sT + (EL ? 2 : 1) * pu * TS, *Td = sT + (EL ? 2 : 1) * pd * TS;
-    double den = 0.0, num = 0.0;
-    // determinants with at most one substitution per spin: one table entry per spin
-    for (int n = sub; n < P.n_det_single; n += LW) {
+    double den = (sub == 0) ? P.d_ref : 0.0, num = 0.0;  // determinants equal to the reference: R = 1, Rd = 0
+    // table entry at byte offset off8 (in units of 8-byte entries) from the walker's up-spin table
+    const char *Tb = reinterpret_cast<const char *>(Tu);
+    auto entry = [&](uint32_t off8, double &R, double &D) {
+      if (EL) {
+        const double2 v = *reinterpret_cast<const double2 *>(Tb + 2 * off8);
+        R = v.x;
+        D = v.y;
+      } else {
+        R = *reinterpret_cast<const double *>(Tb + off8);
+        D = 0.0;
+      }
+    };
+    // class 1: one substitution in one spin -- one table entry
+    for (int n = sub; n < P.n_a1; n += LW) {
+      const DetRec dr = sDet[n];
+      double R, D;
+      entry(dr.up, R, D);
+      den = fma(dr.d, R, den);
+      if (EL) num = fma(dr.d, D, num);
+    }
+    // class 2: one substitution in each spin -- two table entries
+    for (int n = P.n_a1 + sub; n < P.n_a2; n += LW) {
       const DetRec dr = sDet[n];
       double Ru, Du, Rd, Dd;
-      excite_single<EL>(dr.up, Tu, Ru, Du);
-      excite_single<EL>(dr.dn, Td, Rd, Dd);
+      entry(dr.up, Ru, Du);
+      entry(dr.dn, Rd, Dd);
       const double w = dr.d * Ru;
       den = fma(w, Rd, den);
       if (EL) num = fma(dr.d, Du * Rd, fma(w, Dd, num));
     }
-    // the rest: 2x2 sub-determinants
-    for (int n = P.n_det_single + sub; n < P.n_det; n += LW) {
+    // class 3: two substitutions in one spin, the other spin as in the reference -- one 2x2 block
+    for (int n = P.n_a2 + sub; n < P.n_b; n += LW) {
+      const DetRec dr = sDet[n];
+      double a, am, b, bm, c, cm, d, dm;
+      entry(dr.up & 0xffffu, a, am);
+      entry(dr.up >> 16, b, bm);
+      entry(dr.dn & 0xffffu, c, cm);
+      entry(dr.dn >> 16, d, dm);
+      den = fma(dr.d, fma(a, d, -b * c), den);
+      if (EL) num = fma(dr.d, fma(d, am, fma(a, dm, -fma(b, cm, c * bm))), num);
+    }
+    // class 4: the rest with at most two per spin -- 2x2 sub-determinants in both spins
+    for (int n = P.n_b + sub; n < P.n_det; n += LW) {
       const DetRec dr = sDet[n];
       double Ru, Du, Rd, Dd;
       excite_double<EL>(dr.up, Tu, Ru, Du);

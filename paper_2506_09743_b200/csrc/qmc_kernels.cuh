@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
 // Persistent all-electron Metropolis (readings Q9, Q10).
 // Walker coordinates and log|Psi| stay in registers for all sweeps.
 // ---------------------------------------------------------------------------------
-template <int NS, int NMO, bool WITH_EL, bool X, int WPB>
+template <int NS, int NMO, bool X, int WPB>
 __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     metropolis_kernel(const __grid_constant__ SysParams P, const WalkerIO io, const MetroParams mp) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -173,9 +173,13 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     } else {
       dummy_xyz(lane, x, y, z);
     }
-    double lp = 0.0, sg = 0.0, eacc = 0.0;
-    // sweep -1 evaluates the starting point (always "accepted", no draws)
-    for (int sw = -1; sw < mp.n_sweeps; ++sw) {
+    double lp = 0.0, sg = 0.0;
+    if (mp.resume && own) {
+      lp = io.logpsi[w];
+      sg = io.sign[w];
+    }
+    // sweep -1 evaluates the starting point (always "accepted", no draws) unless a previous launch left it
+    for (int sw = mp.resume ? 0 : -1; sw < mp.n_sweeps; ++sw) {
       double xp = x, yp = y, zp = z, logu = 0.0;
       if (sw >= 0) {
         // --- draws: lanes share the (walker, pair) Philox blocks of the G walkers
@@ -215,11 +219,6 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
         acc_count += ok ? 1 : 0;
       }
       __syncwarp();
-      if (WITH_EL && sw >= 0) {
-        eval_walkers<NS, NMO, true, X>(P, sExp, sC, sDet, ws, x, y, z, lane);
-        eacc += sRes[rg + 2];
-        __syncwarp();
-      }
     }
     if (own) {
       io.r_out[((int64_t)e * 3 + 0) * io.M + w] = x;
@@ -228,7 +227,6 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
       if (e == 0) {
         if (io.logpsi) io.logpsi[w] = lp;
         if (io.sign) io.sign[w] = sg;
-        if (WITH_EL) mp.eloc_acc[w] = eacc;
       }
     }
     __syncwarp();
@@ -237,6 +235,11 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     for (int m = 16; m > 0; m >>= 1) acc_count += __shfl_xor_sync(0xffffffffu, acc_count, m);
     if (lane == 0 && acc_count) atomicAdd(mp.n_accepted, acc_count);
   }
+}
+
+// acc[i] += x[i]  (E_L on every sweep, BASELINE config 5)
+__global__ void __launch_bounds__(256) accumulate_kernel(double *__restrict__ acc, const double *__restrict__ x, int64_t M) {
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < M; i += (int64_t)gridDim.x * blockDim.x) acc[i] += x[i];
 }
 
 // ---------------------------------------------------------------------------------
