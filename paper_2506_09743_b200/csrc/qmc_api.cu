@@ -86,7 +86,7 @@ struct qmc_system {
   SysParams P{};
   Variant var{};
   int smem_el = 0, smem_psi = 0;  // dynamic shared memory of the E_L kernels (kWarpsEl warps) / values-only kernels
-  int blocks_el = 0, blocks_psi = 0, blocks_metro = 0;
+  int blocks_el = 0, blocks_psi = 0, blocks_metro = 0, blocks_expl = 0;
   void *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr;
   int n_sm = 0;
   double *d_stats = nullptr;
@@ -494,10 +494,9 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     qmc_destroy(s);
     return QMC_EUNSUPPORTED;
   }
-  int blocks_expl = 0;
   s->n_sm = n_sm;
   const void *ks[4] = {var->k_el, var->k_psi, var->k_metro, var->k_expl};
-  int *nb[4] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro, &blocks_expl};
+  int *nb[4] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro, &s->blocks_expl};
   const int kw[4] = {kWarpsEl, kWarpsPsi, kWarpsPsi, kWarpsEl};
   const int ksm[4] = {s->smem_el, s->smem_psi, s->smem_psi, s->smem_el};
   for (int i = 0; i < 4; ++i) {
@@ -533,19 +532,26 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
   const int wpb = el ? kWarpsEl : kWarpsPsi, smem = el ? s->smem_el : s->smem_psi;
   const int64_t need = (groups + wpb - 1) / wpb;
   const int grid = (int)std::min<int64_t>(need, el ? s->blocks_el : s->blocks_psi);
-  int *fb = nullptr;
+  double *fb = nullptr;
   const bool fallback = el && s->P.n_det_all > 1;  // a single determinant has no reference to be ill-conditioned against
-  if (fallback) {  // work list of the explicit fallback: [0] = counter, [1..] = group indices (stream-ordered scratch)
-    CK(cudaMallocAsync(&fb, (size_t)(groups + 1) * sizeof(int), st));
-    CK(cudaMemsetAsync(fb, 0, sizeof(int), st));
-    io.fb_count = fb;
-    io.fb_list = fb + 1;
+  const int64_t expl_warps = (int64_t)s->blocks_expl * kWarpsEl;
+  if (fallback) {
+    // stream-ordered scratch of the explicit fallback: partial sums [groups + warps][G][2] doubles, then
+    // ints: [0] = counter, [1 ..] = listed group indices, then the per-group slice counters
+    const size_t n_part = (size_t)(groups + expl_warps) * (size_t)s->P.G * 2;
+    CK(cudaMallocAsync(&fb, n_part * sizeof(double) + (size_t)(2 * groups + 2) * sizeof(int), st));
+    int *fbi = reinterpret_cast<int *>(fb + n_part);
+    CK(cudaMemsetAsync(fbi, 0, sizeof(int), st));
+    io.fb_part = fb;
+    io.fb_count = fbi;
+    io.fb_list = fbi + 1;
+    io.fb_done = fbi + 1 + groups;
   }
   void *args[2] = {(void *)&s->P, (void *)&io};
   CK(cudaLaunchKernel(el ? s->var.k_el : s->var.k_psi, dim3(grid), dim3(wpb * 32), args, smem, st));
   ++g_launches;
   if (fallback) {
-    CK(cudaLaunchKernel(s->var.k_expl, dim3(grid), dim3(kWarpsEl * 32), args, s->smem_el, st));
+    CK(cudaLaunchKernel(s->var.k_expl, dim3(s->blocks_expl), dim3(kWarpsEl * 32), args, s->smem_el, st));
     ++g_launches;
     CK(cudaFreeAsync(fb, st));
   }

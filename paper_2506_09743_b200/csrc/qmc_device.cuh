@@ -86,10 +86,11 @@ struct DetCols {
   double d;
 };
 
-// |Sigma / D_0| above which a walker is re-evaluated with every determinant eliminated explicitly:
-// the table path (F.6/F.7) loses about log10((Sigma/D_0)^2) digits when the reference determinant
-// is nearly singular while the expansion is not.
-constexpr double kFallbackRatio = 1024.0;  // measured: E_L error ~ 1.2e-15 (Sigma/D_0)^2  ->  1.3e-9 at the threshold
+// A walker is re-evaluated with every determinant eliminated explicitly when (Sigma / D_0)^2 exceeds
+// kFallbackK max(1, |E_L|): the table path (F.6/F.7) loses about log10((Sigma/D_0)^2) digits when the
+// reference determinant is nearly singular while the expansion is not.  Measured:
+// E_L error ~ 1.2e-15 (Sigma/D_0)^2, so K = 8e5 keeps it below 1e-9 max(1, |E_L|), a tenth of the parity bound.
+constexpr double kFallbackK = 8.0e5;
 
 struct SysParams {  // passed by value to every kernel
   int n_atoms, n_up, n_dn, n_e;
@@ -123,6 +124,8 @@ struct WalkerIO {
   // explicit-fallback work list: groups whose walkers need re-evaluation (filled by the fast kernel)
   int *fb_list;        // device [ceil(M / G)] group indices, or null
   int *fb_count;       // device counter
+  int *fb_done;        // device [ceil(M / G)] per listed group: slices finished (zeroed when the group is listed)
+  double *fb_part;     // device [items][G][2] partial sums {Sigma, Sum d D t} of the explicit kernel's work items
   const double *r_in;  // [n_e][3][M]
   double *r_out;       // Metropolis: same buffer
   double *logpsi, *sign, *eloc;

@@ -301,7 +301,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
   if (EXPL) {
     // ---- explicit path (Fig. 11's "explicit"): every determinant is eliminated on its own,
     // D_n = det A_n, t_n = Tr(A_n^-1 B_n) (G.7 with the combined operator); no excitation tables.
-    // Used for walkers whose reference determinant is nearly singular (kFallbackRatio).
+    // Used for walkers whose reference determinant is nearly singular (kFallbackK).
     const int c = lane % LP, slot = lane / LP, gbase = lane - c;
     const int nprob = 2 * G;
     double sig = 0.0, numk = 0.0;
@@ -615,8 +615,11 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       const double sgn = sProb[pu * 4 + 1] * sProb[pd * 4 + 1];
       sRes[wg * 4 + 0] = Jsum + lu + ld + log(fabs(den));
       sRes[wg * 4 + 1] = sgn * ((den > 0.0) ? 1.0 : ((den < 0.0) ? -1.0 : 0.0));
-      if (EL) sRes[wg * 4 + 2] = esum + (sProb[pu * 4 + 2] + sProb[pd * 4 + 2]) + num / den + P.vnn;
-      sRes[wg * 4 + 3] = (fabs(den) <= kFallbackRatio) ? 0.0 : 1.0;  // also set for NaN (singular reference)
+      const double eloc = EL ? esum + (sProb[pu * 4 + 2] + sProb[pd * 4 + 2]) + num / den + P.vnn : 0.0;
+      if (EL) sRes[wg * 4 + 2] = eloc;
+      // explicit fallback when the estimated table-path error 1.2e-15 (Sigma/D_0)^2 exceeds a tenth of the
+      // parity bound 1e-8 max(1, |E_L|); also set for NaN (singular reference)
+      sRes[wg * 4 + 3] = (den * den <= kFallbackK * fmax(1.0, fabs(eloc))) ? 0.0 : 1.0;
     }
   }
   __syncwarp();

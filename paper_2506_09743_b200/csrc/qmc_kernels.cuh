@@ -79,13 +79,21 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     // walkers whose reference determinant is nearly singular go to the explicit kernel
     if (EL && io.fb_list) {
       const unsigned any = __ballot_sync(0xffffffffu, flagged);
-      if (any && lane == 0) io.fb_list[atomicAdd(io.fb_count, 1)] = (int)grp;
+      if (any && lane == 0) {
+        const int idx = atomicAdd(io.fb_count, 1);
+        io.fb_list[idx] = (int)grp;
+        io.fb_done[idx] = 0;
+      }
     }
     __syncwarp();
   }
 }
 
-// Explicit re-evaluation of the groups listed by the fast kernel (rare; see kFallbackRatio).
+// Explicit re-evaluation of the groups listed by the fast kernel (rare; see kFallbackK).
+// Work item = (listed group, determinant slice): the determinants of a group are dealt over SL warps of
+// the whole grid, every warp rebuilds the MO rows of its group, eliminates its determinants and stores
+// its partial sums; the warp that finishes a group last adds the partials in slice order (deterministic)
+// and writes the outputs.
 template <int NS, int NMO, bool X, int WPB>
 __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     explicit_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
@@ -102,9 +110,14 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   double *ws = wsBase + warp * GE::total;
   const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
   const int g = lane / ne, e = lane - g * ne;
-  // one block per listed group: every warp rebuilds the MO rows, the determinants are dealt over the warps
-  for (int it = blockIdx.x; it < n_list; it += gridDim.x) {
-    const int64_t grp = io.fb_list[it];
+  const int total_warps = (int)gridDim.x * WPB;
+  int SL = total_warps / n_list;                       // slices per group
+  SL = min(SL, (P.n_det_all + 3) / 4);                 // at least ~4 determinants per slice
+  SL = max(SL, 1);
+  const int64_t n_items = (int64_t)n_list * SL;
+  for (int64_t item = (int64_t)blockIdx.x * WPB + warp; item < n_items; item += total_warps) {
+    const int entry = (int)(item / SL), slice = (int)(item - (int64_t)entry * SL);
+    const int64_t grp = io.fb_list[entry];
     const int64_t w = grp * G + g;
     double x, y, z;
     if ((g < G) && (w < io.M)) {
@@ -114,24 +127,32 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     } else {
       dummy_xyz(lane, x, y, z);
     }
-    eval_walkers<NS, NMO, true, X, true>(P, sExp, sC, sDet, ws, x, y, z, lane, warp, WPB);
-    __syncthreads();
-    if (warp == 0 && lane < G) {
+    eval_walkers<NS, NMO, true, X, true>(P, sExp, sC, sDet, ws, x, y, z, lane, slice, SL);
+    const double *res = ws + GE::oRes + (lane < G ? lane : 0) * 4;  // {Sigma, Sum d D t, J, energy share}
+    if (lane < G) {
+      io.fb_part[(item * G + lane) * 2 + 0] = res[0];   // eq. 4
+      io.fb_part[(item * G + lane) * 2 + 1] = res[1];   // F.2 / F.4 with G.7
+    }
+    __threadfence();
+    int last = 0;
+    if (lane == 0) last = (atomicAdd(io.fb_done + entry, 1) == SL - 1) ? 1 : 0;
+    last = __shfl_sync(0xffffffffu, last, 0);
+    if (last) {
+      __threadfence();
       const int64_t wo = grp * G + lane;
-      double sig = 0.0, numk = 0.0;
-      for (int ww = 0; ww < WPB; ++ww) {
-        const double *res = wsBase + ww * GE::total + GE::oRes + lane * 4;
-        sig += res[0];      // eq. 4
-        numk += res[1];     // F.2 / F.4 with G.7
-      }
-      const double *mine = ws + GE::oRes + lane * 4;
-      if (wo < io.M) {
-        if (io.logpsi) io.logpsi[wo] = mine[2] + log(fabs(sig));
+      if (lane < G && wo < io.M) {
+        double sig = 0.0, numk = 0.0;
+        for (int sl = 0; sl < SL; ++sl) {
+          const double *pp = io.fb_part + (((int64_t)entry * SL + sl) * G + lane) * 2;
+          sig += __ldcg(pp);
+          numk += __ldcg(pp + 1);
+        }
+        if (io.logpsi) io.logpsi[wo] = res[2] + log(fabs(sig));
         if (io.sign) io.sign[wo] = (sig > 0.0) ? 1.0 : ((sig < 0.0) ? -1.0 : 0.0);
-        if (io.eloc) io.eloc[wo] = mine[3] + numk / sig + P.vnn;
+        if (io.eloc) io.eloc[wo] = res[3] + numk / sig + P.vnn;
       }
     }
-    __syncthreads();
+    __syncwarp();
   }
 }
 
