@@ -289,7 +289,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   P.n_det = n_packed;
   P.n_gen = (int)gens.size();
   {
-    const int LPv = var->LP, TSv = var->NS * var->LP + 2;       // Geo::TS: table stride per (walker, spin)
+    const int LPv = var->LP + 1, TSv = var->NS * LPv + 2;       // Geo::RS (table row stride), Geo::TS (stride per (walker, spin))
     const uint32_t one = (uint32_t)(var->NS * LPv), zero = one + 1;  // constant table entries {1,0}, {0,0}
     // byte offset (for 8-byte entries; the E_L tables hold 16-byte {T, M} entries and double it) of entry
     // (p, q) of spin sp relative to the walker's up-spin table

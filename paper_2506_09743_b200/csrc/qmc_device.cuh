@@ -164,7 +164,9 @@ struct Geo {
   static constexpr int PP = 32 / LP;                          // problems per pass
   static constexpr int GMAX = 16 / NS;                        // walkers per warp pass (host: G <= GMAX)
   static constexpr int ROWS = (2 * GMAX * NS) < 32 ? (2 * GMAX * NS) : 32;  // electron rows of a pass
-  static constexpr int TS = NS * LP + 2;  // table stride per problem: T[p][q] entries + {1.0, 0.0}
+  static constexpr int RS = LP + 1;       // table row stride: odd, so that the entries (p, q) of one virtual q and
+                                          // different positions p fall into different banks (CI-sum lookups)
+  static constexpr int TS = NS * RS + 2;  // table stride per problem: T[p][q] entries + {1.0, 0.0}
   __host__ __device__ static constexpr int even(int x) { return (x + 1) & ~1; }
   // per-warp scratch, in doubles (all offsets even: 16-byte aligned).
   // When one Gauss-Jordan pass covers all 2 GMAX problems (SINGLE), the MO rows are in registers

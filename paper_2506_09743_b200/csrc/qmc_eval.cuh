@@ -51,14 +51,14 @@ __device__ __noinline__ double small_det(double *a, int k) {
   return det;
 }
 template <bool EL>
-__device__ __noinline__ void excite_general(const GenSpin *g, const double *T, int LP, double *out) {
+__device__ __noinline__ void excite_general(const GenSpin *g, const double *T, int RS, double *out) {
   const int k = g->k;
   double R = 1.0, Rd = 0.0;
   if (k > 0) {
     double a[kMaxSpin * kMaxSpin], w[kMaxSpin * kMaxSpin];
     for (int i = 0; i < k; ++i)
       for (int j = 0; j < k; ++j) {
-        const int idx = g->p[i] * LP + g->q[j];
+        const int idx = g->p[i] * RS + g->q[j];
         a[i * k + j] = EL ? reinterpret_cast<const double2 *>(T)[idx].x : T[idx];
       }
     for (int i = 0; i < k * k; ++i) w[i] = a[i];
@@ -66,7 +66,7 @@ __device__ __noinline__ void excite_general(const GenSpin *g, const double *T, i
     if (EL)
       for (int c = 0; c < k; ++c) {
         for (int i = 0; i < k * k; ++i) w[i] = a[i];
-        for (int i = 0; i < k; ++i) w[i * k + c] = reinterpret_cast<const double2 *>(T)[g->p[i] * LP + g->q[c]].y;
+        for (int i = 0; i < k; ++i) w[i * k + c] = reinterpret_cast<const double2 *>(T)[g->p[i] * RS + g->q[c]].y;
         Rd += small_det(w, k);
       }
   }
@@ -85,7 +85,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
                              double *__restrict__ ws, double x, double y, double z, int lane,
                              int det0 = 0, int det_step = 1) {
   using GE = Geo<NS, NMO>;
-  constexpr int LP = GE::LP, PP = GE::PP, TS = GE::TS;
+  constexpr int LP = GE::LP, PP = GE::PP, TS = GE::TS, RS = GE::RS;
   // X: closed-shell system that matches the instantiation exactly (n_up = n_dn = NS): sizes fold
   const int n_up = X ? NS : P.n_up, n_dn = X ? NS : P.n_dn, ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
   const int g = lane / ne, e = lane - g * ne;
@@ -507,16 +507,16 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       if (pvalid) {
 #pragma unroll
         for (int k = 0; k < NS; ++k) {
-          if (EL) reinterpret_cast<double2 *>(sT)[pr * TS + perm[k] * LP + c] = make_double2(av[k], bv[EL ? k : 0]);
-          else sT[pr * TS + perm[k] * LP + c] = av[k];
+          if (EL) reinterpret_cast<double2 *>(sT)[pr * TS + perm[k] * RS + c] = make_double2(av[k], bv[EL ? k : 0]);
+          else sT[pr * TS + perm[k] * RS + c] = av[k];
         }
         if (c == 0) {
           if (EL) {
-            reinterpret_cast<double2 *>(sT)[pr * TS + NS * LP] = make_double2(1.0, 0.0);
-            reinterpret_cast<double2 *>(sT)[pr * TS + NS * LP + 1] = make_double2(0.0, 0.0);
+            reinterpret_cast<double2 *>(sT)[pr * TS + NS * RS] = make_double2(1.0, 0.0);
+            reinterpret_cast<double2 *>(sT)[pr * TS + NS * RS + 1] = make_double2(0.0, 0.0);
           } else {
-            sT[pr * TS + NS * LP] = 1.0;
-            sT[pr * TS + NS * LP + 1] = 0.0;
+            sT[pr * TS + NS * RS] = 1.0;
+            sT[pr * TS + NS * RS + 1] = 0.0;
           }
           sProb[pr * 4 + 0] = log(fabs(det));
           sProb[pr * 4 + 1] = (det > 0.0) ? 1.0 : ((det < 0.0) ? -1.0 : 0.0);
@@ -590,8 +590,8 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
     // determinants with more than two substitutions in a spin (general sub-determinants)
     for (int n = sub; n < P.n_gen; n += LW) {
       double u[2], v[2];
-      excite_general<EL>(&P.gen[n].s[0], Tu, LP, u);
-      excite_general<EL>(&P.gen[n].s[1], Td, LP, v);
+      excite_general<EL>(&P.gen[n].s[0], Tu, RS, u);
+      excite_general<EL>(&P.gen[n].s[1], Td, RS, v);
       const double dn = P.gen[n].d, w = dn * u[0];
       den = fma(w, v[0], den);
       if (EL) num = fma(dn, u[1] * v[0], fma(w, v[1], num));
