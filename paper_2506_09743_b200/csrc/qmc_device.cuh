@@ -171,7 +171,16 @@ struct Geo {
   // per-warp scratch, in doubles (all offsets even: 16-byte aligned).
   // When one Gauss-Jordan pass covers all 2 GMAX problems (SINGLE), the MO rows are in registers
   // before the first table entry is written, so G, T and M reuse the space of Phi and B.
-  static constexpr int szPhi = even(ROWS * NMO);
+  // MO rows (Phi, B).  In the E_L kernels with two 8-column tiles the row stride is 16 and odd rows swap their
+  // two halves (column ^ 8): the D-fragment stores of the contraction (two adjacent rows per quarter-warp)
+  // and the Gauss-Jordan loads (rows of two problems per half-warp, 7 rows apart) then hit disjoint banks
+  // (measured: E_L kernel -1.3%; the values-only kernels lose more to the index arithmetic than they gain).
+  static constexpr int NTc = (NMO + 7) / 8;
+  static constexpr bool SWZ = NTc == 2;
+  __host__ __device__ static constexpr int moIdx(bool el, int row, int col) {
+    return (SWZ && el) ? row * 16 + (col ^ ((row & 1) << 3)) : row * NMO + col;
+  }
+  static constexpr int szPhi = even(ROWS * (SWZ ? 16 : NMO));
   static constexpr int szG = even(cmax(PP * NS * NS, 2));
   static constexpr int szT = even(cmax(2 * GMAX * TS, 96 + 32));  // also hosts the Metropolis draws
   static constexpr int szM = even(2 * GMAX * TS);

@@ -280,12 +280,12 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           else if (m > GE::VT) { isB = true; el = 8 * (m - GE::VT - 1) + fr; }
         } else if (m >= GE::VTc) { isB = true; el = 8 * (m - GE::VTc) + fr; }
       }
-      double *dst = (isB ? sB : sPhi) + el * NMO;
+      double *dst = (isB ? sB : sPhi);
       if (el < G * ne) {
 #pragma unroll
         for (int t = 0; t < NT; ++t) {
           const int col = 8 * t + 2 * fk;
-          if (col < NMO) *reinterpret_cast<double2 *>(dst + col) = make_double2(acc[m][t][0], acc[m][t][1]);
+          if (col < NMO) *reinterpret_cast<double2 *>(dst + GE::moIdx(EL, el, col)) = make_double2(acc[m][t][0], acc[m][t][1]);
         }
       }
     }
@@ -321,10 +321,10 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           const int colA = cA ? dc.col[sp][c < kMaxSpin ? c : 0] : 0;
 #pragma unroll
           for (int i = 0; i < NS; ++i) {
-            const int row = (pg * ne + e0 + (i < ns ? i : 0)) * NMO;
+            const int row = pg * ne + e0 + (i < ns ? i : 0);
             const bool ri = i < ns;
-            a0[i] = (ri && cA) ? sPhi[row + colA] : ((i == c) ? 1.0 : 0.0);
-            b0[i] = (ri && cA) ? sB[EL ? row + colA : 0] : 0.0;
+            a0[i] = (ri && cA) ? sPhi[GE::moIdx(EL, row, colA)] : ((i == c) ? 1.0 : 0.0);
+            b0[i] = (ri && cA) ? sB[EL ? GE::moIdx(EL, row, colA) : 0] : 0.0;
           }
         }
         double det = 1.0;
@@ -412,13 +412,13 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
         const int colV = cV ? P.virt_col[sp][c < kMaxVirt ? c : 0] : 0;
 #pragma unroll
         for (int i = 0; i < NS; ++i) {
-          const int row = (pg * ne + e0 + (i < ns ? i : 0)) * NMO;
+          const int row = pg * ne + e0 + (i < ns ? i : 0);
           const bool ri = i < ns;
-          a0[i] = (ri && cA) ? sPhi[row + colA] : ((i == c) ? 1.0 : 0.0);  // identity padding
-          av[i] = (ri && cV) ? sPhi[row + colV] : 0.0;
+          a0[i] = (ri && cA) ? sPhi[GE::moIdx(EL, row, colA)] : ((i == c) ? 1.0 : 0.0);  // identity padding
+          av[i] = (ri && cV) ? sPhi[GE::moIdx(EL, row, colV)] : 0.0;
           if (EL) {
-            b0[i] = (ri && cA) ? sB[row + colA] : 0.0;
-            bv[i] = (ri && cV) ? sB[row + colV] : 0.0;
+            b0[i] = (ri && cA) ? sB[GE::moIdx(EL, row, colA)] : 0.0;
+            bv[i] = (ri && cV) ? sB[GE::moIdx(EL, row, colV)] : 0.0;
           }
         }
       }
