@@ -122,7 +122,9 @@ int qmc_log_psi(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi,
  *   d_sign     device, out: [M]                                    (may be NULL)
  *   d_accept   device, out: uint8 [n_sweeps][M] accept mask        (may be NULL)
  *   d_eloc_acc device, out: [M] sum over the sweeps of E_L evaluated after each sweep
- *              (BASELINE config 5: "E_L on every sweep")           (may be NULL)
+ *              (BASELINE config 5: "E_L on every sweep"); when given, the call alternates
+ *              one-sweep sampler launches with the full qmc_local_energy path, so the
+ *              energies carry the explicit fallback correction          (may be NULL)
  *   h_n_accepted host, out: total number of accepted moves; if non-NULL the call
  *              synchronises cuda_stream                              (may be NULL)
  * sweep_offset + n_sweeps must be < 2^32. */
