@@ -100,6 +100,13 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   extern __shared__ __align__(16) unsigned char smem[];
   const int n_list = *io.fb_count;
   if (n_list == 0) return;
+  const int total_warps = (int)gridDim.x * WPB;
+  int SL = total_warps / n_list;                       // slices per group
+  SL = min(SL, (P.n_det_all + 3) / 4);                 // at least ~4 determinants per slice
+  SL = max(SL, 1);
+  const int64_t n_items = (int64_t)n_list * SL;
+  // items are dealt block-first (item = round * grid + block), so few items spread over many SMs
+  if ((int64_t)blockIdx.x >= n_items) return;          // nothing for this block: skip the constants
   const double *sC;
   const double *sExp;
   const DetRec *sDet;
@@ -110,12 +117,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   double *ws = wsBase + warp * GE::total;
   const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
   const int g = lane / ne, e = lane - g * ne;
-  const int total_warps = (int)gridDim.x * WPB;
-  int SL = total_warps / n_list;                       // slices per group
-  SL = min(SL, (P.n_det_all + 3) / 4);                 // at least ~4 determinants per slice
-  SL = max(SL, 1);
-  const int64_t n_items = (int64_t)n_list * SL;
-  for (int64_t item = (int64_t)blockIdx.x * WPB + warp; item < n_items; item += total_warps) {
+  for (int64_t item = (int64_t)warp * gridDim.x + blockIdx.x; item < n_items; item += total_warps) {
     const int entry = (int)(item / SL), slice = (int)(item - (int64_t)entry * SL);
     const int64_t grp = io.fb_list[entry];
     const int64_t w = grp * G + g;
@@ -139,14 +141,23 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     last = __shfl_sync(0xffffffffu, last, 0);
     if (last) {
       __threadfence();
+      // slice-ordered sums, the slices dealt over the lanes (fixed tree: deterministic); lane gw keeps walker gw
+      double sig = 0.0, numk = 0.0;
+      for (int gw = 0; gw < G; ++gw) {
+        double a = 0.0, b = 0.0;
+        for (int sl = lane; sl < SL; sl += 32) {
+          const double *pp = io.fb_part + (((int64_t)entry * SL + sl) * G + gw) * 2;
+          a += __ldcg(pp);       // eq. 4
+          b += __ldcg(pp + 1);   // F.2 / F.4 with G.7
+        }
+        for (int m = 16; m > 0; m >>= 1) {
+          a += shfl_xor_d(a, m);
+          b += shfl_xor_d(b, m);
+        }
+        if (lane == gw) { sig = a; numk = b; }
+      }
       const int64_t wo = grp * G + lane;
       if (lane < G && wo < io.M) {
-        double sig = 0.0, numk = 0.0;
-        for (int sl = 0; sl < SL; ++sl) {
-          const double *pp = io.fb_part + (((int64_t)entry * SL + sl) * G + lane) * 2;
-          sig += __ldcg(pp);
-          numk += __ldcg(pp + 1);
-        }
         if (io.logpsi) io.logpsi[wo] = res[2] + log(fabs(sig));
         if (io.sign) io.sign[wo] = (sig > 0.0) ? 1.0 : ((sig < 0.0) ? -1.0 : 0.0);
         if (io.eloc) io.eloc[wo] = res[3] + numk / sig + P.vnn;
