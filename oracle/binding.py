@@ -71,6 +71,10 @@ def lib():
                                             C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
             L.oracle_batch_stats.restype = None
             L.oracle_batch_stats.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+            L.oracle_log_derivatives.restype = C.c_int
+            L.oracle_log_derivatives.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p]
+            L.oracle_energy_gradient.restype = None
+            L.oracle_energy_gradient.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
             _lib = L
     return _lib
 
@@ -199,3 +203,33 @@ def batch_stats(x):
     m, s = C.c_double(), C.c_double()
     lib().oracle_batch_stats(_p(x), x.shape[0], C.addressof(m), C.addressof(s))
     return m.value, s.value
+
+
+def log_derivatives(sysd: OracleSystem, r_soa, threads: int = 1):
+    """O[M, 3 + n_det] = (dPsi/dtheta)/Psi for theta = (a_par, a_anti, b, d_0 .. d_{n_det-1}) (eq. 6)."""
+    r = np.ascontiguousarray(r_soa, np.float64)
+    M = r.shape[2]
+    O = np.empty((M, 3 + int(sysd.c.n_det)))
+    L = lib()
+
+    def run(rng):
+        rc = L.oracle_log_derivatives(sysd.ref, _p(r), M, rng[0], rng[1], _p(O))
+        assert rc == 0
+
+    rs = _ranges(M, threads)
+    if len(rs) == 1:
+        run(rs[0])
+    else:
+        with ThreadPoolExecutor(len(rs)) as ex:
+            list(ex.map(run, rs))
+    return O
+
+
+def energy_gradient(eloc, O):
+    """eq. 6: (E_v, grad[n_param]) with grad_p = (2/M) sum_m O[m,p] (E_L[m] - E_v)."""
+    e = np.ascontiguousarray(eloc, np.float64)
+    Oc = np.ascontiguousarray(O, np.float64)
+    ev = C.c_double()
+    g = np.empty(Oc.shape[1])
+    lib().oracle_energy_gradient(_p(e), _p(Oc), e.shape[0], Oc.shape[1], C.addressof(ev), _p(g))
+    return ev.value, g

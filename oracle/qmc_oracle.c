@@ -504,3 +504,86 @@ void oracle_batch_stats(const double *x, int64_t M, double *mean, double *stderr
   if (mean) *mean = mu;
   if (stderr_out) *stderr_out = (M > 1) ? sqrt(s2 / (double)(M - 1) / (double)M) : 0.0;
 }
+
+/* ------------------------------------------------------------------ */
+/* Parameter derivatives of ln Psi and the gradient estimator (eq. 6,   */
+/* PAPER.md:78).  theta = (a_par, a_anti, b, d_0 .. d_{n_det-1}).       */
+/* ------------------------------------------------------------------ */
+
+int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
+                           int64_t w1, double *O) {
+  int ne = s->n_up + s->n_dn, nmo = s->n_mo, np = 3 + s->n_det;
+  double *mo = (double *)malloc(sizeof(double) * (size_t)(ne * nmo + 1));
+  double *A = (double *)malloc(sizeof(double) * (size_t)(ne * ne + 1));
+  double *pos = (double *)malloc(sizeof(double) * (size_t)(3 * ne + 1));
+  double *prod = (double *)malloc(sizeof(double) * (size_t)(s->n_det + 1));
+  if (!mo || !A || !pos || !prod) return -1;
+  double ao[5];
+  for (int64_t w = w0; w < w1; ++w) {
+    gather_walker(r, M, w, ne, pos);
+    double *out = O + (size_t)w * (size_t)np;
+    /* Jastrow: K = a r / (1 + b r)  (D.1):  dK/da = r / (1 + b r),  dK/db = -a r^2 / (1 + b r)^2 */
+    double da_par = 0.0, da_anti = 0.0, db = 0.0;
+    for (int i = 0; i < ne; ++i)
+      for (int j = i + 1; j < ne; ++j) {
+        int same = spin_of(s, i) == spin_of(s, j);
+        double a = same ? s->jastrow_a_par : s->jastrow_a_anti;
+        double dx = pos[3 * i] - pos[3 * j], dy = pos[3 * i + 1] - pos[3 * j + 1], dz = pos[3 * i + 2] - pos[3 * j + 2];
+        double rij = sqrt(dx * dx + dy * dy + dz * dz);
+        double den = 1.0 + s->jastrow_b * rij;
+        if (same) da_par += rij / den; else da_anti += rij / den;
+        db += -a * rij * rij / (den * den);
+      }
+    out[0] = da_par;
+    out[1] = da_anti;
+    out[2] = db;
+    /* CI: Sigma = sum_n d_n D_n^up D_n^dn  (eq. 4):  d ln Sigma / d d_n = D_n^up D_n^dn / Sigma */
+    for (int i = 0; i < ne * nmo; ++i) mo[i] = 0.0;
+    for (int i = 0; i < ne; ++i)
+      for (int beta = 0; beta < s->n_ao; ++beta) {
+        oracle_ao_eval(s, beta, pos + 3 * i, ao);
+        for (int alpha = 0; alpha < nmo; ++alpha) mo[i * nmo + alpha] += s->mo_coeff[beta * nmo + alpha] * ao[0];
+      }
+    double sigma = 0.0;
+    for (int n = 0; n < s->n_det; ++n) {
+      double D[2];
+      for (int sp = 0; sp < 2; ++sp) {
+        int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
+        const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
+        for (int i = 0; i < ns; ++i)
+          for (int j = 0; j < ns; ++j) A[i * ns + j] = mo[(e0 + i) * nmo + lst[j]];
+        D[sp] = oracle_det_inv(ns, A, NULL);
+      }
+      prod[n] = D[0] * D[1];
+      sigma += s->ci_coeff[n] * prod[n];
+    }
+    for (int n = 0; n < s->n_det; ++n) out[3 + n] = prod[n] / sigma;
+  }
+  free(mo); free(A); free(pos); free(prod);
+  return 0;
+}
+
+static double kahan_mean(const double *x, int64_t M) {
+  double sum = 0.0, c = 0.0;
+  for (int64_t i = 0; i < M; ++i) {
+    double y = x[i] - c, t = sum + y;
+    c = (t - sum) - y;
+    sum = t;
+  }
+  return sum / (double)M;
+}
+
+void oracle_energy_gradient(const double *eloc, const double *O, int64_t M, int32_t n_param,
+                            double *Ev, double *grad) {
+  double ev = kahan_mean(eloc, M);
+  if (Ev) *Ev = ev;
+  for (int p = 0; p < n_param; ++p) {
+    double sum = 0.0, c = 0.0;
+    for (int64_t m = 0; m < M; ++m) {
+      double y = O[(size_t)m * (size_t)n_param + p] * (eloc[m] - ev) - c, t = sum + y;
+      c = (t - sum) - y;
+      sum = t;
+    }
+    grad[p] = 2.0 * sum / (double)M;
+  }
+}

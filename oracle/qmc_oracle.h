@@ -14,7 +14,10 @@
  * harmonic (1s, 2s, 2p x3, 3d x5), He-like closed form with the Pade Jastrow,
  * n-electron hydrogenic determinants (exact sum of orbital energies), central
  * finite differences of the plain Psi, antisymmetry, Leibniz determinants,
- * nuclear repulsion, cusp finiteness, Philox known answers, sampler moments.
+ * nuclear repulsion, cusp finiteness, Philox known answers, sampler moments;
+ * parameter derivatives (eq. 6): central differences of log|Psi| in every
+ * parameter, sum rule sum_n d_n O_n = 1, He-like closed form, zero gradient for
+ * an exact eigenfunction.
  * Unpinned by anything but those: absolute energies of the random-MO
  * synthetic LiH / Li2 / CO configs (no physical reference exists for them).
  */
@@ -85,6 +88,20 @@ int oracle_metropolis(const oracle_system_desc_t *s, double *r, int64_t M, int64
 
 /* Mean and standard error of the mean (eq. 3), Kahan sums. */
 void oracle_batch_stats(const double *x, int64_t M, double *mean, double *stderr_out);
+
+/* Logarithmic derivatives O_p(r) = (d Psi / d theta_p) / Psi, the factor of eq. 6
+ * (PAPER.md:78), for theta = (jastrow_a_par, jastrow_a_anti, jastrow_b, d_0 .. d_{n_det-1})
+ * in that order; O is [M][3 + n_det] row-major, rows w0 <= w < w1 are written.
+ * Psi = e^J Sigma (eq. 4), so d ln Psi / d(Jastrow parameter) is the
+ * parameter derivative of D.1 summed over pairs, and
+ * d ln Psi / d d_n = D_n^up D_n^dn / Sigma, every determinant factored explicitly. */
+int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
+                           int64_t w1, double *O);
+
+/* Estimator of eq. 6: E_v = mean E_L, grad_p = (2/M) sum_m O[m][p] (E_L[m] - E_v).
+ * Kahan sums.  Ev may be NULL. */
+void oracle_energy_gradient(const double *eloc, const double *O, int64_t M, int32_t n_param,
+                            double *Ev, double *grad);
 
 #ifdef __cplusplus
 }

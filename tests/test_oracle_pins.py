@@ -550,3 +550,90 @@ def test_batch_stats():
     m, s = ob.batch_stats(x)
     assert abs(m - math.fsum(x) / len(x)) < 1e-9
     assert abs(s - x.std(ddof=1) / math.sqrt(len(x))) < 1e-12
+
+
+# ---------------------------------------------------------------- parameter derivatives (eq. 6)
+def _with_param(d, p, value):
+    """copy of the system with parameter p of theta = (a_par, a_anti, b, d_0 ...) set to value"""
+    import copy
+    d2 = copy.copy(d)
+    if p == 0:
+        d2.jastrow_a_par = value
+    elif p == 1:
+        d2.jastrow_a_anti = value
+    elif p == 2:
+        d2.jastrow_b = value
+    else:
+        ci = np.array(d.ci_coeff, np.float64, copy=True)
+        ci[p - 3] = value
+        d2.ci_coeff = ci
+    return d2
+
+
+def _param(d, p):
+    return [d.jastrow_a_par, d.jastrow_a_anti, d.jastrow_b][p] if p < 3 else float(d.ci_coeff[p - 3])
+
+
+@pytest.mark.parametrize("name,M", [("H2", 12), ("LiH", 10), ("Li2", 8), ("CO", 5)])
+def test_log_derivatives_vs_central_differences_of_log_psi(name, M):
+    # the oracle's O_p against central differences of its own log|Psi| in EVERY parameter
+    # (Richardson h, h/2): pins sign, pair bookkeeping (which a), the b derivative and D_n / Sigma
+    d, r = wl.CONFIGS[name](M=M)
+    O = ob.log_derivatives(ob.OracleSystem(d), r)
+    assert O.shape == (M, 3 + len(d.ci_coeff))
+    params = list(range(3)) + list(range(3, O.shape[1], max(1, (O.shape[1] - 3) // 7)))
+    for p in params:
+        t0 = _param(d, p)
+
+        def cd(h):
+            lp_p = ob.local_energy(ob.OracleSystem(_with_param(d, p, t0 + h)), r)[0]
+            lp_m = ob.local_energy(ob.OracleSystem(_with_param(d, p, t0 - h)), r)[0]
+            return (lp_p - lp_m) / (2 * h)
+
+        h = 1e-3 * max(1.0, abs(t0)) if p < 3 else 1e-3 * max(abs(t0), 1e-2)
+        fd = (4 * cd(h / 2) - cd(h)) / 3
+        assert np.max(np.abs(O[:, p] - fd) / np.maximum(1, np.abs(fd))) < 1e-7, (name, p)
+
+
+def test_log_derivatives_sum_rule_and_helium_closed_form():
+    # sum_n d_n O_n = 1 (Sigma is linear in d)
+    d, r = wl.li2(M=20)
+    O = ob.log_derivatives(ob.OracleSystem(d), r)
+    assert np.max(np.abs(O[:, 3:] @ np.asarray(d.ci_coeff) - 1.0)) < 1e-11
+    # He-like 1s^2 + Pade: O_a_anti = r12/(1+b r12), O_b = -a r12^2/(1+b r12)^2, O_a_par = 0, O_d0 = 1/d0
+    a, b = 0.37, 0.6
+    d = atom_system(2.0, [(1, 0, 0, 1.6875)], [[1.0]], 1, 1, a_par=0.25, a_anti=a, b=b, ci=[0.8])
+    rr = _rand_pos(50, 2, 1.0, rmin=0.05, seed=77)
+    O = ob.log_derivatives(ob.OracleSystem(d), soa(rr))
+    r12 = np.linalg.norm(rr[:, 0] - rr[:, 1], axis=1)
+    assert np.max(np.abs(O[:, 0])) == 0.0
+    assert np.max(np.abs(O[:, 1] - r12 / (1 + b * r12))) < 1e-14
+    assert np.max(np.abs(O[:, 2] + a * r12 ** 2 / (1 + b * r12) ** 2)) < 1e-14
+    assert np.max(np.abs(O[:, 3] - 1 / 0.8)) < 1e-13
+    # three same-spin electrons: only a_par pairs contribute
+    aos, C, e = hydrogenic_set(1.0)
+    d = atom_system(1.0, aos, C[:, [0, 2, 4]], 3, 0, norm=np.ones(len(aos)), a_par=0.25, a_anti=0.5, b=0.9)
+    rr = _rand_pos(20, 3, 2.0, rmin=0.2, seed=78)
+    O = ob.log_derivatives(ob.OracleSystem(d), soa(rr))
+    s = sum(np.linalg.norm(rr[:, i] - rr[:, j], axis=1) / (1 + 0.9 * np.linalg.norm(rr[:, i] - rr[:, j], axis=1))
+            for i in range(3) for j in range(i))
+    assert np.max(np.abs(O[:, 0] - s)) < 1e-13 and np.max(np.abs(O[:, 1])) == 0.0
+
+
+def test_energy_gradient_estimator():
+    rng = np.random.default_rng(5)
+    M, n_p = 1000, 7
+    e = rng.standard_normal(M) * 3 - 10
+    O = rng.standard_normal((M, n_p))
+    ev, g = ob.energy_gradient(e, O)
+    assert abs(ev - math.fsum(e) / M) < 1e-13
+    ref = np.array([2 * math.fsum(O[:, p] * (e - math.fsum(e) / M)) / M for p in range(n_p)])
+    assert np.max(np.abs(g - ref)) < 1e-13
+    # an exact eigenfunction has E_L constant, so the estimator vanishes identically whatever O is (eq. 6):
+    # hydrogen atom, exact 1s, two "determinants" that are the same orbital
+    d = atom_system(1, [(1, 0, 0, 1.0)], [[1.0]], 1, 0, det_up=[[0], [0]], det_dn=np.zeros((2, 0), np.int32), ci=[0.7, 0.2])
+    r = soa(_rand_pos(64, 1, 2.0, rmin=0.1, seed=6))
+    o = ob.OracleSystem(d)
+    el = ob.local_energy(o, r)[2]
+    ev, g = ob.energy_gradient(el, ob.log_derivatives(o, r))
+    assert abs(ev + 0.5) < 1e-12 and np.max(np.abs(g)) < 1e-11
