@@ -137,6 +137,29 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
  * Deterministic (fixed reduction tree, compensated).  Synchronises cuda_stream. */
 int qmc_batch_stats(const double *d_x, int64_t M, double *h_mean, double *h_stderr, void *cuda_stream);
 
+/* ---- the factors of the gradient estimator, eq. 6 ----
+ * Variational parameters handled: theta = (jastrow_a_par, jastrow_a_anti, jastrow_b,
+ * d_0 .. d_{n_det-1}) in that order, n_param = 3 + n_det (qmc_n_param).  MO and AO parameters
+ * (mu, zeta of PAPER.md:55-57) are not handled yet. */
+int qmc_n_param(const qmc_system_t *s);
+
+/* qmc_local_energy plus the logarithmic derivatives O_p(r) = (dPsi/dtheta_p)/Psi:
+ *   d_O device, out: double [M][n_param] row-major (required)
+ * Psi = e^J Sigma (eq. 4): O for a Jastrow parameter is dJ/dtheta from D.1,
+ * O for d_n is D_n^up D_n^dn / Sigma, formed from the excitation tables of the same launch.
+ * d_logpsi / d_sign / d_eloc as in qmc_local_energy (E_L carries the explicit fallback
+ * correction; O comes from the table path, whose relative error for a nearly singular
+ * reference is eps * cond(A_0), not the squared amplification E_L suffers).  Asynchronous. */
+int qmc_log_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign,
+                        double *d_eloc, double *d_O, void *cuda_stream);
+
+/* Estimator of eq. 6: E_v = mean E_L, grad_p = (2/M) sum_m O[m][p] (E_L[m] - E_v).
+ *   d_eloc device in [M]; d_O device in [M][n_param]; h_Ev host out (may be NULL);
+ *   h_grad host out [n_param].  Deterministic (fixed partition, compensated sums).
+ * Synchronises cuda_stream. */
+int qmc_energy_gradient(const double *d_eloc, const double *d_O, int64_t M, int32_t n_param, double *h_Ev,
+                        double *h_grad, void *cuda_stream);
+
 /* Measured FP64 throughput of the current device, the roofline denominator of this
  * path (BASELINE.json north_star: "the chip's FP64 peak, measured by a DFMA
  * microbenchmark in the same run").  kind 0: dependent-chain DFMA kernel, 1: DMMA

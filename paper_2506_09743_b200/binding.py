@@ -15,7 +15,8 @@ QMC_OK, QMC_EINVAL, QMC_EUNSUPPORTED, QMC_ECUDA, QMC_ENOMEM = 0, -1, -2, -3, -4
 _lib = None
 
 EXPORTS = ["qmc_setup", "qmc_destroy", "qmc_local_energy", "qmc_log_psi", "qmc_metropolis", "qmc_batch_stats",
-           "qmc_fp64_peak", "qmc_model_flops", "qmc_launch_count", "qmc_status_string"]
+           "qmc_fp64_peak", "qmc_model_flops", "qmc_launch_count", "qmc_status_string", "qmc_n_param",
+           "qmc_log_derivatives", "qmc_energy_gradient"]
 
 
 class QmcError(RuntimeError):
@@ -65,6 +66,12 @@ def lib():
         L.qmc_model_flops.argtypes = [vp, C.c_int]
         L.qmc_launch_count.restype = i64
         L.qmc_launch_count.argtypes = [C.c_int]
+        L.qmc_n_param.restype = C.c_int
+        L.qmc_n_param.argtypes = [vp]
+        L.qmc_log_derivatives.restype = C.c_int
+        L.qmc_log_derivatives.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp]
+        L.qmc_energy_gradient.restype = C.c_int
+        L.qmc_energy_gradient.argtypes = [vp, vp, i64, C.c_int32, vp, vp, vp]
         L.qmc_status_string.restype = C.c_char_p
         L.qmc_status_string.argtypes = [C.c_int]
         _lib = L
@@ -170,6 +177,23 @@ class QmcSystem:
         return dict(logpsi=logpsi, sign=sign, accept=accept, eloc_acc=eloc_acc,
                     n_accepted=nacc.value if count else None)
 
+    def n_param(self) -> int:
+        return int(lib().qmc_n_param(self._h))
+
+    def log_derivatives(self, r, logpsi=None, sign=None, eloc=None, O=None, stream=None):
+        """qmc_log_derivatives: (logpsi, sign, eloc, O[M, n_param]) with O_p = (dPsi/dtheta_p)/Psi (eq. 6)."""
+        M = self._chk_r(r)
+        new = lambda: torch.empty(M, dtype=torch.float64, device=r.device)
+        logpsi = new() if logpsi is None else logpsi
+        sign = new() if sign is None else sign
+        eloc = new() if eloc is None else eloc
+        if O is None:
+            O = torch.empty((M, self.n_param()), dtype=torch.float64, device=r.device)
+        assert O.is_cuda and O.dtype == torch.float64 and O.is_contiguous() and tuple(O.shape) == (M, self.n_param())
+        _check(lib().qmc_log_derivatives(self._h, _dp(r), M, _dp(logpsi), _dp(sign), _dp(eloc), _dp(O),
+                                         _stream(stream)))
+        return logpsi, sign, eloc, O
+
     def model_flops(self, which: int) -> float:
         return lib().qmc_model_flops(self._h, which)
 
@@ -180,6 +204,17 @@ def batch_stats(x, stream=None):
     m, s = C.c_double(), C.c_double()
     _check(lib().qmc_batch_stats(_dp(x), x.numel(), C.addressof(m), C.addressof(s), _stream(stream)))
     return m.value, s.value
+
+
+def energy_gradient(eloc, O, stream=None):
+    """qmc_energy_gradient: (E_v, grad[n_param]) of eq. 6 from device E_L [M] and O [M, n_param]."""
+    assert eloc.is_cuda and O.is_cuda and eloc.dtype == O.dtype == torch.float64
+    assert eloc.is_contiguous() and O.is_contiguous() and O.shape[0] == eloc.numel()
+    ev = C.c_double()
+    g = np.empty(int(O.shape[1]))
+    _check(lib().qmc_energy_gradient(_dp(eloc), _dp(O), eloc.numel(), int(O.shape[1]), C.addressof(ev), _np(g),
+                                     _stream(stream)))
+    return ev.value, g
 
 
 def fp64_peak(kind: int = 0, reps: int = 5, device: int = 0) -> float:

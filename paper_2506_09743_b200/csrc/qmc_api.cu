@@ -34,7 +34,7 @@ int cuda_fail(cudaError_t e, const char *what) {
 struct Variant {
   int NS, NMO, LP, ws_doubles;
   bool exact;  // compiled for n_up = n_dn = NS
-  const void *k_el, *k_psi, *k_metro, *k_expl;
+  const void *k_el, *k_psi, *k_metro, *k_expl, *k_el_deriv;
 };
 
 template <int NS, int NMO, bool X>
@@ -49,6 +49,7 @@ Variant make_variant() {
   v.k_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi>;
   v.k_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi>;
   v.k_expl = (const void *)explicit_energy_kernel<NS, NMO, X, kWarpsEl>;
+  v.k_el_deriv = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true>;
   return v;
 }
 
@@ -86,8 +87,8 @@ struct qmc_system {
   SysParams P{};
   Variant var{};
   int smem_el = 0, smem_psi = 0;  // dynamic shared memory of the E_L kernels (kWarpsEl warps) / values-only kernels
-  int blocks_el = 0, blocks_psi = 0, blocks_metro = 0, blocks_expl = 0;
-  void *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr;
+  int blocks_el = 0, blocks_psi = 0, blocks_metro = 0, blocks_expl = 0, blocks_deriv = 0;
+  void *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr, *d_orig = nullptr;
   int n_sm = 0;
   double *d_stats = nullptr;
   unsigned long long *d_counter = nullptr;
@@ -120,6 +121,7 @@ void qmc_destroy(qmc_system_t *s) {
   cudaFree(s->d_dets);
   cudaFree(s->d_gen);
   cudaFree(s->d_cols);
+  cudaFree(s->d_orig);
   cudaFree(s->d_stats);
   cudaFree(s->d_counter);
   delete s;
@@ -185,7 +187,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     return (int)used.size() - 1;
   };
   std::vector<int> virt[2];  // caller MO index of virtual q
-  struct Exc { int k[2]; int p[2][kMaxSpin]; int q[2][kMaxSpin]; double d; };
+  struct Exc { int k[2]; int p[2][kMaxSpin]; int q[2][kMaxSpin]; double d; int orig; };
   std::vector<Exc> excs(d->n_det);
   bool unsupported = false;
   for (int sp = 0; sp < 2; ++sp)
@@ -193,6 +195,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   for (int n = 0; n < d->n_det; ++n) {
     Exc &x = excs[n];
     x.d = d->ci_coeff[n];
+    x.orig = n;
     for (int sp = 0; sp < 2; ++sp) {
       int k = 0;
       for (int j = 0; j < nsp[sp]; ++j) {
@@ -233,6 +236,9 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   const int n_packed = n_cls[1] + n_cls[2] + n_cls[3] + n_cls[4];  // packed 16-byte records (classes 1-4)
   P.d_ref = 0.0;
   for (int n = 0; n < n_ref; ++n) P.d_ref += excs[n].d;
+  P.n_ref = n_ref;
+  std::vector<int> det_orig(d->n_det);  // kernel order -> caller's determinant index (parameter derivatives)
+  for (int n = 0; n < d->n_det; ++n) det_orig[n] = excs[n].orig;
   P.n_a1 = n_cls[1];
   P.n_a2 = P.n_a1 + n_cls[2];
   P.n_b = P.n_a2 + n_cls[3];
@@ -472,7 +478,9 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
       (e = cudaMalloc(&s->d_gen, std::max<size_t>(gens.size(), 1) * sizeof(GenDet))) != cudaSuccess ||
       (!gens.empty() && (e = cudaMemcpy(s->d_gen, gens.data(), gens.size() * sizeof(GenDet), cudaMemcpyHostToDevice)) != cudaSuccess) ||
       (e = cudaMalloc(&s->d_cols, cols.size() * sizeof(DetCols))) != cudaSuccess ||
-      (e = cudaMemcpy(s->d_cols, cols.data(), cols.size() * sizeof(DetCols), cudaMemcpyHostToDevice)) != cudaSuccess) {
+      (e = cudaMemcpy(s->d_cols, cols.data(), cols.size() * sizeof(DetCols), cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMalloc(&s->d_orig, det_orig.size() * sizeof(int))) != cudaSuccess ||
+      (e = cudaMemcpy(s->d_orig, det_orig.data(), det_orig.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) {
     int rc = cuda_fail(e, "qmc_setup upload");
     qmc_destroy(s);
     return rc;
@@ -483,6 +491,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   P.dets = (const DetRec *)s->d_dets;
   P.gen = (const GenDet *)s->d_gen;
   P.det_cols = (const DetCols *)s->d_cols;
+  P.det_orig = (const int *)s->d_orig;
   P.smem_const_bytes = (int)((szC + szD + 15) / 16 * 16);
   s->smem_el = P.smem_const_bytes + kWarpsEl * var->ws_doubles * (int)sizeof(double);
   s->smem_psi = P.smem_const_bytes + kWarpsPsi * var->ws_doubles * (int)sizeof(double);
@@ -495,11 +504,11 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     return QMC_EUNSUPPORTED;
   }
   s->n_sm = n_sm;
-  const void *ks[4] = {var->k_el, var->k_psi, var->k_metro, var->k_expl};
-  int *nb[4] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro, &s->blocks_expl};
-  const int kw[4] = {kWarpsEl, kWarpsPsi, kWarpsPsi, kWarpsEl};
-  const int ksm[4] = {s->smem_el, s->smem_psi, s->smem_psi, s->smem_el};
-  for (int i = 0; i < 4; ++i) {
+  const void *ks[5] = {var->k_el, var->k_psi, var->k_metro, var->k_expl, var->k_el_deriv};
+  int *nb[5] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro, &s->blocks_expl, &s->blocks_deriv};
+  const int kw[5] = {kWarpsEl, kWarpsPsi, kWarpsPsi, kWarpsEl, kWarpsEl};
+  const int ksm[5] = {s->smem_el, s->smem_psi, s->smem_psi, s->smem_el, s->smem_el};
+  for (int i = 0; i < 5; ++i) {
     if ((e = cudaFuncSetAttribute(ks[i], cudaFuncAttributeMaxDynamicSharedMemorySize, ksm[i])) != cudaSuccess) {
       int rc = cuda_fail(e, "cudaFuncSetAttribute");
       qmc_destroy(s);
@@ -518,7 +527,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
 }
 
 static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, double *d_eloc,
-                       void *stream, bool el) {
+                       void *stream, bool el, double *d_O = nullptr) {
   if (!s || !d_r || M <= 0) return QMC_EINVAL;
   CK(cudaSetDevice(s->device));
   cudaStream_t st = (cudaStream_t)stream;
@@ -527,11 +536,12 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
   io.logpsi = d_logpsi;
   io.sign = d_sign;
   io.eloc = d_eloc;
+  io.O = d_O;
   io.M = M;
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
   const int wpb = el ? kWarpsEl : kWarpsPsi, smem = el ? s->smem_el : s->smem_psi;
   const int64_t need = (groups + wpb - 1) / wpb;
-  const int grid = (int)std::min<int64_t>(need, el ? s->blocks_el : s->blocks_psi);
+  const int grid = (int)std::min<int64_t>(need, d_O ? s->blocks_deriv : (el ? s->blocks_el : s->blocks_psi));
   double *fb = nullptr;
   const bool fallback = el && s->P.n_det_all > 1;  // a single determinant has no reference to be ill-conditioned against
   const int64_t expl_warps = (int64_t)s->blocks_expl * kWarpsEl;
@@ -548,7 +558,7 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
     io.fb_done = fbi + 1 + groups;
   }
   void *args[2] = {(void *)&s->P, (void *)&io};
-  CK(cudaLaunchKernel(el ? s->var.k_el : s->var.k_psi, dim3(grid), dim3(wpb * 32), args, smem, st));
+  CK(cudaLaunchKernel(d_O ? s->var.k_el_deriv : (el ? s->var.k_el : s->var.k_psi), dim3(grid), dim3(wpb * 32), args, smem, st));
   ++g_launches;
   if (fallback) {
     CK(cudaLaunchKernel(s->var.k_expl, dim3(s->blocks_expl), dim3(kWarpsEl * 32), args, s->smem_el, st));
@@ -638,6 +648,36 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
     CK(cudaStreamSynchronize(st));
     *h_n_accepted = (int64_t)v;
   }
+  return QMC_OK;
+}
+
+int qmc_n_param(const qmc_system_t *s) { return s ? 3 + s->P.n_det_all : QMC_EINVAL; }
+
+int qmc_log_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, double *d_eloc,
+                        double *d_O, void *cuda_stream) {
+  if (!d_O) return QMC_EINVAL;
+  return launch_eval(s, d_r, M, d_logpsi, d_sign, d_eloc, cuda_stream, true, d_O);
+}
+
+int qmc_energy_gradient(const double *d_eloc, const double *d_O, int64_t M, int32_t n_param, double *h_Ev, double *h_grad,
+                        void *cuda_stream) {
+  if (!d_eloc || !d_O || M <= 0 || n_param < 1 || !h_grad) return QMC_EINVAL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int nblk = (int)std::min<int64_t>(1184, (M + 63) / 64);  // >= 64 rows per block
+  double *scr = nullptr;  // [2] stats, [n_param] gradient, [nblk][n_param] partials
+  CK(cudaMallocAsync(&scr, ((size_t)2 + (size_t)n_param * (size_t)(nblk + 1)) * sizeof(double), st));
+  double *d_stats = scr, *d_grad = scr + 2, *d_part = d_grad + n_param;
+  batch_stats_kernel<<<1, 1024, 0, st>>>(d_eloc, M, d_stats);
+  gradient_partial_kernel<<<nblk, 128, 0, st>>>(d_eloc, d_O, M, n_param, d_stats, d_part);
+  gradient_final_kernel<<<(n_param + 127) / 128, 128, 0, st>>>(d_part, nblk, n_param, M, d_grad);
+  g_launches += 3;
+  std::vector<double> h((size_t)n_param + 2);
+  cudaError_t e = cudaMemcpyAsync(h.data(), scr, h.size() * sizeof(double), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFreeAsync(scr, st);
+  if (e != cudaSuccess) return cuda_fail(e, "qmc_energy_gradient");
+  if (h_Ev) *h_Ev = h[0];
+  for (int p = 0; p < n_param; ++p) h_grad[p] = h[2 + p];
   return QMC_OK;
 }
 

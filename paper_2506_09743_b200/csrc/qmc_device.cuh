@@ -98,6 +98,9 @@ struct SysParams {  // passed by value to every kernel
   int n_a1, n_a2, n_b;             // class boundaries in dets[]: [0,n_a1) one entry, [n_a1,n_a2) two entries,
                                    // [n_a2,n_b) one 2x2 block, [n_b,n_det) two 2x2 blocks (qmc_setup)
   double d_ref;                    // summed coefficients of the determinants equal to the reference
+  int n_ref;                       // how many determinants equal the reference
+  const int *det_orig;             // device [n_det_all]: caller's index of the determinants in kernel order
+                                   // (reference-equal ones, then dets[] classes 1-4, then gen[])
   int nv[2];                       // virtual orbitals per spin
   int G;                           // walkers per warp pass
   int smem_const_bytes;
@@ -129,6 +132,15 @@ struct WalkerIO {
   const double *r_in;  // [n_e][3][M]
   double *r_out;       // Metropolis: same buffer
   double *logpsi, *sign, *eloc;
+  double *O;           // device [M][3 + n_det_all] parameter derivatives (DerivOut), or null
+  int64_t M;
+};
+
+// Parameter-derivative output (eq. 6): O[w][p] = (dPsi/dtheta_p)/Psi for
+// theta = (a_par, a_anti, b, d_0 .. d_{n_det-1}); row-major [M][3 + n_det_all].
+struct DerivOut {
+  double *O;      // device, or null
+  int64_t w0;     // first walker of the group being evaluated
   int64_t M;
 };
 

@@ -79,11 +79,12 @@ __device__ __noinline__ void excite_general(const GenSpin *g, const double *T, i
 // at (x, y, z).  Results for walker g are left in ws[oRes + 4 g + {0,1,2}] =
 // {log|Psi|, sign, E_L} (E_L only if EL).  All 32 lanes must call.
 // ---------------------------------------------------------------------------------
-template <int NS, int NMO, bool EL, bool X, bool EXPL = false>
+// DERIV: also write the logarithmic parameter derivatives of eq. 6 for the G walkers to dv.O.
+template <int NS, int NMO, bool EL, bool X, bool EXPL = false, bool DERIV = false>
 __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp,
                              const double *__restrict__ sC, const DetRec *__restrict__ sDet,
                              double *__restrict__ ws, double x, double y, double z, int lane,
-                             int det0 = 0, int det_step = 1) {
+                             int det0 = 0, int det_step = 1, const DerivOut dv = DerivOut{}) {
   using GE = Geo<NS, NMO>;
   constexpr int LP = GE::LP, PP = GE::PP, TS = GE::TS, RS = GE::RS;
   // X: closed-shell system that matches the instantiation exactly (n_up = n_dn = NS): sizes fold
@@ -105,6 +106,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
   // and for even ne the lower half also takes e+ne/2; the partner's share of the gradient (the
   // opposite vector) travels by shuffle from the lane that computed the pair.
   double Jp = 0.0, gJx = 0.0, gJy = 0.0, gJz = 0.0, lapJ = 0.0, vee = 0.0;
+  double dJa_par = 0.0, dJa_anti = 0.0, dJb = 0.0;  // DERIV: this lane's share of dJ/da_par, dJ/da_anti, dJ/db
   {
     const bool up = e < n_up;
     const int base = (active ? g : 0) * ne;
@@ -126,6 +128,14 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       const double di = rcp_fast(fma(P.b, r, 1.0));
       const double adi = a * di;
       Jp = fma(adi, r, Jp);  // u = a r / (1 + b r)
+      if (DERIV) {
+        // D.1: dK/da = r / (1 + b r) for the pair's own a, dK/db = -a r^2 / (1 + b r)^2
+        const double rd = take ? r * di : 0.0;
+        const bool same = (j < n_up) == up;
+        dJa_par += same ? rd : 0.0;
+        dJa_anti += same ? 0.0 : rd;
+        dJb = fma(-adi * r, rd, dJb);
+      }
       if (EL) {
         const double u1 = adi * di;              // u'  = a / (1 + b r)^2
         const double u2 = -2.0 * P.b * u1 * di;  // u'' = -2 a b / (1 + b r)^3
@@ -295,6 +305,11 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
     // per-electron scalars: J/2-sum and the electron's share of the energy
     sPart[lane * 2 + 0] = Jp;
     sPart[lane * 2 + 1] = EL ? (fma(-0.5, lapJ + fma(gJx, gJx, fma(gJy, gJy, gJz * gJz)), vee + ven)) : 0.0;
+    if (DERIV) {  // the coordinate scratch is dead (and the tile that overlaid it too)
+      sXYZ[lane * 3 + 0] = dJa_par;
+      sXYZ[lane * 3 + 1] = dJa_anti;
+      sXYZ[lane * 3 + 2] = dJb;
+    }
   }
   __syncwarp();
 
@@ -620,6 +635,50 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       // explicit fallback when the estimated table-path error 1.2e-15 (Sigma/D_0)^2 exceeds a tenth of the
       // parity bound 1e-8 max(1, |E_L|); also set for NaN (singular reference)
       sRes[wg * 4 + 3] = (den * den <= kFallbackK * fmax(1.0, fabs(eloc))) ? 0.0 : 1.0;
+    }
+    if (DERIV) {
+      // ---- eq. 6 factors O_p = (dPsi/dtheta_p)/Psi, theta = (a_par, a_anti, b, d_0 ...):
+      // Jastrow: dJ/dtheta summed over the walker's electrons; CI: d ln Sigma / d d_n = R_n^up R_n^dn / den
+      // (D_n / D_0 over Sigma / D_0), a second, values-only pass over the determinant classes.
+      const int64_t wo = dv.w0 + wg;
+      if (wvalid && wo < dv.M && dv.O) {
+        const int np = 3 + P.n_det_all;
+        double *row = dv.O + wo * np;
+        for (int k = sub; k < 3; k += LW) {
+          double t = 0.0;
+          for (int j = 0; j < ne; ++j) t += sXYZ[(wg * ne + j) * 3 + k];
+          row[k] = t;
+        }
+        const double iden = 1.0 / den;
+        const int *orig = P.det_orig;
+        double *rowd = row + 3;
+        for (int n = sub; n < P.n_ref; n += LW) rowd[orig[n]] = iden;
+        orig += P.n_ref;
+        const char *Tb = reinterpret_cast<const char *>(Tu);
+        auto val = [&](uint32_t off8) {
+          return EL ? reinterpret_cast<const double2 *>(Tb + 2 * off8)->x : *reinterpret_cast<const double *>(Tb + off8);
+        };
+        for (int n = sub; n < P.n_a1; n += LW) rowd[orig[n]] = val(sDet[n].up) * iden;
+        for (int n = P.n_a1 + sub; n < P.n_a2; n += LW) rowd[orig[n]] = val(sDet[n].up) * val(sDet[n].dn) * iden;
+        for (int n = P.n_a2 + sub; n < P.n_b; n += LW) {
+          const DetRec dr = sDet[n];
+          rowd[orig[n]] = fma(val(dr.up & 0xffffu), val(dr.dn >> 16), -val(dr.up >> 16) * val(dr.dn & 0xffffu)) * iden;
+        }
+        for (int n = P.n_b + sub; n < P.n_det; n += LW) {
+          const DetRec dr = sDet[n];
+          double Ru, Du, Rd, Dd;
+          excite_double<EL>(dr.up, Tu, Ru, Du);
+          excite_double<EL>(dr.dn, Td, Rd, Dd);
+          rowd[orig[n]] = Ru * Rd * iden;
+        }
+        orig += P.n_det;
+        for (int n = sub; n < P.n_gen; n += LW) {
+          double u[2], v[2];
+          excite_general<EL>(&P.gen[n].s[0], Tu, RS, u);
+          excite_general<EL>(&P.gen[n].s[1], Td, RS, v);
+          rowd[orig[n]] = u[0] * v[0] * iden;
+        }
+      }
     }
   }
   __syncwarp();

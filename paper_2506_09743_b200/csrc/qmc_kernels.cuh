@@ -35,7 +35,7 @@ __device__ __forceinline__ void dummy_xyz(int lane, double &x, double &y, double
   z = 0.53 - 0.05 * lane;
 }
 
-template <int NS, int NMO, bool EL, bool X, int WPB>
+template <int NS, int NMO, bool EL, bool X, int WPB, bool DERIV = false>
 __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     local_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -64,7 +64,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   for (int64_t grp = (int64_t)blockIdx.x * WPB + warp; grp < n_groups; grp += stride) {
     double x, y, z;
     fetch(grp, x, y, z);
-    eval_walkers<NS, NMO, EL, X>(P, sExp, sC, sDet, ws, x, y, z, lane);
+    eval_walkers<NS, NMO, EL, X, false, DERIV>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1, DerivOut{io.O, grp * G, io.M});
     bool flagged = false;
     if (lane < G) {
       const int64_t wo = grp * G + lane;
@@ -272,6 +272,40 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
 // acc[i] += x[i]  (E_L on every sweep, BASELINE config 5)
 __global__ void __launch_bounds__(256) accumulate_kernel(double *__restrict__ acc, const double *__restrict__ x, int64_t M) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < M; i += (int64_t)gridDim.x * blockDim.x) acc[i] += x[i];
+}
+
+// ---------------------------------------------------------------------------------
+// Gradient estimator of eq. 6: grad_p = (2/M) sum_m O[m][p] (E_L[m] - E_v).
+// Deterministic: block b sums its contiguous rows per column (Kahan), then one thread per column adds
+// the block partials in order.  stats[0] = E_v (batch_stats_kernel).
+// ---------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) gradient_partial_kernel(const double *__restrict__ eloc, const double *__restrict__ O,
+                                                               int64_t M, int np, const double *__restrict__ stats,
+                                                               double *__restrict__ partial) {
+  const double ev = stats[0];
+  const int64_t rows = (M + gridDim.x - 1) / gridDim.x;
+  const int64_t m0 = (int64_t)blockIdx.x * rows, m1 = (m0 + rows < M) ? m0 + rows : M;
+  for (int p = threadIdx.x; p < np; p += blockDim.x) {
+    double s = 0.0, c = 0.0;
+    for (int64_t m = m0; m < m1; ++m) {
+      const double y = O[m * np + p] * (eloc[m] - ev) - c, t = s + y;
+      c = (t - s) - y;
+      s = t;
+    }
+    partial[(int64_t)blockIdx.x * np + p] = s;
+  }
+}
+__global__ void __launch_bounds__(128) gradient_final_kernel(const double *__restrict__ partial, int nblk, int np, int64_t M,
+                                                             double *__restrict__ grad) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= np) return;
+  double s = 0.0, c = 0.0;
+  for (int b = 0; b < nblk; ++b) {
+    const double y = partial[(int64_t)b * np + p] - c, t = s + y;
+    c = (t - s) - y;
+    s = t;
+  }
+  grad[p] = 2.0 * s / (double)M;
 }
 
 // ---------------------------------------------------------------------------------

@@ -315,3 +315,65 @@ def test_triple_and_quadruple_substitutions(env):
     up[9] = [0, 1, 2, 13, 12, 11, 6]
     d.det_up, d.det_dn = up, dn
     check_local_energy(env, d, r, threads=8)
+
+
+# ----------------------------------------------------------------------------- parameter derivatives (eq. 6)
+def check_log_derivatives(env, d, r, threads=8):
+    """O_p = (dPsi/dtheta_p)/Psi and the gradient estimator of eq. 6 against the oracle.
+    Tolerance: 1e-8 * max(1, |O|) per element for walkers with |Psi|/max|Psi| > 1e-6,
+    E_L as in check_local_energy, gradient 1e-8 of its absolute-sum scale."""
+    torch, ob, qb = env
+    o = ob.OracleSystem(d)
+    lp0, sg0, el0 = ob.local_energy(o, r, threads=threads)
+    O0 = ob.log_derivatives(o, r, threads=threads)
+    s = qb.QmcSystem(d)
+    assert s.n_param() == O0.shape[1]
+    rg = _to_gpu(torch, r)
+    lp, sg, el, O = s.log_derivatives(rg)
+    el_plain = s.local_energy(rg)[2]
+    torch.cuda.synchronize()
+    assert torch.equal(el, el_plain), "E_L of the derivative kernel differs from qmc_local_energy"
+    ev, g = qb.energy_gradient(el, O)
+    lpn, sgn, eln, On = (t.cpu().numpy() for t in (lp, sg, el, O))
+    s.close()
+    assert np.array_equal(sgn, sg0) and np.max(np.abs(lpn - lp0)) < 1e-10
+    keep = lp0 - lp0.max() > math.log(1e-6)
+    err = np.abs(On - O0) / np.maximum(1.0, np.abs(O0))
+    assert np.max(err[keep]) < 1e-8, (np.max(err[keep]), np.unravel_index(np.argmax(err * keep[:, None]), err.shape))
+    # sum rule on the GPU result itself
+    assert np.max(np.abs(On[keep, 3:] @ np.asarray(d.ci_coeff) - 1.0)) < 1e-9
+    # estimator: the oracle's reduction applied to the oracle's E_L and O
+    ev0, g0 = ob.energy_gradient(el0, O0)
+    scale = 2.0 * np.mean(np.abs(O0) * np.abs(el0 - ev0)[:, None], axis=0)
+    assert abs(ev - ev0) <= 1e-10 * abs(ev0)
+    assert np.max(np.abs(g - g0) / np.maximum(scale, 1e-300)) < 1e-8, np.max(np.abs(g - g0) / np.maximum(scale, 1e-300))
+    # and the GPU reduction applied to identical inputs agrees with the oracle's to rounding
+    ev1, g1 = qb.energy_gradient(torch.from_numpy(el0).cuda(), torch.from_numpy(O0).cuda())
+    assert abs(ev1 - ev0) <= 1e-13 * abs(ev0) and np.max(np.abs(g1 - g0) / np.maximum(scale, 1e-300)) < 1e-12
+
+
+@pytest.mark.parametrize("name,M", [("H2", 1024), ("LiH", 700), ("Li2", 1027), ("CO", 1025)])
+def test_log_derivatives_configs(env, name, M):
+    d, r = wl.CONFIGS[name](M=M)
+    check_log_derivatives(env, d, r)
+
+
+def test_log_derivatives_co_500_determinants_and_ragged(env):
+    d, r = wl.co_scan(M=301, n_geom=2)[1]
+    check_log_derivatives(env, d, r)
+    d, r = wl.co(M=3)
+    check_log_derivatives(env, d, r, threads=1)
+
+
+def test_log_derivatives_general_substitutions_and_unequal_spins(env):
+    rng = np.random.default_rng(11)
+    aos = [(1, 0, 0, 2.0), (2, 0, 0, 1.5), (2, 1, 0, 1.3), (2, 1, 1, 1.3), (2, 1, 2, 1.3), (3, 2, 3, 0.9), (3, 0, 0, 1.2),
+           (1, 0, 0, 0.8)]
+    C = rng.standard_normal((len(aos), 8))
+    # reference, a repeated reference, singles, a same-spin double, a triple (general path) and mixed ones
+    det_up = [[0, 1, 2, 3], [0, 1, 2, 3], [0, 4, 2, 3], [5, 1, 6, 3], [4, 5, 6, 3], [0, 1, 2, 7], [4, 1, 5, 3]]
+    det_dn = [[0, 1], [0, 1], [0, 1], [0, 1], [2, 1], [0, 3], [4, 5]]
+    d = atom_system(4.0, aos, C, 4, 2, det_up=det_up, det_dn=det_dn, ci=[0.8, 0.1, -0.3, 0.15, 0.05, 0.2, -0.1],
+                    a_par=0.25, a_anti=0.5, b=0.8, xyz=(0.1, -0.2, 0.3))
+    r = soa(rng.standard_normal((257, 6, 3)) * 1.3)
+    check_log_derivatives(env, d, r, threads=2)
