@@ -128,6 +128,9 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+K_DERIV = 5  # timed repetitions of the NEXT-1 block
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -231,6 +234,25 @@ def main():
     t_e2e = a.elapsed_time(b) * 1e-3
     clocks = sampler.stop()
 
+    # ---- E_L + parameter derivatives O (eq. 6 factors) and the gradient estimator,
+    # reported beside the headline (same walkers; O is [M][3 + n_det] doubles written to and read from HBM)
+    n_par = sysh.n_param()
+    O = torch.empty((M, n_par), dtype=torch.float64, device=dev)
+    t_d = t_g = 0.0
+    for k in range(3 + K_DERIV):
+        flush.fill_(k & 0xFF)
+        a, b, c = ev(), ev(), ev()
+        a.record(st)
+        sysh.log_derivatives(r, lp, sg, el, O)
+        b.record(st)
+        e_v, grad = qb.energy_gradient(el, O)
+        c.record(st)
+        torch.cuda.synchronize()
+        if k >= 3:
+            t_d += a.elapsed_time(b) * 1e-3
+            t_g += b.elapsed_time(c) * 1e-3
+    del O
+
     t_met, t_el, t_all, t_e2e = max_over_ranks([t_met, t_el, t_all, t_e2e], device=dev)
 
     K = args.steps
@@ -270,6 +292,11 @@ def main():
             "cpu_baseline": cpu,
             "e2e": {"value": e2e_rate, "unit": UNIT, "h2d_bytes_per_step": int(r_pin.numel() * 8),
                     "d2h_bytes_per_step": int(out_pin.numel() * 8)},
+            "log_derivatives": {"n_param": n_par, "ms_local_energy_plus_O": 1e3 * t_d / K_DERIV,
+                                "ms_energy_gradient": 1e3 * t_g / K_DERIV, "O_bytes": int(M) * n_par * 8,
+                                "gradient_hbm_gbs": int(M) * (n_par + 1) * 8 / (t_g / K_DERIV) / 1e9,
+                                "E_v": e_v, "grad_norm": float(np.linalg.norm(grad)),
+                                "note": "SURVEY 8(f) NEXT-1, eq. 6; gradient time includes batch stats, the D2H of the result and a stream synchronise"},
             "gpu_launches": int(launches),
             "clocks": clocks,
             "last_step": {"mean_E_L": mean, "stderr": err},

@@ -669,7 +669,7 @@ int qmc_energy_gradient(const double *d_eloc, const double *d_O, int64_t M, int3
   double *d_stats = scr, *d_grad = scr + 2, *d_part = d_grad + n_param;
   batch_stats_kernel<<<1, 1024, 0, st>>>(d_eloc, M, d_stats);
   gradient_partial_kernel<<<nblk, 128, 0, st>>>(d_eloc, d_O, M, n_param, d_stats, d_part);
-  gradient_final_kernel<<<(n_param + 127) / 128, 128, 0, st>>>(d_part, nblk, n_param, M, d_grad);
+  gradient_final_kernel<<<n_param, 128, 0, st>>>(d_part, nblk, n_param, M, d_grad);
   g_launches += 3;
   std::vector<double> h((size_t)n_param + 2);
   cudaError_t e = cudaMemcpyAsync(h.data(), scr, h.size() * sizeof(double), cudaMemcpyDeviceToHost, st);

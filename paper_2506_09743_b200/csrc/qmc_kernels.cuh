@@ -297,15 +297,22 @@ __global__ void __launch_bounds__(128) gradient_partial_kernel(const double *__r
 }
 __global__ void __launch_bounds__(128) gradient_final_kernel(const double *__restrict__ partial, int nblk, int np, int64_t M,
                                                              double *__restrict__ grad) {
-  const int p = blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= np) return;
+  // one block per parameter: thread t adds the block partials t, t + 128, ... in order, then a fixed tree
+  __shared__ double sh[128];
+  const int p = blockIdx.x;
   double s = 0.0, c = 0.0;
-  for (int b = 0; b < nblk; ++b) {
+  for (int b = threadIdx.x; b < nblk; b += blockDim.x) {
     const double y = partial[(int64_t)b * np + p] - c, t = s + y;
     c = (t - s) - y;
     s = t;
   }
-  grad[p] = 2.0 * s / (double)M;
+  sh[threadIdx.x] = s;
+  __syncthreads();
+  for (int w = 64; w > 0; w >>= 1) {
+    if ((int)threadIdx.x < w) sh[threadIdx.x] += sh[threadIdx.x + w];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) grad[p] = 2.0 * sh[0] / (double)M;
 }
 
 // ---------------------------------------------------------------------------------
