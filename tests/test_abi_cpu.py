@@ -32,6 +32,20 @@ def test_status_strings_and_null_arguments():
     assert L.qmc_metropolis(None, None, 4, 0.1, 1, 0, 0, 0, None, None, None, None, None, None) == qb.QMC_EINVAL
     L.qmc_destroy(None)
     assert L.qmc_model_flops(None, 0) == 0.0
+    assert L.qmc_n_param(None) == qb.QMC_EINVAL
+    assert L.qmc_log_derivatives(None, None, 4, None, None, None, None, None) == qb.QMC_EINVAL
+    g = np.zeros(3)
+    assert L.qmc_energy_gradient(None, None, 4, 3, None, g.ctypes.data, None) == qb.QMC_EINVAL
+
+
+def test_record_stream_limit_is_reported_before_any_cuda_call():
+    # more shell + atom records than the kernel parameter block holds: QMC_EUNSUPPORTED, not a crash
+    from tests.helpers import atom_system
+    n = 230
+    d = atom_system(1.0, [(1, 0, 0, 0.5 + 0.01 * i) for i in range(n)], np.ones((n, 1)), 1, 0)
+    desc, keep = qb.make_desc(d)
+    h = C.c_void_p()
+    assert qb.lib().qmc_setup(C.addressof(desc), 0, C.byref(h)) == qb.QMC_EUNSUPPORTED
 
 
 def test_setup_validation_happens_before_any_cuda_call():

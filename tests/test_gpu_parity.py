@@ -130,6 +130,26 @@ def test_three_atoms_many_shell_kinds(env):
     check_local_energy(env, d, r, threads=4)
 
 
+def test_centre_without_basis_functions_and_many_shells(env):
+    # a bare point charge (no AOs on it) still enters V_en and V_nn; 40 s shells on the other centre cross
+    # several 16-row AO chunks
+    rng = np.random.default_rng(9)
+    from paper_2506_09743_b200.workloads import SystemDesc
+    xyz = np.array([[0.0, 0.0, 0.0], [0.0, 1.1, 1.7]])
+    n = 40
+    zeta = rng.uniform(0.4, 3.0, n)
+    z = np.zeros(n, np.int32)
+    Cm = np.linalg.qr(rng.standard_normal((n, n)))[0][:, :4]
+    d = SystemDesc("bare", xyz, np.array([3.0, 2.0]), 2, 1, z, np.ones(n, np.int32), z, z, zeta, None, Cm,
+                   np.array([[0, 1], [0, 2], [3, 1]], np.int32), np.array([[0], [0], [1]], np.int32),
+                   np.array([0.9, 0.2, -0.1]))
+    r = wl.make_walkers(rng, xyz, 3, 129)
+    el0, el = check_local_energy(env, d, r, threads=2)
+    torch, ob, qb = env
+    parts = ob.local_energy(ob.OracleSystem(d), r, parts=True)[3]
+    assert abs(parts[0, 3] - 3.0 * 2.0 / np.linalg.norm(xyz[1])) < 1e-13  # V_nn counts the bare charge
+
+
 # ----------------------------------------------------------------------------- Metropolis
 def check_metropolis(env, d, r, step, n_sweeps, seed, threads=8, eloc_acc=False):
     torch, ob, qb = env
