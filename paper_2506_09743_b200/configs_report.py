@@ -1,0 +1,120 @@
+"""All five BASELINE.json configurations on one GPU: absolute rates and the fraction of the FP64 roofline.
+
+    python -m paper_2506_09743_b200.configs_report [--scan-geometries 16]
+
+Per configuration: device time of qmc_local_energy (walker*E_L/s) and of qmc_metropolis with the
+configuration's own sweep count and step (walker-steps/s), both as model FP64 TFLOP/s (qmc_model_flops) and as
+a fraction of the DFMA peak measured in the same process.  Configuration 5 (CO dissociation scan) runs its 50
+sweeps with E_L after every sweep and reports mean E_L and its standard error per geometry (DESIGN.md reading
+Q16: per-walker sweep average first, then the standard error over walkers; no burn-in is discarded -- this is a
+throughput and parity benchmark, not a physics result).  CUDA events on the current stream around 10 back-to-back calls, 3 warm-ups,
+best of 3 batches.  There is no CPU fallback: without a GPU this raises.
+"""
+from __future__ import annotations
+
+import argparse
+
+import torch
+
+from . import binding as qb
+from . import workloads as wl
+
+
+def _time(fn, reps=10, warm=3):
+    """mean device time of fn: `reps` calls enqueued back to back between two events (the host runs ahead,
+    so launch latency is not part of the figure), best of 3 such batches"""
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    best = float("inf")
+    for _ in range(3):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        best = min(best, a.elapsed_time(b) * 1e-3 / reps)
+    return best
+
+
+def measure(name, d, r_host, peak):
+    s = qb.QmcSystem(d, 0)
+    M = r_host.shape[2]
+    r0 = torch.from_numpy(r_host).cuda()
+    r = r0.clone()
+    lp = torch.empty(M, dtype=torch.float64, device="cuda")
+    sg, el = torch.empty_like(lp), torch.empty_like(lp)
+    sweeps, step = int(d.extra.get("sweeps", 10)), float(d.extra.get("step", 0.3))
+    s.metropolis(r, step, sweeps, seed=1, logpsi=lp, sign=sg)  # equilibrate a little: time E_L on sampled walkers
+    t_el = _time(lambda: s.local_energy(r, lp, sg, el))
+
+    def met():
+        r.copy_(r0)
+        s.metropolis(r, step, sweeps, seed=1, logpsi=lp, sign=sg)
+
+    t_cp = _time(lambda: r.copy_(r0))
+    t_met = _time(met) - t_cp
+    f_el, f_st = s.model_flops(0), s.model_flops(1)
+    row = dict(config=name, n_e=d.n_e, n_ao=d.n_ao, n_det=d.n_det, walkers=M, el_ms=1e3 * t_el, el_rate=M / t_el,
+               el_tflops=f_el * M / t_el / 1e12, el_frac=f_el * M / t_el / 1e12 / peak, sweeps=sweeps,
+               met_ms=1e3 * t_met, met_rate=M * sweeps / t_met, met_tflops=f_st * M * sweeps / t_met / 1e12,
+               met_frac=f_st * M * sweeps / t_met / 1e12 / peak)
+    s.close()
+    return row
+
+
+def scan(n_geom, peak):
+    """BASELINE configs[4]: per geometry 50 sweeps with E_L after every sweep."""
+    out = []
+    t_total = 0.0
+    for d, r_host in wl.co_scan(n_geom=n_geom):
+        s = qb.QmcSystem(d, 0)
+        M = r_host.shape[2]
+        r = torch.from_numpy(r_host).cuda()
+        sweeps, step = int(d.extra["sweeps"]), float(d.extra["step"])
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        res = s.metropolis(r, step, sweeps, seed=5, want_eloc_acc=True)
+        mean, err = qb.batch_stats(res["eloc_acc"] / sweeps)
+        b.record()
+        torch.cuda.synchronize()
+        t = a.elapsed_time(b) * 1e-3
+        t_total += t
+        flops = (s.model_flops(0) + s.model_flops(1)) * M * sweeps
+        out.append(dict(R=float(d.extra["R"]), mean_E_L=mean, stderr=err, seconds=t, tflops=flops / t / 1e12,
+                        frac=flops / t / 1e12 / peak, walkers=M, sweeps=sweeps))
+        s.close()
+    return out, t_total
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--scan-geometries", type=int, default=16)
+    args = ap.parse_args()
+    if not torch.cuda.is_available():
+        raise SystemExit("configs_report needs a CUDA device: the product path has no CPU fallback")
+    peak = qb.fp64_peak(0, reps=5)
+    rows = [measure("H2", *wl.h2(), peak), measure("LiH", *wl.lih(), peak), measure("Li2 (30 AOs)", *wl.li2(), peak),
+            measure("Li2-28", *wl.li2(variant="28"), peak), measure("CO", *wl.co(), peak)]
+    print(f"DFMA peak measured in this process: {peak:.1f} TFLOP/s")
+    print("| config | N_e | N_AO | N_det | walkers | E_L call ms | M walker*E_L/s | model TFLOP/s | of DFMA peak | sweeps | "
+          "Metropolis ms | M walker-steps/s | model TFLOP/s | of DFMA peak |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+    for x in rows:
+        print(f"| {x['config']} | {x['n_e']} | {x['n_ao']} | {x['n_det']} | {x['walkers']} | {x['el_ms']:.3f} | "
+              f"{x['el_rate'] / 1e6:.1f} | {x['el_tflops']:.2f} | {100 * x['el_frac']:.1f} % | {x['sweeps']} | "
+              f"{x['met_ms']:.3f} | {x['met_rate'] / 1e6:.1f} | {x['met_tflops']:.2f} | {100 * x['met_frac']:.1f} % |")
+    if args.scan_geometries > 0:
+        geo, t_total = scan(args.scan_geometries, peak)
+        print(f"\nCO scan (500 determinants, {geo[0]['walkers']} walkers per geometry, {geo[0]['sweeps']} sweeps + E_L on every "
+              f"sweep): {len(geo)} geometries in {t_total:.2f} s")
+        print("| R (bohr) | mean E_L (Ha) | std error | seconds | model TFLOP/s | of DFMA peak |")
+        print("|---|---|---|---|---|---|")
+        for g in geo:
+            print(f"| {g['R']:.2f} | {g['mean_E_L']:.5f} | {g['stderr']:.5f} | {g['seconds']:.3f} | {g['tflops']:.2f} | "
+                  f"{100 * g['frac']:.1f} % |")
+
+
+if __name__ == "__main__":
+    main()
