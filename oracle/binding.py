@@ -41,6 +41,7 @@ class _Desc(C.Structure):
         ("n_mo", C.c_int32), ("mo_coeff", C.c_void_p),
         ("n_det", C.c_int32), ("det_up", C.c_void_p), ("det_dn", C.c_void_p), ("ci_coeff", C.c_void_p),
         ("jastrow_a_par", C.c_double), ("jastrow_a_anti", C.c_double), ("jastrow_b", C.c_double),
+        ("jastrow_en_w0", C.c_double), ("jastrow_en_w1", C.c_double), ("jastrow_en_w2", C.c_double),
     ]
 
 
@@ -102,7 +103,9 @@ class OracleSystem:
                        self.n_ao, _p(k["ao_atom"]), _p(k["ao_n"]), _p(k["ao_l"]), _p(k["ao_m"]),
                        _p(k["ao_zeta"]), _p(k["ao_norm"]), int(k["mo_coeff"].shape[1]), _p(k["mo_coeff"]),
                        int(k["ci_coeff"].shape[0]), _p(k["det_up"]), _p(k["det_dn"]), _p(k["ci_coeff"]),
-                       float(d.jastrow_a_par), float(d.jastrow_a_anti), float(d.jastrow_b))
+                       float(d.jastrow_a_par), float(d.jastrow_a_anti), float(d.jastrow_b),
+                 float(getattr(d, "jastrow_en_w0", 0.0)), float(getattr(d, "jastrow_en_w1", 0.0)),
+                 float(getattr(d, "jastrow_en_w2", 0.0)))
         self.ref = C.addressof(self.c)
 
 

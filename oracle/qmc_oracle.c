@@ -182,6 +182,39 @@ static void jastrow_all(const oracle_system_desc_t *s, const double *r, double *
       /* lap_i K + lap_j K = 2 (u'' + 2 u'/r) */
       *lapJ += 2.0 * (u2 + 2.0 * u1 / rij);
     }
+  /* electron-nucleus kernel (D.2): K_en(r) = N / D, N = w0 r + w1 r^2, D = 1 + w2 r,
+   * summed over every (electron, nucleus) pair; quotient rule long-hand */
+  double w0 = s->jastrow_en_w0, w1 = s->jastrow_en_w1, w2 = s->jastrow_en_w2;
+  if (w0 != 0.0 || w1 != 0.0)
+    for (int i = 0; i < ne; ++i)
+      for (int at = 0; at < s->n_atoms; ++at) {
+        double d[3];
+        for (int c = 0; c < 3; ++c) d[c] = r[3 * i + c] - s->atom_xyz[3 * at + c];
+        double ria = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        double N = w0 * ria + w1 * ria * ria, D = 1.0 + w2 * ria;
+        double N1 = w0 + 2.0 * w1 * ria, N2 = 2.0 * w1, D1 = w2;
+        double K = N / D;
+        double K1 = (N1 * D - N * D1) / (D * D);
+        /* (N'D - N D')' = N''D - N D'' = N''D ;  K'' = N''D / D^2 - 2 D' (N'D - N D') / D^3 */
+        double K2 = N2 * D / (D * D) - 2.0 * D1 * (N1 * D - N * D1) / (D * D * D);
+        *J += K;
+        for (int c = 0; c < 3; ++c) gJ[3 * i + c] += K1 * d[c] / ria;
+        *lapJ += K2 + 2.0 * K1 / ria;
+      }
+}
+
+/* value of the electron-nucleus part of J alone (D.2) */
+static double jastrow_en_value(const oracle_system_desc_t *s, const double *r) {
+  int ne = s->n_up + s->n_dn;
+  double J = 0.0;
+  for (int i = 0; i < ne; ++i)
+    for (int at = 0; at < s->n_atoms; ++at) {
+      double dx = r[3 * i] - s->atom_xyz[3 * at], dy = r[3 * i + 1] - s->atom_xyz[3 * at + 1],
+             dz = r[3 * i + 2] - s->atom_xyz[3 * at + 2];
+      double ria = sqrt(dx * dx + dy * dy + dz * dz);
+      J += (s->jastrow_en_w0 * ria + s->jastrow_en_w1 * ria * ria) / (1.0 + s->jastrow_en_w2 * ria);
+    }
+  return J;
 }
 
 /* ------------------------------------------------------------------ */
@@ -415,6 +448,7 @@ static void logpsi_one(const oracle_system_desc_t *s, const double *r, double *w
       double rij = sqrt(dx * dx + dy * dy + dz * dz);
       J += a * rij / (1.0 + s->jastrow_b * rij);
     }
+  J += jastrow_en_value(s, r);
   double sigma = 0.0;
   for (int n = 0; n < s->n_det; ++n) {
     double D[2];

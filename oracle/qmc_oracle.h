@@ -44,6 +44,8 @@ typedef struct {
   const int32_t *det_up, *det_dn; /* [n_det][n_up], [n_det][n_dn] ordered MO columns */
   const double *ci_coeff;         /* [n_det] */
   double jastrow_a_par, jastrow_a_anti, jastrow_b;
+  /* electron-nucleus kernel (D.2): K_en(r) = (w0 r + w1 r^2) / (1 + w2 r), all zero = absent */
+  double jastrow_en_w0, jastrow_en_w1, jastrow_en_w2;
 } oracle_system_desc_t;
 
 /* All pointers are HOST pointers.  Walker arrays are SoA [n_e][3][M]; the

@@ -34,6 +34,7 @@ class _Desc(C.Structure):
         ("n_mo", C.c_int32), ("mo_coeff", C.c_void_p),
         ("n_det", C.c_int32), ("det_up", C.c_void_p), ("det_dn", C.c_void_p), ("ci_coeff", C.c_void_p),
         ("jastrow_a_par", C.c_double), ("jastrow_a_anti", C.c_double), ("jastrow_b", C.c_double),
+        ("jastrow_en_w0", C.c_double), ("jastrow_en_w1", C.c_double), ("jastrow_en_w2", C.c_double),
     ]
 
 
@@ -108,7 +109,9 @@ def make_desc(d):
                  int(k["ao_atom"].shape[0]), _np(k["ao_atom"]), _np(k["ao_n"]), _np(k["ao_l"]), _np(k["ao_m"]),
                  _np(k["ao_zeta"]), _np(k["ao_norm"]), int(k["mo_coeff"].shape[1]), _np(k["mo_coeff"]),
                  int(k["ci_coeff"].shape[0]), _np(k["det_up"]), _np(k["det_dn"]), _np(k["ci_coeff"]),
-                 float(d.jastrow_a_par), float(d.jastrow_a_anti), float(d.jastrow_b))
+                 float(d.jastrow_a_par), float(d.jastrow_a_anti), float(d.jastrow_b),
+                 float(getattr(d, "jastrow_en_w0", 0.0)), float(getattr(d, "jastrow_en_w1", 0.0)),
+                 float(getattr(d, "jastrow_en_w2", 0.0)))
     return desc, k
 
 

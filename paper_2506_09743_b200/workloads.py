@@ -47,6 +47,9 @@ class SystemDesc:
     jastrow_a_par: float = 0.25
     jastrow_a_anti: float = 0.5
     jastrow_b: float = 1.0
+    jastrow_en_w0: float = 0.0  # electron-nucleus kernel (D.2), all zero = absent
+    jastrow_en_w1: float = 0.0
+    jastrow_en_w2: float = 0.0
     extra: dict = field(default_factory=dict)
 
     @property

@@ -637,3 +637,60 @@ def test_energy_gradient_estimator():
     el = ob.local_energy(o, r)[2]
     ev, g = ob.energy_gradient(el, ob.log_derivatives(o, r))
     assert abs(ev + 0.5) < 1e-12 and np.max(np.abs(g)) < 1e-11
+
+
+# ---------------------------------------------------------------- electron-nucleus Jastrow (D.2)
+def _with_en(d, w0, w1, w2):
+    import copy
+    d2 = copy.copy(d)
+    d2.jastrow_en_w0, d2.jastrow_en_w1, d2.jastrow_en_w2 = w0, w1, w2
+    return d2
+
+
+@pytest.mark.parametrize("Z,zeta,w", [(1.0, 1.0, (0.3, -0.05, 0.7)), (3.0, 2.2, (-0.4, 0.1, 1.3))])
+def test_en_jastrow_hydrogenlike_closed_form(Z, zeta, w):
+    # one electron: Psi = N exp(f(r)), f = -zeta r + K_en(r); E_L = -1/2 (f'' + 2 f'/r + f'^2) - Z/r.
+    # K' and K'' from the partial-fraction form K = A r + B (1 - 1/(1 + w2 r)), A = w1/w2, B = (w0 - A)/w2,
+    # an algebraically different route from the oracle's quotient rule
+    w0, w1, w2 = w
+    d = _with_en(atom_system(Z, [(1, 0, 0, zeta)], [[1.0]], 1, 0), w0, w1, w2)
+    rr = _rand_pos(100, 1, 1.5, rmin=0.05, seed=90)
+    lp, sg, el = ob.local_energy(ob.OracleSystem(d), soa(rr))
+    r = np.linalg.norm(rr[:, 0], axis=1)
+    A = w1 / w2
+    B = (w0 - A) / w2
+    D = 1 + w2 * r
+    K = A * r + B * (1 - 1 / D)
+    K1 = A + B * w2 / D ** 2
+    K2 = -2 * B * w2 ** 2 / D ** 3
+    f1 = -zeta + K1
+    ref = -0.5 * (K2 + 2 * f1 / r + f1 ** 2) - Z / r
+    assert np.max(np.abs(el - ref) / np.maximum(1, np.abs(ref))) < 1e-12
+    N = zeta ** 1.5 / math.sqrt(math.pi)
+    assert np.max(np.abs(lp - (math.log(N) - zeta * r + K))) < 1e-12
+
+
+def test_en_jastrow_finite_differences_and_sampler_value():
+    # analytic grad / Laplacian of the e-n term against Richardson differences of the plain Psi (two centres,
+    # several electrons, together with the e-e term), and the sampler's value-only route against it
+    for name, M in (("LiH", 6), ("CO", 3)):
+        d, r = wl.CONFIGS[name](M=64)
+        d = _with_en(d, 0.35, -0.04, 0.9)
+        o = ob.OracleSystem(d)
+        lp_all = ob.local_energy(o, r)[0]
+        idx = _keep_away(d, r)
+        idx = idx[np.argsort(-lp_all[idx])][:M]  # well away from nuclei and nodes (Q17)
+        rk = np.ascontiguousarray(r[:, :, idx])
+        _fd_check(d, rk, nwalk=len(idx), tol=2e-6)
+        lp = ob.local_energy(o, rk)[0]
+        out = ob.metropolis(o, rk, 0.2, 0, seed=1)
+        assert np.max(np.abs(out["logpsi"] - lp)) < 1e-12
+
+
+def test_en_jastrow_absent_when_parameters_are_zero():
+    d, r = wl.li2(M=16)
+    a = ob.local_energy(ob.OracleSystem(d), r)
+    b = ob.local_energy(ob.OracleSystem(_with_en(d, 0.0, 0.0, 0.8)), r)
+    assert all(np.array_equal(x, y) for x, y in zip(a, b))
+    c = ob.local_energy(ob.OracleSystem(_with_en(d, 0.2, 0.0, 0.8)), r)
+    assert np.max(np.abs(c[2] - a[2])) > 1e-3
