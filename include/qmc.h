@@ -75,6 +75,10 @@ typedef struct {
   double jastrow_a_par;  /* w0 for parallel spins      (cusp value 1/4) */
   double jastrow_a_anti; /* w0 for anti-parallel spins (cusp value 1/2) */
   double jastrow_b;      /* w */
+  /* Electron-nucleus Jastrow kernel (D.2), summed over every
+   * (electron, nucleus) pair with one parameter set: K_en(r) = (w0 r + w1 r^2) / (1 + w2 r).
+   * w0 = w1 = 0 switches the term off. */
+  double jastrow_en_w0, jastrow_en_w1, jastrow_en_w2;
 } qmc_system_desc_t;
 
 /* Validate `desc`, preprocess it (shell grouping, excitation tables relative to

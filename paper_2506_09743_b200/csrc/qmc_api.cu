@@ -166,6 +166,10 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   P.a_par = d->jastrow_a_par;
   P.a_anti = d->jastrow_a_anti;
   P.b = d->jastrow_b;
+  P.en_w0 = d->jastrow_en_w0;
+  P.en_w1 = d->jastrow_en_w1;
+  P.en_w2 = d->jastrow_en_w2;
+  P.has_en = (d->jastrow_en_w0 != 0.0 || d->jastrow_en_w1 != 0.0) ? 1 : 0;
   for (int a = 0; a < d->n_atoms; ++a) {
     for (int c = 0; c < 3; ++c) P.atom[a][c] = d->atom_xyz[3 * a + c];
     P.atom[a][3] = d->atom_Z[a];
@@ -461,9 +465,13 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     }
     s->flops_el = ne * nat * (8 + csqrt + cdiv) + ne * nsh * (8 + cexp) + ne * nao * 21 + 2 * ne * nao * nmo * 2 +
                   npair * (35 + csqrt + 2 * cdiv) + lu_el + 15 * nd + 100;
+    if (P.has_en) {  // D.2 per (electron, nucleus): K, K', K'', gradient and Laplacian shares (the distance is reused)
+      s->flops_el += ne * nat * (22 + cdiv);
+    }
     const double npr = std::ceil(3 * ne / 2);
     s->flops_step = ne * nat * (8 + csqrt + cdiv) + ne * nsh * (2 + cexp) + ne * nao * 3 + 2 * ne * nao * nmo +
                     npair * (12 + csqrt + cdiv) + lu_st + 3 * nd + 3 * ne * 2 + npr * (10 + clog + csqrt + csincos) + clog;
+    if (P.has_en) s->flops_step += ne * nat * (5 + cdiv);
   }
 
   // ---- upload

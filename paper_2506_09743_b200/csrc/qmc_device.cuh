@@ -107,6 +107,8 @@ struct SysParams {  // passed by value to every kernel
   int c_doubles;                   // size of the C fragment table
   int n_chunks;                    // AO chunks of kChunk rows
   double a_par, a_anti, b, vnn;
+  double en_w0, en_w1, en_w2;      // electron-nucleus Jastrow kernel (D.2); has_en = 0 when w0 = w1 = 0
+  int has_en;
   double atom[kMaxAtoms][4];       // x, y, z, Z
   int shell_begin[kMaxAtoms + 1];  // shells of atom a: [shell_begin[a], shell_begin[a+1])
   int8_t ref_col[2][kMaxSpin];     // kernel MO column of reference position j, per spin

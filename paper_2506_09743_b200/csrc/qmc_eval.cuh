@@ -153,6 +153,30 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
     }
   }
 
+  // ---- electron-nucleus Jastrow kernel (D.2): K = N / D, N = w0 r + w1 r^2, D = 1 + w2 r,
+  //   K' = (N' - w2 K) / D,  K'' = (N'' - 2 w2 K') / D;  grad_i J += K' d / r,  lap_i J += K'' + 2 K'/r.
+  // It has to precede the AO stage, whose combined operator uses the complete grad J.
+  if (P.has_en) {
+    for (int at = 0; at < P.n_atoms; ++at) {
+      const double dx = x - P.atom[at][0], dy = y - P.atom[at][1], dz = z - P.atom[at][2];
+      const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+      const double ri = rsqrt_fast(r2);
+      const double r = r2 * ri;
+      const double di = rcp_fast(fma(P.en_w2, r, 1.0));
+      const double K = r * fma(P.en_w1, r, P.en_w0) * di;
+      Jp += K;
+      if (EL) {
+        const double K1 = (fma(2.0 * P.en_w1, r, P.en_w0) - P.en_w2 * K) * di;
+        const double K2 = 2.0 * fma(-P.en_w2, K1, P.en_w1) * di;
+        const double sc = K1 * ri;
+        gJx = fma(sc, dx, gJx);
+        gJy = fma(sc, dy, gJy);
+        gJz = fma(sc, dz, gJz);
+        lapJ += fma(2.0, sc, K2);
+      }
+    }
+  }
+
   // ---- stages a1-a4: STO shells and AO -> MO contraction.
   // For E_L the gradient and Laplacian are folded into ONE operator per AO (stage a6):
   //   b = -1/2 lap(phi) - grad_i J . grad(phi)      (middle and last terms of F.1)

@@ -397,3 +397,39 @@ def test_log_derivatives_general_substitutions_and_unequal_spins(env):
                     a_par=0.25, a_anti=0.5, b=0.8, xyz=(0.1, -0.2, 0.3))
     r = soa(rng.standard_normal((257, 6, 3)) * 1.3)
     check_log_derivatives(env, d, r, threads=2)
+
+
+# ----------------------------------------------------------------------------- electron-nucleus Jastrow (D.2)
+def _with_en(d, w0, w1, w2):
+    import copy
+    d2 = copy.copy(d)
+    d2.jastrow_en_w0, d2.jastrow_en_w1, d2.jastrow_en_w2 = w0, w1, w2
+    return d2
+
+
+@pytest.mark.parametrize("name,M", [("H2", 515), ("LiH", 700), ("Li2", 1027), ("CO", 1025)])
+def test_en_jastrow_local_energy_and_metropolis(env, name, M):
+    d, r = wl.CONFIGS[name](M=M)
+    d = _with_en(d, 0.35, -0.04, 0.9)
+    el0, el = check_local_energy(env, d, r)
+    # the term is really there: E_L differs from the e-e-only wavefunction's
+    torch, ob, qb = env
+    el_plain = ob.local_energy(ob.OracleSystem(_with_en(d, 0.0, 0.0, 0.9)), r[:, :, :8])[2]
+    assert np.max(np.abs(el_plain - el0[:8])) > 1e-3
+    check_metropolis(env, d, r[:, :, :257], 0.25, 6, seed=11)
+    check_log_derivatives(env, d, r[:, :, :129])
+
+
+def test_en_jastrow_three_atoms_unequal_spins(env):
+    rng = np.random.default_rng(21)
+    from paper_2506_09743_b200.workloads import SystemDesc, expand_shells
+    xyz = np.array([[0, 0, 0], [1.8, 0.2, 0], [-0.5, 1.6, 0.4]], float)
+    ao = expand_shells([["1s", "2s", "2p"], ["1s", "2p"], ["1s", "1s"]], rng.uniform(0.6, 3.0, 7))
+    n_ao = len(ao[0])
+    Cm = np.linalg.qr(rng.standard_normal((n_ao, n_ao)))[0][:, :6]
+    d = SystemDesc("tri-en", xyz, np.array([4.0, 1.0, 1.0]), 3, 2, *ao, None, Cm,
+                   np.array([[0, 1, 2], [0, 3, 2], [4, 1, 5]], np.int32), np.array([[0, 1], [0, 1], [2, 1]], np.int32),
+                   np.array([0.9, 0.2, -0.15]), 0.25, 0.5, 0.8, -0.3, 0.06, 1.1)
+    r = wl.make_walkers(rng, xyz, 5, 333)
+    check_local_energy(env, d, r, threads=4)
+    check_metropolis(env, d, r[:, :, :200], 0.3, 5, seed=3)
