@@ -106,6 +106,16 @@ void qmc_destroy(qmc_system_t *s);
 int qmc_local_energy(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign,
                      double *d_eloc, void *cuda_stream);
 
+/* qmc_local_energy with HOST buffers (the end-to-end call): h_r host double [n_e][3][M], outputs host
+ * double [M] each (any may be NULL).  The walkers are cut into n_chunks contiguous ranges that are
+ * pipelined over two internal streams -- strided H2D copy of the range, the kernels, D2H of the three
+ * outputs -- so copies overlap computation; page-locked host memory is needed for that overlap, pageable
+ * memory works but serialises.  Device scratch (double-buffered, sized for one chunk) belongs to the handle,
+ * so concurrent host-variant calls on ONE handle are not allowed.  Synchronous: the outputs are in host
+ * memory on return.  Results are identical to qmc_local_energy's (walkers are independent). */
+int qmc_local_energy_host(qmc_system_t *s, const double *h_r, int64_t M, double *h_logpsi, double *h_sign,
+                          double *h_eloc, int32_t n_chunks);
+
 /* log|Psi| and sign only (the part of the path the sampler needs). Same arguments. */
 int qmc_log_psi(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign,
                 void *cuda_stream);

@@ -16,7 +16,7 @@ _lib = None
 
 EXPORTS = ["qmc_setup", "qmc_destroy", "qmc_local_energy", "qmc_log_psi", "qmc_metropolis", "qmc_batch_stats",
            "qmc_fp64_peak", "qmc_model_flops", "qmc_launch_count", "qmc_status_string", "qmc_n_param",
-           "qmc_log_derivatives", "qmc_energy_gradient"]
+           "qmc_log_derivatives", "qmc_energy_gradient", "qmc_local_energy_host"]
 
 
 class QmcError(RuntimeError):
@@ -55,6 +55,8 @@ def lib():
         L.qmc_destroy.argtypes = [vp]
         L.qmc_local_energy.restype = C.c_int
         L.qmc_local_energy.argtypes = [vp, vp, i64, vp, vp, vp, vp]
+        L.qmc_local_energy_host.restype = C.c_int
+        L.qmc_local_energy_host.argtypes = [vp, vp, i64, vp, vp, vp, C.c_int32]
         L.qmc_log_psi.restype = C.c_int
         L.qmc_log_psi.argtypes = [vp, vp, i64, vp, vp, vp]
         L.qmc_metropolis.restype = C.c_int
@@ -153,6 +155,20 @@ class QmcSystem:
         eloc = new() if eloc is None else eloc
         _check(lib().qmc_local_energy(self._h, _dp(r), M, _dp(logpsi), _dp(sign), _dp(eloc), _stream(stream)))
         return logpsi, sign, eloc
+
+    def local_energy_host(self, r_host, out_host=None, n_chunks: int = 2):
+        """qmc_local_energy_host: r_host float64 CPU tensor [n_e,3,M] (pinned for copy/compute overlap) ->
+        out_host float64 CPU tensor [3,M] = (logpsi, sign, eloc).  Synchronous."""
+        assert (not r_host.is_cuda) and r_host.dtype == torch.float64 and r_host.is_contiguous()
+        assert r_host.dim() == 3 and r_host.shape[0] == self.n_e and r_host.shape[1] == 3
+        M = int(r_host.shape[2])
+        if out_host is None:
+            out_host = torch.empty((3, M), dtype=torch.float64).pin_memory()
+        assert (not out_host.is_cuda) and out_host.dtype == torch.float64 and out_host.is_contiguous()
+        assert tuple(out_host.shape) == (3, M)
+        _check(lib().qmc_local_energy_host(self._h, r_host.data_ptr(), M, out_host[0].data_ptr(), out_host[1].data_ptr(),
+                                           out_host[2].data_ptr(), int(n_chunks)))
+        return out_host
 
     def log_psi(self, r, logpsi=None, sign=None, stream=None):
         M = self._chk_r(r)

@@ -93,6 +93,10 @@ struct qmc_system {
   double *d_stats = nullptr;
   unsigned long long *d_counter = nullptr;
   double flops_el = 0, flops_step = 0;
+  // qmc_local_energy_host: two internal streams and double-buffered device scratch (grown on demand)
+  cudaStream_t hst[2] = {nullptr, nullptr};
+  double *hbuf[2] = {nullptr, nullptr};
+  int64_t hbuf_walkers = 0;
 };
 
 extern "C" {
@@ -124,6 +128,10 @@ void qmc_destroy(qmc_system_t *s) {
   cudaFree(s->d_orig);
   cudaFree(s->d_stats);
   cudaFree(s->d_counter);
+  for (int i = 0; i < 2; ++i) {
+    if (s->hst[i]) cudaStreamDestroy(s->hst[i]);
+    cudaFree(s->hbuf[i]);
+  }
   delete s;
 }
 
@@ -579,6 +587,47 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
 int qmc_local_energy(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, double *d_eloc,
                      void *cuda_stream) {
   return launch_eval(s, d_r, M, d_logpsi, d_sign, d_eloc, cuda_stream, true);
+}
+
+int qmc_local_energy_host(qmc_system_t *s, const double *h_r, int64_t M, double *h_logpsi, double *h_sign,
+                          double *h_eloc, int32_t n_chunks) {
+  if (!s || !h_r || M <= 0 || n_chunks < 1) return QMC_EINVAL;
+  CK(cudaSetDevice(s->device));
+  const int ne = s->P.n_e;
+  int64_t Mc = (M + n_chunks - 1) / n_chunks;
+  Mc = (Mc + 31) / 32 * 32;  // whole warps' worth of groups per chunk
+  if (Mc > s->hbuf_walkers) {  // [3 n_e + 3][Mc] doubles per buffer: coordinates, then log|Psi|, sign, E_L
+    for (int i = 0; i < 2; ++i) {
+      if (!s->hst[i]) CK(cudaStreamCreateWithFlags(&s->hst[i], cudaStreamNonBlocking));
+      CK(cudaStreamSynchronize(s->hst[i]));
+      cudaFree(s->hbuf[i]);
+      s->hbuf[i] = nullptr;
+      CK(cudaMalloc(&s->hbuf[i], (size_t)(3 * ne + 3) * (size_t)Mc * sizeof(double)));
+    }
+    s->hbuf_walkers = Mc;
+  }
+  int rc = QMC_OK;
+  int c = 0;
+  for (int64_t a = 0; a < M && rc == QMC_OK; a += Mc, ++c) {
+    const int64_t m = std::min<int64_t>(Mc, M - a);
+    cudaStream_t st = s->hst[c & 1];
+    double *d_r = s->hbuf[c & 1], *d_out = d_r + (size_t)3 * ne * (size_t)m;
+    // rows of the SoA array are M doubles apart on the host and m doubles apart in the chunk buffer
+    CK(cudaMemcpy2DAsync(d_r, (size_t)m * sizeof(double), h_r + a, (size_t)M * sizeof(double), (size_t)m * sizeof(double),
+                         (size_t)3 * ne, cudaMemcpyHostToDevice, st));
+    rc = launch_eval(s, d_r, m, h_logpsi ? d_out : nullptr, h_sign ? d_out + m : nullptr, h_eloc ? d_out + 2 * m : nullptr,
+                     st, true);
+    if (rc != QMC_OK) break;
+    if (h_logpsi) CK(cudaMemcpyAsync(h_logpsi + a, d_out, (size_t)m * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (h_sign) CK(cudaMemcpyAsync(h_sign + a, d_out + m, (size_t)m * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (h_eloc) CK(cudaMemcpyAsync(h_eloc + a, d_out + 2 * m, (size_t)m * sizeof(double), cudaMemcpyDeviceToHost, st));
+  }
+  for (int i = 0; i < 2; ++i)
+    if (s->hst[i]) {
+      cudaError_t e = cudaStreamSynchronize(s->hst[i]);
+      if (e != cudaSuccess && rc == QMC_OK) rc = cuda_fail(e, "qmc_local_energy_host");
+    }
+  return rc;
 }
 
 int qmc_log_psi(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, void *cuda_stream) {

@@ -433,3 +433,21 @@ def test_en_jastrow_three_atoms_unequal_spins(env):
     r = wl.make_walkers(rng, xyz, 5, 333)
     check_local_energy(env, d, r, threads=4)
     check_metropolis(env, d, r[:, :, :200], 0.3, 5, seed=3)
+
+
+# ----------------------------------------------------------------------------- host-buffer entry point
+@pytest.mark.parametrize("M,chunks,pinned", [(1027, 4, True), (1027, 1, True), (33, 8, True), (515, 3, False)])
+def test_local_energy_host_matches_device_call(env, M, chunks, pinned):
+    torch, ob, qb = env
+    d, r = wl.co(M=M)
+    s = qb.QmcSystem(d)
+    ref = torch.stack(s.local_energy(_to_gpu(torch, r))).cpu()
+    rh = torch.from_numpy(np.ascontiguousarray(r))
+    out = torch.empty((3, M), dtype=torch.float64)
+    if pinned:
+        rh, out = rh.pin_memory(), out.pin_memory()
+    got = s.local_energy_host(rh, out, n_chunks=chunks)
+    assert torch.equal(got, ref)  # walkers are independent: chunking changes nothing, bit for bit
+    got2 = s.local_energy_host(rh, None, n_chunks=2)  # reuses / regrows the handle's scratch
+    assert torch.equal(got2, ref)
+    s.close()
