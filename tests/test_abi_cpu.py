@@ -86,3 +86,21 @@ def test_workload_shapes():
     d2, r2 = wl.co(M=16)
     d3, r3 = wl.co(M=16)
     assert np.array_equal(r2, r3) and np.array_equal(d2.ci_coeff, d3.ci_coeff)
+
+
+def test_bench_reference_arm_contract():
+    # bench.py --impl reference runs on the host cores (no GPU) and prints ONE JSON line with the contract's keys
+    import json
+    import subprocess
+    import sys
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
+                          "--warmup", "0"], capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for k in ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
+              "scaling", "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e", "gpu_launches"):
+        assert k in d, k
+    assert d["impl"] == "reference" and d["cpu_baseline"]["kind"] == "oracle" and d["value"] > 0
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["vs_baseline"] is None and d["dtype"] == "f64"
