@@ -10,9 +10,16 @@
  *
  * Conventions
  *  - "host" / "device" is stated for every pointer.  The caller owns every
- *    walker / output buffer; a qmc_system_t owns only device copies of the
- *    constants given to qmc_setup and is immutable afterwards (so it may be
- *    used from several streams concurrently).
+ *    walker / output buffer; a qmc_system_t owns device copies of the
+ *    constants given to qmc_setup, which are immutable afterwards, and small
+ *    scratch buffers: one per calling stream for the explicit fallback of
+ *    qmc_local_energy (grown on demand under a mutex), so calls on different
+ *    streams may run concurrently, and the double buffers of
+ *    qmc_local_energy_host (one such call at a time per handle).
+ *  - qmc_local_energy, qmc_log_psi, qmc_log_derivatives and qmc_metropolis
+ *    (without d_eloc_acc and h_n_accepted) make no allocation once a call of
+ *    the same size has been made on the stream, and can then be captured in
+ *    a CUDA graph.
  *  - Walker coordinates are SoA: double r[n_e][3][M], walker index fastest,
  *    electrons 0..n_up-1 spin-up, the rest spin-down, units bohr.
  *  - Every call returns QMC_OK (0) or a negative status; nothing aborts or

@@ -10,6 +10,8 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <mutex>
+#include <unordered_map>
 #include <vector>
 
 #include "qmc_kernels.cuh"
@@ -93,6 +95,11 @@ struct qmc_system {
   double *d_stats = nullptr;
   unsigned long long *d_counter = nullptr;
   double flops_el = 0, flops_step = 0;
+  // scratch of the explicit fallback, one buffer per calling stream (grown on demand, kept until qmc_destroy):
+  // no allocation on the hot call, and the call can be captured in a CUDA graph after one warm-up call
+  struct Scratch { void *p = nullptr; size_t bytes = 0; };
+  std::mutex scratch_mu;
+  std::unordered_map<cudaStream_t, Scratch> scratch;
   // qmc_local_energy_host: two internal streams and double-buffered device scratch (grown on demand)
   cudaStream_t hst[2] = {nullptr, nullptr};
   double *hbuf[2] = {nullptr, nullptr};
@@ -128,6 +135,7 @@ void qmc_destroy(qmc_system_t *s) {
   cudaFree(s->d_orig);
   cudaFree(s->d_stats);
   cudaFree(s->d_counter);
+  for (auto &kv : s->scratch) cudaFree(kv.second.p);
   for (int i = 0; i < 2; ++i) {
     if (s->hst[i]) cudaStreamDestroy(s->hst[i]);
     cudaFree(s->hbuf[i]);
@@ -565,7 +573,20 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
     // stream-ordered scratch of the explicit fallback: partial sums [groups + warps][G][2] doubles, then
     // ints: [0] = counter, [1 ..] = listed group indices, then the per-group slice counters
     const size_t n_part = (size_t)(groups + expl_warps) * (size_t)s->P.G * 2;
-    CK(cudaMallocAsync(&fb, n_part * sizeof(double) + (size_t)(2 * groups + 2) * sizeof(int), st));
+    const size_t need_bytes = n_part * sizeof(double) + (size_t)(2 * groups + 2) * sizeof(int);
+    {
+      std::lock_guard<std::mutex> lock(s->scratch_mu);
+      qmc_system::Scratch &sc = s->scratch[st];
+      if (sc.bytes < need_bytes) {  // grow: earlier work on this stream may still use the old buffer
+        CK(cudaStreamSynchronize(st));
+        cudaFree(sc.p);
+        sc.p = nullptr;
+        sc.bytes = 0;
+        CK(cudaMalloc(&sc.p, need_bytes));
+        sc.bytes = need_bytes;
+      }
+      fb = static_cast<double *>(sc.p);
+    }
     int *fbi = reinterpret_cast<int *>(fb + n_part);
     CK(cudaMemsetAsync(fbi, 0, sizeof(int), st));
     io.fb_part = fb;
@@ -579,7 +600,6 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
   if (fallback) {
     CK(cudaLaunchKernel(s->var.k_expl, dim3(s->blocks_expl), dim3(kWarpsEl * 32), args, s->smem_el, st));
     ++g_launches;
-    CK(cudaFreeAsync(fb, st));
   }
   return QMC_OK;
 }

@@ -94,7 +94,8 @@ constexpr double kFallbackK = 8.0e5;
 
 struct SysParams {  // passed by value to every kernel
   int n_atoms, n_up, n_dn, n_e;
-  int n_shell, n_ao, n_mo, n_det;  // n_mo = orbitals referenced (kernel order)
+  int n_shell, n_ao, n_mo, n_det;  // n_shell = records of the shell/atom stream; n_mo = orbitals referenced (kernel
+                                   // order); n_det = packed determinant records (classes 1-4)
   int n_a1, n_a2, n_b;             // class boundaries in dets[]: [0,n_a1) one entry, [n_a1,n_a2) two entries,
                                    // [n_a2,n_b) one 2x2 block, [n_b,n_det) two 2x2 blocks (qmc_setup)
   double d_ref;                    // summed coefficients of the determinants equal to the reference
@@ -110,7 +111,6 @@ struct SysParams {  // passed by value to every kernel
   double en_w0, en_w1, en_w2;      // electron-nucleus Jastrow kernel (D.2); has_en = 0 when w0 = w1 = 0
   int has_en;
   double atom[kMaxAtoms][4];       // x, y, z, Z
-  int shell_begin[kMaxAtoms + 1];  // shells of atom a: [shell_begin[a], shell_begin[a+1])
   int8_t ref_col[2][kMaxSpin];     // kernel MO column of reference position j, per spin
   int8_t virt_col[2][kMaxVirt];    // kernel MO column of virtual q, per spin
   ShellRec shells[kMaxShells];     // [n_shell] record stream: {SH_ATOM a, shells of a} per atom (n_shell counts both)

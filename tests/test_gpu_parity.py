@@ -451,3 +451,42 @@ def test_local_energy_host_matches_device_call(env, M, chunks, pinned):
     got2 = s.local_energy_host(rh, None, n_chunks=2)  # reuses / regrows the handle's scratch
     assert torch.equal(got2, ref)
     s.close()
+
+
+# ----------------------------------------------------------------------------- CUDA graphs
+@pytest.mark.parametrize("name", ["H2", "Li2"])
+def test_calls_can_be_captured_in_a_cuda_graph(env, name):
+    # after one warm-up call (which sizes the handle's per-stream fallback scratch) qmc_metropolis and
+    # qmc_local_energy contain nothing that breaks stream capture; a replay reproduces the eager run bit for bit
+    torch, ob, qb = env
+    d, r = wl.CONFIGS[name](M=777)
+    s = qb.QmcSystem(d)
+    r0 = _to_gpu(torch, r)
+    rg = r0.clone()
+    M = r.shape[2]
+    lp = torch.empty(M, dtype=torch.float64, device="cuda")
+    sg, el, acc = torch.empty_like(lp), torch.empty_like(lp), torch.zeros_like(lp)
+    st = torch.cuda.Stream()
+
+    def body(k):
+        s.metropolis(rg, 0.3, 1, seed=7, sweep_offset=k, logpsi=lp, sign=sg, stream=st)
+        s.local_energy(rg, lp, sg, el, stream=st)
+        acc.add_(el)
+
+    with torch.cuda.stream(st):
+        for k in range(4):
+            body(k)
+        ref_acc, ref_r = acc.clone(), rg.clone()
+        rg.copy_(r0)
+        acc.zero_()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            for k in range(4):
+                body(k)
+        rg.copy_(r0)
+        acc.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+    assert torch.equal(acc, ref_acc) and torch.equal(rg, ref_r)
+    s.close()
