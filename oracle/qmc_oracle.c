@@ -541,12 +541,12 @@ void oracle_batch_stats(const double *x, int64_t M, double *mean, double *stderr
 
 /* ------------------------------------------------------------------ */
 /* Parameter derivatives of ln Psi and the gradient estimator (eq. 6,   */
-/* PAPER.md:78).  theta = (a_par, a_anti, b, d_0 .. d_{n_det-1}).       */
+/* PAPER.md:78).  theta = (a_par, a_anti, b, en_w0, en_w1, en_w2, d_n). */
 /* ------------------------------------------------------------------ */
 
 int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                            int64_t w1, double *O) {
-  int ne = s->n_up + s->n_dn, nmo = s->n_mo, np = 3 + s->n_det;
+  int ne = s->n_up + s->n_dn, nmo = s->n_mo, np = 6 + s->n_det;
   double *mo = (double *)malloc(sizeof(double) * (size_t)(ne * nmo + 1));
   double *A = (double *)malloc(sizeof(double) * (size_t)(ne * ne + 1));
   double *pos = (double *)malloc(sizeof(double) * (size_t)(3 * ne + 1));
@@ -571,6 +571,22 @@ int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64
     out[0] = da_par;
     out[1] = da_anti;
     out[2] = db;
+    /* electron-nucleus kernel K = (w0 r + w1 r^2) / (1 + w2 r)  (D.2):
+     * dK/dw0 = r / D,  dK/dw1 = r^2 / D,  dK/dw2 = -(w0 r + w1 r^2) r / D^2,  D = 1 + w2 r */
+    double dw0 = 0.0, dw1 = 0.0, dw2 = 0.0;
+    for (int i = 0; i < ne; ++i)
+      for (int at = 0; at < s->n_atoms; ++at) {
+        double dx = pos[3 * i] - s->atom_xyz[3 * at], dy = pos[3 * i + 1] - s->atom_xyz[3 * at + 1],
+               dz = pos[3 * i + 2] - s->atom_xyz[3 * at + 2];
+        double ria = sqrt(dx * dx + dy * dy + dz * dz);
+        double D = 1.0 + s->jastrow_en_w2 * ria;
+        dw0 += ria / D;
+        dw1 += ria * ria / D;
+        dw2 += -(s->jastrow_en_w0 * ria + s->jastrow_en_w1 * ria * ria) * ria / (D * D);
+      }
+    out[3] = dw0;
+    out[4] = dw1;
+    out[5] = dw2;
     /* CI: Sigma = sum_n d_n D_n^up D_n^dn  (eq. 4):  d ln Sigma / d d_n = D_n^up D_n^dn / Sigma */
     for (int i = 0; i < ne * nmo; ++i) mo[i] = 0.0;
     for (int i = 0; i < ne; ++i)
@@ -591,7 +607,7 @@ int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64
       prod[n] = D[0] * D[1];
       sigma += s->ci_coeff[n] * prod[n];
     }
-    for (int n = 0; n < s->n_det; ++n) out[3 + n] = prod[n] / sigma;
+    for (int n = 0; n < s->n_det; ++n) out[6 + n] = prod[n] / sigma;
   }
   free(mo); free(A); free(pos); free(prod);
   return 0;

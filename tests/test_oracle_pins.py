@@ -554,7 +554,7 @@ def test_batch_stats():
 
 # ---------------------------------------------------------------- parameter derivatives (eq. 6)
 def _with_param(d, p, value):
-    """copy of the system with parameter p of theta = (a_par, a_anti, b, d_0 ...) set to value"""
+    """copy of the system with parameter p of theta = (a_par, a_anti, b, en_w0, en_w1, en_w2, d_0 ...) set to value"""
     import copy
     d2 = copy.copy(d)
     if p == 0:
@@ -563,15 +563,25 @@ def _with_param(d, p, value):
         d2.jastrow_a_anti = value
     elif p == 2:
         d2.jastrow_b = value
+    elif p == 3:
+        d2.jastrow_en_w0 = value
+    elif p == 4:
+        d2.jastrow_en_w1 = value
+    elif p == 5:
+        d2.jastrow_en_w2 = value
     else:
         ci = np.array(d.ci_coeff, np.float64, copy=True)
-        ci[p - 3] = value
+        ci[p - NJ] = value
         d2.ci_coeff = ci
     return d2
 
 
+NJ = 6  # Jastrow parameters ahead of the CI coefficients
+
+
 def _param(d, p):
-    return [d.jastrow_a_par, d.jastrow_a_anti, d.jastrow_b][p] if p < 3 else float(d.ci_coeff[p - 3])
+    jp = [d.jastrow_a_par, d.jastrow_a_anti, d.jastrow_b, d.jastrow_en_w0, d.jastrow_en_w1, d.jastrow_en_w2]
+    return jp[p] if p < NJ else float(d.ci_coeff[p - NJ])
 
 
 @pytest.mark.parametrize("name,M", [("H2", 12), ("LiH", 10), ("Li2", 8), ("CO", 5)])
@@ -579,9 +589,10 @@ def test_log_derivatives_vs_central_differences_of_log_psi(name, M):
     # the oracle's O_p against central differences of its own log|Psi| in EVERY parameter
     # (Richardson h, h/2): pins sign, pair bookkeeping (which a), the b derivative and D_n / Sigma
     d, r = wl.CONFIGS[name](M=M)
+    d = _with_en(d, 0.35, -0.04, 0.9)  # all six Jastrow parameters active
     O = ob.log_derivatives(ob.OracleSystem(d), r)
-    assert O.shape == (M, 3 + len(d.ci_coeff))
-    params = list(range(3)) + list(range(3, O.shape[1], max(1, (O.shape[1] - 3) // 7)))
+    assert O.shape == (M, NJ + len(d.ci_coeff))
+    params = list(range(NJ)) + list(range(NJ, O.shape[1], max(1, (O.shape[1] - NJ) // 7)))
     for p in params:
         t0 = _param(d, p)
 
@@ -590,7 +601,7 @@ def test_log_derivatives_vs_central_differences_of_log_psi(name, M):
             lp_m = ob.local_energy(ob.OracleSystem(_with_param(d, p, t0 - h)), r)[0]
             return (lp_p - lp_m) / (2 * h)
 
-        h = 1e-3 * max(1.0, abs(t0)) if p < 3 else 1e-3 * max(abs(t0), 1e-2)
+        h = 1e-3 * max(1.0, abs(t0)) if p < NJ else 1e-3 * max(abs(t0), 1e-2)
         fd = (4 * cd(h / 2) - cd(h)) / 3
         assert np.max(np.abs(O[:, p] - fd) / np.maximum(1, np.abs(fd))) < 1e-7, (name, p)
 
@@ -599,7 +610,7 @@ def test_log_derivatives_sum_rule_and_helium_closed_form():
     # sum_n d_n O_n = 1 (Sigma is linear in d)
     d, r = wl.li2(M=20)
     O = ob.log_derivatives(ob.OracleSystem(d), r)
-    assert np.max(np.abs(O[:, 3:] @ np.asarray(d.ci_coeff) - 1.0)) < 1e-11
+    assert np.max(np.abs(O[:, NJ:] @ np.asarray(d.ci_coeff) - 1.0)) < 1e-11
     # He-like 1s^2 + Pade: O_a_anti = r12/(1+b r12), O_b = -a r12^2/(1+b r12)^2, O_a_par = 0, O_d0 = 1/d0
     a, b = 0.37, 0.6
     d = atom_system(2.0, [(1, 0, 0, 1.6875)], [[1.0]], 1, 1, a_par=0.25, a_anti=a, b=b, ci=[0.8])
@@ -609,7 +620,11 @@ def test_log_derivatives_sum_rule_and_helium_closed_form():
     assert np.max(np.abs(O[:, 0])) == 0.0
     assert np.max(np.abs(O[:, 1] - r12 / (1 + b * r12))) < 1e-14
     assert np.max(np.abs(O[:, 2] + a * r12 ** 2 / (1 + b * r12) ** 2)) < 1e-14
-    assert np.max(np.abs(O[:, 3] - 1 / 0.8)) < 1e-13
+    assert np.max(np.abs(O[:, NJ] - 1 / 0.8)) < 1e-13
+    # e-n kernel switched off (w = 0): dK/dw0 = r, dK/dw1 = r^2, dK/dw2 = 0 summed over both electrons
+    n1, n2 = np.linalg.norm(rr[:, 0], axis=1), np.linalg.norm(rr[:, 1], axis=1)
+    assert np.max(np.abs(O[:, 3] - (n1 + n2))) < 1e-13 and np.max(np.abs(O[:, 4] - (n1 ** 2 + n2 ** 2))) < 1e-13
+    assert np.max(np.abs(O[:, 5])) == 0.0
     # three same-spin electrons: only a_par pairs contribute
     aos, C, e = hydrogenic_set(1.0)
     d = atom_system(1.0, aos, C[:, [0, 2, 4]], 3, 0, norm=np.ones(len(aos)), a_par=0.25, a_anti=0.5, b=0.9)
