@@ -160,7 +160,8 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
   // ---- electron-nucleus Jastrow kernel (D.2): K = N / D, N = w0 r + w1 r^2, D = 1 + w2 r,
   //   K' = (N' - w2 K) / D,  K'' = (N'' - 2 w2 K') / D;  grad_i J += K' d / r,  lap_i J += K'' + 2 K'/r.
   // It has to precede the AO stage, whose combined operator uses the complete grad J.
-  if (P.has_en) {
+  double dEn0 = 0.0, dEn1 = 0.0, dEn2 = 0.0;  // DERIV: this lane's share of dJ/dw0, dJ/dw1, dJ/dw2 (D.2)
+  if (P.has_en || DERIV) {  // the parameter derivatives are defined (and wanted) at w = 0 too
     for (int at = 0; at < P.n_atoms; ++at) {
       const double dx = x - P.atom[at][0], dy = y - P.atom[at][1], dz = z - P.atom[at][2];
       const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
@@ -169,6 +170,12 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       const double di = rcp_fast(fma(P.en_w2, r, 1.0));
       const double K = r * fma(P.en_w1, r, P.en_w0) * di;
       Jp += K;
+      if (DERIV) {  // dK/dw0 = r / D, dK/dw1 = r^2 / D, dK/dw2 = -N r / D^2 = -K r / D
+        const double rd = r * di;
+        dEn0 += rd;
+        dEn1 = fma(r, rd, dEn1);
+        dEn2 = fma(-K, rd, dEn2);
+      }
       if (EL) {
         const double K1 = (fma(2.0 * P.en_w1, r, P.en_w0) - P.en_w2 * K) * di;
         const double K2 = 2.0 * fma(-P.en_w2, K1, P.en_w1) * di;
@@ -675,16 +682,31 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       // (D_n / D_0 over Sigma / D_0), a second, values-only pass over the determinant classes.
       const int64_t wo = dv.w0 + wg;
       if (wvalid && wo < dv.M && dv.O) {
-        const int np = 3 + P.n_det_all;
+        const int np = kJastrowParams + P.n_det_all;
         double *row = dv.O + wo * np;
         for (int k = sub; k < 3; k += LW) {
           double t = 0.0;
           for (int j = 0; j < ne; ++j) t += sXYZ[(wg * ne + j) * 3 + k];
           row[k] = t;
         }
+      }
+      // second round through the same scratch: the electron-nucleus parameters
+      __syncwarp();
+      sXYZ[lane * 3 + 0] = dEn0;
+      sXYZ[lane * 3 + 1] = dEn1;
+      sXYZ[lane * 3 + 2] = dEn2;
+      __syncwarp();
+      if (wvalid && wo < dv.M && dv.O) {
+        const int np = kJastrowParams + P.n_det_all;
+        double *row = dv.O + wo * np;
+        for (int k = sub; k < 3; k += LW) {
+          double t = 0.0;
+          for (int j = 0; j < ne; ++j) t += sXYZ[(wg * ne + j) * 3 + k];
+          row[3 + k] = t;
+        }
         const double iden = 1.0 / den;
         const int *orig = P.det_orig;
-        double *rowd = row + 3;
+        double *rowd = row + kJastrowParams;
         for (int n = sub; n < P.n_ref; n += LW) rowd[orig[n]] = iden;
         orig += P.n_ref;
         const char *Tb = reinterpret_cast<const char *>(Tu);

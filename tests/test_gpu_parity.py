@@ -361,7 +361,7 @@ def check_log_derivatives(env, d, r, threads=8):
     err = np.abs(On - O0) / np.maximum(1.0, np.abs(O0))
     assert np.max(err[keep]) < 1e-8, (np.max(err[keep]), np.unravel_index(np.argmax(err * keep[:, None]), err.shape))
     # sum rule on the GPU result itself
-    assert np.max(np.abs(On[keep, 3:] @ np.asarray(d.ci_coeff) - 1.0)) < 1e-9
+    assert np.max(np.abs(On[keep, 6:] @ np.asarray(d.ci_coeff) - 1.0)) < 1e-9
     # estimator: the oracle's reduction applied to the oracle's E_L and O
     ev0, g0 = ob.energy_gradient(el0, O0)
     scale = 2.0 * np.mean(np.abs(O0) * np.abs(el0 - ev0)[:, None], axis=0)
