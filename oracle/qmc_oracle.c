@@ -155,6 +155,7 @@ double oracle_det_inv(int n, const double *A, double *inv) {
 /* ------------------------------------------------------------------ */
 
 static int spin_of(const oracle_system_desc_t *s, int i) { return i < s->n_up ? 0 : 1; }
+static void jastrow_een_add(const oracle_system_desc_t *s, const double *r, double *J, double *gJ, double *lapJ);
 
 /* J, grad_i J [n_e][3], lap J (sum over all electrons), pair loop. r is AoS [n_e][3]. */
 static void jastrow_all(const oracle_system_desc_t *s, const double *r, double *J, double *gJ,
@@ -200,6 +201,60 @@ static void jastrow_all(const oracle_system_desc_t *s, const double *r, double *
         *J += K;
         for (int c = 0; c < 3; ++c) gJ[3 * i + c] += K1 * d[c] / ria;
         *lapJ += K2 + 2.0 * K1 / ria;
+      }
+  if (s->n_een > 0) jastrow_een_add(s, r, J, gJ, lapJ);
+}
+
+/* electron-electron-nucleus kernel (D.3), reading Q22: ordered pairs i != j, every nucleus.
+ * One term T = c f(r_ai) g(r_aj) h(r_ij), Pade factors p(r) = a r/(1 + b r), p' = a/(1 + b r)^2,
+ * p'' = -2 a b/(1 + b r)^3.  Product rule long-hand:
+ *   grad_i T = c g [f' h e_ai + f h' e_ij]            e_ai = (r_i - R_a)/r_ai, e_ij = (r_i - r_j)/r_ij
+ *   grad_j T = c f [g' h e_aj - g h' e_ij]
+ *   lap_i T  = c g [(f'' + 2 f'/r_ai) h + f (h'' + 2 h'/r_ij) + 2 f' h' e_ai.e_ij]
+ *   lap_j T  = c f [(g'' + 2 g'/r_aj) h + g (h'' + 2 h'/r_ij) - 2 g' h' e_aj.e_ij]
+ * Adds to J, gJ, lapJ; any of gJ / lapJ may be NULL (value only). */
+static void pade3(double a, double b, double r, double *p, double *p1, double *p2) {
+  double D = 1.0 + b * r;
+  *p = a * r / D;
+  *p1 = a / (D * D);
+  *p2 = -2.0 * a * b / (D * D * D);
+}
+
+static void jastrow_een_add(const oracle_system_desc_t *s, const double *r, double *J, double *gJ, double *lapJ) {
+  int ne = s->n_up + s->n_dn;
+  for (int at = 0; at < s->n_atoms; ++at)
+    for (int i = 0; i < ne; ++i)
+      for (int j = 0; j < ne; ++j) {
+        if (i == j) continue;
+        double eai[3], eaj[3], eij[3];
+        for (int c = 0; c < 3; ++c) {
+          eai[c] = r[3 * i + c] - s->atom_xyz[3 * at + c];
+          eaj[c] = r[3 * j + c] - s->atom_xyz[3 * at + c];
+          eij[c] = r[3 * i + c] - r[3 * j + c];
+        }
+        double rai = sqrt(eai[0] * eai[0] + eai[1] * eai[1] + eai[2] * eai[2]);
+        double raj = sqrt(eaj[0] * eaj[0] + eaj[1] * eaj[1] + eaj[2] * eaj[2]);
+        double rij = sqrt(eij[0] * eij[0] + eij[1] * eij[1] + eij[2] * eij[2]);
+        for (int c = 0; c < 3; ++c) { eai[c] /= rai; eaj[c] /= raj; eij[c] /= rij; }
+        double ai_ij = eai[0] * eij[0] + eai[1] * eij[1] + eai[2] * eij[2];
+        double aj_ij = eaj[0] * eij[0] + eaj[1] * eij[1] + eaj[2] * eij[2];
+        for (int mu = 0; mu < s->n_een; ++mu) {
+          const double *q = s->een_params + 7 * mu;
+          double f, f1, f2, g, g1, g2, h, h1, h2;
+          pade3(q[1], q[2], rai, &f, &f1, &f2);
+          pade3(q[3], q[4], raj, &g, &g1, &g2);
+          pade3(q[5], q[6], rij, &h, &h1, &h2);
+          *J += q[0] * f * g * h;
+          if (gJ)
+            for (int c = 0; c < 3; ++c) {
+              gJ[3 * i + c] += q[0] * g * (f1 * h * eai[c] + f * h1 * eij[c]);
+              gJ[3 * j + c] += q[0] * f * (g1 * h * eaj[c] - g * h1 * eij[c]);
+            }
+          if (lapJ) {
+            *lapJ += q[0] * g * ((f2 + 2.0 * f1 / rai) * h + f * (h2 + 2.0 * h1 / rij) + 2.0 * f1 * h1 * ai_ij);
+            *lapJ += q[0] * f * ((g2 + 2.0 * g1 / raj) * h + g * (h2 + 2.0 * h1 / rij) - 2.0 * g1 * h1 * aj_ij);
+          }
+        }
       }
 }
 
@@ -449,6 +504,7 @@ static void logpsi_one(const oracle_system_desc_t *s, const double *r, double *w
       J += a * rij / (1.0 + s->jastrow_b * rij);
     }
   J += jastrow_en_value(s, r);
+  if (s->n_een > 0) jastrow_een_add(s, r, &J, NULL, NULL);
   double sigma = 0.0;
   for (int n = 0; n < s->n_det; ++n) {
     double D[2];

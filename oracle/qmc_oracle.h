@@ -46,6 +46,11 @@ typedef struct {
   double jastrow_a_par, jastrow_a_anti, jastrow_b;
   /* electron-nucleus kernel (D.2): K_en(r) = (w0 r + w1 r^2) / (1 + w2 r), all zero = absent */
   double jastrow_en_w0, jastrow_en_w1, jastrow_en_w2;
+  /* electron-electron-nucleus kernel (D.3): n_een terms, each 7 doubles
+   * (c, a1, b1, a2, b2, a3, b3):  K_een = sum_mu c [a1 r_ai/(1+b1 r_ai)] [a2 r_aj/(1+b2 r_aj)] [a3 r_ij/(1+b3 r_ij)],
+   * summed over every nucleus a and every ORDERED electron pair i != j (reading Q22); n_een = 0 = absent */
+  int32_t n_een;
+  const double *een_params; /* [n_een][7] or NULL */
 } oracle_system_desc_t;
 
 /* All pointers are HOST pointers.  Walker arrays are SoA [n_e][3][M]; the

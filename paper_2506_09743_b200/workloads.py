@@ -50,6 +50,7 @@ class SystemDesc:
     jastrow_en_w0: float = 0.0  # electron-nucleus kernel (D.2), all zero = absent
     jastrow_en_w1: float = 0.0
     jastrow_en_w2: float = 0.0
+    jastrow_een: np.ndarray | None = None  # electron-electron-nucleus kernel (D.3): [n_terms, 7] = (c, a1, b1, a2, b2, a3, b3)
     extra: dict = field(default_factory=dict)
 
     @property
