@@ -86,6 +86,13 @@ typedef struct {
    * (electron, nucleus) pair with one parameter set: K_en(r) = (w0 r + w1 r^2) / (1 + w2 r).
    * w0 = w1 = 0 switches the term off. */
   double jastrow_en_w0, jastrow_en_w1, jastrow_en_w2;
+  /* Electron-electron-nucleus Jastrow kernel (D.3): n_een terms (at most 6; the paper uses 5),
+   * een_params host [n_een][7] = (c, a1, b1, a2, b2, a3, b3) per term:
+   *   K_een = sum_mu c [a1 r_ai / (1 + b1 r_ai)] [a2 r_aj / (1 + b2 r_aj)] [a3 r_ij / (1 + b3 r_ij)],
+   * summed over every nucleus a and every ORDERED electron pair i != j (the paper does not say; only the
+   * ordered sum is symmetric under electron exchange when the first two factors differ).  n_een = 0: absent. */
+  int32_t n_een;
+  const double *een_params;
 } qmc_system_desc_t;
 
 /* Validate `desc`, preprocess it (shell grouping, excitation tables relative to

@@ -37,6 +37,7 @@ struct Variant {
   int NS, NMO, LP, ws_doubles;
   bool exact;  // compiled for n_up = n_dn = NS
   const void *k_el, *k_psi, *k_metro, *k_expl, *k_el_deriv;
+  const void *e_el, *e_psi, *e_metro, *e_expl, *e_el_deriv;  // the same with the e-e-n Jastrow kernel D.3 (EEN)
 };
 
 template <int NS, int NMO, bool X>
@@ -52,6 +53,11 @@ Variant make_variant() {
   v.k_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi>;
   v.k_expl = (const void *)explicit_energy_kernel<NS, NMO, X, kWarpsEl>;
   v.k_el_deriv = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true>;
+  v.e_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, false, true>;
+  v.e_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi, false, true>;
+  v.e_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi, true>;
+  v.e_expl = (const void *)explicit_energy_kernel<NS, NMO, X, kWarpsEl, true>;
+  v.e_el_deriv = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true, true>;
   return v;
 }
 
@@ -186,6 +192,17 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   P.en_w1 = d->jastrow_en_w1;
   P.en_w2 = d->jastrow_en_w2;
   P.has_en = (d->jastrow_en_w0 != 0.0 || d->jastrow_en_w1 != 0.0) ? 1 : 0;
+  if (d->n_een < 0 || (d->n_een > 0 && !d->een_params)) {
+    delete s;
+    return QMC_EINVAL;
+  }
+  if (d->n_een > kMaxEen) {
+    delete s;
+    return QMC_EUNSUPPORTED;
+  }
+  P.n_een = d->n_een;
+  for (int mu = 0; mu < d->n_een; ++mu)
+    for (int t = 0; t < 7; ++t) P.een[mu][t] = d->een_params[7 * mu + t];
   for (int a = 0; a < d->n_atoms; ++a) {
     for (int c = 0; c < 3; ++c) P.atom[a][c] = d->atom_xyz[3 * a + c];
     P.atom[a][3] = d->atom_Z[a];
@@ -297,6 +314,13 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     return QMC_EUNSUPPORTED;
   }
   s->var = *var;
+  if (P.n_een > 0) {  // the instantiations that carry the e-e-n Jastrow kernel
+    s->var.k_el = var->e_el;
+    s->var.k_psi = var->e_psi;
+    s->var.k_metro = var->e_metro;
+    s->var.k_expl = var->e_expl;
+    s->var.k_el_deriv = var->e_el_deriv;
+  }
   const int NMO = var->NMO;
   std::vector<DetRec> dets(n_packed);
   std::vector<GenDet> gens;
@@ -488,6 +512,10 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     s->flops_step = ne * nat * (8 + csqrt + cdiv) + ne * nsh * (2 + cexp) + ne * nao * 3 + 2 * ne * nao * nmo +
                     npair * (12 + csqrt + cdiv) + lu_st + 3 * nd + 3 * ne * 2 + npr * (10 + clog + csqrt + csincos) + clog;
     if (P.has_en) s->flops_step += ne * nat * (5 + cdiv);
+    if (P.n_een > 0) {  // D.3 per (nucleus, ordered pair, term): three Pade factors and their products
+      s->flops_el += nat * ne * (ne - 1) * P.n_een * (30 + 3 * cdiv);
+      s->flops_step += nat * ne * (ne - 1) * P.n_een * (10 + 3 * cdiv);
+    }
   }
 
   // ---- upload
@@ -528,7 +556,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     return QMC_EUNSUPPORTED;
   }
   s->n_sm = n_sm;
-  const void *ks[5] = {var->k_el, var->k_psi, var->k_metro, var->k_expl, var->k_el_deriv};
+  const void *ks[5] = {s->var.k_el, s->var.k_psi, s->var.k_metro, s->var.k_expl, s->var.k_el_deriv};
   int *nb[5] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro, &s->blocks_expl, &s->blocks_deriv};
   const int kw[5] = {kWarpsEl, kWarpsPsi, kWarpsPsi, kWarpsEl, kWarpsEl};
   const int ksm[5] = {s->smem_el, s->smem_psi, s->smem_psi, s->smem_el, s->smem_el};

@@ -15,6 +15,7 @@ namespace qmc {
 constexpr int kMaxAtoms = 16;
 constexpr int kMaxSpin = 8;   // electrons per spin
 constexpr int kMaxVirt = 8;   // distinct virtual orbitals per spin
+constexpr int kMaxEen = 6;    // terms of the electron-electron-nucleus Jastrow kernel (D.3; the paper uses 5)
 // tuning knobs (defaults are the measured best on B200)
 #ifndef QMC_WARPS
 #define QMC_WARPS 8          // warps per block
@@ -110,6 +111,8 @@ struct SysParams {  // passed by value to every kernel
   double a_par, a_anti, b, vnn;
   double en_w0, en_w1, en_w2;      // electron-nucleus Jastrow kernel (D.2); has_en = 0 when w0 = w1 = 0
   int has_en;
+  int n_een;                       // electron-electron-nucleus kernel (D.3): terms (c, a1, b1, a2, b2, a3, b3)
+  double een[kMaxEen][7];
   double atom[kMaxAtoms][4];       // x, y, z, Z
   int8_t ref_col[2][kMaxSpin];     // kernel MO column of reference position j, per spin
   int8_t virt_col[2][kMaxVirt];    // kernel MO column of virtual q, per spin

@@ -79,12 +79,104 @@ __device__ __noinline__ void excite_general(const GenSpin *g, const double *T, i
 }
 
 // ---------------------------------------------------------------------------------
+// Electron-electron-nucleus Jastrow kernel (D.3; reading Q22): for the lane's electron i
+//   J_een = sum_a sum_{j != i} sum_mu c f(r_ai) g(r_aj) h(r_ij)   (ordered pairs), Pade factors p(r) = a r/(1 + b r).
+// The lane keeps only its own electron's share: of the two ordered pairs (i,j) and (j,i)
+//   u  = c (g_j f_i + f_j g_i),  v' = c (g_j f'_i + f_j g'_i),  vL = c (g_j (f''_i + 2f'_i/r_ai) + f_j (g''_i + 2g'_i/r_ai))
+//   J share 1/2 u h;  grad_i += v' h e_ai + u h' e_ij;  lap_i += vL h + u (h'' + 2h'/r_ij) + 2 v' h' e_ai.e_ij.
+// Out of line (rare option, keeps the hot kernels small).  out = {J share, grad x, y, z, lap}.
+// ---------------------------------------------------------------------------------
+template <bool EL>
+__device__ __noinline__ void een_terms(const SysParams &P, const double *sXYZ, int base, int ne, int e, double x, double y,
+                                       double z, double *out) {
+  double Jp = 0.0, gx = 0.0, gy = 0.0, gz = 0.0, lap = 0.0;
+  const int n = P.n_een;
+  for (int at = 0; at < P.n_atoms; ++at) {
+    const double ax = P.atom[at][0], ay = P.atom[at][1], az = P.atom[at][2];
+    const double aix = x - ax, aiy = y - ay, aiz = z - az;
+    const double rai2 = fma(aix, aix, fma(aiy, aiy, aiz * aiz));
+    const double irai = rsqrt_fast(rai2), rai = rai2 * irai;
+    // this electron's factors for every term: value, first derivative, p'' + 2 p'/r
+    double fi[kMaxEen], f1[kMaxEen], fL[kMaxEen], gi[kMaxEen], g1[kMaxEen], gL[kMaxEen];
+#pragma unroll
+    for (int mu = 0; mu < kMaxEen; ++mu) {
+      if (mu < n) {
+        const double *q = P.een[mu];
+        const double d1 = rcp_fast(fma(q[2], rai, 1.0)), d2 = rcp_fast(fma(q[4], rai, 1.0));
+        fi[mu] = q[1] * rai * d1;
+        gi[mu] = q[3] * rai * d2;
+        if (EL) {
+          f1[mu] = q[1] * d1 * d1;
+          g1[mu] = q[3] * d2 * d2;
+          fL[mu] = 2.0 * f1[mu] * (irai - q[2] * d1);   // -2 a b D^-3 + 2 a D^-2 / r
+          gL[mu] = 2.0 * g1[mu] * (irai - q[4] * d2);
+        }
+      }
+    }
+    double ga = 0.0;  // coefficient of e_ai in grad_i, summed over partners and terms
+    for (int o = 1; o < ne; ++o) {
+      int j = e + o;
+      j -= (j >= ne) ? ne : 0;
+      const double xj = sXYZ[base + j], yj = sXYZ[32 + base + j], zj = sXYZ[64 + base + j];
+      const double ijx = x - xj, ijy = y - yj, ijz = z - zj;
+      const double rij2 = fma(ijx, ijx, fma(ijy, ijy, ijz * ijz));
+      const double irij = rsqrt_fast(rij2), rij = rij2 * irij;
+      const double ajx = xj - ax, ajy = yj - ay, ajz = zj - az;
+      const double raj2 = fma(ajx, ajx, fma(ajy, ajy, ajz * ajz));
+      const double raj = raj2 * rsqrt_fast(raj2);
+      const double cosA = fma(aix, ijx, fma(aiy, ijy, aiz * ijz)) * irai * irij;  // e_ai . e_ij
+      double gij = 0.0;  // coefficient of e_ij in grad_i
+#pragma unroll
+      for (int mu = 0; mu < kMaxEen; ++mu) {
+        if (mu < n) {
+          const double *q = P.een[mu];
+          const double fj = q[1] * raj * rcp_fast(fma(q[2], raj, 1.0));
+          const double gj = q[3] * raj * rcp_fast(fma(q[4], raj, 1.0));
+          const double dh = rcp_fast(fma(q[6], rij, 1.0));
+          const double h = q[5] * rij * dh;
+          const double u = q[0] * fma(gj, fi[mu], fj * gi[mu]);
+          Jp = fma(0.5 * u, h, Jp);
+          if (EL) {
+            const double h1 = q[5] * dh * dh;
+            const double hL = 2.0 * h1 * (irij - q[6] * dh);
+            const double v1 = q[0] * fma(gj, f1[mu], fj * g1[mu]);
+            const double vL = q[0] * fma(gj, fL[mu], fj * gL[mu]);
+            ga = fma(v1, h, ga);
+            gij = fma(u, h1, gij);
+            lap += fma(vL, h, fma(u, hL, 2.0 * v1 * h1 * cosA));
+          }
+        }
+      }
+      if (EL) {
+        const double sc = gij * irij;
+        gx = fma(sc, ijx, gx);
+        gy = fma(sc, ijy, gy);
+        gz = fma(sc, ijz, gz);
+      }
+    }
+    if (EL) {
+      const double sc = ga * irai;
+      gx = fma(sc, aix, gx);
+      gy = fma(sc, aiy, gy);
+      gz = fma(sc, aiz, gz);
+    }
+  }
+  out[0] = Jp;
+  out[1] = gx;
+  out[2] = gy;
+  out[3] = gz;
+  out[4] = lap;
+}
+
+// ---------------------------------------------------------------------------------
 // Evaluate the G walkers of this warp.  Lane = g * n_e + e holds electron e of walker g
 // at (x, y, z).  Results for walker g are left in ws[oRes + 4 g + {0,1,2}] =
 // {log|Psi|, sign, E_L} (E_L only if EL).  All 32 lanes must call.
 // ---------------------------------------------------------------------------------
 // DERIV: also write the logarithmic parameter derivatives of eq. 6 for the G walkers to dv.O.
-template <int NS, int NMO, bool EL, bool X, bool EXPL = false, bool DERIV = false>
+// EEN: the wavefunction carries the electron-electron-nucleus kernel D.3 (separate instantiations, so that the
+// kernels of the common case stay free of the call and its register spills: measured 459 -> 508 us otherwise).
+template <int NS, int NMO, bool EL, bool X, bool EXPL = false, bool DERIV = false, bool EEN = false>
 __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp,
                              const double *__restrict__ sC, const DetRec *__restrict__ sDet,
                              double *__restrict__ ws, double x, double y, double z, int lane,
@@ -185,6 +277,18 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
         gJz = fma(sc, dz, gJz);
         lapJ += fma(2.0, sc, K2);
       }
+    }
+  }
+
+  if (EEN) {  // electron-electron-nucleus kernel (D.3); sXYZ still holds the coordinates
+    double t[5];
+    een_terms<EL>(P, sXYZ, (active ? g : 0) * ne, ne, e, x, y, z, t);
+    Jp += t[0];
+    if (EL) {
+      gJx += t[1];
+      gJy += t[2];
+      gJz += t[3];
+      lapJ += t[4];
     }
   }
 

@@ -35,7 +35,7 @@ __device__ __forceinline__ void dummy_xyz(int lane, double &x, double &y, double
   z = 0.53 - 0.05 * lane;
 }
 
-template <int NS, int NMO, bool EL, bool X, int WPB, bool DERIV = false>
+template <int NS, int NMO, bool EL, bool X, int WPB, bool DERIV = false, bool EEN = false>
 __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     local_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -64,7 +64,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   for (int64_t grp = (int64_t)blockIdx.x * WPB + warp; grp < n_groups; grp += stride) {
     double x, y, z;
     fetch(grp, x, y, z);
-    eval_walkers<NS, NMO, EL, X, false, DERIV>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1, DerivOut{io.O, grp * G, io.M});
+    eval_walkers<NS, NMO, EL, X, false, DERIV, EEN>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1, DerivOut{io.O, grp * G, io.M});
     bool flagged = false;
     if (lane < G) {
       const int64_t wo = grp * G + lane;
@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
 // the whole grid, every warp rebuilds the MO rows of its group, eliminates its determinants and stores
 // its partial sums; the warp that finishes a group last adds the partials in slice order (deterministic)
 // and writes the outputs.
-template <int NS, int NMO, bool X, int WPB>
+template <int NS, int NMO, bool X, int WPB, bool EEN = false>
 __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     explicit_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     } else {
       dummy_xyz(lane, x, y, z);
     }
-    eval_walkers<NS, NMO, true, X, true>(P, sExp, sC, sDet, ws, x, y, z, lane, slice, SL);
+    eval_walkers<NS, NMO, true, X, true, false, EEN>(P, sExp, sC, sDet, ws, x, y, z, lane, slice, SL);
     const double *res = ws + GE::oRes + (lane < G ? lane : 0) * 4;  // {Sigma, Sum d D t, J, energy share}
     if (lane < G) {
       io.fb_part[(item * G + lane) * 2 + 0] = res[0];   // eq. 4
@@ -171,7 +171,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
 // Persistent all-electron Metropolis (readings Q9, Q10).
 // Walker coordinates and log|Psi| stay in registers for all sweeps.
 // ---------------------------------------------------------------------------------
-template <int NS, int NMO, bool X, int WPB>
+template <int NS, int NMO, bool X, int WPB, bool EEN = false>
 __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     metropolis_kernel(const __grid_constant__ SysParams P, const WalkerIO io, const MetroParams mp) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -241,7 +241,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
         logu = sLogU[own ? g : 0];
         __syncwarp();
       }
-      eval_walkers<NS, NMO, false, X>(P, sExp, sC, sDet, ws, xp, yp, zp, lane);
+      eval_walkers<NS, NMO, false, X, false, false, EEN>(P, sExp, sC, sDet, ws, xp, yp, zp, lane);
       const double lp2 = sRes[rg + 0], sg2 = sRes[rg + 1];
       // accept iff log u < 2 (log|Psi'| - log|Psi|): false for NaN and for Psi' = 0
       const bool ok = (sw < 0) || (own && (logu < 2.0 * (lp2 - lp)));
