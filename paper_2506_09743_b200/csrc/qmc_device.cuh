@@ -92,6 +92,9 @@ struct DetCols {
 // reference determinant is nearly singular while the expansion is not.  Measured:
 // E_L error ~ 1.2e-15 (Sigma/D_0)^2, so K = 8e5 keeps it below 1e-9 max(1, |E_L|), a tenth of the parity bound.
 constexpr double kFallbackK = 8.0e5;
+// ... and in any case when |Sigma / D_0| > 1e4: log|Psi| of the table path is off by ~1e-15 |Sigma/D_0| (1e-12 at
+// 1024), and its parity bound 1e-10 is ABSOLUTE, so walkers with a huge |E_L| must not escape through the first test.
+constexpr double kFallbackCap = 1.0e8;
 
 struct SysParams {  // passed by value to every kernel
   int n_atoms, n_up, n_dn, n_e;

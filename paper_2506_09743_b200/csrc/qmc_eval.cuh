@@ -776,9 +776,10 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       sRes[wg * 4 + 1] = sgn * ((den > 0.0) ? 1.0 : ((den < 0.0) ? -1.0 : 0.0));
       const double eloc = EL ? esum + (sProb[pu * 4 + 2] + sProb[pd * 4 + 2]) + num / den + P.vnn : 0.0;
       if (EL) sRes[wg * 4 + 2] = eloc;
-      // explicit fallback when the estimated table-path error 1.2e-15 (Sigma/D_0)^2 exceeds a tenth of the
-      // parity bound 1e-8 max(1, |E_L|); also set for NaN (singular reference)
-      sRes[wg * 4 + 3] = (den * den <= kFallbackK * fmax(1.0, fabs(eloc))) ? 0.0 : 1.0;
+      // explicit fallback when the estimated table-path error of E_L, 1.2e-15 (Sigma/D_0)^2, exceeds a tenth of the
+      // parity bound 1e-8 max(1, |E_L|), or that of log|Psi|, ~1e-15 |Sigma/D_0|, a tenth of its absolute bound
+      // 1e-10 (kFallbackCap); also set for NaN (singular reference)
+      sRes[wg * 4 + 3] = (den * den <= fmin(kFallbackK * fmax(1.0, fabs(eloc)), kFallbackCap)) ? 0.0 : 1.0;
     }
     if (DERIV) {
       // ---- eq. 6 factors O_p = (dPsi/dtheta_p)/Psi, theta = (a_par, a_anti, b, d_0 ...):
