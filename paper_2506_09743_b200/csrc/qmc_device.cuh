@@ -242,6 +242,18 @@ struct Geo {
   __host__ __device__ static constexpr int mergeShift(int fr) { return (fr & 4) << 3; }  // rows 4..7: + 32
   static constexpr int total = cmax(layout_total, kChunk * S2);
   static constexpr int NT = (NMO + 7) / 8;                    // 8-column MO tiles
+  // bounds of the overlays (compile-time hygiene: no memory checker runs on this pool)
+  static_assert(NS >= 1 && NS <= kMaxSpin && NMO <= 16, "instantiation outside the register-array limits");
+  static_assert(ROWS <= 32 && 2 * GMAX * NS >= ROWS, "electron rows of a pass exceed the warp");
+  static_assert(opCol(31) < S2 && 31 < S1, "tile columns exceed the row stride");
+  static_assert(tileCol(true, mTiles(true) - 1) + 7 < S2 && (!MERGE || tileCol(true, VT) + 7 + mergeShift(7) < S2),
+                "operator tiles exceed the row stride");
+  static_assert(kChunk * S2 <= total && layout_total <= total, "scratch smaller than its overlays");
+  static_assert(oB + szPhi <= oPart, "MO rows overlap the per-electron scalars");
+  static_assert(SINGLE ? (oM + szM <= oPart) : true, "tables overlap the per-electron scalars");
+  static_assert(2 * GMAX * TS * 2 <= szT + szM, "interleaved {T, M} tables exceed their region");
+  static_assert(NS * RS + 1 < 256 && 8 * (2 * TS) < 65536, "table indices exceed the packed determinant records");
+  static_assert(oProp + 96 + GMAX <= oPart, "Metropolis draws exceed the table region");
 };
 
 // ---------------------------------------------------------------------------------
