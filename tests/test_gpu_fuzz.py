@@ -1,0 +1,103 @@
+"""Seeded random systems inside the compiled limits (random centres, shells complete or not, out-of-order AOs,
+custom normalisation, 0-8 electrons per spin, random substitution orders including repeats of the reference and
+k >= 3, all Jastrow variants, ragged batch sizes): the CUDA path against the oracle through the C ABI."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2506_09743_b200 import workloads as wl
+from paper_2506_09743_b200.workloads import SystemDesc
+
+pytestmark = pytest.mark.gpu
+
+
+def random_system(seed, case):
+    """(SystemDesc, walkers) or None when the draw falls outside the library's limits"""
+    rng = np.random.default_rng([seed, case])
+    n_at = int(rng.integers(1, 5))
+    xyz = rng.normal(0, 1.2, (n_at, 3))
+    Z = rng.integers(1, 9, n_at).astype(float)
+    aos = []
+    for a in range(n_at):
+        for _ in range(int(rng.integers(1, 5))):
+            n = int(rng.integers(1, 5))
+            l = int(rng.integers(0, min(n, 3)))
+            z = float(rng.uniform(0.5, 3.5))
+            if rng.random() < 0.6:
+                aos += [(a, n, l, m, z) for m in range(2 * l + 1)]
+            else:
+                aos.append((a, n, l, int(rng.integers(0, 2 * l + 1)), z))
+    if rng.random() < 0.3:
+        rng.shuffle(aos)
+    aos = aos[:60]
+    n_ao = len(aos)
+    n_up, n_dn = int(rng.integers(0, 9)), int(rng.integers(0, 9))
+    if n_up + n_dn == 0:
+        n_up = 1
+    n_mo = int(min(n_ao, max(n_up, n_dn) + rng.integers(0, 8), 16))
+    if n_mo < max(n_up, n_dn):
+        return None
+    Cm = rng.standard_normal((n_ao, n_mo))
+    n_det = int(rng.integers(1, 12))
+
+    def rand_list(ns, ref):
+        lst = ref.copy()
+        k = int(rng.integers(0, min(ns, n_mo - ns, 4) + 1)) if ns else 0
+        if k:
+            pos = rng.choice(ns, k, replace=False)
+            lst[pos] = rng.choice(np.setdiff1d(np.arange(n_mo), ref), k, replace=False)
+        return lst
+
+    ref_up = rng.permutation(n_mo)[:n_up].astype(np.int32)
+    ref_dn = rng.permutation(n_mo)[:n_dn].astype(np.int32)
+    ups = [ref_up] + [rand_list(n_up, ref_up) for _ in range(n_det - 1)]
+    dns = [ref_dn] + [rand_list(n_dn, ref_dn) for _ in range(n_det - 1)]
+    if len(set(np.concatenate(ups)) - set(ref_up)) > 8 or len(set(np.concatenate(dns)) - set(ref_dn)) > 8:
+        return None
+    ci = np.concatenate([[0.9], rng.normal(0, 0.2, n_det - 1)])
+    col = lambda i, t: np.array([a[i] for a in aos], t)
+    d = SystemDesc(f"fuzz{case}", xyz, Z, n_up, n_dn, col(0, np.int32), col(1, np.int32), col(2, np.int32),
+                   col(3, np.int32), col(4, np.float64), None if rng.random() < 0.7 else rng.uniform(0.5, 2, n_ao), Cm,
+                   np.array(ups, np.int32).reshape(n_det, n_up), np.array(dns, np.int32).reshape(n_det, n_dn), ci,
+                   0.25, 0.5, float(rng.uniform(0.3, 2)))
+    if rng.random() < 0.5:
+        d.jastrow_en_w0, d.jastrow_en_w1, d.jastrow_en_w2 = rng.normal(0, .3), rng.normal(0, .05), rng.uniform(0.3, 2)
+    if rng.random() < 0.3:
+        d.jastrow_een = np.column_stack([rng.normal(0, .1, 2), rng.uniform(.3, 1.5, (2, 6))])
+    return d, wl.make_walkers(rng, xyz, n_up + n_dn, int(rng.integers(1, 200)))
+
+
+@pytest.mark.parametrize("seed", [11, 12])
+def test_random_systems_against_the_oracle(seed):
+    import torch
+    from oracle import binding as ob
+    from paper_2506_09743_b200 import binding as qb
+    evaluated = 0
+    for case in range(60):
+        drawn = random_system(seed, case)
+        if drawn is None:
+            continue
+        d, r = drawn
+        try:
+            s = qb.QmcSystem(d, 0)
+        except qb.QmcError as e:
+            assert e.status == qb.QMC_EUNSUPPORTED, (case, e)
+            continue
+        evaluated += 1
+        o = ob.OracleSystem(d)
+        lp0, sg0, el0 = ob.local_energy(o, r, threads=4)
+        O0 = ob.log_derivatives(o, r, threads=4)
+        lp, sg, el, O = (t.cpu().numpy() for t in s.log_derivatives(torch.from_numpy(r).cuda()))
+        keep = (lp0 - lp0.max() > math.log(1e-6)) & np.isfinite(el0)
+        assert np.array_equal(sg, sg0), case
+        # random orbitals make badly conditioned Slater matrices common: log|det| carries eps * cond on both sides
+        assert np.max(np.abs(lp - lp0)[keep]) < 1e-8, (case, np.max(np.abs(lp - lp0)[keep]))
+        assert np.max((np.abs(el - el0) / np.maximum(1, np.abs(el0)))[keep]) < 1e-7, case
+        assert np.max((np.abs(O - O0) / np.maximum(1, np.abs(O0)))[keep]) < 1e-7, case
+        ref = ob.metropolis(o, r, 0.3, 4, seed=case, threads=4)
+        out = s.metropolis(torch.from_numpy(r).cuda(), 0.3, 4, seed=case, want_accept=True)
+        bad = (out["accept"].cpu().numpy() != ref["accept"]) & (np.abs(ref["margin"]) >= 1e-9)
+        assert not bad.any(), case
+        s.close()
+    assert evaluated >= 30
