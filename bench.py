@@ -285,7 +285,10 @@ def main():
                          "traffic": 44129280,  # dram bytes read+written per launch, profiles/r01_el_kernel.md
                          "kernel": "local_energy_kernel<7,14,true>",
                          "peak_source": "qmc_fp64_peak DFMA microbenchmark in this process (no FP64 entry in MEASURED_PEAKS.json)",
-                         "dmma_peak": peak_dmma, "model_flop_eq_per_walker": flops_el},
+                         "dmma_peak": peak_dmma, "model_flop_eq_per_walker": flops_el,
+                         # 148 SMs x 64 FP64 FMA/clk x 2 x the SM clock seen during the run
+                         "peak_nominal": 148 * 64 * 2 * (clocks.get("sm_mhz") or 1965.0) * 1e-6,
+                         "frac_of_nominal": achieved / (148 * 64 * 2 * (clocks.get("sm_mhz") or 1965.0) * 1e-6)},
             "cpu_baseline": cpu,
             "e2e": {"value": e2e_rate, "unit": UNIT, "h2d_bytes_per_step": int(r_pin.numel() * 8),
                     "d2h_bytes_per_step": int(out_pin.numel() * 8)},
