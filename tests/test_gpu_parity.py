@@ -556,3 +556,19 @@ def test_vmc_example_gradient_descent_lowers_the_h2_energy(env):
     assert min(e[1:]) < e[0] - 4 * err, (e, err)
     assert hist[1][2] < 0.5 * hist[0][2]
     assert d_opt.jastrow_en_w1 != 0.0 and -1.20 < e[-1] < -1.10   # exact H2: -1.1745 Ha; HF-like orbital + Jastrow ~ -1.15
+
+
+def test_results_are_repeatable_bit_for_bit(env):
+    # the fallback work list fills in a nondeterministic order, the results must not depend on it (slice-ordered sums)
+    torch, ob, qb = env
+    d, r = wl.li2(M=16384)   # initial Li2 walkers: a few dozen groups take the explicit fallback
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    ref = [t.clone() for t in s.local_energy(rg)]
+    for _ in range(4):
+        assert all(torch.equal(a, b) for a, b in zip(s.local_energy(rg), ref))
+    r1, r2 = rg.clone(), rg.clone()
+    a = s.metropolis(r1, 0.3, 3, seed=9, want_accept=True, want_eloc_acc=True)
+    b = s.metropolis(r2, 0.3, 3, seed=9, want_accept=True, want_eloc_acc=True)
+    assert torch.equal(r1, r2) and torch.equal(a["accept"], b["accept"]) and torch.equal(a["eloc_acc"], b["eloc_acc"])
+    s.close()
