@@ -572,3 +572,18 @@ def test_results_are_repeatable_bit_for_bit(env):
     b = s.metropolis(r2, 0.3, 3, seed=9, want_accept=True, want_eloc_acc=True)
     assert torch.equal(r1, r2) and torch.equal(a["accept"], b["accept"]) and torch.equal(a["eloc_acc"], b["eloc_acc"])
     s.close()
+
+
+def test_metropolis_zero_sweeps_only_evaluates(env):
+    torch, ob, qb = env
+    d, r = wl.li2(M=333)
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    r0 = rg.clone()
+    out = s.metropolis(rg, 0.3, 0, seed=1, want_accept=True, count=True)
+    lp, sg = s.log_psi(r0)
+    assert torch.equal(rg, r0) and torch.equal(out["logpsi"], lp) and torch.equal(out["sign"], sg)
+    assert out["n_accepted"] == 0 and tuple(out["accept"].shape) == (0, 333)
+    out = s.metropolis(rg, 0.3, 0, seed=1, want_eloc_acc=True)
+    assert float(out["eloc_acc"].abs().max()) == 0.0 and torch.equal(out["logpsi"], lp)
+    s.close()
