@@ -75,6 +75,9 @@ def lib():
             L.oracle_batch_stats.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
             L.oracle_log_derivatives.restype = C.c_int
             L.oracle_log_derivatives.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p]
+            L.oracle_orbital_derivatives.restype = C.c_int
+            L.oracle_orbital_derivatives.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p,
+                                                     C.c_void_p]
             L.oracle_energy_gradient.restype = None
             L.oracle_energy_gradient.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
             _lib = L
@@ -242,3 +245,24 @@ def energy_gradient(eloc, O):
     g = np.empty(Oc.shape[1])
     lib().oracle_energy_gradient(_p(e), _p(Oc), e.shape[0], Oc.shape[1], C.addressof(ev), _p(g))
     return ev.value, g
+
+
+def orbital_derivatives(sysd: OracleSystem, r_soa, threads: int = 1):
+    """(dC[M, n_ao, n_mo], dzeta[M, n_ao]) = d ln Psi / d C[beta][alpha], d ln Psi / d zeta_beta."""
+    r = np.ascontiguousarray(r_soa, np.float64)
+    M = r.shape[2]
+    dC = np.empty((M, sysd.n_ao, int(sysd.c.n_mo)))
+    dz = np.empty((M, sysd.n_ao))
+    L = lib()
+
+    def run(rng):
+        rc = L.oracle_orbital_derivatives(sysd.ref, _p(r), M, rng[0], rng[1], _p(dC), _p(dz))
+        assert rc == 0
+
+    rs = _ranges(M, threads)
+    if len(rs) == 1:
+        run(rs[0])
+    else:
+        with ThreadPoolExecutor(len(rs)) as ex:
+            list(ex.map(run, rs))
+    return dC, dz

@@ -693,3 +693,81 @@ void oracle_energy_gradient(const double *eloc, const double *O, int64_t M, int3
     grad[p] = 2.0 * sum / (double)M;
   }
 }
+
+/* ------------------------------------------------------------------ */
+/* Orbital-parameter derivatives of ln Psi (AO exponents, MO            */
+/* coefficients), every determinant inverted explicitly */
+/* ------------------------------------------------------------------ */
+
+int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
+                               int64_t w1, double *dC, double *dzeta) {
+  int ne = s->n_up + s->n_dn, nmo = s->n_mo, nao = s->n_ao;
+  double *aov = (double *)malloc(sizeof(double) * (size_t)(ne * nao + 1));      /* ao_beta(r_i) */
+  double *aoz = (double *)malloc(sizeof(double) * (size_t)(ne * nao + 1));      /* d ao_beta / d zeta (r_i) */
+  double *mo = (double *)malloc(sizeof(double) * (size_t)(ne * nmo + 1));
+  double *A = (double *)malloc(sizeof(double) * (size_t)(ne * ne + 1));
+  double *Ai = (double *)malloc(sizeof(double) * (size_t)(2 * ne * ne + 2));    /* both spins' inverses of one determinant */
+  double *gam = (double *)malloc(sizeof(double) * (size_t)(ne * nmo + 1));      /* Gamma[i][alpha], not yet / Sigma */
+  double *pos = (double *)malloc(sizeof(double) * (size_t)(3 * ne + 1));
+  if (!aov || !aoz || !mo || !A || !Ai || !gam || !pos) return -1;
+  double ao[5];
+  for (int64_t w = w0; w < w1; ++w) {
+    gather_walker(r, M, w, ne, pos);
+    for (int i = 0; i < ne; ++i)
+      for (int beta = 0; beta < nao; ++beta) {
+        oracle_ao_eval(s, beta, pos + 3 * i, ao);
+        aov[i * nao + beta] = ao[0];
+        /* phi = N S r^k e^{-zeta r}: d phi / d zeta = phi (d ln N / d zeta - r) */
+        int at = s->ao_atom[beta];
+        double dx = pos[3 * i] - s->atom_xyz[3 * at], dy = pos[3 * i + 1] - s->atom_xyz[3 * at + 1],
+               dz = pos[3 * i + 2] - s->atom_xyz[3 * at + 2];
+        double rr = sqrt(dx * dx + dy * dy + dz * dz);
+        double dlnN = s->ao_norm ? 0.0 : ((double)s->ao_n[beta] + 0.5) / s->ao_zeta[beta];
+        aoz[i * nao + beta] = ao[0] * (dlnN - rr);
+      }
+    for (int i = 0; i < ne * nmo; ++i) { mo[i] = 0.0; gam[i] = 0.0; }
+    for (int i = 0; i < ne; ++i)
+      for (int beta = 0; beta < nao; ++beta)
+        for (int alpha = 0; alpha < nmo; ++alpha) mo[i * nmo + alpha] += s->mo_coeff[beta * nmo + alpha] * aov[i * nao + beta];
+    double sigma = 0.0;
+    for (int n = 0; n < s->n_det; ++n) {
+      double D[2];
+      for (int sp = 0; sp < 2; ++sp) {
+        int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
+        const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
+        for (int i = 0; i < ns; ++i)
+          for (int j = 0; j < ns; ++j) A[i * ns + j] = mo[(e0 + i) * nmo + lst[j]];
+        D[sp] = oracle_det_inv(ns, A, Ai + sp * ne * ne);
+      }
+      double wn = s->ci_coeff[n] * D[0] * D[1];
+      sigma += wn;
+      for (int sp = 0; sp < 2; ++sp) {
+        int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
+        const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
+        const double *inv = Ai + sp * ne * ne;
+        /* d ln D / d A[i][j] = A^-1[j][i]; column j of A_n holds MO lst[j] */
+        for (int i = 0; i < ns; ++i)
+          for (int j = 0; j < ns; ++j) gam[(e0 + i) * nmo + lst[j]] += wn * inv[j * ns + i];
+      }
+    }
+    if (dC)
+      for (int beta = 0; beta < nao; ++beta)
+        for (int alpha = 0; alpha < nmo; ++alpha) {
+          double t = 0.0;
+          for (int i = 0; i < ne; ++i) t += aov[i * nao + beta] * gam[i * nmo + alpha];
+          dC[((size_t)w * nao + beta) * nmo + alpha] = t / sigma;
+        }
+    if (dzeta)
+      for (int beta = 0; beta < nao; ++beta) {
+        double t = 0.0;
+        for (int alpha = 0; alpha < nmo; ++alpha) {
+          double u = 0.0;
+          for (int i = 0; i < ne; ++i) u += aoz[i * nao + beta] * gam[i * nmo + alpha];
+          t += s->mo_coeff[beta * nmo + alpha] * u;
+        }
+        dzeta[(size_t)w * nao + beta] = t / sigma;
+      }
+  }
+  free(aov); free(aoz); free(mo); free(A); free(Ai); free(gam); free(pos);
+  return 0;
+}

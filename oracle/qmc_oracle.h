@@ -106,6 +106,18 @@ void oracle_batch_stats(const double *x, int64_t M, double *mean, double *stderr
 int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                            int64_t w1, double *O);
 
+/* Logarithmic derivatives with respect to the orbital parameters (eq. 6 factors for the AO and MO layers,
+ * PAPER.md:55-57): dC [M][n_ao][n_mo] = d ln Psi / d C[beta][alpha] (the derivative in the scaling mu_{beta,alpha}
+ * of PAPER.md:57 is c_{beta,alpha} times it) and dzeta [M][n_ao] = d ln Psi / d zeta_beta, each AO's exponent on
+ * its own; the standard normalisation depends on zeta, (2 zeta)^(n+1/2): d ln N / d zeta = (n + 1/2) / zeta, a
+ * caller-supplied ao_norm does not.  Every determinant is inverted explicitly:
+ *   d ln Sigma / d A_n[i][j] = A_n^-1[j][i]  =>  Gamma[i][alpha] = sum_n w_n A_n^-1[pos_n(alpha)][i],
+ *   w_n = d_n D_n^up D_n^dn / Sigma;  dC[beta][alpha] = sum_i ao_beta(r_i) Gamma[i][alpha];
+ *   dzeta[beta] = sum_alpha C[beta][alpha] sum_i (d ao_beta / d zeta)(r_i) Gamma[i][alpha].
+ * Either output may be NULL.  Rows w0 <= w < w1. */
+int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
+                               int64_t w1, double *dC, double *dzeta);
+
 /* Estimator of eq. 6: E_v = mean E_L, grad_p = (2/M) sum_m O[m][p] (E_L[m] - E_v).
  * Kahan sums.  Ev may be NULL. */
 void oracle_energy_gradient(const double *eloc, const double *O, int64_t M, int32_t n_param,

@@ -769,3 +769,66 @@ def test_een_jastrow_absent_without_terms():
     assert all(np.array_equal(x, y) for x, y in zip(a, b))
     c = ob.local_energy(ob.OracleSystem(_with_een(d)), r)
     assert np.max(np.abs(c[2] - a[2])) > 1e-3
+
+
+# ---------------------------------------------------------------- orbital parameters (AO exponents, MO coefficients)
+@pytest.mark.parametrize("name,M", [("H2", 6), ("LiH", 5), ("Li2", 3), ("CO", 2)])
+def test_orbital_derivatives_vs_central_differences_of_log_psi(name, M):
+    # d ln Psi / d zeta_beta and d ln Psi / d C[beta][alpha] against Richardson central differences of the
+    # oracle's own log|Psi| (rebuilt with one AO exponent / one MO coefficient perturbed): pins the inverse
+    # transposition, the column bookkeeping over determinants, the CI weights and d(norm)/d zeta
+    import copy
+    d, r = wl.CONFIGS[name](M=M)
+    o = ob.OracleSystem(d)
+    dC, dz = ob.orbital_derivatives(o, r)
+    rng = np.random.default_rng(3)
+    used = sorted(set(np.asarray(d.det_up).ravel()) | set(np.asarray(d.det_dn).ravel()))
+
+    def fd(make, t0, h):
+        def cd(hh):
+            lp_p = ob.local_energy(ob.OracleSystem(make(t0 + hh)), r)[0]
+            lp_m = ob.local_energy(ob.OracleSystem(make(t0 - hh)), r)[0]
+            return (lp_p - lp_m) / (2 * hh)
+        return (4 * cd(h / 2) - cd(h)) / 3
+
+    for beta in rng.choice(d.n_ao, min(4, d.n_ao), replace=False):
+        def mk(z, beta=beta):
+            d2 = copy.copy(d)
+            zz = np.array(d.ao_zeta, np.float64, copy=True)
+            zz[beta] = z
+            d2.ao_zeta = zz
+            return d2
+        ref = fd(mk, float(d.ao_zeta[beta]), 1e-3)
+        assert np.max(np.abs(dz[:, beta] - ref) / np.maximum(1, np.abs(ref))) < 1e-7, (name, "zeta", beta)
+        alpha = int(rng.choice(used))
+        def mkc(c, beta=beta, alpha=alpha):
+            d2 = copy.copy(d)
+            cc = np.array(d.mo_coeff, np.float64, copy=True)
+            cc[beta, alpha] = c
+            d2.mo_coeff = cc
+            return d2
+        ref = fd(mkc, float(d.mo_coeff[beta, alpha]), 1e-3)
+        assert np.max(np.abs(dC[:, beta, alpha] - ref) / np.maximum(1, np.abs(ref))) < 1e-7, (name, "C", beta, alpha)
+    # an MO that no determinant uses cannot matter
+    unused = [a for a in range(d.n_mo) if a not in used]
+    if unused:
+        assert np.max(np.abs(dC[:, :, unused])) == 0.0
+
+
+def test_orbital_derivatives_closed_form_and_scaling_identity():
+    # hydrogen-like 1s: ln Psi = ln N(zeta) - zeta r  =>  d/dzeta = 3/(2 zeta) - r ; d/dC = 1/C
+    zeta, c = 1.3, 0.7
+    d = atom_system(1.0, [(1, 0, 0, zeta)], [[c]], 1, 0)
+    rr = _rand_pos(40, 1, 1.5, rmin=0.05, seed=95)
+    dC, dz = ob.orbital_derivatives(ob.OracleSystem(d), soa(rr))
+    rad = np.linalg.norm(rr[:, 0], axis=1)
+    assert np.max(np.abs(dz[:, 0] - (1.5 / zeta - rad))) < 1e-13 and np.max(np.abs(dC[:, 0, 0] - 1 / c)) < 1e-13
+    # custom normalisation: no d(norm)/d zeta
+    d = atom_system(1.0, [(1, 0, 0, zeta)], [[c]], 1, 0, norm=[2.0])
+    dz = ob.orbital_derivatives(ob.OracleSystem(d), soa(rr))[1]
+    assert np.max(np.abs(dz[:, 0] + rad)) < 1e-13
+    # Euler: scaling every coefficient of the MOs by t scales each determinant by t^(n_e): sum C dlnPsi/dC = n_e
+    # (every determinant here uses n_up + n_dn columns)
+    d, r = wl.li2(M=10)
+    dC, _ = ob.orbital_derivatives(ob.OracleSystem(d), r)
+    assert np.max(np.abs(np.einsum("mba,ba->m", dC, d.mo_coeff) - d.n_e)) < 1e-10
