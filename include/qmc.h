@@ -168,7 +168,7 @@ int qmc_batch_stats(const double *d_x, int64_t M, double *h_mean, double *h_stde
 /* ---- the factors of the gradient estimator, eq. 6 ----
  * Variational parameters handled: theta = (jastrow_a_par, jastrow_a_anti, jastrow_b, jastrow_en_w0,
  * jastrow_en_w1, jastrow_en_w2, d_0 .. d_{n_det-1}) in that order, n_param = 6 + n_det (qmc_n_param).
- * MO and AO parameters (mu, zeta of PAPER.md:55-57) are not handled yet. */
+ * The MO and AO parameters (mu, zeta of PAPER.md:55-57) have their own call, qmc_orbital_derivatives. */
 int qmc_n_param(const qmc_system_t *s);
 
 /* qmc_local_energy plus the logarithmic derivatives O_p(r) = (dPsi/dtheta_p)/Psi:
@@ -180,6 +180,17 @@ int qmc_n_param(const qmc_system_t *s);
  * reference is eps * cond(A_0), not the squared amplification E_L suffers).  Asynchronous. */
 int qmc_log_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign,
                         double *d_eloc, double *d_O, void *cuda_stream);
+
+/* Logarithmic derivatives with respect to the orbital parameters:
+ *   d_dC    device, out: double [M][n_ao][n_mo]  d ln Psi / d C[beta][alpha] (MO coefficients; the derivative in
+ *           the scaling mu_{beta,alpha} of PAPER.md:57 is c_{beta,alpha} times it; zero for MOs no determinant uses)
+ *   d_dzeta device, out: double [M][n_ao]        d ln Psi / d zeta_beta, each AO's exponent on its own (with the
+ *           standard normalisation d ln N / d zeta = (n + 1/2) / zeta is included; a caller-supplied ao_norm is
+ *           taken as independent of zeta)
+ * Either may be NULL.  First version: every determinant is inverted explicitly for every walker (N_det
+ * eliminations per walker), i.e. it is correct but far slower than qmc_local_energy.  Asynchronous. */
+int qmc_orbital_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d_dC, double *d_dzeta,
+                            void *cuda_stream);
 
 /* Estimator of eq. 6: E_v = mean E_L, grad_p = (2/M) sum_m O[m][p] (E_L[m] - E_v).
  *   d_eloc device in [M]; d_O device in [M][n_param]; h_Ev host out (may be NULL);

@@ -16,7 +16,7 @@ _lib = None
 
 EXPORTS = ["qmc_setup", "qmc_destroy", "qmc_local_energy", "qmc_log_psi", "qmc_metropolis", "qmc_batch_stats",
            "qmc_fp64_peak", "qmc_model_flops", "qmc_launch_count", "qmc_status_string", "qmc_n_param",
-           "qmc_log_derivatives", "qmc_energy_gradient", "qmc_local_energy_host"]
+           "qmc_log_derivatives", "qmc_energy_gradient", "qmc_local_energy_host", "qmc_orbital_derivatives"]
 
 
 class QmcError(RuntimeError):
@@ -56,6 +56,8 @@ def lib():
         L.qmc_destroy.argtypes = [vp]
         L.qmc_local_energy.restype = C.c_int
         L.qmc_local_energy.argtypes = [vp, vp, i64, vp, vp, vp, vp]
+        L.qmc_orbital_derivatives.restype = C.c_int
+        L.qmc_orbital_derivatives.argtypes = [vp, vp, i64, vp, vp, vp]
         L.qmc_local_energy_host.restype = C.c_int
         L.qmc_local_energy_host.argtypes = [vp, vp, i64, vp, vp, vp, C.c_int32]
         L.qmc_log_psi.restype = C.c_int
@@ -200,6 +202,14 @@ class QmcSystem:
                                     C.addressof(nacc) if count else None, _stream(stream)))
         return dict(logpsi=logpsi, sign=sign, accept=accept, eloc_acc=eloc_acc,
                     n_accepted=nacc.value if count else None)
+
+    def orbital_derivatives(self, r, n_ao: int, n_mo: int, stream=None):
+        """qmc_orbital_derivatives: (dC[M, n_ao, n_mo], dzeta[M, n_ao]) = d ln Psi / d C, d ln Psi / d zeta."""
+        M = self._chk_r(r)
+        dC = torch.empty((M, n_ao, n_mo), dtype=torch.float64, device=r.device)
+        dz = torch.empty((M, n_ao), dtype=torch.float64, device=r.device)
+        _check(lib().qmc_orbital_derivatives(self._h, _dp(r), M, _dp(dC), _dp(dz), _stream(stream)))
+        return dC, dz
 
     def n_param(self) -> int:
         return int(lib().qmc_n_param(self._h))

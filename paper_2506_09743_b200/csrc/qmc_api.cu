@@ -37,7 +37,9 @@ struct Variant {
   int NS, NMO, LP, ws_doubles;
   bool exact;  // compiled for n_up = n_dn = NS
   const void *k_el, *k_psi, *k_metro, *k_expl, *k_el_deriv;
-  const void *e_el, *e_psi, *e_metro, *e_expl, *e_el_deriv;  // the same with the e-e-n Jastrow kernel D.3 (EEN)
+  const void *e_el, *e_psi, *e_metro, *e_expl, *e_el_deriv;
+  const void *k_orb;  // orbital-parameter derivatives
+  int orb_ws_doubles;  // the same with the e-e-n Jastrow kernel D.3 (EEN)
 };
 
 template <int NS, int NMO, bool X>
@@ -53,6 +55,8 @@ Variant make_variant() {
   v.k_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi>;
   v.k_expl = (const void *)explicit_energy_kernel<NS, NMO, X, kWarpsEl>;
   v.k_el_deriv = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true>;
+  v.k_orb = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsEl>;
+  v.orb_ws_doubles = Geo<NS, NMO>::total + Geo<NS, NMO>::orbExtra;
   v.e_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, false, true>;
   v.e_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi, false, true>;
   v.e_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi, true>;
@@ -96,7 +100,8 @@ struct qmc_system {
   Variant var{};
   int smem_el = 0, smem_psi = 0;  // dynamic shared memory of the E_L kernels (kWarpsEl warps) / values-only kernels
   int blocks_el = 0, blocks_psi = 0, blocks_metro = 0, blocks_expl = 0, blocks_deriv = 0;
-  void *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr, *d_orig = nullptr;
+  void *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr, *d_orig = nullptr, *d_rowao = nullptr,
+       *d_rownrm = nullptr;
   int n_sm = 0;
   double *d_stats = nullptr;
   unsigned long long *d_counter = nullptr;
@@ -107,6 +112,8 @@ struct qmc_system {
   std::mutex scratch_mu;
   std::unordered_map<cudaStream_t, Scratch> scratch;
   // qmc_local_energy_host: two internal streams and double-buffered device scratch (grown on demand)
+  bool orb_ready = false;  // orbital-derivative kernel configured (lazily: most users never call it)
+  int blocks_orb = 0;
   cudaStream_t hst[2] = {nullptr, nullptr};
   double *hbuf[2] = {nullptr, nullptr};
   int64_t hbuf_walkers = 0;
@@ -139,6 +146,8 @@ void qmc_destroy(qmc_system_t *s) {
   cudaFree(s->d_gen);
   cudaFree(s->d_cols);
   cudaFree(s->d_orig);
+  cudaFree(s->d_rowao);
+  cudaFree(s->d_rownrm);
   cudaFree(s->d_stats);
   cudaFree(s->d_counter);
   for (auto &kv : s->scratch) cudaFree(kv.second.p);
@@ -397,6 +406,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     rc.r.c2 = (double)(k * (k + 2 * l + 1));
     rc.r.kd = (double)k;
     rc.r.pad = 0;
+    rc.r.dlnN = d->ao_norm ? 0.0 : (n + 0.5) / z;
     int kind;
     if (l == 0) { kind = SH_S; rc.aos = {b}; b += 1; }
     else if (full) { kind = (l == 1) ? SH_P : SH_D; for (int t = 0; t < nfun; ++t) rc.aos.push_back(b + t); b += nfun; }
@@ -414,6 +424,8 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   std::vector<ShellRec> shells;
   int n_real_shells = 0;
   std::vector<std::vector<double>> crow;  // kernel AO row -> coefficients of the referenced MOs (or empty = pad)
+  std::vector<int> row_ao;                // kernel AO row -> caller's AO index (-1 = pad)
+  std::vector<double> row_nrm;            // kernel AO row -> normalisation
   {
     int row = 0;
     int n_real = 0;
@@ -438,7 +450,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
       ++n_real;
       if (row % kChunk + nf > kChunk) {
         last_shell().meta |= (row % kChunk) << 20;
-        while (row % kChunk) { crow.emplace_back(); ++row; }
+        while (row % kChunk) { crow.emplace_back(); row_ao.push_back(-1); row_nrm.push_back(0.0); ++row; }
       }
       recs[i].r.meta |= (row % kChunk) << 12;
       for (int b : recs[i].aos) {
@@ -446,6 +458,8 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
         std::vector<double> c(P.n_mo);
         for (int mo = 0; mo < P.n_mo; ++mo) c[mo] = nrm * d->mo_coeff[(size_t)b * d->n_mo + used[mo]];
         crow.push_back(c);
+        row_ao.push_back(b);
+        row_nrm.push_back(nrm);
         ++row;
       }
       shells.push_back(recs[i].r);
@@ -454,7 +468,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     }
     if (row % kChunk) {
       last_shell().meta |= (row % kChunk) << 20;
-      while (row % kChunk) { crow.emplace_back(); ++row; }
+      while (row % kChunk) { crow.emplace_back(); row_ao.push_back(-1); row_nrm.push_back(0.0); ++row; }
     }
     n_real_shells = n_real;
   }
@@ -532,7 +546,11 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
       (e = cudaMalloc(&s->d_cols, cols.size() * sizeof(DetCols))) != cudaSuccess ||
       (e = cudaMemcpy(s->d_cols, cols.data(), cols.size() * sizeof(DetCols), cudaMemcpyHostToDevice)) != cudaSuccess ||
       (e = cudaMalloc(&s->d_orig, det_orig.size() * sizeof(int))) != cudaSuccess ||
-      (e = cudaMemcpy(s->d_orig, det_orig.data(), det_orig.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess) {
+      (e = cudaMemcpy(s->d_orig, det_orig.data(), det_orig.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMalloc(&s->d_rowao, row_ao.size() * sizeof(int))) != cudaSuccess ||
+      (e = cudaMemcpy(s->d_rowao, row_ao.data(), row_ao.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMalloc(&s->d_rownrm, row_nrm.size() * sizeof(double))) != cudaSuccess ||
+      (e = cudaMemcpy(s->d_rownrm, row_nrm.data(), row_nrm.size() * sizeof(double), cudaMemcpyHostToDevice)) != cudaSuccess) {
     int rc = cuda_fail(e, "qmc_setup upload");
     qmc_destroy(s);
     return rc;
@@ -544,6 +562,10 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   P.gen = (const GenDet *)s->d_gen;
   P.det_cols = (const DetCols *)s->d_cols;
   P.det_orig = (const int *)s->d_orig;
+  P.ao_orig = (const int *)s->d_rowao;
+  P.ao_nrm = (const double *)s->d_rownrm;
+  for (int a = 0; a < 16; ++a) P.mo_orig[a] = a < P.n_mo ? used[a] : 0;
+  P.n_mo_all = d->n_mo;
   P.smem_const_bytes = (int)((szC + szD + 15) / 16 * 16);
   s->smem_el = P.smem_const_bytes + kWarpsEl * var->ws_doubles * (int)sizeof(double);
   s->smem_psi = P.smem_const_bytes + kWarpsPsi * var->ws_doubles * (int)sizeof(double);
@@ -783,6 +805,37 @@ int qmc_energy_gradient(const double *d_eloc, const double *d_O, int64_t M, int3
   if (e != cudaSuccess) return cuda_fail(e, "qmc_energy_gradient");
   if (h_Ev) *h_Ev = h[0];
   for (int p = 0; p < n_param; ++p) h_grad[p] = h[2 + p];
+  return QMC_OK;
+}
+
+int qmc_orbital_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d_dC, double *d_dzeta, void *cuda_stream) {
+  if (!s || !d_r || M <= 0 || (!d_dC && !d_dzeta)) return QMC_EINVAL;
+  CK(cudaSetDevice(s->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int smem = s->P.smem_const_bytes + kWarpsEl * s->var.orb_ws_doubles * (int)sizeof(double);
+  if (!s->orb_ready) {
+    int dev_smem = 0;
+    cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, s->device);
+    if (smem > dev_smem) return QMC_EUNSUPPORTED;
+    CK(cudaFuncSetAttribute(s->var.k_orb, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    int per_sm = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, s->var.k_orb, kWarpsEl * 32, smem));
+    if (per_sm < 1) return QMC_EUNSUPPORTED;
+    s->blocks_orb = per_sm * s->n_sm;
+    s->orb_ready = true;
+  }
+  // coefficients of MOs that no determinant uses have a zero derivative and are not touched by the kernel
+  if (d_dC) CK(cudaMemsetAsync(d_dC, 0, (size_t)M * (size_t)s->P.n_ao * (size_t)s->P.n_mo_all * sizeof(double), st));
+  WalkerIO io{};
+  io.r_in = d_r;
+  io.M = M;
+  io.logpsi = d_dC;    // this kernel's outputs travel in the two output slots: dC [M][n_ao][n_mo], dzeta [M][n_ao]
+  io.eloc = d_dzeta;
+  const int64_t groups = (M + s->P.G - 1) / s->P.G;
+  const int grid = (int)std::min<int64_t>((groups + kWarpsEl - 1) / kWarpsEl, s->blocks_orb);
+  void *args[2] = {(void *)&s->P, (void *)&io};
+  CK(cudaLaunchKernel(s->var.k_orb, dim3(grid), dim3(kWarpsEl * 32), args, smem, st));
+  ++g_launches;
   return QMC_OK;
 }
 

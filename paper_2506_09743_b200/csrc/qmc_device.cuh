@@ -37,7 +37,7 @@ constexpr int kWarpsMax = kWarpsEl > kWarpsPsi ? kWarpsEl : kWarpsPsi;
 
 // shell record kinds
 enum : int { SH_S = 0, SH_P = 1, SH_D = 2, SH_P1 = 3, SH_D1 = 4, SH_ATOM = 5 };
-constexpr int kMaxShells = 208;  // shell + atom records; they live in the kernel parameter block (constant bank, uniform data path)
+constexpr int kMaxShells = 192;  // shell + atom records; they live in the kernel parameter block (constant bank, uniform data path)
 
 // One shell = the AOs that share a centre, n, l and zeta (one radial factor).  Every lane reads the same
 // record, so the records sit in the kernel parameters: the loads go through the uniform data path
@@ -49,6 +49,7 @@ struct ShellRec {
   double kd;     // (double) k,  k = n - 1 - l the radial power
   int32_t meta;  // kind | k << 4 | m << 8 | row in chunk << 12 | flush << 20
   int32_t pad;
+  double dlnN;   // d ln(normalisation) / d zeta = (n + 1/2) / zeta, or 0 with a caller-supplied ao_norm (orbital derivatives)
 };
 // meta fields: kind = SH_*; m = harmonic index of the single-function kinds; row = first AO row of the record
 // inside its chunk; flush = 0, or on the last record of a chunk the number of rows the chunk uses
@@ -129,6 +130,12 @@ struct SysParams {  // passed by value to every kernel
   int n_gen;
   int n_det_all;                   // all determinants
   const DetCols *det_cols;         // device [n_det_all]
+  // orbital-parameter derivatives (qmc_orbital_derivatives): kernel AO row -> caller's AO index (-1 = padding row)
+  // and normalisation, kernel MO column -> caller's MO index
+  const int *ao_orig;              // device [n_chunks * kChunk]
+  const double *ao_nrm;            // device [n_chunks * kChunk]
+  int mo_orig[16];
+  int n_mo_all;                    // MOs of the caller's coefficient matrix
 };
 
 struct WalkerIO {
@@ -242,6 +249,12 @@ struct Geo {
   __host__ __device__ static constexpr int mergeShift(int fr) { return (fr & 4) << 3; }  // rows 4..7: + 32
   static constexpr int total = cmax(layout_total, kChunk * S2);
   static constexpr int NT = (NMO + 7) / 8;                    // 8-column MO tiles
+  // orbital-derivative kernel only: behind the common scratch, Gamma [ROWS][NMO], then the inverses of one determinant's
+  // problems [2 GMAX][NS][NS] and their column indices [2 GMAX][NS] (ints)
+  static constexpr int oGam = total;
+  static constexpr int oInv = oGam + even(ROWS * NMO);
+  static constexpr int oCol = oInv + even(2 * GMAX * NS * NS);
+  static constexpr int orbExtra = even(ROWS * NMO) + even(2 * GMAX * NS * NS) + even(GMAX * NS);
   // bounds of the overlays (compile-time hygiene: no memory checker runs on this pool)
   static_assert(NS >= 1 && NS <= kMaxSpin && NMO <= 16, "instantiation outside the register-array limits");
   static_assert(ROWS <= 32 && 2 * GMAX * NS >= ROWS, "electron rows of a pass exceed the warp");

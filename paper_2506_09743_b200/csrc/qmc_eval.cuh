@@ -176,7 +176,9 @@ __device__ __noinline__ void een_terms(const SysParams &P, const double *sXYZ, i
 // DERIV: also write the logarithmic parameter derivatives of eq. 6 for the G walkers to dv.O.
 // EEN: the wavefunction carries the electron-electron-nucleus kernel D.3 (separate instantiations, so that the
 // kernels of the common case stay free of the call and its register spills: measured 459 -> 508 us otherwise).
-template <int NS, int NMO, bool EL, bool X, bool EXPL = false, bool DERIV = false, bool EEN = false>
+// ORB (with EXPL): B = I, i.e. every determinant's inverse; Gamma[i][alpha] = sum_n d_n D_n^up D_n^dn A_n^-1[pos_n(alpha)][i]
+// is accumulated behind the common scratch (Geo::oGam), for the orbital-parameter derivatives.
+template <int NS, int NMO, bool EL, bool X, bool EXPL = false, bool DERIV = false, bool EEN = false, bool ORB = false>
 __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp,
                              const double *__restrict__ sC, const DetRec *__restrict__ sDet,
                              double *__restrict__ ws, double x, double y, double z, int lane,
@@ -459,6 +461,12 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
     const int c = lane % LP, slot = lane / LP, gbase = lane - c;
     const int nprob = 2 * G;
     double sig = 0.0, numk = 0.0;
+    double *sGam = ws + GE::oGam, *sInv = ws + GE::oInv;
+    int *sCol = reinterpret_cast<int *>(ws + GE::oCol);
+    if (ORB) {
+      for (int i = lane; i < GE::ROWS * NMO; i += 32) sGam[i] = 0.0;
+      __syncwarp();
+    }
     // this warp takes determinants det0, det0 + det_step, ... (the block shares one walker group)
     DetCols nxt = P.det_cols[det0 < P.n_det_all ? det0 : 0];
     for (int n = det0; n < P.n_det_all; n += det_step) {
@@ -478,7 +486,8 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
             const int row = pg * ne + e0 + (i < ns ? i : 0);
             const bool ri = i < ns;
             a0[i] = (ri && cA) ? sPhi[GE::moIdx(EL, row, colA)] : ((i == c) ? 1.0 : 0.0);
-            b0[i] = (ri && cA) ? sB[EL ? GE::moIdx(EL, row, colA) : 0] : 0.0;
+            if (ORB) b0[i] = (ri && cA && i == c) ? 1.0 : 0.0;  // B = I: the reduced block is A_n^-1 itself
+            else b0[i] = (ri && cA) ? sB[EL ? GE::moIdx(EL, row, colA) : 0] : 0.0;
           }
         }
         double det = 1.0;
@@ -523,8 +532,35 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           sProb[pr * 4 + 0] = det;
           sProb[pr * 4 + 2] = t0;
         }
+        if (ORB && pvalid && c < NS) {
+          // row k of the reduced block belongs to reference position perm[k]: b0[k] = A_n^-1[perm[k]][electron c]
+#pragma unroll
+          for (int k = 0; k < NS; ++k) {
+            sInv[(pr * NS + k) * NS + c] = b0[k];
+            if (c == 0) sCol[pr * NS + k] = (perm[k] < ns) ? (int)dc.col[sp][perm[k] < kMaxSpin ? perm[k] : 0] : -1;
+          }
+        }
       }
       __syncwarp();
+      if (ORB) {
+        // d ln D / d A[i][j] = A^-1[j][i], weighted by d_n D_n^up D_n^dn (both determinants are known only now)
+        for (int pass = 0; pass * PP < nprob; ++pass) {
+          const int pr = pass * PP + slot;
+          if (pr < nprob) {
+            const int pg = pr >> 1, sp = pr & 1;
+            const int ns = sp ? n_dn : n_up, e0 = sp ? n_up : 0;
+            const double w = dc.d * sProb[pr * 4 + 0] * sProb[(pr ^ 1) * 4 + 0];
+            if (c < ns) {
+              const int row = pg * ne + e0 + c;
+#pragma unroll
+              for (int k = 0; k < NS; ++k) {
+                const int col = sCol[pr * NS + k];
+                if (col >= 0) sGam[row * NMO + col] = fma(w, sInv[(pr * NS + k) * NS + c], sGam[row * NMO + col]);
+              }
+            }
+          }
+        }
+      }
       if (lane < G) {
         const double w = dc.d * sProb[(2 * lane) * 4 + 0] * sProb[(2 * lane + 1) * 4 + 0];
         sig += w;                                                                  // eq. 4

@@ -168,6 +168,135 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
 }
 
 // ---------------------------------------------------------------------------------
+// Orbital-parameter derivatives (eq. 6 factors of the AO and MO layers):
+//   dC[w][beta][alpha] = d ln Psi / d C[beta][alpha] = sum_i phi_beta(r_i) Gamma[i][alpha]
+//   dzeta[w][beta]     = d ln Psi / d zeta_beta      = sum_alpha C[beta][alpha] sum_i (d phi_beta / d zeta)(r_i) Gamma[i][alpha]
+// with Gamma = d ln Sigma / d Phi from every determinant's explicit inverse (eval_walkers<..., ORB>), then a second
+// pass over the shells that rebuilds phi and d phi / d zeta = phi (d ln N / d zeta - r) in the AO tile and contracts
+// them with Gamma.  Correct and simple, not fast: N_det eliminations per walker (DESIGN.md section 9 has the
+// table-based plan).  Outputs travel in io.logpsi (dC) and io.eloc (dzeta); either may be null.
+// ---------------------------------------------------------------------------------
+template <int NS, int NMO, bool X, int WPB>
+__global__ void __launch_bounds__(WPB * 32, 1)
+    orbital_derivatives_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const double *sC;
+  const double *sExp;
+  const DetRec *sDet;
+  double *wsBase;
+  load_constants<NMO>(P, smem, sC, sExp, sDet, wsBase);
+  using GE = Geo<NS, NMO>;
+  constexpr int S = GE::S2, NT = GE::NT;
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
+  double *ws = wsBase + warp * (GE::total + GE::orbExtra);
+  const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
+  const int g = lane / ne, e = lane - g * ne;
+  const int64_t n_groups = (io.M + G - 1) / G;
+  const int64_t stride = (int64_t)gridDim.x * WPB;
+  double *dC = io.logpsi, *dZ = io.eloc;
+  double *sGam = ws + GE::oGam;
+  const double *sRes = ws + GE::oRes;
+  for (int64_t grp = (int64_t)blockIdx.x * WPB + warp; grp < n_groups; grp += stride) {
+    const int64_t w = grp * G + g;
+    double x, y, z;
+    if ((g < G) && (w < io.M)) {
+      x = io.r_in[((int64_t)e * 3 + 0) * io.M + w];
+      y = io.r_in[((int64_t)e * 3 + 1) * io.M + w];
+      z = io.r_in[((int64_t)e * 3 + 2) * io.M + w];
+    } else {
+      dummy_xyz(lane, x, y, z);
+    }
+    // MO values, then every determinant's inverse -> unnormalised Gamma and Sigma (sRes[4 g])
+    eval_walkers<NS, NMO, false, X, true, false, false, true>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
+    for (int i = lane; i < G * ne * NMO; i += 32) sGam[i] /= sRes[(i / (ne * NMO)) * 4 + 0];
+    __syncwarp();
+    // second pass over the shells: phi into column lane, d phi / d zeta into column opCol(lane) of the tile
+    double *const tile = ws;
+    double *const tl = tile + lane, *const tz = tile + GE::opCol(lane);
+    int chunk = 0;
+    double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1.0, r = 1.0;
+    for (int s = 0; s < P.n_shell; ++s) {
+      const ShellRec &sh = P.shells[s];
+      const int meta = sh.meta, kind = meta & 15;
+      if (kind == SH_ATOM) {
+        dx = x - sh.zeta;
+        dy = y - sh.c1;
+        dz = z - sh.c2;
+        r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+        r = r2 * rsqrt_fast(r2);
+        continue;
+      }
+      double gr = exp_neg(-sh.zeta * r, sExp);
+      if (meta & kMetaK1) gr *= r;
+      if (meta & kMetaK2) gr *= r2;
+      const double zf = sh.dlnN - r;  // d ln phi / d zeta
+      const int row = (meta >> 12) & 15, m = (meta >> 8) & 15;
+      double ang[5];
+      int nf = 1;
+      if (kind == SH_S) {
+        ang[0] = 1.0;
+      } else if (kind == SH_P) {
+        ang[0] = dx; ang[1] = dy; ang[2] = dz; nf = 3;
+      } else if (kind == SH_P1) {
+        ang[0] = (m == 0) ? dx : ((m == 1) ? dy : dz);
+      } else {
+        const double dd[5] = {dx * dy, dy * dz, dz * dx, fma(dx, dx, -dy * dy), fma(2.0 * dz, dz, -fma(dx, dx, dy * dy))};
+        if (kind == SH_D) {
+#pragma unroll
+          for (int t = 0; t < 5; ++t) ang[t] = dd[t];
+          nf = 5;
+        } else {
+          ang[0] = dd[m < 5 ? m : 0];
+        }
+      }
+      for (int t = 0; t < nf; ++t) {
+        const double phi = gr * ang[t];
+        tl[(row + t) * S] = phi;
+        tz[(row + t) * S] = phi * zf;
+      }
+      const int flush = meta >> 20;
+      if (flush) {
+        for (int pr = flush; pr < kChunk; ++pr) { tl[pr * S] = 0.0; tz[pr * S] = 0.0; }
+        __syncwarp();
+        // kernel-order (N C)[R][col] from the DMMA B-fragment table: [chunk][k-step][MO tile][4 n + k]
+        const double *cfr = sC + chunk * ((kChunk / 4) * NT * 32);
+        if (dC)
+          for (int idx = lane; idx < G * kChunk * NMO; idx += 32) {
+            const int gg = idx / (kChunk * NMO), rem = idx - gg * (kChunk * NMO), rw = rem / NMO, col = rem - rw * NMO;
+            const int R = chunk * kChunk + rw, beta = P.ao_orig[R];
+            const int64_t wo = grp * G + gg;
+            if (beta >= 0 && col < P.n_mo && wo < io.M) {
+              double t = 0.0;
+              for (int i = 0; i < ne; ++i) t = fma(tile[rw * S + gg * ne + i], sGam[(gg * ne + i) * NMO + col], t);
+              dC[(wo * P.n_ao + beta) * P.n_mo_all + P.mo_orig[col]] = P.ao_nrm[R] * t;
+            }
+          }
+        if (dZ)
+          for (int idx = lane; idx < G * kChunk; idx += 32) {
+            const int gg = idx / kChunk, rw = idx - gg * kChunk;
+            const int R = chunk * kChunk + rw, beta = P.ao_orig[R];
+            const int64_t wo = grp * G + gg;
+            if (beta >= 0 && wo < io.M) {
+              double acc = 0.0;
+              for (int col = 0; col < P.n_mo; ++col) {
+                double t = 0.0;
+                for (int i = 0; i < ne; ++i)
+                  t = fma(tile[rw * S + GE::opCol(gg * ne + i)], sGam[(gg * ne + i) * NMO + col], t);
+                const double nc = cfr[(((rw >> 2) * NT) + (col >> 3)) * 32 + 4 * (col & 7) + (rw & 3)];
+                acc = fma(nc, t, acc);
+              }
+              dZ[wo * P.n_ao + beta] = acc;
+            }
+          }
+        __syncwarp();
+        ++chunk;
+      }
+    }
+    __syncwarp();
+  }
+}
+
+// ---------------------------------------------------------------------------------
 // Persistent all-electron Metropolis (readings Q9, Q10).
 // Walker coordinates and log|Psi| stay in registers for all sweeps.
 // ---------------------------------------------------------------------------------

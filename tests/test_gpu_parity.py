@@ -587,3 +587,39 @@ def test_metropolis_zero_sweeps_only_evaluates(env):
     out = s.metropolis(rg, 0.3, 0, seed=1, want_eloc_acc=True)
     assert float(out["eloc_acc"].abs().max()) == 0.0 and torch.equal(out["logpsi"], lp)
     s.close()
+
+
+# ----------------------------------------------------------------------------- orbital-parameter derivatives
+def check_orbital_derivatives(env, d, r, threads=8):
+    torch, ob, qb = env
+    o = ob.OracleSystem(d)
+    lp0 = ob.local_energy(o, r, threads=threads)[0]
+    dC0, dz0 = ob.orbital_derivatives(o, r, threads=threads)
+    s = qb.QmcSystem(d)
+    dC, dz = (t.cpu().numpy() for t in s.orbital_derivatives(_to_gpu(torch, r), d.n_ao, d.n_mo))
+    s.close()
+    keep = lp0 - lp0.max() > math.log(1e-6)
+    eC = np.abs(dC - dC0) / np.maximum(1.0, np.abs(dC0))
+    ez = np.abs(dz - dz0) / np.maximum(1.0, np.abs(dz0))
+    assert np.max(eC[keep]) < 1e-8, np.max(eC[keep])
+    assert np.max(ez[keep]) < 1e-8, np.max(ez[keep])
+
+
+@pytest.mark.parametrize("name,M", [("H2", 515), ("LiH", 300), ("Li2", 257), ("CO", 129)])
+def test_orbital_derivatives_configs(env, name, M):
+    d, r = wl.CONFIGS[name](M=M)
+    check_orbital_derivatives(env, d, r)
+
+
+def test_orbital_derivatives_odd_system(env):
+    rng = np.random.default_rng(31)
+    aos = [(2, 1, 2, 1.1), (1, 0, 0, 2.0), (3, 2, 3, 0.9), (2, 1, 0, 1.3), (3, 2, 1, 0.7), (2, 0, 0, 1.5),
+           (3, 0, 0, 1.2), (3, 1, 1, 0.8), (2, 1, 1, 1.3)]
+    C = rng.standard_normal((len(aos), 7))
+    det_up = [[4, 0, 2], [4, 5, 2], [1, 0, 2], [4, 3, 5]]
+    det_dn = [[1, 3], [1, 3], [0, 3], [1, 2]]
+    for norm in (None, rng.uniform(0.5, 2, len(aos))):
+        d = atom_system(3.0, aos, C, 3, 2, det_up=det_up, det_dn=det_dn, ci=[0.9, 0.2, -0.3, 0.15], norm=norm,
+                        a_par=0.25, a_anti=0.5, b=0.8, xyz=(0.1, -0.2, 0.3))
+        r = soa(rng.standard_normal((131, 5, 3)) * 1.5)
+        check_orbital_derivatives(env, d, r, threads=2)
