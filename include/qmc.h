@@ -187,8 +187,9 @@ int qmc_log_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d
  *   d_dzeta device, out: double [M][n_ao]        d ln Psi / d zeta_beta, each AO's exponent on its own (with the
  *           standard normalisation d ln N / d zeta = (n + 1/2) / zeta is included; a caller-supplied ao_norm is
  *           taken as independent of zeta)
- * Either may be NULL.  First version: every determinant is inverted explicitly for every walker (N_det
- * eliminations per walker), i.e. it is correct but far slower than qmc_local_energy.  Asynchronous. */
+ * Either may be NULL.  One elimination per spin (the reference's tables); groups of walkers whose reference
+ * determinant is nearly singular, (Sigma/D_0)^2 > 1e4, and expansions with more than two substitutions per spin
+ * invert every determinant explicitly instead.  Deterministic.  Asynchronous. */
 int qmc_orbital_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d_dC, double *d_dzeta,
                             void *cuda_stream);
 

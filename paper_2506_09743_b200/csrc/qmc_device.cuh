@@ -96,6 +96,9 @@ constexpr double kFallbackK = 8.0e5;
 // ... and in any case when |Sigma / D_0| > 1e4: log|Psi| of the table path is off by ~1e-15 |Sigma/D_0| (1e-12 at
 // 1024), and its parity bound 1e-10 is ABSOLUTE, so walkers with a huge |E_L| must not escape through the first test.
 constexpr double kFallbackCap = 1.0e8;
+// Orbital-parameter derivatives: the table-path error of Gamma is ~1.2e-15 (Sigma/D_0)^2 of the walker's largest
+// derivative (measured); beyond (Sigma/D_0)^2 = 1e4 the group takes the explicit route.
+constexpr double kFallbackOrb = 1.0e4;
 
 struct SysParams {  // passed by value to every kernel
   int n_atoms, n_up, n_dn, n_e;
@@ -254,7 +257,8 @@ struct Geo {
   static constexpr int oGam = total;
   static constexpr int oInv = oGam + even(ROWS * NMO);
   static constexpr int oCol = oInv + even(2 * GMAX * NS * NS);
-  static constexpr int orbExtra = even(ROWS * NMO) + even(2 * GMAX * NS * NS) + even(GMAX * NS);
+  static constexpr int oY = oCol + even(GMAX * NS);        // table path: Y = d den / d T, laid out like the T tables
+  static constexpr int orbExtra = even(ROWS * NMO) + even(2 * GMAX * NS * NS) + even(GMAX * NS) + even(2 * GMAX * TS);
   // bounds of the overlays (compile-time hygiene: no memory checker runs on this pool)
   static_assert(NS >= 1 && NS <= kMaxSpin && NMO <= 16, "instantiation outside the register-array limits");
   static_assert(ROWS <= 32 && 2 * GMAX * NS >= ROWS, "electron rows of a pass exceed the warp");

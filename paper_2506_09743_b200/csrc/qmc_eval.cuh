@@ -176,9 +176,11 @@ __device__ __noinline__ void een_terms(const SysParams &P, const double *sXYZ, i
 // DERIV: also write the logarithmic parameter derivatives of eq. 6 for the G walkers to dv.O.
 // EEN: the wavefunction carries the electron-electron-nucleus kernel D.3 (separate instantiations, so that the
 // kernels of the common case stay free of the call and its register spills: measured 459 -> 508 us otherwise).
-// ORB (with EXPL): B = I, i.e. every determinant's inverse; Gamma[i][alpha] = sum_n d_n D_n^up D_n^dn A_n^-1[pos_n(alpha)][i]
+// ORB = 1 (with EXPL): B = I, i.e. every determinant's inverse; Gamma[i][alpha] = sum_n d_n D_n^up D_n^dn A_n^-1[pos_n(alpha)][i]
 // is accumulated behind the common scratch (Geo::oGam), for the orbital-parameter derivatives.
-template <int NS, int NMO, bool EL, bool X, bool EXPL = false, bool DERIV = false, bool EEN = false, bool ORB = false>
+// ORB = 2 (table path, values only): the same Gamma from the reference alone: A0^-1 through an identity block of the
+// elimination, Y = d den / d T accumulated in the CI pass, Gamma_virt = A0^-T Y / den, Gamma_occ = A0^-T - Gamma_virt T^T.
+template <int NS, int NMO, bool EL, bool X, bool EXPL = false, bool DERIV = false, bool EEN = false, int ORB = 0>
 __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp,
                              const double *__restrict__ sC, const DetRec *__restrict__ sDet,
                              double *__restrict__ ws, double x, double y, double z, int lane,
@@ -463,7 +465,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
     double sig = 0.0, numk = 0.0;
     double *sGam = ws + GE::oGam, *sInv = ws + GE::oInv;
     int *sCol = reinterpret_cast<int *>(ws + GE::oCol);
-    if (ORB) {
+    if (ORB == 1) {
       for (int i = lane; i < GE::ROWS * NMO; i += 32) sGam[i] = 0.0;
       __syncwarp();
     }
@@ -486,7 +488,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
             const int row = pg * ne + e0 + (i < ns ? i : 0);
             const bool ri = i < ns;
             a0[i] = (ri && cA) ? sPhi[GE::moIdx(EL, row, colA)] : ((i == c) ? 1.0 : 0.0);
-            if (ORB) b0[i] = (ri && cA && i == c) ? 1.0 : 0.0;  // B = I: the reduced block is A_n^-1 itself
+            if (ORB == 1) b0[i] = (ri && cA && i == c) ? 1.0 : 0.0;  // B = I: the reduced block is A_n^-1 itself
             else b0[i] = (ri && cA) ? sB[EL ? GE::moIdx(EL, row, colA) : 0] : 0.0;
           }
         }
@@ -532,7 +534,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           sProb[pr * 4 + 0] = det;
           sProb[pr * 4 + 2] = t0;
         }
-        if (ORB && pvalid && c < NS) {
+        if (ORB == 1 && pvalid && c < NS) {
           // row k of the reduced block belongs to reference position perm[k]: b0[k] = A_n^-1[perm[k]][electron c]
 #pragma unroll
           for (int k = 0; k < NS; ++k) {
@@ -542,7 +544,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
         }
       }
       __syncwarp();
-      if (ORB) {
+      if (ORB == 1) {
         // d ln D / d A[i][j] = A^-1[j][i], weighted by d_n D_n^up D_n^dn (both determinants are known only now)
         for (int pass = 0; pass * PP < nprob; ++pass) {
           const int pr = pass * PP + slot;
@@ -596,6 +598,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       const int pg = pvalid ? (pr >> 1) : 0, sp = pr & 1;
       const int ns = sp ? n_dn : n_up, nv = P.nv[sp], e0 = sp ? n_up : 0;
       double a0[NS], av[NS], b0[EL ? NS : 1], bv[EL ? NS : 1];
+      double ai[ORB == 2 ? NS : 1];  // ORB = 2: identity block -> A0^-1
       {
         const bool cA = c < ns, cV = c < nv;
         const int colA = cA ? P.ref_col[sp][c < kMaxSpin ? c : 0] : 0;
@@ -606,6 +609,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           const bool ri = i < ns;
           a0[i] = (ri && cA) ? sPhi[GE::moIdx(EL, row, colA)] : ((i == c) ? 1.0 : 0.0);  // identity padding
           av[i] = (ri && cV) ? sPhi[GE::moIdx(EL, row, colV)] : 0.0;
+          if (ORB == 2) ai[i] = (ri && cA && i == c) ? 1.0 : 0.0;
           if (EL) {
             b0[i] = (ri && cA) ? sB[GE::moIdx(EL, row, colA)] : 0.0;
             bv[i] = (ri && cV) ? sB[GE::moIdx(EL, row, colV)] : 0.0;
@@ -650,6 +654,12 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           av[k] = t;
 #pragma unroll
           for (int i = 0; i < NS; ++i) if (i != k) av[i] = fma(-f[i], t, av[i]);
+          if (ORB == 2) {
+            t = ai[k] * inv;
+            ai[k] = t;
+#pragma unroll
+            for (int i = 0; i < NS; ++i) if (i != k) ai[i] = fma(-f[i], t, ai[i]);
+          }
           if (EL) {
             t = b0[k] * inv;
             b0[k] = t;
@@ -699,6 +709,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
         for (int k = 0; k < NS; ++k) {
           if (EL) reinterpret_cast<double2 *>(sT)[pr * TS + perm[k] * RS + c] = make_double2(av[k], bv[EL ? k : 0]);
           else sT[pr * TS + perm[k] * RS + c] = av[k];
+          if (ORB == 2 && c < NS) (ws + GE::oInv)[(pr * NS + perm[k]) * NS + c] = ai[ORB == 2 ? k : 0];  // A0^-1[position][electron]
         }
         if (c == 0) {
           if (EL) {
@@ -816,6 +827,106 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       // parity bound 1e-8 max(1, |E_L|), or that of log|Psi|, ~1e-15 |Sigma/D_0|, a tenth of its absolute bound
       // 1e-10 (kFallbackCap); also set for NaN (singular reference)
       sRes[wg * 4 + 3] = (den * den <= fmin(kFallbackK * fmax(1.0, fabs(eloc)), kFallbackCap)) ? 0.0 : 1.0;
+    }
+    if (ORB == 2) {
+      // ---- Gamma = d ln Sigma / d Phi from the reference alone (lane c of a problem = electron c of that spin):
+      //   Gamma_virt[i][q] = sum_p A0^-1[p][i] Y[p][q] / den,   Gamma_occ[i][j] = A0^-1[j][i] - sum_q Gamma_virt[i][q] T[j][q]
+      // Y = d den / d T first, in the layout of the T tables: a second pass over the determinant classes whose adds
+      // run one lane of a walker at a time, in lane order, so that the sums are the same on every run.
+      static_assert(!(ORB == 2 && EL), "the table-path Gamma is a values-only evaluation");
+      double *sY = ws + GE::oY, *sGamF = ws + GE::oGam;
+      const double *sInvF = ws + GE::oInv;
+      for (int i = lane; i < 2 * G * TS; i += 32) sY[i] = 0.0;
+      for (int i = lane; i < GE::ROWS * NMO; i += 32) sGamF[i] = 0.0;
+      if (wvalid && sub == 0) sProb[pu * 4 + 3] = den;
+      __syncwarp();
+      double *Yw = sY + pu * TS;  // this walker's Y (up spin, then down)
+      for (int n0 = 0; n0 < P.n_det; n0 += LW) {
+        const int n = n0 + sub;
+        const bool act = wvalid && n < P.n_det;
+        int yi[8];
+        double yv[8];
+        int ny = 0;
+        if (act) {
+          const DetRec dr = sDet[n];
+          double D;
+          if (n < P.n_a1) {
+            yi[0] = dr.up >> 3; yv[0] = dr.d; ny = 1;
+          } else if (n < P.n_a2) {
+            double Ru, Rd;
+            entry(dr.up, Ru, D);
+            entry(dr.dn, Rd, D);
+            yi[0] = dr.up >> 3; yv[0] = dr.d * Rd;
+            yi[1] = dr.dn >> 3; yv[1] = dr.d * Ru;
+            ny = 2;
+          } else if (n < P.n_b) {  // cofactors of the 2x2 block {a b; c d}
+            double a, b, c2, d;
+            entry(dr.up & 0xffffu, a, D);
+            entry(dr.up >> 16, b, D);
+            entry(dr.dn & 0xffffu, c2, D);
+            entry(dr.dn >> 16, d, D);
+            yi[0] = (dr.up & 0xffffu) >> 3; yv[0] = dr.d * d;
+            yi[1] = dr.up >> 19; yv[1] = -dr.d * c2;
+            yi[2] = (dr.dn & 0xffffu) >> 3; yv[2] = -dr.d * b;
+            yi[3] = dr.dn >> 19; yv[3] = dr.d * a;
+            ny = 4;
+          } else {  // per spin: cofactors of {T11 T12; T21 T22} times the other spin's R; the constant slots carry no Y
+            double Ru, Rd;
+            excite_double<false>(dr.up, Tu, Ru, D);
+            excite_double<false>(dr.dn, Td, Rd, D);
+#pragma unroll
+            for (int sp2 = 0; sp2 < 2; ++sp2) {
+              const uint32_t ix = sp2 ? dr.dn : dr.up;
+              const double *Tt = sp2 ? Td : Tu;
+              const double wo = dr.d * (sp2 ? Ru : Rd);
+              const int i11 = ix & 255, i12 = (ix >> 8) & 255, i21 = (ix >> 16) & 255, i22 = ix >> 24;
+              yi[4 * sp2 + 0] = sp2 * TS + i11; yv[4 * sp2 + 0] = wo * Tt[i22];
+              yi[4 * sp2 + 1] = sp2 * TS + i22; yv[4 * sp2 + 1] = wo * Tt[i11];
+              yi[4 * sp2 + 2] = sp2 * TS + i12; yv[4 * sp2 + 2] = -wo * Tt[i21];
+              yi[4 * sp2 + 3] = sp2 * TS + i21; yv[4 * sp2 + 3] = -wo * Tt[i12];
+            }
+            ny = 8;
+          }
+        }
+        for (int t = 0; t < LW; ++t) {
+          if (act && sub == t)
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+              if (k < ny) Yw[yi[k]] += yv[k];   // slots NS*RS, NS*RS+1 of a table collect the constants' share: never read
+          __syncwarp();
+        }
+      }
+      const int c = lane % LP, slot = lane / LP;
+      for (int pass = 0; pass * PP < 2 * G; ++pass) {
+        const int pr = pass * PP + slot;
+        if (pr < 2 * G) {
+          const int pg = pr >> 1, sp = pr & 1;
+          const int ns = sp ? n_dn : n_up, nv = P.nv[sp], e0 = sp ? n_up : 0;
+          if (c < ns) {
+            const double iden = 1.0 / sProb[(pr & ~1) * 4 + 3];
+            const int row = (pg * ne + e0 + c) * NMO;
+            double gq[kMaxVirt];
+#pragma unroll
+            for (int q = 0; q < kMaxVirt; ++q) {
+              gq[q] = 0.0;
+              if (q < nv) {
+                double t = 0.0;
+                for (int p = 0; p < ns; ++p) t = fma(sInvF[(pr * NS + p) * NS + c], sY[pr * TS + p * RS + q], t);
+                gq[q] = t * iden;
+                sGamF[row + P.virt_col[sp][q]] = gq[q];
+              }
+            }
+            for (int j = 0; j < ns; ++j) {
+              double t = sInvF[(pr * NS + j) * NS + c];
+#pragma unroll
+              for (int q = 0; q < kMaxVirt; ++q)
+                if (q < nv) t = fma(-gq[q], sT[pr * TS + j * RS + q], t);
+              sGamF[row + P.ref_col[sp][j]] = t;
+            }
+          }
+        }
+      }
+      __syncwarp();
     }
     if (DERIV) {
       // ---- eq. 6 factors O_p = (dPsi/dtheta_p)/Psi, theta = (a_par, a_anti, b, d_0 ...):

@@ -171,10 +171,10 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
 // Orbital-parameter derivatives (eq. 6 factors of the AO and MO layers):
 //   dC[w][beta][alpha] = d ln Psi / d C[beta][alpha] = sum_i phi_beta(r_i) Gamma[i][alpha]
 //   dzeta[w][beta]     = d ln Psi / d zeta_beta      = sum_alpha C[beta][alpha] sum_i (d phi_beta / d zeta)(r_i) Gamma[i][alpha]
-// with Gamma = d ln Sigma / d Phi from every determinant's explicit inverse (eval_walkers<..., ORB>), then a second
-// pass over the shells that rebuilds phi and d phi / d zeta = phi (d ln N / d zeta - r) in the AO tile and contracts
-// them with Gamma.  Correct and simple, not fast: N_det eliminations per walker (DESIGN.md section 9 has the
-// table-based plan).  Outputs travel in io.logpsi (dC) and io.eloc (dzeta); either may be null.
+// with Gamma = d ln Sigma / d Phi from the reference's excitation tables (eval_walkers<..., ORB = 2>: A0^-1, T and
+// Y = d(Sigma/D0)/dT; explicit per-determinant inverses, ORB = 1, for flagged walkers and general determinants), then
+// a second pass over the shells that rebuilds phi and d phi / d zeta = phi (d ln N / d zeta - r) in the AO tile and
+// contracts them with Gamma.  Outputs travel in io.logpsi (dC) and io.eloc (dzeta); either may be null.
 // ---------------------------------------------------------------------------------
 template <int NS, int NMO, bool X, int WPB>
 __global__ void __launch_bounds__(WPB * 32, 1)
@@ -206,10 +206,23 @@ __global__ void __launch_bounds__(WPB * 32, 1)
     } else {
       dummy_xyz(lane, x, y, z);
     }
-    // MO values, then every determinant's inverse -> unnormalised Gamma and Sigma (sRes[4 g])
-    eval_walkers<NS, NMO, false, X, true, false, false, true>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
-    for (int i = lane; i < G * ne * NMO; i += 32) sGam[i] /= sRes[(i / (ne * NMO)) * 4 + 0];
-    __syncwarp();
+    // Gamma = d ln Sigma / d Phi from the reference's tables (one elimination per spin); when a walker of the group
+    // has (Sigma/D_0)^2 > kFallbackOrb (reference near-singular) or the expansion has general determinants, from every
+    // determinant's inverse instead: unnormalised Gamma and Sigma (sRes[4 g])
+    bool expl = P.n_gen > 0;
+    if (!expl) {
+      eval_walkers<NS, NMO, false, X, false, false, false, 2>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
+      for (int gg = 0; gg < G; ++gg) {
+        const double den = (ws + GE::oProb)[gg * 8 + 3];  // Sigma / D_0 of walker gg (NaN for a singular reference)
+        expl |= !(den * den <= kFallbackOrb);
+      }
+      __syncwarp();
+    }
+    if (expl) {
+      eval_walkers<NS, NMO, false, X, true, false, false, 1>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
+      for (int i = lane; i < G * ne * NMO; i += 32) sGam[i] /= sRes[(i / (ne * NMO)) * 4 + 0];
+      __syncwarp();
+    }
     // second pass over the shells: phi into column lane, d phi / d zeta into column opCol(lane) of the tile
     double *const tile = ws;
     double *const tl = tile + lane, *const tz = tile + GE::opCol(lane);

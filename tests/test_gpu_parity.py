@@ -623,3 +623,59 @@ def test_orbital_derivatives_odd_system(env):
                         a_par=0.25, a_anti=0.5, b=0.8, xyz=(0.1, -0.2, 0.3))
         r = soa(rng.standard_normal((131, 5, 3)) * 1.5)
         check_orbital_derivatives(env, d, r, threads=2)
+
+
+def _classes_system(rng, with_general):
+    """4 up / 3 down electrons in 9 random MOs with every determinant class of the table path: one substitution in
+    one spin, one in each, two in one spin, two in both, and (optionally) a triple, which sends the call down the
+    explicit per-determinant route."""
+    aos = [(1, 0, 0, 2.4), (2, 0, 0, 1.1), (2, 1, 0, 1.3), (2, 1, 1, 1.3), (2, 1, 2, 1.3), (3, 0, 0, 0.8),
+           (3, 1, 1, 0.9), (3, 2, 0, 1.0), (3, 2, 4, 1.0), (3, 2, 2, 0.7), (2, 0, 0, 2.0)]
+    C = rng.standard_normal((len(aos), 9))
+    det_up = [[0, 1, 2, 3], [0, 1, 2, 5], [0, 1, 2, 3], [0, 4, 2, 3], [0, 1, 6, 7], [0, 1, 2, 3], [5, 1, 6, 3],
+              [4, 5, 2, 3], [0, 8, 2, 3]]
+    det_dn = [[0, 1, 2], [0, 1, 2], [0, 1, 6], [0, 5, 2], [0, 1, 2], [4, 1, 8], [0, 4, 7], [3, 1, 5], [7, 1, 2]]
+    ci = [0.8, 0.3, -0.25, 0.2, 0.15, -0.1, 0.12, 0.22, -0.18]
+    if with_general:
+        det_up.append([4, 5, 6, 3]); det_dn.append([0, 1, 3]); ci.append(0.14)
+    return atom_system(4.0, aos, C, 4, 3, det_up=det_up, det_dn=det_dn, ci=ci, a_par=0.25, a_anti=0.5, b=0.9,
+                       xyz=(0.2, 0.1, -0.3))
+
+
+@pytest.mark.parametrize("with_general", [False, True])
+def test_orbital_derivatives_every_determinant_class(env, with_general):
+    rng = np.random.default_rng(77)
+    d = _classes_system(rng, with_general)
+    r = soa(rng.standard_normal((203, 7, 3)) * 1.2 + np.array([0.2, 0.1, -0.3]))
+    check_orbital_derivatives(env, d, r, threads=4)
+
+
+def test_orbital_derivatives_near_singular_reference(env):
+    """Walkers on which the reference determinant all but vanishes (two same-spin electrons at almost the same
+    radius in a reference of s orbitals only) while the excited determinants do not: Sigma/D_0 ~ 1e5, the group
+    is flagged and takes the explicit route; the neighbouring groups stay on the tables."""
+    rng = np.random.default_rng(78)
+    aos = [(1, 0, 0, 2.5), (2, 0, 0, 1.0), (3, 0, 0, 0.7), (2, 1, 0, 1.2), (2, 1, 1, 1.2), (2, 1, 2, 1.2)]
+    C = np.zeros((6, 6))
+    C[:3, :2] = rng.standard_normal((3, 2))          # MOs 0, 1: s only
+    C[:, 2:] = rng.standard_normal((6, 4))
+    d = atom_system(3.0, aos, C, 2, 1, det_up=[[0, 1], [0, 2], [3, 1], [2, 4], [5, 3]], det_dn=[[0], [0], [1], [0], [2]],
+                    ci=[0.7, 0.3, -0.2, 0.25, 0.1], a_par=0.25, a_anti=0.5, b=1.0)
+    r = rng.standard_normal((160, 3, 3)) * 1.3
+    for w in range(0, 160, 3):                        # every third walker: |r_1| = |r_0| (1 + 1e-5 u)
+        u = rng.standard_normal(3)
+        r[w, 1] = u / np.linalg.norm(u) * np.linalg.norm(r[w, 0]) * (1.0 + 1e-5 * rng.uniform(0.5, 1.0))
+    r = soa(r)
+    check_orbital_derivatives(env, d, r, threads=2)
+
+
+def test_orbital_derivatives_are_repeatable_bit_for_bit(env):
+    torch, ob, qb = env
+    d, r = wl.co(M=1031)
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    a = [t.clone() for t in s.orbital_derivatives(rg, d.n_ao, d.n_mo)]
+    for _ in range(3):
+        b = s.orbital_derivatives(rg, d.n_ao, d.n_mo)
+        assert torch.equal(a[0], b[0]) and torch.equal(a[1], b[1])
+    s.close()
