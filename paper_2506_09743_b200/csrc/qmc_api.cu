@@ -100,7 +100,7 @@ struct qmc_system {
   Variant var{};
   int smem_el = 0, smem_psi = 0;  // dynamic shared memory of the E_L kernels (kWarpsEl warps) / values-only kernels
   int blocks_el = 0, blocks_psi = 0, blocks_metro = 0, blocks_expl = 0, blocks_deriv = 0;
-  void *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr, *d_orig = nullptr, *d_rowao = nullptr,
+  void *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr, *d_orig = nullptr, *d_yrec = nullptr, *d_ytgt = nullptr, *d_rowao = nullptr,
        *d_rownrm = nullptr;
   int n_sm = 0;
   double *d_stats = nullptr;
@@ -146,6 +146,8 @@ void qmc_destroy(qmc_system_t *s) {
   cudaFree(s->d_gen);
   cudaFree(s->d_cols);
   cudaFree(s->d_orig);
+  cudaFree(s->d_yrec);
+  cudaFree(s->d_ytgt);
   cudaFree(s->d_rowao);
   cudaFree(s->d_rownrm);
   cudaFree(s->d_stats);
@@ -332,6 +334,8 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   }
   const int NMO = var->NMO;
   std::vector<DetRec> dets(n_packed);
+  std::vector<YRec> yrec;
+  std::vector<int2> ytgt;
   std::vector<GenDet> gens;
   for (int n = n_ref + n_packed; n < d->n_det; ++n) {
     GenDet g{};
@@ -385,6 +389,52 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
         r.dn = code[1];
       }
     }
+    // Gather lists for Y = d(Sigma/D_0)/dT (orbital-parameter derivatives): per table entry (spin, p, q) the
+    // determinants that contain it, as {d_n * cofactor sign, the other spin's sub-determinant code, the cofactor's
+    // table index}; entries sorted by list length so that dealing them to lanes round-robin balances the work.
+    std::vector<std::vector<YRec>> lists_y((size_t)2 * TSv);
+    for (int n = 0; n < n_packed; ++n) {
+      const Exc &x = excs[n_ref + n];
+      uint32_t code[2];
+      for (int sp = 0; sp < 2; ++sp) {
+        uint32_t i11 = one, i12 = zero, i21 = zero, i22 = one;
+        if (x.k[sp] >= 1) i11 = (uint32_t)(x.p[sp][0] * LPv + x.q[sp][0]);
+        if (x.k[sp] == 2) {
+          i12 = (uint32_t)(x.p[sp][0] * LPv + x.q[sp][1]);
+          i21 = (uint32_t)(x.p[sp][1] * LPv + x.q[sp][0]);
+          i22 = (uint32_t)(x.p[sp][1] * LPv + x.q[sp][1]);
+        }
+        code[sp] = i11 | (i12 << 8) | (i21 << 16) | (i22 << 24);
+      }
+      for (int sp = 0; sp < 2; ++sp) {
+        auto add = [&](int p, int q, double w, uint32_t cof) {
+          YRec y{};
+          y.w = w;
+          y.oth = code[1 - sp];
+          y.cof = (uint16_t)cof;
+          lists_y[(size_t)sp * TSv + p * LPv + q].push_back(y);
+        };
+        if (x.k[sp] == 1) {
+          add(x.p[sp][0], x.q[sp][0], x.d, one);
+        } else if (x.k[sp] == 2) {  // cofactors of {T11 T12; T21 T22}
+          const int p0 = x.p[sp][0], p1 = x.p[sp][1], q0 = x.q[sp][0], q1 = x.q[sp][1];
+          add(p0, q0, x.d, (uint32_t)(p1 * LPv + q1));
+          add(p0, q1, -x.d, (uint32_t)(p1 * LPv + q0));
+          add(p1, q0, -x.d, (uint32_t)(p0 * LPv + q1));
+          add(p1, q1, x.d, (uint32_t)(p0 * LPv + q0));
+        }
+      }
+    }
+    std::vector<int> order;
+    for (int t = 0; t < 2 * TSv; ++t)
+      if (!lists_y[t].empty()) order.push_back(t);
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return lists_y[a].size() > lists_y[b].size(); });
+    for (int t : order) {
+      ytgt.push_back(make_int2(t, (int)yrec.size()));
+      yrec.insert(yrec.end(), lists_y[t].begin(), lists_y[t].end());
+    }
+    P.n_ytgt = (int)order.size();
+    ytgt.push_back(make_int2(0, (int)yrec.size()));  // end of the last list
   }
   P.G = std::max(1, std::min(32 / P.n_e, 16 / var->NS));
 
@@ -547,6 +597,10 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
       (e = cudaMemcpy(s->d_cols, cols.data(), cols.size() * sizeof(DetCols), cudaMemcpyHostToDevice)) != cudaSuccess ||
       (e = cudaMalloc(&s->d_orig, det_orig.size() * sizeof(int))) != cudaSuccess ||
       (e = cudaMemcpy(s->d_orig, det_orig.data(), det_orig.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess ||
+      (e = cudaMalloc(&s->d_yrec, std::max<size_t>(yrec.size(), 1) * sizeof(YRec))) != cudaSuccess ||
+      (!yrec.empty() && (e = cudaMemcpy(s->d_yrec, yrec.data(), yrec.size() * sizeof(YRec), cudaMemcpyHostToDevice)) != cudaSuccess) ||
+      (e = cudaMalloc(&s->d_ytgt, ytgt.size() * sizeof(int2))) != cudaSuccess ||
+      (e = cudaMemcpy(s->d_ytgt, ytgt.data(), ytgt.size() * sizeof(int2), cudaMemcpyHostToDevice)) != cudaSuccess ||
       (e = cudaMalloc(&s->d_rowao, row_ao.size() * sizeof(int))) != cudaSuccess ||
       (e = cudaMemcpy(s->d_rowao, row_ao.data(), row_ao.size() * sizeof(int), cudaMemcpyHostToDevice)) != cudaSuccess ||
       (e = cudaMalloc(&s->d_rownrm, row_nrm.size() * sizeof(double))) != cudaSuccess ||
@@ -562,6 +616,8 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   P.gen = (const GenDet *)s->d_gen;
   P.det_cols = (const DetCols *)s->d_cols;
   P.det_orig = (const int *)s->d_orig;
+  P.yrec = (const YRec *)s->d_yrec;
+  P.ytgt = (const int2 *)s->d_ytgt;
   P.ao_orig = (const int *)s->d_rowao;
   P.ao_nrm = (const double *)s->d_rownrm;
   for (int a = 0; a < 16; ++a) P.mo_orig[a] = a < P.n_mo ? used[a] : 0;

@@ -100,6 +100,15 @@ constexpr double kFallbackCap = 1.0e8;
 // derivative (measured); beyond (Sigma/D_0)^2 = 1e4 the group takes the explicit route.
 constexpr double kFallbackOrb = 1.0e4;
 
+// One term of Y[spin][p][q] = d(Sigma/D_0)/dT[p][q]: w * R_other * T_spin[cof]  (w = d_n times the cofactor's sign;
+// oth = the other spin's 2x2 code {i11, i12, i21, i22} as in class-4 DetRec, constant slots for k < 2;
+// cof = table index of the cofactor entry, the constant-1 slot for a single substitution)
+struct __align__(16) YRec {
+  double w;
+  uint32_t oth;
+  uint16_t cof, pad;
+};
+
 struct SysParams {  // passed by value to every kernel
   int n_atoms, n_up, n_dn, n_e;
   int n_shell, n_ao, n_mo, n_det;  // n_shell = records of the shell/atom stream; n_mo = orbitals referenced (kernel
@@ -109,6 +118,9 @@ struct SysParams {  // passed by value to every kernel
   double d_ref;                    // summed coefficients of the determinants equal to the reference
   int n_ref;                       // how many determinants equal the reference
   const int *det_orig;             // device [n_det_all]: caller's index of the determinants in kernel order
+  const YRec *yrec;                // device: gather lists of Y = d(Sigma/D_0)/dT, one list per table entry
+  const int2 *ytgt;                // device [n_ytgt + 1]: {entry index in the walker's (up, down) tables, list start}
+  int n_ytgt;
                                    // (reference-equal ones, then dets[] classes 1-4, then gen[])
   int nv[2];                       // virtual orbitals per spin
   int G;                           // walkers per warp pass

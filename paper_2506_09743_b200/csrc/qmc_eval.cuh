@@ -831,8 +831,9 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
     if (ORB == 2) {
       // ---- Gamma = d ln Sigma / d Phi from the reference alone (lane c of a problem = electron c of that spin):
       //   Gamma_virt[i][q] = sum_p A0^-1[p][i] Y[p][q] / den,   Gamma_occ[i][j] = A0^-1[j][i] - sum_q Gamma_virt[i][q] T[j][q]
-      // Y = d den / d T first, in the layout of the T tables: a second pass over the determinant classes whose adds
-      // run one lane of a walker at a time, in lane order, so that the sums are the same on every run.
+      // Y = d den / d T first, in the layout of the T tables, gathered: each lane of a walker owns table entries and
+      // sums the terms of its entries' lists (built at setup, SysParams::yrec) in list order -- no atomics, no
+      // dependence on scheduling: the same bits on every run.
       static_assert(!(ORB == 2 && EL), "the table-path Gamma is a values-only evaluation");
       double *sY = ws + GE::oY, *sGamF = ws + GE::oGam;
       const double *sInvF = ws + GE::oInv;
@@ -840,62 +841,23 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       for (int i = lane; i < GE::ROWS * NMO; i += 32) sGamF[i] = 0.0;
       if (wvalid && sub == 0) sProb[pu * 4 + 3] = den;
       __syncwarp();
-      double *Yw = sY + pu * TS;  // this walker's Y (up spin, then down)
-      for (int n0 = 0; n0 < P.n_det; n0 += LW) {
-        const int n = n0 + sub;
-        const bool act = wvalid && n < P.n_det;
-        int yi[8];
-        double yv[8];
-        int ny = 0;
-        if (act) {
-          const DetRec dr = sDet[n];
-          double D;
-          if (n < P.n_a1) {
-            yi[0] = dr.up >> 3; yv[0] = dr.d; ny = 1;
-          } else if (n < P.n_a2) {
-            double Ru, Rd;
-            entry(dr.up, Ru, D);
-            entry(dr.dn, Rd, D);
-            yi[0] = dr.up >> 3; yv[0] = dr.d * Rd;
-            yi[1] = dr.dn >> 3; yv[1] = dr.d * Ru;
-            ny = 2;
-          } else if (n < P.n_b) {  // cofactors of the 2x2 block {a b; c d}
-            double a, b, c2, d;
-            entry(dr.up & 0xffffu, a, D);
-            entry(dr.up >> 16, b, D);
-            entry(dr.dn & 0xffffu, c2, D);
-            entry(dr.dn >> 16, d, D);
-            yi[0] = (dr.up & 0xffffu) >> 3; yv[0] = dr.d * d;
-            yi[1] = dr.up >> 19; yv[1] = -dr.d * c2;
-            yi[2] = (dr.dn & 0xffffu) >> 3; yv[2] = -dr.d * b;
-            yi[3] = dr.dn >> 19; yv[3] = dr.d * a;
-            ny = 4;
-          } else {  // per spin: cofactors of {T11 T12; T21 T22} times the other spin's R; the constant slots carry no Y
-            double Ru, Rd;
-            excite_double<false>(dr.up, Tu, Ru, D);
-            excite_double<false>(dr.dn, Td, Rd, D);
-#pragma unroll
-            for (int sp2 = 0; sp2 < 2; ++sp2) {
-              const uint32_t ix = sp2 ? dr.dn : dr.up;
-              const double *Tt = sp2 ? Td : Tu;
-              const double wo = dr.d * (sp2 ? Ru : Rd);
-              const int i11 = ix & 255, i12 = (ix >> 8) & 255, i21 = (ix >> 16) & 255, i22 = ix >> 24;
-              yi[4 * sp2 + 0] = sp2 * TS + i11; yv[4 * sp2 + 0] = wo * Tt[i22];
-              yi[4 * sp2 + 1] = sp2 * TS + i22; yv[4 * sp2 + 1] = wo * Tt[i11];
-              yi[4 * sp2 + 2] = sp2 * TS + i12; yv[4 * sp2 + 2] = -wo * Tt[i21];
-              yi[4 * sp2 + 3] = sp2 * TS + i21; yv[4 * sp2 + 3] = -wo * Tt[i12];
-            }
-            ny = 8;
+      if (wvalid)
+        for (int t = sub; t < P.n_ytgt; t += LW) {
+          const int2 tg = __ldg(P.ytgt + t);
+          const int end = __ldg(P.ytgt + t + 1).y;
+          const bool dnT = tg.x >= TS;
+          const double *Ts = dnT ? Td : Tu, *To = dnT ? Tu : Td;
+          double acc = 0.0;
+          for (int k = tg.y; k < end; ++k) {
+            const uint4 raw = __ldg(reinterpret_cast<const uint4 *>(P.yrec + k));
+            const double w = __hiloint2double((int)raw.y, (int)raw.x);
+            const uint32_t ix = raw.z;
+            const double Ro = fma(To[ix & 255], To[ix >> 24], -To[(ix >> 8) & 255] * To[(ix >> 16) & 255]);
+            acc = fma(w * Ro, Ts[raw.w & 0xffffu], acc);
           }
+          sY[pu * TS + tg.x] = acc;
         }
-        for (int t = 0; t < LW; ++t) {
-          if (act && sub == t)
-#pragma unroll
-            for (int k = 0; k < 8; ++k)
-              if (k < ny) Yw[yi[k]] += yv[k];   // slots NS*RS, NS*RS+1 of a table collect the constants' share: never read
-          __syncwarp();
-        }
-      }
+      __syncwarp();
       const int c = lane % LP, slot = lane / LP;
       for (int pass = 0; pass * PP < 2 * G; ++pass) {
         const int pr = pass * PP + slot;

@@ -273,34 +273,42 @@ __global__ void __launch_bounds__(WPB * 32, 1)
         __syncwarp();
         // kernel-order (N C)[R][col] from the DMMA B-fragment table: [chunk][k-step][MO tile][4 n + k]
         const double *cfr = sC + chunk * ((kChunk / 4) * NT * 32);
-        if (dC)
-          for (int idx = lane; idx < G * kChunk * NMO; idx += 32) {
-            const int gg = idx / (kChunk * NMO), rem = idx - gg * (kChunk * NMO), rw = rem / NMO, col = rem - rw * NMO;
+        // lane <-> (walker gg, MO column): Gamma's column in registers, the tile rows read as broadcasts;
+        // dzeta sums its columns across the NMO lanes of a walker
+        constexpr int CW = NMO <= 2 ? 2 : (NMO <= 4 ? 4 : (NMO <= 8 ? 8 : 16));  // aligned power-of-two lane block per walker
+        static_assert(NMO <= CW, "at most 16 MO columns");
+        for (int pi = lane; pi < ((G * CW + 31) & ~31); pi += 32) {
+          const int gq = pi / CW, col = pi & (CW - 1);
+          const bool pv = gq < G && col < NMO;
+          const int gg = pv ? gq : 0;
+          const int64_t wo = grp * G + gg;
+          const bool ok = pv && col < P.n_mo && wo < io.M;
+          double gam[2 * NS];
+#pragma unroll
+          for (int i = 0; i < 2 * NS; ++i) gam[i] = (pv && i < ne) ? sGam[(gg * ne + i) * NMO + col] : 0.0;
+          const int64_t orow = wo * P.n_ao;
+          const int ocol = P.mo_orig[col < NMO ? col : 0];
+          for (int rw = 0; rw < kChunk; ++rw) {
             const int R = chunk * kChunk + rw, beta = P.ao_orig[R];
-            const int64_t wo = grp * G + gg;
-            if (beta >= 0 && col < P.n_mo && wo < io.M) {
-              double t = 0.0;
-              for (int i = 0; i < ne; ++i) t = fma(tile[rw * S + gg * ne + i], sGam[(gg * ne + i) * NMO + col], t);
-              dC[(wo * P.n_ao + beta) * P.n_mo_all + P.mo_orig[col]] = P.ao_nrm[R] * t;
-            }
-          }
-        if (dZ)
-          for (int idx = lane; idx < G * kChunk; idx += 32) {
-            const int gg = idx / kChunk, rw = idx - gg * kChunk;
-            const int R = chunk * kChunk + rw, beta = P.ao_orig[R];
-            const int64_t wo = grp * G + gg;
-            if (beta >= 0 && wo < io.M) {
-              double acc = 0.0;
-              for (int col = 0; col < P.n_mo; ++col) {
-                double t = 0.0;
-                for (int i = 0; i < ne; ++i)
-                  t = fma(tile[rw * S + GE::opCol(gg * ne + i)], sGam[(gg * ne + i) * NMO + col], t);
-                const double nc = cfr[(((rw >> 2) * NT) + (col >> 3)) * 32 + 4 * (col & 7) + (rw & 3)];
-                acc = fma(nc, t, acc);
+            if (beta < 0) continue;
+            const double *trow = tile + rw * S;
+            double t = 0.0, u = 0.0;
+#pragma unroll
+            for (int i = 0; i < 2 * NS; ++i)
+              if (i < ne) {
+                t = fma(trow[gg * ne + i], gam[i], t);
+                u = fma(trow[GE::opCol(gg * ne + i)], gam[i], u);
               }
-              dZ[wo * P.n_ao + beta] = acc;
+            if (dC && ok) dC[(orow + beta) * P.n_mo_all + ocol] = P.ao_nrm[R] * t;
+            if (dZ) {
+              // kernel-order (N C)[R][col] from the DMMA B-fragment table
+              double a = ok ? cfr[(((rw >> 2) * NT) + (col >> 3)) * 32 + 4 * (col & 7) + (rw & 3)] * u : 0.0;
+#pragma unroll
+              for (int m = 1; m < CW; m <<= 1) a += shfl_xor_d(a, m);
+              if (pv && col == 0 && wo < io.M) dZ[orow + beta] = a;
             }
           }
+        }
         __syncwarp();
         ++chunk;
       }
