@@ -602,7 +602,7 @@ void oracle_batch_stats(const double *x, int64_t M, double *mean, double *stderr
 
 int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                            int64_t w1, double *O) {
-  int ne = s->n_up + s->n_dn, nmo = s->n_mo, np = 6 + s->n_det;
+  int ne = s->n_up + s->n_dn, nmo = s->n_mo, nj = 6 + 7 * s->n_een, np = nj + s->n_det;
   double *mo = (double *)malloc(sizeof(double) * (size_t)(ne * nmo + 1));
   double *A = (double *)malloc(sizeof(double) * (size_t)(ne * ne + 1));
   double *pos = (double *)malloc(sizeof(double) * (size_t)(3 * ne + 1));
@@ -643,6 +643,36 @@ int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64
     out[3] = dw0;
     out[4] = dw1;
     out[5] = dw2;
+    /* electron-electron-nucleus kernel (D.3; reading Q22: ordered pairs i != j, every nucleus):
+     * term mu = c f(r_ai) g(r_aj) h(r_ij) with Pade factors p(r) = a r / (1 + b r):
+     * dp/da = r / (1 + b r),  dp/db = -a r^2 / (1 + b r)^2.  Seven parameters per term, in the order of
+     * een_params: c, a_f, b_f, a_g, b_g, a_h, b_h. */
+    for (int mu = 0; mu < s->n_een; ++mu) {
+      const double *q = s->een_params + 7 * mu;
+      double dq[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+      for (int at = 0; at < s->n_atoms; ++at)
+        for (int i = 0; i < ne; ++i)
+          for (int j = 0; j < ne; ++j) {
+            if (i == j) continue;
+            double xi = pos[3 * i] - s->atom_xyz[3 * at], yi = pos[3 * i + 1] - s->atom_xyz[3 * at + 1],
+                   zi = pos[3 * i + 2] - s->atom_xyz[3 * at + 2];
+            double xj = pos[3 * j] - s->atom_xyz[3 * at], yj = pos[3 * j + 1] - s->atom_xyz[3 * at + 1],
+                   zj = pos[3 * j + 2] - s->atom_xyz[3 * at + 2];
+            double xx = pos[3 * i] - pos[3 * j], yy = pos[3 * i + 1] - pos[3 * j + 1], zz = pos[3 * i + 2] - pos[3 * j + 2];
+            double rai = sqrt(xi * xi + yi * yi + zi * zi), raj = sqrt(xj * xj + yj * yj + zj * zj);
+            double rij = sqrt(xx * xx + yy * yy + zz * zz);
+            double Df = 1.0 + q[2] * rai, Dg = 1.0 + q[4] * raj, Dh = 1.0 + q[6] * rij;
+            double f = q[1] * rai / Df, g = q[3] * raj / Dg, h = q[5] * rij / Dh;
+            dq[0] += f * g * h;
+            dq[1] += q[0] * (rai / Df) * g * h;
+            dq[2] += q[0] * (-q[1] * rai * rai / (Df * Df)) * g * h;
+            dq[3] += q[0] * f * (raj / Dg) * h;
+            dq[4] += q[0] * f * (-q[3] * raj * raj / (Dg * Dg)) * h;
+            dq[5] += q[0] * f * g * (rij / Dh);
+            dq[6] += q[0] * f * g * (-q[5] * rij * rij / (Dh * Dh));
+          }
+      for (int k = 0; k < 7; ++k) out[6 + 7 * mu + k] = dq[k];
+    }
     /* CI: Sigma = sum_n d_n D_n^up D_n^dn  (eq. 4):  d ln Sigma / d d_n = D_n^up D_n^dn / Sigma */
     for (int i = 0; i < ne * nmo; ++i) mo[i] = 0.0;
     for (int i = 0; i < ne; ++i)
@@ -663,7 +693,7 @@ int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64
       prod[n] = D[0] * D[1];
       sigma += s->ci_coeff[n] * prod[n];
     }
-    for (int n = 0; n < s->n_det; ++n) out[6 + n] = prod[n] / sigma;
+    for (int n = 0; n < s->n_det; ++n) out[nj + n] = prod[n] / sigma;
   }
   free(mo); free(A); free(pos); free(prod);
   return 0;

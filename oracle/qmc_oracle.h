@@ -98,8 +98,9 @@ void oracle_batch_stats(const double *x, int64_t M, double *mean, double *stderr
 
 /* Logarithmic derivatives O_p(r) = (d Psi / d theta_p) / Psi, the factor of eq. 6
  * (PAPER.md:78), for theta = (jastrow_a_par, jastrow_a_anti, jastrow_b, jastrow_en_w0, jastrow_en_w1,
- * jastrow_en_w2, d_0 .. d_{n_det-1}) in that order; O is [M][6 + n_det] row-major, rows w0 <= w < w1
- * are written.
+ * jastrow_en_w2, then the seven parameters c, a_f, b_f, a_g, b_g, a_h, b_h of every e-e-n term (D.3,
+ * PAPER.md:251) in een_params order, then d_0 .. d_{n_det-1}); O is [M][6 + 7 n_een + n_det] row-major,
+ * rows w0 <= w < w1 are written.
  * Psi = e^J Sigma (eq. 4), so d ln Psi / d(Jastrow parameter) is the
  * parameter derivative of D.1 summed over pairs, and
  * d ln Psi / d d_n = D_n^up D_n^dn / Sigma, every determinant factored explicitly. */

@@ -771,6 +771,56 @@ def test_een_jastrow_absent_without_terms():
     assert np.max(np.abs(c[2] - a[2])) > 1e-3
 
 
+def test_een_parameter_derivatives_vs_central_differences_closed_form_and_layout():
+    # O_p for the 7 n_een parameters of D.3 sit between the six D.1/D.2 parameters and the CI coefficients;
+    # pinned by Richardson central differences of the oracle's own log|Psi| in EVERY such parameter, by the
+    # two-electron closed form, and by Euler's identity for the coefficient c (the term is linear in it)
+    for name, M in (("LiH", 6), ("CO", 3)):
+        d, r = wl.CONFIGS[name](M=M)
+        d = _with_een(_with_en(d, 0.2, -0.03, 0.8))
+        O = ob.log_derivatives(ob.OracleSystem(d), r)
+        n_een = EEN.shape[0]
+        assert O.shape == (M, NJ + 7 * n_een + len(d.ci_coeff))
+        for mu in range(n_een):
+            for k in range(7):
+                t0 = EEN[mu, k]
+
+                def cd(h):
+                    out = []
+                    for sgn in (1.0, -1.0):
+                        e2 = EEN.copy()
+                        e2[mu, k] = t0 + sgn * h
+                        out.append(ob.local_energy(ob.OracleSystem(_with_een(d, e2)), r)[0])
+                    return (out[0] - out[1]) / (2 * h)
+
+                h = 1e-3 * max(1.0, abs(t0))
+                fd = (4 * cd(h / 2) - cd(h)) / 3
+                col = O[:, NJ + 7 * mu + k]
+                assert np.max(np.abs(col - fd) / np.maximum(1, np.abs(fd))) < 1e-7, (name, mu, k)
+        # CI block moved behind the D.3 block, unchanged: sum rule
+        assert np.max(np.abs(O[:, NJ + 7 * n_een:] @ np.asarray(d.ci_coeff) - 1.0)) < 1e-10
+        # the first six columns do not depend on the D.3 terms
+        O0 = ob.log_derivatives(ob.OracleSystem(_with_een(d, np.zeros((0, 7)))), r)
+        assert np.array_equal(O0[:, :NJ], O[:, :NJ]) and O0.shape[1] == NJ + len(d.ci_coeff)
+    # two electrons, one nucleus: J_een = sum_mu c [f(r1) g(r2) + f(r2) g(r1)] h(r12)
+    d0 = _with_een(atom_system(2.0, [(1, 0, 0, 1.7)], [[1.0]], 1, 1, a_par=0.25, a_anti=0.5, b=0.9))
+    rr = _rand_pos(40, 2, 1.2, rmin=0.05, seed=92)
+    O = ob.log_derivatives(ob.OracleSystem(d0), soa(rr))
+    r1, r2 = np.linalg.norm(rr[:, 0], axis=1), np.linalg.norm(rr[:, 1], axis=1)
+    r12 = np.linalg.norm(rr[:, 0] - rr[:, 1], axis=1)
+    pade = lambda a, b, x: a * x / (1 + b * x)
+    da = lambda a, b, x: x / (1 + b * x)
+    db = lambda a, b, x: -a * x * x / (1 + b * x) ** 2
+    for mu, (c, a1, b1, a2, b2, a3, b3) in enumerate(EEN):
+        f1, f2, g1, g2, hh = pade(a1, b1, r1), pade(a1, b1, r2), pade(a2, b2, r1), pade(a2, b2, r2), pade(a3, b3, r12)
+        want = [(f1 * g2 + f2 * g1) * hh,
+                c * (da(a1, b1, r1) * g2 + da(a1, b1, r2) * g1) * hh, c * (db(a1, b1, r1) * g2 + db(a1, b1, r2) * g1) * hh,
+                c * (f1 * da(a2, b2, r2) + f2 * da(a2, b2, r1)) * hh, c * (f1 * db(a2, b2, r2) + f2 * db(a2, b2, r1)) * hh,
+                c * (f1 * g2 + f2 * g1) * da(a3, b3, r12), c * (f1 * g2 + f2 * g1) * db(a3, b3, r12)]
+        for k in range(7):
+            assert np.max(np.abs(O[:, NJ + 7 * mu + k] - want[k])) < 1e-13, (mu, k)
+
+
 # ---------------------------------------------------------------- orbital parameters (AO exponents, MO coefficients)
 @pytest.mark.parametrize("name,M", [("H2", 6), ("LiH", 5), ("Li2", 3), ("CO", 2)])
 def test_orbital_derivatives_vs_central_differences_of_log_psi(name, M):
