@@ -232,7 +232,7 @@ def main():
     clocks = sampler.stop()
 
     # ---- E_L + parameter derivatives O (eq. 6 factors) and the gradient estimator,
-    # reported beside the headline (same walkers; O is [M][6 + n_det] doubles written to and read from HBM)
+    # reported beside the headline (same walkers; O is [M][n_param = 6 + n_det] doubles written to and read from HBM)
     n_par = sysh.n_param()
     O = torch.empty((M, n_par), dtype=torch.float64, device=dev)
     t_d = t_g = 0.0

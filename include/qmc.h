@@ -167,13 +167,14 @@ int qmc_batch_stats(const double *d_x, int64_t M, double *h_mean, double *h_stde
 
 /* ---- the factors of the gradient estimator, eq. 6 ----
  * Variational parameters handled: theta = (jastrow_a_par, jastrow_a_anti, jastrow_b, jastrow_en_w0,
- * jastrow_en_w1, jastrow_en_w2, d_0 .. d_{n_det-1}) in that order, n_param = 6 + n_det (qmc_n_param).
+ * jastrow_en_w1, jastrow_en_w2, then the seven parameters c, a_f, b_f, a_g, b_g, a_h, b_h of every e-e-n term in
+ * een_params order (D.3), then d_0 .. d_{n_det-1}); n_param = 6 + 7 n_een + n_det (qmc_n_param).
  * The MO and AO parameters (mu, zeta of PAPER.md:55-57) have their own call, qmc_orbital_derivatives. */
 int qmc_n_param(const qmc_system_t *s);
 
 /* qmc_local_energy plus the logarithmic derivatives O_p(r) = (dPsi/dtheta_p)/Psi:
  *   d_O device, out: double [M][n_param] row-major (required)
- * Psi = e^J Sigma (eq. 4): O for a Jastrow parameter is dJ/dtheta from D.1 / D.2,
+ * Psi = e^J Sigma (eq. 4): O for a Jastrow parameter is dJ/dtheta from D.1 / D.2 / D.3,
  * O for d_n is D_n^up D_n^dn / Sigma, formed from the excitation tables of the same launch.
  * d_logpsi / d_sign / d_eloc as in qmc_local_energy (E_L carries the explicit fallback
  * correction; O comes from the table path, whose relative error for a nearly singular

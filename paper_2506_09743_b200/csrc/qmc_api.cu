@@ -834,7 +834,7 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
   return QMC_OK;
 }
 
-int qmc_n_param(const qmc_system_t *s) { return s ? kJastrowParams + s->P.n_det_all : QMC_EINVAL; }
+int qmc_n_param(const qmc_system_t *s) { return s ? kJastrowParams + 7 * s->P.n_een + s->P.n_det_all : QMC_EINVAL; }
 
 int qmc_log_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, double *d_eloc,
                         double *d_O, void *cuda_stream) {

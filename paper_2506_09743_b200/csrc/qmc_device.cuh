@@ -162,12 +162,13 @@ struct WalkerIO {
   const double *r_in;  // [n_e][3][M]
   double *r_out;       // Metropolis: same buffer
   double *logpsi, *sign, *eloc;
-  double *O;           // device [M][kJastrowParams + n_det_all] parameter derivatives (DerivOut), or null
+  double *O;           // device [M][kJastrowParams + 7 n_een + n_det_all] parameter derivatives (DerivOut), or null
   int64_t M;
 };
 
 // Parameter-derivative output (eq. 6): O[w][p] = (dPsi/dtheta_p)/Psi for
-// theta = (a_par, a_anti, b, en_w0, en_w1, en_w2, d_0 .. d_{n_det-1}); row-major [M][kJastrowParams + n_det_all].
+// theta = (a_par, a_anti, b, en_w0, en_w1, en_w2, {c, a_f, b_f, a_g, b_g, a_h, b_h} of every e-e-n term,
+// d_0 .. d_{n_det-1}); row-major [M][kJastrowParams + 7 n_een + n_det_all].
 constexpr int kJastrowParams = 6;
 struct DerivOut {
   double *O;      // device, or null

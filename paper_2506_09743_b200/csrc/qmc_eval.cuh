@@ -168,6 +168,51 @@ __device__ __noinline__ void een_terms(const SysParams &P, const double *sXYZ, i
   out[4] = lap;
 }
 
+// Parameter derivatives of the e-e-n kernel (eq. 6 factors of D.3): for the lane's electron i and term mu the sums over
+// nuclei a and partners j != i (the ordered pairs that start at i) of d(c f(r_ai) g(r_aj) h(r_ij))/d(c, a_f, b_f, a_g,
+// b_g, a_h, b_h), with p = a r/(1 + b r): dp/da = r/(1 + b r) =: P, dp/db = -a r^2/(1 + b r)^2 = -p P.  Out of line.
+__device__ __noinline__ void een_param_terms(const SysParams &P, const double *sXYZ, int base, int ne, int e, double x,
+                                             double y, double z, int mu, double *dq) {
+  const double q0 = P.een[mu][0], q1 = P.een[mu][1], q2 = P.een[mu][2], q3 = P.een[mu][3], q4 = P.een[mu][4],
+               q5 = P.een[mu][5], q6 = P.een[mu][6];
+  double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0, s4 = 0.0, s5 = 0.0, s6 = 0.0;
+  for (int at = 0; at < P.n_atoms; ++at) {
+    const double ax = P.atom[at][0], ay = P.atom[at][1], az = P.atom[at][2];
+    const double aix = x - ax, aiy = y - ay, aiz = z - az;
+    const double rai2 = fma(aix, aix, fma(aiy, aiy, aiz * aiz));
+    const double rai = rai2 * rsqrt_fast(rai2);
+    const double Pf = rai * rcp_fast(fma(q2, rai, 1.0)), f = q1 * Pf, fb = -f * Pf;
+    for (int o = 1; o < ne; ++o) {
+      int j = e + o;
+      j -= (j >= ne) ? ne : 0;
+      const double xj = sXYZ[base + j], yj = sXYZ[32 + base + j], zj = sXYZ[64 + base + j];
+      const double ijx = x - xj, ijy = y - yj, ijz = z - zj;
+      const double rij2 = fma(ijx, ijx, fma(ijy, ijy, ijz * ijz));
+      const double rij = rij2 * rsqrt_fast(rij2);
+      const double ajx = xj - ax, ajy = yj - ay, ajz = zj - az;
+      const double raj2 = fma(ajx, ajx, fma(ajy, ajy, ajz * ajz));
+      const double raj = raj2 * rsqrt_fast(raj2);
+      const double Pg = raj * rcp_fast(fma(q4, raj, 1.0)), gv = q3 * Pg, gb = -gv * Pg;
+      const double Ph = rij * rcp_fast(fma(q6, rij, 1.0)), h = q5 * Ph, hb = -h * Ph;
+      const double gh = gv * h, fg = f * gv;
+      s0 = fma(f, gh, s0);
+      s1 = fma(Pf, gh, s1);
+      s2 = fma(fb, gh, s2);
+      s3 = fma(f * Pg, h, s3);
+      s4 = fma(f * gb, h, s4);
+      s5 = fma(fg, Ph, s5);
+      s6 = fma(fg, hb, s6);
+    }
+  }
+  dq[0] = s0;
+  dq[1] = q0 * s1;
+  dq[2] = q0 * s2;
+  dq[3] = q0 * s3;
+  dq[4] = q0 * s4;
+  dq[5] = q0 * s5;
+  dq[6] = q0 * s6;
+}
+
 // ---------------------------------------------------------------------------------
 // Evaluate the G walkers of this warp.  Lane = g * n_e + e holds electron e of walker g
 // at (x, y, z).  Results for walker g are left in ws[oRes + 4 g + {0,1,2}] =
@@ -896,7 +941,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       // (D_n / D_0 over Sigma / D_0), a second, values-only pass over the determinant classes.
       const int64_t wo = dv.w0 + wg;
       if (wvalid && wo < dv.M && dv.O) {
-        const int np = kJastrowParams + P.n_det_all;
+        const int np = kJastrowParams + 7 * P.n_een + P.n_det_all;
         double *row = dv.O + wo * np;
         for (int k = sub; k < 3; k += LW) {
           double t = 0.0;
@@ -911,7 +956,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       sXYZ[lane * 3 + 2] = dEn2;
       __syncwarp();
       if (wvalid && wo < dv.M && dv.O) {
-        const int np = kJastrowParams + P.n_det_all;
+        const int np = kJastrowParams + 7 * P.n_een + P.n_det_all;
         double *row = dv.O + wo * np;
         for (int k = sub; k < 3; k += LW) {
           double t = 0.0;
@@ -920,7 +965,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
         }
         const double iden = 1.0 / den;
         const int *orig = P.det_orig;
-        double *rowd = row + kJastrowParams;
+        double *rowd = row + kJastrowParams + 7 * P.n_een;
         for (int n = sub; n < P.n_ref; n += LW) rowd[orig[n]] = iden;
         orig += P.n_ref;
         const char *Tb = reinterpret_cast<const char *>(Tu);
@@ -946,6 +991,32 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           excite_general<EL>(&P.gen[n].s[0], Tu, RS, u);
           excite_general<EL>(&P.gen[n].s[1], Td, RS, v);
           rowd[orig[n]] = u[0] * v[0] * iden;
+        }
+      }
+      if (EEN) {
+        // the seven parameters of every e-e-n term: coordinates back into the scratch, each lane its electron's
+        // ordered pairs, then the walker's electrons summed in lane order
+        __syncwarp();
+        sXYZ[lane] = x;
+        sXYZ[32 + lane] = y;
+        sXYZ[64 + lane] = z;
+        __syncwarp();
+        const int base = active ? g * ne : 0, ee = active ? e : 0;
+        const int64_t wo2 = dv.w0 + g;
+        for (int mu = 0; mu < P.n_een; ++mu) {
+          double dq[7];
+          een_param_terms(P, sXYZ, base, ne, ee, x, y, z, mu, dq);
+#pragma unroll
+          for (int k = 0; k < 7; ++k) {
+            double t = 0.0;
+            for (int j = 0; j < ne; ++j) t += shfl_d(dq[k], base + j, 32);
+            dq[k] = t;
+          }
+          if (active && e == 0 && wo2 < dv.M && dv.O) {
+            double *row = dv.O + wo2 * (kJastrowParams + 7 * P.n_een + P.n_det_all) + kJastrowParams + 7 * mu;
+#pragma unroll
+            for (int k = 0; k < 7; ++k) row[k] = dq[k];
+          }
         }
       }
     }

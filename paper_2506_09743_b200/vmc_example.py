@@ -22,7 +22,7 @@ import torch
 from . import binding as qb
 from . import workloads as wl
 
-N_JASTROW = 6  # (a_par, a_anti, b, en_w0, en_w1, en_w2) precede the CI coefficients in theta
+N_JASTROW = 6  # (a_par, a_anti, b, en_w0, en_w1, en_w2) precede the CI coefficients in theta (no e-e-n terms here)
 
 
 def get_theta(d):

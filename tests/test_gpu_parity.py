@@ -361,7 +361,7 @@ def check_log_derivatives(env, d, r, threads=8):
     err = np.abs(On - O0) / np.maximum(1.0, np.abs(O0))
     assert np.max(err[keep]) < 1e-8, (np.max(err[keep]), np.unravel_index(np.argmax(err * keep[:, None]), err.shape))
     # sum rule on the GPU result itself
-    assert np.max(np.abs(On[keep, 6:] @ np.asarray(d.ci_coeff) - 1.0)) < 1e-9
+    assert np.max(np.abs(On[keep, On.shape[1] - len(d.ci_coeff):] @ np.asarray(d.ci_coeff) - 1.0)) < 1e-9
     # estimator: the oracle's reduction applied to the oracle's E_L and O
     ev0, g0 = ob.energy_gradient(el0, O0)
     scale = 2.0 * np.mean(np.abs(O0) * np.abs(el0 - ev0)[:, None], axis=0)
@@ -539,7 +539,22 @@ def test_een_jastrow_three_atoms_unequal_spins_and_limits(env):
     assert qb.lib().qmc_setup(C.addressof(desc), 0, C.byref(h)) == qb.QMC_EUNSUPPORTED
 
 
-# ----------------------------------------------------------------------------- the pieces together: a VMC loop
+@pytest.mark.parametrize("name,M", [("H2", 515), ("LiH", 300), ("Li2", 259), ("CO", 130)])
+def test_log_derivatives_with_een_terms(env, name, M):
+    """O_p in the seven parameters of every e-e-n term (D.3), between the D.1/D.2 block and the CI block."""
+    d, r = wl.CONFIGS[name](M=M)
+    d = _with_een(_with_en(d, 0.2, -0.03, 0.8))
+    check_log_derivatives(env, d, r)
+
+
+def test_log_derivatives_with_one_and_six_een_terms(env):
+    d, r = wl.lih(M=64)
+    d1 = _with_een(_with_en(d, 0.1, 0.02, 1.1), EEN[:1])
+    check_log_derivatives(env, d1, r, threads=2)
+    d6 = _with_een(d1, np.concatenate([EEN, 0.5 * EEN[:1]]))   # the maximum of six terms
+    check_log_derivatives(env, d6, r, threads=2)
+
+
 def test_vmc_example_gradient_descent_lowers_the_h2_energy(env):
     # eq. 6 end to end on the GPU path (sampler -> E_L + O_p -> estimator -> parameter step -> new handle): for the H2
     # configuration, switching on the electron-nucleus kernel by gradient descent lowers the variational energy by
