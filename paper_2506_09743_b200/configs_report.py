@@ -55,11 +55,19 @@ def measure(name, d, r_host, peak):
 
     t_cp = _time(lambda: r.copy_(r0))
     t_met = _time(met) - t_cp
+    # E_L + O_p (eq. 6 factors) and the orbital-parameter derivatives, on at most 32768 walkers
+    Md = min(M, 32768)
+    rd = r[:, :, :Md].contiguous()
+    O = torch.empty((Md, s.n_param()), dtype=torch.float64, device="cuda")
+    t_el_d = _time(lambda: s.local_energy(rd))
+    t_O = _time(lambda: s.log_derivatives(rd, O=O))
+    t_orb = _time(lambda: s.orbital_derivatives(rd, d.n_ao, d.n_mo))
     f_el, f_st = s.model_flops(0), s.model_flops(1)
-    row = dict(config=name, n_e=d.n_e, n_ao=d.n_ao, n_det=d.n_det, walkers=M, el_ms=1e3 * t_el, el_rate=M / t_el,
+    row = dict(config=name, n_e=d.n_e, n_ao=d.n_ao, n_mo=d.n_mo, n_det=d.n_det, walkers=M, el_ms=1e3 * t_el, el_rate=M / t_el,
                el_tflops=f_el * M / t_el / 1e12, el_frac=f_el * M / t_el / 1e12 / peak, sweeps=sweeps,
                met_ms=1e3 * t_met, met_rate=M * sweeps / t_met, met_tflops=f_st * M * sweeps / t_met / 1e12,
-               met_frac=f_st * M * sweeps / t_met / 1e12 / peak)
+               met_frac=f_st * M * sweeps / t_met / 1e12 / peak, deriv_walkers=Md, n_param=s.n_param(),
+               el_d_ms=1e3 * t_el_d, O_ms=1e3 * t_O, orb_ms=1e3 * t_orb)
     s.close()
     return row
 
@@ -105,6 +113,12 @@ def main():
         print(f"| {x['config']} | {x['n_e']} | {x['n_ao']} | {x['n_det']} | {x['walkers']} | {x['el_ms']:.3f} | "
               f"{x['el_rate'] / 1e6:.1f} | {x['el_tflops']:.2f} | {100 * x['el_frac']:.1f} % | {x['sweeps']} | "
               f"{x['met_ms']:.3f} | {x['met_rate'] / 1e6:.1f} | {x['met_tflops']:.2f} | {100 * x['met_frac']:.1f} % |")
+    print("\nParameter derivatives (eq. 6 factors), same sampled walkers, device time per call:")
+    print("| config | walkers | E_L ms | n_param | E_L + O_p ms | orbital parameters (N_AO x N_MO + N_AO) | dC, dzeta ms |")
+    print("|---|---|---|---|---|---|---|")
+    for x in rows:
+        print(f"| {x['config']} | {x['deriv_walkers']} | {x['el_d_ms']:.3f} | {x['n_param']} | {x['O_ms']:.3f} | "
+              f"{x['n_ao']} x {x['n_mo']} + {x['n_ao']} | {x['orb_ms']:.3f} |")
     if args.scan_geometries > 0:
         geo, t_total = scan(args.scan_geometries, peak)
         print(f"\nCO scan (500 determinants, {geo[0]['walkers']} walkers per geometry, {geo[0]['sweeps']} sweeps + E_L on every "
