@@ -249,6 +249,19 @@ def main():
             t_d += a.elapsed_time(b) * 1e-3
             t_g += b.elapsed_time(c) * 1e-3
     del O
+    # orbital-parameter derivatives (MO coefficients, AO exponents) on the first 32768 walkers of the batch
+    M_orb = min(M, 32768)
+    r_orb = r[:, :, :M_orb].contiguous()
+    t_o = 0.0
+    for k in range(3 + K_DERIV):
+        a, b = ev(), ev()
+        a.record(st)
+        dC, dz = sysh.orbital_derivatives(r_orb, d.n_ao, d.n_mo)
+        b.record(st)
+        torch.cuda.synchronize()
+        if k >= 3:
+            t_o += a.elapsed_time(b) * 1e-3
+    del dC, dz, r_orb
 
     t_met, t_el, t_all, t_e2e = max_over_ranks([t_met, t_el, t_all, t_e2e], device=dev)
 
@@ -297,6 +310,9 @@ def main():
                                 "gradient_hbm_gbs": int(M) * (n_par + 1) * 8 / (t_g / K_DERIV) / 1e9,
                                 "E_v": e_v, "grad_norm": float(np.linalg.norm(grad)),
                                 "note": "SURVEY 8(f) NEXT-1, eq. 6; gradient time includes batch stats, the D2H of the result and a stream synchronise"},
+            "orbital_derivatives": {"walkers": int(M_orb), "outputs_per_walker": int(d.n_ao * d.n_mo + d.n_ao),
+                                    "ms": 1e3 * t_o / K_DERIV,
+                                    "note": "SURVEY 8(f) NEXT-1: d ln Psi / d C and d ln Psi / d zeta per walker"},
             "gpu_launches": int(launches),
             "clocks": clocks,
             "last_step": {"mean_E_L": mean, "stderr": err},

@@ -8,7 +8,9 @@ derivatives O_p with qmc_log_derivatives, form the gradient estimator with qmc_e
 gradient-descent step on the selected parameters and rebuild the handle (a qmc_system_t is immutable).  The paper
 optimises with ADAM through PyTorch autograd; the optimiser is not part of the hot path, so this example keeps the
 simplest one.  Optimised here: the Pade e-e parameter b and the three electron-nucleus parameters (the cusp
-values a_par, a_anti stay fixed) and, for multi-determinant systems, the CI coefficients.
+values a_par, a_anti stay fixed), for multi-determinant systems the CI coefficients, and with
+--orbitals also the AO exponents zeta and the MO coefficients C (qmc_orbital_derivatives; the
+paper finds the exponents the most rewarding parameters).
 There is no CPU fallback: without a GPU this raises.
 """
 from __future__ import annotations
@@ -38,7 +40,8 @@ def set_theta(d, theta):
     return d2
 
 
-def optimise(d, r_host, iterations=12, lr=0.2, sweeps=20, step=0.4, seed=1, optimise_ci=True, verbose=True):
+def optimise(d, r_host, iterations=12, lr=0.2, sweeps=20, step=0.4, seed=1, optimise_ci=True, verbose=True,
+             optimise_orbitals=False, lr_orbitals=0.05):
     """Returns the list of (E_v, standard error, gradient norm) per iteration and the final description."""
     if not torch.cuda.is_available():
         raise RuntimeError("vmc_example needs a CUDA device: the product path has no CPU fallback")
@@ -58,6 +61,14 @@ def optimise(d, r_host, iterations=12, lr=0.2, sweeps=20, step=0.4, seed=1, opti
         if verbose:
             print(f"iteration {it:2d}: E_v = {e_v:+.5f} +- {err:.5f} Ha   |grad| = {history[-1][2]:.4f}   "
                   f"b = {d.jastrow_b:.4f}  en = ({d.jastrow_en_w0:+.4f}, {d.jastrow_en_w1:+.4f}, {d.jastrow_en_w2:.4f})")
+        if optimise_orbitals:   # eq. 6 with O = d ln Psi / d C and d ln Psi / d zeta, same E_L
+            dC, dz = s.orbital_derivatives(r, d.n_ao, d.n_mo)
+            _, g_C = qb.energy_gradient(el, dC.view(dC.shape[0], -1))
+            _, g_z = qb.energy_gradient(el, dz)
+            d = copy.copy(d)
+            d.mo_coeff = np.asarray(d.mo_coeff, np.float64) - lr_orbitals * g_C.reshape(d.n_ao, d.n_mo)
+            d.ao_zeta = np.maximum(np.asarray(d.ao_zeta, np.float64) - lr_orbitals * g_z, 0.1)
+            del dC, dz
         theta = get_theta(d)
         theta[mask] -= lr * grad[mask]
         theta[2] = max(theta[2], 0.05)            # keep the Pade denominators positive
@@ -73,11 +84,13 @@ def main():
     ap.add_argument("--walkers", type=int, default=65536)
     ap.add_argument("--iterations", type=int, default=12)
     ap.add_argument("--lr", type=float, default=0.2)
+    ap.add_argument("--orbitals", action="store_true", help="also optimise AO exponents and MO coefficients")
     args = ap.parse_args()
     d, r = wl.CONFIGS[args.config](M=args.walkers)
     d = copy.copy(d)
     d.jastrow_en_w2 = 1.0                          # the e-n kernel starts switched off (w0 = w1 = 0) with D = 1 + r
-    optimise(d, r, iterations=args.iterations, lr=args.lr, step=float(d.extra.get("step", 0.4)))
+    optimise(d, r, iterations=args.iterations, lr=args.lr, step=float(d.extra.get("step", 0.4)),
+             optimise_orbitals=args.orbitals)
 
 
 if __name__ == "__main__":

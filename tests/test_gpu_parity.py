@@ -573,6 +573,26 @@ def test_vmc_example_gradient_descent_lowers_the_h2_energy(env):
     assert d_opt.jastrow_en_w1 != 0.0 and -1.20 < e[-1] < -1.10   # exact H2: -1.1745 Ha; HF-like orbital + Jastrow ~ -1.15
 
 
+def test_vmc_example_recovers_detuned_exponents_through_the_orbital_derivatives(env):
+    # eq. 6 with O = d ln Psi / d zeta, d ln Psi / d C (qmc_orbital_derivatives): H2 with both AO exponents scaled by 1.35;
+    # descending along the orbital gradient brings zeta back towards its value and the energy down by ten standard
+    # errors relative to optimising the Jastrow parameters alone (seeded, hence reproducible)
+    import copy
+    from paper_2506_09743_b200 import vmc_example as vx
+    d, r = wl.h2(M=65536)
+    d = copy.copy(d)
+    z0 = np.asarray(d.ao_zeta, np.float64)
+    d.ao_zeta = 1.35 * z0
+    d.jastrow_en_w2 = 1.0
+    h_j, _ = vx.optimise(d, r, iterations=8, lr=0.2, step=0.5, verbose=False)
+    h_o, d_o = vx.optimise(d, r, iterations=8, lr=0.2, step=0.5, verbose=False, optimise_orbitals=True, lr_orbitals=0.3)
+    err = max(h[1] for h in h_j + h_o)
+    assert err < 5e-3                                            # detuned exponents break the cusp: larger variance
+    assert h_o[-1][0] < h_j[-1][0] - 6 * err, (h_o[-1], h_j[-1])
+    assert h_o[-1][0] < h_o[1][0] - 3 * err                      # iteration 0 still carries the initial walkers
+    assert np.all(d_o.ao_zeta < 1.35 * z0 - 0.15) and np.all(d_o.ao_zeta > z0)
+
+
 def test_results_are_repeatable_bit_for_bit(env):
     # the fallback work list fills in a nondeterministic order, the results must not depend on it (slice-ordered sums)
     torch, ob, qb = env
