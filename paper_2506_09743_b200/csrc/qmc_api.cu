@@ -38,7 +38,8 @@ struct Variant {
   bool exact;  // compiled for n_up = n_dn = NS
   const void *k_el, *k_psi, *k_metro, *k_expl, *k_el_deriv;
   const void *e_el, *e_psi, *e_metro, *e_expl, *e_el_deriv;
-  const void *k_orb;  // orbital-parameter derivatives
+  const void *k_orb;  // orbital-parameter derivatives, kWarpsOrb warps per block
+  const void *k_orb_small;  // the same with kWarpsOrbSmall warps (less shared memory)
   int orb_ws_doubles;  // the same with the e-e-n Jastrow kernel D.3 (EEN)
 };
 
@@ -55,7 +56,8 @@ Variant make_variant() {
   v.k_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi>;
   v.k_expl = (const void *)explicit_energy_kernel<NS, NMO, X, kWarpsEl>;
   v.k_el_deriv = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true>;
-  v.k_orb = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsEl>;
+  v.k_orb = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrb>;
+  v.k_orb_small = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrbSmall>;
   v.orb_ws_doubles = Geo<NS, NMO>::total + Geo<NS, NMO>::orbExtra;
   v.e_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, false, true>;
   v.e_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi, false, true>;
@@ -113,6 +115,7 @@ struct qmc_system {
   std::unordered_map<cudaStream_t, Scratch> scratch;
   // qmc_local_energy_host: two internal streams and double-buffered device scratch (grown on demand)
   bool orb_ready = false;  // orbital-derivative kernel configured (lazily: most users never call it)
+  int orb_warps = 0;
   int blocks_orb = 0;
   cudaStream_t hst[2] = {nullptr, nullptr};
   double *hbuf[2] = {nullptr, nullptr};
@@ -868,29 +871,34 @@ int qmc_orbital_derivatives(qmc_system_t *s, const double *d_r, int64_t M, doubl
   if (!s || !d_r || M <= 0 || (!d_dC && !d_dzeta)) return QMC_EINVAL;
   CK(cudaSetDevice(s->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  const int smem = s->P.smem_const_bytes + kWarpsEl * s->var.orb_ws_doubles * (int)sizeof(double);
+  auto smem_for = [&](int warps) { return s->P.smem_const_bytes + warps * s->var.orb_ws_doubles * (int)sizeof(double); };
+  std::lock_guard<std::mutex> lock(s->scratch_mu);  // lazy configuration; the launch below is asynchronous
   if (!s->orb_ready) {
     int dev_smem = 0;
     cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, s->device);
-    if (smem > dev_smem) return QMC_EUNSUPPORTED;
-    CK(cudaFuncSetAttribute(s->var.k_orb, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    s->orb_warps = smem_for(kWarpsOrb) <= dev_smem ? kWarpsOrb : kWarpsOrbSmall;
+    if (smem_for(s->orb_warps) > dev_smem) return QMC_EUNSUPPORTED;
+    const void *k = s->orb_warps == kWarpsOrb ? s->var.k_orb : s->var.k_orb_small;
+    CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_for(s->orb_warps)));
     int per_sm = 0;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, s->var.k_orb, kWarpsEl * 32, smem));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, s->orb_warps * 32, smem_for(s->orb_warps)));
     if (per_sm < 1) return QMC_EUNSUPPORTED;
     s->blocks_orb = per_sm * s->n_sm;
     s->orb_ready = true;
   }
+  const int warps = s->orb_warps, smem = smem_for(warps);
+  const void *kern = warps == kWarpsOrb ? s->var.k_orb : s->var.k_orb_small;
   // coefficients of MOs that no determinant uses have a zero derivative and are not touched by the kernel
-  if (d_dC) CK(cudaMemsetAsync(d_dC, 0, (size_t)M * (size_t)s->P.n_ao * (size_t)s->P.n_mo_all * sizeof(double), st));
+  if (d_dC && s->P.n_mo < s->P.n_mo_all) CK(cudaMemsetAsync(d_dC, 0, (size_t)M * (size_t)s->P.n_ao * (size_t)s->P.n_mo_all * sizeof(double), st));
   WalkerIO io{};
   io.r_in = d_r;
   io.M = M;
   io.logpsi = d_dC;    // this kernel's outputs travel in the two output slots: dC [M][n_ao][n_mo], dzeta [M][n_ao]
   io.eloc = d_dzeta;
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
-  const int grid = (int)std::min<int64_t>((groups + kWarpsEl - 1) / kWarpsEl, s->blocks_orb);
+  const int grid = (int)std::min<int64_t>((groups + warps - 1) / warps, s->blocks_orb);
   void *args[2] = {(void *)&s->P, (void *)&io};
-  CK(cudaLaunchKernel(s->var.k_orb, dim3(grid), dim3(kWarpsEl * 32), args, smem, st));
+  CK(cudaLaunchKernel(kern, dim3(grid), dim3(warps * 32), args, smem, st));
   ++g_launches;
   return QMC_OK;
 }

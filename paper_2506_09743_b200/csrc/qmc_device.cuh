@@ -32,7 +32,10 @@ constexpr int kMaxEen = 6;    // terms of the electron-electron-nucleus Jastrow 
 #ifndef QMC_WARPS_PSI
 #define QMC_WARPS_PSI 10     // warps per block of the values-only kernels (log|Psi|, Metropolis): they fit 96 registers
 #endif
-constexpr int kWarpsEl = QMC_WARPS, kWarpsPsi = QMC_WARPS_PSI;
+#ifndef QMC_WARPS_ORB
+#define QMC_WARPS_ORB 12     // warps per block of the orbital-derivative kernel (one block per SM; 8 when shared memory is short)
+#endif
+constexpr int kWarpsEl = QMC_WARPS, kWarpsPsi = QMC_WARPS_PSI, kWarpsOrb = QMC_WARPS_ORB, kWarpsOrbSmall = 8;
 constexpr int kWarpsMax = kWarpsEl > kWarpsPsi ? kWarpsEl : kWarpsPsi;
 
 // shell record kinds
