@@ -130,6 +130,14 @@ int qmc_local_energy(qmc_system_t *s, const double *d_r, int64_t M, double *d_lo
 int qmc_local_energy_host(qmc_system_t *s, const double *h_r, int64_t M, double *h_logpsi, double *h_sign,
                           double *h_eloc, int32_t n_chunks);
 
+/* qmc_local_energy with EVERY walker on the explicit route: each determinant's Slater matrices are eliminated on
+ * their own (G.7 per determinant; what PAPER.md:349 / Fig. 11 calls "explicit"), no excitation tables.
+ * Same arguments, same outputs within rounding; N_det eliminations per walker and spin instead of one.  It exists
+ * for the comparison of Fig. 11 (accelerated vs explicit) and as a cross-check; qmc_local_energy uses this route
+ * only for walkers whose reference determinant is nearly singular.  Asynchronous. */
+int qmc_local_energy_explicit(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign,
+                              double *d_eloc, void *cuda_stream);
+
 /* log|Psi| and sign only (the part of the path the sampler needs). Same arguments. */
 int qmc_log_psi(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign,
                 void *cuda_stream);

@@ -15,7 +15,7 @@ QMC_OK, QMC_EINVAL, QMC_EUNSUPPORTED, QMC_ECUDA, QMC_ENOMEM = 0, -1, -2, -3, -4
 _lib = None
 
 EXPORTS = ["qmc_setup", "qmc_destroy", "qmc_local_energy", "qmc_log_psi", "qmc_metropolis", "qmc_batch_stats",
-           "qmc_fp64_peak", "qmc_model_flops", "qmc_launch_count", "qmc_status_string", "qmc_n_param",
+           "qmc_fp64_peak", "qmc_model_flops", "qmc_launch_count", "qmc_status_string", "qmc_n_param", "qmc_local_energy_explicit",
            "qmc_log_derivatives", "qmc_energy_gradient", "qmc_local_energy_host", "qmc_orbital_derivatives"]
 
 
@@ -56,6 +56,8 @@ def lib():
         L.qmc_destroy.argtypes = [vp]
         L.qmc_local_energy.restype = C.c_int
         L.qmc_local_energy.argtypes = [vp, vp, i64, vp, vp, vp, vp]
+        L.qmc_local_energy_explicit.restype = C.c_int
+        L.qmc_local_energy_explicit.argtypes = [vp, vp, i64, vp, vp, vp, vp]
         L.qmc_orbital_derivatives.restype = C.c_int
         L.qmc_orbital_derivatives.argtypes = [vp, vp, i64, vp, vp, vp]
         L.qmc_local_energy_host.restype = C.c_int
@@ -161,6 +163,17 @@ class QmcSystem:
         sign = new() if sign is None else sign
         eloc = new() if eloc is None else eloc
         _check(lib().qmc_local_energy(self._h, _dp(r), M, _dp(logpsi), _dp(sign), _dp(eloc), _stream(stream)))
+        return logpsi, sign, eloc
+
+    def local_energy_explicit(self, r, logpsi=None, sign=None, eloc=None, stream=None):
+        """qmc_local_energy_explicit: the same outputs with every determinant eliminated on its own (Fig. 11's
+        "explicit" route) for every walker."""
+        M = self._chk_r(r)
+        new = lambda: torch.empty(M, dtype=torch.float64, device=r.device)
+        logpsi = new() if logpsi is None else logpsi
+        sign = new() if sign is None else sign
+        eloc = new() if eloc is None else eloc
+        _check(lib().qmc_local_energy_explicit(self._h, _dp(r), M, _dp(logpsi), _dp(sign), _dp(eloc), _stream(stream)))
         return logpsi, sign, eloc
 
     def local_energy_host(self, r_host, out_host=None, n_chunks: int = 2):

@@ -72,6 +72,25 @@ def measure(name, d, r_host, peak):
     return row
 
 
+def fig11(walkers=32768, n_dets=(1, 4, 20, 100, 500)):
+    """The comparison of PAPER.md:345-349 (Fig. 11): E_L through the excitation tables of the reference
+    (F.6/F.7, qmc_local_energy) against every determinant eliminated on its own (qmc_local_energy_explicit),
+    CO shape, as a function of the number of determinants."""
+    out = []
+    for nd in n_dets:
+        d, r_host = wl.co(M=walkers, n_det=nd)
+        s = qb.QmcSystem(d, 0)
+        r = torch.from_numpy(r_host).cuda()
+        s.metropolis(r, float(d.extra.get("step", 0.2)), 20, seed=1)
+        lp = torch.empty(walkers, dtype=torch.float64, device="cuda")
+        sg, el = torch.empty_like(lp), torch.empty_like(lp)
+        t_tab = _time(lambda: s.local_energy(r, lp, sg, el))
+        t_exp = _time(lambda: s.local_energy_explicit(r, lp, sg, el), reps=3, warm=1)
+        out.append(dict(n_det=nd, walkers=walkers, tab_ms=1e3 * t_tab, exp_ms=1e3 * t_exp))
+        s.close()
+    return out
+
+
 def scan(n_geom, peak):
     """BASELINE configs[4]: per geometry 50 sweeps with E_L after every sweep."""
     out = []
@@ -119,6 +138,11 @@ def main():
     for x in rows:
         print(f"| {x['config']} | {x['deriv_walkers']} | {x['el_d_ms']:.3f} | {x['n_param']} | {x['O_ms']:.3f} | "
               f"{x['n_ao']} x {x['n_mo']} + {x['n_ao']} | {x['orb_ms']:.3f} |")
+    print("\nAccelerated (excitation tables, F.6/F.7) vs explicit per-determinant E_L (PAPER.md:345-349, Fig. 11), CO shape:")
+    print("| N_det | walkers | tables ms | explicit ms | explicit / tables |")
+    print("|---|---|---|---|---|")
+    for x in fig11():
+        print(f"| {x['n_det']} | {x['walkers']} | {x['tab_ms']:.3f} | {x['exp_ms']:.3f} | {x['exp_ms'] / x['tab_ms']:.1f} |")
     if args.scan_geometries > 0:
         geo, t_total = scan(args.scan_geometries, peak)
         print(f"\nCO scan (500 determinants, {geo[0]['walkers']} walkers per geometry, {geo[0]['sweeps']} sweeps + E_L on every "

@@ -660,7 +660,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
 }
 
 static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, double *d_eloc,
-                       void *stream, bool el, double *d_O = nullptr) {
+                       void *stream, bool el, double *d_O = nullptr, bool explicit_only = false) {
   if (!s || !d_r || M <= 0) return QMC_EINVAL;
   CK(cudaSetDevice(s->device));
   cudaStream_t st = (cudaStream_t)stream;
@@ -676,7 +676,7 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
   const int64_t need = (groups + wpb - 1) / wpb;
   const int grid = (int)std::min<int64_t>(need, d_O ? s->blocks_deriv : (el ? s->blocks_el : s->blocks_psi));
   double *fb = nullptr;
-  const bool fallback = el && s->P.n_det_all > 1;  // a single determinant has no reference to be ill-conditioned against
+  const bool fallback = explicit_only || (el && s->P.n_det_all > 1);  // a single determinant has no reference to be ill-conditioned against
   const int64_t expl_warps = (int64_t)s->blocks_expl * kWarpsEl;
   if (fallback) {
     // stream-ordered scratch of the explicit fallback: partial sums [groups + warps][G][2] doubles, then
@@ -704,7 +704,14 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
     io.fb_done = fbi + 1 + groups;
   }
   void *args[2] = {(void *)&s->P, (void *)&io};
-  CK(cudaLaunchKernel(d_O ? s->var.k_el_deriv : (el ? s->var.k_el : s->var.k_psi), dim3(grid), dim3(wpb * 32), args, smem, st));
+  if (explicit_only) {  // every group goes on the list; the table-path kernel is not launched
+    if (groups > (int64_t)INT32_MAX) return QMC_EINVAL;
+    list_all_groups_kernel<<<(int)std::min<int64_t>((groups + 255) / 256, 1024), 256, 0, st>>>(io.fb_count, io.fb_list, io.fb_done,
+                                                                                              (int)groups);
+    CK(cudaGetLastError());
+  } else {
+    CK(cudaLaunchKernel(d_O ? s->var.k_el_deriv : (el ? s->var.k_el : s->var.k_psi), dim3(grid), dim3(wpb * 32), args, smem, st));
+  }
   ++g_launches;
   if (fallback) {
     CK(cudaLaunchKernel(s->var.k_expl, dim3(s->blocks_expl), dim3(kWarpsEl * 32), args, s->smem_el, st));
@@ -716,6 +723,11 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
 int qmc_local_energy(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, double *d_eloc,
                      void *cuda_stream) {
   return launch_eval(s, d_r, M, d_logpsi, d_sign, d_eloc, cuda_stream, true);
+}
+
+int qmc_local_energy_explicit(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign,
+                              double *d_eloc, void *cuda_stream) {
+  return launch_eval(s, d_r, M, d_logpsi, d_sign, d_eloc, cuda_stream, true, nullptr, true);
 }
 
 int qmc_local_energy_host(qmc_system_t *s, const double *h_r, int64_t M, double *h_logpsi, double *h_sign,

@@ -419,6 +419,16 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   }
 }
 
+// every group on the explicit kernel's work list (qmc_local_energy_explicit)
+__global__ void __launch_bounds__(256) list_all_groups_kernel(int *__restrict__ count, int *__restrict__ list,
+                                                              int *__restrict__ done, int n_groups) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_groups; i += gridDim.x * blockDim.x) {
+    list[i] = i;
+    done[i] = 0;
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) *count = n_groups;
+}
+
 // acc[i] += x[i]  (E_L on every sweep, BASELINE config 5)
 __global__ void __launch_bounds__(256) accumulate_kernel(double *__restrict__ acc, const double *__restrict__ x, int64_t M) {
   for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < M; i += (int64_t)gridDim.x * blockDim.x) acc[i] += x[i];

@@ -593,6 +593,26 @@ def test_vmc_example_recovers_detuned_exponents_through_the_orbital_derivatives(
     assert np.all(d_o.ao_zeta < 1.35 * z0 - 0.15) and np.all(d_o.ao_zeta > z0)
 
 
+@pytest.mark.parametrize("name,M", [("H2", 515), ("LiH", 300), ("Li2", 1027), ("CO", 1025)])
+def test_explicit_route_for_every_walker(env, name, M):
+    """qmc_local_energy_explicit (every determinant eliminated on its own, Fig. 11's "explicit") against the oracle,
+    which is built the same way, and against the table path."""
+    torch, ob, qb = env
+    d, r = wl.CONFIGS[name](M=M)
+    o = ob.OracleSystem(d)
+    lp0, sg0, el0 = ob.local_energy(o, r, threads=8)
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    lp, sg, el = (t.cpu().numpy() for t in s.local_energy_explicit(rg))
+    lpt, sgt, elt = (t.cpu().numpy() for t in s.local_energy(rg))
+    s.close()
+    keep = lp0 - lp0.max() > math.log(1e-6)
+    assert np.array_equal(sg, sg0) and np.max(np.abs(lp - lp0)) < 1e-10
+    assert np.max((np.abs(el - el0) / np.maximum(1, np.abs(el0)))[keep]) < 1e-8
+    assert np.array_equal(sg, sgt) and np.max(np.abs(lp - lpt)) < 1e-10
+    assert np.max((np.abs(el - elt) / np.maximum(1, np.abs(el0)))[keep]) < 1e-8
+
+
 def test_results_are_repeatable_bit_for_bit(env):
     # the fallback work list fills in a nondeterministic order, the results must not depend on it (slice-ordered sums)
     torch, ob, qb = env
