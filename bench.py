@@ -130,7 +130,7 @@ def run_reference(args):
 
 
 K_DERIV = 5  # timed repetitions of the NEXT-1 block
-E2E_CHUNKS = 2  # walker ranges pipelined by qmc_local_energy_host
+E2E_CHUNKS = 4  # walker ranges pipelined by qmc_local_energy_host (measured: 1, 2, 4, 8, 16 ranges -> 91, 116, 126, 119, 105 M walker*E_L/s)
 
 
 def main():
