@@ -306,6 +306,48 @@ def test_full_size_co_sampled(env):
     s.close()
 
 
+def test_full_size_co_derivatives_sampled(env):
+    """The NEXT-1 calls in the sizes bench.py times them at: O_p on 131072 CO walkers, the orbital-parameter derivatives
+    on the first 32768; the oracle evaluates a sample of walkers, and the eq. 6 reduction is checked on the full arrays
+    by properties (sum rule per walker, Euler's identity for the MO coefficients)."""
+    torch, ob, qb = env
+    d, r = wl.co()
+    M = r.shape[2]
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    lp, sg, el, O = s.log_derivatives(rg)
+    idx = np.unique(np.concatenate([np.arange(0, 32), np.arange(M - 33, M), np.random.default_rng(1).integers(0, M, 512)]))
+    o = ob.OracleSystem(d)
+    rs = np.ascontiguousarray(r[:, :, idx])
+    lp0 = ob.local_energy(o, rs, threads=os.cpu_count() or 8)[0]
+    O0 = ob.log_derivatives(o, rs, threads=os.cpu_count() or 8)
+    keep = lp0 - float(lp.max()) > math.log(1e-6)
+    On = O[torch.from_numpy(idx).cuda()].cpu().numpy()
+    assert np.max((np.abs(On - O0) / np.maximum(1.0, np.abs(O0)))[keep]) < 1e-8
+    ci = torch.from_numpy(np.asarray(d.ci_coeff)).cuda()
+    lpn = lp.cpu().numpy()
+    good = torch.from_numpy(lpn - lpn.max() > math.log(1e-6)).cuda()
+    assert float(((O[:, 6:] @ ci - 1.0).abs() * good).max()) < 1e-8           # Sigma is linear in the CI coefficients
+    ev, g = qb.energy_gradient(el, O)
+    assert np.isfinite(g).all() and abs(ev - float(el.mean())) < 1e-9 * abs(ev)
+    # orbital parameters
+    Mo = 32768
+    ro = rg[:, :, :Mo].contiguous()
+    dC, dz = s.orbital_derivatives(ro, d.n_ao, d.n_mo)
+    io = idx[idx < Mo]
+    ko = keep[idx < Mo]
+    dC0, dz0 = ob.orbital_derivatives(o, np.ascontiguousarray(r[:, :, io]), threads=os.cpu_count() or 8)
+    sel = torch.from_numpy(io).cuda()
+    eC = np.abs(dC[sel].cpu().numpy() - dC0) / np.maximum(1.0, np.abs(dC0))
+    ez = np.abs(dz[sel].cpu().numpy() - dz0) / np.maximum(1.0, np.abs(dz0))
+    assert np.max(eC[ko]) < 1e-8 and np.max(ez[ko]) < 1e-8
+    # Euler: Psi is homogeneous of degree N_e in the MO coefficients -> sum C dlnPsi/dC = N_e for every walker
+    Cm = torch.from_numpy(np.asarray(d.mo_coeff, np.float64)).cuda()
+    euler = (dC * Cm[None]).sum(dim=(1, 2))
+    assert float(((euler - d.n_e).abs() * good[:Mo]).max()) < 1e-7
+    s.close()
+
+
 def test_co_scan_geometries_sampled(env):
     """BASELINE configs[4] shape: 500 determinants, several bond lengths, E_L accumulated every sweep."""
     torch, ob, qb = env
