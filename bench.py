@@ -213,9 +213,21 @@ def main():
     launches = qb.launch_count()
     if world > 1:
         dist.barrier()
-    t_met = sum(a.elapsed_time(b) for a, b, c, e, _, _ in recs) * 1e-3
-    t_el = sum(b.elapsed_time(c) for a, b, c, e, _, _ in recs) * 1e-3
-    t_all = sum(a.elapsed_time(e) for a, b, c, e, _, _ in recs) * 1e-3
+    t_met = sum(x[0].elapsed_time(x[1]) for x in recs) * 1e-3
+    t_el = sum(x[1].elapsed_time(x[2]) for x in recs) * 1e-3
+    t_all = sum(x[0].elapsed_time(x[3]) for x in recs) * 1e-3
+    # ---- the dominant kernel's own launch duration (roofline): the same K steps once more (flush, sampler, E_L,
+    # statistics) with CUDA events recorded INSIDE the library on the launching stream before and after the
+    # table-path kernel.  Not done in the timed steps above: the extra event records between the two kernels
+    # lengthen the call by ~10 us (measured), which would tax the headline value.
+    sysh.set_kernel_timing(True)
+    t_kmain = t_kfb = 0.0
+    for k in range(args.steps):
+        one_step(args.warmup + args.steps + k, False)   # batch_stats synchronises the stream
+        k_main, k_fb = sysh.kernel_times()
+        t_kmain += k_main * 1e-3
+        t_kfb += k_fb * 1e-3
+    sysh.set_kernel_timing(False)
 
     # ---- end to end through the C ABI with host buffers
     # qmc_local_energy_host: pinned host walkers -> (chunked, pipelined) H2D -> kernels -> D2H of log|Psi|, sign,
@@ -263,14 +275,15 @@ def main():
             t_o += a.elapsed_time(b) * 1e-3
     del dC, dz, r_orb
 
-    t_met, t_el, t_all, t_e2e = max_over_ranks([t_met, t_el, t_all, t_e2e], device=dev)
+    t_met, t_el, t_all, t_e2e, t_kmain, t_kfb = max_over_ranks([t_met, t_el, t_all, t_e2e, t_kmain, t_kfb], device=dev)
 
     K = args.steps
     el_rate = world * M * K / t_el
     met_rate = world * M * n_sweeps * K / t_met
     e2e_rate = world * M * K / t_e2e
     flops_el, flops_st = sysh.model_flops(0), sysh.model_flops(1)
-    achieved = flops_el * M * K / t_el / 1e12  # per GPU
+    achieved = flops_el * M * K / t_kmain / 1e12    # per GPU, the dominant kernel's own launch duration
+    achieved_call = flops_el * M * K / t_el / 1e12  # the whole qmc_local_energy call (kernel + explicit fallback kernel)
     achieved_met = flops_st * M * n_sweeps * K / t_met / 1e12
 
     cpu = None
@@ -295,6 +308,12 @@ def main():
             "local_energy_ms": 1e3 * t_el / K,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_dfma, "unit": "TFLOP/s",
                          "frac": achieved / peak_dfma,
+                         "kernel_ms": 1e3 * t_kmain / K, "fallback_kernel_ms": 1e3 * t_kfb / K,
+                         "achieved_call": achieved_call, "frac_call": achieved_call / peak_dfma,
+                         "timing": "kernel_ms: CUDA events recorded inside qmc_local_energy on the launching stream before and "
+                                   "after the table-path kernel (qmc_set_kernel_timing), mean over a replay of the K steps "
+                                   "(flush, sampler, E_L, statistics) right after the timed ones; *_call: events around the "
+                                   "whole call in the K timed steps, which also runs the explicit fallback kernel",
                          "traffic": 44129280,  # dram bytes read+written per launch, profiles/r01_el_kernel.md
                          "kernel": "local_energy_kernel<7,14,true>",
                          "peak_source": "qmc_fp64_peak DFMA microbenchmark in this process (no FP64 entry in MEASURED_PEAKS.json)",

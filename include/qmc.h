@@ -138,6 +138,14 @@ int qmc_local_energy_host(qmc_system_t *s, const double *h_r, int64_t M, double 
 int qmc_local_energy_explicit(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign,
                               double *d_eloc, void *cuda_stream);
 
+/* Measurement aid (bench.py's roofline): while enabled, qmc_local_energy / qmc_local_energy_host / qmc_log_derivatives
+ * record CUDA events on the stream they launch on -- before the table-path kernel, after it, and after the explicit
+ * fallback kernel -- at a cost of three event records per call.  qmc_kernel_times waits for the most recent such call
+ * and returns the two device durations in milliseconds (fallback = 0 for a single-determinant system); QMC_EINVAL
+ * if timing was never enabled.  One timed call in flight per handle: not for concurrent streams. */
+int qmc_set_kernel_timing(qmc_system_t *s, int enabled);
+int qmc_kernel_times(qmc_system_t *s, double *h_main_ms, double *h_fallback_ms);
+
 /* log|Psi| and sign only (the part of the path the sampler needs). Same arguments. */
 int qmc_log_psi(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign,
                 void *cuda_stream);

@@ -15,7 +15,7 @@ QMC_OK, QMC_EINVAL, QMC_EUNSUPPORTED, QMC_ECUDA, QMC_ENOMEM = 0, -1, -2, -3, -4
 _lib = None
 
 EXPORTS = ["qmc_setup", "qmc_destroy", "qmc_local_energy", "qmc_log_psi", "qmc_metropolis", "qmc_batch_stats",
-           "qmc_fp64_peak", "qmc_model_flops", "qmc_launch_count", "qmc_status_string", "qmc_n_param", "qmc_local_energy_explicit",
+           "qmc_fp64_peak", "qmc_model_flops", "qmc_launch_count", "qmc_status_string", "qmc_n_param", "qmc_local_energy_explicit", "qmc_set_kernel_timing", "qmc_kernel_times",
            "qmc_log_derivatives", "qmc_energy_gradient", "qmc_local_energy_host", "qmc_orbital_derivatives"]
 
 
@@ -58,6 +58,10 @@ def lib():
         L.qmc_local_energy.argtypes = [vp, vp, i64, vp, vp, vp, vp]
         L.qmc_local_energy_explicit.restype = C.c_int
         L.qmc_local_energy_explicit.argtypes = [vp, vp, i64, vp, vp, vp, vp]
+        L.qmc_set_kernel_timing.restype = C.c_int
+        L.qmc_set_kernel_timing.argtypes = [vp, C.c_int]
+        L.qmc_kernel_times.restype = C.c_int
+        L.qmc_kernel_times.argtypes = [vp, vp, vp]
         L.qmc_orbital_derivatives.restype = C.c_int
         L.qmc_orbital_derivatives.argtypes = [vp, vp, i64, vp, vp, vp]
         L.qmc_local_energy_host.restype = C.c_int
@@ -164,6 +168,16 @@ class QmcSystem:
         eloc = new() if eloc is None else eloc
         _check(lib().qmc_local_energy(self._h, _dp(r), M, _dp(logpsi), _dp(sign), _dp(eloc), _stream(stream)))
         return logpsi, sign, eloc
+
+    def set_kernel_timing(self, enabled: bool = True):
+        """qmc_set_kernel_timing: events around the two kernels of every E_L call (bench.py's roofline)."""
+        _check(lib().qmc_set_kernel_timing(self._h, int(bool(enabled))))
+
+    def kernel_times(self):
+        """qmc_kernel_times: (table-path kernel ms, explicit fallback kernel ms) of the most recent timed call."""
+        a, b = C.c_double(), C.c_double()
+        _check(lib().qmc_kernel_times(self._h, C.addressof(a), C.addressof(b)))
+        return a.value, b.value
 
     def local_energy_explicit(self, r, logpsi=None, sign=None, eloc=None, stream=None):
         """qmc_local_energy_explicit: the same outputs with every determinant eliminated on its own (Fig. 11's

@@ -116,6 +116,9 @@ struct qmc_system {
   // qmc_local_energy_host: two internal streams and double-buffered device scratch (grown on demand)
   bool orb_ready = false;  // orbital-derivative kernel configured (lazily: most users never call it)
   int orb_warps = 0;
+  bool time_kernels = false;  // qmc_set_kernel_timing: events around the two kernels of an E_L call
+  cudaEvent_t tev[3] = {nullptr, nullptr, nullptr};
+  bool tev_fallback = false;
   int blocks_orb = 0;
   cudaStream_t hst[2] = {nullptr, nullptr};
   double *hbuf[2] = {nullptr, nullptr};
@@ -148,6 +151,8 @@ void qmc_destroy(qmc_system_t *s) {
   cudaFree(s->d_dets);
   cudaFree(s->d_gen);
   cudaFree(s->d_cols);
+  for (cudaEvent_t e : s->tev)
+    if (e) cudaEventDestroy(e);
   cudaFree(s->d_orig);
   cudaFree(s->d_yrec);
   cudaFree(s->d_ytgt);
@@ -704,6 +709,8 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
     io.fb_done = fbi + 1 + groups;
   }
   void *args[2] = {(void *)&s->P, (void *)&io};
+  const bool timed = s->time_kernels && el && !explicit_only;
+  if (timed) CK(cudaEventRecord(s->tev[0], st));
   if (explicit_only) {  // every group goes on the list; the table-path kernel is not launched
     if (groups > (int64_t)INT32_MAX) return QMC_EINVAL;
     list_all_groups_kernel<<<(int)std::min<int64_t>((groups + 255) / 256, 1024), 256, 0, st>>>(io.fb_count, io.fb_list, io.fb_done,
@@ -713,10 +720,37 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
     CK(cudaLaunchKernel(d_O ? s->var.k_el_deriv : (el ? s->var.k_el : s->var.k_psi), dim3(grid), dim3(wpb * 32), args, smem, st));
   }
   ++g_launches;
+  if (timed) CK(cudaEventRecord(s->tev[1], st));
   if (fallback) {
     CK(cudaLaunchKernel(s->var.k_expl, dim3(s->blocks_expl), dim3(kWarpsEl * 32), args, s->smem_el, st));
     ++g_launches;
   }
+  if (timed) {
+    CK(cudaEventRecord(s->tev[2], st));
+    s->tev_fallback = fallback;
+  }
+  return QMC_OK;
+}
+
+int qmc_set_kernel_timing(qmc_system_t *s, int enabled) {
+  if (!s) return QMC_EINVAL;
+  CK(cudaSetDevice(s->device));
+  if (enabled)
+    for (cudaEvent_t &e : s->tev)
+      if (!e) CK(cudaEventCreate(&e));
+  s->time_kernels = enabled != 0;
+  return QMC_OK;
+}
+
+int qmc_kernel_times(qmc_system_t *s, double *h_main_ms, double *h_fallback_ms) {
+  if (!s || !s->tev[2]) return QMC_EINVAL;
+  CK(cudaSetDevice(s->device));
+  CK(cudaEventSynchronize(s->tev[2]));
+  float a = 0.f, b = 0.f;
+  CK(cudaEventElapsedTime(&a, s->tev[0], s->tev[1]));
+  CK(cudaEventElapsedTime(&b, s->tev[1], s->tev[2]));
+  if (h_main_ms) *h_main_ms = a;
+  if (h_fallback_ms) *h_fallback_ms = s->tev_fallback ? b : 0.0;
   return QMC_OK;
 }
 

@@ -33,7 +33,9 @@ constexpr int kMaxEen = 6;    // terms of the electron-electron-nucleus Jastrow 
 #define QMC_WARPS_PSI 10     // warps per block of the values-only kernels (log|Psi|, Metropolis): they fit 96 registers
 #endif
 #ifndef QMC_WARPS_ORB
-#define QMC_WARPS_ORB 12     // warps per block of the orbital-derivative kernel (one block per SM; 8 when shared memory is short)
+#define QMC_WARPS_ORB 10     // warps per block of the orbital-derivative kernel (one block per SM; 8 when shared memory is short).
+                             // Measured on CO, 32768 walkers, early / equilibrated: 8 warps 0.82 / 0.63 ms, 10: 0.80 / 0.60, 12: 0.78 / 0.80
+                             // (12 x 16.3 KB of scratch leave ~30 KB of L1 for the term lists and the constant tables)
 #endif
 constexpr int kWarpsEl = QMC_WARPS, kWarpsPsi = QMC_WARPS_PSI, kWarpsOrb = QMC_WARPS_ORB, kWarpsOrbSmall = 8;
 constexpr int kWarpsMax = kWarpsEl > kWarpsPsi ? kWarpsEl : kWarpsPsi;

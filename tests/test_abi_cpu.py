@@ -33,6 +33,9 @@ def test_status_strings_and_null_arguments():
     L.qmc_destroy(None)
     assert L.qmc_model_flops(None, 0) == 0.0
     assert L.qmc_n_param(None) == qb.QMC_EINVAL
+    assert L.qmc_local_energy_explicit(None, None, 4, None, None, None, None) == qb.QMC_EINVAL
+    assert L.qmc_set_kernel_timing(None, 1) == qb.QMC_EINVAL
+    assert L.qmc_kernel_times(None, None, None) == qb.QMC_EINVAL
     assert L.qmc_log_derivatives(None, None, 4, None, None, None, None, None) == qb.QMC_EINVAL
     g = np.zeros(3)
     assert L.qmc_energy_gradient(None, None, 4, 3, None, g.ctypes.data, None) == qb.QMC_EINVAL

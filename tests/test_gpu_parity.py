@@ -655,6 +655,37 @@ def test_explicit_route_for_every_walker(env, name, M):
     assert np.max((np.abs(el - elt) / np.maximum(1, np.abs(el0)))[keep]) < 1e-8
 
 
+def test_kernel_timing_events(env):
+    """qmc_set_kernel_timing / qmc_kernel_times (bench.py's roofline): the two kernel durations of an E_L call are
+    positive, add up to no more than the events around the call, and the outputs do not change."""
+    torch, ob, qb = env
+    d, r = wl.co(M=8192)
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    ref = [t.clone() for t in s.local_energy(rg)]
+    with pytest.raises(qb.QmcError):
+        s.kernel_times()                      # never enabled
+    s.set_kernel_timing(True)
+    for _ in range(2):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        out = s.local_energy(rg)
+        b.record()
+        torch.cuda.synchronize()
+        k_main, k_fb = s.kernel_times()
+        assert k_main > 0.0 and k_fb > 0.0 and k_main + k_fb <= a.elapsed_time(b) * 1.001 + 1e-3
+        assert all(torch.equal(x, y) for x, y in zip(out, ref))
+    s.set_kernel_timing(False)
+    s.close()
+    d1, r1 = wl.lih(M=256)                     # single determinant: no fallback kernel
+    s = qb.QmcSystem(d1)
+    s.set_kernel_timing(True)
+    s.local_energy(_to_gpu(torch, r1))
+    k_main, k_fb = s.kernel_times()
+    assert k_main > 0.0 and k_fb == 0.0
+    s.close()
+
+
 def test_results_are_repeatable_bit_for_bit(env):
     # the fallback work list fills in a nondeterministic order, the results must not depend on it (slice-ordered sums)
     torch, ob, qb = env
