@@ -95,6 +95,11 @@ def test_random_systems_against_the_oracle(seed):
         assert np.max(np.abs(lp - lp0)[keep]) < 1e-8, (case, np.max(np.abs(lp - lp0)[keep]))
         assert np.max((np.abs(el - el0) / np.maximum(1, np.abs(el0)))[keep]) < 1e-7, case
         assert np.max((np.abs(O - O0) / np.maximum(1, np.abs(O0)))[keep]) < 1e-7, case
+        # every walker on the explicit per-determinant route
+        lpx, sgx, elx = (t.cpu().numpy() for t in s.local_energy_explicit(torch.from_numpy(r).cuda()))
+        assert np.array_equal(sgx, sg0), case
+        assert np.max(np.abs(lpx - lp0)[keep]) < 1e-8, case
+        assert np.max((np.abs(elx - el0) / np.maximum(1, np.abs(el0)))[keep]) < 1e-7, case
         # orbital-parameter derivatives: table route, explicit route (flagged groups, k >= 3) -- whichever the draw takes
         dC0, dz0 = ob.orbital_derivatives(o, r, threads=4)
         dC, dz = (t.cpu().numpy() for t in s.orbital_derivatives(torch.from_numpy(r).cuda(), d.n_ao, d.n_mo))
