@@ -78,6 +78,8 @@ def lib():
             L.oracle_orbital_derivatives.restype = C.c_int
             L.oracle_orbital_derivatives.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p,
                                                      C.c_void_p]
+            L.oracle_nuclear_log_gradient.restype = C.c_int
+            L.oracle_nuclear_log_gradient.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p]
             L.oracle_energy_gradient.restype = None
             L.oracle_energy_gradient.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
             _lib = L
@@ -266,3 +268,23 @@ def orbital_derivatives(sysd: OracleSystem, r_soa, threads: int = 1):
         with ThreadPoolExecutor(len(rs)) as ex:
             list(ex.map(run, rs))
     return dC, dz
+
+
+def nuclear_log_gradient(sysd: OracleSystem, r_soa, threads: int = 1):
+    """dR[M, n_atoms, 3] = grad_alpha ln|Psi| (eq. 7's grad_alpha ln rho / 2)."""
+    r = np.ascontiguousarray(r_soa, np.float64)
+    M = r.shape[2]
+    dR = np.empty((M, int(sysd.c.n_atoms), 3))
+    L = lib()
+
+    def run(rng):
+        rc = L.oracle_nuclear_log_gradient(sysd.ref, _p(r), M, rng[0], rng[1], _p(dR))
+        assert rc == 0
+
+    rs = _ranges(M, threads)
+    if len(rs) == 1:
+        run(rs[0])
+    else:
+        with ThreadPoolExecutor(len(rs)) as ex:
+            list(ex.map(run, rs))
+    return dR

@@ -801,3 +801,117 @@ int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, i
   free(aov); free(aoz); free(mo); free(A); free(Ai); free(gam); free(pos);
   return 0;
 }
+
+/* ------------------------------------------------------------------ */
+/* Nuclear log-gradient of the wavefunction: grad_alpha ln|Psi|, half   */
+/* of grad_alpha ln rho in the force estimator (eq. 7). */
+/* Every AO of centre a depends on (r_i - R_a) only, so   */
+/* d ao_beta(r_i) / d R_a = -grad_r ao_beta(r_i) for beta on a, else 0; */
+/* the chain rule through every determinant, inverted explicitly, gives */
+/*   d ln Sigma / d R_a = -sum_n w_n sum_{i,j} A_n^-1[j][i]             */
+/*                         sum_{beta on a} C[beta][lst_n[j]] grad ao_beta(r_i)  */
+/* and the Jastrow kernels that see the nuclei (D.2, D.3) add           */
+/*   d K_en(r_ia) / d R_a = -K_en' e_ai,                                 */
+/*   d [c f(r_ai) g(r_aj) h(r_ij)] / d R_a = -c h (f' g e_ai + f g' e_aj). */
+/* The Pade e-e kernel D.1 does not depend on R.                        */
+/* ------------------------------------------------------------------ */
+
+int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
+                                int64_t w1, double *dR) {
+  int ne = s->n_up + s->n_dn, nmo = s->n_mo, nao = s->n_ao, na = s->n_atoms;
+  double *aov = (double *)malloc(sizeof(double) * (size_t)(ne * nao + 1));       /* ao_beta(r_i) */
+  double *aog = (double *)malloc(sizeof(double) * (size_t)(3 * ne * nao + 1));   /* grad ao_beta(r_i) */
+  double *mo = (double *)malloc(sizeof(double) * (size_t)(ne * nmo + 1));
+  double *A = (double *)malloc(sizeof(double) * (size_t)(ne * ne + 1));
+  double *Ai = (double *)malloc(sizeof(double) * (size_t)(2 * ne * ne + 2));
+  double *gam = (double *)malloc(sizeof(double) * (size_t)(ne * nmo + 1));
+  double *pos = (double *)malloc(sizeof(double) * (size_t)(3 * ne + 1));
+  if (!aov || !aog || !mo || !A || !Ai || !gam || !pos) return -1;
+  double ao[5];
+  for (int64_t w = w0; w < w1; ++w) {
+    gather_walker(r, M, w, ne, pos);
+    for (int i = 0; i < ne; ++i)
+      for (int beta = 0; beta < nao; ++beta) {
+        oracle_ao_eval(s, beta, pos + 3 * i, ao);
+        aov[i * nao + beta] = ao[0];
+        for (int c = 0; c < 3; ++c) aog[(i * nao + beta) * 3 + c] = ao[1 + c];
+      }
+    for (int i = 0; i < ne * nmo; ++i) { mo[i] = 0.0; gam[i] = 0.0; }
+    for (int i = 0; i < ne; ++i)
+      for (int beta = 0; beta < nao; ++beta)
+        for (int alpha = 0; alpha < nmo; ++alpha) mo[i * nmo + alpha] += s->mo_coeff[beta * nmo + alpha] * aov[i * nao + beta];
+    double sigma = 0.0;
+    for (int n = 0; n < s->n_det; ++n) {
+      double D[2];
+      for (int sp = 0; sp < 2; ++sp) {
+        int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
+        const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
+        for (int i = 0; i < ns; ++i)
+          for (int j = 0; j < ns; ++j) A[i * ns + j] = mo[(e0 + i) * nmo + lst[j]];
+        D[sp] = oracle_det_inv(ns, A, Ai + sp * ne * ne);
+      }
+      double wn = s->ci_coeff[n] * D[0] * D[1];
+      sigma += wn;
+      for (int sp = 0; sp < 2; ++sp) {
+        int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
+        const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
+        const double *inv = Ai + sp * ne * ne;
+        for (int i = 0; i < ns; ++i)
+          for (int j = 0; j < ns; ++j) gam[(e0 + i) * nmo + lst[j]] += wn * inv[j * ns + i];
+      }
+    }
+    double *out = dR + (size_t)w * (size_t)(3 * na);
+    for (int k = 0; k < 3 * na; ++k) out[k] = 0.0;
+    /* Slater part */
+    for (int beta = 0; beta < nao; ++beta) {
+      int at = s->ao_atom[beta];
+      for (int c = 0; c < 3; ++c) {
+        double t = 0.0;
+        for (int alpha = 0; alpha < nmo; ++alpha) {
+          double u = 0.0;
+          for (int i = 0; i < ne; ++i) u += aog[(i * nao + beta) * 3 + c] * gam[i * nmo + alpha];
+          t += s->mo_coeff[beta * nmo + alpha] * u;
+        }
+        out[3 * at + c] -= t / sigma;
+      }
+    }
+    /* electron-nucleus kernel D.2: K = N/D, N = w0 r + w1 r^2, D = 1 + w2 r */
+    double jw0 = s->jastrow_en_w0, jw1 = s->jastrow_en_w1, jw2 = s->jastrow_en_w2;
+    if (jw0 != 0.0 || jw1 != 0.0)
+      for (int i = 0; i < ne; ++i)
+        for (int at = 0; at < na; ++at) {
+          double d[3];
+          for (int c = 0; c < 3; ++c) d[c] = pos[3 * i + c] - s->atom_xyz[3 * at + c];
+          double ria = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+          double N = jw0 * ria + jw1 * ria * ria, D = 1.0 + jw2 * ria;
+          double K1 = ((jw0 + 2.0 * jw1 * ria) * D - N * jw2) / (D * D);
+          for (int c = 0; c < 3; ++c) out[3 * at + c] -= K1 * d[c] / ria;
+        }
+    /* electron-electron-nucleus kernel D.3 (reading Q22: ordered pairs i != j, every nucleus) */
+    for (int at = 0; at < na; ++at)
+      for (int i = 0; i < ne; ++i)
+        for (int j = 0; j < ne; ++j) {
+          if (i == j || s->n_een == 0) continue;
+          double eai[3], eaj[3], eij[3];
+          for (int c = 0; c < 3; ++c) {
+            eai[c] = pos[3 * i + c] - s->atom_xyz[3 * at + c];
+            eaj[c] = pos[3 * j + c] - s->atom_xyz[3 * at + c];
+            eij[c] = pos[3 * i + c] - pos[3 * j + c];
+          }
+          double rai = sqrt(eai[0] * eai[0] + eai[1] * eai[1] + eai[2] * eai[2]);
+          double raj = sqrt(eaj[0] * eaj[0] + eaj[1] * eaj[1] + eaj[2] * eaj[2]);
+          double rij = sqrt(eij[0] * eij[0] + eij[1] * eij[1] + eij[2] * eij[2]);
+          for (int mu = 0; mu < s->n_een; ++mu) {
+            const double *q = s->een_params + 7 * mu;
+            double f, f1, f2, g, g1, g2, h, h1, h2;
+            pade3(q[1], q[2], rai, &f, &f1, &f2);
+            pade3(q[3], q[4], raj, &g, &g1, &g2);
+            pade3(q[5], q[6], rij, &h, &h1, &h2);
+            for (int c = 0; c < 3; ++c)
+              out[3 * at + c] -= q[0] * h * (f1 * g * eai[c] / rai + f * g1 * eaj[c] / raj);
+          }
+        }
+  }
+  free(aov); free(aog); free(mo); free(A); free(Ai); free(gam); free(pos);
+  return 0;
+}

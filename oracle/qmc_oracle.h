@@ -119,6 +119,14 @@ int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64
 int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                                int64_t w1, double *dC, double *dzeta);
 
+/* Nuclear log-gradient grad_alpha ln|Psi| = (1/2) grad_alpha ln rho, the factor of the second term of the force
+ * estimator (eq. 7), with the atomic positions as parameters of the AO layer:
+ * dR [M][n_atoms][3].  d ao_beta(r_i) / d R_a = -grad_r ao_beta(r_i) for the AOs of centre a; chain rule through
+ * every determinant inverted explicitly (Gamma as in oracle_orbital_derivatives), plus the nuclear dependence of
+ * the Jastrow kernels D.2 and D.3.  Rows w0 <= w < w1. */
+int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
+                                int64_t w1, double *dR);
+
 /* Estimator of eq. 6: E_v = mean E_L, grad_p = (2/M) sum_m O[m][p] (E_L[m] - E_v).
  * Kahan sums.  Ev may be NULL. */
 void oracle_energy_gradient(const double *eloc, const double *O, int64_t M, int32_t n_param,

@@ -882,3 +882,64 @@ def test_orbital_derivatives_closed_form_and_scaling_identity():
     d, r = wl.li2(M=10)
     dC, _ = ob.orbital_derivatives(ob.OracleSystem(d), r)
     assert np.max(np.abs(np.einsum("mba,ba->m", dC, d.mo_coeff) - d.n_e)) < 1e-10
+
+
+# ---------------------------------------------------------------- nuclear log-gradient (eq. 7)
+@pytest.mark.parametrize("name,M", [("H2", 6), ("LiH", 5), ("Li2", 3), ("CO", 2)])
+def test_nuclear_log_gradient_vs_central_differences_of_log_psi(name, M):
+    # grad_alpha ln|Psi| against Richardson central differences of the oracle's own (pinned) log|Psi| with one
+    # nuclear coordinate displaced, D.2 and D.3 switched on: pins the sign of d ao / d R, the AO -> atom
+    # bookkeeping, the CI weights, and both Jastrow chain rules
+    import copy
+    d, r = wl.CONFIGS[name](M=M)
+    d = _with_een(_with_en(d, 0.3, -0.05, 0.7))
+    dR = ob.nuclear_log_gradient(ob.OracleSystem(d), r)
+    assert dR.shape == (M, d.n_atoms, 3)
+
+    def lp(a, c, t):
+        d2 = copy.copy(d)
+        xyz = np.array(d.atom_xyz, np.float64, copy=True)
+        xyz[a, c] += t
+        d2.atom_xyz = xyz
+        return ob.local_energy(ob.OracleSystem(d2), r)[0]
+
+    for a in range(d.n_atoms):
+        for c in range(3):
+            cd = lambda h: (lp(a, c, h) - lp(a, c, -h)) / (2 * h)
+            ref = (4 * cd(1e-4) - cd(2e-4)) / 3
+            # 1e-6: the bound BASELINE.json's north_star gives for central differences at h = 1e-4
+            assert np.max(np.abs(dR[:, a, c] - ref) / np.maximum(1, np.abs(ref))) < 1e-6, (name, a, c)
+
+
+def test_nuclear_log_gradient_closed_form_translation_and_partition():
+    # hydrogen-like 1s at R: ln Psi = const - zeta |r - R|  =>  grad_R ln Psi = zeta (r - R)/|r - R|
+    zeta, R = 1.3, np.array([0.3, -0.2, 0.5])
+    d = atom_system(1.0, [(1, 0, 0, zeta)], [[1.0]], 1, 0, xyz=tuple(R))
+    rr = _rand_pos(40, 1, 1.5, rmin=0.05, seed=96) + R
+    dR = ob.nuclear_log_gradient(ob.OracleSystem(d), soa(rr))
+    u = rr[:, 0] - R
+    assert np.max(np.abs(dR[:, 0] - zeta * u / np.linalg.norm(u, axis=1, keepdims=True))) < 1e-13
+    # translation invariance: Psi depends on r_i - R_a and r_i - r_j only, so
+    # sum_a grad_a ln Psi = -sum_i grad_i ln Psi (the latter by central differences of a rigid electron shift)
+    d, r = wl.li2(M=6)
+    d = _with_een(_with_en(d, 0.3, -0.05, 0.7))
+    o = ob.OracleSystem(d)
+    dR = ob.nuclear_log_gradient(o, r)
+    for c in range(3):
+        def shifted(t):
+            r2 = np.array(r, copy=True)
+            r2[:, c, :] += t
+            return ob.local_energy(o, r2)[0]
+        cd = lambda h: (shifted(h) - shifted(-h)) / (2 * h)
+        ref = (4 * cd(1e-4) - cd(2e-4)) / 3
+        assert np.max(np.abs(dR[:, :, c].sum(axis=1) + ref) / np.maximum(1, np.abs(ref))) < 1e-6
+    # partition independence (threads) and a diatomic on z with sigma orbitals only has no x, y asymmetry pin:
+    # H2 with both electrons on the axis -> gradient along z only
+    d, _ = wl.h2(M=4)
+    rz = np.zeros((4, 2, 3))
+    rz[:, :, 2] = np.random.default_rng(5).uniform(-1.5, 1.5, (4, 2))
+    g = ob.nuclear_log_gradient(ob.OracleSystem(d), soa(rz))
+    assert np.max(np.abs(g[:, :, :2])) < 1e-14 and np.min(np.abs(g[:, :, 2])) > 1e-3
+    d, r = wl.lih(M=9)
+    o = ob.OracleSystem(d)
+    assert np.array_equal(ob.nuclear_log_gradient(o, r, threads=1), ob.nuclear_log_gradient(o, r, threads=3))
