@@ -273,7 +273,17 @@ def main():
         torch.cuda.synchronize()
         if k >= 3:
             t_o += a.elapsed_time(b) * 1e-3
-    del dC, dz, r_orb
+    # nuclear log-gradient (eq. 7's grad_alpha ln rho / 2) on the same walkers
+    t_n = 0.0
+    for k in range(3 + K_DERIV):
+        a, b = ev(), ev()
+        a.record(st)
+        dR = sysh.nuclear_log_gradient(r_orb, d.n_atoms)
+        b.record(st)
+        torch.cuda.synchronize()
+        if k >= 3:
+            t_n += a.elapsed_time(b) * 1e-3
+    del dC, dz, dR, r_orb
 
     t_met, t_el, t_all, t_e2e, t_kmain, t_kfb = max_over_ranks([t_met, t_el, t_all, t_e2e, t_kmain, t_kfb], device=dev)
 
@@ -332,6 +342,9 @@ def main():
             "orbital_derivatives": {"walkers": int(M_orb), "outputs_per_walker": int(d.n_ao * d.n_mo + d.n_ao),
                                     "ms": 1e3 * t_o / K_DERIV,
                                     "note": "SURVEY 8(f) NEXT-1: d ln Psi / d C and d ln Psi / d zeta per walker"},
+            "nuclear_log_gradient": {"walkers": int(M_orb), "outputs_per_walker": int(3 * d.n_atoms),
+                                     "ms": 1e3 * t_n / K_DERIV,
+                                     "note": "SURVEY 8(f) NEXT-4, first half: grad_alpha ln|Psi| of eq. 7 per walker"},
             "gpu_launches": int(launches),
             "clocks": clocks,
             "last_step": {"mean_E_L": mean, "stderr": err},

@@ -210,6 +210,18 @@ int qmc_log_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d
 int qmc_orbital_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d_dC, double *d_dzeta,
                             void *cuda_stream);
 
+/* Nuclear log-gradient of the wavefunction, grad_alpha ln|Psi| = (1/2) grad_alpha ln rho: the factor of the second
+ * term of the force estimator, eq. 7, with the atomic positions as parameters of the AO layer
+ * and of the Jastrow kernels that see the nuclei (D.2, D.3):
+ *   d_r  device, in:  double [n_e][3][M] walker coordinates (as qmc_local_energy)
+ *   d_dR device, out: double [M][n_atoms][3]  d ln|Psi| / d R_alpha,c ; every entry is written
+ * d ao_beta(r_i) / d R_alpha = -grad_r ao_beta(r_i) for the AOs of centre alpha, contracted with Gamma = d ln Sigma /
+ * d Phi exactly as qmc_orbital_derivatives does (same table path and the same explicit route for near-singular
+ * references).  Two launches on cuda_stream (Jastrow part, then the AO part).  Deterministic.  Asynchronous.
+ * Returns QMC_EINVAL for null pointers or M <= 0, QMC_EUNSUPPORTED when the shape does not fit shared memory.
+ * The other half of eq. 7, grad_alpha E_L, is not provided. */
+int qmc_nuclear_log_gradient(qmc_system_t *s, const double *d_r, int64_t M, double *d_dR, void *cuda_stream);
+
 /* Estimator of eq. 6: E_v = mean E_L, grad_p = (2/M) sum_m O[m][p] (E_L[m] - E_v).
  *   d_eloc device in [M]; d_O device in [M][n_param]; h_Ev host out (may be NULL);
  *   h_grad host out [n_param].  Deterministic (fixed partition, compensated sums).

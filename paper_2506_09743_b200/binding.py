@@ -16,7 +16,8 @@ _lib = None
 
 EXPORTS = ["qmc_setup", "qmc_destroy", "qmc_local_energy", "qmc_log_psi", "qmc_metropolis", "qmc_batch_stats",
            "qmc_fp64_peak", "qmc_model_flops", "qmc_launch_count", "qmc_status_string", "qmc_n_param", "qmc_local_energy_explicit", "qmc_set_kernel_timing", "qmc_kernel_times",
-           "qmc_log_derivatives", "qmc_energy_gradient", "qmc_local_energy_host", "qmc_orbital_derivatives"]
+           "qmc_log_derivatives", "qmc_energy_gradient", "qmc_local_energy_host", "qmc_orbital_derivatives",
+           "qmc_nuclear_log_gradient"]
 
 
 class QmcError(RuntimeError):
@@ -64,6 +65,8 @@ def lib():
         L.qmc_kernel_times.argtypes = [vp, vp, vp]
         L.qmc_orbital_derivatives.restype = C.c_int
         L.qmc_orbital_derivatives.argtypes = [vp, vp, i64, vp, vp, vp]
+        L.qmc_nuclear_log_gradient.restype = C.c_int
+        L.qmc_nuclear_log_gradient.argtypes = [vp, vp, i64, vp, vp]
         L.qmc_local_energy_host.restype = C.c_int
         L.qmc_local_energy_host.argtypes = [vp, vp, i64, vp, vp, vp, C.c_int32]
         L.qmc_log_psi.restype = C.c_int
@@ -237,6 +240,13 @@ class QmcSystem:
         dz = torch.empty((M, n_ao), dtype=torch.float64, device=r.device)
         _check(lib().qmc_orbital_derivatives(self._h, _dp(r), M, _dp(dC), _dp(dz), _stream(stream)))
         return dC, dz
+
+    def nuclear_log_gradient(self, r, n_atoms: int, stream=None):
+        """qmc_nuclear_log_gradient: dR[M, n_atoms, 3] = grad_alpha ln|Psi| (eq. 7's grad_alpha ln rho / 2)."""
+        M = self._chk_r(r)
+        dR = torch.empty((M, n_atoms, 3), dtype=torch.float64, device=r.device)
+        _check(lib().qmc_nuclear_log_gradient(self._h, _dp(r), M, _dp(dR), _stream(stream)))
+        return dR
 
     def n_param(self) -> int:
         return int(lib().qmc_n_param(self._h))

@@ -40,6 +40,7 @@ struct Variant {
   const void *e_el, *e_psi, *e_metro, *e_expl, *e_el_deriv;
   const void *k_orb;  // orbital-parameter derivatives, kWarpsOrb warps per block
   const void *k_orb_small;  // the same with kWarpsOrbSmall warps (less shared memory)
+  const void *k_nuc, *k_nuc_small;  // the same kernel in nuclear mode (qmc_nuclear_log_gradient)
   int orb_ws_doubles;  // the same with the e-e-n Jastrow kernel D.3 (EEN)
 };
 
@@ -58,6 +59,8 @@ Variant make_variant() {
   v.k_el_deriv = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true>;
   v.k_orb = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrb>;
   v.k_orb_small = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrbSmall>;
+  v.k_nuc = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrb, true>;
+  v.k_nuc_small = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrbSmall, true>;
   v.orb_ws_doubles = Geo<NS, NMO>::total + Geo<NS, NMO>::orbExtra;
   v.e_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, false, true>;
   v.e_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi, false, true>;
@@ -530,6 +533,10 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     }
     n_real_shells = n_real;
   }
+  {  // second half of the row table: kernel AO row -> centre (-1 = pad), for qmc_nuclear_log_gradient
+    const size_t n_rows = row_ao.size();
+    for (size_t R = 0; R < n_rows; ++R) row_ao.push_back(row_ao[R] < 0 ? -1 : d->ao_atom[row_ao[R]]);
+  }
   for (size_t i = 0; i < shells.size(); ++i) P.shells[i] = shells[i];
   const int n_chunks = (int)crow.size() / kChunk, NT = (NMO + 7) / 8, KS = kChunk / 4;
   P.n_chunks = n_chunks;
@@ -913,8 +920,9 @@ int qmc_energy_gradient(const double *d_eloc, const double *d_O, int64_t M, int3
   return QMC_OK;
 }
 
-int qmc_orbital_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d_dC, double *d_dzeta, void *cuda_stream) {
-  if (!s || !d_r || M <= 0 || (!d_dC && !d_dzeta)) return QMC_EINVAL;
+// one launch of orbital_derivatives_kernel: (dC, dzeta) or, with d_dR, the AO part of the nuclear log-gradient
+static int orbital_launch(qmc_system_t *s, const double *d_r, int64_t M, double *d_dC, double *d_dzeta, double *d_dR,
+                          void *cuda_stream) {
   CK(cudaSetDevice(s->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
   auto smem_for = [&](int warps) { return s->P.smem_const_bytes + warps * s->var.orb_ws_doubles * (int)sizeof(double); };
@@ -926,6 +934,8 @@ int qmc_orbital_derivatives(qmc_system_t *s, const double *d_r, int64_t M, doubl
     if (smem_for(s->orb_warps) > dev_smem) return QMC_EUNSUPPORTED;
     const void *k = s->orb_warps == kWarpsOrb ? s->var.k_orb : s->var.k_orb_small;
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_for(s->orb_warps)));
+    CK(cudaFuncSetAttribute(s->orb_warps == kWarpsOrb ? s->var.k_nuc : s->var.k_nuc_small,
+                            cudaFuncAttributeMaxDynamicSharedMemorySize, smem_for(s->orb_warps)));
     int per_sm = 0;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, s->orb_warps * 32, smem_for(s->orb_warps)));
     if (per_sm < 1) return QMC_EUNSUPPORTED;
@@ -933,7 +943,8 @@ int qmc_orbital_derivatives(qmc_system_t *s, const double *d_r, int64_t M, doubl
     s->orb_ready = true;
   }
   const int warps = s->orb_warps, smem = smem_for(warps);
-  const void *kern = warps == kWarpsOrb ? s->var.k_orb : s->var.k_orb_small;
+  const void *kern = d_dR ? (warps == kWarpsOrb ? s->var.k_nuc : s->var.k_nuc_small)
+                          : (warps == kWarpsOrb ? s->var.k_orb : s->var.k_orb_small);
   // coefficients of MOs that no determinant uses have a zero derivative and are not touched by the kernel
   if (d_dC && s->P.n_mo < s->P.n_mo_all) CK(cudaMemsetAsync(d_dC, 0, (size_t)M * (size_t)s->P.n_ao * (size_t)s->P.n_mo_all * sizeof(double), st));
   WalkerIO io{};
@@ -941,12 +952,29 @@ int qmc_orbital_derivatives(qmc_system_t *s, const double *d_r, int64_t M, doubl
   io.M = M;
   io.logpsi = d_dC;    // this kernel's outputs travel in the two output slots: dC [M][n_ao][n_mo], dzeta [M][n_ao]
   io.eloc = d_dzeta;
+  io.O = d_dR;         // nuclear mode: dR [M][n_atoms][3], decremented by the AO part
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
   const int grid = (int)std::min<int64_t>((groups + warps - 1) / warps, s->blocks_orb);
   void *args[2] = {(void *)&s->P, (void *)&io};
   CK(cudaLaunchKernel(kern, dim3(grid), dim3(warps * 32), args, smem, st));
   ++g_launches;
   return QMC_OK;
+}
+
+int qmc_orbital_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d_dC, double *d_dzeta, void *cuda_stream) {
+  if (!s || !d_r || M <= 0 || (!d_dC && !d_dzeta)) return QMC_EINVAL;
+  return orbital_launch(s, d_r, M, d_dC, d_dzeta, nullptr, cuda_stream);
+}
+
+int qmc_nuclear_log_gradient(qmc_system_t *s, const double *d_r, int64_t M, double *d_dR, void *cuda_stream) {
+  if (!s || !d_r || M <= 0 || !d_dR) return QMC_EINVAL;
+  CK(cudaSetDevice(s->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  // Jastrow part (D.2, D.3) initialises dR, one thread per walker; the AO part is subtracted by the second launch
+  nuclear_jastrow_gradient_kernel<<<(unsigned)((M + 127) / 128), 128, 0, st>>>(s->P, d_r, M, d_dR);
+  CK(cudaGetLastError());
+  ++g_launches;
+  return orbital_launch(s, d_r, M, nullptr, nullptr, d_dR, cuda_stream);
 }
 
 int qmc_batch_stats(const double *d_x, int64_t M, double *h_mean, double *h_stderr, void *cuda_stream) {

@@ -176,7 +176,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
 // a second pass over the shells that rebuilds phi and d phi / d zeta = phi (d ln N / d zeta - r) in the AO tile and
 // contracts them with Gamma.  Outputs travel in io.logpsi (dC) and io.eloc (dzeta); either may be null.
 // ---------------------------------------------------------------------------------
-template <int NS, int NMO, bool X, int WPB>
+template <int NS, int NMO, bool X, int WPB, bool NUC = false>
 __global__ void __launch_bounds__(WPB * 32, 1)
     orbital_derivatives_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -194,6 +194,11 @@ __global__ void __launch_bounds__(WPB * 32, 1)
   const int64_t n_groups = (io.M + G - 1) / G;
   const int64_t stride = (int64_t)gridDim.x * WPB;
   double *dC = io.logpsi, *dZ = io.eloc;
+  // nuclear mode (qmc_nuclear_log_gradient): io.O = dR [M][n_atoms][3]; the second pass runs once per Cartesian
+  // component with d phi / d R_c = -d phi / d r_c in the operator columns, summed over the rows of each centre
+  double *dRo = io.O;
+  constexpr bool nuc = NUC;  // its own instantiation: the parameter-derivative kernel keeps its code and registers
+  const int *row_atom = P.ao_orig + P.n_chunks * kChunk;
   double *sGam = ws + GE::oGam;
   const double *sRes = ws + GE::oRes;
   for (int64_t grp = (int64_t)blockIdx.x * WPB + warp; grp < n_groups; grp += stride) {
@@ -226,6 +231,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
     // second pass over the shells: phi into column lane, d phi / d zeta into column opCol(lane) of the tile
     double *const tile = ws;
     double *const tl = tile + lane, *const tz = tile + GE::opCol(lane);
+    for (int comp = 0; comp < (nuc ? 3 : 1); ++comp) {
     int chunk = 0;
     double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1.0, r = 1.0;
     for (int s = 0; s < P.n_shell; ++s) {
@@ -243,29 +249,39 @@ __global__ void __launch_bounds__(WPB * 32, 1)
       if (meta & kMetaK1) gr *= r;
       if (meta & kMetaK2) gr *= r2;
       const double zf = sh.dlnN - r;  // d ln phi / d zeta
+      // nuclear mode: phi = ang(d) r^k e^{-zeta r}, d phi / d r_c = gr d ang / d d_c + ang gr (k / r^2 - zeta / r) d_c
+      const double dcmp = (comp == 0) ? dx : ((comp == 1) ? dy : dz);
+      const double radc = (sh.kd / r2 - sh.zeta / r) * dcmp;
       const int row = (meta >> 12) & 15, m = (meta >> 8) & 15;
-      double ang[5];
+      double ang[5], dang[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
       int nf = 1;
       if (kind == SH_S) {
         ang[0] = 1.0;
       } else if (kind == SH_P) {
         ang[0] = dx; ang[1] = dy; ang[2] = dz; nf = 3;
+        dang[0] = (comp == 0) ? 1.0 : 0.0; dang[1] = (comp == 1) ? 1.0 : 0.0; dang[2] = (comp == 2) ? 1.0 : 0.0;
       } else if (kind == SH_P1) {
         ang[0] = (m == 0) ? dx : ((m == 1) ? dy : dz);
+        dang[0] = (m == comp) ? 1.0 : 0.0;
       } else {
         const double dd[5] = {dx * dy, dy * dz, dz * dx, fma(dx, dx, -dy * dy), fma(2.0 * dz, dz, -fma(dx, dx, dy * dy))};
+        // gradients of {xy, yz, zx, x^2 - y^2, 2 z^2 - x^2 - y^2}
+        const double gd[5] = {(comp == 0) ? dy : ((comp == 1) ? dx : 0.0), (comp == 0) ? 0.0 : ((comp == 1) ? dz : dy),
+                              (comp == 0) ? dz : ((comp == 1) ? 0.0 : dx), (comp == 0) ? 2.0 * dx : ((comp == 1) ? -2.0 * dy : 0.0),
+                              (comp == 0) ? -2.0 * dx : ((comp == 1) ? -2.0 * dy : 4.0 * dz)};
         if (kind == SH_D) {
 #pragma unroll
-          for (int t = 0; t < 5; ++t) ang[t] = dd[t];
+          for (int t = 0; t < 5; ++t) { ang[t] = dd[t]; dang[t] = gd[t]; }
           nf = 5;
         } else {
           ang[0] = dd[m < 5 ? m : 0];
+          dang[0] = gd[m < 5 ? m : 0];
         }
       }
       for (int t = 0; t < nf; ++t) {
         const double phi = gr * ang[t];
         tl[(row + t) * S] = phi;
-        tz[(row + t) * S] = phi * zf;
+        tz[(row + t) * S] = nuc ? fma(gr, dang[t], phi * radc) : phi * zf;
       }
       const int flush = meta >> 20;
       if (flush) {
@@ -288,6 +304,8 @@ __global__ void __launch_bounds__(WPB * 32, 1)
           for (int i = 0; i < 2 * NS; ++i) gam[i] = (pv && i < ne) ? sGam[(gg * ne + i) * NMO + col] : 0.0;
           const int64_t orow = wo * P.n_ao;
           const int ocol = P.mo_orig[col < NMO ? col : 0];
+          double racc = 0.0;  // nuclear mode: running sum over the rows of centre cur
+          int cur = -1;
           for (int rw = 0; rw < kChunk; ++rw) {
             const int R = chunk * kChunk + rw, beta = P.ao_orig[R];
             if (beta < 0) continue;
@@ -300,20 +318,89 @@ __global__ void __launch_bounds__(WPB * 32, 1)
                 u = fma(trow[GE::opCol(gg * ne + i)], gam[i], u);
               }
             if (dC && ok) dC[(orow + beta) * P.n_mo_all + ocol] = P.ao_nrm[R] * t;
-            if (dZ) {
+            if (dZ || nuc) {
               // kernel-order (N C)[R][col] from the DMMA B-fragment table
               double a = ok ? cfr[(((rw >> 2) * NT) + (col >> 3)) * 32 + 4 * (col & 7) + (rw & 3)] * u : 0.0;
 #pragma unroll
               for (int m = 1; m < CW; m <<= 1) a += shfl_xor_d(a, m);
-              if (pv && col == 0 && wo < io.M) dZ[orow + beta] = a;
+              if (nuc) {
+                // the same lane owns walker gg in every chunk and component, so its read-modify-writes are ordered
+                const int at = row_atom[R];
+                if (at != cur) {
+                  if (cur >= 0 && pv && col == 0 && wo < io.M) dRo[(wo * P.n_atoms + cur) * 3 + comp] -= racc;
+                  cur = at;
+                  racc = 0.0;
+                }
+                racc += a;
+              } else if (pv && col == 0 && wo < io.M) {
+                dZ[orow + beta] = a;
+              }
             }
           }
+          if (nuc && cur >= 0 && pv && col == 0 && wo < io.M) dRo[(wo * P.n_atoms + cur) * 3 + comp] -= racc;
         }
         __syncwarp();
         ++chunk;
       }
     }
     __syncwarp();
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------
+// Nuclear dependence of the Jastrow factor (eq. 7's grad_alpha ln rho): dR[w][a][c] = d J / d R_a,c
+//   D.2: K(r_ia) = (w0 r + w1 r^2) / (1 + w2 r)              ->  -K' e_ai
+//   D.3: c f(r_ai) g(r_aj) h(r_ij), ordered pairs i != j      ->  -c h (f' g e_ai + f g' e_aj)
+// One thread per walker (SoA loads coalesce); writes every entry, zeros without those kernels.  The AO part is
+// subtracted afterwards by orbital_derivatives_kernel in nuclear mode.
+// ---------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128)
+    nuclear_jastrow_gradient_kernel(const __grid_constant__ SysParams P, const double *__restrict__ rin, const int64_t M,
+                                    double *__restrict__ dR) {
+  const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= M) return;
+  const int ne = P.n_e;
+  for (int a = 0; a < P.n_atoms; ++a) {
+    const double X = P.atom[a][0], Y = P.atom[a][1], Z = P.atom[a][2];
+    double gx = 0.0, gy = 0.0, gz = 0.0;
+    for (int i = 0; i < ne; ++i) {
+      const double xi = rin[((int64_t)i * 3 + 0) * M + w], yi = rin[((int64_t)i * 3 + 1) * M + w],
+                   zi = rin[((int64_t)i * 3 + 2) * M + w];
+      const double ax = xi - X, ay = yi - Y, az = zi - Z;
+      const double rai = sqrt(fma(ax, ax, fma(ay, ay, az * az)));
+      if (P.has_en) {
+        const double N = fma(P.en_w1 * rai, rai, P.en_w0 * rai), D = fma(P.en_w2, rai, 1.0);
+        const double K1 = (fma(2.0 * P.en_w1, rai, P.en_w0) * D - N * P.en_w2) / (D * D * rai);
+        gx = fma(-K1, ax, gx);
+        gy = fma(-K1, ay, gy);
+        gz = fma(-K1, az, gz);
+      }
+      if (P.n_een > 0)
+        for (int j = 0; j < ne; ++j) {
+          if (j == i) continue;
+          const double xj = rin[((int64_t)j * 3 + 0) * M + w], yj = rin[((int64_t)j * 3 + 1) * M + w],
+                       zj = rin[((int64_t)j * 3 + 2) * M + w];
+          const double bx = xj - X, by = yj - Y, bz = zj - Z;
+          const double ex = xi - xj, ey = yi - yj, ez = zi - zj;
+          const double raj = sqrt(fma(bx, bx, fma(by, by, bz * bz))), rij = sqrt(fma(ex, ex, fma(ey, ey, ez * ez)));
+          for (int mu = 0; mu < P.n_een; ++mu) {
+            const double *q = P.een[mu];
+            const double Df = fma(q[2], rai, 1.0), Dg = fma(q[4], raj, 1.0), Dh = fma(q[6], rij, 1.0);
+            const double f = q[1] * rai / Df, f1 = q[1] / (Df * Df);
+            const double g = q[3] * raj / Dg, g1 = q[3] / (Dg * Dg);
+            const double ch = q[0] * q[5] * rij / Dh;
+            const double ti = ch * f1 * g / rai, tj = ch * f * g1 / raj;
+            gx -= fma(ti, ax, tj * bx);
+            gy -= fma(ti, ay, tj * by);
+            gz -= fma(ti, az, tj * bz);
+          }
+        }
+    }
+    double *o = dR + (w * P.n_atoms + a) * 3;
+    o[0] = gx;
+    o[1] = gy;
+    o[2] = gz;
   }
 }
 

@@ -807,3 +807,104 @@ def test_orbital_derivatives_are_repeatable_bit_for_bit(env):
         b = s.orbital_derivatives(rg, d.n_ao, d.n_mo)
         assert torch.equal(a[0], b[0]) and torch.equal(a[1], b[1])
     s.close()
+
+
+# ----------------------------------------------------------------------------- nuclear log-gradient (eq. 7)
+def check_nuclear_log_gradient(env, d, r, threads=8):
+    torch, ob, qb = env
+    o = ob.OracleSystem(d)
+    lp0 = ob.local_energy(o, r, threads=threads)[0]
+    g0 = ob.nuclear_log_gradient(o, r, threads=threads)
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    g = s.nuclear_log_gradient(rg, d.n_atoms)
+    g2 = s.nuclear_log_gradient(rg, d.n_atoms)
+    assert torch.equal(g, g2)                         # deterministic
+    g = g.cpu().numpy()
+    s.close()
+    assert g.shape == g0.shape
+    keep = lp0 - lp0.max() > math.log(1e-6)
+    err = np.abs(g - g0) / np.maximum(1.0, np.abs(g0))
+    assert np.max(err[keep]) < 1e-8, np.max(err[keep])
+    return g
+
+
+@pytest.mark.parametrize("name,M", [("H2", 515), ("LiH", 300), ("Li2", 257), ("CO", 129)])
+@pytest.mark.parametrize("many_body", [False, True])
+def test_nuclear_log_gradient_configs(env, name, M, many_body):
+    d, r = wl.CONFIGS[name](M=M)
+    if many_body:
+        d = _with_een(_with_en(d, 0.3, -0.05, 0.7))
+    check_nuclear_log_gradient(env, d, r)
+
+
+def test_nuclear_log_gradient_odd_system_and_determinant_classes(env):
+    rng = np.random.default_rng(31)
+    aos = [(2, 1, 2, 1.1), (1, 0, 0, 2.0), (3, 2, 3, 0.9), (2, 1, 0, 1.3), (3, 2, 1, 0.7), (2, 0, 0, 1.5),
+           (3, 0, 0, 1.2), (3, 1, 1, 0.8), (2, 1, 1, 1.3)]
+    C = rng.standard_normal((len(aos), 7))
+    for norm in (None, rng.uniform(0.5, 2, len(aos))):
+        d = atom_system(3.0, aos, C, 3, 2, det_up=[[4, 0, 2], [4, 5, 2], [1, 0, 2], [4, 3, 5]],
+                        det_dn=[[1, 3], [1, 3], [0, 3], [1, 2]], ci=[0.9, 0.2, -0.3, 0.15], norm=norm,
+                        a_par=0.25, a_anti=0.5, b=0.8, xyz=(0.1, -0.2, 0.3))
+        r = soa(rng.standard_normal((131, 5, 3)) * 1.5)
+        check_nuclear_log_gradient(env, _with_en(d, -0.4, 0.1, 1.3), r, threads=2)
+    for with_general in (False, True):
+        rng = np.random.default_rng(77)
+        d = _classes_system(rng, with_general)
+        r = soa(rng.standard_normal((203, 7, 3)) * 1.2 + np.array([0.2, 0.1, -0.3]))
+        check_nuclear_log_gradient(env, d, r, threads=4)
+
+
+def test_nuclear_log_gradient_full_size_sampled_and_translation_invariance(env):
+    """CO at the size bench.py times the derivative calls (32768 walkers), D.2 and D.3 on: sampled walkers against
+    the oracle; on every walker sum_a grad_a ln|Psi| = -sum_i grad_i ln|Psi|, the right side by central differences
+    of the GPU's own log|Psi| under a rigid shift of all electrons."""
+    torch, ob, qb = env
+    M = 32768
+    d, r = wl.co(M=M)
+    d = _with_een(_with_en(d, 0.3, -0.05, 0.7))
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    g = s.nuclear_log_gradient(rg, d.n_atoms)
+    lp = s.log_psi(rg)[0]
+    idx = np.unique(np.concatenate([np.arange(0, 32), np.arange(M - 33, M), np.random.default_rng(2).integers(0, M, 256)]))
+    o = ob.OracleSystem(d)
+    rs = np.ascontiguousarray(r[:, :, idx])
+    lp0 = ob.local_energy(o, rs, threads=os.cpu_count() or 8)[0]
+    g0 = ob.nuclear_log_gradient(o, rs, threads=os.cpu_count() or 8)
+    keep = lp0 - float(lp.max()) > math.log(1e-6)
+    gn = g[torch.from_numpy(idx).cuda()].cpu().numpy()
+    assert np.max((np.abs(gn - g0) / np.maximum(1.0, np.abs(g0)))[keep]) < 1e-8
+    good = lp - lp.max() > math.log(1e-6)
+    h = 1e-4
+    for c in range(3):
+        def shifted(t):
+            r2 = rg.clone()
+            r2[:, c, :] += t
+            return s.log_psi(r2)[0]
+        cd = lambda hh: (shifted(hh) - shifted(-hh)) / (2 * hh)
+        c1, c2 = cd(h), cd(2 * h)
+        ref = (4 * c1 - c2) / 3
+        # the differences are only trusted where the two step sizes agree (not next to a nucleus' cusp or a node)
+        smooth = good & ((c1 - c2).abs() < 1e-4 * torch.clamp(ref.abs(), min=1.0))
+        assert float(smooth.sum()) > 0.98 * float(good.sum())
+        tot = g[:, :, c].sum(dim=1)
+        rel = (tot + ref).abs() / torch.clamp(ref.abs(), min=1.0)
+        assert float(rel[smooth].max()) < 1e-5, float(rel[smooth].max())
+    s.close()
+
+
+def test_nuclear_log_gradient_near_singular_reference(env):
+    rng = np.random.default_rng(78)
+    aos = [(1, 0, 0, 2.5), (2, 0, 0, 1.0), (3, 0, 0, 0.7), (2, 1, 0, 1.2), (2, 1, 1, 1.2), (2, 1, 2, 1.2)]
+    C = np.zeros((6, 6))
+    C[:3, :2] = rng.standard_normal((3, 2))
+    C[:, 2:] = rng.standard_normal((6, 4))
+    d = atom_system(3.0, aos, C, 2, 1, det_up=[[0, 1], [0, 2], [3, 1], [2, 4], [5, 3]], det_dn=[[0], [0], [1], [0], [2]],
+                    ci=[0.7, 0.3, -0.2, 0.25, 0.1], a_par=0.25, a_anti=0.5, b=1.0)
+    r = rng.standard_normal((160, 3, 3)) * 1.3
+    for w in range(0, 160, 3):
+        u = rng.standard_normal(3)
+        r[w, 1] = u / np.linalg.norm(u) * np.linalg.norm(r[w, 0]) * (1.0 + 1e-5 * rng.uniform(0.5, 1.0))
+    check_nuclear_log_gradient(env, d, soa(r), threads=2)
