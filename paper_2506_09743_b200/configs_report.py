@@ -62,12 +62,13 @@ def measure(name, d, r_host, peak):
     t_el_d = _time(lambda: s.local_energy(rd))
     t_O = _time(lambda: s.log_derivatives(rd, O=O))
     t_orb = _time(lambda: s.orbital_derivatives(rd, d.n_ao, d.n_mo))
+    t_nuc = _time(lambda: s.nuclear_log_gradient(rd, d.n_atoms))
     f_el, f_st = s.model_flops(0), s.model_flops(1)
     row = dict(config=name, n_e=d.n_e, n_ao=d.n_ao, n_mo=d.n_mo, n_det=d.n_det, walkers=M, el_ms=1e3 * t_el, el_rate=M / t_el,
                el_tflops=f_el * M / t_el / 1e12, el_frac=f_el * M / t_el / 1e12 / peak, sweeps=sweeps,
                met_ms=1e3 * t_met, met_rate=M * sweeps / t_met, met_tflops=f_st * M * sweeps / t_met / 1e12,
                met_frac=f_st * M * sweeps / t_met / 1e12 / peak, deriv_walkers=Md, n_param=s.n_param(),
-               el_d_ms=1e3 * t_el_d, O_ms=1e3 * t_O, orb_ms=1e3 * t_orb)
+               el_d_ms=1e3 * t_el_d, O_ms=1e3 * t_O, orb_ms=1e3 * t_orb, nuc_ms=1e3 * t_nuc)
     s.close()
     return row
 
@@ -133,11 +134,11 @@ def main():
               f"{x['el_rate'] / 1e6:.1f} | {x['el_tflops']:.2f} | {100 * x['el_frac']:.1f} % | {x['sweeps']} | "
               f"{x['met_ms']:.3f} | {x['met_rate'] / 1e6:.1f} | {x['met_tflops']:.2f} | {100 * x['met_frac']:.1f} % |")
     print("\nParameter derivatives (eq. 6 factors), same sampled walkers, device time per call:")
-    print("| config | walkers | E_L ms | n_param | E_L + O_p ms | orbital parameters (N_AO x N_MO + N_AO) | dC, dzeta ms |")
-    print("|---|---|---|---|---|---|---|")
+    print("| config | walkers | E_L ms | n_param | E_L + O_p ms | orbital parameters (N_AO x N_MO + N_AO) | dC, dzeta ms | grad_R ln Psi ms |")
+    print("|---|---|---|---|---|---|---|---|")
     for x in rows:
         print(f"| {x['config']} | {x['deriv_walkers']} | {x['el_d_ms']:.3f} | {x['n_param']} | {x['O_ms']:.3f} | "
-              f"{x['n_ao']} x {x['n_mo']} + {x['n_ao']} | {x['orb_ms']:.3f} |")
+              f"{x['n_ao']} x {x['n_mo']} + {x['n_ao']} | {x['orb_ms']:.3f} | {x['nuc_ms']:.3f} |")
     print("\nAccelerated (excitation tables, F.6/F.7) vs explicit per-determinant E_L (PAPER.md:345-349, Fig. 11), CO shape:")
     print("| N_det | walkers | tables ms | explicit ms | explicit / tables |")
     print("|---|---|---|---|---|")

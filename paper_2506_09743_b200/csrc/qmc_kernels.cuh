@@ -194,8 +194,9 @@ __global__ void __launch_bounds__(WPB * 32, 1)
   const int64_t n_groups = (io.M + G - 1) / G;
   const int64_t stride = (int64_t)gridDim.x * WPB;
   double *dC = io.logpsi, *dZ = io.eloc;
-  // nuclear mode (qmc_nuclear_log_gradient): io.O = dR [M][n_atoms][3]; the second pass runs once per Cartesian
-  // component with d phi / d R_c = -d phi / d r_c in the operator columns, summed over the rows of each centre
+  // nuclear mode (qmc_nuclear_log_gradient): io.O = dR [M][n_atoms][3]; d phi / d R_c = -d phi / d r_c takes the place of
+  // phi and d phi / d zeta in the two column sets of the tile: the second pass runs twice, (x, y) then z, and the
+  // contraction is summed over the rows of each centre
   double *dRo = io.O;
   constexpr bool nuc = NUC;  // its own instantiation: the parameter-derivative kernel keeps its code and registers
   const int *row_atom = P.ao_orig + P.n_chunks * kChunk;
@@ -231,7 +232,8 @@ __global__ void __launch_bounds__(WPB * 32, 1)
     // second pass over the shells: phi into column lane, d phi / d zeta into column opCol(lane) of the tile
     double *const tile = ws;
     double *const tl = tile + lane, *const tz = tile + GE::opCol(lane);
-    for (int comp = 0; comp < (nuc ? 3 : 1); ++comp) {
+    for (int pass = 0; pass < (nuc ? 2 : 1); ++pass) {
+    const int comp = pass + 1;  // nuclear mode: component of the operator columns (y, then z); x rides in the phi columns of pass 0
     int chunk = 0;
     double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1.0, r = 1.0;
     for (int s = 0; s < P.n_shell; ++s) {
@@ -251,36 +253,40 @@ __global__ void __launch_bounds__(WPB * 32, 1)
       const double zf = sh.dlnN - r;  // d ln phi / d zeta
       // nuclear mode: phi = ang(d) r^k e^{-zeta r}, d phi / d r_c = gr d ang / d d_c + ang gr (k / r^2 - zeta / r) d_c
       const double dcmp = (comp == 0) ? dx : ((comp == 1) ? dy : dz);
-      const double radc = (sh.kd / r2 - sh.zeta / r) * dcmp;
+      const double rad0 = sh.kd / r2 - sh.zeta / r;
+      const double radc = rad0 * dcmp, radx = rad0 * dx;
       const int row = (meta >> 12) & 15, m = (meta >> 8) & 15;
-      double ang[5], dang[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+      double ang[5], dang[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, dax[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
       int nf = 1;
       if (kind == SH_S) {
         ang[0] = 1.0;
       } else if (kind == SH_P) {
         ang[0] = dx; ang[1] = dy; ang[2] = dz; nf = 3;
-        dang[0] = (comp == 0) ? 1.0 : 0.0; dang[1] = (comp == 1) ? 1.0 : 0.0; dang[2] = (comp == 2) ? 1.0 : 0.0;
+        dang[1] = (comp == 1) ? 1.0 : 0.0; dang[2] = (comp == 2) ? 1.0 : 0.0;
+        dax[0] = 1.0;
       } else if (kind == SH_P1) {
         ang[0] = (m == 0) ? dx : ((m == 1) ? dy : dz);
         dang[0] = (m == comp) ? 1.0 : 0.0;
+        dax[0] = (m == 0) ? 1.0 : 0.0;
       } else {
         const double dd[5] = {dx * dy, dy * dz, dz * dx, fma(dx, dx, -dy * dy), fma(2.0 * dz, dz, -fma(dx, dx, dy * dy))};
         // gradients of {xy, yz, zx, x^2 - y^2, 2 z^2 - x^2 - y^2}
-        const double gd[5] = {(comp == 0) ? dy : ((comp == 1) ? dx : 0.0), (comp == 0) ? 0.0 : ((comp == 1) ? dz : dy),
-                              (comp == 0) ? dz : ((comp == 1) ? 0.0 : dx), (comp == 0) ? 2.0 * dx : ((comp == 1) ? -2.0 * dy : 0.0),
-                              (comp == 0) ? -2.0 * dx : ((comp == 1) ? -2.0 * dy : 4.0 * dz)};
+        const double gd[5] = {(comp == 1) ? dx : 0.0, (comp == 1) ? dz : dy, (comp == 1) ? 0.0 : dx,
+                              (comp == 1) ? -2.0 * dy : 0.0, (comp == 1) ? -2.0 * dy : 4.0 * dz};
+        const double gx[5] = {dy, 0.0, dz, 2.0 * dx, -2.0 * dx};
         if (kind == SH_D) {
 #pragma unroll
-          for (int t = 0; t < 5; ++t) { ang[t] = dd[t]; dang[t] = gd[t]; }
+          for (int t = 0; t < 5; ++t) { ang[t] = dd[t]; dang[t] = gd[t]; dax[t] = gx[t]; }
           nf = 5;
         } else {
           ang[0] = dd[m < 5 ? m : 0];
           dang[0] = gd[m < 5 ? m : 0];
+          dax[0] = gx[m < 5 ? m : 0];
         }
       }
       for (int t = 0; t < nf; ++t) {
         const double phi = gr * ang[t];
-        tl[(row + t) * S] = phi;
+        tl[(row + t) * S] = nuc ? fma(gr, dax[t], phi * radx) : phi;
         tz[(row + t) * S] = nuc ? fma(gr, dang[t], phi * radc) : phi * zf;
       }
       const int flush = meta >> 20;
@@ -304,7 +310,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
           for (int i = 0; i < 2 * NS; ++i) gam[i] = (pv && i < ne) ? sGam[(gg * ne + i) * NMO + col] : 0.0;
           const int64_t orow = wo * P.n_ao;
           const int ocol = P.mo_orig[col < NMO ? col : 0];
-          double racc = 0.0;  // nuclear mode: running sum over the rows of centre cur
+          double racc = 0.0, racx = 0.0;  // nuclear mode: running sums (component comp, x) over the rows of centre cur
           int cur = -1;
           for (int rw = 0; rw < kChunk; ++rw) {
             const int R = chunk * kChunk + rw, beta = P.ao_orig[R];
@@ -314,30 +320,44 @@ __global__ void __launch_bounds__(WPB * 32, 1)
 #pragma unroll
             for (int i = 0; i < 2 * NS; ++i)
               if (i < ne) {
-                t = fma(trow[gg * ne + i], gam[i], t);
+                if (!nuc || pass == 0) t = fma(trow[gg * ne + i], gam[i], t);
                 u = fma(trow[GE::opCol(gg * ne + i)], gam[i], u);
               }
             if (dC && ok) dC[(orow + beta) * P.n_mo_all + ocol] = P.ao_nrm[R] * t;
             if (dZ || nuc) {
               // kernel-order (N C)[R][col] from the DMMA B-fragment table
-              double a = ok ? cfr[(((rw >> 2) * NT) + (col >> 3)) * 32 + 4 * (col & 7) + (rw & 3)] * u : 0.0;
+              const double cf = ok ? cfr[(((rw >> 2) * NT) + (col >> 3)) * 32 + 4 * (col & 7) + (rw & 3)] : 0.0;
+              double a = cf * u;
 #pragma unroll
               for (int m = 1; m < CW; m <<= 1) a += shfl_xor_d(a, m);
               if (nuc) {
-                // the same lane owns walker gg in every chunk and component, so its read-modify-writes are ordered
+                double ax = (pass == 0) ? cf * t : 0.0;
+                if (pass == 0) {
+#pragma unroll
+                  for (int m = 1; m < CW; m <<= 1) ax += shfl_xor_d(ax, m);
+                }
+                // the same lane owns walker gg in every chunk and pass, so its read-modify-writes are ordered
                 const int at = row_atom[R];
                 if (at != cur) {
-                  if (cur >= 0 && pv && col == 0 && wo < io.M) dRo[(wo * P.n_atoms + cur) * 3 + comp] -= racc;
+                  if (cur >= 0 && pv && col == 0 && wo < io.M) {
+                    dRo[(wo * P.n_atoms + cur) * 3 + comp] -= racc;
+                    if (pass == 0) dRo[(wo * P.n_atoms + cur) * 3] -= racx;
+                  }
                   cur = at;
                   racc = 0.0;
+                  racx = 0.0;
                 }
                 racc += a;
+                racx += ax;
               } else if (pv && col == 0 && wo < io.M) {
                 dZ[orow + beta] = a;
               }
             }
           }
-          if (nuc && cur >= 0 && pv && col == 0 && wo < io.M) dRo[(wo * P.n_atoms + cur) * 3 + comp] -= racc;
+          if (nuc && cur >= 0 && pv && col == 0 && wo < io.M) {
+            dRo[(wo * P.n_atoms + cur) * 3 + comp] -= racc;
+            if (pass == 0) dRo[(wo * P.n_atoms + cur) * 3] -= racx;
+          }
         }
         __syncwarp();
         ++chunk;
