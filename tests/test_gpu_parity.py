@@ -908,3 +908,45 @@ def test_nuclear_log_gradient_near_singular_reference(env):
         u = rng.standard_normal(3)
         r[w, 1] = u / np.linalg.norm(u) * np.linalg.norm(r[w, 0]) * (1.0 + 1e-5 * rng.uniform(0.5, 1.0))
     check_nuclear_log_gradient(env, d, soa(r), threads=2)
+
+
+def test_nuclear_log_gradient_edge_sizes_and_a_centre_without_basis_functions(env):
+    import copy
+    torch, ob, qb = env
+    # H2 with both AOs moved to the first nucleus: the second centre is seen by V_en and D.2 only
+    d, r = wl.h2(M=33)
+    d = copy.copy(d)
+    d.ao_atom = np.zeros_like(np.asarray(d.ao_atom))
+    g = check_nuclear_log_gradient(env, _with_en(d, 0.3, -0.05, 0.7), r, threads=1)
+    assert np.abs(g[:, 1]).max() > 1e-3
+    d0 = copy.copy(d)                                   # without D.2 that centre's gradient is exactly zero
+    g = check_nuclear_log_gradient(env, d0, r, threads=1)
+    assert np.all(g[:, 1] == 0.0)
+    for name, M in (("H2", 1), ("LiH", 1), ("Li2", 3), ("CO", 1), ("CO", 2)):
+        dd, rr = wl.CONFIGS[name](M=M)
+        check_nuclear_log_gradient(env, dd, rr, threads=1)
+    s = qb.QmcSystem(d)
+    with pytest.raises(qb.QmcError):
+        s.nuclear_log_gradient(torch.empty((2, 3, 0), dtype=torch.float64, device="cuda"), d.n_atoms)
+    s.close()
+
+
+def test_force_estimator_second_term_through_the_eq6_reduction(env):
+    """Eq. 7 (DESIGN.md section 12 reading): F_alpha = -<grad_alpha E_L> - <(E_L - E_v) grad_alpha ln rho>.
+    The second (Pulay) term is eq. 6's reduction with O = grad_alpha ln|Psi|: -(2/M) sum (E_L - E_v) grad_alpha ln|Psi|,
+    so qmc_energy_gradient serves it; against the oracle's E_L, gradient and reduction on the same walkers."""
+    torch, ob, qb = env
+    d, r = wl.li2(M=2048)
+    o = ob.OracleSystem(d)
+    el0 = ob.local_energy(o, r, threads=os.cpu_count() or 8)[2]
+    g0 = ob.nuclear_log_gradient(o, r, threads=os.cpu_count() or 8)
+    ev0, f0 = ob.energy_gradient(el0, g0.reshape(len(el0), -1))
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    el = s.local_energy(rg)[2]
+    g = s.nuclear_log_gradient(rg, d.n_atoms)
+    ev, f = qb.energy_gradient(el, g.reshape(g.shape[0], -1))
+    s.close()
+    assert abs(ev - ev0) < 1e-10 * abs(ev0)
+    assert np.max(np.abs(f - f0) / np.maximum(1.0, np.abs(f0))) < 1e-8
+    assert np.isfinite(f).all() and np.abs(f).max() > 0
