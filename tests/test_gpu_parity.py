@@ -950,3 +950,28 @@ def test_force_estimator_second_term_through_the_eq6_reduction(env):
     assert abs(ev - ev0) < 1e-10 * abs(ev0)
     assert np.max(np.abs(f - f0) / np.maximum(1.0, np.abs(f0))) < 1e-8
     assert np.isfinite(f).all() and np.abs(f).max() > 0
+
+
+@pytest.mark.parametrize("name,M", [("H2", 70), ("LiH", 37), ("Li2", 23), ("CO", 9)])
+def test_nuclear_log_gradient_writes_exactly_its_output(env, name, M):
+    """Guard words around dR stay untouched and every entry inside is written (NaN-filled before the call); the
+    walker coordinates are not modified.  Raw C-ABI call with a pointer into the middle of a larger buffer."""
+    torch, ob, qb = env
+    d, r = wl.CONFIGS[name](M=M)
+    d = _with_een(_with_en(d, 0.3, -0.05, 0.7))
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    r_before = rg.clone()
+    n, pad = M * d.n_atoms * 3, 4096
+    buf = torch.full((n + 2 * pad,), float("nan"), dtype=torch.float64, device="cuda")
+    buf[:pad] = 12345.0
+    buf[pad + n:] = 12345.0
+    rc = qb.lib().qmc_nuclear_log_gradient(s._h, rg.data_ptr(), M, buf.data_ptr() + 8 * pad,
+                                           torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert rc == 0
+    assert bool((buf[:pad] == 12345.0).all()) and bool((buf[pad + n:] == 12345.0).all())
+    assert bool(torch.isfinite(buf[pad:pad + n]).all())
+    assert torch.equal(rg, r_before)
+    assert torch.equal(buf[pad:pad + n].view(M, d.n_atoms, 3), s.nuclear_log_gradient(rg, d.n_atoms))
+    s.close()
