@@ -17,18 +17,22 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libqmc_oracle.so")
+_SO_LD = os.path.join(_HERE, "libqmc_oracle_ld.so")  # the same source with real = long double (the adjudicator)
 _SRC = os.path.join(_HERE, "qmc_oracle.c")
 _lock = threading.Lock()
-_lib = None
+_libs = {}
 
 
 def build(force: bool = False) -> str:
-    """Compile the oracle with gcc -O2 (no fast-math, no contraction)."""
+    """Compile the oracle with gcc -O2 (no fast-math, no contraction): the float64 build and, from the same
+    source, the extended-precision build (-DORACLE_REAL="long double", x87 80-bit) that adjudicates walkers on
+    which two float64 evaluations cannot agree to the parity bound (reading Q24)."""
     hdr = os.path.join(_HERE, "qmc_oracle.h")
-    stale = (not os.path.exists(_SO)) or any(os.path.getmtime(f) > os.path.getmtime(_SO) for f in (_SRC, hdr))
-    if force or stale:
-        subprocess.check_call(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fPIC", "-shared",
-                               "-o", _SO, _SRC, "-lm"])
+    for so, extra in ((_SO, []), (_SO_LD, ['-DORACLE_REAL=long double'])):
+        stale = (not os.path.exists(so)) or any(os.path.getmtime(f) > os.path.getmtime(so) for f in (_SRC, hdr))
+        if force or stale:
+            subprocess.check_call(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fPIC", "-shared"] + extra +
+                                  ["-o", so, _SRC, "-lm"])
     return _SO
 
 
@@ -46,12 +50,12 @@ class _Desc(C.Structure):
     ]
 
 
-def lib():
-    global _lib
+def lib(extended: bool = False):
+    """The float64 oracle, or with extended=True the long-double build of the same source."""
     with _lock:
-        if _lib is None:
+        if extended not in _libs:
             build()
-            L = C.CDLL(_SO)
+            L = C.CDLL(_SO_LD if extended else _SO)
             L.oracle_sto_norm.restype = C.c_double
             L.oracle_sto_norm.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double]
             L.oracle_det_inv.restype = C.c_double
@@ -82,8 +86,8 @@ def lib():
             L.oracle_nuclear_log_gradient.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p]
             L.oracle_energy_gradient.restype = None
             L.oracle_energy_gradient.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
-            _lib = L
-    return _lib
+            _libs[extended] = L
+    return _libs[extended]
 
 
 def _p(a):
@@ -93,7 +97,8 @@ def _p(a):
 class OracleSystem:
     """Holds contiguous copies of the description arrays + the C struct."""
 
-    def __init__(self, d):
+    def __init__(self, d, extended: bool = False):
+        self.L = lib(extended)
         f64 = lambda a: np.ascontiguousarray(a, np.float64)
         i32 = lambda a: np.ascontiguousarray(a, np.int32)
         self.n_up, self.n_dn = int(d.n_up), int(d.n_dn)
@@ -140,14 +145,14 @@ def det_inv(A):
 def ao_eval(sysd: OracleSystem, ao: int, xyz):
     xyz = np.ascontiguousarray(xyz, np.float64)
     out = np.empty(5)
-    lib().oracle_ao_eval(sysd.ref, ao, _p(xyz), _p(out))
+    sysd.L.oracle_ao_eval(sysd.ref, ao, _p(xyz), _p(out))
     return out
 
 
 def psi_plain(sysd: OracleSystem, r_aos):
     """r_aos: [n_e,3] one walker."""
     r = np.ascontiguousarray(r_aos, np.float64)
-    return lib().oracle_psi_plain(sysd.ref, _p(r))
+    return sysd.L.oracle_psi_plain(sysd.ref, _p(r))
 
 
 def local_energy(sysd: OracleSystem, r_soa, threads: int = 1, parts: bool = False):
@@ -156,7 +161,7 @@ def local_energy(sysd: OracleSystem, r_soa, threads: int = 1, parts: bool = Fals
     M = r.shape[2]
     lp, sg, el = np.empty(M), np.empty(M), np.empty(M)
     pt = np.empty((M, 4)) if parts else None
-    L = lib()
+    L = sysd.L
 
     def run(rng):
         rc = L.oracle_local_energy(sysd.ref, _p(r), M, rng[0], rng[1], _p(lp), _p(sg), _p(el), _p(pt))
@@ -195,7 +200,7 @@ def metropolis(sysd: OracleSystem, r_soa, step, n_sweeps, seed, sweep_offset=0, 
     acc = np.zeros((n_sweeps, M), np.uint8)
     mg = np.zeros((n_sweeps, M))
     ea = np.zeros(M) if want_eloc_acc else None
-    L = lib()
+    L = sysd.L
 
     def run(rng):
         rc = L.oracle_metropolis(sysd.ref, _p(r), M, rng[0], rng[1], step, n_sweeps, seed, sweep_offset,
@@ -224,7 +229,7 @@ def log_derivatives(sysd: OracleSystem, r_soa, threads: int = 1):
     r = np.ascontiguousarray(r_soa, np.float64)
     M = r.shape[2]
     O = np.empty((M, 6 + 7 * int(sysd.c.n_een) + int(sysd.c.n_det)))
-    L = lib()
+    L = sysd.L
 
     def run(rng):
         rc = L.oracle_log_derivatives(sysd.ref, _p(r), M, rng[0], rng[1], _p(O))
@@ -255,7 +260,7 @@ def orbital_derivatives(sysd: OracleSystem, r_soa, threads: int = 1):
     M = r.shape[2]
     dC = np.empty((M, sysd.n_ao, int(sysd.c.n_mo)))
     dz = np.empty((M, sysd.n_ao))
-    L = lib()
+    L = sysd.L
 
     def run(rng):
         rc = L.oracle_orbital_derivatives(sysd.ref, _p(r), M, rng[0], rng[1], _p(dC), _p(dz))
@@ -275,7 +280,7 @@ def nuclear_log_gradient(sysd: OracleSystem, r_soa, threads: int = 1):
     r = np.ascontiguousarray(r_soa, np.float64)
     M = r.shape[2]
     dR = np.empty((M, int(sysd.c.n_atoms), 3))
-    L = lib()
+    L = sysd.L
 
     def run(rng):
         rc = L.oracle_nuclear_log_gradient(sysd.ref, _p(r), M, rng[0], rng[1], _p(dR))

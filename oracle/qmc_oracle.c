@@ -1,4 +1,4 @@
-/* qmc_oracle.c -- plain float64 CPU oracle (see qmc_oracle.h: test
+/* qmc_oracle.c -- plain CPU oracle, float64 unless built as the extended-precision adjudicator (see qmc_oracle.h: test
  * infrastructure only; shares nothing with the CUDA path).
  *
  * Build: gcc -O2 -std=c11 -fPIC -shared -o libqmc_oracle.so qmc_oracle.c -lm
@@ -6,7 +6,18 @@
  */
 #include "qmc_oracle.h"
 
-#include <math.h>
+/* Working precision.  The default build computes in float64 (`real` = double: the oracle proper).  The same source
+ * compiled with -DORACLE_REAL="long double" (libqmc_oracle_ld.so, x87 80-bit, 64-bit mantissa) is the EXTENDED run
+ * that adjudicates walkers on which two float64 evaluations cannot agree to the parity bound (a nearly singular
+ * Slater matrix: DESIGN.md section 2, reading Q24).  No algorithm changes with the type: <tgmath.h> selects the
+ * libm routine of the operand type.  Inputs and outputs of the API stay double; the random-number stream of the
+ * sampler stays float64 in both builds (it is part of the method's definition, reading Q9). */
+#ifndef ORACLE_REAL
+#define ORACLE_REAL double
+#endif
+typedef ORACLE_REAL real;
+
+#include <tgmath.h>
 #include <stdlib.h>
 #include <string.h>
 
@@ -18,16 +29,16 @@
 /* l=0:{1}; l=1:{x,y,z}; l=2:{xy,yz,zx,x^2-y^2,2z^2-x^2-y^2}.           */
 /* ------------------------------------------------------------------ */
 
-static double factorial(int n) {
-  double f = 1.0;
-  for (int i = 2; i <= n; ++i) f *= (double)i;
+static real factorial(int n) {
+  real f = 1.0;
+  for (int i = 2; i <= n; ++i) f *= (real)i;
   return f;
 }
 
-double oracle_sto_norm(int n, int l, int m, double zeta) {
+static real sto_norm_r(int n, int l, int m, real zeta) {
   /* radial: (2 zeta)^(n+1/2) / sqrt((2n)!) ; angular: real spherical harmonic constant */
-  double radial = pow(2.0 * zeta, (double)n + 0.5) / sqrt(factorial(2 * n));
-  double ang = 0.0;
+  real radial = pow(2.0 * zeta, (real)n + 0.5) / sqrt(factorial(2 * n));
+  real ang = 0.0;
   if (l == 0) ang = 1.0 / (2.0 * sqrt(ORACLE_PI));
   else if (l == 1) ang = sqrt(3.0 / (4.0 * ORACLE_PI));
   else if (l == 2) {
@@ -38,9 +49,11 @@ double oracle_sto_norm(int n, int l, int m, double zeta) {
   return radial * ang;
 }
 
+double oracle_sto_norm(int n, int l, int m, double zeta) { return (double)sto_norm_r(n, l, m, (real)zeta); }
+
 /* S, its gradient and its three pure second derivatives, written out. */
-static void solid_harmonic(int l, int m, double x, double y, double z, double *S, double g[3],
-                           double h[3]) {
+static void solid_harmonic(int l, int m, real x, real y, real z, real *S, real g[3],
+                           real h[3]) {
   *S = 0.0;
   g[0] = g[1] = g[2] = 0.0;
   h[0] = h[1] = h[2] = 0.0;
@@ -63,81 +76,87 @@ static void solid_harmonic(int l, int m, double x, double y, double z, double *S
   }
 }
 
-void oracle_ao_eval(const oracle_system_desc_t *s, int ao, const double *xyz, double *out5) {
+static void ao_eval_r(const oracle_system_desc_t *s, int ao, const real *xyz, real *out5) {
   int a = s->ao_atom[ao], n = s->ao_n[ao], l = s->ao_l[ao], m = s->ao_m[ao];
-  double zeta = s->ao_zeta[ao];
-  double N = s->ao_norm ? s->ao_norm[ao] : oracle_sto_norm(n, l, m, zeta);
-  double d[3];
+  real zeta = s->ao_zeta[ao];
+  real N = s->ao_norm ? s->ao_norm[ao] : sto_norm_r(n, l, m, zeta);
+  real d[3];
   for (int c = 0; c < 3; ++c) d[c] = xyz[c] - s->atom_xyz[3 * a + c];
-  double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+  real r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
   int k = n - 1 - l;
 
-  double S, gS[3], hS[3];
+  real S, gS[3], hS[3];
   solid_harmonic(l, m, d[0], d[1], d[2], &S, gS, hS);
 
   /* radial factor f(r) = r^k e^{-zeta r} and its first two derivatives, term by term */
-  double e = exp(-zeta * r);
-  double rk = pow(r, (double)k);                         /* r^k       */
-  double rk1 = (k >= 1) ? pow(r, (double)(k - 1)) : 0.0; /* r^(k-1)   */
-  double rk2 = (k >= 2) ? pow(r, (double)(k - 2)) : 0.0; /* r^(k-2)   */
-  double f = rk * e;
-  double f1 = ((double)k * rk1 - zeta * rk) * e;
-  double f2 = ((double)(k * (k - 1)) * rk2 - 2.0 * (double)k * zeta * rk1 + zeta * zeta * rk) * e;
+  real e = exp(-zeta * r);
+  real rk = pow(r, (real)k);                         /* r^k       */
+  real rk1 = (k >= 1) ? pow(r, (real)(k - 1)) : 0.0; /* r^(k-1)   */
+  real rk2 = (k >= 2) ? pow(r, (real)(k - 2)) : 0.0; /* r^(k-2)   */
+  real f = rk * e;
+  real f1 = ((real)k * rk1 - zeta * rk) * e;
+  real f2 = ((real)(k * (k - 1)) * rk2 - 2.0 * (real)k * zeta * rk1 + zeta * zeta * rk) * e;
 
   /* grad f = f' d/r ; lap f = f'' + 2 f'/r */
-  double gf[3];
+  real gf[3];
   for (int c = 0; c < 3; ++c) gf[c] = f1 * d[c] / r;
-  double lapf = f2 + 2.0 * f1 / r;
+  real lapf = f2 + 2.0 * f1 / r;
 
   /* product rule: grad(S f) = gS f + S gf ; lap(S f) = lapS f + 2 gS.gf + S lapf */
-  double lapS = hS[0] + hS[1] + hS[2];
-  double dot = gS[0] * gf[0] + gS[1] * gf[1] + gS[2] * gf[2];
+  real lapS = hS[0] + hS[1] + hS[2];
+  real dot = gS[0] * gf[0] + gS[1] * gf[1] + gS[2] * gf[2];
   out5[0] = N * S * f;
   for (int c = 0; c < 3; ++c) out5[1 + c] = N * (gS[c] * f + S * gf[c]);
   out5[4] = N * (lapS * f + 2.0 * dot + S * lapf);
+}
+
+void oracle_ao_eval(const oracle_system_desc_t *s, int ao, const double *xyz, double *out5) {
+  real p[3] = {xyz[0], xyz[1], xyz[2]}, o[5];
+  ao_eval_r(s, ao, p, o);
+  for (int q = 0; q < 5; ++q) out5[q] = (double)o[q];
 }
 
 /* ------------------------------------------------------------------ */
 /* Partial-pivot LU: determinant and inverse   */
 /* ------------------------------------------------------------------ */
 
-double oracle_det_inv(int n, const double *A, double *inv) {
+static real det_inv_r(int n, const real *A, real *inv) {
   if (n <= 0) return 1.0;
-  double *lu = (double *)malloc(sizeof(double) * (size_t)n * (size_t)n);
+  real *lu = (real *)malloc(sizeof(real) * (size_t)n * (size_t)n);
   int *perm = (int *)malloc(sizeof(int) * (size_t)n);
-  memcpy(lu, A, sizeof(double) * (size_t)n * (size_t)n);
+  memcpy(lu, A, sizeof(real) * (size_t)n * (size_t)n);
   for (int i = 0; i < n; ++i) perm[i] = i;
-  double det = 1.0;
+  real det = 1.0;
   for (int k = 0; k < n; ++k) {
     int p = k;
-    double best = fabs(lu[k * n + k]);
+    real best = fabs(lu[k * n + k]);
     for (int i = k + 1; i < n; ++i)
       if (fabs(lu[i * n + k]) > best) { best = fabs(lu[i * n + k]); p = i; }
     if (p != k) {
-      for (int j = 0; j < n; ++j) { double t = lu[k * n + j]; lu[k * n + j] = lu[p * n + j]; lu[p * n + j] = t; }
+      for (int j = 0; j < n; ++j) { real t = lu[k * n + j]; lu[k * n + j] = lu[p * n + j]; lu[p * n + j] = t; }
       int t = perm[k]; perm[k] = perm[p]; perm[p] = t;
       det = -det;
     }
-    double piv = lu[k * n + k];
+    real piv = lu[k * n + k];
     det *= piv;
     if (piv == 0.0) continue; /* singular: det = 0, inverse undefined (inf/nan follow) */
     for (int i = k + 1; i < n; ++i) {
       lu[i * n + k] /= piv;
-      double lik = lu[i * n + k];
+      real lik = lu[i * n + k];
       for (int j = k + 1; j < n; ++j) lu[i * n + j] -= lik * lu[k * n + j];
     }
   }
   if (inv) {
     /* solve A x = e_c for every unit vector: P A = L U */
-    double *y = (double *)malloc(sizeof(double) * (size_t)n);
+    real *y = (real *)malloc(sizeof(real) * (size_t)n);
     for (int c = 0; c < n; ++c) {
       for (int i = 0; i < n; ++i) {
-        double v = (perm[i] == c) ? 1.0 : 0.0;
+        real v = (perm[i] == c) ? 1.0 : 0.0;
         for (int j = 0; j < i; ++j) v -= lu[i * n + j] * y[j];
         y[i] = v;
       }
       for (int i = n - 1; i >= 0; --i) {
-        double v = y[i];
+        real v = y[i];
         for (int j = i + 1; j < n; ++j) v -= lu[i * n + j] * inv[j * n + c];
         inv[i * n + c] = v / lu[i * n + i];
       }
@@ -149,32 +168,45 @@ double oracle_det_inv(int n, const double *A, double *inv) {
   return det;
 }
 
+double oracle_det_inv(int n, const double *A, double *inv) {
+  if (n <= 0) return 1.0;
+  size_t nn = (size_t)n * (size_t)n;
+  real *a = (real *)malloc(sizeof(real) * nn), *ai = inv ? (real *)malloc(sizeof(real) * nn) : NULL;
+  for (size_t i = 0; i < nn; ++i) a[i] = A[i];
+  real det = det_inv_r(n, a, ai);
+  if (inv)
+    for (size_t i = 0; i < nn; ++i) inv[i] = (double)ai[i];
+  free(a);
+  free(ai);
+  return (double)det;
+}
+
 /* ------------------------------------------------------------------ */
 /* Pade e-e Jastrow (D.1; cusps C.1):       */
 /* K(r) = w0 r / (1 + w r), w0 = a_par (same spin), a_anti (opposite).  */
 /* ------------------------------------------------------------------ */
 
 static int spin_of(const oracle_system_desc_t *s, int i) { return i < s->n_up ? 0 : 1; }
-static void jastrow_een_add(const oracle_system_desc_t *s, const double *r, double *J, double *gJ, double *lapJ);
+static void jastrow_een_add(const oracle_system_desc_t *s, const real *r, real *J, real *gJ, real *lapJ);
 
 /* J, grad_i J [n_e][3], lap J (sum over all electrons), pair loop. r is AoS [n_e][3]. */
-static void jastrow_all(const oracle_system_desc_t *s, const double *r, double *J, double *gJ,
-                        double *lapJ) {
+static void jastrow_all(const oracle_system_desc_t *s, const real *r, real *J, real *gJ,
+                        real *lapJ) {
   int ne = s->n_up + s->n_dn;
   *J = 0.0;
   *lapJ = 0.0;
   for (int i = 0; i < 3 * ne; ++i) gJ[i] = 0.0;
   for (int i = 0; i < ne; ++i)
     for (int j = i + 1; j < ne; ++j) {
-      double a = (spin_of(s, i) == spin_of(s, j)) ? s->jastrow_a_par : s->jastrow_a_anti;
-      double b = s->jastrow_b;
-      double d[3];
+      real a = (spin_of(s, i) == spin_of(s, j)) ? s->jastrow_a_par : s->jastrow_a_anti;
+      real b = s->jastrow_b;
+      real d[3];
       for (int c = 0; c < 3; ++c) d[c] = r[3 * i + c] - r[3 * j + c];
-      double rij = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-      double den = 1.0 + b * rij;
-      double u = a * rij / den;
-      double u1 = a / (den * den);
-      double u2 = -2.0 * a * b / (den * den * den);
+      real rij = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+      real den = 1.0 + b * rij;
+      real u = a * rij / den;
+      real u1 = a / (den * den);
+      real u2 = -2.0 * a * b / (den * den * den);
       *J += u;
       for (int c = 0; c < 3; ++c) {
         gJ[3 * i + c] += u1 * d[c] / rij;
@@ -185,19 +217,19 @@ static void jastrow_all(const oracle_system_desc_t *s, const double *r, double *
     }
   /* electron-nucleus kernel (D.2): K_en(r) = N / D, N = w0 r + w1 r^2, D = 1 + w2 r,
    * summed over every (electron, nucleus) pair; quotient rule long-hand */
-  double w0 = s->jastrow_en_w0, w1 = s->jastrow_en_w1, w2 = s->jastrow_en_w2;
+  real w0 = s->jastrow_en_w0, w1 = s->jastrow_en_w1, w2 = s->jastrow_en_w2;
   if (w0 != 0.0 || w1 != 0.0)
     for (int i = 0; i < ne; ++i)
       for (int at = 0; at < s->n_atoms; ++at) {
-        double d[3];
+        real d[3];
         for (int c = 0; c < 3; ++c) d[c] = r[3 * i + c] - s->atom_xyz[3 * at + c];
-        double ria = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-        double N = w0 * ria + w1 * ria * ria, D = 1.0 + w2 * ria;
-        double N1 = w0 + 2.0 * w1 * ria, N2 = 2.0 * w1, D1 = w2;
-        double K = N / D;
-        double K1 = (N1 * D - N * D1) / (D * D);
+        real ria = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        real N = w0 * ria + w1 * ria * ria, D = 1.0 + w2 * ria;
+        real N1 = w0 + 2.0 * w1 * ria, N2 = 2.0 * w1, D1 = w2;
+        real K = N / D;
+        real K1 = (N1 * D - N * D1) / (D * D);
         /* (N'D - N D')' = N''D - N D'' = N''D ;  K'' = N''D / D^2 - 2 D' (N'D - N D') / D^3 */
-        double K2 = N2 * D / (D * D) - 2.0 * D1 * (N1 * D - N * D1) / (D * D * D);
+        real K2 = N2 * D / (D * D) - 2.0 * D1 * (N1 * D - N * D1) / (D * D * D);
         *J += K;
         for (int c = 0; c < 3; ++c) gJ[3 * i + c] += K1 * d[c] / ria;
         *lapJ += K2 + 2.0 * K1 / ria;
@@ -213,34 +245,34 @@ static void jastrow_all(const oracle_system_desc_t *s, const double *r, double *
  *   lap_i T  = c g [(f'' + 2 f'/r_ai) h + f (h'' + 2 h'/r_ij) + 2 f' h' e_ai.e_ij]
  *   lap_j T  = c f [(g'' + 2 g'/r_aj) h + g (h'' + 2 h'/r_ij) - 2 g' h' e_aj.e_ij]
  * Adds to J, gJ, lapJ; any of gJ / lapJ may be NULL (value only). */
-static void pade3(double a, double b, double r, double *p, double *p1, double *p2) {
-  double D = 1.0 + b * r;
+static void pade3(real a, real b, real r, real *p, real *p1, real *p2) {
+  real D = 1.0 + b * r;
   *p = a * r / D;
   *p1 = a / (D * D);
   *p2 = -2.0 * a * b / (D * D * D);
 }
 
-static void jastrow_een_add(const oracle_system_desc_t *s, const double *r, double *J, double *gJ, double *lapJ) {
+static void jastrow_een_add(const oracle_system_desc_t *s, const real *r, real *J, real *gJ, real *lapJ) {
   int ne = s->n_up + s->n_dn;
   for (int at = 0; at < s->n_atoms; ++at)
     for (int i = 0; i < ne; ++i)
       for (int j = 0; j < ne; ++j) {
         if (i == j) continue;
-        double eai[3], eaj[3], eij[3];
+        real eai[3], eaj[3], eij[3];
         for (int c = 0; c < 3; ++c) {
           eai[c] = r[3 * i + c] - s->atom_xyz[3 * at + c];
           eaj[c] = r[3 * j + c] - s->atom_xyz[3 * at + c];
           eij[c] = r[3 * i + c] - r[3 * j + c];
         }
-        double rai = sqrt(eai[0] * eai[0] + eai[1] * eai[1] + eai[2] * eai[2]);
-        double raj = sqrt(eaj[0] * eaj[0] + eaj[1] * eaj[1] + eaj[2] * eaj[2]);
-        double rij = sqrt(eij[0] * eij[0] + eij[1] * eij[1] + eij[2] * eij[2]);
+        real rai = sqrt(eai[0] * eai[0] + eai[1] * eai[1] + eai[2] * eai[2]);
+        real raj = sqrt(eaj[0] * eaj[0] + eaj[1] * eaj[1] + eaj[2] * eaj[2]);
+        real rij = sqrt(eij[0] * eij[0] + eij[1] * eij[1] + eij[2] * eij[2]);
         for (int c = 0; c < 3; ++c) { eai[c] /= rai; eaj[c] /= raj; eij[c] /= rij; }
-        double ai_ij = eai[0] * eij[0] + eai[1] * eij[1] + eai[2] * eij[2];
-        double aj_ij = eaj[0] * eij[0] + eaj[1] * eij[1] + eaj[2] * eij[2];
+        real ai_ij = eai[0] * eij[0] + eai[1] * eij[1] + eai[2] * eij[2];
+        real aj_ij = eaj[0] * eij[0] + eaj[1] * eij[1] + eaj[2] * eij[2];
         for (int mu = 0; mu < s->n_een; ++mu) {
           const double *q = s->een_params + 7 * mu;
-          double f, f1, f2, g, g1, g2, h, h1, h2;
+          real f, f1, f2, g, g1, g2, h, h1, h2;
           pade3(q[1], q[2], rai, &f, &f1, &f2);
           pade3(q[3], q[4], raj, &g, &g1, &g2);
           pade3(q[5], q[6], rij, &h, &h1, &h2);
@@ -259,14 +291,14 @@ static void jastrow_een_add(const oracle_system_desc_t *s, const double *r, doub
 }
 
 /* value of the electron-nucleus part of J alone (D.2) */
-static double jastrow_en_value(const oracle_system_desc_t *s, const double *r) {
+static real jastrow_en_value(const oracle_system_desc_t *s, const real *r) {
   int ne = s->n_up + s->n_dn;
-  double J = 0.0;
+  real J = 0.0;
   for (int i = 0; i < ne; ++i)
     for (int at = 0; at < s->n_atoms; ++at) {
-      double dx = r[3 * i] - s->atom_xyz[3 * at], dy = r[3 * i + 1] - s->atom_xyz[3 * at + 1],
+      real dx = r[3 * i] - s->atom_xyz[3 * at], dy = r[3 * i + 1] - s->atom_xyz[3 * at + 1],
              dz = r[3 * i + 2] - s->atom_xyz[3 * at + 2];
-      double ria = sqrt(dx * dx + dy * dy + dz * dz);
+      real ria = sqrt(dx * dx + dy * dy + dz * dz);
       J += (s->jastrow_en_w0 * ria + s->jastrow_en_w1 * ria * ria) / (1.0 + s->jastrow_en_w2 * ria);
     }
   return J;
@@ -277,41 +309,43 @@ static double jastrow_en_value(const oracle_system_desc_t *s, const double *r) {
 /* mo[i][alpha][q], q = value, d/dx, d/dy, d/dz, laplacian              */
 /* ------------------------------------------------------------------ */
 
-static void mo_all(const oracle_system_desc_t *s, const double *r, double *mo) {
+static void mo_all(const oracle_system_desc_t *s, const real *r, real *mo) {
   int ne = s->n_up + s->n_dn;
-  double ao[5];
+  real ao[5];
   for (int i = 0; i < ne * s->n_mo * 5; ++i) mo[i] = 0.0;
   for (int i = 0; i < ne; ++i)
     for (int beta = 0; beta < s->n_ao; ++beta) {
-      oracle_ao_eval(s, beta, r + 3 * i, ao);
+      ao_eval_r(s, beta, r + 3 * i, ao);
       for (int alpha = 0; alpha < s->n_mo; ++alpha)
         for (int q = 0; q < 5; ++q)
           mo[(i * s->n_mo + alpha) * 5 + q] += s->mo_coeff[beta * s->n_mo + alpha] * ao[q];
     }
 }
 
-double oracle_psi_plain(const oracle_system_desc_t *s, const double *r) {
+double oracle_psi_plain(const oracle_system_desc_t *s, const double *r_in) {
   int ne = s->n_up + s->n_dn, nmo = s->n_mo;
-  double *mo = (double *)malloc(sizeof(double) * (size_t)(ne * nmo * 5 + 1));
-  double *gJ = (double *)malloc(sizeof(double) * (size_t)(3 * ne + 1));
-  double *A = (double *)malloc(sizeof(double) * (size_t)(ne * ne + 1));
+  real *r = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
+  for (int i = 0; i < 3 * ne; ++i) r[i] = r_in[i];
+  real *mo = (real *)malloc(sizeof(real) * (size_t)(ne * nmo * 5 + 1));
+  real *gJ = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
+  real *A = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
   mo_all(s, r, mo);
-  double J, lapJ;
+  real J, lapJ;
   jastrow_all(s, r, &J, gJ, &lapJ);
-  double sigma = 0.0;
+  real sigma = 0.0;
   for (int n = 0; n < s->n_det; ++n) {
-    double D[2];
+    real D[2];
     for (int sp = 0; sp < 2; ++sp) {
       int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
       const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
       for (int i = 0; i < ns; ++i)
         for (int j = 0; j < ns; ++j) A[i * ns + j] = mo[((e0 + i) * nmo + lst[j]) * 5 + 0];
-      D[sp] = oracle_det_inv(ns, A, NULL);
+      D[sp] = det_inv_r(ns, A, NULL);
     }
     sigma += s->ci_coeff[n] * D[0] * D[1];
   }
-  free(mo); free(gJ); free(A);
-  return exp(J) * sigma;
+  free(mo); free(gJ); free(A); free(r);
+  return (double)(exp(J) * sigma);
 }
 
 /* ------------------------------------------------------------------ */
@@ -320,70 +354,70 @@ double oracle_psi_plain(const oracle_system_desc_t *s, const double *r) {
 /* eq. 1 (:21).                                                         */
 /* ------------------------------------------------------------------ */
 
-static void local_energy_one(const oracle_system_desc_t *s, const double *r, double *work,
-                             double *logpsi, double *sign, double *eloc, double *parts) {
+static void local_energy_one(const oracle_system_desc_t *s, const real *r, real *work,
+                             real *logpsi, real *sign, real *eloc, real *parts) {
   int ne = s->n_up + s->n_dn, nmo = s->n_mo;
-  double *mo = work;                 /* ne*nmo*5 */
-  double *gJ = mo + ne * nmo * 5;    /* 3 ne */
-  double *gS = gJ + 3 * ne;          /* 3 ne: grad_i Sigma */
-  double *A = gS + 3 * ne;           /* ne*ne */
-  double *Ai = A + ne * ne;          /* ne*ne */
-  double *gdet = Ai + ne * ne;       /* 3 ne: grad_i D / D of the current determinant */
+  real *mo = work;                 /* ne*nmo*5 */
+  real *gJ = mo + ne * nmo * 5;    /* 3 ne */
+  real *gS = gJ + 3 * ne;          /* 3 ne: grad_i Sigma */
+  real *A = gS + 3 * ne;           /* ne*ne */
+  real *Ai = A + ne * ne;          /* ne*ne */
+  real *gdet = Ai + ne * ne;       /* 3 ne: grad_i D / D of the current determinant */
 
   mo_all(s, r, mo);
-  double J, lapJ;
+  real J, lapJ;
   jastrow_all(s, r, &J, gJ, &lapJ);
 
-  double sigma = 0.0, lapS = 0.0;
+  real sigma = 0.0, lapS = 0.0;
   for (int i = 0; i < 3 * ne; ++i) gS[i] = 0.0;
   for (int n = 0; n < s->n_det; ++n) {
-    double D[2], t[2];
+    real D[2], t[2];
     for (int sp = 0; sp < 2; ++sp) {
       int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
       const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
       /* rows = electrons, columns = orbitals (reading Q7) */
       for (int i = 0; i < ns; ++i)
         for (int j = 0; j < ns; ++j) A[i * ns + j] = mo[((e0 + i) * nmo + lst[j]) * 5 + 0];
-      D[sp] = oracle_det_inv(ns, A, Ai);
+      D[sp] = det_inv_r(ns, A, Ai);
       t[sp] = 0.0;
       for (int i = 0; i < ns; ++i) {
         /* G.2: Tr(A^-1 dA/dx_i) = sum_k A^-1[k][i] d phi_k(r_i)/dx_i ; G.7 likewise with lap */
         for (int c = 0; c < 3; ++c) {
-          double g = 0.0;
+          real g = 0.0;
           for (int k = 0; k < ns; ++k) g += Ai[k * ns + i] * mo[((e0 + i) * nmo + lst[k]) * 5 + 1 + c];
           gdet[3 * (e0 + i) + c] = g;
         }
         for (int k = 0; k < ns; ++k) t[sp] += Ai[k * ns + i] * mo[((e0 + i) * nmo + lst[k]) * 5 + 4];
       }
     }
-    double w = s->ci_coeff[n] * D[0] * D[1];
+    real w = s->ci_coeff[n] * D[0] * D[1];
     sigma += w;
     for (int i = 0; i < 3 * ne; ++i) gS[i] += w * gdet[i];   /* F.2 */
     lapS += w * (t[0] + t[1]);                               /* F.4; cross term vanishes (no coordinate in both spins) */
   }
 
   /* F.1 with script-J = e^J (reading Q5): lap Psi / Psi = lapJ + |gJ|^2 + 2 gJ.gS/S + lapS/S */
-  double gJ2 = 0.0, cross = 0.0;
+  real gJ2 = 0.0, cross = 0.0;
   for (int i = 0; i < 3 * ne; ++i) { gJ2 += gJ[i] * gJ[i]; cross += gJ[i] * gS[i]; }
-  double lap_over_psi = lapJ + gJ2 + 2.0 * cross / sigma + lapS / sigma;
-  double kinetic = -0.5 * lap_over_psi;
+  real lap_over_psi = lapJ + gJ2 + 2.0 * cross / sigma + lapS / sigma;
+  real kinetic = -0.5 * lap_over_psi;
 
   /* potential, eq. 1 */
-  double vee = 0.0, ven = 0.0, vnn = 0.0;
+  real vee = 0.0, ven = 0.0, vnn = 0.0;
   for (int i = 0; i < ne; ++i)
     for (int j = i + 1; j < ne; ++j) {
-      double dx = r[3 * i] - r[3 * j], dy = r[3 * i + 1] - r[3 * j + 1], dz = r[3 * i + 2] - r[3 * j + 2];
+      real dx = r[3 * i] - r[3 * j], dy = r[3 * i + 1] - r[3 * j + 1], dz = r[3 * i + 2] - r[3 * j + 2];
       vee += 1.0 / sqrt(dx * dx + dy * dy + dz * dz);
     }
   for (int i = 0; i < ne; ++i)
     for (int a = 0; a < s->n_atoms; ++a) {
-      double dx = r[3 * i] - s->atom_xyz[3 * a], dy = r[3 * i + 1] - s->atom_xyz[3 * a + 1],
+      real dx = r[3 * i] - s->atom_xyz[3 * a], dy = r[3 * i + 1] - s->atom_xyz[3 * a + 1],
              dz = r[3 * i + 2] - s->atom_xyz[3 * a + 2];
       ven -= s->atom_Z[a] / sqrt(dx * dx + dy * dy + dz * dz);
     }
   for (int a = 0; a < s->n_atoms; ++a)
     for (int b = a + 1; b < s->n_atoms; ++b) {
-      double dx = s->atom_xyz[3 * a] - s->atom_xyz[3 * b], dy = s->atom_xyz[3 * a + 1] - s->atom_xyz[3 * b + 1],
+      real dx = s->atom_xyz[3 * a] - s->atom_xyz[3 * b], dy = s->atom_xyz[3 * a + 1] - s->atom_xyz[3 * b + 1],
              dz = s->atom_xyz[3 * a + 2] - s->atom_xyz[3 * b + 2];
       vnn += s->atom_Z[a] * s->atom_Z[b] / sqrt(dx * dx + dy * dy + dz * dz);
     }
@@ -399,7 +433,7 @@ static size_t work_doubles(const oracle_system_desc_t *s) {
   return ne * (size_t)s->n_mo * 5 + 9 * ne + 2 * ne * ne + 16;
 }
 
-static void gather_walker(const double *r, int64_t M, int64_t w, int ne, double *aos) {
+static void gather_walker(const double *r, int64_t M, int64_t w, int ne, real *aos) {
   for (int i = 0; i < ne; ++i)
     for (int c = 0; c < 3; ++c) aos[3 * i + c] = r[((size_t)i * 3 + (size_t)c) * (size_t)M + (size_t)w];
 }
@@ -407,16 +441,18 @@ static void gather_walker(const double *r, int64_t M, int64_t w, int ne, double 
 int oracle_local_energy(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                         int64_t w1, double *logpsi, double *sign, double *eloc, double *parts) {
   int ne = s->n_up + s->n_dn;
-  double *work = (double *)malloc(sizeof(double) * work_doubles(s));
-  double *pos = (double *)malloc(sizeof(double) * (size_t)(3 * ne + 1));
+  real *work = (real *)malloc(sizeof(real) * work_doubles(s));
+  real *pos = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
   if (!work || !pos) return -1;
   for (int64_t w = w0; w < w1; ++w) {
     gather_walker(r, M, w, ne, pos);
-    double lp, sg, el;
-    local_energy_one(s, pos, work, &lp, &sg, &el, parts ? parts + 4 * w : NULL);
-    if (logpsi) logpsi[w] = lp;
-    if (sign) sign[w] = sg;
-    if (eloc) eloc[w] = el;
+    real lp, sg, el, p4[4];
+    local_energy_one(s, pos, work, &lp, &sg, &el, parts ? p4 : NULL);
+    if (parts)
+      for (int q = 0; q < 4; ++q) parts[4 * w + q] = (double)p4[q];
+    if (logpsi) logpsi[w] = (double)lp;
+    if (sign) sign[w] = (double)sg;
+    if (eloc) eloc[w] = (double)el;
   }
   free(work); free(pos);
   return 0;
@@ -483,37 +519,37 @@ void oracle_walker_draws(uint64_t seed, int64_t w, uint64_t sweep, int n_coord, 
 /* log|Psi| and sign from the plain definition (eq. 4)     */
 /* ------------------------------------------------------------------ */
 
-static void logpsi_one(const oracle_system_desc_t *s, const double *r, double *work, double *logpsi,
-                       double *sign) {
+static void logpsi_one(const oracle_system_desc_t *s, const real *r, real *work, real *logpsi,
+                       real *sign) {
   int ne = s->n_up + s->n_dn, nmo = s->n_mo;
-  double *mo = work;              /* ne*nmo (values only) */
-  double *A = mo + ne * nmo * 5;  /* ne*ne, same offsets as local_energy_one's layout */
-  double ao[5];
+  real *mo = work;              /* ne*nmo (values only) */
+  real *A = mo + ne * nmo * 5;  /* ne*ne, same offsets as local_energy_one's layout */
+  real ao[5];
   for (int i = 0; i < ne * nmo; ++i) mo[i] = 0.0;
   for (int i = 0; i < ne; ++i)
     for (int beta = 0; beta < s->n_ao; ++beta) {
-      oracle_ao_eval(s, beta, r + 3 * i, ao);
+      ao_eval_r(s, beta, r + 3 * i, ao);
       for (int alpha = 0; alpha < nmo; ++alpha) mo[i * nmo + alpha] += s->mo_coeff[beta * nmo + alpha] * ao[0];
     }
-  double J = 0.0;
+  real J = 0.0;
   for (int i = 0; i < ne; ++i)
     for (int j = i + 1; j < ne; ++j) {
-      double a = (spin_of(s, i) == spin_of(s, j)) ? s->jastrow_a_par : s->jastrow_a_anti;
-      double dx = r[3 * i] - r[3 * j], dy = r[3 * i + 1] - r[3 * j + 1], dz = r[3 * i + 2] - r[3 * j + 2];
-      double rij = sqrt(dx * dx + dy * dy + dz * dz);
+      real a = (spin_of(s, i) == spin_of(s, j)) ? s->jastrow_a_par : s->jastrow_a_anti;
+      real dx = r[3 * i] - r[3 * j], dy = r[3 * i + 1] - r[3 * j + 1], dz = r[3 * i + 2] - r[3 * j + 2];
+      real rij = sqrt(dx * dx + dy * dy + dz * dz);
       J += a * rij / (1.0 + s->jastrow_b * rij);
     }
   J += jastrow_en_value(s, r);
   if (s->n_een > 0) jastrow_een_add(s, r, &J, NULL, NULL);
-  double sigma = 0.0;
+  real sigma = 0.0;
   for (int n = 0; n < s->n_det; ++n) {
-    double D[2];
+    real D[2];
     for (int sp = 0; sp < 2; ++sp) {
       int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
       const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
       for (int i = 0; i < ns; ++i)
         for (int j = 0; j < ns; ++j) A[i * ns + j] = mo[(e0 + i) * nmo + lst[j]];
-      D[sp] = oracle_det_inv(ns, A, NULL);
+      D[sp] = det_inv_r(ns, A, NULL);
     }
     sigma += s->ci_coeff[n] * D[0] * D[1];
   }
@@ -530,23 +566,24 @@ int oracle_metropolis(const oracle_system_desc_t *s, double *r, int64_t M, int64
                       double *logpsi, double *sign, uint8_t *accept, double *margin,
                       double *eloc_acc) {
   int ne = s->n_up + s->n_dn, nc = 3 * ne;
-  double *work = (double *)malloc(sizeof(double) * work_doubles(s));
-  double *pos = (double *)malloc(sizeof(double) * (size_t)(nc + 1));
-  double *prop = (double *)malloc(sizeof(double) * (size_t)(nc + 1));
+  real *work = (real *)malloc(sizeof(real) * work_doubles(s));
+  real *pos = (real *)malloc(sizeof(real) * (size_t)(nc + 1));
+  real *prop = (real *)malloc(sizeof(real) * (size_t)(nc + 1));
   double *z = (double *)malloc(sizeof(double) * (size_t)(nc + 2));
   if (!work || !pos || !prop || !z) return -1;
   for (int64_t w = w0; w < w1; ++w) {
     gather_walker(r, M, w, ne, pos);
-    double lp, sg;
+    real lp, sg;
     logpsi_one(s, pos, work, &lp, &sg);
-    double acc_e = 0.0;
+    real acc_e = 0.0;
     for (int32_t sw = 0; sw < n_sweeps; ++sw) {
       double u;
       oracle_walker_draws(seed, w, sweep_offset + (uint64_t)sw, nc, z, &u);
-      for (int q = 0; q < nc; ++q) prop[q] = pos[q] + step * z[q];
-      double lp2, sg2;
+      /* the walker's state is float64 in every build: the move is rounded to double */
+      for (int q = 0; q < nc; ++q) prop[q] = (real)((double)pos[q] + step * z[q]);
+      real lp2, sg2;
       logpsi_one(s, prop, work, &lp2, &sg2);
-      double mg = 2.0 * (lp2 - lp) - log(u);
+      real mg = 2.0 * (lp2 - lp) - log(u);
       int ok = (log(u) < 2.0 * (lp2 - lp)) ? 1 : 0; /* false for NaN and for Psi' = 0 */
       if (ok) {
         for (int q = 0; q < nc; ++q) pos[q] = prop[q];
@@ -554,18 +591,18 @@ int oracle_metropolis(const oracle_system_desc_t *s, double *r, int64_t M, int64
         sg = sg2;
       }
       if (accept) accept[(size_t)sw * (size_t)M + (size_t)w] = (uint8_t)ok;
-      if (margin) margin[(size_t)sw * (size_t)M + (size_t)w] = mg;
+      if (margin) margin[(size_t)sw * (size_t)M + (size_t)w] = (double)mg;
       if (eloc_acc) {
-        double l3, s3, el;
+        real l3, s3, el;
         local_energy_one(s, pos, work, &l3, &s3, &el, NULL);
         acc_e += el;
       }
     }
     for (int i = 0; i < ne; ++i)
-      for (int c = 0; c < 3; ++c) r[((size_t)i * 3 + (size_t)c) * (size_t)M + (size_t)w] = pos[3 * i + c];
-    if (logpsi) logpsi[w] = lp;
-    if (sign) sign[w] = sg;
-    if (eloc_acc) eloc_acc[w] = acc_e;
+      for (int c = 0; c < 3; ++c) r[((size_t)i * 3 + (size_t)c) * (size_t)M + (size_t)w] = (double)pos[3 * i + c];
+    if (logpsi) logpsi[w] = (double)lp;
+    if (sign) sign[w] = (double)sg;
+    if (eloc_acc) eloc_acc[w] = (double)acc_e;
   }
   free(work); free(pos); free(prop); free(z);
   return 0;
@@ -603,24 +640,24 @@ void oracle_batch_stats(const double *x, int64_t M, double *mean, double *stderr
 int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                            int64_t w1, double *O) {
   int ne = s->n_up + s->n_dn, nmo = s->n_mo, nj = 6 + 7 * s->n_een, np = nj + s->n_det;
-  double *mo = (double *)malloc(sizeof(double) * (size_t)(ne * nmo + 1));
-  double *A = (double *)malloc(sizeof(double) * (size_t)(ne * ne + 1));
-  double *pos = (double *)malloc(sizeof(double) * (size_t)(3 * ne + 1));
-  double *prod = (double *)malloc(sizeof(double) * (size_t)(s->n_det + 1));
+  real *mo = (real *)malloc(sizeof(real) * (size_t)(ne * nmo + 1));
+  real *A = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
+  real *pos = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
+  real *prod = (real *)malloc(sizeof(real) * (size_t)(s->n_det + 1));
   if (!mo || !A || !pos || !prod) return -1;
-  double ao[5];
+  real ao[5];
   for (int64_t w = w0; w < w1; ++w) {
     gather_walker(r, M, w, ne, pos);
     double *out = O + (size_t)w * (size_t)np;
     /* Jastrow: K = a r / (1 + b r)  (D.1):  dK/da = r / (1 + b r),  dK/db = -a r^2 / (1 + b r)^2 */
-    double da_par = 0.0, da_anti = 0.0, db = 0.0;
+    real da_par = 0.0, da_anti = 0.0, db = 0.0;
     for (int i = 0; i < ne; ++i)
       for (int j = i + 1; j < ne; ++j) {
         int same = spin_of(s, i) == spin_of(s, j);
-        double a = same ? s->jastrow_a_par : s->jastrow_a_anti;
-        double dx = pos[3 * i] - pos[3 * j], dy = pos[3 * i + 1] - pos[3 * j + 1], dz = pos[3 * i + 2] - pos[3 * j + 2];
-        double rij = sqrt(dx * dx + dy * dy + dz * dz);
-        double den = 1.0 + s->jastrow_b * rij;
+        real a = same ? s->jastrow_a_par : s->jastrow_a_anti;
+        real dx = pos[3 * i] - pos[3 * j], dy = pos[3 * i + 1] - pos[3 * j + 1], dz = pos[3 * i + 2] - pos[3 * j + 2];
+        real rij = sqrt(dx * dx + dy * dy + dz * dz);
+        real den = 1.0 + s->jastrow_b * rij;
         if (same) da_par += rij / den; else da_anti += rij / den;
         db += -a * rij * rij / (den * den);
       }
@@ -629,13 +666,13 @@ int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64
     out[2] = db;
     /* electron-nucleus kernel K = (w0 r + w1 r^2) / (1 + w2 r)  (D.2):
      * dK/dw0 = r / D,  dK/dw1 = r^2 / D,  dK/dw2 = -(w0 r + w1 r^2) r / D^2,  D = 1 + w2 r */
-    double dw0 = 0.0, dw1 = 0.0, dw2 = 0.0;
+    real dw0 = 0.0, dw1 = 0.0, dw2 = 0.0;
     for (int i = 0; i < ne; ++i)
       for (int at = 0; at < s->n_atoms; ++at) {
-        double dx = pos[3 * i] - s->atom_xyz[3 * at], dy = pos[3 * i + 1] - s->atom_xyz[3 * at + 1],
+        real dx = pos[3 * i] - s->atom_xyz[3 * at], dy = pos[3 * i + 1] - s->atom_xyz[3 * at + 1],
                dz = pos[3 * i + 2] - s->atom_xyz[3 * at + 2];
-        double ria = sqrt(dx * dx + dy * dy + dz * dz);
-        double D = 1.0 + s->jastrow_en_w2 * ria;
+        real ria = sqrt(dx * dx + dy * dy + dz * dz);
+        real D = 1.0 + s->jastrow_en_w2 * ria;
         dw0 += ria / D;
         dw1 += ria * ria / D;
         dw2 += -(s->jastrow_en_w0 * ria + s->jastrow_en_w1 * ria * ria) * ria / (D * D);
@@ -649,20 +686,20 @@ int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64
      * een_params: c, a_f, b_f, a_g, b_g, a_h, b_h. */
     for (int mu = 0; mu < s->n_een; ++mu) {
       const double *q = s->een_params + 7 * mu;
-      double dq[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+      real dq[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
       for (int at = 0; at < s->n_atoms; ++at)
         for (int i = 0; i < ne; ++i)
           for (int j = 0; j < ne; ++j) {
             if (i == j) continue;
-            double xi = pos[3 * i] - s->atom_xyz[3 * at], yi = pos[3 * i + 1] - s->atom_xyz[3 * at + 1],
+            real xi = pos[3 * i] - s->atom_xyz[3 * at], yi = pos[3 * i + 1] - s->atom_xyz[3 * at + 1],
                    zi = pos[3 * i + 2] - s->atom_xyz[3 * at + 2];
-            double xj = pos[3 * j] - s->atom_xyz[3 * at], yj = pos[3 * j + 1] - s->atom_xyz[3 * at + 1],
+            real xj = pos[3 * j] - s->atom_xyz[3 * at], yj = pos[3 * j + 1] - s->atom_xyz[3 * at + 1],
                    zj = pos[3 * j + 2] - s->atom_xyz[3 * at + 2];
-            double xx = pos[3 * i] - pos[3 * j], yy = pos[3 * i + 1] - pos[3 * j + 1], zz = pos[3 * i + 2] - pos[3 * j + 2];
-            double rai = sqrt(xi * xi + yi * yi + zi * zi), raj = sqrt(xj * xj + yj * yj + zj * zj);
-            double rij = sqrt(xx * xx + yy * yy + zz * zz);
-            double Df = 1.0 + q[2] * rai, Dg = 1.0 + q[4] * raj, Dh = 1.0 + q[6] * rij;
-            double f = q[1] * rai / Df, g = q[3] * raj / Dg, h = q[5] * rij / Dh;
+            real xx = pos[3 * i] - pos[3 * j], yy = pos[3 * i + 1] - pos[3 * j + 1], zz = pos[3 * i + 2] - pos[3 * j + 2];
+            real rai = sqrt(xi * xi + yi * yi + zi * zi), raj = sqrt(xj * xj + yj * yj + zj * zj);
+            real rij = sqrt(xx * xx + yy * yy + zz * zz);
+            real Df = 1.0 + q[2] * rai, Dg = 1.0 + q[4] * raj, Dh = 1.0 + q[6] * rij;
+            real f = q[1] * rai / Df, g = q[3] * raj / Dg, h = q[5] * rij / Dh;
             dq[0] += f * g * h;
             dq[1] += q[0] * (rai / Df) * g * h;
             dq[2] += q[0] * (-q[1] * rai * rai / (Df * Df)) * g * h;
@@ -677,18 +714,18 @@ int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64
     for (int i = 0; i < ne * nmo; ++i) mo[i] = 0.0;
     for (int i = 0; i < ne; ++i)
       for (int beta = 0; beta < s->n_ao; ++beta) {
-        oracle_ao_eval(s, beta, pos + 3 * i, ao);
+        ao_eval_r(s, beta, pos + 3 * i, ao);
         for (int alpha = 0; alpha < nmo; ++alpha) mo[i * nmo + alpha] += s->mo_coeff[beta * nmo + alpha] * ao[0];
       }
-    double sigma = 0.0;
+    real sigma = 0.0;
     for (int n = 0; n < s->n_det; ++n) {
-      double D[2];
+      real D[2];
       for (int sp = 0; sp < 2; ++sp) {
         int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
         const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
         for (int i = 0; i < ns; ++i)
           for (int j = 0; j < ns; ++j) A[i * ns + j] = mo[(e0 + i) * nmo + lst[j]];
-        D[sp] = oracle_det_inv(ns, A, NULL);
+        D[sp] = det_inv_r(ns, A, NULL);
       }
       prod[n] = D[0] * D[1];
       sigma += s->ci_coeff[n] * prod[n];
@@ -732,49 +769,49 @@ void oracle_energy_gradient(const double *eloc, const double *O, int64_t M, int3
 int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                                int64_t w1, double *dC, double *dzeta) {
   int ne = s->n_up + s->n_dn, nmo = s->n_mo, nao = s->n_ao;
-  double *aov = (double *)malloc(sizeof(double) * (size_t)(ne * nao + 1));      /* ao_beta(r_i) */
-  double *aoz = (double *)malloc(sizeof(double) * (size_t)(ne * nao + 1));      /* d ao_beta / d zeta (r_i) */
-  double *mo = (double *)malloc(sizeof(double) * (size_t)(ne * nmo + 1));
-  double *A = (double *)malloc(sizeof(double) * (size_t)(ne * ne + 1));
-  double *Ai = (double *)malloc(sizeof(double) * (size_t)(2 * ne * ne + 2));    /* both spins' inverses of one determinant */
-  double *gam = (double *)malloc(sizeof(double) * (size_t)(ne * nmo + 1));      /* Gamma[i][alpha], not yet / Sigma */
-  double *pos = (double *)malloc(sizeof(double) * (size_t)(3 * ne + 1));
+  real *aov = (real *)malloc(sizeof(real) * (size_t)(ne * nao + 1));      /* ao_beta(r_i) */
+  real *aoz = (real *)malloc(sizeof(real) * (size_t)(ne * nao + 1));      /* d ao_beta / d zeta (r_i) */
+  real *mo = (real *)malloc(sizeof(real) * (size_t)(ne * nmo + 1));
+  real *A = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
+  real *Ai = (real *)malloc(sizeof(real) * (size_t)(2 * ne * ne + 2));    /* both spins' inverses of one determinant */
+  real *gam = (real *)malloc(sizeof(real) * (size_t)(ne * nmo + 1));      /* Gamma[i][alpha], not yet / Sigma */
+  real *pos = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
   if (!aov || !aoz || !mo || !A || !Ai || !gam || !pos) return -1;
-  double ao[5];
+  real ao[5];
   for (int64_t w = w0; w < w1; ++w) {
     gather_walker(r, M, w, ne, pos);
     for (int i = 0; i < ne; ++i)
       for (int beta = 0; beta < nao; ++beta) {
-        oracle_ao_eval(s, beta, pos + 3 * i, ao);
+        ao_eval_r(s, beta, pos + 3 * i, ao);
         aov[i * nao + beta] = ao[0];
         /* phi = N S r^k e^{-zeta r}: d phi / d zeta = phi (d ln N / d zeta - r) */
         int at = s->ao_atom[beta];
-        double dx = pos[3 * i] - s->atom_xyz[3 * at], dy = pos[3 * i + 1] - s->atom_xyz[3 * at + 1],
+        real dx = pos[3 * i] - s->atom_xyz[3 * at], dy = pos[3 * i + 1] - s->atom_xyz[3 * at + 1],
                dz = pos[3 * i + 2] - s->atom_xyz[3 * at + 2];
-        double rr = sqrt(dx * dx + dy * dy + dz * dz);
-        double dlnN = s->ao_norm ? 0.0 : ((double)s->ao_n[beta] + 0.5) / s->ao_zeta[beta];
+        real rr = sqrt(dx * dx + dy * dy + dz * dz);
+        real dlnN = s->ao_norm ? 0.0 : ((real)s->ao_n[beta] + 0.5) / s->ao_zeta[beta];
         aoz[i * nao + beta] = ao[0] * (dlnN - rr);
       }
     for (int i = 0; i < ne * nmo; ++i) { mo[i] = 0.0; gam[i] = 0.0; }
     for (int i = 0; i < ne; ++i)
       for (int beta = 0; beta < nao; ++beta)
         for (int alpha = 0; alpha < nmo; ++alpha) mo[i * nmo + alpha] += s->mo_coeff[beta * nmo + alpha] * aov[i * nao + beta];
-    double sigma = 0.0;
+    real sigma = 0.0;
     for (int n = 0; n < s->n_det; ++n) {
-      double D[2];
+      real D[2];
       for (int sp = 0; sp < 2; ++sp) {
         int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
         const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
         for (int i = 0; i < ns; ++i)
           for (int j = 0; j < ns; ++j) A[i * ns + j] = mo[(e0 + i) * nmo + lst[j]];
-        D[sp] = oracle_det_inv(ns, A, Ai + sp * ne * ne);
+        D[sp] = det_inv_r(ns, A, Ai + sp * ne * ne);
       }
-      double wn = s->ci_coeff[n] * D[0] * D[1];
+      real wn = s->ci_coeff[n] * D[0] * D[1];
       sigma += wn;
       for (int sp = 0; sp < 2; ++sp) {
         int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
         const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
-        const double *inv = Ai + sp * ne * ne;
+        const real *inv = Ai + sp * ne * ne;
         /* d ln D / d A[i][j] = A^-1[j][i]; column j of A_n holds MO lst[j] */
         for (int i = 0; i < ns; ++i)
           for (int j = 0; j < ns; ++j) gam[(e0 + i) * nmo + lst[j]] += wn * inv[j * ns + i];
@@ -783,15 +820,15 @@ int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, i
     if (dC)
       for (int beta = 0; beta < nao; ++beta)
         for (int alpha = 0; alpha < nmo; ++alpha) {
-          double t = 0.0;
+          real t = 0.0;
           for (int i = 0; i < ne; ++i) t += aov[i * nao + beta] * gam[i * nmo + alpha];
           dC[((size_t)w * nao + beta) * nmo + alpha] = t / sigma;
         }
     if (dzeta)
       for (int beta = 0; beta < nao; ++beta) {
-        double t = 0.0;
+        real t = 0.0;
         for (int alpha = 0; alpha < nmo; ++alpha) {
-          double u = 0.0;
+          real u = 0.0;
           for (int i = 0; i < ne; ++i) u += aoz[i * nao + beta] * gam[i * nmo + alpha];
           t += s->mo_coeff[beta * nmo + alpha] * u;
         }
@@ -819,20 +856,20 @@ int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, i
 int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                                 int64_t w1, double *dR) {
   int ne = s->n_up + s->n_dn, nmo = s->n_mo, nao = s->n_ao, na = s->n_atoms;
-  double *aov = (double *)malloc(sizeof(double) * (size_t)(ne * nao + 1));       /* ao_beta(r_i) */
-  double *aog = (double *)malloc(sizeof(double) * (size_t)(3 * ne * nao + 1));   /* grad ao_beta(r_i) */
-  double *mo = (double *)malloc(sizeof(double) * (size_t)(ne * nmo + 1));
-  double *A = (double *)malloc(sizeof(double) * (size_t)(ne * ne + 1));
-  double *Ai = (double *)malloc(sizeof(double) * (size_t)(2 * ne * ne + 2));
-  double *gam = (double *)malloc(sizeof(double) * (size_t)(ne * nmo + 1));
-  double *pos = (double *)malloc(sizeof(double) * (size_t)(3 * ne + 1));
+  real *aov = (real *)malloc(sizeof(real) * (size_t)(ne * nao + 1));       /* ao_beta(r_i) */
+  real *aog = (real *)malloc(sizeof(real) * (size_t)(3 * ne * nao + 1));   /* grad ao_beta(r_i) */
+  real *mo = (real *)malloc(sizeof(real) * (size_t)(ne * nmo + 1));
+  real *A = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
+  real *Ai = (real *)malloc(sizeof(real) * (size_t)(2 * ne * ne + 2));
+  real *gam = (real *)malloc(sizeof(real) * (size_t)(ne * nmo + 1));
+  real *pos = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
   if (!aov || !aog || !mo || !A || !Ai || !gam || !pos) return -1;
-  double ao[5];
+  real ao[5];
   for (int64_t w = w0; w < w1; ++w) {
     gather_walker(r, M, w, ne, pos);
     for (int i = 0; i < ne; ++i)
       for (int beta = 0; beta < nao; ++beta) {
-        oracle_ao_eval(s, beta, pos + 3 * i, ao);
+        ao_eval_r(s, beta, pos + 3 * i, ao);
         aov[i * nao + beta] = ao[0];
         for (int c = 0; c < 3; ++c) aog[(i * nao + beta) * 3 + c] = ao[1 + c];
       }
@@ -840,22 +877,22 @@ int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, 
     for (int i = 0; i < ne; ++i)
       for (int beta = 0; beta < nao; ++beta)
         for (int alpha = 0; alpha < nmo; ++alpha) mo[i * nmo + alpha] += s->mo_coeff[beta * nmo + alpha] * aov[i * nao + beta];
-    double sigma = 0.0;
+    real sigma = 0.0;
     for (int n = 0; n < s->n_det; ++n) {
-      double D[2];
+      real D[2];
       for (int sp = 0; sp < 2; ++sp) {
         int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
         const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
         for (int i = 0; i < ns; ++i)
           for (int j = 0; j < ns; ++j) A[i * ns + j] = mo[(e0 + i) * nmo + lst[j]];
-        D[sp] = oracle_det_inv(ns, A, Ai + sp * ne * ne);
+        D[sp] = det_inv_r(ns, A, Ai + sp * ne * ne);
       }
-      double wn = s->ci_coeff[n] * D[0] * D[1];
+      real wn = s->ci_coeff[n] * D[0] * D[1];
       sigma += wn;
       for (int sp = 0; sp < 2; ++sp) {
         int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
         const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
-        const double *inv = Ai + sp * ne * ne;
+        const real *inv = Ai + sp * ne * ne;
         for (int i = 0; i < ns; ++i)
           for (int j = 0; j < ns; ++j) gam[(e0 + i) * nmo + lst[j]] += wn * inv[j * ns + i];
       }
@@ -866,9 +903,9 @@ int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, 
     for (int beta = 0; beta < nao; ++beta) {
       int at = s->ao_atom[beta];
       for (int c = 0; c < 3; ++c) {
-        double t = 0.0;
+        real t = 0.0;
         for (int alpha = 0; alpha < nmo; ++alpha) {
-          double u = 0.0;
+          real u = 0.0;
           for (int i = 0; i < ne; ++i) u += aog[(i * nao + beta) * 3 + c] * gam[i * nmo + alpha];
           t += s->mo_coeff[beta * nmo + alpha] * u;
         }
@@ -876,15 +913,15 @@ int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, 
       }
     }
     /* electron-nucleus kernel D.2: K = N/D, N = w0 r + w1 r^2, D = 1 + w2 r */
-    double jw0 = s->jastrow_en_w0, jw1 = s->jastrow_en_w1, jw2 = s->jastrow_en_w2;
+    real jw0 = s->jastrow_en_w0, jw1 = s->jastrow_en_w1, jw2 = s->jastrow_en_w2;
     if (jw0 != 0.0 || jw1 != 0.0)
       for (int i = 0; i < ne; ++i)
         for (int at = 0; at < na; ++at) {
-          double d[3];
+          real d[3];
           for (int c = 0; c < 3; ++c) d[c] = pos[3 * i + c] - s->atom_xyz[3 * at + c];
-          double ria = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-          double N = jw0 * ria + jw1 * ria * ria, D = 1.0 + jw2 * ria;
-          double K1 = ((jw0 + 2.0 * jw1 * ria) * D - N * jw2) / (D * D);
+          real ria = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+          real N = jw0 * ria + jw1 * ria * ria, D = 1.0 + jw2 * ria;
+          real K1 = ((jw0 + 2.0 * jw1 * ria) * D - N * jw2) / (D * D);
           for (int c = 0; c < 3; ++c) out[3 * at + c] -= K1 * d[c] / ria;
         }
     /* electron-electron-nucleus kernel D.3 (reading Q22: ordered pairs i != j, every nucleus) */
@@ -892,18 +929,18 @@ int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, 
       for (int i = 0; i < ne; ++i)
         for (int j = 0; j < ne; ++j) {
           if (i == j || s->n_een == 0) continue;
-          double eai[3], eaj[3], eij[3];
+          real eai[3], eaj[3], eij[3];
           for (int c = 0; c < 3; ++c) {
             eai[c] = pos[3 * i + c] - s->atom_xyz[3 * at + c];
             eaj[c] = pos[3 * j + c] - s->atom_xyz[3 * at + c];
             eij[c] = pos[3 * i + c] - pos[3 * j + c];
           }
-          double rai = sqrt(eai[0] * eai[0] + eai[1] * eai[1] + eai[2] * eai[2]);
-          double raj = sqrt(eaj[0] * eaj[0] + eaj[1] * eaj[1] + eaj[2] * eaj[2]);
-          double rij = sqrt(eij[0] * eij[0] + eij[1] * eij[1] + eij[2] * eij[2]);
+          real rai = sqrt(eai[0] * eai[0] + eai[1] * eai[1] + eai[2] * eai[2]);
+          real raj = sqrt(eaj[0] * eaj[0] + eaj[1] * eaj[1] + eaj[2] * eaj[2]);
+          real rij = sqrt(eij[0] * eij[0] + eij[1] * eij[1] + eij[2] * eij[2]);
           for (int mu = 0; mu < s->n_een; ++mu) {
             const double *q = s->een_params + 7 * mu;
-            double f, f1, f2, g, g1, g2, h, h1, h2;
+            real f, f1, f2, g, g1, g2, h, h1, h2;
             pade3(q[1], q[2], rai, &f, &f1, &f2);
             pade3(q[3], q[4], raj, &g, &g1, &g2);
             pade3(q[5], q[6], rij, &h, &h1, &h2);
