@@ -89,8 +89,10 @@ typedef struct {
   /* Electron-electron-nucleus Jastrow kernel (D.3): n_een terms (at most 6; the paper uses 5),
    * een_params host [n_een][7] = (c, a1, b1, a2, b2, a3, b3) per term:
    *   K_een = sum_mu c [a1 r_ai / (1 + b1 r_ai)] [a2 r_aj / (1 + b2 r_aj)] [a3 r_ij / (1 + b3 r_ij)],
-   * summed over every nucleus a and every ORDERED electron pair i != j (the paper does not say; only the
-   * ordered sum is symmetric under electron exchange when the first two factors differ).  n_een = 0: absent. */
+   * summed as eq. 5 says (sum over alpha and i > j, every nucleus, every electron pair once), each pair
+   * symmetrised: 1/2 [K_een(r_ai, r_aj, r_ij) + K_een(r_aj, r_ai, r_ij)].  With a1 = a2, b1 = b2 this is the paper's
+   * literal sum; with different first and second factors the literal K_een is not symmetric in (i, j) and would break
+   * the exchange symmetry of PAPER.md:51, the symmetrised pair does not (reading Q22).  n_een = 0: absent. */
   int32_t n_een;
   const double *een_params;
 } qmc_system_desc_t;

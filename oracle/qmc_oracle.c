@@ -237,8 +237,12 @@ static void jastrow_all(const oracle_system_desc_t *s, const real *r, real *J, r
   if (s->n_een > 0) jastrow_een_add(s, r, J, gJ, lapJ);
 }
 
-/* electron-electron-nucleus kernel (D.3), reading Q22: ordered pairs i != j, every nucleus.
- * One term T = c f(r_ai) g(r_aj) h(r_ij), Pade factors p(r) = a r/(1 + b r), p' = a/(1 + b r)^2,
+/* electron-electron-nucleus kernel (D.3).  Eq. 5 sums K_een over every nucleus and every
+ * pair once, sum_{alpha, i>j}.  With different first and second Pade factors the literal K_een(r_ai, r_aj, r_ij) is not
+ * symmetric in (i, j), which would break the exchange symmetry of PAPER.md:51, so each pair enters symmetrised
+ * (reading Q22):  K_pair = 1/2 [K_een(r_ai, r_aj, r_ij) + K_een(r_aj, r_ai, r_ij)]  -- identical to the paper's literal
+ * sum when the two factors coincide.  Written as a loop over ORDERED pairs i != j with weight 1/2.
+ * One term T = (c/2) f(r_ai) g(r_aj) h(r_ij), Pade factors p(r) = a r/(1 + b r), p' = a/(1 + b r)^2,
  * p'' = -2 a b/(1 + b r)^3.  Product rule long-hand:
  *   grad_i T = c g [f' h e_ai + f h' e_ij]            e_ai = (r_i - R_a)/r_ai, e_ij = (r_i - r_j)/r_ij
  *   grad_j T = c f [g' h e_aj - g h' e_ij]
@@ -276,15 +280,16 @@ static void jastrow_een_add(const oracle_system_desc_t *s, const real *r, real *
           pade3(q[1], q[2], rai, &f, &f1, &f2);
           pade3(q[3], q[4], raj, &g, &g1, &g2);
           pade3(q[5], q[6], rij, &h, &h1, &h2);
-          *J += q[0] * f * g * h;
+          real ch = 0.5 * q[0]; /* each unordered pair is visited twice, as (i,j) and as (j,i) */
+          *J += ch * f * g * h;
           if (gJ)
             for (int c = 0; c < 3; ++c) {
-              gJ[3 * i + c] += q[0] * g * (f1 * h * eai[c] + f * h1 * eij[c]);
-              gJ[3 * j + c] += q[0] * f * (g1 * h * eaj[c] - g * h1 * eij[c]);
+              gJ[3 * i + c] += ch * g * (f1 * h * eai[c] + f * h1 * eij[c]);
+              gJ[3 * j + c] += ch * f * (g1 * h * eaj[c] - g * h1 * eij[c]);
             }
           if (lapJ) {
-            *lapJ += q[0] * g * ((f2 + 2.0 * f1 / rai) * h + f * (h2 + 2.0 * h1 / rij) + 2.0 * f1 * h1 * ai_ij);
-            *lapJ += q[0] * f * ((g2 + 2.0 * g1 / raj) * h + g * (h2 + 2.0 * h1 / rij) - 2.0 * g1 * h1 * aj_ij);
+            *lapJ += ch * g * ((f2 + 2.0 * f1 / rai) * h + f * (h2 + 2.0 * h1 / rij) + 2.0 * f1 * h1 * ai_ij);
+            *lapJ += ch * f * ((g2 + 2.0 * g1 / raj) * h + g * (h2 + 2.0 * h1 / rij) - 2.0 * g1 * h1 * aj_ij);
           }
         }
       }
@@ -680,8 +685,9 @@ int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64
     out[3] = dw0;
     out[4] = dw1;
     out[5] = dw2;
-    /* electron-electron-nucleus kernel (D.3; reading Q22: ordered pairs i != j, every nucleus):
-     * term mu = c f(r_ai) g(r_aj) h(r_ij) with Pade factors p(r) = a r / (1 + b r):
+    /* electron-electron-nucleus kernel (D.3; reading Q22: every nucleus, every pair once and
+     * symmetrised = ordered pairs i != j with weight 1/2):
+     * term mu = (c/2) f(r_ai) g(r_aj) h(r_ij) with Pade factors p(r) = a r / (1 + b r):
      * dp/da = r / (1 + b r),  dp/db = -a r^2 / (1 + b r)^2.  Seven parameters per term, in the order of
      * een_params: c, a_f, b_f, a_g, b_g, a_h, b_h. */
     for (int mu = 0; mu < s->n_een; ++mu) {
@@ -700,13 +706,13 @@ int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64
             real rij = sqrt(xx * xx + yy * yy + zz * zz);
             real Df = 1.0 + q[2] * rai, Dg = 1.0 + q[4] * raj, Dh = 1.0 + q[6] * rij;
             real f = q[1] * rai / Df, g = q[3] * raj / Dg, h = q[5] * rij / Dh;
-            dq[0] += f * g * h;
-            dq[1] += q[0] * (rai / Df) * g * h;
-            dq[2] += q[0] * (-q[1] * rai * rai / (Df * Df)) * g * h;
-            dq[3] += q[0] * f * (raj / Dg) * h;
-            dq[4] += q[0] * f * (-q[3] * raj * raj / (Dg * Dg)) * h;
-            dq[5] += q[0] * f * g * (rij / Dh);
-            dq[6] += q[0] * f * g * (-q[5] * rij * rij / (Dh * Dh));
+            dq[0] += 0.5 * f * g * h;
+            dq[1] += 0.5 * q[0] * (rai / Df) * g * h;
+            dq[2] += 0.5 * q[0] * (-q[1] * rai * rai / (Df * Df)) * g * h;
+            dq[3] += 0.5 * q[0] * f * (raj / Dg) * h;
+            dq[4] += 0.5 * q[0] * f * (-q[3] * raj * raj / (Dg * Dg)) * h;
+            dq[5] += 0.5 * q[0] * f * g * (rij / Dh);
+            dq[6] += 0.5 * q[0] * f * g * (-q[5] * rij * rij / (Dh * Dh));
           }
       for (int k = 0; k < 7; ++k) out[6 + 7 * mu + k] = dq[k];
     }
@@ -849,7 +855,7 @@ int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, i
 /*                         sum_{beta on a} C[beta][lst_n[j]] grad ao_beta(r_i)  */
 /* and the Jastrow kernels that see the nuclei (D.2, D.3) add           */
 /*   d K_en(r_ia) / d R_a = -K_en' e_ai,                                 */
-/*   d [c f(r_ai) g(r_aj) h(r_ij)] / d R_a = -c h (f' g e_ai + f g' e_aj). */
+/*   d [(c/2) f(r_ai) g(r_aj) h(r_ij)] / d R_a = -(c/2) h (f' g e_ai + f g' e_aj). */
 /* The Pade e-e kernel D.1 does not depend on R.                        */
 /* ------------------------------------------------------------------ */
 
@@ -924,7 +930,7 @@ int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, 
           real K1 = ((jw0 + 2.0 * jw1 * ria) * D - N * jw2) / (D * D);
           for (int c = 0; c < 3; ++c) out[3 * at + c] -= K1 * d[c] / ria;
         }
-    /* electron-electron-nucleus kernel D.3 (reading Q22: ordered pairs i != j, every nucleus) */
+    /* electron-electron-nucleus kernel D.3 (reading Q22: ordered pairs i != j with weight 1/2) */
     for (int at = 0; at < na; ++at)
       for (int i = 0; i < ne; ++i)
         for (int j = 0; j < ne; ++j) {
@@ -945,7 +951,7 @@ int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, 
             pade3(q[3], q[4], raj, &g, &g1, &g2);
             pade3(q[5], q[6], rij, &h, &h1, &h2);
             for (int c = 0; c < 3; ++c)
-              out[3 * at + c] -= q[0] * h * (f1 * g * eai[c] / rai + f * g1 * eaj[c] / raj);
+              out[3 * at + c] -= 0.5 * q[0] * h * (f1 * g * eai[c] / rai + f * g1 * eaj[c] / raj);
           }
         }
   }

@@ -48,7 +48,9 @@ typedef struct {
   double jastrow_en_w0, jastrow_en_w1, jastrow_en_w2;
   /* electron-electron-nucleus kernel (D.3): n_een terms, each 7 doubles
    * (c, a1, b1, a2, b2, a3, b3):  K_een = sum_mu c [a1 r_ai/(1+b1 r_ai)] [a2 r_aj/(1+b2 r_aj)] [a3 r_ij/(1+b3 r_ij)],
-   * summed over every nucleus a and every ORDERED electron pair i != j (reading Q22); n_een = 0 = absent */
+   * summed over every nucleus a and every electron pair once (eq. 5: sum_{alpha, i>j}), each pair
+   * symmetrised, 1/2 [K(r_ai, r_aj, r_ij) + K(r_aj, r_ai, r_ij)] (reading Q22: equal to the literal sum when the first
+   * two factors coincide, exchange-symmetric when they do not); n_een = 0 = absent */
   int32_t n_een;
   const double *een_params; /* [n_een][7] or NULL */
 } oracle_system_desc_t;

@@ -44,8 +44,8 @@ def lib():
     """Load libqmcb200.so (building it with nvcc if the sources are newer)."""
     global _lib
     if _lib is None:
-        so = os.environ.get("QMC_LIB") or _build.SO  # QMC_LIB: an alternative build (kernel experiments)
-        if so == _build.SO and _build.needs_build():
+        so = _build.SO
+        if _build.needs_build():
             so = _build.build()
         if not os.path.exists(so):
             raise ImportError("libqmcb200.so is missing and could not be built; there is no CPU fallback")

@@ -223,8 +223,10 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     return QMC_EUNSUPPORTED;
   }
   P.n_een = d->n_een;
+  // D.3 enters eq. 5 once per pair, symmetrised (reading Q22): the kernels run over ordered
+  // pairs, so they carry c / 2
   for (int mu = 0; mu < d->n_een; ++mu)
-    for (int t = 0; t < 7; ++t) P.een[mu][t] = d->een_params[7 * mu + t];
+    for (int t = 0; t < 7; ++t) P.een[mu][t] = (t == 0 ? 0.5 : 1.0) * d->een_params[7 * mu + t];
   for (int a = 0; a < d->n_atoms; ++a) {
     for (int c = 0; c < 3; ++c) P.atom[a][c] = d->atom_xyz[3 * a + c];
     P.atom[a][3] = d->atom_Z[a];

@@ -79,8 +79,10 @@ __device__ __noinline__ void excite_general(const GenSpin *g, const double *T, i
 }
 
 // ---------------------------------------------------------------------------------
-// Electron-electron-nucleus Jastrow kernel (D.3; reading Q22): for the lane's electron i
-//   J_een = sum_a sum_{j != i} sum_mu c f(r_ai) g(r_aj) h(r_ij)   (ordered pairs), Pade factors p(r) = a r/(1 + b r).
+// Electron-electron-nucleus Jastrow kernel (D.3): eq. 5 sums it over every nucleus and every
+// pair once; each pair enters symmetrised, 1/2 [K(r_ai, r_aj, r_ij) + K(r_aj, r_ai, r_ij)] (reading Q22), i.e.
+//   J_een = sum_a sum_{i != j} sum_mu c f(r_ai) g(r_aj) h(r_ij)   over ORDERED pairs with c = c_mu / 2 (P.een[mu][0],
+// halved by qmc_setup), Pade factors p(r) = a r/(1 + b r).  For the lane's electron i:
 // The lane keeps only its own electron's share: of the two ordered pairs (i,j) and (j,i)
 //   u  = c (g_j f_i + f_j g_i),  v' = c (g_j f'_i + f_j g'_i),  vL = c (g_j (f''_i + 2f'_i/r_ai) + f_j (g''_i + 2g'_i/r_ai))
 //   J share 1/2 u h;  grad_i += v' h e_ai + u h' e_ij;  lap_i += vL h + u (h'' + 2h'/r_ij) + 2 v' h' e_ai.e_ij.
@@ -170,7 +172,8 @@ __device__ __noinline__ void een_terms(const SysParams &P, const double *sXYZ, i
 
 // Parameter derivatives of the e-e-n kernel (eq. 6 factors of D.3): for the lane's electron i and term mu the sums over
 // nuclei a and partners j != i (the ordered pairs that start at i) of d(c f(r_ai) g(r_aj) h(r_ij))/d(c, a_f, b_f, a_g,
-// b_g, a_h, b_h), with p = a r/(1 + b r): dp/da = r/(1 + b r) =: P, dp/db = -a r^2/(1 + b r)^2 = -p P.  Out of line.
+// b_g, a_h, b_h), with p = a r/(1 + b r): dp/da = r/(1 + b r) =: P, dp/db = -a r^2/(1 + b r)^2 = -p P.  q0 = c / 2 is the
+// weight of an ordered pair (reading Q22), so d/dc carries the 1/2 explicitly.  Out of line.
 __device__ __noinline__ void een_param_terms(const SysParams &P, const double *sXYZ, int base, int ne, int e, double x,
                                              double y, double z, int mu, double *dq) {
   const double q0 = P.een[mu][0], q1 = P.een[mu][1], q2 = P.een[mu][2], q3 = P.een[mu][3], q4 = P.een[mu][4],
@@ -204,7 +207,7 @@ __device__ __noinline__ void een_param_terms(const SysParams &P, const double *s
       s6 = fma(fg, hb, s6);
     }
   }
-  dq[0] = s0;
+  dq[0] = 0.5 * s0;
   dq[1] = q0 * s1;
   dq[2] = q0 * s2;
   dq[3] = q0 * s3;

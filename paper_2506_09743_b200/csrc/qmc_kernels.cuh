@@ -136,6 +136,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
       io.fb_part[(item * G + lane) * 2 + 1] = res[1];   // F.2 / F.4 with G.7
     }
     __threadfence();
+    __syncwarp();  // every lane's partial is stored and fenced before lane 0 publishes the slice as done
     int last = 0;
     if (lane == 0) last = (atomicAdd(io.fb_done + entry, 1) == SL - 1) ? 1 : 0;
     last = __shfl_sync(0xffffffffu, last, 0);
@@ -371,7 +372,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
 // ---------------------------------------------------------------------------------
 // Nuclear dependence of the Jastrow factor (eq. 7's grad_alpha ln rho): dR[w][a][c] = d J / d R_a,c
 //   D.2: K(r_ia) = (w0 r + w1 r^2) / (1 + w2 r)              ->  -K' e_ai
-//   D.3: c f(r_ai) g(r_aj) h(r_ij), ordered pairs i != j      ->  -c h (f' g e_ai + f g' e_aj)
+//   D.3: c f(r_ai) g(r_aj) h(r_ij), ordered pairs i != j, c = c_mu / 2 (reading Q22)  ->  -c h (f' g e_ai + f g' e_aj)
 // One thread per walker (SoA loads coalesce); writes every entry, zeros without those kernels.  The AO part is
 // subtracted afterwards by orbital_derivatives_kernel in nuclear mode.
 // ---------------------------------------------------------------------------------

@@ -725,7 +725,8 @@ def _with_een(d, een=EEN):
 
 
 def test_een_jastrow_closed_form_two_electrons():
-    # two electrons, one nucleus at the origin: J_een = sum_mu c [f(r1) g(r2) + f(r2) g(r1)] h(r12)  (ordered pairs, Q22)
+    # two electrons, one nucleus at the origin: the one pair of eq. 5's sum_{alpha, i>j}, symmetrised
+    # (reading Q22): J_een = sum_mu (c/2) [f(r1) g(r2) + f(r2) g(r1)] h(r12)
     d0 = atom_system(2.0, [(1, 0, 0, 1.7)], [[1.0]], 1, 1, a_par=0.25, a_anti=0.5, b=0.9)
     rr = _rand_pos(60, 2, 1.2, rmin=0.05, seed=91)
     lp0 = ob.local_energy(ob.OracleSystem(d0), soa(rr))[0]
@@ -733,9 +734,37 @@ def test_een_jastrow_closed_form_two_electrons():
     r1, r2 = np.linalg.norm(rr[:, 0], axis=1), np.linalg.norm(rr[:, 1], axis=1)
     r12 = np.linalg.norm(rr[:, 0] - rr[:, 1], axis=1)
     pade = lambda a, b, r: a * r / (1 + b * r)
-    J = sum(c * (pade(a1, b1, r1) * pade(a2, b2, r2) + pade(a1, b1, r2) * pade(a2, b2, r1)) * pade(a3, b3, r12)
+    J = sum(0.5 * c * (pade(a1, b1, r1) * pade(a2, b2, r2) + pade(a1, b1, r2) * pade(a2, b2, r1)) * pade(a3, b3, r12)
             for c, a1, b1, a2, b2, a3, b3 in EEN)
     assert np.max(np.abs((lp1 - lp0) - J)) < 1e-13
+
+
+def test_een_jastrow_equals_the_literal_pair_sum_of_eq5_for_symmetric_factors():
+    # eq. 5 with D.3 as printed: J_een = sum_alpha sum_{i>j} sum_mu c f(r_ai) g(r_aj) h(r_ij).
+    # With a1 = a2, b1 = b2 (f = g) the symmetrised reading Q22 must reproduce that hand sum exactly -- on a
+    # three-centre, five-electron system so that a factor 2, a missing nucleus or a missing pair all show.
+    een = np.array([[0.30, 0.8, 0.9, 0.8, 0.9, 0.7, 0.6], [-0.12, 1.1, 0.4, 1.1, 0.4, 0.35, 1.2]])
+    xyz = np.array([[0.0, 0.0, 0.0], [0.0, 0.9, 1.8], [1.1, -0.4, 0.3]])
+    from paper_2506_09743_b200.workloads import SystemDesc
+    aos = [(1, 0, 0, 1.3), (1, 0, 0, 0.9), (2, 1, 2, 1.1), (2, 0, 0, 0.8)]
+    d = SystemDesc("3c", xyz, np.array([2.0, 1.0, 2.0]), 3, 2, np.array([0, 1, 2, 2], np.int32),
+                   np.array([a[0] for a in aos], np.int32), np.array([a[1] for a in aos], np.int32),
+                   np.array([a[2] for a in aos], np.int32), np.array([a[3] for a in aos]), None,
+                   np.random.default_rng(5).standard_normal((4, 3)), np.array([[0, 1, 2]], np.int32),
+                   np.array([[0, 1]], np.int32), np.array([1.0]), 0.25, 0.5, 0.9)
+    rr = _rand_pos(25, 5, 1.5, rmin=0.05, seed=93)
+    lp0 = ob.local_energy(ob.OracleSystem(d), soa(rr))[0]
+    lp1 = ob.local_energy(ob.OracleSystem(_with_een(d, een)), soa(rr))[0]
+    pade = lambda a, b, r: a * r / (1 + b * r)
+    J = np.zeros(len(rr))
+    for A in xyz:
+        for i in range(5):
+            for j in range(i):          # i > j: every pair once
+                rai, raj = np.linalg.norm(rr[:, i] - A, axis=1), np.linalg.norm(rr[:, j] - A, axis=1)
+                rij = np.linalg.norm(rr[:, i] - rr[:, j], axis=1)
+                for c, a1, b1, a2, b2, a3, b3 in een:
+                    J += c * pade(a1, b1, rai) * pade(a2, b2, raj) * pade(a3, b3, rij)
+    assert np.max(np.abs((lp1 - lp0) - J)) < 1e-12
 
 
 def test_een_jastrow_finite_differences_exchange_and_sampler_value():
@@ -754,7 +783,7 @@ def test_een_jastrow_finite_differences_exchange_and_sampler_value():
         out = ob.metropolis(o, rk, 0.2, 0, seed=1)    # value-only route of the sampler
         assert np.max(np.abs(out["logpsi"] - lp)) < 1e-12
         # exchanging two same-spin electrons: |Psi| and E_L unchanged, sign flips (the kernel is symmetric only
-        # because BOTH ordered pairs are summed: f != g in EEN)
+        # because every pair enters symmetrised: f != g in EEN)
         rx = rk.copy()
         rx[[0, 1]] = rx[[1, 0]]
         lpx, sgx, elx = ob.local_energy(o, rx)
@@ -802,7 +831,7 @@ def test_een_parameter_derivatives_vs_central_differences_closed_form_and_layout
         # the first six columns do not depend on the D.3 terms
         O0 = ob.log_derivatives(ob.OracleSystem(_with_een(d, np.zeros((0, 7)))), r)
         assert np.array_equal(O0[:, :NJ], O[:, :NJ]) and O0.shape[1] == NJ + len(d.ci_coeff)
-    # two electrons, one nucleus: J_een = sum_mu c [f(r1) g(r2) + f(r2) g(r1)] h(r12)
+    # two electrons, one nucleus: J_een = sum_mu (c/2) [f(r1) g(r2) + f(r2) g(r1)] h(r12)
     d0 = _with_een(atom_system(2.0, [(1, 0, 0, 1.7)], [[1.0]], 1, 1, a_par=0.25, a_anti=0.5, b=0.9))
     rr = _rand_pos(40, 2, 1.2, rmin=0.05, seed=92)
     O = ob.log_derivatives(ob.OracleSystem(d0), soa(rr))
@@ -818,7 +847,7 @@ def test_een_parameter_derivatives_vs_central_differences_closed_form_and_layout
                 c * (f1 * da(a2, b2, r2) + f2 * da(a2, b2, r1)) * hh, c * (f1 * db(a2, b2, r2) + f2 * db(a2, b2, r1)) * hh,
                 c * (f1 * g2 + f2 * g1) * da(a3, b3, r12), c * (f1 * g2 + f2 * g1) * db(a3, b3, r12)]
         for k in range(7):
-            assert np.max(np.abs(O[:, NJ + 7 * mu + k] - want[k])) < 1e-13, (mu, k)
+            assert np.max(np.abs(O[:, NJ + 7 * mu + k] - 0.5 * want[k])) < 1e-13, (mu, k)
 
 
 # ---------------------------------------------------------------- orbital parameters (AO exponents, MO coefficients)
