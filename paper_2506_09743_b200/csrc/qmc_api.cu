@@ -86,6 +86,69 @@ const std::vector<Variant> &variants() {
   return v;
 }
 
+// Scratch of the handle-less reductions (qmc_batch_stats, qmc_energy_gradient), one per (device, stream), created on
+// first use and kept for the life of the process: block partials and the completion counter in device memory, the
+// result in mapped page-locked host memory that the last block writes directly (no allocation, no copy on the call).
+struct ReduceScratch {
+  double *d_partial = nullptr;   // [kReduceBlocks][3] {n, mean, M2} of batch_stats_kernel
+  unsigned int *d_done = nullptr;
+  double *d_stats = nullptr;     // [2] mean, stderr in device memory (read by the gradient kernels)
+  double *h_res = nullptr;       // mapped host memory: [2] mean, stderr, then [res_params] gradient
+  double *d_res = nullptr;       // device alias of h_res
+  size_t res_params = 0;
+  double *d_gpart = nullptr;     // [blocks][n_param] partials of gradient_partial_kernel
+  size_t gpart_doubles = 0;
+};
+constexpr int kReduceBlocks = 592;  // 4 per SM on 148 SMs; any value gives the same result up to rounding order
+std::mutex g_reduce_mu;
+std::unordered_map<uint64_t, ReduceScratch> g_reduce;
+
+int device_of(const void *p, int *dev) {
+  cudaPointerAttributes at{};
+  cudaError_t e = cudaPointerGetAttributes(&at, p);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaPointerGetAttributes");
+  if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged) {
+    g_cuda_err = "pointer is not device memory";
+    return QMC_ECUDA;
+  }
+  *dev = at.device;
+  return QMC_OK;
+}
+
+// the scratch of (dev, st) with room for n_param gradient entries and gpart doubles of partials
+int reduce_scratch(int dev, cudaStream_t st, size_t n_param, size_t gpart, ReduceScratch **out) {
+  std::lock_guard<std::mutex> lock(g_reduce_mu);
+  ReduceScratch &r = g_reduce[((uint64_t)(uint32_t)dev << 48) ^ (uint64_t)(uintptr_t)st];
+  if (!r.d_partial) {
+    CK(cudaMalloc(&r.d_partial, sizeof(double) * 3 * kReduceBlocks));
+    CK(cudaMalloc(&r.d_done, sizeof(unsigned int)));
+    CK(cudaMemset(r.d_done, 0, sizeof(unsigned int)));
+    CK(cudaMalloc(&r.d_stats, sizeof(double) * 2));
+  }
+  if (!r.h_res || r.res_params < n_param) {  // grow (previous results have been consumed: the calls synchronise)
+    if (r.h_res) {
+      CK(cudaStreamSynchronize(st));
+      cudaFreeHost(r.h_res);
+      r.h_res = nullptr;
+    }
+    const size_t np = std::max<size_t>(n_param, 1024);
+    CK(cudaHostAlloc(&r.h_res, sizeof(double) * (2 + np), cudaHostAllocMapped));
+    CK(cudaHostGetDevicePointer(&r.d_res, r.h_res, 0));
+    r.res_params = np;
+  }
+  if (r.gpart_doubles < gpart) {
+    if (r.d_gpart) {
+      CK(cudaStreamSynchronize(st));
+      cudaFree(r.d_gpart);
+      r.d_gpart = nullptr;
+    }
+    CK(cudaMalloc(&r.d_gpart, sizeof(double) * gpart));
+    r.gpart_doubles = gpart;
+  }
+  *out = &r;
+  return QMC_OK;
+}
+
 double sto_norm(int n, int l, int m, double zeta) {
   double fact = 1.0;
   for (int i = 2; i <= 2 * n; ++i) fact *= i;
@@ -108,14 +171,15 @@ struct qmc_system {
   void *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr, *d_orig = nullptr, *d_yrec = nullptr, *d_ytgt = nullptr, *d_rowao = nullptr,
        *d_rownrm = nullptr;
   int n_sm = 0;
-  double *d_stats = nullptr;
-  unsigned long long *d_counter = nullptr;
   double flops_el = 0, flops_step = 0;
   // scratch of the explicit fallback, one buffer per calling stream (grown on demand, kept until qmc_destroy):
   // no allocation on the hot call, and the call can be captured in a CUDA graph after one warm-up call
-  struct Scratch { void *p = nullptr; size_t bytes = 0; };
+  // A buffer that has to grow is retired, not freed (a CUDA graph captured earlier may still replay into it); the
+  // accept counter of qmc_metropolis is per stream too.
+  struct Scratch { void *p = nullptr; size_t bytes = 0; unsigned long long *counter = nullptr; };
   std::mutex scratch_mu;
   std::unordered_map<cudaStream_t, Scratch> scratch;
+  std::vector<void *> retired;
   // qmc_local_energy_host: two internal streams and double-buffered device scratch (grown on demand)
   bool orb_ready = false;  // orbital-derivative kernel configured (lazily: most users never call it)
   int orb_warps = 0;
@@ -161,9 +225,11 @@ void qmc_destroy(qmc_system_t *s) {
   cudaFree(s->d_ytgt);
   cudaFree(s->d_rowao);
   cudaFree(s->d_rownrm);
-  cudaFree(s->d_stats);
-  cudaFree(s->d_counter);
-  for (auto &kv : s->scratch) cudaFree(kv.second.p);
+  for (auto &kv : s->scratch) {
+    cudaFree(kv.second.p);
+    cudaFree(kv.second.counter);
+  }
+  for (void *q : s->retired) cudaFree(q);
   for (int i = 0; i < 2; ++i) {
     if (s->hst[i]) cudaStreamDestroy(s->hst[i]);
     cudaFree(s->hbuf[i]);
@@ -604,8 +670,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   if (e != cudaSuccess) { delete s; return cuda_fail(e, "cudaSetDevice"); }
   const size_t szC = C.size() * sizeof(double), szD = dets.size() * sizeof(DetRec);
   if ((e = cudaMalloc(&s->d_C, szC)) != cudaSuccess ||
-      (e = cudaMalloc(&s->d_dets, szD)) != cudaSuccess || (e = cudaMalloc(&s->d_stats, 2 * sizeof(double))) != cudaSuccess ||
-      (e = cudaMalloc(&s->d_counter, sizeof(unsigned long long))) != cudaSuccess ||
+      (e = cudaMalloc(&s->d_dets, szD)) != cudaSuccess ||
       (e = cudaMemcpy(s->d_C, C.data(), szC, cudaMemcpyHostToDevice)) != cudaSuccess ||
       (e = cudaMemcpy(s->d_dets, dets.data(), szD, cudaMemcpyHostToDevice)) != cudaSuccess ||
       (e = cudaMalloc(&s->d_gen, std::max<size_t>(gens.size(), 1) * sizeof(GenDet))) != cudaSuccess ||
@@ -700,9 +765,8 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
     {
       std::lock_guard<std::mutex> lock(s->scratch_mu);
       qmc_system::Scratch &sc = s->scratch[st];
-      if (sc.bytes < need_bytes) {  // grow: earlier work on this stream may still use the old buffer
-        CK(cudaStreamSynchronize(st));
-        cudaFree(sc.p);
+      if (sc.bytes < need_bytes) {  // grow: the old buffer is kept until qmc_destroy (earlier work on this stream
+        if (sc.p) s->retired.push_back(sc.p);  // and graphs captured from earlier calls may still use it)
         sc.p = nullptr;
         sc.bytes = 0;
         CK(cudaMalloc(&sc.p, need_bytes));
@@ -840,8 +904,15 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
   mp.walker_offset = walker_offset;
   mp.accept = d_accept;
   mp.resume = 0;
-  mp.n_accepted = h_n_accepted ? s->d_counter : nullptr;
-  if (h_n_accepted) CK(cudaMemsetAsync(s->d_counter, 0, sizeof(unsigned long long), st));
+  unsigned long long *d_counter = nullptr;
+  if (h_n_accepted) {  // the accept counter belongs to the calling stream
+    std::lock_guard<std::mutex> lock(s->scratch_mu);
+    qmc_system::Scratch &sc = s->scratch[st];
+    if (!sc.counter) CK(cudaMalloc(&sc.counter, sizeof(unsigned long long)));
+    d_counter = sc.counter;
+  }
+  mp.n_accepted = d_counter;
+  if (h_n_accepted) CK(cudaMemsetAsync(d_counter, 0, sizeof(unsigned long long), st));
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
   const int64_t need = (groups + kWarpsPsi - 1) / kWarpsPsi;
   const int grid = (int)std::min<int64_t>(need, s->blocks_metro);
@@ -857,21 +928,30 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
     double *scratch = nullptr;  // [M] E_L of one sweep, then [M] log|Psi|, [M] sign if the caller gave none
     const size_t n_scr = (size_t)M * (1 + (d_logpsi ? 0 : 1) + (d_sign ? 0 : 1));
     CK(cudaMallocAsync(&scratch, n_scr * sizeof(double), st));
+    // every failure below releases the scratch before returning
+#define CKS(call)                                          \
+  do {                                                     \
+    cudaError_t e__ = (call);                              \
+    if (e__ != cudaSuccess) {                              \
+      cudaFreeAsync(scratch, st);                          \
+      return cuda_fail(e__, #call);                        \
+    }                                                      \
+  } while (0)
     double *nxt = scratch + M;
     if (!d_logpsi) { io.logpsi = nxt; nxt += M; }
     if (!d_sign) io.sign = nxt;
-    CK(cudaMemsetAsync(d_eloc_acc, 0, (size_t)M * sizeof(double), st));
+    CKS(cudaMemsetAsync(d_eloc_acc, 0, (size_t)M * sizeof(double), st));
     mp.n_sweeps = 1;
     if (n_sweeps == 0) {  // nothing to accumulate; still report log|Psi| of the starting positions
       mp.n_sweeps = 0;
-      CK(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_psi, st));
+      CKS(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_psi, st));
       ++g_launches;
     }
     for (int32_t sw = 0; sw < n_sweeps; ++sw) {
       mp.sweep0 = (uint32_t)(sweep_offset + (uint64_t)sw);
       mp.accept = d_accept ? d_accept + (size_t)sw * (size_t)M : nullptr;
       mp.resume = sw > 0 ? 1 : 0;
-      CK(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_psi, st));
+      CKS(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_psi, st));
       ++g_launches;
       int rc = launch_eval(s, d_r, M, nullptr, nullptr, scratch, st, true);
       if (rc != QMC_OK) {
@@ -879,13 +959,15 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
         return rc;
       }
       accumulate_kernel<<<(unsigned)std::min<int64_t>((M + 255) / 256, 4 * s->n_sm), 256, 0, st>>>(d_eloc_acc, scratch, M);
+      CKS(cudaGetLastError());
       ++g_launches;
     }
+#undef CKS
     CK(cudaFreeAsync(scratch, st));
   }
   if (h_n_accepted) {
     unsigned long long v = 0;
-    CK(cudaMemcpyAsync(&v, s->d_counter, sizeof(v), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(&v, d_counter, sizeof(v), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     *h_n_accepted = (int64_t)v;
   }
@@ -903,22 +985,24 @@ int qmc_log_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d
 int qmc_energy_gradient(const double *d_eloc, const double *d_O, int64_t M, int32_t n_param, double *h_Ev, double *h_grad,
                         void *cuda_stream) {
   if (!d_eloc || !d_O || M <= 0 || n_param < 1 || !h_grad) return QMC_EINVAL;
+  int dev = 0;
+  if (int rc = device_of(d_eloc, &dev)) return rc;
+  CK(cudaSetDevice(dev));
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int nblk = (int)std::min<int64_t>(1184, (M + 63) / 64);  // >= 64 rows per block
-  double *scr = nullptr;  // [2] stats, [n_param] gradient, [nblk][n_param] partials
-  CK(cudaMallocAsync(&scr, ((size_t)2 + (size_t)n_param * (size_t)(nblk + 1)) * sizeof(double), st));
-  double *d_stats = scr, *d_grad = scr + 2, *d_part = d_grad + n_param;
-  batch_stats_kernel<<<1, 1024, 0, st>>>(d_eloc, M, d_stats);
-  gradient_partial_kernel<<<nblk, 128, 0, st>>>(d_eloc, d_O, M, n_param, d_stats, d_part);
-  gradient_final_kernel<<<n_param, 128, 0, st>>>(d_part, nblk, n_param, M, d_grad);
+  ReduceScratch *r = nullptr;
+  if (int rc = reduce_scratch(dev, st, (size_t)n_param, (size_t)nblk * (size_t)n_param, &r)) return rc;
+  const int sblk = (int)std::min<int64_t>(kReduceBlocks, (M + kStatsThreads - 1) / kStatsThreads);
+  batch_stats_kernel<<<sblk, kStatsThreads, 0, st>>>(d_eloc, M, r->d_partial, r->d_done, r->d_stats);
+  CK(cudaGetLastError());
+  gradient_partial_kernel<<<nblk, 128, 0, st>>>(d_eloc, d_O, M, n_param, r->d_stats, r->d_gpart);
+  CK(cudaGetLastError());
+  gradient_final_kernel<<<n_param, 128, 0, st>>>(r->d_gpart, nblk, n_param, M, r->d_stats, r->d_res);
+  CK(cudaGetLastError());
   g_launches += 3;
-  std::vector<double> h((size_t)n_param + 2);
-  cudaError_t e = cudaMemcpyAsync(h.data(), scr, h.size() * sizeof(double), cudaMemcpyDeviceToHost, st);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  cudaFreeAsync(scr, st);
-  if (e != cudaSuccess) return cuda_fail(e, "qmc_energy_gradient");
-  if (h_Ev) *h_Ev = h[0];
-  for (int p = 0; p < n_param; ++p) h_grad[p] = h[2 + p];
+  CK(cudaStreamSynchronize(st));  // the final kernel wrote {E_v, stderr, grad[...]} into mapped host memory
+  if (h_Ev) *h_Ev = r->h_res[0];
+  for (int p = 0; p < n_param; ++p) h_grad[p] = r->h_res[2 + p];
   return QMC_OK;
 }
 
@@ -981,18 +1065,19 @@ int qmc_nuclear_log_gradient(qmc_system_t *s, const double *d_r, int64_t M, doub
 
 int qmc_batch_stats(const double *d_x, int64_t M, double *h_mean, double *h_stderr, void *cuda_stream) {
   if (!d_x || M <= 0) return QMC_EINVAL;
+  int dev = 0;
+  if (int rc = device_of(d_x, &dev)) return rc;
+  CK(cudaSetDevice(dev));
   cudaStream_t st = (cudaStream_t)cuda_stream;
-  double *d_out = nullptr;
-  CK(cudaMallocAsync(&d_out, 2 * sizeof(double), st));
-  batch_stats_kernel<<<1, 1024, 0, st>>>(d_x, M, d_out);
+  ReduceScratch *r = nullptr;
+  if (int rc = reduce_scratch(dev, st, 0, 0, &r)) return rc;
+  const int nblk = (int)std::min<int64_t>(kReduceBlocks, (M + kStatsThreads - 1) / kStatsThreads);
+  batch_stats_kernel<<<nblk, kStatsThreads, 0, st>>>(d_x, M, r->d_partial, r->d_done, r->d_res);
+  CK(cudaGetLastError());
   ++g_launches;
-  double h[2] = {0, 0};
-  cudaError_t e = cudaMemcpyAsync(h, d_out, sizeof(h), cudaMemcpyDeviceToHost, st);
-  if (e == cudaSuccess) e = cudaFreeAsync(d_out, st);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-  if (e != cudaSuccess) return cuda_fail(e, "qmc_batch_stats");
-  if (h_mean) *h_mean = h[0];
-  if (h_stderr) *h_stderr = h[1];
+  CK(cudaStreamSynchronize(st));  // the last block wrote {mean, stderr} into mapped host memory
+  if (h_mean) *h_mean = r->h_res[0];
+  if (h_stderr) *h_stderr = r->h_res[1];
   return QMC_OK;
 }
 

@@ -97,13 +97,31 @@ struct DetCols {
 // kFallbackK max(1, |E_L|): the table path (F.6/F.7) loses about log10((Sigma/D_0)^2) digits when the
 // reference determinant is nearly singular while the expansion is not.  Measured:
 // E_L error ~ 1.2e-15 (Sigma/D_0)^2, so K = 8e5 keeps it below 1e-9 max(1, |E_L|), a tenth of the parity bound.
-constexpr double kFallbackK = 8.0e5;
+#ifndef QMC_FALLBACK_K
+#define QMC_FALLBACK_K 8.0e5
+#endif
+constexpr double kFallbackK = QMC_FALLBACK_K;
 // ... and in any case when |Sigma / D_0| > 1e4: log|Psi| of the table path is off by ~1e-15 |Sigma/D_0| (1e-12 at
 // 1024), and its parity bound 1e-10 is ABSOLUTE, so walkers with a huge |E_L| must not escape through the first test.
-constexpr double kFallbackCap = 1.0e8;
+#ifndef QMC_FALLBACK_CAP
+#define QMC_FALLBACK_CAP 1.0e8
+#endif
+constexpr double kFallbackCap = QMC_FALLBACK_CAP;
+// The same loss when the reference ALONE is nearly singular while Sigma / D_0 stays moderate (the CI coefficients of
+// the large determinants are small): T, G, H carry relative errors eps * cond(A_0) and their O(cond^2) parts cancel.
+// kappa = max |T[p][q]| of a spin estimates cond(A_0) at no cost.  Measured on all 131072 CO, 32768 Li2 and
+// 32768 CO-500 walkers against the long-double oracle with the fallback off: worst error of
+// a walker with kappa^2 <= 1e6 max(1, |E_L|) is 2.8e-10 max(1, |E_L|); 0.12% / 0.16% / 0.07% of the walkers exceed it.
+// (The (Sigma/D_0)^2 test alone left a CO walker at 2.0e-7: kappa 4.8e4, Sigma/D_0 = -118.)
+#ifndef QMC_FALLBACK_KAPPA
+#define QMC_FALLBACK_KAPPA 1.0e6
+#endif
+constexpr double kFallbackKappa = QMC_FALLBACK_KAPPA;
+constexpr double kFallbackKappaCap = (QMC_FALLBACK_KAPPA > 1.0e100) ? QMC_FALLBACK_KAPPA : 1.0e10;
 // Orbital-parameter derivatives: the table-path error of Gamma is ~1.2e-15 (Sigma/D_0)^2 of the walker's largest
 // derivative (measured); beyond (Sigma/D_0)^2 = 1e4 the group takes the explicit route.
 constexpr double kFallbackOrb = 1.0e4;
+constexpr double kFallbackOrbKappa = 1.0e6;  // ... or kappa^2 beyond 1e6 (same conditioning estimate as E_L's)
 
 // One term of Y[spin][p][q] = d(Sigma/D_0)/dT[p][q]: w * R_other * T_spin[cof]  (w = d_n times the cofactor's sign;
 // oth = the other spin's 2x2 code {i11, i12, i21, i22} as in class-4 DetRec, constant slots for k < 2;

@@ -728,6 +728,19 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           for (int k2 = k + 1; k2 < NS; ++k2) inversions += (perm[k] > perm[k2]) ? 1 : 0;
         if (inversions & 1) det = -det;
       }
+      // kappa = max |T[p][q]| of this problem: the conditioning estimate of the explicit-fallback criterion
+      // (kFallbackKappa; T = A0^-1 Av blows up like 1/sigma_min(A0) when the reference alone is nearly singular).
+      // Arg-max on the high word of |T| (monotone for positive doubles; Inf and NaN of a singular reference sort above
+      // every finite value, are clamped to +Inf and so flag the walker): kappa to a relative 2^-20.
+      double kap = 0.0;
+      if (EL || ORB == 2) {
+        unsigned kk = 0u;
+#pragma unroll
+        for (int k = 0; k < NS; ++k) kk = max(kk, (unsigned)(__double2hiint(av[k]) & 0x7fffffff));  // columns c >= nv hold zeros
+#pragma unroll
+        for (int m = 1; m < LP; m <<= 1) kk = max(kk, __shfl_xor_sync(0xffffffffu, kk, m));
+        kap = __hiloint2double((int)min(kk, 0x7ff00000u), 0);  // Inf for every non-finite entry
+      }
       // t0 = Tr(A0^-1 B0)   (G.7, applied to the combined operator)
       double t0 = 0.0;
       if (EL) {
@@ -770,6 +783,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           sProb[pr * 4 + 0] = log(fabs(det));
           sProb[pr * 4 + 1] = (det > 0.0) ? 1.0 : ((det < 0.0) ? -1.0 : 0.0);
           sProb[pr * 4 + 2] = t0;
+          if (EL || ORB == 2) sProb[pr * 4 + 3] = kap;
         }
       }
     }
@@ -871,10 +885,16 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       sRes[wg * 4 + 1] = sgn * ((den > 0.0) ? 1.0 : ((den < 0.0) ? -1.0 : 0.0));
       const double eloc = EL ? esum + (sProb[pu * 4 + 2] + sProb[pd * 4 + 2]) + num / den + P.vnn : 0.0;
       if (EL) sRes[wg * 4 + 2] = eloc;
-      // explicit fallback when the estimated table-path error of E_L, 1.2e-15 (Sigma/D_0)^2, exceeds a tenth of the
-      // parity bound 1e-8 max(1, |E_L|), or that of log|Psi|, ~1e-15 |Sigma/D_0|, a tenth of its absolute bound
-      // 1e-10 (kFallbackCap); also set for NaN (singular reference)
-      sRes[wg * 4 + 3] = (den * den <= fmin(kFallbackK * fmax(1.0, fabs(eloc)), kFallbackCap)) ? 0.0 : 1.0;
+      // explicit fallback when the estimated table-path error of E_L exceeds a tenth of the parity bound
+      // 1e-8 max(1, |E_L|): ~1e-15 kappa^2 with kappa = max |T| of either spin (a nearly
+      // singular reference whatever the size of Sigma) or 1.2e-15 (Sigma/D_0)^2; or when that of log|Psi|,
+      // ~1e-15 max(kappa, |Sigma/D_0|), nears a tenth of its absolute bound 1e-10 (the two caps); NaN / Inf flag too
+      if (EL) {
+        const double ku = sProb[pu * 4 + 3], kd = sProb[pd * 4 + 3];
+        const double scale = fmax(1.0, fabs(eloc)), kthr = fmin(kFallbackKappa * scale, kFallbackKappaCap);
+        const bool ok = (den * den <= fmin(kFallbackK * scale, kFallbackCap)) && (ku * ku <= kthr) && (kd * kd <= kthr);
+        sRes[wg * 4 + 3] = ok ? 0.0 : 1.0;
+      }
     }
     if (ORB == 2) {
       // ---- Gamma = d ln Sigma / d Phi from the reference alone (lane c of a problem = electron c of that spin):
@@ -887,7 +907,11 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       const double *sInvF = ws + GE::oInv;
       for (int i = lane; i < 2 * G * TS; i += 32) sY[i] = 0.0;
       for (int i = lane; i < GE::ROWS * NMO; i += 32) sGamF[i] = 0.0;
-      if (wvalid && sub == 0) sProb[pu * 4 + 3] = den;
+      if (wvalid && sub == 0) {  // {Sigma / D_0, kappa} for the caller's choice of route
+        const double ku = sProb[pu * 4 + 3], kd = sProb[pd * 4 + 3];
+        sProb[pu * 4 + 3] = den;
+        sProb[pd * 4 + 3] = (ku <= kd) ? kd : ku;  // the larger (non-finite entries arrive as +Inf)
+      }
       __syncwarp();
       if (wvalid)
         for (int t = sub; t < P.n_ytgt; t += LW) {

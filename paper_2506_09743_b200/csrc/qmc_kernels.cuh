@@ -221,7 +221,8 @@ __global__ void __launch_bounds__(WPB * 32, 1)
       eval_walkers<NS, NMO, false, X, false, false, false, 2>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
       for (int gg = 0; gg < G; ++gg) {
         const double den = (ws + GE::oProb)[gg * 8 + 3];  // Sigma / D_0 of walker gg (NaN for a singular reference)
-        expl |= !(den * den <= kFallbackOrb);
+        const double kap = (ws + GE::oProb)[gg * 8 + 7];  // max |T| over both spins
+        expl |= !(den * den <= kFallbackOrb) || !(kap * kap <= kFallbackOrbKappa);
       }
       __syncwarp();
     }
@@ -564,7 +565,7 @@ __global__ void __launch_bounds__(128) gradient_partial_kernel(const double *__r
   }
 }
 __global__ void __launch_bounds__(128) gradient_final_kernel(const double *__restrict__ partial, int nblk, int np, int64_t M,
-                                                             double *__restrict__ grad) {
+                                                             const double *__restrict__ stats, double *__restrict__ res) {
   // one block per parameter: thread t adds the block partials t, t + 128, ... in order, then a fixed tree
   __shared__ double sh[128];
   const int p = blockIdx.x;
@@ -580,50 +581,100 @@ __global__ void __launch_bounds__(128) gradient_final_kernel(const double *__res
     if ((int)threadIdx.x < w) sh[threadIdx.x] += sh[threadIdx.x + w];
     __syncthreads();
   }
-  if (threadIdx.x == 0) grad[p] = 2.0 * sh[0] / (double)M;
+  if (threadIdx.x == 0) {  // res (mapped host memory) = {E_v, stderr, grad[0 .. np-1]}
+    res[2 + p] = 2.0 * sh[0] / (double)M;
+    if (p == 0) { res[0] = stats[0]; res[1] = stats[1]; }
+  }
 }
 
 // ---------------------------------------------------------------------------------
-// batch mean and standard error (eq. 3): one block, fixed tree, two passes
-// out[0] = mean, out[1] = stderr
+// batch mean and standard error (eq. 3).  One launch, every SM: block b takes a contiguous range of
+// the M values and reduces it to {n_b, mean_b, M2_b = sum (x - mean_b)^2} (two passes over its own range, Kahan
+// per thread, fixed shuffle tree); the block that finishes last combines the partials pairwise in a fixed tree
+// with the exact update  n = n_a + n_b, d = mean_b - mean_a, mean = mean_a + d n_b / n,
+// M2 = M2_a + M2_b + d^2 n_a n_b / n  -- deterministic, no atomics on the data -- and writes
+// out[0] = mean, out[1] = stderr (out may be mapped host memory).
 // ---------------------------------------------------------------------------------
-__device__ __forceinline__ double block_sum_1024(double v, double *sh) {
+constexpr int kStatsThreads = 256;
+__device__ __forceinline__ double block_sum_256(double v, double *sh) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int m = 16; m > 0; m >>= 1) v += shfl_xor_d(v, m);
   __syncthreads();
   if (lane == 0) sh[warp] = v;
   __syncthreads();
-  double t = (threadIdx.x < (blockDim.x >> 5)) ? sh[threadIdx.x] : 0.0;
+  double t = (threadIdx.x < (kStatsThreads >> 5)) ? sh[threadIdx.x] : 0.0;
   if (warp == 0) {
-    for (int m = 16; m > 0; m >>= 1) t += shfl_xor_d(t, m);
-    if (lane == 0) sh[32] = t;
+    for (int m = 4; m > 0; m >>= 1) t += shfl_xor_d(t, m);
+    if (lane == 0) sh[8] = t;
   }
   __syncthreads();
-  return sh[32];
+  return sh[8];
 }
 
-__global__ void __launch_bounds__(1024) batch_stats_kernel(const double *__restrict__ x, int64_t M, double *out) {
-  __shared__ double sh[33];
-  // pass 1: Kahan partial sums per thread
+__global__ void __launch_bounds__(kStatsThreads) batch_stats_kernel(const double *__restrict__ x, int64_t M, double *__restrict__ partial,
+                                                                    unsigned int *__restrict__ done, double *__restrict__ out) {
+  __shared__ double sh[9];
+  __shared__ double cn[kStatsThreads], cm[kStatsThreads], c2[kStatsThreads];
+  __shared__ int is_last;
+  const int64_t per = (M + gridDim.x - 1) / gridDim.x;
+  const int64_t i0 = (int64_t)blockIdx.x * per, i1 = (i0 + per < M) ? i0 + per : M;
+  const double nb = (i1 > i0) ? (double)(i1 - i0) : 0.0;
   double s = 0.0, c = 0.0;
-  for (int64_t i = threadIdx.x; i < M; i += blockDim.x) {
-    double y = x[i] - c, t = s + y;
+  for (int64_t i = i0 + threadIdx.x; i < i1; i += kStatsThreads) {
+    const double y = x[i] - c, t = s + y;
     c = (t - s) - y;
     s = t;
   }
-  const double mean = block_sum_1024(s, sh) / (double)M;
+  const double tot = block_sum_256(s, sh);
+  const double mean = (nb > 0.0) ? tot / nb : 0.0;
   s = 0.0;
   c = 0.0;
-  for (int64_t i = threadIdx.x; i < M; i += blockDim.x) {
-    double d = x[i] - mean;
-    double y = d * d - c, t = s + y;
+  for (int64_t i = i0 + threadIdx.x; i < i1; i += kStatsThreads) {
+    const double d = x[i] - mean;
+    const double y = d * d - c, t = s + y;
     c = (t - s) - y;
     s = t;
   }
-  const double ss = block_sum_1024(s, sh);
+  const double m2 = block_sum_256(s, sh);
   if (threadIdx.x == 0) {
-    out[0] = mean;
-    out[1] = (M > 1) ? sqrt(ss / (double)(M - 1) / (double)M) : 0.0;
+    partial[3 * blockIdx.x + 0] = nb;
+    partial[3 * blockIdx.x + 1] = mean;
+    partial[3 * blockIdx.x + 2] = m2;
+    __threadfence();
+    is_last = (atomicAdd(done, 1u) == gridDim.x - 1) ? 1 : 0;
+  }
+  __syncthreads();
+  if (!is_last) return;
+  __threadfence();
+  // thread t folds the partials t, t + 256, ... in order, then a fixed binary tree over the threads
+  double n = 0.0, mu = 0.0, q = 0.0;
+  for (int b = threadIdx.x; b < (int)gridDim.x; b += kStatsThreads) {
+    const double n2 = __ldcg(partial + 3 * b), mu2 = __ldcg(partial + 3 * b + 1), q2 = __ldcg(partial + 3 * b + 2);
+    if (n2 > 0.0) {
+      const double nt = n + n2, dl = mu2 - mu;
+      mu = fma(dl, n2 / nt, mu);
+      q = q + q2 + dl * dl * (n * n2 / nt);
+      n = nt;
+    }
+  }
+  cn[threadIdx.x] = n; cm[threadIdx.x] = mu; c2[threadIdx.x] = q;
+  __syncthreads();
+  for (int w = kStatsThreads / 2; w > 0; w >>= 1) {
+    if ((int)threadIdx.x < w) {
+      const double na = cn[threadIdx.x], nb2 = cn[threadIdx.x + w];
+      if (nb2 > 0.0) {
+        const double nt = na + nb2, dl = cm[threadIdx.x + w] - cm[threadIdx.x];
+        cm[threadIdx.x] = fma(dl, nb2 / nt, cm[threadIdx.x]);
+        c2[threadIdx.x] = c2[threadIdx.x] + c2[threadIdx.x + w] + dl * dl * (na * nb2 / nt);
+        cn[threadIdx.x] = nt;
+      }
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    out[0] = cm[0];
+    out[1] = (M > 1) ? sqrt(c2[0] / (double)(M - 1) / (double)M) : 0.0;
+    *done = 0u;  // ready for the next launch on this stream
   }
 }
 
