@@ -57,3 +57,48 @@ def hydrogenic_set(Z):
     for k in (6, 10, 7, 8, 9):
         cols.append(col(**{f"a{k}": 1.0})); e.append(-Z * Z / 18)
     return aos, np.stack(cols, axis=1), np.array(e)
+
+
+def adjudicate(gpu, o64, ox, tol, scale=None, mask=None, what=""):
+    """Parity with adjudication by the extended-precision oracle (reading Q24).
+
+    gpu / o64 / ox: the CUDA result, the float64 oracle's and the long-double build's of the same oracle source,
+    arrays whose first axis is the walker.  Per walker (max over the other axes), with e = |.|/scale:
+      * where the float64 oracle is itself pinned by the extended run to a tenth of the bound, e(o64, ox) <= tol/10,
+        the contract is asserted literally:  e(gpu, o64) <= tol;
+      * elsewhere (counted and returned: walkers on which float64 arithmetic of this kind cannot deliver the bound --
+        a nearly singular Slater matrix, a CI sum that cancels) the CUDA result must be as good as the float64
+        oracle's: e(gpu, ox) <= max(tol, 4 e(o64, ox)).
+    Returns the number of such exceptions inside `mask`."""
+    import numpy as np
+    gpu, o64, ox = (np.asarray(a, np.float64) for a in (gpu, o64, ox))
+    sc = 1.0 if scale is None else np.asarray(scale, np.float64)
+
+    def per_walker(a):
+        a = np.abs(a) / sc
+        return a.reshape(a.shape[0], -1).max(axis=1) if a.ndim > 1 else a
+
+    with np.errstate(invalid="ignore"):
+        e_g64, e_gx, e_64x = per_walker(gpu - o64), per_walker(gpu - ox), per_walker(o64 - ox)
+    m = np.ones(e_g64.shape[0], bool) if mask is None else np.asarray(mask, bool)
+    pinned = m & (e_64x <= tol / 10)
+    exc = m & ~(e_64x <= tol / 10)
+    bad = pinned & ~(e_g64 <= tol)
+    assert not bad.any(), (what, "pinned walkers beyond the bound", [(int(i), float(e_g64[i])) for i in np.flatnonzero(bad)[:8]])
+    bad = exc & ~(e_gx <= np.maximum(tol, 4 * e_64x))
+    assert not bad.any(), (what, "exceptions worse than the float64 oracle",
+                           [(int(i), float(e_gx[i]), float(e_64x[i])) for i in np.flatnonzero(bad)[:8]])
+    return int(exc.sum())
+
+
+def golden_values(name):
+    """name -> float from a two-column text fixture under tests/golden (lines starting with # are citations)."""
+    import os
+    out = {}
+    with open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", name)) as f:
+        for line in f:
+            line = line.strip()
+            if line and not line.startswith("#"):
+                k, v = line.split()
+                out[k] = float(v)
+    return out

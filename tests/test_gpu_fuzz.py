@@ -70,10 +70,16 @@ def random_system(seed, case):
 
 @pytest.mark.parametrize("seed", [11, 12])
 def test_random_systems_against_the_oracle(seed):
+    """The contract's own tolerances (sign exact, log|Psi| 1e-10, E_L / O_p / orbital derivatives 1e-8 max(1, |.|), accept
+    masks outside a 1e-12 window) on every walker the float64 oracle is pinned on by its long-double build; random
+    orbitals make badly conditioned Slater matrices common, and those walkers are adjudicated by the long-double run
+    (tests.helpers.adjudicate, reading Q24) and counted."""
     import torch
     from oracle import binding as ob
     from paper_2506_09743_b200 import binding as qb
-    evaluated = 0
+    from tests.helpers import adjudicate
+    evaluated = walkers = 0
+    exc = dict(lp=0, el=0, O=0, lpx=0, elx=0, dC=0, dz=0)
     for case in range(60):
         drawn = random_system(seed, case)
         if drawn is None:
@@ -85,29 +91,45 @@ def test_random_systems_against_the_oracle(seed):
             assert e.status == qb.QMC_EUNSUPPORTED, (case, e)
             continue
         evaluated += 1
-        o = ob.OracleSystem(d)
+        o, ox = ob.OracleSystem(d), ob.OracleSystem(d, extended=True)
         lp0, sg0, el0 = ob.local_energy(o, r, threads=4)
-        O0 = ob.log_derivatives(o, r, threads=4)
+        lpX, sgX, elX = ob.local_energy(ox, r, threads=4)
+        O0, OX = ob.log_derivatives(o, r, threads=4), ob.log_derivatives(ox, r, threads=4)
         lp, sg, el, O = (t.cpu().numpy() for t in s.log_derivatives(torch.from_numpy(r).cuda()))
-        keep = (lp0 - lp0.max() > math.log(1e-6)) & np.isfinite(el0)
-        assert np.array_equal(sg, sg0), case
-        # random orbitals make badly conditioned Slater matrices common: log|det| carries eps * cond on both sides
-        assert np.max(np.abs(lp - lp0)[keep]) < 1e-8, (case, np.max(np.abs(lp - lp0)[keep]))
-        assert np.max((np.abs(el - el0) / np.maximum(1, np.abs(el0)))[keep]) < 1e-7, case
-        assert np.max((np.abs(O - O0) / np.maximum(1, np.abs(O0)))[keep]) < 1e-7, case
+        keep = (lpX - lpX.max() > math.log(1e-6)) & np.isfinite(elX)
+        walkers += int(keep.sum())
+        assert np.array_equal(sg[keep], sg0[keep]), case
+        esc = np.maximum(1, np.abs(elX))
+        exc["lp"] += adjudicate(lp, lp0, lpX, 1e-10, mask=keep, what=(case, "log|Psi|"))
+        exc["el"] += adjudicate(el, el0, elX, 1e-8, scale=esc, mask=keep, what=(case, "E_L"))
+        exc["O"] += adjudicate(O, O0, OX, 1e-8, scale=np.maximum(1, np.abs(OX)), mask=keep, what=(case, "O_p"))
         # every walker on the explicit per-determinant route
-        lpx, sgx, elx = (t.cpu().numpy() for t in s.local_energy_explicit(torch.from_numpy(r).cuda()))
-        assert np.array_equal(sgx, sg0), case
-        assert np.max(np.abs(lpx - lp0)[keep]) < 1e-8, case
-        assert np.max((np.abs(elx - el0) / np.maximum(1, np.abs(el0)))[keep]) < 1e-7, case
+        lpe, sge, ele = (t.cpu().numpy() for t in s.local_energy_explicit(torch.from_numpy(r).cuda()))
+        assert np.array_equal(sge[keep], sg0[keep]), case
+        exc["lpx"] += adjudicate(lpe, lp0, lpX, 1e-10, mask=keep, what=(case, "log|Psi| explicit"))
+        exc["elx"] += adjudicate(ele, el0, elX, 1e-8, scale=esc, mask=keep, what=(case, "E_L explicit"))
         # orbital-parameter derivatives: table route, explicit route (flagged groups, k >= 3) -- whichever the draw takes
         dC0, dz0 = ob.orbital_derivatives(o, r, threads=4)
+        dCX, dzX = ob.orbital_derivatives(ox, r, threads=4)
         dC, dz = (t.cpu().numpy() for t in s.orbital_derivatives(torch.from_numpy(r).cuda(), d.n_ao, d.n_mo))
-        assert np.max((np.abs(dC - dC0) / np.maximum(1, np.abs(dC0)))[keep]) < 1e-7, case
-        assert np.max((np.abs(dz - dz0) / np.maximum(1, np.abs(dz0)))[keep]) < 1e-7, case
+        exc["dC"] += adjudicate(dC, dC0, dCX, 1e-8, scale=np.maximum(1, np.abs(dCX)), mask=keep, what=(case, "dC"))
+        exc["dz"] += adjudicate(dz, dz0, dzX, 1e-8, scale=np.maximum(1, np.abs(dzX)), mask=keep, what=(case, "dzeta"))
+        # sampler: a decision may differ only inside the tie window, 1e-12 or -- where the float64 oracle's own margin
+        # is less certain than that -- four times its distance from the long-double run's
         ref = ob.metropolis(o, r, 0.3, 4, seed=case, threads=4)
+        refx = ob.metropolis(ox, r, 0.3, 4, seed=case, threads=4)
         out = s.metropolis(torch.from_numpy(r).cuda(), 0.3, 4, seed=case, want_accept=True)
-        bad = (out["accept"].cpu().numpy() != ref["accept"]) & (np.abs(ref["margin"]) >= 1e-9)
-        assert not bad.any(), case
+        acc = out["accept"].cpu().numpy()
+        alive = np.ones(r.shape[2], bool)
+        for sw in range(4):
+            with np.errstate(invalid="ignore"):
+                window = np.maximum(1e-12, 4 * np.abs(ref["margin"][sw] - refx["margin"][sw]))
+                window = np.where(np.isfinite(window), window, np.inf)
+            diff = (acc[sw] != ref["accept"][sw]) & alive
+            assert not (diff & (np.abs(ref["margin"][sw]) >= window)).any(), (case, sw)
+            alive &= ~diff & (ref["accept"][sw] == refx["accept"][sw])
         s.close()
     assert evaluated >= 30
+    # exceptions stay a small minority of the walkers compared (reported by -rA / on failure)
+    print(f"fuzz seed {seed}: {evaluated} systems, {walkers} walkers, adjudicated exceptions {exc}")
+    assert max(exc.values()) <= 0.1 * walkers, (exc, walkers)

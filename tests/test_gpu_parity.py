@@ -10,7 +10,7 @@ import numpy as np
 import pytest
 
 from paper_2506_09743_b200 import workloads as wl
-from tests.helpers import atom_system, hydrogenic_set, soa
+from tests.helpers import adjudicate, atom_system, hydrogenic_set, soa
 
 pytestmark = pytest.mark.gpu
 
@@ -177,10 +177,13 @@ def check_metropolis(env, d, r, step, n_sweeps, seed, threads=8, eloc_acc=False)
     assert np.max(np.abs(out["logpsi"].cpu().numpy()[alive] - ref["logpsi"][alive])) < 1e-10
     assert np.array_equal(out["sign"].cpu().numpy()[alive], ref["sign"][alive])
     if eloc_acc:
-        ea, ea0 = out["eloc_acc"].cpu().numpy()[alive], ref["eloc_acc"][alive]
-        # a sweep-summed E_L can pass near a node: compare the bulk tightly, everything loosely
-        err = np.abs(ea - ea0) / np.maximum(1.0, np.abs(ea0))
-        assert np.median(err) < 1e-10 and np.quantile(err, 0.99) < 1e-7
+        # per-walker sweep-summed E_L, element-wise at the contract's 1e-8 max(1, |.|); a walker that passed near a node
+        # during the sweeps is adjudicated by the long-double run of the same oracle (reading Q24) and counted
+        refx = ob.metropolis(ob.OracleSystem(d, extended=True), r, step, n_sweeps, seed, threads=threads, want_eloc_acc=True)
+        same = alive & (refx["accept"] == ref["accept"]).all(axis=0)
+        ea, ea0, eax = out["eloc_acc"].cpu().numpy(), ref["eloc_acc"], refx["eloc_acc"]
+        n_exc = adjudicate(ea, ea0, eax, 1e-8, scale=np.maximum(1.0, np.abs(eax)), mask=same, what="sum of E_L over the sweeps")
+        assert same.sum() >= 0.99 * M and n_exc <= max(2, M // 50), (int(same.sum()), n_exc)
     rate = acc.mean()
     assert 0.02 < rate < 0.99
     s.close()
@@ -265,44 +268,105 @@ def test_full_size_small_configs(env, name):
     check_local_energy(env, d, r, threads=os.cpu_count() or 8)
 
 
-def test_full_size_co_sampled(env):
-    """BASELINE configs[3] at 131072 walkers in the launch configuration bench.py times; the oracle
-    evaluates a sample of walkers (E_L of a walker does not depend on the others)."""
+def test_full_size_co_every_walker(env):
+    """BASELINE configs[3] at its stated size, in the launch configuration bench.py times: ALL 131072 walkers against
+    the oracle -- sign exact, log|Psi| 1e-10, E_L 1e-8 max(1, |E_L|) on walkers with |Psi|/max|Psi| > 1e-6, batch mean
+    1e-10.  Walkers on which the float64 oracle is itself more than a tenth of the bound away from the long-double run
+    of the same source are adjudicated by that run (tests.helpers.adjudicate, reading Q24) and counted."""
     torch, ob, qb = env
     d, r = wl.co()
     M = r.shape[2]
+    nt = os.cpu_count() or 8
     s = qb.QmcSystem(d)
     lp, sg, el = (t.cpu().numpy() for t in s.local_energy(_to_gpu(torch, r)))
-    idx = np.unique(np.concatenate([np.arange(0, 64), np.arange(M - 65, M),
-                                    np.random.default_rng(0).integers(0, M, 2048)]))
-    o = ob.OracleSystem(d)
-    lp0, sg0, el0 = ob.local_energy(o, np.ascontiguousarray(r[:, :, idx]), threads=os.cpu_count() or 8)
-    assert np.array_equal(sg[idx], sg0)
-    assert np.max(np.abs(lp[idx] - lp0)) < 1e-10
-    keep = lp0 - lp.max() > math.log(1e-6)
-    err = np.abs(el[idx] - el0) / np.maximum(1.0, np.abs(el0))
-    assert np.max(err[keep]) < 1e-8
-    # properties that hold at any size: finite outputs, sign is +-1, mean agrees with the device reduction
-    assert np.isfinite(lp).all() and np.isin(sg, (-1.0, 1.0)).all()
+    lp2, sg2 = (t.cpu().numpy() for t in s.log_psi(_to_gpu(torch, r)))
+    lp0, sg0, el0 = ob.local_energy(ob.OracleSystem(d), r, threads=nt)
+    lpx, sgx, elx = ob.local_energy(ob.OracleSystem(d, extended=True), r, threads=nt)
+    assert np.array_equal(sg0, sgx)
+    assert np.array_equal(sg, sg0) and np.array_equal(sg2, sg0), int((sg != sg0).sum())
+    n_lp = adjudicate(lp, lp0, lpx, 1e-10, what="log|Psi| (E_L kernel)")
+    n_lp2 = adjudicate(lp2, lp0, lpx, 1e-10, what="log|Psi| (values-only kernel)")
+    keep = lp0 - lp0.max() > math.log(1e-6)
+    n_el = adjudicate(el, el0, elx, 1e-8, scale=np.maximum(1.0, np.abs(elx)), mask=keep, what="E_L")
+    # measured on this batch: 26 walkers of 131072 for log|Psi| (near-singular Slater matrices or a cancelling CI sum,
+    # the float64 oracle itself up to 6.8e-10 from the long-double value), none for E_L
+    assert n_lp <= 64 and n_lp2 <= 64 and n_el <= 4, (n_lp, n_lp2, n_el)
+    m0, _ = ob.batch_stats(el0)
+    m1, _ = ob.batch_stats(el)
+    assert abs(m1 - m0) <= 1e-10 * abs(m0), (m0, m1)            # batch mean over ALL walkers (reading Q15)
     m, e = qb.batch_stats(torch.from_numpy(el).cuda())
-    m0, e0 = ob.batch_stats(el)
-    assert abs(m - m0) < 1e-11 * abs(m0) and abs(e - e0) < 1e-8 * e0
+    mo, eo = ob.batch_stats(el)
+    assert abs(m - mo) < 1e-12 * abs(mo) and abs(e - eo) < 1e-10 * eo
     # Metropolis at full size: contiguous sample ranges, global walker indices
     rg = _to_gpu(torch, r)
     out = s.metropolis(rg, 0.2, 5, seed=4242, want_accept=True)
     acc = out["accept"].cpu().numpy()
     rf = rg.cpu().numpy()
-    L = ob.lib()
+    o = ob.OracleSystem(d)
     for w0 in (0, 40001, M - 96):
         w1 = w0 + 96
         rr = np.array(r, order="C", copy=True)
         a0 = np.zeros((5, M), np.uint8); mg = np.zeros((5, M)); l0 = np.zeros(M); s0 = np.zeros(M)
-        assert L.oracle_metropolis(o.ref, rr.ctypes.data, M, w0, w1, 0.2, 5, 4242, 0, l0.ctypes.data, s0.ctypes.data,
-                                   a0.ctypes.data, mg.ctypes.data, None) == 0
+        assert o.L.oracle_metropolis(o.ref, rr.ctypes.data, M, w0, w1, 0.2, 5, 4242, 0, l0.ctypes.data, s0.ctypes.data,
+                                     a0.ctypes.data, mg.ctypes.data, None) == 0
         bad = (acc[:, w0:w1] != a0[:, w0:w1]) & (np.abs(mg[:, w0:w1]) >= 1e-12)
         assert not bad.any()
         same = (acc[:, w0:w1] == a0[:, w0:w1]).all(axis=0)
         assert np.max(np.abs(rf[:, :, w0:w1][:, :, same] - rr[:, :, w0:w1][:, :, same])) < 1e-12
+    s.close()
+
+
+def test_full_size_co_scan_geometry(env):
+    """BASELINE configs[4] at its stated size for one geometry: 262144 walkers, 500 determinants, 50 sweeps with E_L
+    after every sweep.  The oracle follows the first 1024 walkers (Philox is keyed by the global walker index, so a
+    prefix reproduces exactly those trajectories): accept masks bit-exact outside the tie window, final positions,
+    per-walker sweep-averaged E_L element-wise at 1e-8 max(1, |.|) with adjudication (walkers that pass near a node
+    are counted, not hidden), and the reported quantity of reading Q16: mean and standard error over walkers."""
+    torch, ob, qb = env
+    d, r = wl.co_scan(M=262144, n_geom=6)[5]      # R = 2.40 bohr
+    M, P, n_sweeps, step, seed = r.shape[2], 1024, 50, 0.2, 777
+    nt = os.cpu_count() or 8
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    out = s.metropolis(rg, step, n_sweeps, seed, want_accept=True, want_eloc_acc=True, count=True)
+    torch.cuda.synchronize()
+    acc = out["accept"].cpu().numpy()
+    assert out["n_accepted"] == int(acc.sum())
+    ea = out["eloc_acc"].cpu().numpy()
+    assert np.isfinite(ea).all()
+    rp = np.ascontiguousarray(r[:, :, :P])
+    ref = ob.metropolis(ob.OracleSystem(d), rp, step, n_sweeps, seed, threads=nt, want_eloc_acc=True)
+    refx = ob.metropolis(ob.OracleSystem(d, extended=True), rp, step, n_sweeps, seed, threads=nt, want_eloc_acc=True)
+    alive = np.ones(P, bool)
+    excused = 0
+    for sw in range(n_sweeps):
+        diff = (acc[sw, :P] != ref["accept"][sw]) & alive
+        if diff.any():
+            assert np.all(np.abs(ref["margin"][sw])[diff] < 1e-12), f"sweep {sw}: decisions differ outside the tie window"
+            excused += int(diff.sum())
+            alive &= ~diff
+    assert excused <= 1
+    rf = rg[:, :, :P].cpu().numpy()
+    assert np.max(np.abs(rf[:, :, alive] - ref["r"][:, :, alive])) < 1e-12
+    lp = out["logpsi"].cpu().numpy()[:P]
+    same = alive & (refx["accept"] == ref["accept"]).all(axis=0)
+    adjudicate(lp, ref["logpsi"], refx["logpsi"], 1e-10, mask=same, what="final log|Psi|")
+    assert np.array_equal(out["sign"].cpu().numpy()[:P][alive], ref["sign"][alive])
+    eb, eb0, ebx = ea[:P] / n_sweeps, ref["eloc_acc"] / n_sweeps, refx["eloc_acc"] / n_sweeps
+    n_exc = adjudicate(eb, eb0, ebx, 1e-8, scale=np.maximum(1.0, np.abs(ebx)), mask=same, what="sweep-averaged E_L per walker")
+    assert same.sum() >= P - 8 and n_exc <= P // 50, (int(same.sum()), n_exc)
+    # reading Q16: mean and standard error over walkers of the per-walker sweep averages -- on the prefix against the
+    # oracle (device reduction on the GPU's own values), and the full-size device reduction against the oracle's
+    # reduction of the same array
+    sel = torch.from_numpy(np.flatnonzero(same)).cuda()
+    mg_, eg_ = qb.batch_stats((out["eloc_acc"][:P] / n_sweeps)[sel].contiguous())
+    m0, e0 = ob.batch_stats(eb0[same])
+    assert abs(mg_ - m0) <= 1e-10 * abs(m0) and abs(eg_ - e0) <= 1e-8 * e0, (mg_, m0, eg_, e0)
+    mf, ef = qb.batch_stats((out["eloc_acc"] / n_sweeps).contiguous())
+    mo, eo = ob.batch_stats(ea / n_sweeps)
+    assert abs(mf - mo) <= 1e-12 * abs(mo) and abs(ef - eo) <= 1e-10 * eo
+    rate = acc.mean()
+    assert 0.05 < rate < 0.95
     s.close()
 
 
@@ -974,4 +1038,88 @@ def test_nuclear_log_gradient_writes_exactly_its_output(env, name, M):
     assert bool(torch.isfinite(buf[pad:pad + n]).all())
     assert torch.equal(rg, r_before)
     assert torch.equal(buf[pad:pad + n].view(M, d.n_atoms, 3), s.nuclear_log_gradient(rg, d.n_atoms))
+    s.close()
+
+
+# ----------------------------------------------------------------------------- output bounds (no memory checker on this pool)
+class _Guarded:
+    """A device buffer of n elements carved from the middle of a larger allocation: guard words on both sides, the
+    payload pre-filled with a sentinel (NaN for doubles, 0xAB for bytes) that a complete write must replace."""
+
+    PAD = 2048
+
+    def __init__(self, torch, n, dtype=None):
+        self.torch, self.n = torch, n
+        self.dtype = dtype or torch.float64
+        if self.dtype == torch.float64:
+            self.buf = torch.full((n + 2 * self.PAD,), float("nan"), dtype=self.dtype, device="cuda")
+            self.guard = 12345.0
+        else:
+            self.buf = torch.full((n + 2 * self.PAD,), 0xAB, dtype=self.dtype, device="cuda")
+            self.guard = 0x5C
+        self.buf[:self.PAD] = self.guard
+        self.buf[self.PAD + n:] = self.guard
+
+    @property
+    def ptr(self):
+        return self.buf.data_ptr() + self.buf.element_size() * self.PAD
+
+    @property
+    def view(self):
+        return self.buf[self.PAD:self.PAD + self.n]
+
+    def check(self, what):
+        assert bool((self.buf[:self.PAD] == self.guard).all()) and bool((self.buf[self.PAD + self.n:] == self.guard).all()), \
+            f"{what}: guard words overwritten"
+        if self.dtype == self.torch.float64:
+            assert bool(self.torch.isfinite(self.view).all()), f"{what}: entries left unwritten"
+        else:
+            assert bool((self.view <= 1).all()), f"{what}: entries left unwritten"
+
+
+@pytest.mark.parametrize("name,M", [("H2", 1), ("LiH", 37), ("Li2", 131), ("CO", 67), ("CO", 2049)])
+def test_every_call_writes_exactly_its_outputs(env, name, M):
+    """Raw C-ABI calls with every output pointing into the middle of a larger buffer, at ragged batch sizes (walkers
+    that do not fill the last warp pass): guard words stay untouched, every entry is written, inputs are not
+    modified.  Covers qmc_local_energy, qmc_log_psi, qmc_local_energy_explicit, qmc_log_derivatives,
+    qmc_orbital_derivatives and qmc_metropolis (accept mask, summed E_L, in-place walkers)."""
+    torch, ob, qb = env
+    d, r = wl.CONFIGS[name](M=M)
+    s = qb.QmcSystem(d)
+    L, st = qb.lib(), torch.cuda.current_stream().cuda_stream
+    rg = _to_gpu(torch, r)
+    r_before = rg.clone()
+    G = lambda n, dt=None: _Guarded(torch, n, dt)
+    for call in ("qmc_local_energy", "qmc_local_energy_explicit"):
+        a, b, c = G(M), G(M), G(M)
+        assert getattr(L, call)(s._h, rg.data_ptr(), M, a.ptr, b.ptr, c.ptr, st) == 0
+        torch.cuda.synchronize()
+        for g, nm in ((a, "logpsi"), (b, "sign"), (c, "eloc")):
+            g.check(f"{call} {nm}")
+    a, b = G(M), G(M)
+    assert L.qmc_log_psi(s._h, rg.data_ptr(), M, a.ptr, b.ptr, st) == 0
+    torch.cuda.synchronize()
+    a.check("qmc_log_psi logpsi"); b.check("qmc_log_psi sign")
+    npar = s.n_param()
+    a, b, c, O = G(M), G(M), G(M), G(M * npar)
+    assert L.qmc_log_derivatives(s._h, rg.data_ptr(), M, a.ptr, b.ptr, c.ptr, O.ptr, st) == 0
+    torch.cuda.synchronize()
+    for g, nm in ((a, "logpsi"), (b, "sign"), (c, "eloc"), (O, "O")):
+        g.check(f"qmc_log_derivatives {nm}")
+    dC, dz = G(M * d.n_ao * d.n_mo), G(M * d.n_ao)
+    assert L.qmc_orbital_derivatives(s._h, rg.data_ptr(), M, dC.ptr, dz.ptr, st) == 0
+    torch.cuda.synchronize()
+    dC.check("qmc_orbital_derivatives dC"); dz.check("qmc_orbital_derivatives dzeta")
+    assert torch.equal(rg, r_before)
+    # sampler: walkers in place inside a guarded buffer, accept mask, summed E_L
+    n_sweeps = 3
+    for with_acc in (False, True):
+        rw = G(r.size)
+        rw.view.copy_(rg.reshape(-1))
+        a, b, acc, ea = G(M), G(M), G(n_sweeps * M, torch.uint8), G(M)
+        assert L.qmc_metropolis(s._h, rw.ptr, M, 0.3, n_sweeps, 5, 0, 0, a.ptr, b.ptr, acc.ptr, ea.ptr if with_acc else None,
+                                None, st) == 0
+        torch.cuda.synchronize()
+        for g, nm in ((rw, "walkers"), (a, "logpsi"), (b, "sign"), (acc, "accept")) + (((ea, "eloc_acc"),) if with_acc else ()):
+            g.check(f"qmc_metropolis {nm}")
     s.close()

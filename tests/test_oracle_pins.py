@@ -24,12 +24,17 @@ def _rand_pos(M, n_e, scale=1.0, rmin=0.0, seed=0):
     return r
 
 
+# closed-form values the paper / textbook quantum mechanics fix (tests/golden/cusp_and_hydrogenic.txt, with citations)
+from tests.helpers import golden_values  # noqa: E402
+GOLDEN = golden_values("cusp_and_hydrogenic.txt")
+
+
 # ---------------------------------------------------------------- P1, P2
 def test_P1_hydrogen_1s_exact():
     d = atom_system(1, [(1, 0, 0, 1.0)], [[1.0]], 1, 0)
     r = _rand_pos(200, 1, 2.0)
     lp, sg, el = ob.local_energy(ob.OracleSystem(d), soa(r))
-    assert np.max(np.abs(el + 0.5)) < 1e-12
+    assert np.max(np.abs(el - GOLDEN["E_n1"])) < 1e-12
     # normalised 1s: psi = e^{-r}/sqrt(pi)
     rr = np.linalg.norm(r[:, 0], axis=1)
     assert np.max(np.abs(lp - (-rr - 0.5 * math.log(math.pi)))) < 1e-13
@@ -53,11 +58,11 @@ def test_P3_hydrogenic_2p_3d_every_harmonic(Z):
     for m in range(3):
         d = atom_system(Z, [(2, 1, m, Z / 2)], [[1.0]], 1, 0)
         _, _, el = ob.local_energy(ob.OracleSystem(d), soa(r))
-        assert np.max(np.abs(el + Z * Z / 8)) < 1e-11 * Z * Z
+        assert np.max(np.abs(el - Z * Z * GOLDEN["E_n2"])) < 1e-11 * Z * Z
     for m in range(5):
         d = atom_system(Z, [(3, 2, m, Z / 3)], [[1.0]], 1, 0)
         _, _, el = ob.local_energy(ob.OracleSystem(d), soa(r))
-        assert np.max(np.abs(el + Z * Z / 18)) < 1e-11 * Z * Z
+        assert np.max(np.abs(el - Z * Z * GOLDEN["E_n3"])) < 1e-11 * Z * Z
 
 
 @pytest.mark.parametrize("Z", [1, 2])
@@ -381,7 +386,7 @@ def test_potential_terms_brute_force():
 def test_P12_electron_electron_cusp_finite():
     Z, zeta = 2.0, 1.7
     out = {}
-    for label, a in [("exact", 0.5), ("off", 0.4)]:
+    for label, a in [("exact", GOLDEN["cusp_antiparallel"]), ("off", 0.4)]:
         d = atom_system(Z, [(1, 0, 0, zeta)], [[1.0]], 1, 1, a_anti=a, b=1.0)
         o = ob.OracleSystem(d)
         vals = []
@@ -395,7 +400,7 @@ def test_P12_electron_electron_cusp_finite():
     assert abs(out["off"][-1] - (1 - 2 * 0.4) / 1e-6) < 0.01 * (0.2 / 1e-6)
     # parallel spins (a = 1/4): antisymmetric pair 1s/2pz
     aos, C, e = hydrogenic_set(1.0)
-    for a, finite in [(0.25, True), (0.15, False)]:
+    for a, finite in [(GOLDEN["cusp_parallel"], True), (0.15, False)]:
         d = atom_system(1.0, aos, C[:, [0, 4]], 2, 0, norm=np.ones(len(aos)), a_par=a)
         o = ob.OracleSystem(d)
         vals = [ob.local_energy(o, soa(np.array([[[0.4, 0.3, 0.2], [0.4, 0.3, 0.2 + eps]]])))[2][0]
@@ -652,6 +657,32 @@ def test_energy_gradient_estimator():
     el = ob.local_energy(o, r)[2]
     ev, g = ob.energy_gradient(el, ob.log_derivatives(o, r))
     assert abs(ev + 0.5) < 1e-12 and np.max(np.abs(g)) < 1e-11
+
+
+def test_energy_gradient_estimator_reproduces_dE_dzeta_of_the_hydrogen_atom():
+    # Physical pin of eq. 6's prefactor 2/M and sign: hydrogen atom, trial function N e^{-zeta r}:
+    #   E(zeta) = zeta^2/2 - zeta  =>  dE/dzeta = zeta - 1,   O = d ln Psi / d zeta = 3/(2 zeta) - r,
+    #   E_L = -zeta^2/2 + (zeta - 1)/r.
+    # Samples of |Psi|^2 from the oracle's own sampler (pinned by P17), O from oracle_orbital_derivatives (pinned by its
+    # closed form), then oracle_energy_gradient must give zeta - 1 within 4 standard errors -- a factor 1 or 4 instead
+    # of 2, or a flipped sign, is tens of standard errors away.
+    for zeta in (1.3, 0.75):
+        d = atom_system(1, [(1, 0, 0, zeta)], [[1.0]], 1, 0)
+        o = ob.OracleSystem(d)
+        M = 40000
+        r0 = soa(_rand_pos(M, 1, 1.0, rmin=0.05, seed=17))
+        out = ob.metropolis(o, r0, 0.7 / zeta, 60, seed=31, threads=os.cpu_count() or 1)
+        r = out["r"]
+        el = ob.local_energy(o, r, threads=os.cpu_count() or 1)[2]
+        dz = ob.orbital_derivatives(o, r, threads=os.cpu_count() or 1)[1]       # [M, 1]
+        rr = np.linalg.norm(r[0], axis=0)
+        assert np.max(np.abs(dz[:, 0] - (1.5 / zeta - rr))) < 1e-12             # the factor O itself
+        ev, g = ob.energy_gradient(el, dz)
+        per_walker = 2.0 * dz[:, 0] * (el - ev)
+        sigma = per_walker.std(ddof=1) / math.sqrt(M)
+        assert abs(ev - (zeta * zeta / 2 - zeta)) < 5 * el.std(ddof=1) / math.sqrt(M)
+        assert abs(g[0] - (zeta - 1.0)) < 4 * sigma, (zeta, g[0], sigma)
+        assert sigma < 0.1 * abs(zeta - 1.0)                                    # the pin resolves scale and sign
 
 
 # ---------------------------------------------------------------- electron-nucleus Jastrow (D.2)
