@@ -110,7 +110,7 @@ constexpr double kFallbackCap = QMC_FALLBACK_CAP;
 // The same loss when the reference ALONE is nearly singular while Sigma / D_0 stays moderate (the CI coefficients of
 // the large determinants are small): T, G, H carry relative errors eps * cond(A_0) and their O(cond^2) parts cancel.
 // kappa = max |T[p][q]| of a spin estimates cond(A_0) at no cost.  Measured on all 131072 CO, 32768 Li2 and
-// 32768 CO-500 walkers against the long-double oracle with the fallback off: worst error of
+// 32768 CO-500 walkers against the oracle (its long-double build) with the fallback off: worst error of
 // a walker with kappa^2 <= 1e6 max(1, |E_L|) is 2.8e-10 max(1, |E_L|); 0.12% / 0.16% / 0.07% of the walkers exceed it.
 // (The (Sigma/D_0)^2 test alone left a CO walker at 2.0e-7: kappa 4.8e4, Sigma/D_0 = -118.)
 #ifndef QMC_FALLBACK_KAPPA
