@@ -35,6 +35,7 @@ int cuda_fail(cudaError_t e, const char *what) {
 
 struct Variant {
   int NS, NMO, LP, ws_doubles;
+  int metro_ws_doubles;  // the sampler's per-warp scratch: the evaluator's plus two sweeps of draws
   bool exact;  // compiled for n_up = n_dn = NS
   const void *k_el, *k_psi, *k_metro, *k_expl, *k_el_deriv;
   const void *e_el, *e_psi, *e_metro, *e_expl, *e_el_deriv;
@@ -52,6 +53,7 @@ Variant make_variant() {
   v.LP = Geo<NS, NMO>::LP;
   v.exact = X;
   v.ws_doubles = Geo<NS, NMO>::total;
+  v.metro_ws_doubles = Geo<NS, NMO>::total + 2 * kDrawDoubles<NS>;
   v.k_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl>;
   v.k_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi>;
   v.k_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi>;
@@ -167,6 +169,7 @@ struct qmc_system {
   SysParams P{};
   Variant var{};
   int smem_el = 0, smem_psi = 0;  // dynamic shared memory of the E_L kernels (kWarpsEl warps) / values-only kernels
+  int smem_metro = 0;             // ... of the sampler
   int blocks_el = 0, blocks_psi = 0, blocks_metro = 0, blocks_expl = 0, blocks_deriv = 0;
   void *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr, *d_orig = nullptr, *d_yrec = nullptr, *d_ytgt = nullptr, *d_rowao = nullptr,
        *d_rownrm = nullptr;
@@ -268,6 +271,18 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   if (!s) return QMC_ENOMEM;
   s->device = device;
   SysParams &P = s->P;
+  {  // constants of the device's elementary functions (qmc_device.cuh)
+    MathConsts &K = P.mc;
+    K.e_scale = 92.33248261689366;
+    K.e_ln2hi = -6.93147180369123816490e-01 / 64;
+    K.e_ln2lo = -1.90821492927058770002e-10 / 64;
+    K.e_c5 = 1.0 / 120; K.e_c4 = 1.0 / 24; K.e_c3 = 1.0 / 6;
+    K.l_c7 = 1.0 / 7; K.l_c6 = -1.0 / 6; K.l_c5 = 1.0 / 5; K.l_c3 = 1.0 / 3;
+    K.l_ln2hi = 6.93147180369123816490e-01; K.l_ln2lo = 1.90821492927058770002e-10;
+    K.s_2pi = 6.283185307179586;
+    K.s_c7 = -1.0 / 5040; K.s_c5 = 1.0 / 120; K.s_c3 = -1.0 / 6;
+    K.s_c8 = 1.0 / 40320; K.s_c6 = -1.0 / 720; K.s_c4 = 1.0 / 24;
+  }
   P.n_atoms = d->n_atoms;
   P.n_up = d->n_up;
   P.n_dn = d->n_dn;
@@ -707,11 +722,12 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   P.smem_const_bytes = (int)((szC + szD + 15) / 16 * 16);
   s->smem_el = P.smem_const_bytes + kWarpsEl * var->ws_doubles * (int)sizeof(double);
   s->smem_psi = P.smem_const_bytes + kWarpsPsi * var->ws_doubles * (int)sizeof(double);
+  s->smem_metro = P.smem_const_bytes + kWarpsPsi * var->metro_ws_doubles * (int)sizeof(double);
 
   int dev_smem = 0, n_sm = 0;
   cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
   cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device);
-  if (std::max(s->smem_el, s->smem_psi) > dev_smem) {
+  if (std::max(s->smem_el, s->smem_metro) > dev_smem) {
     qmc_destroy(s);
     return QMC_EUNSUPPORTED;
   }
@@ -719,7 +735,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   const void *ks[5] = {s->var.k_el, s->var.k_psi, s->var.k_metro, s->var.k_expl, s->var.k_el_deriv};
   int *nb[5] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro, &s->blocks_expl, &s->blocks_deriv};
   const int kw[5] = {kWarpsEl, kWarpsPsi, kWarpsPsi, kWarpsEl, kWarpsEl};
-  const int ksm[5] = {s->smem_el, s->smem_psi, s->smem_psi, s->smem_el, s->smem_el};
+  const int ksm[5] = {s->smem_el, s->smem_psi, s->smem_metro, s->smem_el, s->smem_el};
   for (int i = 0; i < 5; ++i) {
     if ((e = cudaFuncSetAttribute(ks[i], cudaFuncAttributeMaxDynamicSharedMemorySize, ksm[i])) != cudaSuccess) {
       int rc = cuda_fail(e, "cudaFuncSetAttribute");
@@ -919,7 +935,7 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
   void *args[3] = {(void *)&s->P, (void *)&io, (void *)&mp};
   if (!d_eloc_acc) {
     // one persistent launch for all sweeps: coordinates and log|Psi| stay in registers
-    CK(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_psi, st));
+    CK(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_metro, st));
     ++g_launches;
   } else {
     // E_L after every sweep (BASELINE config 5): one-sweep launches of the sampler alternate with the
@@ -944,14 +960,14 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
     mp.n_sweeps = 1;
     if (n_sweeps == 0) {  // nothing to accumulate; still report log|Psi| of the starting positions
       mp.n_sweeps = 0;
-      CKS(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_psi, st));
+      CKS(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_metro, st));
       ++g_launches;
     }
     for (int32_t sw = 0; sw < n_sweeps; ++sw) {
       mp.sweep0 = (uint32_t)(sweep_offset + (uint64_t)sw);
       mp.accept = d_accept ? d_accept + (size_t)sw * (size_t)M : nullptr;
       mp.resume = sw > 0 ? 1 : 0;
-      CKS(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_psi, st));
+      CKS(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_metro, st));
       ++g_launches;
       int rc = launch_eval(s, d_r, M, nullptr, nullptr, scratch, st, true);
       if (rc != QMC_OK) {

@@ -64,7 +64,19 @@ constexpr int kMetaK1 = 1 << 4, kMetaK2 = 2 << 4;
 #define QMC_CHUNK 16         // AO rows per DMMA chunk (8 or 16: 2 or 4 k-steps of the m8n8k4 shape)
 #endif
 constexpr int kChunk = QMC_CHUNK;
+// Metropolis: doubles of one sweep's draws per warp: normals [G][3 n_e] (G n_e <= 32), then log u [G]
+template <int NS>
+constexpr int kDrawDoubles = 96 + ((16 / NS + 1) & ~1);
 constexpr int kExpTab = 64;  // entries of the 2^(j/64) table of exp_neg
+constexpr int kRngTab = 256; // doubles of the log / sincos tables of the Box-Muller transform
+
+// Constants of the elementary functions (exp_neg, log_pos, sincos_2pi), filled by qmc_setup from the same literal
+// expressions the functions used to carry; they travel in the kernel parameter block.
+struct MathConsts {
+  double e_scale, e_ln2hi, e_ln2lo, e_c5, e_c4, e_c3;            // 64/ln2, -ln2_hi/64, -ln2_lo/64, 1/120, 1/24, 1/6
+  double l_c7, l_c6, l_c5, l_c3, l_ln2hi, l_ln2lo;               // 1/7, -1/6, 1/5, 1/3, ln2 hi, ln2 lo
+  double s_2pi, s_c7, s_c5, s_c3, s_c8, s_c6, s_c4;              // 2 pi, -1/5040, 1/120, -1/6, 1/40320, -1/720, 1/24
+};
 
 // One determinant relative to the reference; the meaning of the two words depends on the class (qmc_setup):
 // one or two byte offsets of table entries (class 1, 2), four 16-bit byte offsets {11,12 | 21,22} of a 2x2
@@ -133,6 +145,7 @@ struct __align__(16) YRec {
 };
 
 struct SysParams {  // passed by value to every kernel
+  MathConsts mc;
   int n_atoms, n_up, n_dn, n_e;
   int n_shell, n_ao, n_mo, n_det;  // n_shell = records of the shell/atom stream; n_mo = orbitals referenced (kernel
                                    // order); n_det = packed determinant records (classes 1-4)
@@ -249,14 +262,13 @@ struct Geo {
   }
   static constexpr int szPhi = even(ROWS * (SWZ ? 16 : NMO));
   static constexpr int szG = even(cmax(PP * NS * NS, 2));
-  static constexpr int szT = even(cmax(2 * GMAX * TS, 96 + 32));  // also hosts the Metropolis draws
+  static constexpr int szT = even(cmax(2 * GMAX * TS, 96 + 32));
   static constexpr int szM = even(2 * GMAX * TS);
   static constexpr bool SINGLE = (2 * GMAX <= PP) && (2 * szPhi >= szG + szT + szM);
   static constexpr int oPhi = 0;
   static constexpr int oB = oPhi + szPhi;
   static constexpr int oG = SINGLE ? 0 : oB + szPhi;
   static constexpr int oT = oG + szG;
-  static constexpr int oProp = oT;                            // Metropolis draws are consumed before T is written
   static constexpr int oM = oT + szT;
   static constexpr int oPart = SINGLE ? oB + szPhi : oM + szM;
   static constexpr int oXYZ = oPart + 64;                     // coordinates (pair loop)
@@ -306,7 +318,6 @@ struct Geo {
   static_assert(SINGLE ? (oM + szM <= oPart) : true, "tables overlap the per-electron scalars");
   static_assert(2 * GMAX * TS * 2 <= szT + szM, "interleaved {T, M} tables exceed their region");
   static_assert(NS * RS + 1 < 256 && 8 * (2 * TS) < 65536, "table indices exceed the packed determinant records");
-  static_assert(oProp + 96 + GMAX <= oPart, "Metropolis draws exceed the table region");
 };
 
 // ---------------------------------------------------------------------------------
@@ -354,20 +365,21 @@ __device__ __forceinline__ double rsqrt_fast(double x) {
 //   e^x = 2^n * 2^(j/64) * (1 + q(f)),  q = f + f^2 (1/2 + f/6 + f^2 (1/24 + f/120))   (truncation 3.5e-17)
 // with 2^(j/64) from a 64-entry shared-memory table (correctly rounded doubles, built by qmc_setup) and
 // 2^n applied to the exponent field.  Arguments below -690 are clamped (value ~1e-300, zero for every
-// use here); NaN stays NaN.
-// Constants are literals: one constant per FMA comes straight from the compiler's constant bank or, when
-// its low word is zero (the rounding magic, 1/2), as an immediate -- no load instructions.
-__device__ __forceinline__ double exp_neg(double x, const double *__restrict__ tab) {
+// use here) by one unsigned minimum on the high word (negative doubles order like their bit patterns); the clamp
+// also swallows a NaN argument -- a NaN coordinate still reaches log|Psi| and E_L through the distances of
+// the Jastrow factor and the potential.
+// The constants come from the kernel parameter block (MathConsts): an FP64 instruction takes one of them straight
+// from the constant bank; as literals each cost two 32-bit moves per use (measured: 12 of the 33 instructions).
+__device__ __forceinline__ double exp_neg(double x, const double *__restrict__ tab, const MathConsts &K) {
   constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52
-  x = (x < -690.0) ? -690.0 : x;
-  const double t = fma(x, 92.33248261689366, kMagic);  // round(64 x / ln2) in the low mantissa bits
+  x = __hiloint2double((int)min((unsigned)__double2hiint(x), 0xC0859000u), __double2loint(x));  // x >= -690
+  const double t = fma(x, K.e_scale, kMagic);  // round(64 x / ln2) in the low mantissa bits
   const int n = __double2loint(t);
   const double nd = t - kMagic;
-  double f = fma(nd, -6.93147180369123816490e-01 / 64, x);
-  f = fma(nd, -1.90821492927058770002e-10 / 64, f);
+  double f = fma(nd, K.e_ln2hi, x);
+  f = fma(nd, K.e_ln2lo, f);
   const double f2 = f * f;
-  const double c4 = 1.0 / 24, c5 = 1.0 / 120;
-  const double a = fma(f, c5, c4), b = fma(f, 1.0 / 6, 0.5);
+  const double a = fma(f, K.e_c5, K.e_c4), b = fma(f, K.e_c3, 0.5);
   const double q = fma(f2, fma(f2, a, b), f);
   const double T = tab[n & (kExpTab - 1)];
   const double p = fma(T, q, T);
@@ -379,25 +391,24 @@ __device__ __forceinline__ double exp_neg(double x, const double *__restrict__ t
 // normal pair costs ~40 FP64 instructions.  Tables are built in long double by qmc_setup (kRngTab
 // doubles: 64 {1/c_j, -log(1/c_j)} pairs, then 64 {cos, sin}(2 pi j / 64) pairs) and sit in shared memory.
 // ---------------------------------------------------------------------------------
-constexpr int kRngTab = 256;
-// log(u) for a positive normal u (here u in (0,1)): u = 2^e m, m in [sqrt(1/2), sqrt(2)); the top six bits
+// log(u) for a positive normal u: u = 2^e m, m in [sqrt(1/2), sqrt(2)); the top six bits
 // of m's offset in that range select c_j; r = m / c_j - 1, |r| <= 0.0079;
 // log u = e ln2 - log(1/c_j) + (r - r^2/2 + ... + r^7/7)      (truncation r^8/8 < 2e-18)
-__device__ __forceinline__ double log_pos(double u, const double2 *__restrict__ tab) {
+__device__ __forceinline__ double log_pos(double u, const double2 *__restrict__ tab, const MathConsts &K) {
   int hx = __double2hiint(u) + (0x3ff00000 - 0x3fe6a09e);
   const int e = (hx >> 20) - 1023;
   hx &= 0xfffff;
   const double m = __hiloint2double(hx + 0x3fe6a09e, __double2loint(u));
   const double2 t = tab[hx >> 14];
   const double r = fma(m, t.x, -1.0);
-  double p = fma(r, 1.0 / 7, -1.0 / 6);
-  p = fma(p, r, 1.0 / 5);
+  double p = fma(r, K.l_c7, K.l_c6);
+  p = fma(p, r, K.l_c5);
   p = fma(p, r, -0.25);
-  p = fma(p, r, 1.0 / 3);
+  p = fma(p, r, K.l_c3);
   p = fma(p, r, -0.5);
   const double lg = fma(r * r, p, r);
   const double ed = (double)e;
-  return fma(ed, 6.93147180369123816490e-01, t.y) + fma(ed, 1.90821492927058770002e-10, lg);  // ln2 hi, lo
+  return fma(ed, K.l_ln2hi, t.y) + fma(ed, K.l_ln2lo, lg);  // ln2 hi, lo
 }
 // sqrt(x), x > 0 normal: x * rsqrt(x) with one correction step (error < 1 ulp)
 __device__ __forceinline__ double sqrt_pos(double x) {
@@ -407,15 +418,15 @@ __device__ __forceinline__ double sqrt_pos(double x) {
 }
 // sin and cos of 2 pi u, u in [0,1): u = j/64 + f, |f| <= 1/128 (exact), a = 2 pi f, |a| <= 0.0491;
 // short Taylor polynomials in a (truncation < 5e-18) rotated by the tabulated {cos, sin}(2 pi j/64).
-__device__ __forceinline__ void sincos_2pi(double u, const double2 *__restrict__ tab, double &sn, double &cs) {
+__device__ __forceinline__ void sincos_2pi(double u, const double2 *__restrict__ tab, const MathConsts &K, double &sn, double &cs) {
   constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52
   const double t = fma(u, 64.0, kMagic);  // round(64 u) in the low mantissa bits
   const double f = fma(t - kMagic, -1.0 / 64, u);
   const double2 w = tab[__double2loint(t) & 63];
-  const double a = f * 6.283185307179586;
+  const double a = f * K.s_2pi;
   const double a2 = a * a;
-  const double sa = fma(a * a2, fma(a2, fma(a2, -1.0 / 5040, 1.0 / 120), -1.0 / 6), a);           // sin a
-  const double qc = a2 * fma(a2, fma(a2, fma(a2, 1.0 / 40320, -1.0 / 720), 1.0 / 24), -0.5);      // cos a - 1
+  const double sa = fma(a * a2, fma(a2, fma(a2, K.s_c7, K.s_c5), K.s_c3), a);                 // sin a
+  const double qc = a2 * fma(a2, fma(a2, fma(a2, K.s_c8, K.s_c6), K.s_c4), -0.5);             // cos a - 1
   cs = fma(-w.y, sa, fma(w.x, qc, w.x));
   sn = fma(w.x, sa, fma(w.y, qc, w.y));
 }

@@ -390,7 +390,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           }
           continue;
         }
-        double gr = exp_neg(-sh.zeta * r, sExp);          // r^k e^{-zeta r}
+        double gr = exp_neg(-sh.zeta * r, sExp, P.mc);          // r^k e^{-zeta r}
         if (meta & kMetaK1) gr *= r;
         if (meta & kMetaK2) gr *= r2;
         double h = 0.0;
@@ -780,8 +780,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
             sT[pr * TS + NS * RS] = 1.0;
             sT[pr * TS + NS * RS + 1] = 0.0;
           }
-          sProb[pr * 4 + 0] = log(fabs(det));
-          sProb[pr * 4 + 1] = (det > 0.0) ? 1.0 : ((det < 0.0) ? -1.0 : 0.0);
+          sProb[pr * 4 + 0] = det;  // det A0 of this spin; the logarithm is taken once, of D0^up D0^dn (Sigma / D0)
           sProb[pr * 4 + 2] = t0;
           if (EL || ORB == 2) sProb[pr * 4 + 3] = kap;
         }
@@ -879,10 +878,23 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       }
     }
     if (wvalid && sub == 0) {
-      const double lu = sProb[pu * 4 + 0], ld = sProb[pd * 4 + 0];
-      const double sgn = sProb[pu * 4 + 1] * sProb[pd * 4 + 1];
-      sRes[wg * 4 + 0] = Jsum + lu + ld + log(fabs(den));
-      sRes[wg * 4 + 1] = sgn * ((den > 0.0) ? 1.0 : ((den < 0.0) ? -1.0 : 0.0));
+      // Sigma = D0^up D0^dn (Sigma / D0) (eq. 4): one table-driven logarithm of the product when it and its
+      // intermediate are comfortably normal, else the library's, factor by factor (tiny or huge determinants, zeros,
+      // NaN).  sign(Sigma) likewise.
+      const double du = sProb[pu * 4 + 0], dd = sProb[pd * 4 + 0];
+      const double d2 = du * dd, sig = d2 * den;
+      const double a2 = fabs(d2), as = fabs(sig);
+      double lg, sgn;
+      if (a2 > 1e-280 && a2 < 1e280 && as > 1e-280 && as < 1e280) {
+        lg = log_pos(as, reinterpret_cast<const double2 *>(sExp + kExpTab), P.mc);
+        sgn = (sig > 0.0) ? 1.0 : -1.0;
+      } else {
+        lg = log(fabs(du)) + log(fabs(dd)) + log(fabs(den));
+        const double s1 = (du > 0.0) ? 1.0 : ((du < 0.0) ? -1.0 : 0.0), s2 = (dd > 0.0) ? 1.0 : ((dd < 0.0) ? -1.0 : 0.0);
+        sgn = s1 * s2 * ((den > 0.0) ? 1.0 : ((den < 0.0) ? -1.0 : 0.0));
+      }
+      sRes[wg * 4 + 0] = Jsum + lg;
+      sRes[wg * 4 + 1] = sgn;
       const double eloc = EL ? esum + (sProb[pu * 4 + 2] + sProb[pd * 4 + 2]) + num / den + P.vnn : 0.0;
       if (EL) sRes[wg * 4 + 2] = eloc;
       // explicit fallback when the estimated table-path error of E_L exceeds a tenth of the parity bound

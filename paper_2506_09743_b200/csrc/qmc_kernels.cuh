@@ -249,7 +249,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
         r = r2 * rsqrt_fast(r2);
         continue;
       }
-      double gr = exp_neg(-sh.zeta * r, sExp);
+      double gr = exp_neg(-sh.zeta * r, sExp, P.mc);
       if (meta & kMetaK1) gr *= r;
       if (meta & kMetaK2) gr *= r2;
       const double zf = sh.dlnN - r;  // d ln phi / d zeta
@@ -441,11 +441,14 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   load_constants<NMO>(P, smem, sC, sExp, sDet, wsBase);
   using GE = Geo<NS, NMO>;
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;  // shfl: tells the compiler it is warp-uniform
-  double *ws = wsBase + warp * GE::total;
+  // per-warp scratch: the evaluator's, then the draws of TWO sweeps (they survive the evaluation in between):
+  // G (ceil(3 n_e / 2) + 1) Philox blocks per sweep rarely fill the 32 lanes evenly (CO: 44 = 32 + 12), two sweeps' worth
+  // do better (88 of 96)
+  constexpr int DR = kDrawDoubles<NS>;  // one sweep: normals [G][3 n_e] (<= 96 doubles), then log u [G]
+  double *ws = wsBase + warp * (GE::total + 2 * DR);
   const double2 *sLogT = reinterpret_cast<const double2 *>(sExp + kExpTab);  // log_pos table
   const double2 *sSinT = sLogT + 64;                                         // sincos_2pi table
-  double *sProp = ws + GE::oProp;       // [G][3 ne] normals
-  double *sLogU = sProp + 96;           // [G]
+  double *sDraw = ws + GE::total;
   const double *sRes = ws + GE::oRes;
   const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G, nc = 3 * ne, npair = (nc + 1) / 2;
   const int g = lane / ne, e = lane - g * ne;
@@ -473,32 +476,37 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     for (int sw = mp.resume ? 0 : -1; sw < mp.n_sweeps; ++sw) {
       double xp = x, yp = y, zp = z, logu = 0.0;
       if (sw >= 0) {
-        // --- draws: lanes share the (walker, pair) Philox blocks of the G walkers
-        for (int idx = lane; idx < G * (npair + 1); idx += 32) {
-          const int dg = idx / (npair + 1), j = idx - dg * (npair + 1);
-          const uint64_t gw = (uint64_t)(mp.walker_offset + grp * G + dg);
-          uint32_t o[4];
-          philox4x32_10((uint32_t)gw, mp.sweep0 + (uint32_t)sw, (j == npair) ? 0xFFFFFFFFu : (uint32_t)j,
-                        (uint32_t)(gw >> 32), mp.key0, mp.key1, o);
-          const double lu = log_pos(u53(o[0], o[1]), sLogT);
-          if (j == npair) {
-            sLogU[dg] = lu;
-          } else {
-            const double rho = sqrt_pos(-2.0 * lu);
-            double sn, cs;
-            sincos_2pi(u53(o[2], o[3]), sSinT, sn, cs);
-            sProp[dg * nc + 2 * j] = rho * cs;
-            if (2 * j + 1 < nc) sProp[dg * nc + 2 * j + 1] = rho * sn;
+        // --- draws: lanes share the (sweep, walker, pair) Philox blocks of the G walkers, two sweeps at a time
+        if ((sw & 1) == 0) {
+          const int per = G * (npair + 1), nsw = (sw + 1 < mp.n_sweeps) ? 2 : 1;
+          for (int idx = lane; idx < nsw * per; idx += 32) {
+            const int ds = (idx >= per) ? 1 : 0, id2 = idx - ds * per;
+            const int dg = id2 / (npair + 1), j = id2 - dg * (npair + 1);
+            const uint64_t gw = (uint64_t)(mp.walker_offset + grp * G + dg);
+            uint32_t o[4];
+            philox4x32_10((uint32_t)gw, mp.sweep0 + (uint32_t)(sw + ds), (j == npair) ? 0xFFFFFFFFu : (uint32_t)j,
+                          (uint32_t)(gw >> 32), mp.key0, mp.key1, o);
+            const double lu = log_pos(u53(o[0], o[1]), sLogT, P.mc);
+            double *dst = sDraw + ds * DR;
+            if (j == npair) {
+              dst[96 + dg] = lu;
+            } else {
+              const double rho = sqrt_pos(-2.0 * lu);
+              double sn, cs;
+              sincos_2pi(u53(o[2], o[3]), sSinT, P.mc, sn, cs);
+              dst[dg * nc + 2 * j] = rho * cs;
+              if (2 * j + 1 < nc) dst[dg * nc + 2 * j + 1] = rho * sn;
+            }
           }
+          __syncwarp();
         }
-        __syncwarp();
+        const double *sProp = sDraw + (sw & 1) * DR, *sLogU = sProp + 96;
         if (own) {
           xp = fma(mp.step, sProp[g * nc + 3 * e + 0], x);
           yp = fma(mp.step, sProp[g * nc + 3 * e + 1], y);
           zp = fma(mp.step, sProp[g * nc + 3 * e + 2], z);
         }
         logu = sLogU[own ? g : 0];
-        __syncwarp();
       }
       eval_walkers<NS, NMO, false, X, false, false, EEN>(P, sExp, sC, sDet, ws, xp, yp, zp, lane);
       const double lp2 = sRes[rg + 0], sg2 = sRes[rg + 1];
