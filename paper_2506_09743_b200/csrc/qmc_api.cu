@@ -35,6 +35,7 @@ int cuda_fail(cudaError_t e, const char *what) {
 
 struct Variant {
   int NS, NMO, LP, ws_doubles;
+  int psi_ws_doubles;    // the values-only kernels' compact scratch
   int metro_ws_doubles;  // the sampler's per-warp scratch: the evaluator's plus two sweeps of draws
   bool exact;  // compiled for n_up = n_dn = NS
   const void *k_el, *k_psi, *k_metro, *k_expl, *k_el_deriv;
@@ -53,7 +54,8 @@ Variant make_variant() {
   v.LP = Geo<NS, NMO>::LP;
   v.exact = X;
   v.ws_doubles = Geo<NS, NMO>::total;
-  v.metro_ws_doubles = Geo<NS, NMO>::total + 2 * kDrawDoubles<NS>;
+  v.psi_ws_doubles = Geo<NS, NMO>::totalC(true);
+  v.metro_ws_doubles = Geo<NS, NMO>::totalC(true) + 2 * kDrawDoubles<NS>;
   v.k_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl>;
   v.k_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi>;
   v.k_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi>;
@@ -721,7 +723,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   P.n_mo_all = d->n_mo;
   P.smem_const_bytes = (int)((szC + szD + 15) / 16 * 16);
   s->smem_el = P.smem_const_bytes + kWarpsEl * var->ws_doubles * (int)sizeof(double);
-  s->smem_psi = P.smem_const_bytes + kWarpsPsi * var->ws_doubles * (int)sizeof(double);
+  s->smem_psi = P.smem_const_bytes + kWarpsPsi * var->psi_ws_doubles * (int)sizeof(double);
   s->smem_metro = P.smem_const_bytes + kWarpsPsi * var->metro_ws_doubles * (int)sizeof(double);
 
   int dev_smem = 0, n_sm = 0;

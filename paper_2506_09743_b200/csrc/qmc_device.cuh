@@ -30,7 +30,9 @@ constexpr int kMaxEen = 6;    // terms of the electron-electron-nucleus Jastrow 
 #define QMC_EARLY_INV 0      // Gauss-Jordan: invert every pivot candidate before the arg-max is known
 #endif
 #ifndef QMC_WARPS_PSI
-#define QMC_WARPS_PSI 10     // warps per block of the values-only kernels (log|Psi|, Metropolis): they fit 96 registers
+#define QMC_WARPS_PSI 12     // warps per block of the values-only kernels (log|Psi|, Metropolis): 24 warps per SM at 80 registers
+                             // (96 bytes of spills) with the compact scratch layout; measured 5.62 ms per 20 CO sweeps against
+                             // 5.69 with 10 warps per block (96 registers, no spills)
 #endif
 #ifndef QMC_WARPS_ORB
 #define QMC_WARPS_ORB 10     // warps per block of the orbital-derivative kernel (one block per SM; 8 when shared memory is short).
@@ -275,6 +277,14 @@ struct Geo {
   static constexpr int oProb = oXYZ + 96;
   static constexpr int oRes = oProb + 2 * GMAX * 4;           // per walker {log|Psi|, sign, E_L, -}
   static constexpr int layout_total = oRes + GMAX * 4;
+  // Compact layout of the values-only evaluator (log|Psi| kernel, sampler): no operator rows B, no G staging, no M
+  // tables -- the per-electron scalars, coordinates and results follow the values-only AO tile / the T tables
+  // directly (CO: 760 doubles per warp instead of 1088), which is what lets 24 warps share an SM.
+  static constexpr int psiBase = even(cmax(cmax(kChunk * 36, oT + szT), szPhi));
+  __host__ __device__ static constexpr int oPartC(bool c) { return c ? psiBase : oPart; }
+  __host__ __device__ static constexpr int oXYZC(bool c) { return oPartC(c) + 64; }
+  __host__ __device__ static constexpr int oProbC(bool c) { return oXYZC(c) + 96; }
+  __host__ __device__ static constexpr int oResC(bool c) { return oProbC(c) + 2 * GMAX * 4; }
   // DMMA contraction scratch, from offset 0 (everything it overlays is dead while it is live): the AO
   // tile [kChunk AO rows][S].  Column = lane for the AO values; for E_L the combined operator of the
   // lane sits in column opCol(lane) >= 32, so every lane (also one that owns no electron) stores
@@ -299,6 +309,7 @@ struct Geo {
   }
   __host__ __device__ static constexpr int mergeShift(int fr) { return (fr & 4) << 3; }  // rows 4..7: + 32
   static constexpr int total = cmax(layout_total, kChunk * S2);
+  __host__ __device__ static constexpr int totalC(bool c) { return c ? oResC(true) + GMAX * 4 : total; }
   static constexpr int NT = (NMO + 7) / 8;                    // 8-column MO tiles
   // orbital-derivative kernel only: behind the common scratch, Gamma [ROWS][NMO], then the inverses of one determinant's
   // problems [2 GMAX][NS][NS] and their column indices [2 GMAX][NS] (ints)

@@ -228,6 +228,10 @@ __device__ __noinline__ void een_param_terms(const SysParams &P, const double *s
 // is accumulated behind the common scratch (Geo::oGam), for the orbital-parameter derivatives.
 // ORB = 2 (table path, values only): the same Gamma from the reference alone: A0^-1 through an identity block of the
 // elimination, Y = d den / d T accumulated in the CI pass, Gamma_virt = A0^-T Y / den, Gamma_occ = A0^-T - Gamma_virt T^T.
+// the values-only evaluation on its own (log|Psi| kernel, sampler) uses the compact scratch layout
+template <bool EL, bool EXPL, int ORB>
+constexpr bool kCompact = !EL && !EXPL && ORB == 0;
+
 template <int NS, int NMO, bool EL, bool X, bool EXPL = false, bool DERIV = false, bool EEN = false, int ORB = 0>
 __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp,
                              const double *__restrict__ sC, const DetRec *__restrict__ sDet,
@@ -239,9 +243,10 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
   const int n_up = X ? NS : P.n_up, n_dn = X ? NS : P.n_dn, ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
   const int g = lane / ne, e = lane - g * ne;
   const bool active = lane < G * ne;
-  double *sPhi = ws + GE::oPhi, *sB = ws + GE::oB, *sXYZ = ws + GE::oXYZ, *sPart = ws + GE::oPart;
-  double *sG = ws + GE::oG, *sT = ws + GE::oT, *sProb = ws + GE::oProb;
-  double *sRes = ws + GE::oRes;
+  constexpr bool CP = kCompact<EL, EXPL, ORB>;  // values-only evaluation: compact scratch layout (Geo::oPartC ...)
+  double *sPhi = ws + GE::oPhi, *sB = ws + GE::oB, *sXYZ = ws + GE::oXYZC(CP), *sPart = ws + GE::oPartC(CP);
+  double *sG = ws + GE::oG, *sT = ws + GE::oT, *sProb = ws + GE::oProbC(CP);
+  double *sRes = ws + GE::oResC(CP);
 
   // ---- publish coordinates for the pair loop
   sXYZ[lane] = x;  // [xyz][lane]: the pair loop reads consecutive lanes

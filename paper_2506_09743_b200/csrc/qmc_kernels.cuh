@@ -46,7 +46,8 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   load_constants<NMO>(P, smem, sC, sExp, sDet, wsBase);
   using GE = Geo<NS, NMO>;
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;  // shfl: tells the compiler it is warp-uniform
-  double *ws = wsBase + warp * GE::total;
+  constexpr bool CP = kCompact<EL, false, 0>;
+  double *ws = wsBase + warp * GE::totalC(CP);
   const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
   const int g = lane / ne, e = lane - g * ne;
   const int64_t n_groups = (io.M + G - 1) / G;
@@ -69,7 +70,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     if (lane < G) {
       const int64_t wo = grp * G + lane;
       if (wo < io.M) {
-        const double *res = ws + GE::oRes + lane * 4;
+        const double *res = ws + GE::oResC(CP) + lane * 4;
         if (io.logpsi) io.logpsi[wo] = res[0];
         if (io.sign) io.sign[wo] = res[1];
         if (EL && io.eloc) io.eloc[wo] = res[2];
@@ -445,11 +446,11 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   // G (ceil(3 n_e / 2) + 1) Philox blocks per sweep rarely fill the 32 lanes evenly (CO: 44 = 32 + 12), two sweeps' worth
   // do better (88 of 96)
   constexpr int DR = kDrawDoubles<NS>;  // one sweep: normals [G][3 n_e] (<= 96 doubles), then log u [G]
-  double *ws = wsBase + warp * (GE::total + 2 * DR);
+  double *ws = wsBase + warp * (GE::totalC(true) + 2 * DR);
   const double2 *sLogT = reinterpret_cast<const double2 *>(sExp + kExpTab);  // log_pos table
   const double2 *sSinT = sLogT + 64;                                         // sincos_2pi table
-  double *sDraw = ws + GE::total;
-  const double *sRes = ws + GE::oRes;
+  double *sDraw = ws + GE::totalC(true);
+  const double *sRes = ws + GE::oResC(true);
   const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G, nc = 3 * ne, npair = (nc + 1) / 2;
   const int g = lane / ne, e = lane - g * ne;
   const int64_t n_groups = (io.M + G - 1) / G;
