@@ -86,6 +86,12 @@ def lib(extended: bool = False):
             L.oracle_nuclear_log_gradient.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p]
             L.oracle_energy_gradient.restype = None
             L.oracle_energy_gradient.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
+            L.oracle_ao_eval2.restype = None
+            L.oracle_ao_eval2.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+            L.oracle_nuclear_energy_gradient.restype = C.c_int
+            L.oracle_nuclear_energy_gradient.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p]
+            L.oracle_force.restype = None
+            L.oracle_force.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
             _libs[extended] = L
     return _libs[extended]
 
@@ -293,3 +299,43 @@ def nuclear_log_gradient(sysd: OracleSystem, r_soa, threads: int = 1):
         with ThreadPoolExecutor(len(rs)) as ex:
             list(ex.map(run, rs))
     return dR
+
+
+def ao_eval2(sysd: OracleSystem, ao: int, xyz):
+    """{phi, grad[3], lap, Hessian xx yy zz xy yz zx, grad lap[3]} of one AO at one point."""
+    xyz = np.ascontiguousarray(xyz, np.float64)
+    out = np.empty(14)
+    sysd.L.oracle_ao_eval2(sysd.ref, ao, _p(xyz), _p(out))
+    return out
+
+
+def nuclear_energy_gradient(sysd: OracleSystem, r_soa, threads: int = 1):
+    """dE[M, n_atoms, 3] = grad_alpha E_L (first term of eq. 7); Pade e-e Jastrow only."""
+    r = np.ascontiguousarray(r_soa, np.float64)
+    M = r.shape[2]
+    dE = np.empty((M, int(sysd.c.n_atoms), 3))
+    L = sysd.L
+
+    def run(rng):
+        rc = L.oracle_nuclear_energy_gradient(sysd.ref, _p(r), M, rng[0], rng[1], _p(dE))
+        assert rc == 0, rc
+
+    rs = _ranges(M, threads)
+    if len(rs) == 1:
+        run(rs[0])
+    else:
+        with ThreadPoolExecutor(len(rs)) as ex:
+            list(ex.map(run, rs))
+    return dE
+
+
+def force(eloc, dE, dlnpsi):
+    """eq. 7: (F[n_atoms, 3], terms[2, n_atoms, 3]) from E_L [M], grad_alpha E_L and grad_alpha ln|Psi| [M, n_atoms, 3]."""
+    e = np.ascontiguousarray(eloc, np.float64)
+    a = np.ascontiguousarray(dE, np.float64)
+    b = np.ascontiguousarray(dlnpsi, np.float64)
+    na = a.shape[1]
+    F = np.empty((na, 3))
+    T = np.empty((2, na, 3))
+    lib().oracle_force(_p(e), _p(a), _p(b), e.shape[0], na, _p(F), _p(T))
+    return F, T

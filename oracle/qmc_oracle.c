@@ -958,3 +958,283 @@ int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, 
   free(aov); free(aog); free(mo); free(A); free(Ai); free(gam); free(pos);
   return 0;
 }
+
+/* ------------------------------------------------------------------ */
+/* Second-level AO derivatives for the forces (eq. 7):    */
+/* the atomic positions are inputs of the AO layer,  */
+/* d ao(r_i) / d R = -grad_r ao(r_i), so grad_R E_L needs the Hessian  */
+/* of every AO and the gradient of its Laplacian.  Product rule term   */
+/* by term on phi = N S(d) f(r), f = r^k e^{-zeta r}, u = d / r:        */
+/*  d_c d_e phi = N [S_ce f + (S_c u_e + S_e u_c) f' + S (f'' u_c u_e  */
+/*                   + f' (delta_ce - u_c u_e) / r)]                    */
+/*  lap phi     = N [lapS f + 2 f' (grad S . u) + S (f'' + 2 f'/r)]     */
+/*  d_c lap phi = N [lapS f' u_c + 2 f'' u_c (grad S . u)               */
+/*                   + 2 f' d_c(grad S . u) + S_c (f'' + 2 f'/r)        */
+/*                   + S (f''' + 2 f''/r - 2 f'/r^2) u_c]               */
+/*  d_c (grad S . u) = sum_e [S_ec u_e + S_e (delta_ec - u_e u_c) / r]  */
+/* out14 = {phi, grad[3], lap, hess xx yy zz xy yz zx, grad lap[3]}    */
+/* ------------------------------------------------------------------ */
+
+static void solid_harmonic_hessian(int l, int m, real H[3][3]) {
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b) H[a][b] = 0.0;
+  if (l != 2) return; /* S is constant or linear */
+  if (m == 0) H[0][1] = H[1][0] = 1.0;                          /* xy */
+  if (m == 1) H[1][2] = H[2][1] = 1.0;                          /* yz */
+  if (m == 2) H[0][2] = H[2][0] = 1.0;                          /* zx */
+  if (m == 3) { H[0][0] = 2.0; H[1][1] = -2.0; }                /* x^2 - y^2 */
+  if (m == 4) { H[0][0] = -2.0; H[1][1] = -2.0; H[2][2] = 4.0; } /* 2 z^2 - x^2 - y^2 */
+}
+
+static void ao_eval2_r(const oracle_system_desc_t *s, int ao, const real *xyz, real *out14) {
+  int a = s->ao_atom[ao], n = s->ao_n[ao], l = s->ao_l[ao], m = s->ao_m[ao];
+  real zeta = s->ao_zeta[ao];
+  real N = s->ao_norm ? s->ao_norm[ao] : sto_norm_r(n, l, m, zeta);
+  real d[3], u[3];
+  for (int c = 0; c < 3; ++c) d[c] = xyz[c] - s->atom_xyz[3 * a + c];
+  real r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+  for (int c = 0; c < 3; ++c) u[c] = d[c] / r;
+  int k = n - 1 - l;
+  real S, gS[3], hS[3], HS[3][3];
+  solid_harmonic(l, m, d[0], d[1], d[2], &S, gS, hS);
+  solid_harmonic_hessian(l, m, HS);
+  real lapS = HS[0][0] + HS[1][1] + HS[2][2];
+  /* radial factor and three derivatives, term by term */
+  real e = exp(-zeta * r);
+  real rk = pow(r, (real)k);
+  real rk1 = (k >= 1) ? pow(r, (real)(k - 1)) : 0.0;
+  real rk2 = (k >= 2) ? pow(r, (real)(k - 2)) : 0.0;
+  real rk3 = (k >= 3) ? pow(r, (real)(k - 3)) : 0.0;
+  real f = rk * e;
+  real f1 = ((real)k * rk1 - zeta * rk) * e;
+  real f2 = ((real)(k * (k - 1)) * rk2 - 2.0 * (real)k * zeta * rk1 + zeta * zeta * rk) * e;
+  real f3 = ((real)(k * (k - 1) * (k - 2)) * rk3 - 3.0 * (real)(k * (k - 1)) * zeta * rk2 + 3.0 * (real)k * zeta * zeta * rk1 -
+             zeta * zeta * zeta * rk) * e;
+  real gSu = gS[0] * u[0] + gS[1] * u[1] + gS[2] * u[2];
+  out14[0] = N * S * f;
+  for (int c = 0; c < 3; ++c) out14[1 + c] = N * (gS[c] * f + S * f1 * u[c]);
+  out14[4] = N * (lapS * f + 2.0 * f1 * gSu + S * (f2 + 2.0 * f1 / r));
+  real hess[3][3];
+  for (int c = 0; c < 3; ++c)
+    for (int q = 0; q < 3; ++q) {
+      real dl = (c == q) ? 1.0 : 0.0;
+      hess[c][q] = N * (HS[c][q] * f + (gS[c] * u[q] + gS[q] * u[c]) * f1 + S * (f2 * u[c] * u[q] + f1 * (dl - u[c] * u[q]) / r));
+    }
+  out14[5] = hess[0][0]; out14[6] = hess[1][1]; out14[7] = hess[2][2];
+  out14[8] = hess[0][1]; out14[9] = hess[1][2]; out14[10] = hess[2][0];
+  for (int c = 0; c < 3; ++c) {
+    real dgSu = 0.0;
+    for (int q = 0; q < 3; ++q) dgSu += HS[q][c] * u[q] + gS[q] * (((q == c) ? 1.0 : 0.0) - u[q] * u[c]) / r;
+    out14[11 + c] = N * (lapS * f1 * u[c] + 2.0 * f2 * u[c] * gSu + 2.0 * f1 * dgSu + gS[c] * (f2 + 2.0 * f1 / r) +
+                         S * (f3 + 2.0 * f2 / r - 2.0 * f1 / (r * r)) * u[c]);
+  }
+}
+
+void oracle_ao_eval2(const oracle_system_desc_t *s, int ao, const double *xyz, double *out14) {
+  real p[3] = {xyz[0], xyz[1], xyz[2]}, o[14];
+  ao_eval2_r(s, ao, p, o);
+  for (int q = 0; q < 14; ++q) out14[q] = (double)o[q];
+}
+
+/* ------------------------------------------------------------------ */
+/* grad_alpha E_L, the first term of the force estimator (eq. 7,       */
+/* PAPER.md:86), for the Pade e-e Jastrow D.1 (which does not see the  */
+/* nuclei).  Differentiates, long-hand, exactly what local_energy_one  */
+/* evaluates:                                                           */
+/*   E_L = -1/2 [lapJ + |gJ|^2 + 2 gJ . gS / S + lapS / S] + V          */
+/*   S = sum_n w_n, w_n = d_n D_n^up D_n^dn; gS = sum_n w_n gamma_n,     */
+/*   gamma_n[i] = sum_k A^-1[k][i] grad phi_k(r_i) (F.3 / G.2);          */
+/*   lapS = sum_n w_n t_n, t_n = sum_ik A^-1[k][i] lap phi_k(r_i) (G.7)  */
+/* with, for a displacement of R_alpha,c (written d_j below):            */
+/*   d_j A[i][k] = -sum_{beta on alpha} C[beta][k] d_c ao_beta(r_i)      */
+/*   d_j ln D = Tr(A^-1 d_j A),  d_j A^-1 = -A^-1 (d_j A) A^-1           */
+/*   d_j w_n = w_n (Tr^up + Tr^dn)                                       */
+/* and the same chain rule on gamma_n and t_n (AO Hessian, gradient of   */
+/* the AO Laplacian), every determinant inverted explicitly.  The        */
+/* potential adds  d V_en / d R_alpha = -Z_alpha sum_i (r_i - R_alpha) / */
+/* |r_i - R_alpha|^3  and  d V_nn / d R_alpha = -Z_alpha sum_beta Z_beta */
+/* (R_alpha - R_beta) / |R_alpha - R_beta|^3   (eq. 1).     */
+/* dE [M][n_atoms][3].  Returns -2 when the wavefunction carries the     */
+/* e-n / e-e-n Jastrow kernels (their R-dependence is not derived here). */
+/* ------------------------------------------------------------------ */
+
+int oracle_nuclear_energy_gradient(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
+                                   int64_t w1, double *dE) {
+  if (s->jastrow_en_w0 != 0.0 || s->jastrow_en_w1 != 0.0 || s->n_een > 0) return -2;
+  int ne = s->n_up + s->n_dn, nmo = s->n_mo, nao = s->n_ao, na = s->n_atoms, nj = 3 * na;
+  size_t nem = (size_t)ne * (size_t)nmo;
+  real *mo = (real *)malloc(sizeof(real) * (nem * 5 + 1));                 /* [i][a]{val, gx, gy, gz, lap} */
+  real *dval = (real *)malloc(sizeof(real) * ((size_t)nj * nem + 1));       /* d_j phi_a(r_i) */
+  real *dgrd = (real *)malloc(sizeof(real) * ((size_t)nj * nem * 3 + 1));   /* d_j d_q phi_a(r_i) */
+  real *dlap = (real *)malloc(sizeof(real) * ((size_t)nj * nem + 1));       /* d_j lap phi_a(r_i) */
+  real *A = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
+  real *Ai = (real *)malloc(sizeof(real) * (size_t)(2 * ne * ne + 2));
+  real *dA = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
+  real *dAi = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
+  real *tmp = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
+  real *gam = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));          /* gamma_n of the current determinant */
+  real *dgam = (real *)malloc(sizeof(real) * (size_t)(nj * 3 * ne + 1));    /* d_j gamma_n */
+  real *gS = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
+  real *dgS = (real *)malloc(sizeof(real) * (size_t)(nj * 3 * ne + 1));
+  real *gJ = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
+  real *pos = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
+  real *tr = (real *)malloc(sizeof(real) * (size_t)(2 * nj + 1));
+  real *dt = (real *)malloc(sizeof(real) * (size_t)(2 * nj + 1));
+  real *dSig = (real *)malloc(sizeof(real) * (size_t)(nj + 1));
+  real *dlapS = (real *)malloc(sizeof(real) * (size_t)(nj + 1));
+  if (!mo || !dval || !dgrd || !dlap || !A || !Ai || !dA || !dAi || !tmp || !gam || !dgam || !gS || !dgS || !gJ || !pos ||
+      !tr || !dt || !dSig || !dlapS)
+    return -1;
+  real ao[14];
+  for (int64_t w = w0; w < w1; ++w) {
+    gather_walker(r, M, w, ne, pos);
+    for (size_t q = 0; q < nem * 5; ++q) mo[q] = 0.0;
+    for (size_t q = 0; q < (size_t)nj * nem; ++q) { dval[q] = 0.0; dlap[q] = 0.0; }
+    for (size_t q = 0; q < (size_t)nj * nem * 3; ++q) dgrd[q] = 0.0;
+    for (int i = 0; i < ne; ++i)
+      for (int beta = 0; beta < nao; ++beta) {
+        ao_eval2_r(s, beta, pos + 3 * i, ao);
+        int at = s->ao_atom[beta];
+        real hess[3][3] = {{ao[5], ao[8], ao[10]}, {ao[8], ao[6], ao[9]}, {ao[10], ao[9], ao[7]}};
+        for (int a = 0; a < nmo; ++a) {
+          real cf = s->mo_coeff[beta * nmo + a];
+          for (int q = 0; q < 5; ++q) mo[((size_t)i * nmo + a) * 5 + q] += cf * ao[q];
+          for (int c = 0; c < 3; ++c) { /* d / d R_{at,c} = - d / d r_c on this AO */
+            size_t j = (size_t)(3 * at + c);
+            dval[j * nem + (size_t)i * nmo + a] -= cf * ao[1 + c];
+            for (int q = 0; q < 3; ++q) dgrd[(j * nem + (size_t)i * nmo + a) * 3 + q] -= cf * hess[c][q];
+            dlap[j * nem + (size_t)i * nmo + a] -= cf * ao[11 + c];
+          }
+        }
+      }
+    real J, lapJ;
+    jastrow_all(s, pos, &J, gJ, &lapJ);
+    real sigma = 0.0, lapS = 0.0;
+    for (int i = 0; i < 3 * ne; ++i) gS[i] = 0.0;
+    for (int j = 0; j < nj; ++j) { dSig[j] = 0.0; dlapS[j] = 0.0; }
+    for (int q = 0; q < nj * 3 * ne; ++q) dgS[q] = 0.0;
+    for (int n = 0; n < s->n_det; ++n) {
+      real D[2], t[2];
+      for (int sp = 0; sp < 2; ++sp) {
+        int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
+        const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
+        real *inv = Ai + sp * ne * ne;
+        for (int i = 0; i < ns; ++i)
+          for (int k = 0; k < ns; ++k) A[i * ns + k] = mo[((size_t)(e0 + i) * nmo + lst[k]) * 5 + 0];
+        D[sp] = det_inv_r(ns, A, inv);
+        t[sp] = 0.0;
+        for (int i = 0; i < ns; ++i) {
+          for (int c = 0; c < 3; ++c) {
+            real g = 0.0;
+            for (int k = 0; k < ns; ++k) g += inv[k * ns + i] * mo[((size_t)(e0 + i) * nmo + lst[k]) * 5 + 1 + c];
+            gam[3 * (e0 + i) + c] = g;
+          }
+          for (int k = 0; k < ns; ++k) t[sp] += inv[k * ns + i] * mo[((size_t)(e0 + i) * nmo + lst[k]) * 5 + 4];
+        }
+        for (int j = 0; j < nj; ++j) {
+          const real *dv = dval + (size_t)j * nem, *dg = dgrd + (size_t)j * nem * 3, *dl = dlap + (size_t)j * nem;
+          for (int i = 0; i < ns; ++i)
+            for (int k = 0; k < ns; ++k) dA[i * ns + k] = dv[(size_t)(e0 + i) * nmo + lst[k]];
+          real trj = 0.0;
+          for (int i = 0; i < ns; ++i)
+            for (int k = 0; k < ns; ++k) trj += inv[k * ns + i] * dA[i * ns + k];
+          tr[2 * j + sp] = trj;
+          /* d A^-1 = -A^-1 dA A^-1 */
+          for (int i = 0; i < ns; ++i)
+            for (int k = 0; k < ns; ++k) {
+              real v = 0.0;
+              for (int q = 0; q < ns; ++q) v += dA[i * ns + q] * inv[q * ns + k];
+              tmp[i * ns + k] = v;
+            }
+          for (int i = 0; i < ns; ++i)
+            for (int k = 0; k < ns; ++k) {
+              real v = 0.0;
+              for (int q = 0; q < ns; ++q) v += inv[i * ns + q] * tmp[q * ns + k];
+              dAi[i * ns + k] = -v;
+            }
+          real dtj = 0.0;
+          for (int i = 0; i < ns; ++i) {
+            for (int c = 0; c < 3; ++c) {
+              real g = 0.0;
+              for (int k = 0; k < ns; ++k)
+                g += dAi[k * ns + i] * mo[((size_t)(e0 + i) * nmo + lst[k]) * 5 + 1 + c] +
+                     inv[k * ns + i] * dg[((size_t)(e0 + i) * nmo + lst[k]) * 3 + c];
+              dgam[(j * ne + e0 + i) * 3 + c] = g;
+            }
+            for (int k = 0; k < ns; ++k)
+              dtj += dAi[k * ns + i] * mo[((size_t)(e0 + i) * nmo + lst[k]) * 5 + 4] + inv[k * ns + i] * dl[(size_t)(e0 + i) * nmo + lst[k]];
+          }
+          dt[2 * j + sp] = dtj;
+        }
+      }
+      real wn = s->ci_coeff[n] * D[0] * D[1];
+      sigma += wn;
+      for (int i = 0; i < 3 * ne; ++i) gS[i] += wn * gam[i];
+      lapS += wn * (t[0] + t[1]);
+      for (int j = 0; j < nj; ++j) {
+        real dw = wn * (tr[2 * j] + tr[2 * j + 1]);
+        dSig[j] += dw;
+        for (int i = 0; i < 3 * ne; ++i) dgS[j * 3 * ne + i] += dw * gam[i] + wn * dgam[j * 3 * ne + i];
+        dlapS[j] += dw * (t[0] + t[1]) + wn * (dt[2 * j] + dt[2 * j + 1]);
+      }
+    }
+    double *out = dE + (size_t)w * (size_t)nj;
+    for (int at = 0; at < na; ++at)
+      for (int c = 0; c < 3; ++c) {
+        int j = 3 * at + c;
+        /* kinetic: -1/2 [2 gJ . d(gS/S) + d(lapS/S)] */
+        real cross = 0.0;
+        for (int i = 0; i < 3 * ne; ++i) cross += gJ[i] * (dgS[j * 3 * ne + i] / sigma - gS[i] * dSig[j] / (sigma * sigma));
+        real dkin = -0.5 * (2.0 * cross + dlapS[j] / sigma - lapS * dSig[j] / (sigma * sigma));
+        /* potential */
+        real dven = 0.0, dvnn = 0.0;
+        for (int i = 0; i < ne; ++i) {
+          real dx = pos[3 * i] - s->atom_xyz[3 * at], dy = pos[3 * i + 1] - s->atom_xyz[3 * at + 1],
+               dz = pos[3 * i + 2] - s->atom_xyz[3 * at + 2];
+          real rho = sqrt(dx * dx + dy * dy + dz * dz);
+          real dc = (c == 0) ? dx : ((c == 1) ? dy : dz);
+          dven -= s->atom_Z[at] * dc / (rho * rho * rho);
+        }
+        for (int b = 0; b < na; ++b) {
+          if (b == at) continue;
+          real dx = s->atom_xyz[3 * at] - s->atom_xyz[3 * b], dy = s->atom_xyz[3 * at + 1] - s->atom_xyz[3 * b + 1],
+               dz = s->atom_xyz[3 * at + 2] - s->atom_xyz[3 * b + 2];
+          real rho = sqrt(dx * dx + dy * dy + dz * dz);
+          real dc = (c == 0) ? dx : ((c == 1) ? dy : dz);
+          dvnn -= s->atom_Z[at] * s->atom_Z[b] * dc / (rho * rho * rho);
+        }
+        out[j] = (double)(dkin + dven + dvnn);
+      }
+  }
+  free(mo); free(dval); free(dgrd); free(dlap); free(A); free(Ai); free(dA); free(dAi); free(tmp); free(gam); free(dgam);
+  free(gS); free(dgS); free(gJ); free(pos); free(tr); free(dt); free(dSig); free(dlapS);
+  return 0;
+}
+
+/* ------------------------------------------------------------------ */
+/* Force estimator, eq. 7 (reading Q23: the minus sign     */
+/* covers both terms, ln rho = 2 ln|Psi|):                              */
+/*   F_alpha = -(1/M) sum_m [grad_alpha E_L + 2 (E_L - E_v) grad_alpha ln|Psi|] */
+/* Kahan sums.  F [n_atoms][3]; terms [2][n_atoms][3] (may be NULL)     */
+/* receives the two contributions separately.                           */
+/* ------------------------------------------------------------------ */
+
+void oracle_force(const double *eloc, const double *dE, const double *dlnpsi, int64_t M, int32_t n_atoms,
+                  double *F, double *terms) {
+  double ev = kahan_mean(eloc, M);
+  for (int j = 0; j < 3 * n_atoms; ++j) {
+    double s1 = 0.0, c1 = 0.0, s2 = 0.0, c2 = 0.0;
+    for (int64_t m = 0; m < M; ++m) {
+      double y = dE[(size_t)m * (size_t)(3 * n_atoms) + j] - c1, t = s1 + y;
+      c1 = (t - s1) - y;
+      s1 = t;
+      y = 2.0 * (eloc[m] - ev) * dlnpsi[(size_t)m * (size_t)(3 * n_atoms) + j] - c2;
+      t = s2 + y;
+      c2 = (t - s2) - y;
+      s2 = t;
+    }
+    double a = -s1 / (double)M, b = -s2 / (double)M;
+    F[j] = a + b;
+    if (terms) { terms[j] = a; terms[3 * n_atoms + j] = b; }
+  }
+}

@@ -129,6 +129,22 @@ int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, i
 int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                                 int64_t w1, double *dR);
 
+/* One AO at one point with its second-level derivatives: out14 = {phi, grad[3], lap, Hessian xx yy zz xy yz zx,
+ * grad lap [3]}.  PAPER.md:55; needed because d ao / d R = -grad_r ao. */
+void oracle_ao_eval2(const oracle_system_desc_t *s, int ao, const double *xyz, double *out14);
+
+/* grad_alpha E_L, the first term of the force estimator (eq. 7): dE [M][n_atoms][3], rows w0 <= w < w1.
+ * Pade e-e Jastrow (D.1) only: returns -2 when the e-n / e-e-n kernels are switched on.  Every determinant is
+ * inverted explicitly and the chain rule is applied long-hand to what oracle_local_energy evaluates. */
+int oracle_nuclear_energy_gradient(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
+                                   int64_t w1, double *dE);
+
+/* Force estimator of eq. 7 (reading Q23):
+ *   F_alpha = -(1/M) sum_m [grad_alpha E_L + 2 (E_L - E_v) grad_alpha ln|Psi|].
+ * eloc [M]; dE, dlnpsi [M][n_atoms][3]; F [n_atoms][3]; terms [2][n_atoms][3] (the two contributions) may be NULL. */
+void oracle_force(const double *eloc, const double *dE, const double *dlnpsi, int64_t M, int32_t n_atoms,
+                  double *F, double *terms);
+
 /* Estimator of eq. 6: E_v = mean E_L, grad_p = (2/M) sum_m O[m][p] (E_L[m] - E_v).
  * Kahan sums.  Ev may be NULL. */
 void oracle_energy_gradient(const double *eloc, const double *O, int64_t M, int32_t n_param,

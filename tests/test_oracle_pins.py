@@ -1003,3 +1003,148 @@ def test_nuclear_log_gradient_closed_form_translation_and_partition():
     d, r = wl.lih(M=9)
     o = ob.OracleSystem(d)
     assert np.array_equal(ob.nuclear_log_gradient(o, r, threads=1), ob.nuclear_log_gradient(o, r, threads=3))
+
+
+# ---------------------------------------------------------------- forces: grad_alpha E_L and the estimator of eq. 7
+def test_ao_hessian_and_laplacian_gradient_vs_central_differences():
+    # oracle_ao_eval2's new outputs against Richardson central differences of the PINNED first-level outputs of
+    # oracle_ao_eval (gradient -> Hessian, Laplacian -> its gradient), for every kind of AO: s with k = 0, 1, 2,
+    # every p and d harmonic, with a radial power
+    aos = [(1, 0, 0, 1.3), (2, 0, 0, 0.9), (3, 0, 0, 1.1)] + [(2, 1, m, 1.2) for m in range(3)] + \
+          [(3, 1, m, 0.8) for m in range(3)] + [(3, 2, m, 1.0) for m in range(5)] + [(4, 2, m, 1.4) for m in range(5)]
+    d = atom_system(1.0, aos, np.eye(len(aos))[:, :1], 1, 0, xyz=(0.2, -0.1, 0.3))
+    o = ob.OracleSystem(d)
+    rng = np.random.default_rng(11)
+    pairs = {(0, 0): 5, (1, 1): 6, (2, 2): 7, (0, 1): 8, (1, 2): 9, (2, 0): 10}
+    for ao in range(len(aos)):
+        for _ in range(3):
+            x = np.array([0.2, -0.1, 0.3]) + rng.standard_normal(3) * 0.7 + 0.3
+            v = ob.ao_eval2(o, ao, x)
+            assert np.max(np.abs(v[:5] - ob.ao_eval(o, ao, x))) < 1e-14 * max(1.0, np.max(np.abs(v[:5])))
+
+            def cd(q, c, h):
+                e = np.zeros(3); e[c] = h
+                return (ob.ao_eval(o, ao, x + e)[q] - ob.ao_eval(o, ao, x - e)[q]) / (2 * h)
+
+            scale = max(1.0, np.max(np.abs(v)))
+            for (a, b), k in pairs.items():
+                fd = (4 * cd(1 + a, b, 5e-4) - cd(1 + a, b, 1e-3)) / 3     # d_b of (d_a phi)
+                assert abs(v[k] - fd) < 2e-8 * scale, (aos[ao], a, b, v[k], fd)
+            for c in range(3):
+                fd = (4 * cd(4, c, 5e-4) - cd(4, c, 1e-3)) / 3             # d_c of lap phi
+                assert abs(v[11 + c] - fd) < 2e-7 * scale, (aos[ao], c, v[11 + c], fd)
+
+
+@pytest.mark.parametrize("name,M", [("H2", 5), ("LiH", 4), ("Li2", 3), ("CO", 2)])
+def test_nuclear_energy_gradient_vs_central_differences_of_E_L(name, M):
+    # grad_alpha E_L against Richardson central differences of the oracle's own pinned E_L with one nuclear
+    # coordinate displaced: a wrong sign of d ao / d R, a dropped d(A^-1) term, a wrong CI weight derivative or a
+    # missing potential term each fail it
+    import copy
+    d, r = wl.CONFIGS[name](M=64)
+    lp_all = ob.local_energy(ob.OracleSystem(d), r)[0]
+    idx = _keep_away(d, r)
+    idx = idx[np.argsort(-lp_all[idx])][:M]                 # away from nuclei and nodes (Q17)
+    rk = np.ascontiguousarray(r[:, :, idx])
+    dE = ob.nuclear_energy_gradient(ob.OracleSystem(d), rk)
+    assert dE.shape == (len(idx), d.n_atoms, 3)
+
+    def el(a, c, t):
+        d2 = copy.copy(d)
+        xyz = np.array(d.atom_xyz, np.float64, copy=True)
+        xyz[a, c] += t
+        d2.atom_xyz = xyz
+        return ob.local_energy(ob.OracleSystem(d2, extended=True), rk)[2]
+
+    for a in range(d.n_atoms):
+        for c in range(3):
+            cd = lambda h: (el(a, c, h) - el(a, c, -h)) / (2 * h)
+            ref = (4 * cd(1e-4) - cd(2e-4)) / 3
+            assert np.max(np.abs(dE[:, a, c] - ref) / np.maximum(1, np.abs(ref))) < 1e-6, (name, a, c, dE[:, a, c], ref)
+
+
+def test_nuclear_energy_gradient_closed_forms_and_translation_invariance():
+    # hydrogen-like 1s (zeta) on a nucleus Z at R plus a bare charge q at R2 (no basis functions on it):
+    #   E_L = -zeta^2/2 + (zeta - Z)/|r - R| - q/|r - R2| + Z q/|R - R2|
+    #   grad_R  E_L = (zeta - Z)(r - R)/|r - R|^3 - Z q (R - R2)/|R - R2|^3
+    #   grad_R2 E_L = -q (r - R2)/|r - R2|^3      + Z q (R - R2)/|R - R2|^3
+    from paper_2506_09743_b200.workloads import SystemDesc
+    Z, zeta, q = 2.0, 1.6, 0.7
+    R, R2 = np.array([0.3, -0.2, 0.5]), np.array([-1.1, 0.9, 2.0])
+    d = SystemDesc("h-like+q", np.array([R, R2]), np.array([Z, q]), 1, 0, np.zeros(1, np.int32), np.ones(1, np.int32),
+                   np.zeros(1, np.int32), np.zeros(1, np.int32), np.array([zeta]), None, np.array([[1.0]]),
+                   np.zeros((1, 1), np.int32), np.zeros((1, 0), np.int32), np.array([1.0]), 0.25, 0.5, 1.0)
+    rr = _rand_pos(60, 1, 1.5, rmin=0.05, seed=97) + R
+    dE = ob.nuclear_energy_gradient(ob.OracleSystem(d), soa(rr))
+    v, v2, RR = rr[:, 0] - R, rr[:, 0] - R2, R - R2
+    want = np.stack([(zeta - Z) * v / np.linalg.norm(v, axis=1, keepdims=True) ** 3 - Z * q * RR / np.linalg.norm(RR) ** 3,
+                     -q * v2 / np.linalg.norm(v2, axis=1, keepdims=True) ** 3 + Z * q * RR / np.linalg.norm(RR) ** 3], axis=1)
+    assert np.max(np.abs(dE - want) / np.maximum(1, np.abs(want))) < 1e-12
+    # translation invariance of E_L(r; R): sum_alpha grad_alpha E_L = -sum_i grad_i E_L, the right side by Richardson
+    # central differences of the oracle's E_L under a rigid shift of every electron (Li2, 20 determinants)
+    dsys, r = wl.li2(M=64)
+    o = ob.OracleSystem(dsys)
+    lp_all = ob.local_energy(o, r)[0]
+    idx = _keep_away(dsys, r)
+    idx = idx[np.argsort(-lp_all[idx])][:4]
+    rk = np.ascontiguousarray(r[:, :, idx])
+    tot = ob.nuclear_energy_gradient(o, rk).sum(axis=1)
+    ox = ob.OracleSystem(dsys, extended=True)
+    for c in range(3):
+        def shifted(t):
+            r2 = rk.copy()
+            r2[:, c, :] += t
+            return ob.local_energy(ox, r2)[2]
+        cd = lambda h: (shifted(h) - shifted(-h)) / (2 * h)
+        ref = -(4 * cd(1e-4) - cd(2e-4)) / 3
+        assert np.max(np.abs(tot[:, c] - ref) / np.maximum(1, np.abs(ref))) < 1e-6, (c, tot[:, c], ref)
+    # the e-n / e-e-n kernels are not covered: the call says so instead of returning a partial derivative
+    L = ob.lib()
+    o2 = ob.OracleSystem(_with_en(dsys, 0.2, 0.0, 0.8))
+    out = np.zeros((rk.shape[2], 2, 3))
+    assert L.oracle_nuclear_energy_gradient(o2.ref, rk.ctypes.data, rk.shape[2], 0, rk.shape[2], out.ctypes.data) == -2
+
+
+def test_force_estimator_formula_and_physical_pin():
+    # (i) the reduction itself against math.fsum of eq. 7 (reading Q23)
+    rng = np.random.default_rng(8)
+    M, na = 500, 3
+    e = rng.standard_normal(M) * 2 - 7
+    dE, dl = rng.standard_normal((M, na, 3)), rng.standard_normal((M, na, 3))
+    F, T = ob.force(e, dE, dl)
+    ev = math.fsum(e) / M
+    for a in range(na):
+        for c in range(3):
+            t1 = -math.fsum(dE[:, a, c]) / M
+            t2 = -math.fsum(2 * (e - ev) * dl[:, a, c]) / M
+            assert abs(T[0, a, c] - t1) < 1e-13 and abs(T[1, a, c] - t2) < 1e-13 and abs(F[a, c] - (t1 + t2)) < 1e-13
+    # (ii) physical pin of both terms' signs and of the factor 2: He+-like exact 1s (zeta = Z = 2) on nucleus A at the
+    # origin, a bare charge q at distance R on the z axis.  The variational energy depends on R only through
+    #   E(R) = const + Z q / R - q phi(R),  phi(R) = [1 - e^{-2 zeta R}(1 + zeta R)] / R  (potential of the 1s density),
+    # so F_B = -dE/dR = q [(Z - 1)/R^2 + e^{-2 zeta R}(1/R^2 + 2 zeta/R + 2 zeta^2)] along +z and F_A = -F_B.
+    # For B only the first term of eq. 7 contributes (Psi does not depend on R_B); for A the second term carries
+    # +q/R^2 of the total (1 - Z) q/R^2 to leading order, so a factor 1 instead of 2 would be ~50% off.
+    from paper_2506_09743_b200.workloads import SystemDesc
+    Z = zeta = 2.0
+    q, R = 0.5, 3.0
+    d = SystemDesc("He+ + q", np.array([[0.0, 0.0, 0.0], [0.0, 0.0, R]]), np.array([Z, q]), 1, 0, np.zeros(1, np.int32),
+                   np.ones(1, np.int32), np.zeros(1, np.int32), np.zeros(1, np.int32), np.array([zeta]), None,
+                   np.array([[1.0]]), np.zeros((1, 1), np.int32), np.zeros((1, 0), np.int32), np.array([1.0]), 0.25, 0.5, 1.0)
+    o = ob.OracleSystem(d)
+    M = 60000
+    nt = os.cpu_count() or 1
+    out = ob.metropolis(o, soa(_rand_pos(M, 1, 0.5, rmin=0.02, seed=19)), 0.45, 60, seed=77, threads=nt)
+    r = out["r"]
+    el = ob.local_energy(o, r, threads=nt)[2]
+    dE = ob.nuclear_energy_gradient(o, r, threads=nt)
+    dl = ob.nuclear_log_gradient(o, r, threads=nt)
+    F, T = ob.force(el, dE, dl)
+    FB = q * ((Z - 1) / R ** 2 + math.exp(-2 * zeta * R) * (1 / R ** 2 + 2 * zeta / R + 2 * zeta ** 2))
+    ev = el.mean()
+    per_walker = -(dE + 2 * (el - ev)[:, None, None] * dl)
+    sig = per_walker.std(axis=0, ddof=1) / math.sqrt(M)
+    assert abs(F[1, 2] - FB) < 4 * sig[1, 2] and abs(F[0, 2] + FB) < 4 * sig[0, 2], (F, FB, sig)
+    assert sig[0, 2] < 0.05 * FB and sig[1, 2] < 0.05 * FB                     # the pin resolves sign and scale
+    assert np.max(np.abs(F[:, :2])) < 4 * np.max(sig[:, :2]) + 1e-12           # no force off the axis
+    assert abs(T[1, 1, 2]) < 1e-12                                             # Psi does not depend on R_B
+    assert abs(T[1, 0, 2] - q / R ** 2) < 0.15 * q / R ** 2                    # second term: +q/R^2 to leading order
