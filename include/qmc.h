@@ -220,9 +220,29 @@ int qmc_orbital_derivatives(qmc_system_t *s, const double *d_r, int64_t M, doubl
  * d ao_beta(r_i) / d R_alpha = -grad_r ao_beta(r_i) for the AOs of centre alpha, contracted with Gamma = d ln Sigma /
  * d Phi exactly as qmc_orbital_derivatives does (same table path and the same explicit route for near-singular
  * references).  Two launches on cuda_stream (Jastrow part, then the AO part).  Deterministic.  Asynchronous.
- * Returns QMC_EINVAL for null pointers or M <= 0, QMC_EUNSUPPORTED when the shape does not fit shared memory.
- * The other half of eq. 7, grad_alpha E_L, is not provided. */
+ * Returns QMC_EINVAL for null pointers or M <= 0, QMC_EUNSUPPORTED when the shape does not fit shared memory. */
 int qmc_nuclear_log_gradient(qmc_system_t *s, const double *d_r, int64_t M, double *d_dR, void *cuda_stream);
+
+/* Nuclear gradient of the local energy, grad_alpha E_L: the first term of the force estimator, eq. 7 (
+ * the paper obtains it by automatic differentiation through the AO layer's atomic coordinates; here
+ * it is analytic):
+ *   d_r  device, in:  double [n_e][3][M]
+ *   d_dE device, out: double [M][n_atoms][3]  d E_L / d R_alpha,c ; every entry is written
+ * E_L = -1/2 lap Psi / Psi + V of eq. 1-3 with d ao_beta(r_i) / d R_alpha = -grad_r ao_beta(r_i) for the AOs of centre
+ * alpha: the AO Hessian and the gradient of the AO Laplacian enter, and d (V_en + V_nn) / d R_alpha (eq. 1).  Every
+ * determinant is eliminated on its own (the explicit route of PAPER.md:349) for every walker, so the cost is
+ * proportional to n_det.  Covers the Pade e-e Jastrow D.1 (which does not see the nuclei); with the e-n / e-e-n kernels
+ * D.2 / D.3 switched on the call returns QMC_EUNSUPPORTED.  Two launches on cuda_stream.  Deterministic.  Asynchronous.
+ * QMC_EINVAL for null pointers or M <= 0. */
+int qmc_nuclear_energy_gradient(qmc_system_t *s, const double *d_r, int64_t M, double *d_dE, void *cuda_stream);
+
+/* Force estimator of eq. 7 (reading Q23: the minus sign covers both terms, ln rho = 2 ln|Psi|):
+ *   F_alpha = -(1/M) sum_m [ grad_alpha E_L(r_m) + 2 (E_L(r_m) - E_v) grad_alpha ln|Psi(r_m)| ]
+ *   d_eloc device in [M]; d_dE (qmc_nuclear_energy_gradient) and d_dlnpsi (qmc_nuclear_log_gradient) device in
+ *   [M][n_atoms][3]; h_F host out [n_atoms][3]; h_terms host out [2][n_atoms][3], the two contributions (may be NULL).
+ * Deterministic (fixed partition, compensated sums).  Synchronises cuda_stream. */
+int qmc_force(const double *d_eloc, const double *d_dE, const double *d_dlnpsi, int64_t M, int32_t n_atoms, double *h_F,
+              double *h_terms, void *cuda_stream);
 
 /* Estimator of eq. 6: E_v = mean E_L, grad_p = (2/M) sum_m O[m][p] (E_L[m] - E_v).
  *   d_eloc device in [M]; d_O device in [M][n_param]; h_Ev host out (may be NULL);

@@ -17,7 +17,7 @@ _lib = None
 EXPORTS = ["qmc_setup", "qmc_destroy", "qmc_local_energy", "qmc_log_psi", "qmc_metropolis", "qmc_batch_stats",
            "qmc_fp64_peak", "qmc_model_flops", "qmc_launch_count", "qmc_status_string", "qmc_n_param", "qmc_local_energy_explicit", "qmc_set_kernel_timing", "qmc_kernel_times",
            "qmc_log_derivatives", "qmc_energy_gradient", "qmc_local_energy_host", "qmc_orbital_derivatives",
-           "qmc_nuclear_log_gradient"]
+           "qmc_nuclear_log_gradient", "qmc_nuclear_energy_gradient", "qmc_force"]
 
 
 class QmcError(RuntimeError):
@@ -67,6 +67,10 @@ def lib():
         L.qmc_orbital_derivatives.argtypes = [vp, vp, i64, vp, vp, vp]
         L.qmc_nuclear_log_gradient.restype = C.c_int
         L.qmc_nuclear_log_gradient.argtypes = [vp, vp, i64, vp, vp]
+        L.qmc_nuclear_energy_gradient.restype = C.c_int
+        L.qmc_nuclear_energy_gradient.argtypes = [vp, vp, i64, vp, vp]
+        L.qmc_force.restype = C.c_int
+        L.qmc_force.argtypes = [vp, vp, vp, i64, C.c_int32, vp, vp, vp]
         L.qmc_local_energy_host.restype = C.c_int
         L.qmc_local_energy_host.argtypes = [vp, vp, i64, vp, vp, vp, C.c_int32]
         L.qmc_log_psi.restype = C.c_int
@@ -248,6 +252,13 @@ class QmcSystem:
         _check(lib().qmc_nuclear_log_gradient(self._h, _dp(r), M, _dp(dR), _stream(stream)))
         return dR
 
+    def nuclear_energy_gradient(self, r, n_atoms: int, stream=None):
+        """qmc_nuclear_energy_gradient: dE[M, n_atoms, 3] = grad_alpha E_L (first term of eq. 7)."""
+        M = self._chk_r(r)
+        dE = torch.empty((M, n_atoms, 3), dtype=torch.float64, device=r.device)
+        _check(lib().qmc_nuclear_energy_gradient(self._h, _dp(r), M, _dp(dE), _stream(stream)))
+        return dE
+
     def n_param(self) -> int:
         return int(lib().qmc_n_param(self._h))
 
@@ -287,6 +298,18 @@ def energy_gradient(eloc, O, stream=None):
     _check(lib().qmc_energy_gradient(_dp(eloc), _dp(O), eloc.numel(), int(O.shape[1]), C.addressof(ev), _np(g),
                                      _stream(stream)))
     return ev.value, g
+
+
+def force(eloc, dE, dlnpsi, stream=None):
+    """qmc_force: (F[n_atoms, 3], terms[2, n_atoms, 3]) of eq. 7 from device E_L [M], grad_alpha E_L and
+    grad_alpha ln|Psi| [M, n_atoms, 3]."""
+    assert eloc.is_cuda and dE.is_cuda and dlnpsi.is_cuda and eloc.dtype == dE.dtype == dlnpsi.dtype == torch.float64
+    assert eloc.is_contiguous() and dE.is_contiguous() and dlnpsi.is_contiguous()
+    assert dE.shape == dlnpsi.shape and dE.shape[0] == eloc.numel() and dE.shape[2] == 3
+    na = int(dE.shape[1])
+    F, T = np.empty((na, 3)), np.empty((2, na, 3))
+    _check(lib().qmc_force(_dp(eloc), _dp(dE), _dp(dlnpsi), eloc.numel(), na, _np(F), _np(T), _stream(stream)))
+    return F, T
 
 
 def fp64_peak(kind: int = 0, reps: int = 5, device: int = 0) -> float:

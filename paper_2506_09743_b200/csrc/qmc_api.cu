@@ -43,7 +43,9 @@ struct Variant {
   const void *k_orb;  // orbital-parameter derivatives, kWarpsOrb warps per block
   const void *k_orb_small;  // the same with kWarpsOrbSmall warps (less shared memory)
   const void *k_nuc, *k_nuc_small;  // the same kernel in nuclear mode (qmc_nuclear_log_gradient)
-  int orb_ws_doubles;  // the same with the e-e-n Jastrow kernel D.3 (EEN)
+  int orb_ws_doubles;
+  const void *k_frc, *k_frc_small;  // nuclear energy gradient (8 / 4 warps per block)
+  int frc_ws_doubles;
 };
 
 template <int NS, int NMO, bool X>
@@ -66,6 +68,9 @@ Variant make_variant() {
   v.k_nuc = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrb, true>;
   v.k_nuc_small = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrbSmall, true>;
   v.orb_ws_doubles = Geo<NS, NMO>::total + Geo<NS, NMO>::orbExtra;
+  v.k_frc = (const void *)nuclear_energy_gradient_kernel<NS, NMO, X, 8>;
+  v.k_frc_small = (const void *)nuclear_energy_gradient_kernel<NS, NMO, X, 4>;
+  v.frc_ws_doubles = Geo<NS, NMO>::total + Geo<NS, NMO>::frcExtra;
   v.e_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, false, true>;
   v.e_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi, false, true>;
   v.e_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi, true>;
@@ -186,6 +191,8 @@ struct qmc_system {
   std::unordered_map<cudaStream_t, Scratch> scratch;
   std::vector<void *> retired;
   // qmc_local_energy_host: two internal streams and double-buffered device scratch (grown on demand)
+  bool frc_ready = false;  // nuclear energy-gradient kernel configured (lazily)
+  int frc_warps = 0, blocks_frc = 0;
   bool orb_ready = false;  // orbital-derivative kernel configured (lazily: most users never call it)
   int orb_warps = 0;
   bool time_kernels = false;  // qmc_set_kernel_timing: events around the two kernels of an E_L call
@@ -1079,6 +1086,73 @@ int qmc_nuclear_log_gradient(qmc_system_t *s, const double *d_r, int64_t M, doub
   CK(cudaGetLastError());
   ++g_launches;
   return orbital_launch(s, d_r, M, nullptr, nullptr, d_dR, cuda_stream);
+}
+
+int qmc_nuclear_energy_gradient(qmc_system_t *s, const double *d_r, int64_t M, double *d_dE, void *cuda_stream) {
+  if (!s || !d_r || M <= 0 || !d_dE) return QMC_EINVAL;
+  if (s->P.has_en || s->P.n_een > 0) return QMC_EUNSUPPORTED;  // the R-dependence of D.2 / D.3 inside E_L is not derived
+  CK(cudaSetDevice(s->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  auto smem_for = [&](int warps) { return s->P.smem_const_bytes + warps * s->var.frc_ws_doubles * (int)sizeof(double); };
+  {
+    std::lock_guard<std::mutex> lock(s->scratch_mu);  // lazy configuration
+    if (!s->frc_ready) {
+      int dev_smem = 0;
+      cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, s->device);
+      s->frc_warps = smem_for(8) <= dev_smem ? 8 : 4;
+      if (smem_for(s->frc_warps) > dev_smem) return QMC_EUNSUPPORTED;
+      const void *k = s->frc_warps == 8 ? s->var.k_frc : s->var.k_frc_small;
+      CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_for(s->frc_warps)));
+      int per_sm = 0;
+      CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, s->frc_warps * 32, smem_for(s->frc_warps)));
+      if (per_sm < 1) return QMC_EUNSUPPORTED;
+      s->blocks_frc = per_sm * s->n_sm;
+      s->frc_ready = true;
+    }
+  }
+  // d V / d R initialises dE, one thread per walker; the wavefunction part is added by the second launch
+  nuclear_potential_gradient_kernel<<<(unsigned)((M + 127) / 128), 128, 0, st>>>(s->P, d_r, M, d_dE);
+  CK(cudaGetLastError());
+  ++g_launches;
+  WalkerIO io{};
+  io.r_in = d_r;
+  io.M = M;
+  io.O = d_dE;
+  const int warps = s->frc_warps;
+  const int64_t groups = (M + s->P.G - 1) / s->P.G;
+  const int grid = (int)std::min<int64_t>((groups + warps - 1) / warps, s->blocks_frc);
+  void *args[2] = {(void *)&s->P, (void *)&io};
+  CK(cudaLaunchKernel(warps == 8 ? s->var.k_frc : s->var.k_frc_small, dim3(grid), dim3(warps * 32), args, smem_for(warps), st));
+  ++g_launches;
+  return QMC_OK;
+}
+
+int qmc_force(const double *d_eloc, const double *d_dE, const double *d_dlnpsi, int64_t M, int32_t n_atoms, double *h_F,
+              double *h_terms, void *cuda_stream) {
+  if (!d_eloc || !d_dE || !d_dlnpsi || M <= 0 || n_atoms < 1 || !h_F) return QMC_EINVAL;
+  int dev = 0;
+  if (int rc = device_of(d_eloc, &dev)) return rc;
+  CK(cudaSetDevice(dev));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int nc = 3 * n_atoms;
+  const int nblk = (int)std::min<int64_t>(1184, (M + 63) / 64);
+  ReduceScratch *r = nullptr;
+  if (int rc = reduce_scratch(dev, st, (size_t)2 * nc, (size_t)nblk * 2 * (size_t)nc, &r)) return rc;
+  const int sblk = (int)std::min<int64_t>(kReduceBlocks, (M + kStatsThreads - 1) / kStatsThreads);
+  batch_stats_kernel<<<sblk, kStatsThreads, 0, st>>>(d_eloc, M, r->d_partial, r->d_done, r->d_stats);
+  CK(cudaGetLastError());
+  force_partial_kernel<<<nblk, 128, 0, st>>>(d_eloc, d_dE, d_dlnpsi, M, nc, r->d_stats, r->d_gpart);
+  CK(cudaGetLastError());
+  force_final_kernel<<<2 * nc, 128, 0, st>>>(r->d_gpart, nblk, nc, M, r->d_stats, r->d_res);
+  CK(cudaGetLastError());
+  g_launches += 3;
+  CK(cudaStreamSynchronize(st));
+  for (int j = 0; j < nc; ++j) {
+    const double t1 = r->h_res[2 + j], t2 = r->h_res[2 + nc + j];
+    h_F[j] = t1 + t2;
+    if (h_terms) { h_terms[j] = t1; h_terms[nc + j] = t2; }
+  }
+  return QMC_OK;
 }
 
 int qmc_batch_stats(const double *d_x, int64_t M, double *h_mean, double *h_stderr, void *cuda_stream) {

@@ -318,6 +318,15 @@ struct Geo {
   static constexpr int oCol = oInv + even(2 * GMAX * NS * NS);
   static constexpr int oY = oCol + even(GMAX * NS);        // table path: Y = d den / d T, laid out like the T tables
   static constexpr int orbExtra = even(ROWS * NMO) + even(2 * GMAX * NS * NS) + even(GMAX * NS) + even(2 * GMAX * TS);
+  // nuclear energy-gradient kernel only (eval_walkers<..., ORB = 3>), behind the orbital-derivative extras: the second
+  // weight matrix Gamma2 [ROWS][NMO], grad_i J [3][32], the staging of A_n^-1 B_n for one pass of problems
+  // [PP][NS][NS] and X_n = A_n^-1 B_n A_n^-1 of one determinant's problems [2 GMAX][NS][NS]
+  static constexpr int oGam2 = oY + even(2 * GMAX * TS);
+  static constexpr int oGJ = oGam2 + even(ROWS * NMO);
+  static constexpr int oStage = oGJ + 96;
+  static constexpr int oX = oStage + even(PP * NS * NS);
+  static constexpr int frcExtra = orbExtra + even(ROWS * NMO) + 96 + even(PP * NS * NS) + even(2 * GMAX * NS * NS);
+  static_assert(oX + even(2 * GMAX * NS * NS) == total + frcExtra, "force-kernel scratch regions do not add up");
   // bounds of the overlays (compile-time hygiene: no memory checker runs on this pool)
   static_assert(NS >= 1 && NS <= kMaxSpin && NMO <= 16, "instantiation outside the register-array limits");
   static_assert(ROWS <= 32 && 2 * GMAX * NS >= ROWS, "electron rows of a pass exceed the warp");

@@ -226,6 +226,11 @@ __device__ __noinline__ void een_param_terms(const SysParams &P, const double *s
 // kernels of the common case stay free of the call and its register spills: measured 459 -> 508 us otherwise).
 // ORB = 1 (with EXPL): B = I, i.e. every determinant's inverse; Gamma[i][alpha] = sum_n d_n D_n^up D_n^dn A_n^-1[pos_n(alpha)][i]
 // is accumulated behind the common scratch (Geo::oGam), for the orbital-parameter derivatives.
+// ORB = 3 (with EXPL and EL): [A_n | B_n | I] is eliminated, so that both A_n^-1 and P_n = A_n^-1 B_n are at hand;
+// besides Gamma (= d Sigma / d Phi, unnormalised) the second weight matrix of the nuclear energy gradient is accumulated,
+//   Gamma2[i][alpha] = sum_n d_n D_n^up D_n^dn (t_n A_n^-1 - A_n^-1 B_n A_n^-1)[pos_n(alpha)][i],  t_n = t_n^up + t_n^dn
+// (= d (sum_n w_n t_n) / d Phi at fixed B; the derivative with respect to B is Gamma itself), and grad_i J is left in
+// Geo::oGJ for the caller.
 // ORB = 2 (table path, values only): the same Gamma from the reference alone: A0^-1 through an identity block of the
 // elimination, Y = d den / d T accumulated in the CI pass, Gamma_virt = A0^-T Y / den, Gamma_occ = A0^-T - Gamma_virt T^T.
 // the values-only evaluation on its own (log|Psi| kernel, sampler) uses the compact scratch layout
@@ -347,6 +352,13 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       gJz += t[3];
       lapJ += t[4];
     }
+  }
+
+  if (ORB == 3) {  // grad_i J for the caller (nuclear energy gradient: d B / d R needs it)
+    double *sGJ = ws + GE::oGJ;
+    sGJ[lane] = gJx;
+    sGJ[32 + lane] = gJy;
+    sGJ[64 + lane] = gJz;
   }
 
   // ---- stages a1-a4: STO shells and AO -> MO contraction.
@@ -518,8 +530,12 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
     double sig = 0.0, numk = 0.0;
     double *sGam = ws + GE::oGam, *sInv = ws + GE::oInv;
     int *sCol = reinterpret_cast<int *>(ws + GE::oCol);
-    if (ORB == 1) {
-      for (int i = lane; i < GE::ROWS * NMO; i += 32) sGam[i] = 0.0;
+    double *sGam2 = ws + GE::oGam2, *sStage = ws + GE::oStage, *sX = ws + GE::oX;
+    if (ORB == 1 || ORB == 3) {
+      for (int i = lane; i < GE::ROWS * NMO; i += 32) {
+        sGam[i] = 0.0;
+        if (ORB == 3) sGam2[i] = 0.0;
+      }
       __syncwarp();
     }
     // this warp takes determinants det0, det0 + det_step, ... (the block shares one walker group)
@@ -533,6 +549,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
         const int pg = pvalid ? (pr >> 1) : 0, sp = pr & 1;
         const int ns = sp ? n_dn : n_up, e0 = sp ? n_up : 0;
         double a0[NS], b0[NS];
+        double bi[ORB == 3 ? NS : 1];  // ORB = 3: identity block beside B
         {
           const bool cA = c < ns;
           const int colA = cA ? dc.col[sp][c < kMaxSpin ? c : 0] : 0;
@@ -543,6 +560,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
             a0[i] = (ri && cA) ? sPhi[GE::moIdx(EL, row, colA)] : ((i == c) ? 1.0 : 0.0);
             if (ORB == 1) b0[i] = (ri && cA && i == c) ? 1.0 : 0.0;  // B = I: the reduced block is A_n^-1 itself
             else b0[i] = (ri && cA) ? sB[EL ? GE::moIdx(EL, row, colA) : 0] : 0.0;
+            if (ORB == 3) bi[i] = (ri && cA && i == c) ? 1.0 : 0.0;
           }
         }
         double det = 1.0;
@@ -571,6 +589,12 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           b0[k] = t;
 #pragma unroll
           for (int i = 0; i < NS; ++i) if (i != k) b0[i] = fma(-f[i], t, b0[i]);
+          if (ORB == 3) {
+            t = bi[k] * inv;
+            bi[k] = t;
+#pragma unroll
+            for (int i = 0; i < NS; ++i) if (i != k) bi[i] = fma(-f[i], t, bi[i]);
+          }
         }
         int inversions = 0;
 #pragma unroll
@@ -587,17 +611,43 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           sProb[pr * 4 + 0] = det;
           sProb[pr * 4 + 2] = t0;
         }
-        if (ORB == 1 && pvalid && c < NS) {
-          // row k of the reduced block belongs to reference position perm[k]: b0[k] = A_n^-1[perm[k]][electron c]
+        if ((ORB == 1 || ORB == 3) && pvalid && c < NS) {
+          // row k of the reduced block belongs to reference position perm[k]: A_n^-1[perm[k]][electron c]
 #pragma unroll
           for (int k = 0; k < NS; ++k) {
-            sInv[(pr * NS + k) * NS + c] = b0[k];
+            sInv[(pr * NS + k) * NS + c] = (ORB == 3) ? bi[ORB == 3 ? k : 0] : b0[k];
             if (c == 0) sCol[pr * NS + k] = (perm[k] < ns) ? (int)dc.col[sp][perm[k] < kMaxSpin ? perm[k] : 0] : -1;
+          }
+        }
+        if (ORB == 3) {
+          // X = P A^-1, P = A^-1 B: lane c holds column c of P (rows in elimination order) and column c (electron c)
+          // of A^-1; P is staged so that every lane reads all of it:
+          //   X[perm[k']][e] = sum_k P[perm[k']][perm[k]] A^-1[perm[k]][e],  P[perm[k']][perm[k]] = stage[perm[k]][k']
+          double *gs = sStage + slot * NS * NS;
+          if (c < NS) {
+#pragma unroll
+            for (int k = 0; k < NS; ++k) gs[c * NS + k] = b0[k];
+          }
+          __syncwarp();
+          double xk[NS];
+#pragma unroll
+          for (int k2 = 0; k2 < NS; ++k2) xk[k2] = 0.0;
+#pragma unroll
+          for (int k = 0; k < NS; ++k) {
+            const double ak = bi[ORB == 3 ? k : 0];
+            const double *gcol = gs + perm[k] * NS;
+#pragma unroll
+            for (int k2 = 0; k2 < NS; ++k2) xk[k2] = fma(gcol[k2], ak, xk[k2]);
+          }
+          __syncwarp();
+          if (pvalid && c < NS) {
+#pragma unroll
+            for (int k2 = 0; k2 < NS; ++k2) sX[(pr * NS + k2) * NS + c] = xk[k2];
           }
         }
       }
       __syncwarp();
-      if (ORB == 1) {
+      if (ORB == 1 || ORB == 3) {
         // d ln D / d A[i][j] = A^-1[j][i], weighted by d_n D_n^up D_n^dn (both determinants are known only now)
         for (int pass = 0; pass * PP < nprob; ++pass) {
           const int pr = pass * PP + slot;
@@ -605,12 +655,17 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
             const int pg = pr >> 1, sp = pr & 1;
             const int ns = sp ? n_dn : n_up, e0 = sp ? n_up : 0;
             const double w = dc.d * sProb[pr * 4 + 0] * sProb[(pr ^ 1) * 4 + 0];
+            const double tt = sProb[pr * 4 + 2] + sProb[(pr ^ 1) * 4 + 2];  // t_n = t_n^up + t_n^dn
             if (c < ns) {
               const int row = pg * ne + e0 + c;
 #pragma unroll
               for (int k = 0; k < NS; ++k) {
                 const int col = sCol[pr * NS + k];
-                if (col >= 0) sGam[row * NMO + col] = fma(w, sInv[(pr * NS + k) * NS + c], sGam[row * NMO + col]);
+                if (col >= 0) {
+                  const double ai = sInv[(pr * NS + k) * NS + c];
+                  sGam[row * NMO + col] = fma(w, ai, sGam[row * NMO + col]);
+                  if (ORB == 3) sGam2[row * NMO + col] = fma(w, fma(tt, ai, -sX[(pr * NS + k) * NS + c]), sGam2[row * NMO + col]);
+                }
               }
             }
           }

@@ -428,6 +428,285 @@ __global__ void __launch_bounds__(128)
 }
 
 // ---------------------------------------------------------------------------------
+// Nuclear gradient of the local energy, grad_alpha E_L: the first term of the force estimator, eq. 7.
+// The atomic positions are inputs of the AO layer: d phi_beta(r_i) / d R_alpha = -grad phi_beta(r_i)
+// for the AOs of centre alpha.  With the Pade e-e Jastrow D.1 (which does not see the nuclei)
+//   E_L = -1/2 (lap J + |grad J|^2) + K + V,   K = sum_n w_n t_n / sum_n w_n,  w_n = d_n D_n^up D_n^dn,
+//   t_n = Tr(A_n^-1 B_n),  B = -1/2 lap phi - grad_i J . grad phi   (F.1-F.4, G.7 with the combined operator),
+// and the chain rule through every determinant collapses into two weight matrices (electrons x MOs),
+//   Gamma  = d Sigma / d Phi  = d (sum w t) / d B,      Gamma2 = d (sum w t) / d Phi   (eval_walkers<..., ORB = 3>):
+//   d_j K = [ (Gamma2 - K Gamma) : d_j Phi + Gamma : d_j B ] / Sigma.
+// At AO level, for a harmonic S (lap S = 0, grad S . d = l S), f = r^k e^{-zeta r}, u = d / r, rho = f'/f = k/r - zeta,
+// F2 = f''/f = rho^2 - k/r^2, lambda = lap(S f)/(S f) = zeta^2 - c1/r + c2/r^2 (c1, c2 of the shell record),
+// lambda' = c1/r^2 - 2 c2/r^3, q = grad_i J . u, gs = grad_i J . grad S, w_c = sum_e (grad_i J)_e S_ce:
+//   -d_c phi = -f (S_c + S rho u_c)                                                              (value columns)
+//   1/2 d_c lap phi + grad_i J . d_c grad phi = f [ S_c (lambda/2 + rho q) + w_c + S rho (grad_i J)_c / r
+//        + u_c ( S (rho lambda + lambda')/2 + rho gs + S q (F2 - rho / r) ) ]                   (operator columns)
+// One pass over the shell records per Cartesian component; the tile is contracted with the two weight matrices and
+// the (N C) fragments and summed per centre.  d V / d R_alpha was written by nuclear_potential_gradient_kernel.
+// This is the explicit route (every determinant eliminated on its own) for every walker.
+// ---------------------------------------------------------------------------------
+template <int CMP>
+__device__ __forceinline__ void force_ao_pair(double f, double S, double Sx, double Sy, double Sz, double wc, double gs,
+                                              double ux, double uy, double uz, double gJx, double gJy, double gJz, double ri,
+                                              double rho, double q, double lam, double dlam, double F2, double &val, double &op) {
+  const double Sc = (CMP == 0) ? Sx : ((CMP == 1) ? Sy : Sz);
+  const double uc = (CMP == 0) ? ux : ((CMP == 1) ? uy : uz);
+  const double gc = (CMP == 0) ? gJx : ((CMP == 1) ? gJy : gJz);
+  val = -f * fma(S * rho, uc, Sc);
+  const double inner = fma(0.5 * S, fma(rho, lam, dlam), fma(rho, gs, S * q * (F2 - rho * ri)));
+  op = f * (fma(Sc, fma(rho, q, 0.5 * lam), wc) + fma(uc, inner, S * rho * gc * ri));
+}
+
+template <int NS, int NMO, bool X, int WPB>
+__global__ void __launch_bounds__(WPB * 32, 1)
+    nuclear_energy_gradient_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const double *sC;
+  const double *sExp;
+  const DetRec *sDet;
+  double *wsBase;
+  load_constants<NMO>(P, smem, sC, sExp, sDet, wsBase);
+  using GE = Geo<NS, NMO>;
+  constexpr int S = GE::S2, NT = GE::NT;
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
+  double *ws = wsBase + warp * (GE::total + GE::frcExtra);
+  const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
+  const int g = lane / ne, e = lane - g * ne;
+  const int64_t n_groups = (io.M + G - 1) / G;
+  const int64_t stride = (int64_t)gridDim.x * WPB;
+  double *dEo = io.O;  // [M][n_atoms][3], initialised with d V / d R
+  const int *row_atom = P.ao_orig + P.n_chunks * kChunk;
+  double *sGam = ws + GE::oGam, *sGam2 = ws + GE::oGam2;
+  const double *sGJ = ws + GE::oGJ;
+  const double *sRes = ws + GE::oRes;
+  for (int64_t grp = (int64_t)blockIdx.x * WPB + warp; grp < n_groups; grp += stride) {
+    const int64_t w = grp * G + g;
+    double x, y, z;
+    if ((g < G) && (w < io.M)) {
+      x = io.r_in[((int64_t)e * 3 + 0) * io.M + w];
+      y = io.r_in[((int64_t)e * 3 + 1) * io.M + w];
+      z = io.r_in[((int64_t)e * 3 + 2) * io.M + w];
+    } else {
+      dummy_xyz(lane, x, y, z);
+    }
+    eval_walkers<NS, NMO, true, X, true, false, false, 3>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
+    // G1 = Gamma / Sigma, G2 = (Gamma2 - K Gamma) / Sigma, K = sum w t / Sigma
+    for (int i = lane; i < G * ne * NMO; i += 32) {
+      const int gg = i / (ne * NMO);
+      const double sig = sRes[gg * 4 + 0], K = sRes[gg * 4 + 1] / sig;
+      const double g1 = sGam[i] / sig;
+      sGam2[i] = sGam2[i] / sig - K * g1;
+      sGam[i] = g1;
+    }
+    const double gJx = sGJ[lane], gJy = sGJ[32 + lane], gJz = sGJ[64 + lane];
+    __syncwarp();
+    double *const tile = ws;
+    double *const tl = tile + lane, *const tz = tile + GE::opCol(lane);
+#pragma unroll 1
+    for (int cmp = 0; cmp < 3; ++cmp) {
+      int chunk = 0;
+      double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1.0, r = 1.0, ri = 1.0, q = 0.0;
+      for (int s = 0; s < P.n_shell; ++s) {
+        const ShellRec &sh = P.shells[s];
+        const int meta = sh.meta, kind = meta & 15;
+        if (kind == SH_ATOM) {
+          dx = x - sh.zeta;
+          dy = y - sh.c1;
+          dz = z - sh.c2;
+          r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+          ri = rsqrt_fast(r2);
+          r = r2 * ri;
+          q = fma(gJx, dx, fma(gJy, dy, gJz * dz)) * ri;
+          continue;
+        }
+        double f = exp_neg(-sh.zeta * r, sExp, P.mc);
+        if (meta & kMetaK1) f *= r;
+        if (meta & kMetaK2) f *= r2;
+        const double ux = dx * ri, uy = dy * ri, uz = dz * ri;
+        const double rho = fma(sh.kd, ri, -sh.zeta);
+        const double F2 = fma(rho, rho, -sh.kd * ri * ri);
+        const double lam = fma(fma(sh.c2, ri, -sh.c1), ri, sh.zeta * sh.zeta);
+        const double dlam = fma(-2.0 * sh.c2, ri, sh.c1) * ri * ri;
+        const int row = (meta >> 12) & 15, m = (meta >> 8) & 15;
+        // harmonics of this record: S, grad S, w = Hess(S) grad_i J, gs = grad_i J . grad S
+        double Sv[5], Sx[5], Sy[5], Sz[5], wx[5], wy[5], wz[5];
+        int nf = 1;
+        Sv[0] = 1.0; Sx[0] = Sy[0] = Sz[0] = 0.0; wx[0] = wy[0] = wz[0] = 0.0;
+        if (kind == SH_P || kind == SH_P1) {
+          const double pv[3] = {dx, dy, dz};
+          if (kind == SH_P) {
+            nf = 3;
+#pragma unroll
+            for (int t = 0; t < 3; ++t) { Sv[t] = pv[t]; Sx[t] = (t == 0); Sy[t] = (t == 1); Sz[t] = (t == 2); wx[t] = wy[t] = wz[t] = 0.0; }
+          } else {
+            Sv[0] = (m == 0) ? dx : ((m == 1) ? dy : dz);
+            Sx[0] = (m == 0); Sy[0] = (m == 1); Sz[0] = (m == 2);
+          }
+        } else if (kind == SH_D || kind == SH_D1) {
+          const double dS[5] = {dx * dy, dy * dz, dz * dx, fma(dx, dx, -dy * dy), fma(2.0 * dz, dz, -fma(dx, dx, dy * dy))};
+          const double dSx[5] = {dy, 0.0, dz, 2.0 * dx, -2.0 * dx};
+          const double dSy[5] = {dx, dz, 0.0, -2.0 * dy, -2.0 * dy};
+          const double dSz[5] = {0.0, dy, dx, 0.0, 4.0 * dz};
+          const double dwx[5] = {gJy, 0.0, gJz, 2.0 * gJx, -2.0 * gJx};
+          const double dwy[5] = {gJx, gJz, 0.0, -2.0 * gJy, -2.0 * gJy};
+          const double dwz[5] = {0.0, gJy, gJx, 0.0, 4.0 * gJz};
+          if (kind == SH_D) {
+            nf = 5;
+#pragma unroll
+            for (int t = 0; t < 5; ++t) { Sv[t] = dS[t]; Sx[t] = dSx[t]; Sy[t] = dSy[t]; Sz[t] = dSz[t]; wx[t] = dwx[t]; wy[t] = dwy[t]; wz[t] = dwz[t]; }
+          } else {
+#pragma unroll
+            for (int t = 0; t < 5; ++t)
+              if (t == m) { Sv[0] = dS[t]; Sx[0] = dSx[t]; Sy[0] = dSy[t]; Sz[0] = dSz[t]; wx[0] = dwx[t]; wy[0] = dwy[t]; wz[0] = dwz[t]; }
+          }
+        }
+#pragma unroll
+        for (int t = 0; t < 5; ++t) {
+          if (t < nf) {
+            const double gs = fma(gJx, Sx[t], fma(gJy, Sy[t], gJz * Sz[t]));
+            double val, op;
+            if (cmp == 0) force_ao_pair<0>(f, Sv[t], Sx[t], Sy[t], Sz[t], wx[t], gs, ux, uy, uz, gJx, gJy, gJz, ri, rho, q, lam, dlam, F2, val, op);
+            else if (cmp == 1) force_ao_pair<1>(f, Sv[t], Sx[t], Sy[t], Sz[t], wy[t], gs, ux, uy, uz, gJx, gJy, gJz, ri, rho, q, lam, dlam, F2, val, op);
+            else force_ao_pair<2>(f, Sv[t], Sx[t], Sy[t], Sz[t], wz[t], gs, ux, uy, uz, gJx, gJy, gJz, ri, rho, q, lam, dlam, F2, val, op);
+            tl[(row + t) * S] = val;
+            tz[(row + t) * S] = op;
+          }
+        }
+        const int flush = meta >> 20;
+        if (flush) {
+          for (int pr = flush; pr < kChunk; ++pr) { tl[pr * S] = 0.0; tz[pr * S] = 0.0; }
+          __syncwarp();
+          const double *cfr = sC + chunk * ((kChunk / 4) * NT * 32);
+          constexpr int CW = NMO <= 2 ? 2 : (NMO <= 4 ? 4 : (NMO <= 8 ? 8 : 16));
+          for (int pi = lane; pi < ((G * CW + 31) & ~31); pi += 32) {
+            const int gq = pi / CW, col = pi & (CW - 1);
+            const bool pv = gq < G && col < NMO;
+            const int gg = pv ? gq : 0;
+            const int64_t wo = grp * G + gg;
+            const bool ok = pv && col < P.n_mo && wo < io.M;
+            double g1[2 * NS], g2[2 * NS];
+#pragma unroll
+            for (int i = 0; i < 2 * NS; ++i) {
+              g1[i] = (pv && i < ne) ? sGam[(gg * ne + i) * NMO + col] : 0.0;
+              g2[i] = (pv && i < ne) ? sGam2[(gg * ne + i) * NMO + col] : 0.0;
+            }
+            double racc = 0.0;
+            int cur = -1;
+            for (int rw = 0; rw < kChunk; ++rw) {
+              const int R = chunk * kChunk + rw;
+              if (P.ao_orig[R] < 0) continue;
+              const double *trow = tile + rw * S;
+              double t = 0.0;
+#pragma unroll
+              for (int i = 0; i < 2 * NS; ++i)
+                if (i < ne) t = fma(trow[gg * ne + i], g2[i], fma(trow[GE::opCol(gg * ne + i)], g1[i], t));
+              const double cf = ok ? cfr[(((rw >> 2) * NT) + (col >> 3)) * 32 + 4 * (col & 7) + (rw & 3)] : 0.0;
+              double a = cf * t;
+#pragma unroll
+              for (int mm = 1; mm < CW; mm <<= 1) a += shfl_xor_d(a, mm);
+              const int at = row_atom[R];
+              if (at != cur) {  // the same lane owns walker gg in every chunk and pass: ordered read-modify-writes
+                if (cur >= 0 && pv && col == 0 && wo < io.M) dEo[(wo * P.n_atoms + cur) * 3 + cmp] += racc;
+                cur = at;
+                racc = 0.0;
+              }
+              racc += a;
+            }
+            if (cur >= 0 && pv && col == 0 && wo < io.M) dEo[(wo * P.n_atoms + cur) * 3 + cmp] += racc;
+          }
+          __syncwarp();
+          ++chunk;
+        }
+      }
+      __syncwarp();
+    }
+  }
+}
+
+// d (V_en + V_nn) / d R_alpha (eq. 1): -Z_alpha sum_i (r_i - R_alpha) / |r_i - R_alpha|^3
+// - Z_alpha sum_beta Z_beta (R_alpha - R_beta) / |R_alpha - R_beta|^3.  One thread per walker; writes every entry of dE.
+__global__ void __launch_bounds__(128)
+    nuclear_potential_gradient_kernel(const __grid_constant__ SysParams P, const double *__restrict__ rin, const int64_t M,
+                                      double *__restrict__ dE) {
+  const int64_t w = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= M) return;
+  for (int a = 0; a < P.n_atoms; ++a) {
+    const double Xa = P.atom[a][0], Ya = P.atom[a][1], Za = P.atom[a][2], Q = P.atom[a][3];
+    double gx = 0.0, gy = 0.0, gz = 0.0;
+    for (int b = 0; b < P.n_atoms; ++b) {
+      if (b == a) continue;
+      const double dx = Xa - P.atom[b][0], dy = Ya - P.atom[b][1], dz = Za - P.atom[b][2];
+      const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+      const double s = -Q * P.atom[b][3] / (r2 * sqrt(r2));
+      gx = fma(s, dx, gx);
+      gy = fma(s, dy, gy);
+      gz = fma(s, dz, gz);
+    }
+    for (int i = 0; i < P.n_e; ++i) {
+      const double dx = rin[((int64_t)i * 3 + 0) * M + w] - Xa, dy = rin[((int64_t)i * 3 + 1) * M + w] - Ya,
+                   dz = rin[((int64_t)i * 3 + 2) * M + w] - Za;
+      const double r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+      const double s = -Q / (r2 * sqrt(r2));
+      gx = fma(s, dx, gx);
+      gy = fma(s, dy, gy);
+      gz = fma(s, dz, gz);
+    }
+    double *o = dE + (w * P.n_atoms + a) * 3;
+    o[0] = gx;
+    o[1] = gy;
+    o[2] = gz;
+  }
+}
+
+// Force estimator, eq. 7 (reading Q23): per column j of [M][3 n_atoms]
+//   term1_j = -(1/M) sum_m dE[m][j],   term2_j = -(2/M) sum_m (E_L[m] - E_v) dlnpsi[m][j].
+// Block b sums a contiguous range of rows (Kahan), one block per column finishes in a fixed order.  stats[0] = E_v.
+__global__ void __launch_bounds__(128) force_partial_kernel(const double *__restrict__ eloc, const double *__restrict__ dE,
+                                                            const double *__restrict__ dl, int64_t M, int nc,
+                                                            const double *__restrict__ stats, double *__restrict__ partial) {
+  const double ev = stats[0];
+  const int64_t rows = (M + gridDim.x - 1) / gridDim.x;
+  const int64_t m0 = (int64_t)blockIdx.x * rows, m1 = (m0 + rows < M) ? m0 + rows : M;
+  for (int j = threadIdx.x; j < nc; j += blockDim.x) {
+    double s1 = 0.0, c1 = 0.0, s2 = 0.0, c2 = 0.0;
+    for (int64_t m = m0; m < m1; ++m) {
+      double yv = dE[m * nc + j] - c1, t = s1 + yv;
+      c1 = (t - s1) - yv;
+      s1 = t;
+      yv = (eloc[m] - ev) * dl[m * nc + j] - c2;
+      t = s2 + yv;
+      c2 = (t - s2) - yv;
+      s2 = t;
+    }
+    partial[((int64_t)blockIdx.x * 2 + 0) * nc + j] = s1;
+    partial[((int64_t)blockIdx.x * 2 + 1) * nc + j] = s2;
+  }
+}
+__global__ void __launch_bounds__(128) force_final_kernel(const double *__restrict__ partial, int nblk, int nc, int64_t M,
+                                                          const double *__restrict__ stats, double *__restrict__ res) {
+  // block (j, which): thread t adds the block partials t, t + 128, ... in order, then a fixed tree
+  __shared__ double sh[128];
+  const int j = blockIdx.x % nc, which = blockIdx.x / nc;
+  double s = 0.0, c = 0.0;
+  for (int b = threadIdx.x; b < nblk; b += blockDim.x) {
+    const double yv = partial[((int64_t)b * 2 + which) * nc + j] - c, t = s + yv;
+    c = (t - s) - yv;
+    s = t;
+  }
+  sh[threadIdx.x] = s;
+  __syncthreads();
+  for (int w = 64; w > 0; w >>= 1) {
+    if ((int)threadIdx.x < w) sh[threadIdx.x] += sh[threadIdx.x + w];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {  // res (mapped host memory) = {E_v, stderr, term1[nc], term2[nc]}
+    res[2 + which * nc + j] = (which == 0 ? -1.0 : -2.0) * sh[0] / (double)M;
+    if (blockIdx.x == 0) { res[0] = stats[0]; res[1] = stats[1]; }
+  }
+}
+
+// ---------------------------------------------------------------------------------
 // Persistent all-electron Metropolis (readings Q9, Q10).
 // Walker coordinates and log|Psi| stay in registers for all sweeps.
 // ---------------------------------------------------------------------------------

@@ -1123,3 +1123,143 @@ def test_every_call_writes_exactly_its_outputs(env, name, M):
         for g, nm in ((rw, "walkers"), (a, "logpsi"), (b, "sign"), (acc, "accept")) + (((ea, "eloc_acc"),) if with_acc else ()):
             g.check(f"qmc_metropolis {nm}")
     s.close()
+
+
+# ----------------------------------------------------------------------------- forces: grad_alpha E_L and eq. 7
+def check_nuclear_energy_gradient(env, d, r, threads=8):
+    """qmc_nuclear_energy_gradient against the oracle at 1e-8 max(1, |.|) on walkers with |Psi|/max|Psi| > 1e-6, with
+    long-double adjudication (tests.helpers.adjudicate); deterministic; returns (GPU array, exceptions)."""
+    torch, ob, qb = env
+    o, ox = ob.OracleSystem(d), ob.OracleSystem(d, extended=True)
+    lp0 = ob.local_energy(o, r, threads=threads)[0]
+    g0 = ob.nuclear_energy_gradient(o, r, threads=threads)
+    gx = ob.nuclear_energy_gradient(ox, r, threads=threads)
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    g = s.nuclear_energy_gradient(rg, d.n_atoms)
+    g2 = s.nuclear_energy_gradient(rg, d.n_atoms)
+    assert torch.equal(g, g2)
+    g = g.cpu().numpy()
+    s.close()
+    assert g.shape == g0.shape
+    keep = (lp0 - lp0.max() > math.log(1e-6)) & np.isfinite(gx).all(axis=(1, 2))
+    assert keep.sum() > 0
+    n_exc = adjudicate(g, g0, gx, 1e-8, scale=np.maximum(1.0, np.abs(gx)), mask=keep, what="grad_alpha E_L")
+    return g, n_exc
+
+
+@pytest.mark.parametrize("name,M", [("H2", 515), ("LiH", 300), ("Li2", 257), ("CO", 129)])
+def test_nuclear_energy_gradient_configs(env, name, M):
+    d, r = wl.CONFIGS[name](M=M)
+    g, n_exc = check_nuclear_energy_gradient(env, d, r)
+    assert n_exc <= max(2, M // 50)
+
+
+def test_nuclear_energy_gradient_odd_systems_determinant_classes_and_500_determinants(env):
+    rng = np.random.default_rng(31)
+    aos = [(2, 1, 2, 1.1), (1, 0, 0, 2.0), (3, 2, 3, 0.9), (2, 1, 0, 1.3), (3, 2, 1, 0.7), (2, 0, 0, 1.5),
+           (3, 0, 0, 1.2), (3, 1, 1, 0.8), (2, 1, 1, 1.3), (4, 2, 4, 1.1), (4, 1, 0, 0.9)]
+    C = rng.standard_normal((len(aos), 7))
+    for norm in (None, rng.uniform(0.5, 2, len(aos))):   # lone p / d functions, radial powers, custom normalisation, 3 up 2 down
+        d = atom_system(3.0, aos, C, 3, 2, det_up=[[4, 0, 2], [4, 5, 2], [1, 0, 2], [4, 3, 5]],
+                        det_dn=[[1, 3], [1, 3], [0, 3], [1, 2]], ci=[0.9, 0.2, -0.3, 0.15], norm=norm,
+                        a_par=0.25, a_anti=0.5, b=0.8, xyz=(0.1, -0.2, 0.3))
+        check_nuclear_energy_gradient(env, d, soa(rng.standard_normal((131, 5, 3)) * 1.5), threads=2)
+    for with_general in (False, True):                   # every determinant class, with and without a triple substitution
+        rng = np.random.default_rng(77)
+        d = _classes_system(rng, with_general)
+        check_nuclear_energy_gradient(env, d, soa(rng.standard_normal((203, 7, 3)) * 1.2 + np.array([0.2, 0.1, -0.3])), threads=4)
+    d, r = wl.co_scan(M=40, n_geom=2)[1]                 # 500 determinants
+    check_nuclear_energy_gradient(env, d, r)
+
+
+def test_nuclear_energy_gradient_three_centres_bare_charge_edge_sizes_and_unsupported(env):
+    torch, ob, qb = env
+    rng = np.random.default_rng(4)
+    from paper_2506_09743_b200.workloads import SystemDesc, expand_shells
+    xyz = np.array([[0, 0, 0], [1.8, 0.2, 0], [-0.5, 1.6, 0.4], [0.3, -1.5, 1.1]], float)
+    shells = [["1s", "2s", "2p", "3d"], ["1s", "2p"], ["1s", "1s", "2s"], []]      # the last centre is a bare charge
+    ao = expand_shells(shells, rng.uniform(0.6, 3.0, 9))
+    n_ao = len(ao[0])
+    Cm = np.linalg.qr(rng.standard_normal((n_ao, n_ao)))[0][:, :7]
+    up, dn = wl.select_determinants(rng, 4, [4, 5, 6], 12)
+    d = SystemDesc("tri+q", xyz, np.array([6.0, 1.0, 1.0, 0.5]), 4, 4, *ao, None, Cm, up, dn,
+                   np.concatenate([[0.9], rng.normal(0, 0.1, 11)]))
+    for M in (1, 2, 3, 333):
+        check_nuclear_energy_gradient(env, d, wl.make_walkers(rng, xyz, 8, M), threads=4)
+    # hydrogen-like closed form on the GPU: grad_R E_L = (zeta - Z)(r - R)/|r - R|^3
+    Z, zeta, R = 2.0, 1.6, np.array([0.3, -0.2, 0.5])
+    da = atom_system(Z, [(1, 0, 0, zeta)], [[1.0]], 1, 0, xyz=tuple(R))
+    rr = rng.standard_normal((257, 1, 3)) * 1.5 + R
+    s = qb.QmcSystem(da)
+    g = s.nuclear_energy_gradient(_to_gpu(torch, soa(rr)), 1).cpu().numpy()
+    v = rr[:, 0] - R
+    want = (zeta - Z) * v / np.linalg.norm(v, axis=1, keepdims=True) ** 3
+    assert np.max(np.abs(g[:, 0] - want) / np.maximum(1, np.abs(want))) < 1e-10
+    with pytest.raises(qb.QmcError) as ei:                          # empty batch
+        s.nuclear_energy_gradient(torch.empty((1, 3, 0), dtype=torch.float64, device="cuda"), 1)
+    assert ei.value.status == qb.QMC_EINVAL
+    s.close()
+    dl, rl = wl.lih(M=8)                                            # the e-n kernel is not covered: the call says so
+    s = qb.QmcSystem(_with_en(dl, 0.3, -0.05, 0.7))
+    with pytest.raises(qb.QmcError) as ei:
+        s.nuclear_energy_gradient(_to_gpu(torch, rl), 2)
+    assert ei.value.status == qb.QMC_EUNSUPPORTED
+    s.close()
+
+
+def test_nuclear_energy_gradient_near_singular_reference(env):
+    rng = np.random.default_rng(78)
+    aos = [(1, 0, 0, 2.5), (2, 0, 0, 1.0), (3, 0, 0, 0.7), (2, 1, 0, 1.2), (2, 1, 1, 1.2), (2, 1, 2, 1.2)]
+    C = np.zeros((6, 6))
+    C[:3, :2] = rng.standard_normal((3, 2))
+    C[:, 2:] = rng.standard_normal((6, 4))
+    d = atom_system(3.0, aos, C, 2, 1, det_up=[[0, 1], [0, 2], [3, 1], [2, 4], [5, 3]], det_dn=[[0], [0], [1], [0], [2]],
+                    ci=[0.7, 0.3, -0.2, 0.25, 0.1], a_par=0.25, a_anti=0.5, b=1.0)
+    r = rng.standard_normal((160, 3, 3)) * 1.3
+    for w in range(0, 160, 3):   # the two up electrons at (nearly) the same distance: the s-only reference all but vanishes
+        u = rng.standard_normal(3)
+        r[w, 1] = u / np.linalg.norm(u) * np.linalg.norm(r[w, 0]) * (1.0 + 1e-5 * rng.uniform(0.5, 1.0))
+    check_nuclear_energy_gradient(env, d, soa(r), threads=2)
+
+
+@pytest.mark.parametrize("name,M", [("H2", 1), ("Li2", 131), ("CO", 67)])
+def test_nuclear_energy_gradient_writes_exactly_its_output(env, name, M):
+    torch, ob, qb = env
+    d, r = wl.CONFIGS[name](M=M)
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    r_before = rg.clone()
+    out = _Guarded(torch, M * d.n_atoms * 3)
+    assert qb.lib().qmc_nuclear_energy_gradient(s._h, rg.data_ptr(), M, out.ptr, torch.cuda.current_stream().cuda_stream) == 0
+    torch.cuda.synchronize()
+    out.check("qmc_nuclear_energy_gradient dE")
+    assert torch.equal(rg, r_before)
+    assert torch.equal(out.view.view(M, d.n_atoms, 3), s.nuclear_energy_gradient(rg, d.n_atoms))
+    s.close()
+
+
+def test_force_estimator_end_to_end(env):
+    """eq. 7 through the C ABI on Li2 (20 determinants, 2048 equilibrated walkers): E_L, grad_alpha E_L and
+    grad_alpha ln|Psi| from the GPU, reduced by qmc_force, against the oracle's arrays reduced by the oracle; the GPU
+    reduction applied to the oracle's own arrays; and the symmetry of the molecule: the force is along z."""
+    torch, ob, qb = env
+    d, r = wl.li2(M=2048)
+    nt = os.cpu_count() or 8
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    s.metropolis(rg, 0.3, 30, seed=5)
+    rr = rg.cpu().numpy()
+    lp, sg, el = s.local_energy(rg)
+    dE = s.nuclear_energy_gradient(rg, d.n_atoms)
+    dl = s.nuclear_log_gradient(rg, d.n_atoms)
+    F, T = qb.force(el, dE, dl)
+    o = ob.OracleSystem(d)
+    el0 = ob.local_energy(o, rr, threads=nt)[2]
+    dE0, dl0 = ob.nuclear_energy_gradient(o, rr, threads=nt), ob.nuclear_log_gradient(o, rr, threads=nt)
+    F0, T0 = ob.force(el0, dE0, dl0)
+    scale = np.abs(dE0).mean(axis=0) + 2 * (np.abs(el0 - el0.mean())[:, None, None] * np.abs(dl0)).mean(axis=0)
+    assert np.max(np.abs(F - F0) / scale) < 1e-8 and np.max(np.abs(T - T0) / scale) < 1e-8, (F, F0)
+    F1, T1 = qb.force(torch.from_numpy(el0).cuda(), torch.from_numpy(dE0).cuda(), torch.from_numpy(dl0).cuda())
+    assert np.max(np.abs(F1 - F0)) < 1e-12 * np.max(scale) and np.max(np.abs(T1 - T0)) < 1e-12 * np.max(scale)
+    s.close()
