@@ -12,8 +12,9 @@ value   = walker*E_L evaluations per second (M / device time of qmc_local_energy
 e2e     = the same metric through the C ABI call that takes HOST buffers (qmc_local_energy_host): pinned
           host walkers -> H2D -> kernels -> D2H of log|Psi|, sign, E_L, all inside the timed region (the
           call pipelines walker ranges over two streams so the copies overlap the kernels).
-roofline= model FP64 flop-equivalents of the E_L kernel / its mean launch time, against the
-          DFMA peak measured in this same process (qmc_fp64_peak).
+roofline= model FP64 flop-equivalents of the E_L kernel / its mean launch time, against the FP64 peak measured in
+          this same process: the largest of the DFMA and DMMA microbenchmarks of qmc_fp64_peak (they run on one
+          pipe); the sampler and the whole call are reported against the same denominator.
 cpu_baseline = the CPU oracle, as it stands, on the host cores, on a bounded sample.
 
 N > 1 (torchrun): walkers are sharded, M per GPU fixed (weak scaling), no data-path
@@ -130,6 +131,17 @@ def run_reference(args):
 
 
 K_DERIV = 5  # timed repetitions of the NEXT-1 block
+
+
+def profile_traffic():
+    """DRAM bytes (read + written) per launch of the dominant kernel, from the committed ncu summary."""
+    import re
+    path = os.path.join(ROOT, "profiles", "r02_el_kernel.md")
+    try:
+        m = re.search(r"dram_bytes_per_launch:\s*(\d+)", open(path).read())
+        return int(m.group(1)) if m else None
+    except OSError:
+        return None
 E2E_CHUNKS = 4  # walker ranges pipelined by qmc_local_energy_host (measured: 1, 2, 4, 8, 16 ranges -> 91, 116, 126, 119, 105 M walker*E_L/s)
 
 
@@ -172,6 +184,10 @@ def main():
 
     peak_dfma = qb.fp64_peak(0, reps=5, device=local_rank)
     peak_dmma = qb.fp64_peak(1, reps=5, device=local_rank)
+    peak_dfma2 = qb.fp64_peak(3, reps=5, device=local_rank)   # two-register operand form
+    peak_dfma3 = qb.fp64_peak(4, reps=5, device=local_rank)   # three distinct registers
+    rate_chain = qb.fp64_peak(5, reps=5, device=local_rank)   # one dependent chain per SM sub-partition (latency)
+    peak = max(peak_dfma, peak_dmma, peak_dfma2)              # DFMA and DMMA share the FP64 pipe: its demonstrated rate
 
     r0 = torch.from_numpy(r_host).to(dev)
     r = r0.clone()
@@ -283,7 +299,21 @@ def main():
         torch.cuda.synchronize()
         if k >= 3:
             t_n += a.elapsed_time(b) * 1e-3
-    del dC, dz, dR, r_orb
+    # nuclear energy gradient (first term of eq. 7, explicit route) and the force estimator on the same walkers
+    t_f = t_fr = 0.0
+    lp_o, sg_o, el_o = sysh.local_energy(r_orb)
+    for k in range(3 + K_DERIV):
+        a, b, c = ev(), ev(), ev()
+        a.record(st)
+        dE = sysh.nuclear_energy_gradient(r_orb, d.n_atoms)
+        b.record(st)
+        F, Fterms = qb.force(el_o, dE, dR)
+        c.record(st)
+        torch.cuda.synchronize()
+        if k >= 3:
+            t_f += a.elapsed_time(b) * 1e-3
+            t_fr += b.elapsed_time(c) * 1e-3
+    del dC, dz, dR, dE, r_orb
 
     t_met, t_el, t_all, t_e2e, t_kmain, t_kfb = max_over_ranks([t_met, t_el, t_all, t_e2e, t_kmain, t_kfb], device=dev)
 
@@ -314,20 +344,29 @@ def main():
                        "l2": "flushed between steps (256 MB write, outside the event-timed regions)",
                        "timing": "CUDA events on torch's current stream around each call; sums over the K steps; max over ranks"},
             "metropolis": {"value": met_rate, "unit": "walker-steps/s", "ms_per_call": 1e3 * t_met / K,
-                           "model_tflops": achieved_met, "frac_of_dfma_peak": achieved_met / peak_dfma},
+                           "model_tflops": achieved_met, "frac": achieved_met / peak,
+                           "frac_of_dfma_peak": achieved_met / peak_dfma,
+                           "model_flop_eq_per_walker_step": flops_st},
             "local_energy_ms": 1e3 * t_el / K,
-            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_dfma, "unit": "TFLOP/s",
-                         "frac": achieved / peak_dfma,
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                         "frac": achieved / peak,
                          "kernel_ms": 1e3 * t_kmain / K, "fallback_kernel_ms": 1e3 * t_kfb / K,
-                         "achieved_call": achieved_call, "frac_call": achieved_call / peak_dfma,
+                         "achieved_call": achieved_call, "frac_call": achieved_call / peak,
+                         "achieved_sampler": achieved_met, "frac_sampler": achieved_met / peak,
+                         "frac_of_dfma_microbenchmark": achieved / peak_dfma,
                          "timing": "kernel_ms: CUDA events recorded inside qmc_local_energy on the launching stream before and "
                                    "after the table-path kernel (qmc_set_kernel_timing), mean over a replay of the K steps "
                                    "(flush, sampler, E_L, statistics) right after the timed ones; *_call: events around the "
                                    "whole call in the K timed steps, which also runs the explicit fallback kernel",
-                         "traffic": 44129280,  # dram bytes read+written per launch, profiles/r01_el_kernel.md
+                         "traffic": profile_traffic(),
                          "kernel": "local_energy_kernel<7,14,true>",
-                         "peak_source": "qmc_fp64_peak DFMA microbenchmark in this process (no FP64 entry in MEASURED_PEAKS.json)",
-                         "dmma_peak": peak_dmma, "model_flop_eq_per_walker": flops_el,
+                         "peak_source": "max of the qmc_fp64_peak DFMA (8 chains), DFMA (two-register form) and DMMA m8n8k4 "
+                                        "microbenchmarks measured in this process: one shared FP64 pipe (no FP64 entry in "
+                                        "MEASURED_PEAKS.json)",
+                         "dfma_peak": peak_dfma, "dfma_two_register_peak": peak_dfma2, "dfma_three_register_rate": peak_dfma3,
+                         "dmma_peak": peak_dmma,
+                         "dfma_dependent_latency_cycles": 64.0 * 4 * 148 * (clocks.get("sm_mhz") or 1965.0) * 1e6 / (rate_chain * 1e12),
+                         "model_flop_eq_per_walker": flops_el,
                          # 148 SMs x 64 FP64 FMA/clk x 2 x the SM clock seen during the run
                          "peak_nominal": 148 * 64 * 2 * (clocks.get("sm_mhz") or 1965.0) * 1e-6,
                          "frac_of_nominal": achieved / (148 * 64 * 2 * (clocks.get("sm_mhz") or 1965.0) * 1e-6)},
@@ -345,6 +384,12 @@ def main():
             "nuclear_log_gradient": {"walkers": int(M_orb), "outputs_per_walker": int(3 * d.n_atoms),
                                      "ms": 1e3 * t_n / K_DERIV,
                                      "note": "SURVEY 8(f) NEXT-4, first half: grad_alpha ln|Psi| of eq. 7 per walker"},
+            "nuclear_energy_gradient": {"walkers": int(M_orb), "outputs_per_walker": int(3 * d.n_atoms),
+                                        "ms": 1e3 * t_f / K_DERIV, "ms_force_reduction": 1e3 * t_fr / K_DERIV,
+                                        "F_z": [float(F[a_, 2]) for a_ in range(d.n_atoms)],
+                                        "note": "SURVEY 8(f) NEXT-4: grad_alpha E_L per walker (explicit route: every determinant "
+                                                "eliminated on its own) and the estimator of eq. 7; the walkers are not "
+                                                "equilibrated here, so F is a throughput figure, not a physical force"},
             "gpu_launches": int(launches),
             "clocks": clocks,
             "last_step": {"mean_E_L": mean, "stderr": err},

@@ -253,9 +253,12 @@ int qmc_energy_gradient(const double *d_eloc, const double *d_O, int64_t M, int3
 
 /* Measured FP64 throughput of the current device, the roofline denominator of this
  * path (BASELINE.json north_star: "the chip's FP64 peak, measured by a DFMA
- * microbenchmark in the same run").  kind 0: dependent-chain DFMA kernel, 1: DMMA
- * m8n8k4 kernel, 2: both interleaved in one kernel.  h_tflops host out: best of
- * `reps` launches, counting 2 flops per FMA.  Synchronous. */
+ * microbenchmark in the same run").  kind 0: DFMA kernel, 8 independent chains a = fma(a, x, y) per thread; 1: DMMA
+ * m8n8k4 kernel; 2: both interleaved in one kernel; probes of the operand forms and of the latency that
+ * DESIGN.md section 6 quotes: 3: a = fma(a, x, a), two distinct registers per instruction, 16 chains;
+ * 4: a = fma(b, c, a), three distinct registers; 5: ONE dependent chain with one warp per SM sub-partition (the
+ * DFMA latency in cycles is 64 n_warps f_clk / rate).  h_tflops host out: best of `reps` launches, counting 2 flops
+ * per FMA.  The roofline denominator bench.py uses is the largest of kinds 0, 1 and 3.  Synchronous. */
 int qmc_fp64_peak(int device, int kind, int reps, double *h_tflops);
 
 /* Model FP64 work per walker of this system for one E_L evaluation (which = 0) or one

@@ -1174,7 +1174,7 @@ int qmc_batch_stats(const double *d_x, int64_t M, double *h_mean, double *h_stde
 }
 
 int qmc_fp64_peak(int device, int kind, int reps, double *h_tflops) {
-  if (!h_tflops || kind < 0 || kind > 2 || reps < 1) return QMC_EINVAL;
+  if (!h_tflops || kind < 0 || kind > 5 || reps < 1) return QMC_EINVAL;
   CK(cudaSetDevice(device));
   int n_sm = 0;
   CK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device));
@@ -1183,20 +1183,24 @@ int qmc_fp64_peak(int device, int kind, int reps, double *h_tflops) {
   cudaEvent_t e0, e1;
   CK(cudaEventCreate(&e0));
   CK(cudaEventCreate(&e1));
-  const int iters = 4096, blocks = n_sm * 8, threads = 256;
+  const int iters = 4096, threads = (kind == 5) ? 128 : 256;  // kind 5: one warp per SM sub-partition
+  const int blocks = (kind == 5) ? n_sm : n_sm * 8;
   double best = 0.0;
   for (int r = 0; r < reps + 1; ++r) {
     CK(cudaEventRecord(e0, 0));
     if (kind == 0) fp64_peak_kernel<0><<<blocks, threads>>>(d_out, iters, 1.0);
     if (kind == 1) fp64_peak_kernel<1><<<blocks, threads>>>(d_out, iters, 1.0);
     if (kind == 2) fp64_peak_kernel<2><<<blocks, threads>>>(d_out, iters, 1.0);
+    if (kind == 3) fp64_probe_kernel<3><<<blocks, threads>>>(d_out, iters, 1.0);
+    if (kind == 4) fp64_probe_kernel<4><<<blocks, threads>>>(d_out, iters, 1.0);
+    if (kind == 5) fp64_probe_kernel<5><<<blocks, threads>>>(d_out, iters, 1.0);
     ++g_launches;
     CK(cudaEventRecord(e1, 0));
     CK(cudaEventSynchronize(e1));
     float ms = 0;
     CK(cudaEventElapsedTime(&ms, e0, e1));
     double flops_thread = 0;
-    if (kind == 0 || kind == 2) flops_thread += (double)iters * 32 * 2;
+    if (kind == 0 || kind == 2 || kind >= 3) flops_thread += (double)iters * 32 * 2;
     if (kind == 1 || kind == 2) flops_thread += (double)iters * 4 * 512 / 32;
     const double tf = flops_thread * blocks * threads / (ms * 1e-3) / 1e12;
     if (r > 0 && tf > best) best = tf;  // first launch is warm-up

@@ -997,4 +997,47 @@ __global__ void __launch_bounds__(256) fp64_peak_kernel(double *out, int iters, 
   if (s == 123.456) out[0] = s;  // keep the work alive
 }
 
+// Operand-form and latency probes of the FP64 pipe (what DESIGN.md section 6 quotes), 32 DFMA per thread and iteration:
+//   KIND 3: a = fma(a, x, a)         two distinct registers per instruction, 16 independent chains
+//   KIND 4: a = fma(b, c, a)         three distinct registers per instruction, 8 independent chains
+//   KIND 5: a = fma(a, x, y)         ONE dependent chain (launched with one warp per SM sub-partition): latency
+template <int KIND>
+__global__ void __launch_bounds__(256) fp64_probe_kernel(double *out, int iters, double seed) {
+  double s = 0.0;
+  const double x = 1.0 + seed * 1e-9, y = seed * 1e-7;
+  if (KIND == 3) {
+    double a[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) a[i] = seed * 1e-3 + threadIdx.x * 1e-6 + i * 1e-4;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+      for (int r = 0; r < 2; ++r)
+#pragma unroll
+        for (int i = 0; i < 16; ++i) a[i] = fma(a[i], x, a[i]);
+    }
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += a[i];
+  } else if (KIND == 4) {
+    double a[8], b[8], c[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { a[i] = seed + i; b[i] = 1.0 + (threadIdx.x + i) * 1e-9; c[i] = 1.0 - (threadIdx.x + 2 * i) * 1e-9; }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+      for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int i = 0; i < 8; ++i) a[i] = fma(b[i], c[(i + r) & 7], a[i]);
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += a[i];
+  } else {
+    double a = seed + threadIdx.x * 1e-3;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+      for (int r = 0; r < 32; ++r) a = fma(a, x, y);
+    }
+    s = a;
+  }
+  if (s == 123.456) out[0] = s;
+}
+
 }  // namespace qmc
