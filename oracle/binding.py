@@ -46,7 +46,7 @@ class _Desc(C.Structure):
         ("n_det", C.c_int32), ("det_up", C.c_void_p), ("det_dn", C.c_void_p), ("ci_coeff", C.c_void_p),
         ("jastrow_a_par", C.c_double), ("jastrow_a_anti", C.c_double), ("jastrow_b", C.c_double),
         ("jastrow_en_w0", C.c_double), ("jastrow_en_w1", C.c_double), ("jastrow_en_w2", C.c_double),
-        ("n_een", C.c_int32), ("een_params", C.c_void_p),
+        ("n_een", C.c_int32), ("een_params", C.c_void_p), ("backflow_w", C.c_double),
     ]
 
 
@@ -86,6 +86,8 @@ def lib(extended: bool = False):
             L.oracle_nuclear_log_gradient.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int64, C.c_int64, C.c_void_p]
             L.oracle_energy_gradient.restype = None
             L.oracle_energy_gradient.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p]
+            L.oracle_backflow_coords.restype = None
+            L.oracle_backflow_coords.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
             L.oracle_ao_eval2.restype = None
             L.oracle_ao_eval2.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
             L.oracle_nuclear_energy_gradient.restype = C.c_int
@@ -122,7 +124,7 @@ class OracleSystem:
                        int(k["ci_coeff"].shape[0]), _p(k["det_up"]), _p(k["det_dn"]), _p(k["ci_coeff"]),
                        float(d.jastrow_a_par), float(d.jastrow_a_anti), float(d.jastrow_b),
                  float(getattr(d, "jastrow_en_w0", 0.0)), float(getattr(d, "jastrow_en_w1", 0.0)),
-                 float(getattr(d, "jastrow_en_w2", 0.0)), 0, None)
+                 float(getattr(d, "jastrow_en_w2", 0.0)), 0, None, float(getattr(d, "backflow_w", 0.0)))
         een = getattr(d, "jastrow_een", None)
         if een is not None and len(een):
             k["een"] = np.ascontiguousarray(een, np.float64).reshape(-1, 7)
@@ -339,3 +341,11 @@ def force(eloc, dE, dlnpsi):
     T = np.empty((2, na, 3))
     lib().oracle_force(_p(e), _p(a), _p(b), e.shape[0], na, _p(F), _p(T))
     return F, T
+
+
+def backflow_coords(sysd: OracleSystem, r_aos):
+    """rt [n_e, 3] of one walker r [n_e, 3]."""
+    r = np.ascontiguousarray(r_aos, np.float64)
+    rt = np.empty_like(r)
+    sysd.L.oracle_backflow_coords(sysd.ref, _p(r), _p(rt))
+    return rt

@@ -310,6 +310,78 @@ static real jastrow_en_value(const oracle_system_desc_t *s, const real *r) {
 }
 
 /* ------------------------------------------------------------------ */
+/* Backflow transformation:                               */
+/*   rt_i = r_i + sum_{j != i} K_BF(r_ij) (r_i - r_j),  over ALL other   */
+/* electrons, with the inverse kernel K_BF(r) = w / r.     */
+/* The orbitals are evaluated at rt, the Jastrow factor at r (PAPER.md:  */
+/* 61).  With t_a(d) = K(|d|) d_a, d = r_i - r_j:                         */
+/*   d_b t_a     = K' d_a d_b / r + K delta_ab                            */
+/*   d_b d_b t_a = K'' d_b^2 d_a / r^2 + K' d_a (1/r - d_b^2/r^3)         */
+/*                 + 2 K' d_b delta_ab / r                                */
+/* and d/dx_i = +d/dd, d/dx_j = -d/dd.  Outputs (any may be NULL):       */
+/*   rt  [ne][3];  jac [ne][3][3 ne] = d rt_i^a / d x_l  (l = 3 m + b);   */
+/*   lap2 [ne][3][3 ne] = d^2 rt_i^a / d x_l^2.                           */
+/* ------------------------------------------------------------------ */
+static void backflow_kernel(real w, real r, real *K, real *K1, real *K2) {
+  *K = w / r;
+  *K1 = -w / (r * r);
+  *K2 = 2.0 * w / (r * r * r);
+}
+
+static void backflow_map(const oracle_system_desc_t *s, const real *r, real *rt, real *jac, real *lap2) {
+  int ne = s->n_up + s->n_dn, nc = 3 * ne;
+  real w = s->backflow_w;
+  if (jac)
+    for (int q = 0; q < ne * 3 * nc; ++q) jac[q] = 0.0;
+  if (lap2)
+    for (int q = 0; q < ne * 3 * nc; ++q) lap2[q] = 0.0;
+  for (int i = 0; i < ne; ++i) {
+    for (int a = 0; a < 3; ++a) {
+      rt[3 * i + a] = r[3 * i + a];
+      if (jac) jac[(3 * i + a) * nc + 3 * i + a] = 1.0;
+    }
+    for (int j = 0; j < ne; ++j) {
+      if (j == i) continue;
+      real d[3];
+      for (int a = 0; a < 3; ++a) d[a] = r[3 * i + a] - r[3 * j + a];
+      real rij = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+      real K, K1, K2;
+      backflow_kernel(w, rij, &K, &K1, &K2);
+      for (int a = 0; a < 3; ++a) {
+        rt[3 * i + a] += K * d[a];
+        for (int b = 0; b < 3; ++b) {
+          real dl = (a == b) ? 1.0 : 0.0;
+          real t1 = K1 * d[a] * d[b] / rij + K * dl;
+          real t2 = K2 * d[b] * d[b] * d[a] / (rij * rij) + K1 * d[a] * (1.0 / rij - d[b] * d[b] / (rij * rij * rij)) +
+                    2.0 * K1 * d[b] * dl / rij;
+          if (jac) {
+            jac[(3 * i + a) * nc + 3 * i + b] += t1;
+            jac[(3 * i + a) * nc + 3 * j + b] -= t1;
+          }
+          if (lap2) {
+            lap2[(3 * i + a) * nc + 3 * i + b] += t2;
+            lap2[(3 * i + a) * nc + 3 * j + b] += t2;
+          }
+        }
+      }
+    }
+  }
+}
+
+void oracle_backflow_coords(const oracle_system_desc_t *s, const double *r_in, double *rt_out) {
+  int ne = s->n_up + s->n_dn;
+  real *r = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1)), *rt = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
+  for (int q = 0; q < 3 * ne; ++q) r[q] = r_in[q];
+  backflow_map(s, r, rt, NULL, NULL);
+  for (int q = 0; q < 3 * ne; ++q) rt_out[q] = (double)rt[q];
+  free(r); free(rt);
+}
+
+static void ao_eval2_r(const oracle_system_desc_t *s, int ao, const real *xyz, real *out14);
+static void local_energy_backflow_one(const oracle_system_desc_t *s, const real *r, real *logpsi, real *sign, real *eloc,
+                                      real *parts);
+
+/* ------------------------------------------------------------------ */
 /* AO -> MO: phi_alpha = sum_beta C[beta][alpha] ao_beta  */
 /* mo[i][alpha][q], q = value, d/dx, d/dy, d/dz, laplacian              */
 /* ------------------------------------------------------------------ */
@@ -334,7 +406,14 @@ double oracle_psi_plain(const oracle_system_desc_t *s, const double *r_in) {
   real *mo = (real *)malloc(sizeof(real) * (size_t)(ne * nmo * 5 + 1));
   real *gJ = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
   real *A = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
-  mo_all(s, r, mo);
+  if (s->backflow_w != 0.0) { /* orbitals at the backflow coordinates, Jastrow at the electrons' own */
+    real *rt = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
+    backflow_map(s, r, rt, NULL, NULL);
+    mo_all(s, rt, mo);
+    free(rt);
+  } else {
+    mo_all(s, r, mo);
+  }
   real J, lapJ;
   jastrow_all(s, r, &J, gJ, &lapJ);
   real sigma = 0.0;
@@ -369,6 +448,10 @@ static void local_energy_one(const oracle_system_desc_t *s, const real *r, real 
   real *Ai = A + ne * ne;          /* ne*ne */
   real *gdet = Ai + ne * ne;       /* 3 ne: grad_i D / D of the current determinant */
 
+  if (s->backflow_w != 0.0) { /* every row of A depends on every electron: the general formulas (F.4 cross term, F.5) */
+    local_energy_backflow_one(s, r, logpsi, sign, eloc, parts);
+    return;
+  }
   mo_all(s, r, mo);
   real J, lapJ;
   jastrow_all(s, r, &J, gJ, &lapJ);
@@ -530,10 +613,14 @@ static void logpsi_one(const oracle_system_desc_t *s, const real *r, real *work,
   real *mo = work;              /* ne*nmo (values only) */
   real *A = mo + ne * nmo * 5;  /* ne*ne, same offsets as local_energy_one's layout */
   real ao[5];
+  real *rt = A + ne * ne;        /* 3 ne: orbital arguments (the backflow coordinates, or r itself) */
+  if (s->backflow_w != 0.0) backflow_map(s, r, rt, NULL, NULL);
+  else
+    for (int q = 0; q < 3 * ne; ++q) rt[q] = r[q];
   for (int i = 0; i < ne * nmo; ++i) mo[i] = 0.0;
   for (int i = 0; i < ne; ++i)
     for (int beta = 0; beta < s->n_ao; ++beta) {
-      ao_eval_r(s, beta, r + 3 * i, ao);
+      ao_eval_r(s, beta, rt + 3 * i, ao);
       for (int alpha = 0; alpha < nmo; ++alpha) mo[i * nmo + alpha] += s->mo_coeff[beta * nmo + alpha] * ao[0];
     }
   real J = 0.0;
@@ -644,6 +731,7 @@ void oracle_batch_stats(const double *x, int64_t M, double *mean, double *stderr
 
 int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                            int64_t w1, double *O) {
+  if (s->backflow_w != 0.0) return -2; /* parameter / nuclear derivatives are not derived for backflow wavefunctions */
   int ne = s->n_up + s->n_dn, nmo = s->n_mo, nj = 6 + 7 * s->n_een, np = nj + s->n_det;
   real *mo = (real *)malloc(sizeof(real) * (size_t)(ne * nmo + 1));
   real *A = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
@@ -774,6 +862,7 @@ void oracle_energy_gradient(const double *eloc, const double *O, int64_t M, int3
 
 int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                                int64_t w1, double *dC, double *dzeta) {
+  if (s->backflow_w != 0.0) return -2; /* parameter / nuclear derivatives are not derived for backflow wavefunctions */
   int ne = s->n_up + s->n_dn, nmo = s->n_mo, nao = s->n_ao;
   real *aov = (real *)malloc(sizeof(real) * (size_t)(ne * nao + 1));      /* ao_beta(r_i) */
   real *aoz = (real *)malloc(sizeof(real) * (size_t)(ne * nao + 1));      /* d ao_beta / d zeta (r_i) */
@@ -861,6 +950,7 @@ int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, i
 
 int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                                 int64_t w1, double *dR) {
+  if (s->backflow_w != 0.0) return -2; /* parameter / nuclear derivatives are not derived for backflow wavefunctions */
   int ne = s->n_up + s->n_dn, nmo = s->n_mo, nao = s->n_ao, na = s->n_atoms;
   real *aov = (real *)malloc(sizeof(real) * (size_t)(ne * nao + 1));       /* ao_beta(r_i) */
   real *aog = (real *)malloc(sizeof(real) * (size_t)(3 * ne * nao + 1));   /* grad ao_beta(r_i) */
@@ -1060,7 +1150,7 @@ void oracle_ao_eval2(const oracle_system_desc_t *s, int ao, const double *xyz, d
 
 int oracle_nuclear_energy_gradient(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                                    int64_t w1, double *dE) {
-  if (s->jastrow_en_w0 != 0.0 || s->jastrow_en_w1 != 0.0 || s->n_een > 0) return -2;
+  if (s->jastrow_en_w0 != 0.0 || s->jastrow_en_w1 != 0.0 || s->n_een > 0 || s->backflow_w != 0.0) return -2;
   int ne = s->n_up + s->n_dn, nmo = s->n_mo, nao = s->n_ao, na = s->n_atoms, nj = 3 * na;
   size_t nem = (size_t)ne * (size_t)nmo;
   real *mo = (real *)malloc(sizeof(real) * (nem * 5 + 1));                 /* [i][a]{val, gx, gy, gz, lap} */
@@ -1237,4 +1327,134 @@ void oracle_force(const double *eloc, const double *dE, const double *dlnpsi, in
     F[j] = a + b;
     if (terms) { terms[j] = a; terms[3 * n_atoms + j] = b; }
   }
+}
+
+
+/* ------------------------------------------------------------------ */
+/* Local energy of a backflow-transformed wavefunction (PAPER.md:53;    */
+/* F.1, F.2, F.4 with its cross term, F.3, F.5).       */
+/* The plain definition, coordinate by coordinate: for each of the 3 N_e */
+/* electron coordinates x_l the dense derivative matrices                */
+/*   (d_l A)[i][k]   = sum_a d_a phi_k(rt_i) J[i][a][l]                   */
+/*   (d_l^2 A)[i][k] = sum_aa' H_aa' phi_k(rt_i) J[i][a][l] J[i][a'][l]   */
+/*                     + sum_a d_a phi_k(rt_i) d^2 rt_i^a / d x_l^2        */
+/* (J = Jacobian of the backflow map) and for every determinant and spin */
+/*   d_l D / D     = Tr(A^-1 d_l A)                                (F.3)  */
+/*   d_l^2 D / D   = Tr(A^-1 d_l^2 A) + Tr(A^-1 d_l A)^2                  */
+/*                   - Tr(A^-1 d_l A A^-1 d_l A)                   (F.5)  */
+/*   grad Sigma    = sum_n w_n (grad D^up/D^up + grad D^dn/D^dn)   (F.2)  */
+/*   lap Sigma     = sum_n w_n (lap D^up/D^up + 2 grad D^up/D^up . grad   */
+/*                   D^dn/D^dn + lap D^dn/D^dn)                    (F.4)  */
+/* then F.1 and eq. 1 as in local_energy_one.                            */
+/* ------------------------------------------------------------------ */
+static void local_energy_backflow_one(const oracle_system_desc_t *s, const real *r, real *logpsi, real *sign, real *eloc,
+                                      real *parts) {
+  int ne = s->n_up + s->n_dn, nmo = s->n_mo, nc = 3 * ne;
+  size_t nem = (size_t)ne * (size_t)nmo;
+  real *rt = (real *)malloc(sizeof(real) * (size_t)(nc + 1));
+  real *jac = (real *)malloc(sizeof(real) * (size_t)(ne * 3 * nc + 1));
+  real *lap2 = (real *)malloc(sizeof(real) * (size_t)(ne * 3 * nc + 1));
+  real *mo = (real *)malloc(sizeof(real) * (nem * 10 + 1));  /* [i][k]{val, gx, gy, gz, hxx, hyy, hzz, hxy, hyz, hzx} */
+  real *dA = (real *)malloc(sizeof(real) * ((size_t)nc * nem + 1));   /* [l][i][k] first derivative of the MO matrix */
+  real *d2A = (real *)malloc(sizeof(real) * ((size_t)nc * nem + 1));  /* [l][i][k] second */
+  real *A = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
+  real *Ai = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
+  real *G = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
+  real *gJ = (real *)malloc(sizeof(real) * (size_t)(nc + 1));
+  real *gS = (real *)malloc(sizeof(real) * (size_t)(nc + 1));
+  real *tr1 = (real *)malloc(sizeof(real) * (size_t)(2 * nc + 1));
+  backflow_map(s, r, rt, jac, lap2);
+  real ao[14];
+  for (size_t q = 0; q < nem * 10; ++q) mo[q] = 0.0;
+  for (int i = 0; i < ne; ++i)
+    for (int beta = 0; beta < s->n_ao; ++beta) {
+      ao_eval2_r(s, beta, rt + 3 * i, ao);
+      for (int k = 0; k < nmo; ++k) {
+        real cf = s->mo_coeff[beta * nmo + k];
+        real *m = mo + ((size_t)i * nmo + k) * 10;
+        m[0] += cf * ao[0];
+        for (int a = 0; a < 3; ++a) m[1 + a] += cf * ao[1 + a];
+        for (int q = 0; q < 6; ++q) m[4 + q] += cf * ao[5 + q];
+      }
+    }
+  for (int l = 0; l < nc; ++l)
+    for (int i = 0; i < ne; ++i)
+      for (int k = 0; k < nmo; ++k) {
+        const real *m = mo + ((size_t)i * nmo + k) * 10;
+        real H[3][3] = {{m[4], m[7], m[9]}, {m[7], m[5], m[8]}, {m[9], m[8], m[6]}};
+        real d1 = 0.0, d2 = 0.0;
+        for (int a = 0; a < 3; ++a) {
+          real ja = jac[(3 * i + a) * nc + l];
+          d1 += m[1 + a] * ja;
+          d2 += m[1 + a] * lap2[(3 * i + a) * nc + l];
+          for (int b = 0; b < 3; ++b) d2 += H[a][b] * ja * jac[(3 * i + b) * nc + l];
+        }
+        dA[(size_t)l * nem + (size_t)i * nmo + k] = d1;
+        d2A[(size_t)l * nem + (size_t)i * nmo + k] = d2;
+      }
+  real J, lapJ;
+  jastrow_all(s, r, &J, gJ, &lapJ);
+  real sigma = 0.0, lapS = 0.0;
+  for (int l = 0; l < nc; ++l) gS[l] = 0.0;
+  for (int n = 0; n < s->n_det; ++n) {
+    real D[2], lapD[2];
+    for (int sp = 0; sp < 2; ++sp) {
+      int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
+      const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
+      for (int i = 0; i < ns; ++i)
+        for (int k = 0; k < ns; ++k) A[i * ns + k] = mo[((size_t)(e0 + i) * nmo + lst[k]) * 10];
+      D[sp] = det_inv_r(ns, A, Ai);
+      lapD[sp] = 0.0;
+      for (int l = 0; l < nc; ++l) {
+        const real *d1 = dA + (size_t)l * nem, *d2 = d2A + (size_t)l * nem;
+        /* G = A^-1 d_l A  (orbital positions x orbital positions) */
+        real t1 = 0.0, t2 = 0.0, tl = 0.0;
+        for (int p = 0; p < ns; ++p)
+          for (int q = 0; q < ns; ++q) {
+            real v = 0.0, u = 0.0;
+            for (int i = 0; i < ns; ++i) {
+              v += Ai[p * ns + i] * d1[(size_t)(e0 + i) * nmo + lst[q]];
+              if (p == q) u += Ai[p * ns + i] * d2[(size_t)(e0 + i) * nmo + lst[q]];
+            }
+            G[p * ns + q] = v;
+            if (p == q) { t1 += v; tl += u; }
+          }
+        for (int p = 0; p < ns; ++p)
+          for (int q = 0; q < ns; ++q) t2 += G[p * ns + q] * G[q * ns + p];
+        tr1[sp * nc + l] = t1;                 /* F.3 */
+        lapD[sp] += tl + t1 * t1 - t2;         /* F.5 */
+      }
+    }
+    real wn = s->ci_coeff[n] * D[0] * D[1];
+    real cross = 0.0;
+    for (int l = 0; l < nc; ++l) cross += tr1[l] * tr1[nc + l];
+    sigma += wn;
+    for (int l = 0; l < nc; ++l) gS[l] += wn * (tr1[l] + tr1[nc + l]);   /* F.2 */
+    lapS += wn * (lapD[0] + 2.0 * cross + lapD[1]);                      /* F.4 */
+  }
+  real gJ2 = 0.0, crossJ = 0.0;
+  for (int l = 0; l < nc; ++l) { gJ2 += gJ[l] * gJ[l]; crossJ += gJ[l] * gS[l]; }
+  real kinetic = -0.5 * (lapJ + gJ2 + 2.0 * crossJ / sigma + lapS / sigma);   /* F.1 */
+  real vee = 0.0, ven = 0.0, vnn = 0.0;
+  for (int i = 0; i < ne; ++i)
+    for (int j = i + 1; j < ne; ++j) {
+      real dx = r[3 * i] - r[3 * j], dy = r[3 * i + 1] - r[3 * j + 1], dz = r[3 * i + 2] - r[3 * j + 2];
+      vee += 1.0 / sqrt(dx * dx + dy * dy + dz * dz);
+    }
+  for (int i = 0; i < ne; ++i)
+    for (int a = 0; a < s->n_atoms; ++a) {
+      real dx = r[3 * i] - s->atom_xyz[3 * a], dy = r[3 * i + 1] - s->atom_xyz[3 * a + 1], dz = r[3 * i + 2] - s->atom_xyz[3 * a + 2];
+      ven -= s->atom_Z[a] / sqrt(dx * dx + dy * dy + dz * dz);
+    }
+  for (int a = 0; a < s->n_atoms; ++a)
+    for (int b = a + 1; b < s->n_atoms; ++b) {
+      real dx = s->atom_xyz[3 * a] - s->atom_xyz[3 * b], dy = s->atom_xyz[3 * a + 1] - s->atom_xyz[3 * b + 1],
+           dz = s->atom_xyz[3 * a + 2] - s->atom_xyz[3 * b + 2];
+      vnn += s->atom_Z[a] * s->atom_Z[b] / sqrt(dx * dx + dy * dy + dz * dz);
+    }
+  *logpsi = J + log(fabs(sigma));
+  *sign = (sigma > 0.0) ? 1.0 : ((sigma < 0.0) ? -1.0 : 0.0);
+  *eloc = kinetic + vee + ven + vnn;
+  if (parts) { parts[0] = kinetic; parts[1] = vee; parts[2] = ven; parts[3] = vnn; }
+  free(rt); free(jac); free(lap2); free(mo); free(dA); free(d2A); free(A); free(Ai); free(G); free(gJ); free(gS); free(tr1);
 }

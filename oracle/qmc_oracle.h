@@ -53,6 +53,9 @@ typedef struct {
    * two factors coincide, exchange-symmetric when they do not); n_een = 0 = absent */
   int32_t n_een;
   const double *een_params; /* [n_een][7] or NULL */
+  /* inverse backflow: rt_i = r_i + sum_{j != i} (w / r_ij)(r_i - r_j) over all other electrons; the
+   * orbitals are evaluated at rt, the Jastrow factor at r; 0 = no backflow */
+  double backflow_w;
 } oracle_system_desc_t;
 
 /* All pointers are HOST pointers.  Walker arrays are SoA [n_e][3][M]; the
@@ -73,7 +76,8 @@ double oracle_det_inv(int n, const double *A, double *inv);
  * for ONE walker given as AoS r[n_e][3].  Used for finite differences. */
 double oracle_psi_plain(const oracle_system_desc_t *s, const double *r);
 
-/* log|Psi|, sign, E_L = H Psi / Psi (eq. 1; F.1-F.4, G.7).
+/* log|Psi|, sign, E_L = H Psi / Psi (eq. 1; F.1-F.4, G.7; with backflow_w != 0 the general formulas:
+ * F.4 with its cross term and F.5, coordinate by coordinate on every determinant).
  * parts, if non-NULL, receives [M][4] = {kinetic, V_ee, V_en, V_nn}. */
 int oracle_local_energy(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                         int64_t w1, double *logpsi, double *sign, double *eloc, double *parts);
@@ -128,6 +132,9 @@ int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, i
  * the Jastrow kernels D.2 and D.3.  Rows w0 <= w < w1. */
 int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                                 int64_t w1, double *dR);
+
+/* The backflow coordinates of ONE walker: r, rt AoS [n_e][3]. */
+void oracle_backflow_coords(const oracle_system_desc_t *s, const double *r, double *rt);
 
 /* One AO at one point with its second-level derivatives: out14 = {phi, grad[3], lap, Hessian xx yy zz xy yz zx,
  * grad lap [3]}.  PAPER.md:55; needed because d ao / d R = -grad_r ao. */

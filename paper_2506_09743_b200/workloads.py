@@ -51,6 +51,7 @@ class SystemDesc:
     jastrow_en_w1: float = 0.0
     jastrow_en_w2: float = 0.0
     jastrow_een: np.ndarray | None = None  # electron-electron-nucleus kernel (D.3): [n_terms, 7] = (c, a1, b1, a2, b2, a3, b3)
+    backflow_w: float = 0.0  # inverse backflow kernel K_BF(r) = w / r; 0 = none
     extra: dict = field(default_factory=dict)
 
     @property

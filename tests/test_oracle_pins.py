@@ -1148,3 +1148,78 @@ def test_force_estimator_formula_and_physical_pin():
     assert np.max(np.abs(F[:, :2])) < 4 * np.max(sig[:, :2]) + 1e-12           # no force off the axis
     assert abs(T[1, 1, 2]) < 1e-12                                             # Psi does not depend on R_B
     assert abs(T[1, 0, 2] - q / R ** 2) < 0.15 * q / R ** 2                    # second term: +q/R^2 to leading order
+
+
+# ---------------------------------------------------------------- inverse backflow (F.4 cross term, F.5)
+def _with_bf(d, w):
+    import copy
+    d2 = copy.copy(d)
+    d2.backflow_w = w
+    return d2
+
+
+def test_backflow_map_is_a_push_of_w_along_every_unit_vector():
+    # K_BF(r) = w / r  =>  rt_i = r_i + w sum_{j != i} (r_i - r_j)/|r_i - r_j|, over ALL other electrons (both spins)
+    d, r = wl.li2(M=5)
+    o = ob.OracleSystem(_with_bf(d, 0.17))
+    for w in range(5):
+        rr = r[:, :, w]
+        rt = ob.backflow_coords(o, rr)
+        want = rr.copy()
+        for i in range(6):
+            for j in range(6):
+                if j != i:
+                    want[i] += 0.17 * (rr[i] - rr[j]) / np.linalg.norm(rr[i] - rr[j])
+        assert np.max(np.abs(rt - want)) < 1e-14
+    # a single electron has no partner: the hydrogen atom stays exact
+    da = _with_bf(atom_system(1, [(1, 0, 0, 1.0)], [[1.0]], 1, 0), 0.3)
+    el = ob.local_energy(ob.OracleSystem(da), soa(_rand_pos(50, 1, 2.0, seed=3)))[2]
+    assert np.max(np.abs(el - GOLDEN["E_n1"])) < 1e-12
+
+
+@pytest.mark.parametrize("name,M,w", [("H2", 4, 0.2), ("LiH", 4, 0.12), ("Li2", 3, 0.08), ("CO", 2, 0.05)])
+def test_backflow_local_energy_vs_finite_differences_of_the_plain_psi(name, M, w):
+    # the whole general chain (Jacobian and second derivatives of the map, AO Hessians, F.3, F.5, the cross term of
+    # F.4, F.1) against Richardson central differences of the plain definition e^J sum_n d_n det det evaluated at the
+    # backflow coordinates (oracle_psi_plain): a dropped cross term or a wrong sign in F.5 is O(w), far above the bound
+    d, r = wl.CONFIGS[name](M=64)
+    d = _with_bf(d, w)
+    o = ob.OracleSystem(d)
+    lp_all = ob.local_energy(o, r)[0]
+    idx = _keep_away(d, r)
+    # also keep electrons apart: the inverse kernel is singular at coalescence
+    rr = r.transpose(2, 0, 1)
+    dmin = np.array([min(np.linalg.norm(rr[k, i] - rr[k, j]) for i in range(d.n_e) for j in range(i)) for k in range(rr.shape[0])])
+    idx = np.array([k for k in idx if dmin[k] > 0.4])
+    idx = idx[np.argsort(-lp_all[idx])][:M]
+    _fd_check(d, np.ascontiguousarray(r[:, :, idx]), nwalk=len(idx), tol=3e-6)
+
+
+def test_backflow_limit_antisymmetry_and_sampler_value():
+    d, r = wl.li2(M=24)
+    o0 = ob.OracleSystem(d)
+    lp0, sg0, el0 = ob.local_energy(o0, r)
+    # w -> 0: the general formulas (every coordinate's dense d_l A, F.5 with both extra traces, F.4's cross term) must
+    # collapse onto the single-electron-orbital result G.7 (Appendix G)
+    lp1, sg1, el1 = ob.local_energy(ob.OracleSystem(_with_bf(d, 1e-200)), r)
+    assert np.array_equal(sg1, sg0) and np.max(np.abs(lp1 - lp0)) < 1e-12
+    keep = lp0 - lp0.max() > math.log(1e-6)
+    assert np.max((np.abs(el1 - el0) / np.maximum(1, np.abs(el0)))[keep]) < 1e-9
+    # a finite w changes the energy, is antisymmetric under same-spin exchange (the map treats all
+    # electrons alike), and the sampler's value-only route agrees with the E_L route
+    db = _with_bf(d, 0.1)
+    ob_ = ob.OracleSystem(db)
+    lp, sg, el = ob.local_energy(ob_, r)
+    assert np.max(np.abs(el - el0)) > 1e-3
+    rx = r.copy()
+    rx[[0, 2]] = rx[[2, 0]]
+    lpx, sgx, elx = ob.local_energy(ob_, rx)
+    assert np.array_equal(sgx, -sg) and np.max(np.abs(lpx - lp)) < 1e-11
+    assert np.max((np.abs(elx - el) / np.maximum(1, np.abs(el)))[keep]) < 1e-9
+    out = ob.metropolis(ob_, r, 0.2, 0, seed=1)
+    assert np.max(np.abs(out["logpsi"] - lp)) < 1e-12
+    # parameter and nuclear derivatives are not derived for backflow wavefunctions: the calls say so
+    L = ob.lib()
+    buf = np.zeros((24, 64))
+    assert L.oracle_log_derivatives(ob_.ref, r.ctypes.data, 24, 0, 24, buf.ctypes.data) == -2
+    assert L.oracle_nuclear_energy_gradient(ob_.ref, r.ctypes.data, 24, 0, 24, buf.ctypes.data) == -2
