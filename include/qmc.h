@@ -95,6 +95,14 @@ typedef struct {
    * the exchange symmetry of PAPER.md:51, the symmetrised pair does not (reading Q22).  n_een = 0: absent. */
   int32_t n_een;
   const double *een_params;
+  /* Inverse backflow transformation (PAPER.md:53 with the kernel of PAPER.md:97):
+   *   rt_i = r_i + sum_{j != i} K_BF(r_ij) (r_i - r_j),  K_BF(r) = backflow_w / r,  over all other electrons.
+   * The orbitals are evaluated at rt, the Jastrow factor at r.  0 = no backflow.  With backflow on, qmc_local_energy
+   * (and the E_L of qmc_metropolis' d_eloc_acc) evaluates the general formulas F.4 / F.5 with
+   * every determinant eliminated on its own; qmc_log_psi and qmc_metropolis keep the excitation tables (values only);
+   * the derivative calls (qmc_log_derivatives, qmc_orbital_derivatives, qmc_nuclear_*) return QMC_EUNSUPPORTED, and so
+   * does qmc_setup when backflow is combined with the D.2 / D.3 Jastrow kernels. */
+  double backflow_w;
 } qmc_system_desc_t;
 
 /* Validate `desc`, preprocess it (shell grouping, excitation tables relative to

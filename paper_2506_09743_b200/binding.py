@@ -36,7 +36,7 @@ class _Desc(C.Structure):
         ("n_det", C.c_int32), ("det_up", C.c_void_p), ("det_dn", C.c_void_p), ("ci_coeff", C.c_void_p),
         ("jastrow_a_par", C.c_double), ("jastrow_a_anti", C.c_double), ("jastrow_b", C.c_double),
         ("jastrow_en_w0", C.c_double), ("jastrow_en_w1", C.c_double), ("jastrow_en_w2", C.c_double),
-        ("n_een", C.c_int32), ("een_params", C.c_void_p),
+        ("n_een", C.c_int32), ("een_params", C.c_void_p), ("backflow_w", C.c_double),
     ]
 
 
@@ -129,7 +129,7 @@ def make_desc(d):
                  int(k["ci_coeff"].shape[0]), _np(k["det_up"]), _np(k["det_dn"]), _np(k["ci_coeff"]),
                  float(d.jastrow_a_par), float(d.jastrow_a_anti), float(d.jastrow_b),
                  float(getattr(d, "jastrow_en_w0", 0.0)), float(getattr(d, "jastrow_en_w1", 0.0)),
-                 float(getattr(d, "jastrow_en_w2", 0.0)), 0, None)
+                 float(getattr(d, "jastrow_en_w2", 0.0)), 0, None, float(getattr(d, "backflow_w", 0.0)))
     een = getattr(d, "jastrow_een", None)
     if een is not None and len(een):
         k["een"] = np.ascontiguousarray(een, np.float64).reshape(-1, 7)

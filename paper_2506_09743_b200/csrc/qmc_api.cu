@@ -45,6 +45,8 @@ struct Variant {
   const void *k_nuc, *k_nuc_small;  // the same kernel in nuclear mode (qmc_nuclear_log_gradient)
   int orb_ws_doubles;
   const void *k_frc, *k_frc_small;  // nuclear energy gradient (8 / 4 warps per block)
+  const void *b_psi, *b_metro, *b_el;  // backflow: values-only kernels, and the E_L kernel (explicit route)
+  int bf_ws_doubles;
   int frc_ws_doubles;
 };
 
@@ -71,6 +73,10 @@ Variant make_variant() {
   v.k_frc = (const void *)nuclear_energy_gradient_kernel<NS, NMO, X, 8>;
   v.k_frc_small = (const void *)nuclear_energy_gradient_kernel<NS, NMO, X, 4>;
   v.frc_ws_doubles = Geo<NS, NMO>::total + Geo<NS, NMO>::frcExtra;
+  v.b_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi, false, false, true>;
+  v.b_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi, false, true>;
+  v.b_el = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBf>;
+  v.bf_ws_doubles = BfGeo<NS, NMO>::total;
   v.e_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, false, true>;
   v.e_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi, false, true>;
   v.e_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi, true>;
@@ -191,6 +197,8 @@ struct qmc_system {
   std::unordered_map<cudaStream_t, Scratch> scratch;
   std::vector<void *> retired;
   // qmc_local_energy_host: two internal streams and double-buffered device scratch (grown on demand)
+  bool bf_ready = false;   // backflow E_L kernel configured (lazily)
+  int blocks_bf = 0;
   bool frc_ready = false;  // nuclear energy-gradient kernel configured (lazily)
   int frc_warps = 0, blocks_frc = 0;
   bool orb_ready = false;  // orbital-derivative kernel configured (lazily: most users never call it)
@@ -304,6 +312,15 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   P.en_w1 = d->jastrow_en_w1;
   P.en_w2 = d->jastrow_en_w2;
   P.has_en = (d->jastrow_en_w0 != 0.0 || d->jastrow_en_w1 != 0.0) ? 1 : 0;
+  P.bf_w = d->backflow_w;
+  if (!(d->backflow_w == d->backflow_w)) {  // NaN
+    delete s;
+    return QMC_EINVAL;
+  }
+  if (d->backflow_w != 0.0 && (d->n_een > 0 || P.has_en)) {  // backflow is built with the Pade e-e Jastrow only
+    delete s;
+    return QMC_EUNSUPPORTED;
+  }
   if (d->n_een < 0 || (d->n_een > 0 && !d->een_params)) {
     delete s;
     return QMC_EINVAL;
@@ -428,6 +445,10 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     return QMC_EUNSUPPORTED;
   }
   s->var = *var;
+  if (P.bf_w != 0.0) {  // the values-only instantiations that evaluate the orbitals at the backflow coordinates
+    s->var.k_psi = var->b_psi;
+    s->var.k_metro = var->b_metro;
+  }
   if (P.n_een > 0) {  // the instantiations that carry the e-e-n Jastrow kernel
     s->var.k_el = var->e_el;
     s->var.k_psi = var->e_psi;
@@ -775,6 +796,31 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
   io.eloc = d_eloc;
   io.O = d_O;
   io.M = M;
+  if (s->P.bf_w != 0.0 && el) {
+    // backflow wavefunction: E_L by its own kernel, every determinant explicit (qmc_backflow.cuh);
+    // the parameter derivatives are not derived for it
+    if (d_O) return QMC_EUNSUPPORTED;
+    const int smem = s->P.smem_const_bytes + kWarpsBf * s->var.bf_ws_doubles * (int)sizeof(double);
+    {
+      std::lock_guard<std::mutex> lock(s->scratch_mu);
+      if (!s->bf_ready) {
+        int dev_smem = 0;
+        cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, s->device);
+        if (smem > dev_smem) return QMC_EUNSUPPORTED;
+        CK(cudaFuncSetAttribute(s->var.b_el, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        int per_sm = 0;
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, s->var.b_el, kWarpsBf * 32, smem));
+        if (per_sm < 1) return QMC_EUNSUPPORTED;
+        s->blocks_bf = per_sm * s->n_sm;
+        s->bf_ready = true;
+      }
+    }
+    const int grid = (int)std::min<int64_t>((M + kWarpsBf - 1) / kWarpsBf, s->blocks_bf);
+    void *bargs[2] = {(void *)&s->P, (void *)&io};
+    CK(cudaLaunchKernel(s->var.b_el, dim3(grid), dim3(kWarpsBf * 32), bargs, smem, st));
+    ++g_launches;
+    return QMC_OK;
+  }
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
   const int wpb = el ? kWarpsEl : kWarpsPsi, smem = el ? s->smem_el : s->smem_psi;
   const int64_t need = (groups + wpb - 1) / wpb;
@@ -1074,11 +1120,13 @@ static int orbital_launch(qmc_system_t *s, const double *d_r, int64_t M, double 
 
 int qmc_orbital_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d_dC, double *d_dzeta, void *cuda_stream) {
   if (!s || !d_r || M <= 0 || (!d_dC && !d_dzeta)) return QMC_EINVAL;
+  if (s->P.bf_w != 0.0) return QMC_EUNSUPPORTED;  // not derived for backflow wavefunctions
   return orbital_launch(s, d_r, M, d_dC, d_dzeta, nullptr, cuda_stream);
 }
 
 int qmc_nuclear_log_gradient(qmc_system_t *s, const double *d_r, int64_t M, double *d_dR, void *cuda_stream) {
   if (!s || !d_r || M <= 0 || !d_dR) return QMC_EINVAL;
+  if (s->P.bf_w != 0.0) return QMC_EUNSUPPORTED;  // not derived for backflow wavefunctions
   CK(cudaSetDevice(s->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
   // Jastrow part (D.2, D.3) initialises dR, one thread per walker; the AO part is subtracted by the second launch
@@ -1090,7 +1138,7 @@ int qmc_nuclear_log_gradient(qmc_system_t *s, const double *d_r, int64_t M, doub
 
 int qmc_nuclear_energy_gradient(qmc_system_t *s, const double *d_r, int64_t M, double *d_dE, void *cuda_stream) {
   if (!s || !d_r || M <= 0 || !d_dE) return QMC_EINVAL;
-  if (s->P.has_en || s->P.n_een > 0) return QMC_EUNSUPPORTED;  // the R-dependence of D.2 / D.3 inside E_L is not derived
+  if (s->P.has_en || s->P.n_een > 0 || s->P.bf_w != 0.0) return QMC_EUNSUPPORTED;  // D.2 / D.3 / backflow inside E_L: not derived
   CK(cudaSetDevice(s->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
   auto smem_for = [&](int warps) { return s->P.smem_const_bytes + warps * s->var.frc_ws_doubles * (int)sizeof(double); };

@@ -40,6 +40,7 @@ constexpr int kMaxEen = 6;    // terms of the electron-electron-nucleus Jastrow 
                              // (12 x 16.3 KB of scratch leave ~30 KB of L1 for the term lists and the constant tables)
 #endif
 constexpr int kWarpsEl = QMC_WARPS, kWarpsPsi = QMC_WARPS_PSI, kWarpsOrb = QMC_WARPS_ORB, kWarpsOrbSmall = 8;
+constexpr int kWarpsBf = 4;  // warps (= walkers in flight) per block of the backflow E_L kernel
 constexpr int kWarpsMax = kWarpsEl > kWarpsPsi ? kWarpsEl : kWarpsPsi;
 
 // shell record kinds
@@ -166,6 +167,7 @@ struct SysParams {  // passed by value to every kernel
   int c_doubles;                   // size of the C fragment table
   int n_chunks;                    // AO chunks of kChunk rows
   double a_par, a_anti, b, vnn;
+  double bf_w;                     // inverse backflow kernel K_BF(r) = bf_w / r; 0 = none
   double en_w0, en_w1, en_w2;      // electron-nucleus Jastrow kernel (D.2); has_en = 0 when w0 = w1 = 0
   int has_en;
   int n_een;                       // electron-electron-nucleus kernel (D.3): terms (c, a1, b1, a2, b2, a3, b3)

@@ -237,7 +237,10 @@ __device__ __noinline__ void een_param_terms(const SysParams &P, const double *s
 template <bool EL, bool EXPL, int ORB>
 constexpr bool kCompact = !EL && !EXPL && ORB == 0;
 
-template <int NS, int NMO, bool EL, bool X, bool EXPL = false, bool DERIV = false, bool EEN = false, int ORB = 0>
+// BF (values only): the orbitals are evaluated at the backflow coordinates rt_i = r_i + w sum_{j != i} (r_i - r_j)/r_ij
+// (PAPER.md:53 with the inverse kernel of PAPER.md:97), the Jastrow factor at r; the determinant algebra is unchanged.
+// E_L of a backflow wavefunction has its own kernel (qmc_backflow.cuh).
+template <int NS, int NMO, bool EL, bool X, bool EXPL = false, bool DERIV = false, bool EEN = false, int ORB = 0, bool BF = false>
 __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp,
                              const double *__restrict__ sC, const DetRec *__restrict__ sDet,
                              double *__restrict__ ws, double x, double y, double z, int lane,
@@ -253,11 +256,29 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
   double *sG = ws + GE::oG, *sT = ws + GE::oT, *sProb = ws + GE::oProbC(CP);
   double *sRes = ws + GE::oResC(CP);
 
+  static_assert(!BF || (!EL && !EXPL && !DERIV && ORB == 0), "backflow: values-only evaluation here");
   // ---- publish coordinates for the pair loop
   sXYZ[lane] = x;  // [xyz][lane]: the pair loop reads consecutive lanes
   sXYZ[32 + lane] = y;
   sXYZ[64 + lane] = z;
   __syncwarp();
+  double xa = x, ya = y, za = z;  // where the lane's orbitals are evaluated
+  if (BF) {
+    const int base = (active ? g : 0) * ne;
+    double px = 0.0, py = 0.0, pz = 0.0;
+    for (int o = 1; o < ne; ++o) {
+      int j = e + o;
+      j -= (j >= ne) ? ne : 0;
+      const double dx = x - sXYZ[base + j], dy = y - sXYZ[32 + base + j], dz = z - sXYZ[64 + base + j];
+      const double ri = rsqrt_fast(fma(dx, dx, fma(dy, dy, dz * dz)));
+      px = fma(dx, ri, px);
+      py = fma(dy, ri, py);
+      pz = fma(dz, ri, pz);
+    }
+    xa = fma(P.bf_w, px, x);
+    ya = fma(P.bf_w, py, y);
+    za = fma(P.bf_w, pz, z);
+  }
 
   // ---- stage a5: Pade Jastrow (D.1) and e-e repulsion (eq. 1).
   // Every unordered pair is evaluated once: electron e takes the partners e+1 .. e+(ne-1)/2 (cyclic),
@@ -395,9 +416,9 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
         const ShellRec &sh = P.shells[s];
         const int meta = sh.meta;
         if ((meta & 15) == SH_ATOM) {  // new centre: {zeta, c1, c2, kd} = {X, Y, Z, charge}
-          dx = x - sh.zeta;
-          dy = y - sh.c1;
-          dz = z - sh.c2;
+          dx = xa - sh.zeta;
+          dy = ya - sh.c1;
+          dz = za - sh.c2;
           r2 = fma(dx, dx, fma(dy, dy, dz * dz));
           ri = rsqrt_fast(r2);
           r = r2 * ri;

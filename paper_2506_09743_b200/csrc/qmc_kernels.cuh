@@ -2,6 +2,7 @@
 // Metropolis, batch statistics.  One warp = G walkers per pass, grid-stride over groups.
 #pragma once
 #include "qmc_eval.cuh"
+#include "qmc_backflow.cuh"
 
 namespace qmc {
 
@@ -35,7 +36,7 @@ __device__ __forceinline__ void dummy_xyz(int lane, double &x, double &y, double
   z = 0.53 - 0.05 * lane;
 }
 
-template <int NS, int NMO, bool EL, bool X, int WPB, bool DERIV = false, bool EEN = false>
+template <int NS, int NMO, bool EL, bool X, int WPB, bool DERIV = false, bool EEN = false, bool BF = false>
 __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     local_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -65,7 +66,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   for (int64_t grp = (int64_t)blockIdx.x * WPB + warp; grp < n_groups; grp += stride) {
     double x, y, z;
     fetch(grp, x, y, z);
-    eval_walkers<NS, NMO, EL, X, false, DERIV, EEN>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1, DerivOut{io.O, grp * G, io.M});
+    eval_walkers<NS, NMO, EL, X, false, DERIV, EEN, 0, BF>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1, DerivOut{io.O, grp * G, io.M});
     bool flagged = false;
     if (lane < G) {
       const int64_t wo = grp * G + lane;
@@ -710,7 +711,7 @@ __global__ void __launch_bounds__(128) force_final_kernel(const double *__restri
 // Persistent all-electron Metropolis (readings Q9, Q10).
 // Walker coordinates and log|Psi| stay in registers for all sweeps.
 // ---------------------------------------------------------------------------------
-template <int NS, int NMO, bool X, int WPB, bool EEN = false>
+template <int NS, int NMO, bool X, int WPB, bool EEN = false, bool BF = false>
 __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     metropolis_kernel(const __grid_constant__ SysParams P, const WalkerIO io, const MetroParams mp) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -788,7 +789,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
         }
         logu = sLogU[own ? g : 0];
       }
-      eval_walkers<NS, NMO, false, X, false, false, EEN>(P, sExp, sC, sDet, ws, xp, yp, zp, lane);
+      eval_walkers<NS, NMO, false, X, false, false, EEN, 0, BF>(P, sExp, sC, sDet, ws, xp, yp, zp, lane);
       const double lp2 = sRes[rg + 0], sg2 = sRes[rg + 1];
       // accept iff log u < 2 (log|Psi'| - log|Psi|): false for NaN and for Psi' = 0
       const bool ok = (sw < 0) || (own && (logu < 2.0 * (lp2 - lp)));

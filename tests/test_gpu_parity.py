@@ -1263,3 +1263,99 @@ def test_force_estimator_end_to_end(env):
     F1, T1 = qb.force(torch.from_numpy(el0).cuda(), torch.from_numpy(dE0).cuda(), torch.from_numpy(dl0).cuda())
     assert np.max(np.abs(F1 - F0)) < 1e-12 * np.max(scale) and np.max(np.abs(T1 - T0)) < 1e-12 * np.max(scale)
     s.close()
+
+
+# ----------------------------------------------------------------------------- NEXT-3: inverse backflow
+def _with_bf(d, w):
+    import copy
+    d2 = copy.copy(d)
+    d2.backflow_w = w
+    return d2
+
+
+def check_backflow(env, d, r, threads=8):
+    """log|Psi| / sign from the values-only kernel and from the E_L kernel, and E_L, against the oracle's general
+    formulas (F.4 with its cross term, F.5 coordinate by coordinate), contract tolerances with adjudication Q24."""
+    torch, ob, qb = env
+    o, ox = ob.OracleSystem(d), ob.OracleSystem(d, extended=True)
+    lp0, sg0, el0 = ob.local_energy(o, r, threads=threads)
+    lpx, sgx, elx = ob.local_energy(ox, r, threads=threads)
+    s = qb.QmcSystem(d)
+    lp, sg, el = (t.cpu().numpy() for t in s.local_energy(_to_gpu(torch, r)))
+    lp2, sg2 = (t.cpu().numpy() for t in s.log_psi(_to_gpu(torch, r)))
+    el_b = s.local_energy(_to_gpu(torch, r))[2].cpu().numpy()
+    s.close()
+    assert np.array_equal(el, el_b)                               # deterministic
+    keep = (lpx - lpx.max() > math.log(1e-6)) & np.isfinite(elx)
+    assert np.array_equal(sg[keep], sg0[keep]) and np.array_equal(sg2[keep], sg0[keep])
+    n1 = adjudicate(lp, lp0, lpx, 1e-10, mask=keep, what="backflow log|Psi| (E_L kernel)")
+    n2 = adjudicate(lp2, lp0, lpx, 1e-10, mask=keep, what="backflow log|Psi| (values-only kernel)")
+    n3 = adjudicate(el, el0, elx, 1e-8, scale=np.maximum(1.0, np.abs(elx)), mask=keep, what="backflow E_L")
+    return n1, n2, n3, int(keep.sum())
+
+
+@pytest.mark.parametrize("name,M,w", [("H2", 515, 0.2), ("LiH", 300, 0.12), ("Li2", 257, 0.08), ("CO", 129, 0.05), ("CO", 3, 0.05)])
+def test_backflow_configs(env, name, M, w):
+    d, r = wl.CONFIGS[name](M=M)
+    n1, n2, n3, nk = check_backflow(env, _with_bf(d, w), r)
+    assert max(n1, n2, n3) <= max(2, nk // 20), (n1, n2, n3, nk)
+
+
+def test_backflow_odd_systems_500_determinants_and_the_zero_limit(env):
+    torch, ob, qb = env
+    rng = np.random.default_rng(31)
+    aos = [(2, 1, 2, 1.1), (1, 0, 0, 2.0), (3, 2, 3, 0.9), (2, 1, 0, 1.3), (3, 2, 1, 0.7), (2, 0, 0, 1.5),
+           (3, 0, 0, 1.2), (3, 1, 1, 0.8), (2, 1, 1, 1.3), (4, 2, 4, 1.1), (4, 1, 0, 0.9)]
+    C = rng.standard_normal((len(aos), 7))
+    for norm in (None, rng.uniform(0.5, 2, len(aos))):   # lone p / d functions, radial powers, custom normalisation, 3 up 2 down
+        d = atom_system(3.0, aos, C, 3, 2, det_up=[[4, 0, 2], [4, 5, 2], [1, 0, 2], [4, 3, 5]],
+                        det_dn=[[1, 3], [1, 3], [0, 3], [1, 2]], ci=[0.9, 0.2, -0.3, 0.15], norm=norm,
+                        a_par=0.25, a_anti=0.5, b=0.8, xyz=(0.1, -0.2, 0.3))
+        check_backflow(env, _with_bf(d, 0.15), soa(rng.standard_normal((131, 5, 3)) * 1.5), threads=2)
+    for with_general in (False, True):                   # every determinant class; spin-polarised 4 up / 3 down
+        rng = np.random.default_rng(77)
+        d = _classes_system(rng, with_general)
+        check_backflow(env, _with_bf(d, -0.07), soa(rng.standard_normal((203, 7, 3)) * 1.2 + np.array([0.2, 0.1, -0.3])), threads=4)
+    d, r = wl.co_scan(M=24, n_geom=2)[1]                 # 500 determinants
+    check_backflow(env, _with_bf(d, 0.04), r)
+    # one electron: the map is the identity, the hydrogen atom stays exact
+    da = _with_bf(atom_system(1, [(1, 0, 0, 1.0)], [[1.0]], 1, 0), 0.3)
+    s = qb.QmcSystem(da)
+    el = s.local_energy(_to_gpu(torch, soa(rng.standard_normal((257, 1, 3)) * 2)))[2]
+    assert float((el + 0.5).abs().max()) < 1e-12
+    s.close()
+    # w -> 0: the backflow kernel's general formulas against the plain path of the same library
+    d, r = wl.li2(M=200)
+    s0, s1 = qb.QmcSystem(d), qb.QmcSystem(_with_bf(d, 1e-200))
+    lp0, sg0, el0 = (t.cpu().numpy() for t in s0.local_energy(_to_gpu(torch, r)))
+    lp1, sg1, el1 = (t.cpu().numpy() for t in s1.local_energy(_to_gpu(torch, r)))
+    keep = lp0 - lp0.max() > math.log(1e-6)
+    assert np.array_equal(sg0, sg1) and np.max(np.abs(lp1 - lp0)) < 1e-10
+    assert np.max((np.abs(el1 - el0) / np.maximum(1, np.abs(el0)))[keep]) < 1e-8
+    s0.close(); s1.close()
+
+
+def test_backflow_sampler_unsupported_calls_and_output_bounds(env):
+    torch, ob, qb = env
+    d, r = wl.li2(M=301)
+    d = _with_bf(d, 0.1)
+    check_metropolis(env, d, r, 0.3, 8, seed=11)
+    d5, r5 = wl.co(M=64)
+    check_metropolis(env, _with_bf(d5, 0.05), r5, 0.2, 4, seed=12, eloc_acc=True)
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    for call in (lambda: s.log_derivatives(rg), lambda: s.orbital_derivatives(rg, d.n_ao, d.n_mo),
+                 lambda: s.nuclear_log_gradient(rg, d.n_atoms), lambda: s.nuclear_energy_gradient(rg, d.n_atoms)):
+        with pytest.raises(qb.QmcError) as ei:
+            call()
+        assert ei.value.status == qb.QMC_EUNSUPPORTED
+    M = 131
+    a, b, c = _Guarded(torch, M), _Guarded(torch, M), _Guarded(torch, M)
+    rq = rg[:, :, :M].contiguous()
+    assert qb.lib().qmc_local_energy(s._h, rq.data_ptr(), M, a.ptr, b.ptr, c.ptr, torch.cuda.current_stream().cuda_stream) == 0
+    torch.cuda.synchronize()
+    a.check("backflow logpsi"); b.check("backflow sign"); c.check("backflow eloc")
+    s.close()
+    with pytest.raises(qb.QmcError) as ei:     # backflow with the many-body Jastrow kernels is outside what is built
+        qb.QmcSystem(_with_en(d, 0.3, -0.05, 0.7))
+    assert ei.value.status == qb.QMC_EUNSUPPORTED
