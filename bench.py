@@ -313,7 +313,30 @@ def main():
         if k >= 3:
             t_f += a.elapsed_time(b) * 1e-3
             t_fr += b.elapsed_time(c) * 1e-3
-    del dC, dz, dR, dE, r_orb
+    # NEXT-3: the same wavefunction with the inverse backflow transformation (w = 0.05): E_L by the explicit-route
+    # backflow kernel, log|Psi| and the sampler with the orbitals at the backflow coordinates
+    import copy
+    d_bf = copy.copy(d)
+    d_bf.backflow_w = 0.05
+    sys_bf = qb.QmcSystem(d_bf, device=local_rank)
+    r_bf = r0.clone()
+    t_b = [0.0, 0.0, 0.0]
+    for k in range(3 + K_DERIV):
+        e0_, e1_, e2_, e3_ = ev(), ev(), ev(), ev()
+        e0_.record(st)
+        sys_bf.local_energy(r_orb, lp_o, sg_o, el_o)
+        e1_.record(st)
+        sys_bf.log_psi(r_bf, lp, sg)
+        e2_.record(st)
+        sys_bf.metropolis(r_bf, step_size, n_sweeps, seed, sweep_offset=k * n_sweeps, walker_offset=rank * M, logpsi=lp, sign=sg)
+        e3_.record(st)
+        torch.cuda.synchronize()
+        if k >= 3:
+            t_b[0] += e0_.elapsed_time(e1_) * 1e-3
+            t_b[1] += e1_.elapsed_time(e2_) * 1e-3
+            t_b[2] += e2_.elapsed_time(e3_) * 1e-3
+    sys_bf.close()
+    del dC, dz, dR, dE, r_orb, r_bf
 
     t_met, t_el, t_all, t_e2e, t_kmain, t_kfb = max_over_ranks([t_met, t_el, t_all, t_e2e, t_kmain, t_kfb], device=dev)
 
@@ -390,6 +413,11 @@ def main():
                                         "note": "SURVEY 8(f) NEXT-4: grad_alpha E_L per walker (explicit route: every determinant "
                                                 "eliminated on its own) and the estimator of eq. 7; the walkers are not "
                                                 "equilibrated here, so F is a throughput figure, not a physical force"},
+            "backflow": {"w": 0.05, "ms_local_energy": 1e3 * t_b[0] / K_DERIV, "walkers_local_energy": int(M_orb),
+                         "ms_log_psi": 1e3 * t_b[1] / K_DERIV, "ms_metropolis": 1e3 * t_b[2] / K_DERIV, "walkers": int(M),
+                         "walker_steps_per_s": world * M * n_sweeps / (t_b[2] / K_DERIV),
+                         "note": "SURVEY 8(f) NEXT-3: inverse backflow K_BF = w/r; E_L on the explicit route (every determinant "
+                                 "eliminated on its own), values-only kernels on the excitation tables"},
             "gpu_launches": int(launches),
             "clocks": clocks,
             "last_step": {"mean_E_L": mean, "stderr": err},
