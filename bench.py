@@ -277,6 +277,16 @@ def main():
             t_d += a.elapsed_time(b) * 1e-3
             t_g += b.elapsed_time(c) * 1e-3
     del O
+    t_fu = 0.0
+    for k in range(3 + K_DERIV):
+        flush.fill_(k & 0xFF)
+        a, b = ev(), ev()
+        a.record(st)
+        _, _, _, e_vf, grad_f = sysh.local_energy_gradient(r, lp, sg, el)
+        b.record(st)
+        torch.cuda.synchronize()
+        if k >= 3:
+            t_fu += a.elapsed_time(b) * 1e-3
     # orbital-parameter derivatives (MO coefficients, AO exponents) on the first 32768 walkers of the batch
     M_orb = min(M, 32768)
     r_orb = r[:, :, :M_orb].contiguous()
@@ -400,6 +410,9 @@ def main():
                                 "ms_energy_gradient": 1e3 * t_g / K_DERIV, "O_bytes": int(M) * n_par * 8,
                                 "gradient_hbm_gbs": int(M) * (n_par + 1) * 8 / (t_g / K_DERIV) / 1e9,
                                 "E_v": e_v, "grad_norm": float(np.linalg.norm(grad)),
+                                "ms_fused_local_energy_and_gradient": 1e3 * t_fu / K_DERIV,
+                                "fused_over_plain_local_energy": (t_fu / K_DERIV) / (t_el / K),
+                                "fused_grad_max_abs_diff": float(np.max(np.abs(grad_f - grad))),
                                 "note": "SURVEY 8(f) NEXT-1, eq. 6; gradient time includes batch stats, the D2H of the result and a stream synchronise"},
             "orbital_derivatives": {"walkers": int(M_orb), "outputs_per_walker": int(d.n_ao * d.n_mo + d.n_ao),
                                     "ms": 1e3 * t_o / K_DERIV,

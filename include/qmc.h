@@ -208,6 +208,19 @@ int qmc_n_param(const qmc_system_t *s);
 int qmc_log_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign,
                         double *d_eloc, double *d_O, void *cuda_stream);
 
+/* qmc_local_energy and the estimator of eq. 6 in one pass, the reduction fused into the E_L kernel
+ * (SURVEY.md 8(f) NEXT-1): the per-walker derivatives O[w][p] never reach HBM.  Each warp keeps sum_w O_p and
+ * sum_w O_p E_L over its walkers in shared memory; groups whose E_L is corrected by the explicit fallback park their
+ * rows in a small scratch and are added afterwards with the corrected energies; a final kernel forms
+ *   E_v = (1/M) sum_w E_L,   grad_p = (2/M) [ sum_w O_p E_L - (sum_w O_p) E_v ]       (theta as in qmc_n_param)
+ * in a fixed order (bit-repeatable).
+ *   d_logpsi, d_sign device out [M] (may be NULL);  d_eloc device out [M] (required);
+ *   h_Ev host out (may be NULL);  h_grad host out [n_param].
+ * Synchronises cuda_stream.  QMC_EUNSUPPORTED when the rows of a warp's walkers do not fit shared memory (very long
+ * expansions: use qmc_log_derivatives + qmc_energy_gradient) or for a backflow wavefunction. */
+int qmc_local_energy_gradient(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, double *d_eloc,
+                              double *h_Ev, double *h_grad, void *cuda_stream);
+
 /* Logarithmic derivatives with respect to the orbital parameters:
  *   d_dC    device, out: double [M][n_ao][n_mo]  d ln Psi / d C[beta][alpha] (MO coefficients; the derivative in
  *           the scaling mu_{beta,alpha} of PAPER.md:57 is c_{beta,alpha} times it; zero for MOs no determinant uses)

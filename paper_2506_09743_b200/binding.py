@@ -17,7 +17,7 @@ _lib = None
 EXPORTS = ["qmc_setup", "qmc_destroy", "qmc_local_energy", "qmc_log_psi", "qmc_metropolis", "qmc_batch_stats",
            "qmc_fp64_peak", "qmc_model_flops", "qmc_launch_count", "qmc_status_string", "qmc_n_param", "qmc_local_energy_explicit", "qmc_set_kernel_timing", "qmc_kernel_times",
            "qmc_log_derivatives", "qmc_energy_gradient", "qmc_local_energy_host", "qmc_orbital_derivatives",
-           "qmc_nuclear_log_gradient", "qmc_nuclear_energy_gradient", "qmc_force"]
+           "qmc_nuclear_log_gradient", "qmc_nuclear_energy_gradient", "qmc_force", "qmc_local_energy_gradient"]
 
 
 class QmcError(RuntimeError):
@@ -67,6 +67,8 @@ def lib():
         L.qmc_orbital_derivatives.argtypes = [vp, vp, i64, vp, vp, vp]
         L.qmc_nuclear_log_gradient.restype = C.c_int
         L.qmc_nuclear_log_gradient.argtypes = [vp, vp, i64, vp, vp]
+        L.qmc_local_energy_gradient.restype = C.c_int
+        L.qmc_local_energy_gradient.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp, vp]
         L.qmc_nuclear_energy_gradient.restype = C.c_int
         L.qmc_nuclear_energy_gradient.argtypes = [vp, vp, i64, vp, vp]
         L.qmc_force.restype = C.c_int
@@ -276,6 +278,20 @@ class QmcSystem:
         _check(lib().qmc_log_derivatives(self._h, _dp(r), M, _dp(logpsi), _dp(sign), _dp(eloc), _dp(O),
                                          _stream(stream)))
         return logpsi, sign, eloc, O
+
+    def local_energy_gradient(self, r, logpsi=None, sign=None, eloc=None, stream=None):
+        """qmc_local_energy_gradient: (logpsi, sign, eloc, E_v, grad[n_param]) -- E_L and the eq. 6 estimator in one pass,
+        the per-walker derivatives never leave the SMs."""
+        M = self._chk_r(r)
+        new = lambda: torch.empty(M, dtype=torch.float64, device=r.device)
+        logpsi = new() if logpsi is None else logpsi
+        sign = new() if sign is None else sign
+        eloc = new() if eloc is None else eloc
+        ev = C.c_double()
+        g = np.empty(self.n_param())
+        _check(lib().qmc_local_energy_gradient(self._h, _dp(r), M, _dp(logpsi), _dp(sign), _dp(eloc), C.addressof(ev), _np(g),
+                                               _stream(stream)))
+        return logpsi, sign, eloc, ev.value, g
 
     def model_flops(self, which: int) -> float:
         return lib().qmc_model_flops(self._h, which)

@@ -45,6 +45,7 @@ struct Variant {
   const void *k_nuc, *k_nuc_small;  // the same kernel in nuclear mode (qmc_nuclear_log_gradient)
   int orb_ws_doubles;
   const void *k_frc, *k_frc_small;  // nuclear energy gradient (8 / 4 warps per block)
+  const void *k_el_fuse, *e_el_fuse;   // E_L + fused eq. 6 reduction (without / with the e-e-n kernel)
   const void *b_psi, *b_metro, *b_el;  // backflow: values-only kernels, and the E_L kernel (explicit route)
   int bf_ws_doubles;
   int frc_ws_doubles;
@@ -73,6 +74,8 @@ Variant make_variant() {
   v.k_frc = (const void *)nuclear_energy_gradient_kernel<NS, NMO, X, 8>;
   v.k_frc_small = (const void *)nuclear_energy_gradient_kernel<NS, NMO, X, 4>;
   v.frc_ws_doubles = Geo<NS, NMO>::total + Geo<NS, NMO>::frcExtra;
+  v.k_el_fuse = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true, false, false, true>;
+  v.e_el_fuse = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true, true, false, true>;
   v.b_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi, false, false, true>;
   v.b_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi, false, true>;
   v.b_el = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBf>;
@@ -192,11 +195,16 @@ struct qmc_system {
   // no allocation on the hot call, and the call can be captured in a CUDA graph after one warm-up call
   // A buffer that has to grow is retired, not freed (a CUDA graph captured earlier may still replay into it); the
   // accept counter of qmc_metropolis is per stream too.
-  struct Scratch { void *p = nullptr; size_t bytes = 0; unsigned long long *counter = nullptr; };
+  struct Scratch {
+    void *p = nullptr; size_t bytes = 0; unsigned long long *counter = nullptr;
+    void *fuse = nullptr; size_t fuse_bytes = 0;  // qmc_local_energy_gradient: warp partials, parked O rows, order list
+  };
   std::mutex scratch_mu;
   std::unordered_map<cudaStream_t, Scratch> scratch;
   std::vector<void *> retired;
   // qmc_local_energy_host: two internal streams and double-buffered device scratch (grown on demand)
+  bool fuse_ready = false; // fused E_L + eq. 6 kernel configured (lazily)
+  int blocks_fuse = 0, smem_fuse = 0;
   bool bf_ready = false;   // backflow E_L kernel configured (lazily)
   int blocks_bf = 0;
   bool frc_ready = false;  // nuclear energy-gradient kernel configured (lazily)
@@ -248,6 +256,7 @@ void qmc_destroy(qmc_system_t *s) {
   for (auto &kv : s->scratch) {
     cudaFree(kv.second.p);
     cudaFree(kv.second.counter);
+    cudaFree(kv.second.fuse);
   }
   for (void *q : s->retired) cudaFree(q);
   for (int i = 0; i < 2; ++i) {
@@ -1134,6 +1143,114 @@ int qmc_nuclear_log_gradient(qmc_system_t *s, const double *d_r, int64_t M, doub
   CK(cudaGetLastError());
   ++g_launches;
   return orbital_launch(s, d_r, M, nullptr, nullptr, d_dR, cuda_stream);
+}
+
+int qmc_local_energy_gradient(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, double *d_eloc,
+                              double *h_Ev, double *h_grad, void *cuda_stream) {
+  if (!s || !d_r || M <= 0 || !d_eloc || !h_grad) return QMC_EINVAL;
+  if (s->P.bf_w != 0.0) return QMC_EUNSUPPORTED;
+  CK(cudaSetDevice(s->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int np = kJastrowParams + 7 * s->P.n_een + s->P.n_det_all, G = s->P.G;
+  const int fuse_stride = ((G + 2) * np + G + 1) & ~1;  // G rows, two accumulator rows, 1 / (Sigma / D_0) per walker
+  const void *kern = s->P.n_een > 0 ? s->var.e_el_fuse : s->var.k_el_fuse;
+  {
+    std::lock_guard<std::mutex> lock(s->scratch_mu);  // lazy configuration
+    if (!s->fuse_ready) {
+      int dev_smem = 0;
+      cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, s->device);
+      s->smem_fuse = s->smem_el + kWarpsEl * fuse_stride * (int)sizeof(double);
+      if (s->smem_fuse > dev_smem) return QMC_EUNSUPPORTED;  // too many parameters for the fused rows: use qmc_log_derivatives
+      CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, s->smem_fuse));
+      int per_sm = 0;
+      CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kWarpsEl * 32, s->smem_fuse));
+      if (per_sm < 1) return QMC_EUNSUPPORTED;
+      s->blocks_fuse = per_sm * s->n_sm;
+      s->fuse_ready = true;
+    }
+  }
+  const int64_t groups = (M + G - 1) / G;
+  const int grid = (int)std::min<int64_t>((groups + kWarpsEl - 1) / kWarpsEl, s->blocks_fuse);
+  const int n_warps = grid * kWarpsEl;
+  const bool fallback = s->P.n_det_all > 1;
+  const int cap = (int)std::min<int64_t>(groups, 8192);
+  // scratch of the explicit fallback (as qmc_local_energy) and of the fused reduction, both per stream
+  const int64_t expl_warps = (int64_t)s->blocks_expl * kWarpsEl;
+  const size_t n_part = (size_t)(groups + expl_warps) * (size_t)G * 2;
+  const size_t need_fb = n_part * sizeof(double) + (size_t)(2 * groups + 2) * sizeof(int);
+  const size_t n_fpart = (size_t)n_warps * (size_t)(2 * np + 2), n_fbO = (size_t)cap * (size_t)G * (size_t)np;
+  const size_t need_fuse = (n_fpart + n_fbO) * sizeof(double) + (size_t)(cap + 2) * sizeof(int);
+  double *fb = nullptr, *fz = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(s->scratch_mu);
+    qmc_system::Scratch &sc = s->scratch[st];
+    if (sc.bytes < need_fb) {
+      if (sc.p) s->retired.push_back(sc.p);
+      sc.p = nullptr;
+      sc.bytes = 0;
+      CK(cudaMalloc(&sc.p, need_fb));
+      sc.bytes = need_fb;
+    }
+    if (sc.fuse_bytes < need_fuse) {
+      if (sc.fuse) s->retired.push_back(sc.fuse);
+      sc.fuse = nullptr;
+      sc.fuse_bytes = 0;
+      CK(cudaMalloc(&sc.fuse, need_fuse));
+      sc.fuse_bytes = need_fuse;
+    }
+    fb = static_cast<double *>(sc.p);
+    fz = static_cast<double *>(sc.fuse);
+  }
+  int dev = s->device;
+  ReduceScratch *rs = nullptr;
+  if (int rc = reduce_scratch(dev, st, (size_t)np, 0, &rs)) return rc;
+  int *fbi = reinterpret_cast<int *>(fb + n_part);
+  int *fzi = reinterpret_cast<int *>(fz + n_fpart + n_fbO);  // [0] = overflow flag, [1 ..] = order
+  CK(cudaMemsetAsync(fbi, 0, sizeof(int), st));
+  CK(cudaMemsetAsync(fzi, 0, sizeof(int), st));
+  WalkerIO io{};
+  io.r_in = d_r;
+  io.logpsi = d_logpsi;
+  io.sign = d_sign;
+  io.eloc = d_eloc;
+  io.M = M;
+  io.fuse_part = fz;
+  io.fb_O = fz + n_fpart;
+  io.fb_cap = cap;
+  io.fb_over = fzi;
+  io.fuse_stride = fuse_stride;
+  if (fallback) {
+    io.fb_part = fb;
+    io.fb_count = fbi;
+    io.fb_list = fbi + 1;
+    io.fb_done = fbi + 1 + groups;
+  }
+  void *args[2] = {(void *)&s->P, (void *)&io};
+  CK(cudaLaunchKernel(kern, dim3(grid), dim3(kWarpsEl * 32), args, s->smem_fuse, st));
+  ++g_launches;
+  if (fallback) {
+    CK(cudaLaunchKernel(s->var.k_expl, dim3(s->blocks_expl), dim3(kWarpsEl * 32), args, s->smem_el, st));
+    order_flagged_kernel<<<1, 1024, 0, st>>>(io.fb_count, io.fb_list, cap, fzi + 1);
+    CK(cudaGetLastError());
+    g_launches += 2;
+  }
+  fused_gradient_final_kernel<<<np, 128, 0, st>>>(fz, n_warps, np, fallback ? io.fb_count : nullptr, io.fb_list, fzi + 1, io.fb_O, cap,
+                                                d_eloc, G, M, kJastrowParams + 7 * s->P.n_een, s->P.det_orig, fzi, rs->d_res);
+  CK(cudaGetLastError());
+  ++g_launches;
+  CK(cudaStreamSynchronize(st));  // the final kernel wrote {E_v, overflow flag, grad} into mapped host memory
+  if (rs->h_res[1] != 0.0) {
+    // more groups took the explicit route than the parking area holds (pathological batch): the unfused path
+    double *d_O = nullptr;
+    CK(cudaMalloc(&d_O, (size_t)M * (size_t)np * sizeof(double)));
+    int rc = launch_eval(s, d_r, M, d_logpsi, d_sign, d_eloc, cuda_stream, true, d_O);
+    if (rc == QMC_OK) rc = qmc_energy_gradient(d_eloc, d_O, M, np, h_Ev, h_grad, cuda_stream);
+    cudaFree(d_O);
+    return rc;
+  }
+  if (h_Ev) *h_Ev = rs->h_res[0];
+  for (int p = 0; p < np; ++p) h_grad[p] = rs->h_res[2 + p];
+  return QMC_OK;
 }
 
 int qmc_nuclear_energy_gradient(qmc_system_t *s, const double *d_r, int64_t M, double *d_dE, void *cuda_stream) {

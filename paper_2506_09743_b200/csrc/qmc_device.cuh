@@ -204,6 +204,12 @@ struct WalkerIO {
   double *logpsi, *sign, *eloc;
   double *O;           // device [M][kJastrowParams + 7 n_een + n_det_all] parameter derivatives (DerivOut), or null
   int64_t M;
+  // fused eq. 6 reduction (qmc_local_energy_gradient): per-warp partial sums and the O rows of the listed groups
+  double *fuse_part;   // device [2 n_param + 1][grid warps]: sum O_p, sum O_p E_L, then sum E_L
+  double *fb_O;        // device [fb_cap][G][n_param]: O rows of the groups on the explicit work list
+  int fb_cap;          // rows of fb_O; a listed group beyond it sets fb_over
+  int *fb_over;        // device flag
+  int fuse_stride;     // doubles each warp's scratch is extended by: (G + 2) n_param, even
 };
 
 // Parameter-derivative output (eq. 6): O[w][p] = (dPsi/dtheta_p)/Psi for

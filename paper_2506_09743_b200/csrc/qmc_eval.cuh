@@ -240,7 +240,10 @@ constexpr bool kCompact = !EL && !EXPL && ORB == 0;
 // BF (values only): the orbitals are evaluated at the backflow coordinates rt_i = r_i + w sum_{j != i} (r_i - r_j)/r_ij
 // (PAPER.md:53 with the inverse kernel of PAPER.md:97), the Jastrow factor at r; the determinant algebra is unchanged.
 // E_L of a backflow wavefunction has its own kernel (qmc_backflow.cuh).
-template <int NS, int NMO, bool EL, bool X, bool EXPL = false, bool DERIV = false, bool EEN = false, int ORB = 0, bool BF = false>
+// FUSE (with DERIV): the rows O[w][:] of the G walkers are left in shared memory behind the evaluator's scratch
+// (ws + Geo::total, row stride n_param) instead of going to HBM: the caller reduces them for the eq. 6 estimator.
+template <int NS, int NMO, bool EL, bool X, bool EXPL = false, bool DERIV = false, bool EEN = false, int ORB = 0, bool BF = false,
+          bool FUSE = false>
 __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp,
                              const double *__restrict__ sC, const DetRec *__restrict__ sDet,
                              double *__restrict__ ws, double x, double y, double z, int lane,
@@ -892,6 +895,10 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       }
     };
     constexpr int kCiUnroll = QMC_CI_UNROLL;
+    // FUSE: D_n / D_0 of every determinant is kept (kernel order: reference-equal ones, classes 1-4, general) in the
+    // walker's shared-memory row; the caller divides by Sigma / D_0 -- no second pass over the determinants
+    double *const sRn = ws + GE::total + (wvalid ? wg : 0) * (kJastrowParams + 7 * P.n_een + P.n_det_all) + kJastrowParams +
+                        7 * P.n_een + P.n_ref;
     // class 1: one substitution in one spin -- one table entry
 #pragma unroll kCiUnroll
     for (int n = sub; n < P.n_a1; n += LW) {
@@ -900,6 +907,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       entry(dr.up, R, D);
       den = fma(dr.d, R, den);
       if (EL) num = fma(dr.d, D, num);
+      if (FUSE && wvalid) sRn[n] = R;
     }
     // class 2: one substitution in each spin -- two table entries
 #pragma unroll kCiUnroll
@@ -911,6 +919,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       const double w = dr.d * Ru;
       den = fma(w, Rd, den);
       if (EL) num = fma(dr.d, Du * Rd, fma(w, Dd, num));
+      if (FUSE && wvalid) sRn[n] = Ru * Rd;
     }
     // class 3: two substitutions in one spin, the other spin as in the reference -- one 2x2 block
 #pragma unroll kCiUnroll
@@ -921,8 +930,10 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       entry(dr.up >> 16, b, bm);
       entry(dr.dn & 0xffffu, c, cm);
       entry(dr.dn >> 16, d, dm);
-      den = fma(dr.d, fma(a, d, -b * c), den);
+      const double R3 = fma(a, d, -b * c);
+      den = fma(dr.d, R3, den);
       if (EL) num = fma(dr.d, fma(d, am, fma(a, dm, -fma(b, cm, c * bm))), num);
+      if (FUSE && wvalid) sRn[n] = R3;
     }
     // class 4: the rest with at most two per spin -- 2x2 sub-determinants in both spins
 #pragma unroll kCiUnroll
@@ -934,6 +945,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       const double w = dr.d * Ru;
       den = fma(w, Rd, den);
       if (EL) num = fma(dr.d, Du * Rd, fma(w, Dd, num));
+      if (FUSE && wvalid) sRn[n] = Ru * Rd;
     }
     // determinants with more than two substitutions in a spin (general sub-determinants)
     for (int n = sub; n < P.n_gen; n += LW) {
@@ -943,6 +955,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       const double dn = P.gen[n].d, w = dn * u[0];
       den = fma(w, v[0], den);
       if (EL) num = fma(dn, u[1] * v[0], fma(w, v[1], num));
+      if (FUSE && wvalid) sRn[P.n_det + n] = u[0] * v[0];
     }
     double Jsum = 0.0, esum = 0.0;
     if (wvalid)
@@ -976,6 +989,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       }
       sRes[wg * 4 + 0] = Jsum + lg;
       sRes[wg * 4 + 1] = sgn;
+      if (FUSE) (ws + GE::total)[(G + 2) * (kJastrowParams + 7 * P.n_een + P.n_det_all) + wg] = 1.0 / den;
       const double eloc = EL ? esum + (sProb[pu * 4 + 2] + sProb[pd * 4 + 2]) + num / den + P.vnn : 0.0;
       if (EL) sRes[wg * 4 + 2] = eloc;
       // explicit fallback when the estimated table-path error of E_L exceeds a tenth of the parity bound
@@ -1060,9 +1074,9 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       // Jastrow: dJ/dtheta summed over the walker's electrons; CI: d ln Sigma / d d_n = R_n^up R_n^dn / den
       // (D_n / D_0 over Sigma / D_0), a second, values-only pass over the determinant classes.
       const int64_t wo = dv.w0 + wg;
-      if (wvalid && wo < dv.M && dv.O) {
+      if (wvalid && wo < dv.M && (FUSE || dv.O)) {
         const int np = kJastrowParams + 7 * P.n_een + P.n_det_all;
-        double *row = dv.O + wo * np;
+        double *row = FUSE ? (ws + GE::total + (wvalid ? wg : 0) * np) : (dv.O + wo * np);
         for (int k = sub; k < 3; k += LW) {
           double t = 0.0;
           for (int j = 0; j < ne; ++j) t += sXYZ[(wg * ne + j) * 3 + k];
@@ -1075,14 +1089,15 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       sXYZ[lane * 3 + 1] = dEn1;
       sXYZ[lane * 3 + 2] = dEn2;
       __syncwarp();
-      if (wvalid && wo < dv.M && dv.O) {
+      if (wvalid && wo < dv.M && (FUSE || dv.O)) {
         const int np = kJastrowParams + 7 * P.n_een + P.n_det_all;
-        double *row = dv.O + wo * np;
+        double *row = FUSE ? (ws + GE::total + (wvalid ? wg : 0) * np) : (dv.O + wo * np);
         for (int k = sub; k < 3; k += LW) {
           double t = 0.0;
           for (int j = 0; j < ne; ++j) t += sXYZ[(wg * ne + j) * 3 + k];
           row[3 + k] = t;
         }
+        if (!FUSE) {
         const double iden = 1.0 / den;
         const int *orig = P.det_orig;
         double *rowd = row + kJastrowParams + 7 * P.n_een;
@@ -1112,6 +1127,10 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           excite_general<EL>(&P.gen[n].s[1], Td, RS, v);
           rowd[orig[n]] = u[0] * v[0] * iden;
         }
+        } else {
+          double *rowd = row + kJastrowParams + 7 * P.n_een;
+          for (int n = sub; n < P.n_ref; n += LW) rowd[n] = 1.0;  // determinants equal to the reference: D_n / D_0 = 1
+        }
       }
       if (EEN) {
         // the seven parameters of every e-e-n term: coordinates back into the scratch, each lane its electron's
@@ -1132,8 +1151,9 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
             for (int j = 0; j < ne; ++j) t += shfl_d(dq[k], base + j, 32);
             dq[k] = t;
           }
-          if (active && e == 0 && wo2 < dv.M && dv.O) {
-            double *row = dv.O + wo2 * (kJastrowParams + 7 * P.n_een + P.n_det_all) + kJastrowParams + 7 * mu;
+          if (active && e == 0 && wo2 < dv.M && (FUSE || dv.O)) {
+            const int np2 = kJastrowParams + 7 * P.n_een + P.n_det_all;
+            double *row = (FUSE ? (ws + GE::total + g * np2) : (dv.O + wo2 * np2)) + kJastrowParams + 7 * mu;
 #pragma unroll
             for (int k = 0; k < 7; ++k) row[k] = dq[k];
           }

@@ -36,7 +36,10 @@ __device__ __forceinline__ void dummy_xyz(int lane, double &x, double &y, double
   z = 0.53 - 0.05 * lane;
 }
 
-template <int NS, int NMO, bool EL, bool X, int WPB, bool DERIV = false, bool EEN = false, bool BF = false>
+// FUSE (with DERIV): the eq. 6 reduction is fused: the rows O[w][:] stay in shared memory,
+// each warp keeps sum_w O_p and sum_w O_p E_L over its walkers and writes them once at the end; a group on the explicit
+// work list (its E_L is corrected later) parks its rows in io.fb_O instead; fused_gradient_final_kernel finishes.
+template <int NS, int NMO, bool EL, bool X, int WPB, bool DERIV = false, bool EEN = false, bool BF = false, bool FUSE = false>
 __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
     local_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -48,11 +51,18 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   using GE = Geo<NS, NMO>;
   const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;  // shfl: tells the compiler it is warp-uniform
   constexpr bool CP = kCompact<EL, false, 0>;
-  double *ws = wsBase + warp * GE::totalC(CP);
+  double *ws = wsBase + warp * (GE::totalC(CP) + (FUSE ? io.fuse_stride : 0));
   const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
   const int g = lane / ne, e = lane - g * ne;
   const int64_t n_groups = (io.M + G - 1) / G;
   const int64_t stride = (int64_t)gridDim.x * WPB;
+  const int np = kJastrowParams + 7 * P.n_een + P.n_det_all;
+  double *sO = ws + GE::total, *accO = sO + G * np, *accOE = accO + np;  // FUSE only
+  double accE = 0.0;
+  if (FUSE) {
+    for (int p = lane; p < 2 * np; p += 32) accO[p] = 0.0;
+    __syncwarp();
+  }
   auto fetch = [&](int64_t grp, double &x, double &y, double &z) {
     const int64_t w = grp * G + g;
     if ((g < G) && (w < io.M)) {
@@ -66,7 +76,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   for (int64_t grp = (int64_t)blockIdx.x * WPB + warp; grp < n_groups; grp += stride) {
     double x, y, z;
     fetch(grp, x, y, z);
-    eval_walkers<NS, NMO, EL, X, false, DERIV, EEN, 0, BF>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1, DerivOut{io.O, grp * G, io.M});
+    eval_walkers<NS, NMO, EL, X, false, DERIV, EEN, 0, BF, FUSE>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1, DerivOut{io.O, grp * G, io.M});
     bool flagged = false;
     if (lane < G) {
       const int64_t wo = grp * G + lane;
@@ -79,15 +89,53 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
       }
     }
     // walkers whose reference determinant is nearly singular go to the explicit kernel
+    int idx = -1;
     if (EL && io.fb_list) {
       const unsigned any = __ballot_sync(0xffffffffu, flagged);
       if (any && lane == 0) {
-        const int idx = atomicAdd(io.fb_count, 1);
+        idx = atomicAdd(io.fb_count, 1);
         io.fb_list[idx] = (int)grp;
         io.fb_done[idx] = 0;
       }
+      if (FUSE) idx = __shfl_sync(0xffffffffu, idx, 0);
+    }
+    if (FUSE) {
+      // rows in kernel order: Jastrow entries are final, the CI entries hold D_n / D_0 and want 1 / (Sigma / D_0)
+      const double *res = ws + GE::oResC(CP);
+      const double *sIden = sO + (G + 2) * np;
+      const int nj = kJastrowParams + 7 * P.n_een;
+      if (idx >= 0) {  // E_L of this group is still to be corrected: park its rows for the final kernel
+        if (idx < io.fb_cap) {
+          for (int wg = 0; wg < G; ++wg)
+            if (grp * G + wg < io.M) {
+              const double iden = sIden[wg];
+              for (int p = lane; p < np; p += 32) io.fb_O[((int64_t)idx * G + wg) * np + p] = sO[wg * np + p] * ((p >= nj) ? iden : 1.0);
+            }
+        } else if (lane == 0) {
+          *io.fb_over = 1;
+        }
+      } else {
+        const int nw = (int)min((int64_t)G, io.M - grp * G);  // walkers of this group (the last one may be ragged)
+        for (int p = lane; p < np; p += 32) {
+          double so = 0.0, soe = 0.0;
+          for (int wg = 0; wg < nw; ++wg) {
+            const double v = sO[wg * np + p] * ((p >= nj) ? sIden[wg] : 1.0);
+            so += v;
+            soe = fma(v, res[wg * 4 + 2], soe);
+          }
+          accO[p] += so;
+          accOE[p] += soe;
+        }
+        for (int wg = 0; wg < nw; ++wg) accE += res[wg * 4 + 2];  // every lane keeps the same sum
+      }
     }
     __syncwarp();
+  }
+  if (FUSE) {
+    // transposed, [2 n_param + 1][grid warps], so that the final kernel reads each parameter's column contiguously
+    const int64_t nwarps = (int64_t)gridDim.x * WPB, me = (int64_t)blockIdx.x * WPB + warp;
+    for (int p = lane; p < 2 * np; p += 32) io.fuse_part[p * nwarps + me] = accO[p];
+    if (lane == 0) io.fuse_part[(int64_t)2 * np * nwarps + me] = accE;
   }
 }
 
@@ -873,6 +921,71 @@ __global__ void __launch_bounds__(128) gradient_final_kernel(const double *__res
   if (threadIdx.x == 0) {  // res (mapped host memory) = {E_v, stderr, grad[0 .. np-1]}
     res[2 + p] = 2.0 * sh[0] / (double)M;
     if (p == 0) { res[0] = stats[0]; res[1] = stats[1]; }
+  }
+}
+
+// ---------------------------------------------------------------------------------
+// Fused eq. 6: finish grad_p = (2/M) [sum_w O_p E_L - (sum_w O_p)(sum_w E_L)/M] from the per-warp
+// partial sums of local_energy_kernel<..., FUSE> and the parked rows of the groups that took the explicit route
+// (their E_L is read back from eloc, where explicit_energy_kernel wrote it).  The work list is filled in a
+// non-deterministic order, so order_flagged_kernel ranks its entries by group index first: every sum below then
+// runs in a fixed order and the result is bit-repeatable.
+// ---------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) order_flagged_kernel(const int *__restrict__ fb_count, const int *__restrict__ fb_list,
+                                                             int cap, int *__restrict__ order) {
+  const int n = min(*fb_count, cap);
+  for (int e = threadIdx.x; e < n; e += blockDim.x) {
+    const int g = fb_list[e];
+    int rank = 0;
+    for (int k = 0; k < n; ++k) rank += (fb_list[k] < g) ? 1 : 0;  // group indices are distinct
+    order[rank] = e;
+  }
+}
+
+__device__ __forceinline__ double block_tree_128(double v, double *sh) {
+  sh[threadIdx.x] = v;
+  __syncthreads();
+  for (int w = 64; w > 0; w >>= 1) {
+    if ((int)threadIdx.x < w) sh[threadIdx.x] += sh[threadIdx.x + w];
+    __syncthreads();
+  }
+  const double r = sh[0];
+  __syncthreads();
+  return r;
+}
+
+__global__ void __launch_bounds__(128)
+    fused_gradient_final_kernel(const double *__restrict__ part, int n_warps, int np, const int *__restrict__ fb_count,
+                                const int *__restrict__ fb_list, const int *__restrict__ order, const double *__restrict__ fbO,
+                                int cap, const double *__restrict__ eloc, int G, int64_t M, int nj,
+                                const int *__restrict__ det_orig, const int *__restrict__ fb_over, double *__restrict__ res) {
+  __shared__ double sh[128];
+  const int p = blockIdx.x;
+  double so = 0.0, soe = 0.0, se = 0.0;
+  for (int b = threadIdx.x; b < n_warps; b += blockDim.x) {  // thread t: warps t, t + 128, ... in order
+    so += part[(int64_t)p * n_warps + b];
+    soe += part[(int64_t)(np + p) * n_warps + b];
+    se += part[(int64_t)2 * np * n_warps + b];
+  }
+  const int n = fb_count ? min(*fb_count, cap) : 0;
+  for (int k = threadIdx.x; k < n; k += blockDim.x) {        // listed groups in order of their group index
+    const int e = order[k];
+    const int64_t grp = fb_list[e];
+    for (int wg = 0; wg < G; ++wg) {
+      const int64_t wo = grp * G + wg;
+      if (wo < M) {
+        const double v = fbO[((int64_t)e * G + wg) * np + p], E = eloc[wo];
+        so += v;
+        soe = fma(v, E, soe);
+        se += E;
+      }
+    }
+  }
+  const double SO = block_tree_128(so, sh), SOE = block_tree_128(soe, sh), SE = block_tree_128(se, sh);
+  if (threadIdx.x == 0) {  // res (mapped host memory) = {E_v, -, grad[0 .. np-1]}; rows were in kernel order
+    const double ev = SE / (double)M;
+    res[2 + ((p < nj) ? p : nj + det_orig[p - nj])] = 2.0 * (SOE - SO * ev) / (double)M;
+    if (p == 0) { res[0] = ev; res[1] = (double)*fb_over; }  // res[1] != 0: the parking area overflowed
   }
 }
 

@@ -460,6 +460,11 @@ def check_log_derivatives(env, d, r, threads=8):
     torch.cuda.synchronize()
     assert torch.equal(el, el_plain), "E_L of the derivative kernel differs from qmc_local_energy"
     ev, g = qb.energy_gradient(el, O)
+    # the fused call (qmc_local_energy_gradient): same E_L bit for bit, the estimator without O in HBM, bit-repeatable
+    lpf, sgf, elf, evf, gf = s.local_energy_gradient(rg)
+    assert torch.equal(elf, el) and torch.equal(lpf, lp) and torch.equal(sgf, sg)
+    evf2, gf2 = s.local_energy_gradient(rg)[3:]
+    assert evf2 == evf and np.array_equal(gf2, gf)
     lpn, sgn, eln, On = (t.cpu().numpy() for t in (lp, sg, el, O))
     s.close()
     assert np.array_equal(sgn, sg0) and np.max(np.abs(lpn - lp0)) < 1e-10
@@ -473,6 +478,8 @@ def check_log_derivatives(env, d, r, threads=8):
     scale = 2.0 * np.mean(np.abs(O0) * np.abs(el0 - ev0)[:, None], axis=0)
     assert abs(ev - ev0) <= 1e-10 * abs(ev0)
     assert np.max(np.abs(g - g0) / np.maximum(scale, 1e-300)) < 1e-8, np.max(np.abs(g - g0) / np.maximum(scale, 1e-300))
+    assert abs(evf - ev0) <= 1e-10 * abs(ev0)
+    assert np.max(np.abs(gf - g0) / np.maximum(scale, 1e-300)) < 1e-8, np.max(np.abs(gf - g0) / np.maximum(scale, 1e-300))
     # and the GPU reduction applied to identical inputs agrees with the oracle's to rounding
     ev1, g1 = qb.energy_gradient(torch.from_numpy(el0).cuda(), torch.from_numpy(O0).cuda())
     assert abs(ev1 - ev0) <= 1e-13 * abs(ev0) and np.max(np.abs(g1 - g0) / np.maximum(scale, 1e-300)) < 1e-12
@@ -1359,3 +1366,33 @@ def test_backflow_sampler_unsupported_calls_and_output_bounds(env):
     with pytest.raises(qb.QmcError) as ei:     # backflow with the many-body Jastrow kernels is outside what is built
         qb.QmcSystem(_with_en(d, 0.3, -0.05, 0.7))
     assert ei.value.status == qb.QMC_EUNSUPPORTED
+
+
+def test_fused_energy_gradient_with_listed_groups_and_at_full_size(env):
+    """qmc_local_energy_gradient where many groups take the explicit route (their rows are parked and added with the
+    corrected energies): a system whose reference all but vanishes on a third of the walkers, against the unfused
+    path of the same library and the oracle; then CO at 131072 walkers, fused against unfused."""
+    torch, ob, qb = env
+    rng = np.random.default_rng(78)
+    aos = [(1, 0, 0, 2.5), (2, 0, 0, 1.0), (3, 0, 0, 0.7), (2, 1, 0, 1.2), (2, 1, 1, 1.2), (2, 1, 2, 1.2)]
+    C = np.zeros((6, 6))
+    C[:3, :2] = rng.standard_normal((3, 2))
+    C[:, 2:] = rng.standard_normal((6, 4))
+    d = atom_system(3.0, aos, C, 2, 1, det_up=[[0, 1], [0, 2], [3, 1], [2, 4], [5, 3]], det_dn=[[0], [0], [1], [0], [2]],
+                    ci=[0.7, 0.3, -0.2, 0.25, 0.1], a_par=0.25, a_anti=0.5, b=1.0)
+    r = rng.standard_normal((1601, 3, 3)) * 1.3
+    for w in range(0, 1601, 3):
+        u = rng.standard_normal(3)
+        r[w, 1] = u / np.linalg.norm(u) * np.linalg.norm(r[w, 0]) * (1.0 + 1e-5 * rng.uniform(0.5, 1.0))
+    check_log_derivatives(env, d, soa(r), threads=4)
+    d, r = wl.co()
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    lp, sg, el, O = s.log_derivatives(rg)
+    ev, g = qb.energy_gradient(el, O)
+    del O
+    lpf, sgf, elf, evf, gf = s.local_energy_gradient(rg)
+    assert torch.equal(elf, el) and torch.equal(lpf, lp)
+    scale = np.maximum(np.abs(g), 1e-3 * np.max(np.abs(g)))
+    assert abs(evf - ev) <= 1e-12 * abs(ev) and np.max(np.abs(gf - g) / scale) < 1e-9, np.max(np.abs(gf - g) / scale)
+    s.close()
