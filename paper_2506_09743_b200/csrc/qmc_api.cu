@@ -597,8 +597,13 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     rc.r.meta = kind | (k << 4) | ((l == 0 || full ? 0 : d->ao_m[rc.aos[0]]) << 8);
     recs.push_back(rc);
   }
-  std::stable_sort(recs.begin(), recs.end(), [](const Rec &a, const Rec &b) { return a.atom < b.atom; });
-  if (recs.size() + (size_t)d->n_atoms > (size_t)kMaxShells) {
+  // per atom, shells in order of their radial power k (stable): one SH_POW record ahead of each power > 0
+  auto rec_k = [](const Rec &a) { return (a.r.meta >> 4) & 3; };
+  std::stable_sort(recs.begin(), recs.end(), [&](const Rec &a, const Rec &b) { return a.atom != b.atom ? a.atom < b.atom : rec_k(a) < rec_k(b); });
+  size_t n_pow = 0;
+  for (size_t q = 0; q < recs.size(); ++q)
+    if (rec_k(recs[q]) > 0 && (q == 0 || recs[q - 1].atom != recs[q].atom || rec_k(recs[q - 1]) != rec_k(recs[q]))) ++n_pow;
+  if (recs.size() + (size_t)d->n_atoms + n_pow > (size_t)kMaxShells) {
     delete s;
     return QMC_EUNSUPPORTED;
   }
@@ -614,7 +619,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     int n_real = 0;
     auto last_shell = [&]() -> ShellRec & {  // the last shell record (an atom record cannot carry the flush)
       size_t j = shells.size();
-      while ((shells[j - 1].meta & 15) == SH_ATOM) --j;
+      while ((shells[j - 1].meta & 15) == SH_ATOM || (shells[j - 1].meta & 15) == SH_POW) --j;
       return shells[j - 1];
     };
     size_t i = 0;
@@ -628,9 +633,16 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
         ar.meta = SH_ATOM;
         shells.push_back(ar);
       }
+      int cur_k = 0;
       for (; i < recs.size() && recs[i].atom == a; ++i) {
       const int nf = (int)recs[i].aos.size();
       ++n_real;
+      if (rec_k(recs[i]) != cur_k) {  // the shells from here on carry r^k
+        cur_k = rec_k(recs[i]);
+        ShellRec pr{};
+        pr.meta = SH_POW | (cur_k << 4);
+        shells.push_back(pr);
+      }
       if (row % kChunk + nf > kChunk) {
         last_shell().meta |= (row % kChunk) << 20;
         while (row % kChunk) { crow.emplace_back(); row_ao.push_back(-1); row_nrm.push_back(0.0); ++row; }

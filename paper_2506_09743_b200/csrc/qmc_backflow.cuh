@@ -178,6 +178,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
       for (int s = 0; s < P.n_shell; ++s) {
         const ShellRec &sh = P.shells[s];
         const int meta = sh.meta, kind = meta & 15;
+        if (kind == SH_POW) continue;  // the radial power is in the shell records' own meta word
         if (kind == SH_ATOM) {
           dx = xt - sh.zeta; dy = yt - sh.c1; dz = zt - sh.c2;
           r2 = fma(dx, dx, fma(dy, dy, dz * dz));

@@ -44,7 +44,11 @@ constexpr int kWarpsBf = 4;  // warps (= walkers in flight) per block of the bac
 constexpr int kWarpsMax = kWarpsEl > kWarpsPsi ? kWarpsEl : kWarpsPsi;
 
 // shell record kinds
-enum : int { SH_S = 0, SH_P = 1, SH_D = 2, SH_P1 = 3, SH_D1 = 4, SH_ATOM = 5 };
+enum : int { SH_S = 0, SH_P = 1, SH_D = 2, SH_P1 = 3, SH_D1 = 4, SH_ATOM = 5, SH_POW = 6 };
+// Record stream: per atom {SH_ATOM, the shells with radial power k = 0, then for every further power in use
+// {SH_POW k, its shells}}.  SH_POW sets the factor r^k that the hot loop multiplies every following radial function
+// by (one multiplication per shell instead of two predicated ones and their selects); the shell records keep k in
+// their meta word for the kernels that read them one at a time.
 constexpr int kMaxShells = 192;  // shell + atom records; they live in the kernel parameter block (constant bank, uniform data path)
 
 // One shell = the AOs that share a centre, n, l and zeta (one radial factor).  Every lane reads the same

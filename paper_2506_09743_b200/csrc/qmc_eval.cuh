@@ -412,13 +412,20 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
     const uint32_t to32 = EL ? opaque_u32(tl32 + 8u * (uint32_t)oo) : 0u;
     const double *const afrag = tile + fk * S + fr;                // A fragments: + 4 ks S + tile column
     int chunk = 0;
-    double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1.0, r = 1.0, ri = 1.0, gd = 0.0;
+    double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1.0, r = 1.0, ri = 1.0, gd = 0.0, pw = 1.0;
+    uint32_t tr = tl32, tro = to32;  // this lane's tile cells of the next AO row (rows follow the record stream)
     // one uniform loop over the record stream [ATOM a][shells of a] ... (every lane reads the same record)
     {
       for (int s = 0; s < P.n_shell; ++s) {
         const ShellRec &sh = P.shells[s];
         const int meta = sh.meta;
+        if ((meta & 15) == SH_POW) {   // the shells that follow carry the radial power r^k
+          const int k = (meta >> 4) & 3;
+          pw = (k == 1) ? r : ((k == 2) ? r2 : r * r2);
+          continue;
+        }
         if ((meta & 15) == SH_ATOM) {  // new centre: {zeta, c1, c2, kd} = {X, Y, Z, charge}
+          pw = 1.0;
           dx = xa - sh.zeta;
           dy = ya - sh.c1;
           dz = za - sh.c2;
@@ -431,9 +438,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           }
           continue;
         }
-        double gr = exp_neg(-sh.zeta * r, sExp, P.mc);          // r^k e^{-zeta r}
-        if (meta & kMetaK1) gr *= r;
-        if (meta & kMetaK2) gr *= r2;
+        const double gr = exp_neg(-sh.zeta * r, sExp, P.mc) * pw;  // r^k e^{-zeta r}
         double h = 0.0;
         if (EL) {
           // lap(S r^k e^{-zeta r}) = phi * [zeta^2 - 2 zeta (k+l+1)/r + k (k+2l+1)/r^2]
@@ -441,8 +446,6 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           const double radlog = fma(sh.kd, ri, -sh.zeta);  // g'/g
           h = fma(-0.5, lapfac, -radlog * gd);
         }
-        const uint32_t rofs = (uint32_t)(((meta >> 12) & 15) * (S * 8));
-        const uint32_t tr = tl32 + rofs, tro = to32 + rofs;
         // value into column lane, combined operator into column opCol(lane): every lane stores
 #define put(t, phi, bop)                          \
   do {                                            \
@@ -450,13 +453,16 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
     if (EL) sts_f64<(t) * S * 8>(tro, (bop));     \
   } while (0)
         const int kind = meta & 15;
+        uint32_t adv = S * 8;  // bytes the row pointers advance by: one row per AO of the record
         if (kind == SH_S) {
           put(0, gr, gr * h);
         } else if (kind == SH_P) {
           put(0, gr * dx, gr * fma(dx, h, -gJx));
           put(1, gr * dy, gr * fma(dy, h, -gJy));
           put(2, gr * dz, gr * fma(dz, h, -gJz));
+          adv = 3 * S * 8;
         } else if (kind == SH_D) {
+          adv = 5 * S * 8;
           double Sh, gs;
           Sh = dx * dy; gs = fma(gJx, dy, gJy * dx);
           put(0, gr * Sh, gr * fma(Sh, h, -gs));
@@ -483,8 +489,12 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           put(0, gr * Sh, gr * fma(Sh, h, -gs));
         }
 #undef put
+        tr += adv;
+        if (EL) tro += adv;
         const int flush = meta >> 20;
         if (flush) {
+          tr = tl32;
+          tro = to32;
           // unused rows of the chunk meet zero rows of C, but must themselves be finite
           for (int pr = flush; pr < kChunk; ++pr) {
             tl[pr * S] = 0.0;

