@@ -423,9 +423,10 @@ def main():
             "nuclear_energy_gradient": {"walkers": int(M_orb), "outputs_per_walker": int(3 * d.n_atoms),
                                         "ms": 1e3 * t_f / K_DERIV, "ms_force_reduction": 1e3 * t_fr / K_DERIV,
                                         "F_z": [float(F[a_, 2]) for a_ in range(d.n_atoms)],
-                                        "note": "SURVEY 8(f) NEXT-4: grad_alpha E_L per walker (explicit route: every determinant "
-                                                "eliminated on its own) and the estimator of eq. 7; the walkers are not "
-                                                "equilibrated here, so F is a throughput figure, not a physical force"},
+                                        "note": "SURVEY 8(f) NEXT-4: grad_alpha E_L per walker (weight matrices from the reference's "
+                                                "tables, explicit route for groups with a near-singular reference) and the "
+                                                "estimator of eq. 7; the walkers are not equilibrated here, so F is a throughput "
+                                                "figure, not a physical force"},
             "backflow": {"w": 0.05, "ms_local_energy": 1e3 * t_b[0] / K_DERIV, "walkers_local_energy": int(M_orb),
                          "ms_log_psi": 1e3 * t_b[1] / K_DERIV, "ms_metropolis": 1e3 * t_b[2] / K_DERIV, "walkers": int(M),
                          "walker_steps_per_s": world * M * n_sweeps / (t_b[2] / K_DERIV),

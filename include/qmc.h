@@ -250,9 +250,11 @@ int qmc_nuclear_log_gradient(qmc_system_t *s, const double *d_r, int64_t M, doub
  *   d_r  device, in:  double [n_e][3][M]
  *   d_dE device, out: double [M][n_atoms][3]  d E_L / d R_alpha,c ; every entry is written
  * E_L = -1/2 lap Psi / Psi + V of eq. 1-3 with d ao_beta(r_i) / d R_alpha = -grad_r ao_beta(r_i) for the AOs of centre
- * alpha: the AO Hessian and the gradient of the AO Laplacian enter, and d (V_en + V_nn) / d R_alpha (eq. 1).  Every
- * determinant is eliminated on its own (the explicit route of PAPER.md:349) for every walker, so the cost is
- * proportional to n_det.  Covers the Pade e-e Jastrow D.1 (which does not see the nuclei); with the e-n / e-e-n kernels
+ * alpha: the AO Hessian and the gradient of the AO Laplacian enter, and d (V_en + V_nn) / d R_alpha (eq. 1).  The
+ * chain rule through the determinants collapses into two weight matrices, obtained from the reference's excitation
+ * tables (F.6/F.7) by reverse differentiation -- one elimination per spin; groups of walkers whose
+ * reference determinant is nearly singular, and expansions with more than two substitutions per spin, eliminate every
+ * determinant on its own instead (the explicit route of PAPER.md:349).  Covers the Pade e-e Jastrow D.1 (which does not see the nuclei); with the e-n / e-e-n kernels
  * D.2 / D.3 switched on the call returns QMC_EUNSUPPORTED.  Two launches on cuda_stream.  Deterministic.  Asynchronous.
  * QMC_EINVAL for null pointers or M <= 0. */
 int qmc_nuclear_energy_gradient(qmc_system_t *s, const double *d_r, int64_t M, double *d_dE, void *cuda_stream);

@@ -337,8 +337,12 @@ struct Geo {
   static constexpr int oGJ = oGam2 + even(ROWS * NMO);
   static constexpr int oStage = oGJ + 96;
   static constexpr int oX = oStage + even(PP * NS * NS);
-  static constexpr int frcExtra = orbExtra + even(ROWS * NMO) + 96 + even(PP * NS * NS) + even(2 * GMAX * NS * NS);
-  static_assert(oX + even(2 * GMAX * NS * NS) == total + frcExtra, "force-kernel scratch regions do not add up");
+  // ... and for its table route (ORB = 4): H = A0^-1 Bv [2 GMAX][NS][LP] and Z = d num / d T, laid out like the T tables
+  static constexpr int oH = oX + even(2 * GMAX * NS * NS);
+  static constexpr int oZ = oH + even(2 * GMAX * NS * LP);
+  static constexpr int frcExtra = orbExtra + even(ROWS * NMO) + 96 + even(PP * NS * NS) + even(2 * GMAX * NS * NS) +
+                                  even(2 * GMAX * NS * LP) + even(2 * GMAX * TS);
+  static_assert(oZ + even(2 * GMAX * TS) == total + frcExtra, "force-kernel scratch regions do not add up");
   // bounds of the overlays (compile-time hygiene: no memory checker runs on this pool)
   static_assert(NS >= 1 && NS <= kMaxSpin && NMO <= 16, "instantiation outside the register-array limits");
   static_assert(ROWS <= 32 && 2 * GMAX * NS >= ROWS, "electron rows of a pass exceed the warp");

@@ -378,7 +378,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
     }
   }
 
-  if (ORB == 3) {  // grad_i J for the caller (nuclear energy gradient: d B / d R needs it)
+  if (ORB == 3 || ORB == 4) {  // grad_i J for the caller (nuclear energy gradient: d B / d R needs it)
     double *sGJ = ws + GE::oGJ;
     sGJ[lane] = gJx;
     sGJ[32 + lane] = gJy;
@@ -740,7 +740,8 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       const int pg = pvalid ? (pr >> 1) : 0, sp = pr & 1;
       const int ns = sp ? n_dn : n_up, nv = P.nv[sp], e0 = sp ? n_up : 0;
       double a0[NS], av[NS], b0[EL ? NS : 1], bv[EL ? NS : 1];
-      double ai[ORB == 2 ? NS : 1];  // ORB = 2: identity block -> A0^-1
+      constexpr bool INV = (ORB == 2 || ORB == 4);  // identity block -> A0^-1
+      double ai[INV ? NS : 1];
       {
         const bool cA = c < ns, cV = c < nv;
         const int colA = cA ? P.ref_col[sp][c < kMaxSpin ? c : 0] : 0;
@@ -751,7 +752,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           const bool ri = i < ns;
           a0[i] = (ri && cA) ? sPhi[GE::moIdx(EL, row, colA)] : ((i == c) ? 1.0 : 0.0);  // identity padding
           av[i] = (ri && cV) ? sPhi[GE::moIdx(EL, row, colV)] : 0.0;
-          if (ORB == 2) ai[i] = (ri && cA && i == c) ? 1.0 : 0.0;
+          if (INV) ai[i] = (ri && cA && i == c) ? 1.0 : 0.0;
           if (EL) {
             b0[i] = (ri && cA) ? sB[GE::moIdx(EL, row, colA)] : 0.0;
             bv[i] = (ri && cV) ? sB[GE::moIdx(EL, row, colV)] : 0.0;
@@ -796,7 +797,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           av[k] = t;
 #pragma unroll
           for (int i = 0; i < NS; ++i) if (i != k) av[i] = fma(-f[i], t, av[i]);
-          if (ORB == 2) {
+          if (INV) {
             t = ai[k] * inv;
             ai[k] = t;
 #pragma unroll
@@ -827,7 +828,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
       // Arg-max on the high word of |T| (monotone for positive doubles; Inf and NaN of a singular reference sort above
       // every finite value, are clamped to +Inf and so flag the walker): kappa to a relative 2^-20.
       double kap = 0.0;
-      if (EL || ORB == 2) {
+      if (EL || INV) {
         unsigned kk = 0u;
 #pragma unroll
         for (int k = 0; k < NS; ++k) kk = max(kk, (unsigned)(__double2hiint(av[k]) & 0x7fffffff));  // columns c >= nv hold zeros
@@ -849,6 +850,13 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
 #pragma unroll
           for (int i = 0; i < NS; ++i) gs[c * NS + i] = b0[i];  // gs[j][k] = Gm[perm[k]][j]
         }
+        if (ORB == 4 && pvalid) {  // keep G = A0^-1 B0 and H = A0^-1 Bv in position order for the adjoint assembly
+#pragma unroll
+          for (int k = 0; k < NS; ++k) {
+            if (c < NS) (ws + GE::oX)[(pr * NS + perm[k]) * NS + c] = b0[k];
+            (ws + GE::oH)[(pr * NS + perm[k]) * LP + c] = bv[k];
+          }
+        }
         __syncwarp();
 #pragma unroll
         for (int k = 0; k < NS; ++k) {
@@ -864,7 +872,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
         for (int k = 0; k < NS; ++k) {
           if (EL) reinterpret_cast<double2 *>(sT)[pr * TS + perm[k] * RS + c] = make_double2(av[k], bv[EL ? k : 0]);
           else sT[pr * TS + perm[k] * RS + c] = av[k];
-          if (ORB == 2 && c < NS) (ws + GE::oInv)[(pr * NS + perm[k]) * NS + c] = ai[ORB == 2 ? k : 0];  // A0^-1[position][electron]
+          if (INV && c < NS) (ws + GE::oInv)[(pr * NS + perm[k]) * NS + c] = ai[INV ? k : 0];  // A0^-1[position][electron]
         }
         if (c == 0) {
           if (EL) {
@@ -876,7 +884,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           }
           sProb[pr * 4 + 0] = det;  // det A0 of this spin; the logarithm is taken once, of D0^up D0^dn (Sigma / D0)
           sProb[pr * 4 + 2] = t0;
-          if (EL || ORB == 2) sProb[pr * 4 + 3] = kap;
+          if (EL || INV) sProb[pr * 4 + 3] = kap;
         }
       }
     }
@@ -1012,6 +1020,111 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
         const bool ok = (den * den <= fmin(kFallbackK * scale, kFallbackCap)) && (ku * ku <= kthr) && (kd * kd <= kthr);
         sRes[wg * 4 + 3] = ok ? 0.0 : 1.0;
       }
+    }
+    if (ORB == 4) {
+      // ---- table route of the nuclear energy gradient: the two weight matrices of d_j K, K = F / den,
+      //   F = den (t0^up + t0^dn) + num,  d_j K = (d_j F - K d_j den) / den,
+      // by reverse differentiation through the tables T = A0^-1 Av, G = A0^-1 B0, H = A0^-1 Bv, M = H - G T:
+      //   Y = d den / d T = d num / d M,   Z = d num / d T   (gathered per table entry, lists built at setup)
+      //   Tbar = Z - (num/den) Y - G^T Y,  Hbar = Y,  Gbar = den 1 - Y T^T
+      //   d/dAv = A0^-T Tbar,  d/dBv = A0^-T Y,  d/dB0 = A0^-T Gbar,  d/dA0 = -A0^-T (Tbar T^T + Gbar G^T + Y H^T)
+      // written (divided by den) into Gamma (weights of d_j B) and Gamma2 (weights of d_j Phi).
+      static_assert(ORB != 4 || EL, "the energy-gradient tables need the operator rows");
+      double *sY = ws + GE::oY, *sZ = ws + GE::oZ, *sG1 = ws + GE::oGam, *sG2 = ws + GE::oGam2;
+      const double *sInvF = ws + GE::oInv, *sGm = ws + GE::oX, *sHm = ws + GE::oH;
+      for (int i = lane; i < 2 * G * TS; i += 32) { sY[i] = 0.0; sZ[i] = 0.0; }
+      for (int i = lane; i < GE::ROWS * NMO; i += 32) { sG1[i] = 0.0; sG2[i] = 0.0; }
+      if (wvalid && sub == 0) {
+        sProb[pu * 4 + 1] = num / den;
+        sProb[pd * 4 + 1] = den;
+      }
+      __syncwarp();
+      if (wvalid)
+        for (int t = sub; t < P.n_ytgt; t += LW) {
+          const int2 tg = __ldg(P.ytgt + t);
+          const int end = __ldg(P.ytgt + t + 1).y;
+          const bool dnT = tg.x >= TS;
+          const double *Ts = dnT ? Td : Tu, *To = dnT ? Tu : Td;
+          const double2 *TMs = reinterpret_cast<const double2 *>(Ts);
+          double accY = 0.0, accZ = 0.0;
+          for (int k = tg.y; k < end; ++k) {
+            const uint4 raw = __ldg(reinterpret_cast<const uint4 *>(P.yrec + k));
+            const double w = __hiloint2double((int)raw.y, (int)raw.x);
+            double Ro, Rdo;
+            excite_double<true>(raw.z, To, Ro, Rdo);
+            const double2 cf = TMs[raw.w & 0xffffu];
+            accY = fma(w * Ro, cf.x, accY);
+            accZ = fma(w, fma(Ro, cf.y, Rdo * cf.x), accZ);
+          }
+          sY[pu * TS + tg.x] = accY;
+          sZ[pu * TS + tg.x] = accZ;
+        }
+      __syncwarp();
+      const int c = lane % LP, slot = lane / LP;
+      for (int pass = 0; pass * PP < 2 * G; ++pass) {
+        const int pr = pass * PP + slot;
+        if (pr < 2 * G) {
+          const int pg = pr >> 1, sp = pr & 1;
+          const int ns = sp ? n_dn : n_up, nv = P.nv[sp], e0 = sp ? n_up : 0;
+          if (c < ns) {
+            const double rnd = sProb[(pr & ~1) * 4 + 1], dn_ = sProb[(pr | 1) * 4 + 1], iden = 1.0 / dn_;
+            const double2 *TM = reinterpret_cast<const double2 *>(sT) + pr * TS;
+            const int row = (pg * ne + e0 + c) * NMO;
+            double ainv[NS], ag[NS];
+#pragma unroll
+            for (int p = 0; p < NS; ++p) ainv[p] = (p < ns) ? sInvF[(pr * NS + p) * NS + c] : 0.0;
+#pragma unroll
+            for (int p2 = 0; p2 < NS; ++p2) {
+              double t = 0.0;
+#pragma unroll
+              for (int p = 0; p < NS; ++p)
+                if (p < ns && p2 < ns) t = fma(sGm[(pr * NS + p2) * NS + p], ainv[p], t);
+              ag[p2] = t;
+            }
+            double avq[kMaxVirt], bvq[kMaxVirt];
+#pragma unroll
+            for (int q = 0; q < kMaxVirt; ++q) {
+              avq[q] = bvq[q] = 0.0;
+              if (q < nv) {
+                double tb = 0.0, ta = 0.0;
+                for (int p = 0; p < ns; ++p) {
+                  const double yv = sY[pr * TS + p * RS + q], zv = sZ[pr * TS + p * RS + q];
+                  tb = fma(ainv[p], yv, tb);
+                  ta = fma(fma(-rnd, ainv[p], -ag[p]), yv, fma(ainv[p], zv, ta));
+                }
+                bvq[q] = tb;
+                avq[q] = ta;
+                sG1[row + P.virt_col[sp][q]] = tb * iden;
+                sG2[row + P.virt_col[sp][q]] = ta * iden;
+              }
+            }
+            double b0j[NS];
+#pragma unroll
+            for (int j = 0; j < NS; ++j) {
+              double t = dn_ * ainv[j];
+#pragma unroll
+              for (int q = 0; q < kMaxVirt; ++q)
+                if (q < nv && j < ns) t = fma(-bvq[q], TM[j * RS + q].x, t);
+              b0j[j] = (j < ns) ? t : 0.0;
+            }
+#pragma unroll
+            for (int j = 0; j < NS; ++j) {
+              if (j < ns) {
+                double t = 0.0;
+#pragma unroll
+                for (int q = 0; q < kMaxVirt; ++q)
+                  if (q < nv) t = fma(-avq[q], TM[j * RS + q].x, fma(-bvq[q], sHm[(pr * NS + j) * LP + q], t));
+#pragma unroll
+                for (int p2 = 0; p2 < NS; ++p2)
+                  if (p2 < ns) t = fma(-b0j[p2], sGm[(pr * NS + j) * NS + p2], t);
+                sG1[row + P.ref_col[sp][j]] = b0j[j] * iden;
+                sG2[row + P.ref_col[sp][j]] = t * iden;
+              }
+            }
+          }
+        }
+      }
+      __syncwarp();
     }
     if (ORB == 2) {
       // ---- Gamma = d ln Sigma / d Phi from the reference alone (lane c of a problem = electron c of that spin):

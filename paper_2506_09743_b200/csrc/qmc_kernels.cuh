@@ -540,14 +540,30 @@ __global__ void __launch_bounds__(WPB * 32, 1)
     } else {
       dummy_xyz(lane, x, y, z);
     }
-    eval_walkers<NS, NMO, true, X, true, false, false, 3>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
-    // G1 = Gamma / Sigma, G2 = (Gamma2 - K Gamma) / Sigma, K = sum w t / Sigma
-    for (int i = lane; i < G * ne * NMO; i += 32) {
-      const int gg = i / (ne * NMO);
-      const double sig = sRes[gg * 4 + 0], K = sRes[gg * 4 + 1] / sig;
-      const double g1 = sGam[i] / sig;
-      sGam2[i] = sGam2[i] / sig - K * g1;
-      sGam[i] = g1;
+    // The two weight matrices G1 (of d_j B) and G2 (of d_j Phi): from the reference's tables (one elimination per
+    // spin, eval_walkers<..., ORB = 4>); for a group with a walker whose reference is nearly singular (the E_L flag, or
+    // (Sigma/D_0)^2 > kFallbackOrb, kappa^2 > kFallbackOrbKappa) and for expansions with general determinants, from
+    // every determinant's own elimination (ORB = 3): G1 = Gamma / Sigma, G2 = (Gamma2 - K Gamma) / Sigma.
+    bool expl = P.n_gen > 0;
+    if (!expl) {
+      eval_walkers<NS, NMO, true, X, false, false, false, 4>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
+      const double *sProb = ws + GE::oProb;
+      for (int gg = 0; gg < G; ++gg) {
+        const double den = sProb[(2 * gg + 1) * 4 + 1], ku = sProb[(2 * gg) * 4 + 3], kd = sProb[(2 * gg + 1) * 4 + 3];
+        expl |= (sRes[gg * 4 + 3] != 0.0) || !(den * den <= kFallbackOrb) || !(ku * ku <= kFallbackOrbKappa) ||
+                !(kd * kd <= kFallbackOrbKappa);
+      }
+      __syncwarp();
+    }
+    if (expl) {
+      eval_walkers<NS, NMO, true, X, true, false, false, 3>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
+      for (int i = lane; i < G * ne * NMO; i += 32) {
+        const int gg = i / (ne * NMO);
+        const double sig = sRes[gg * 4 + 0], K = sRes[gg * 4 + 1] / sig;
+        const double g1 = sGam[i] / sig;
+        sGam2[i] = sGam2[i] / sig - K * g1;
+        sGam[i] = g1;
+      }
     }
     const double gJx = sGJ[lane], gJy = sGJ[32 + lane], gJz = sGJ[64 + lane];
     __syncwarp();

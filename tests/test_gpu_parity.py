@@ -1404,3 +1404,43 @@ def test_fused_energy_gradient_with_listed_groups_and_at_full_size(env):
     scale = np.maximum(np.abs(g), 1e-3 * np.max(np.abs(g)))
     assert abs(evf - ev) <= 1e-12 * abs(ev) and np.max(np.abs(gf - g) / scale) < 1e-9, np.max(np.abs(gf - g) / scale)
     s.close()
+
+
+def test_nuclear_energy_gradient_full_size_sampled_and_translation_invariance(env):
+    """CO at the size bench.py times the call (32768 walkers, initial and after 30 sweeps): sampled walkers against the
+    oracle with adjudication; on every walker translation invariance, sum_alpha grad_alpha E_L = -sum_i grad_i E_L, the
+    right side by Richardson central differences of the GPU's own E_L under a rigid shift of all electrons."""
+    torch, ob, qb = env
+    M = 32768
+    d, r = wl.co(M=M)
+    s = qb.QmcSystem(d)
+    o, ox = ob.OracleSystem(d), ob.OracleSystem(d, extended=True)
+    nt = os.cpu_count() or 8
+    rg = _to_gpu(torch, r)
+    for stage in ("initial", "equilibrated"):
+        if stage == "equilibrated":
+            s.metropolis(rg, 0.2, 30, seed=9)
+        g = s.nuclear_energy_gradient(rg, d.n_atoms)
+        lp = s.log_psi(rg)[0].cpu().numpy()
+        rr = rg.cpu().numpy()
+        idx = np.unique(np.concatenate([np.arange(0, 32), np.arange(M - 33, M), np.random.default_rng(3).integers(0, M, 448)]))
+        rs = np.ascontiguousarray(rr[:, :, idx])
+        g0, gx = ob.nuclear_energy_gradient(o, rs, threads=nt), ob.nuclear_energy_gradient(ox, rs, threads=nt)
+        keep = lp[idx] - lp.max() > math.log(1e-6)
+        n_exc = adjudicate(g.cpu().numpy()[idx], g0, gx, 1e-8, scale=np.maximum(1.0, np.abs(gx)), mask=keep, what=f"grad_alpha E_L ({stage})")
+        assert n_exc <= 8, n_exc
+        # translation invariance on every walker
+        def el_shift(c, t):
+            r2 = rg.clone()
+            r2[:, c, :] += t
+            return s.local_energy(r2)[2]
+        tot = g.sum(dim=1)
+        good = torch.from_numpy(lp - lp.max() > math.log(1e-6)).cuda()
+        for c in range(3):
+            cd = lambda h: (el_shift(c, h) - el_shift(c, -h)) / (2 * h)
+            a, b = cd(1e-4), cd(2e-4)
+            ref = -(4 * a - b) / 3
+            ok = good & ((a - b).abs() <= 1e-5 * torch.clamp(ref.abs(), min=1.0))   # where the two step sizes agree
+            err = ((tot[:, c] - ref).abs() / torch.clamp(ref.abs(), min=1.0))[ok]
+            assert float(ok.float().mean()) > 0.15 and float(err.max()) < 1e-5, (stage, c, float(ok.float().mean()), float(err.max()))
+    s.close()
