@@ -1444,3 +1444,25 @@ def test_nuclear_energy_gradient_full_size_sampled_and_translation_invariance(en
             err = ((tot[:, c] - ref).abs() / torch.clamp(ref.abs(), min=1.0))[ok]
             assert float(ok.float().mean()) > 0.15 and float(err.max()) < 1e-5, (stage, c, float(ok.float().mean()), float(err.max()))
     s.close()
+
+
+def test_h2_force_is_along_the_axis_and_antisymmetric(env):
+    """eq. 7 on the H2 config (the force component along the molecular axis): 131072 walkers equilibrated
+    on the GPU; by the symmetry of the molecule the force has no x, y component and F_z(A) = -F_z(B), both within the
+    statistical error of the estimator (per-walker terms from the GPU, standard error over walkers)."""
+    torch, ob, qb = env
+    d, r = wl.h2(M=131072)
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    s.metropolis(rg, 0.5, 60, seed=21)
+    lp, sg, el = s.local_energy(rg)
+    dE = s.nuclear_energy_gradient(rg, 2)
+    dl = s.nuclear_log_gradient(rg, 2)
+    F, T = qb.force(el, dE, dl)
+    per = -(dE + 2.0 * (el - el.mean())[:, None, None] * dl)
+    sig = (per.std(dim=0) / math.sqrt(per.shape[0])).cpu().numpy()
+    assert np.all(np.abs(F[:, :2]) < 5 * sig[:, :2] + 1e-12), (F, sig)
+    both = per[:, 0, 2] + per[:, 1, 2]
+    assert abs(F[0, 2] + F[1, 2]) < 5 * float(both.std() / math.sqrt(both.numel())), (F, sig)
+    assert np.all(np.isfinite(F)) and abs(F[0, 2]) < 1.0
+    s.close()
