@@ -30,9 +30,10 @@ constexpr int kMaxEen = 6;    // terms of the electron-electron-nucleus Jastrow 
 #define QMC_EARLY_INV 0      // Gauss-Jordan: invert every pivot candidate before the arg-max is known
 #endif
 #ifndef QMC_WARPS_PSI
-#define QMC_WARPS_PSI 12     // warps per block of the values-only kernels (log|Psi|, Metropolis): 24 warps per SM at 80 registers
-                             // (96 bytes of spills) with the compact scratch layout; measured 5.62 ms per 20 CO sweeps against
-                             // 5.69 with 10 warps per block (96 registers, no spills)
+#define QMC_WARPS_PSI 14     // warps per block of the values-only kernels (log|Psi|, Metropolis): 28 warps per SM at 72 registers
+                             // (172 bytes of spills) with the compact scratch layout, the most that fits two blocks per SM;
+                             // measured per 20 CO sweeps: 10 warps (96 registers, no spills) 5.69 ms, 12 (80 registers) 5.62 /
+                             // 5.52 after the record-stream change, 14: 5.39, 16 (one block per SM): 6.46
 #endif
 #ifndef QMC_WARPS_ORB
 #define QMC_WARPS_ORB 10     // warps per block of the orbital-derivative kernel (one block per SM; 8 when shared memory is short).
