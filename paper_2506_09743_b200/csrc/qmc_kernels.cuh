@@ -348,6 +348,68 @@ __global__ void __launch_bounds__(WPB * 32, 1)
         __syncwarp();
         // kernel-order (N C)[R][col] from the DMMA B-fragment table: [chunk][k-step][MO tile][4 n + k]
         const double *cfr = sC + chunk * ((kChunk / 4) * NT * 32);
+        if (!nuc) {
+          // Parameter mode on the FP64 tensor cores: per walker, D[AO row][MO] = sum_i tile[AO row][electron i] Gamma[i][MO]
+          // with mma.m8n8k4 -- A fragments straight from the tile (rows = AO rows, k = the walker's electrons, four at a
+          // time; columns past the walker's last electron meet zero rows of B), B fragments from Gamma, the D fragments
+          // scaled and written out: dC from the value columns, dzeta = sum_MO (N C)[row][MO] D_zeta[row][MO] from the
+          // operator columns (reduced over the four lanes that share a row).
+          const int fr = lane >> 2, fk = lane & 3;
+          constexpr int KS = (2 * NS + 3) / 4;
+          for (int gg = 0; gg < G; ++gg) {
+            const int64_t wo = grp * G + gg;
+            double accv[2][NT][2], accz[2][NT][2];
+#pragma unroll
+            for (int m = 0; m < 2; ++m)
+#pragma unroll
+              for (int t = 0; t < NT; ++t) accv[m][t][0] = accv[m][t][1] = accz[m][t][0] = accz[m][t][1] = 0.0;
+#pragma unroll
+            for (int ks = 0; ks < KS; ++ks) {
+              const int ie = 4 * ks + fk;                        // electron of this lane's A column / B row
+              const int iec = (ie < ne) ? ie : (ne - 1);         // any finite tile cell where B is zero
+              double bfr[NT];
+#pragma unroll
+              for (int t = 0; t < NT; ++t) {
+                const int col = 8 * t + fr;                      // B fragment: lane 4 n + k holds B[k][n]
+                bfr[t] = (ie < ne && col < NMO) ? sGam[(gg * ne + ie) * NMO + col] : 0.0;
+              }
+#pragma unroll
+              for (int m = 0; m < 2; ++m) {
+                const double av = tile[(8 * m + fr) * S + gg * ne + iec];
+                const double az = tile[(8 * m + fr) * S + GE::opCol(gg * ne + iec)];
+#pragma unroll
+                for (int t = 0; t < NT; ++t) {
+                  dmma884(accv[m][t][0], accv[m][t][1], av, bfr[t]);
+                  dmma884(accz[m][t][0], accz[m][t][1], az, bfr[t]);
+                }
+              }
+            }
+            // D fragment: lane 4 r + k holds D[r][2k], D[r][2k + 1]
+#pragma unroll
+            for (int m = 0; m < 2; ++m) {
+              const int rw = 8 * m + fr, R = chunk * kChunk + rw, beta = P.ao_orig[R];
+              double zsum = 0.0;
+#pragma unroll
+              for (int t = 0; t < NT; ++t)
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                  const int col = 8 * t + 2 * fk + j;
+                  if (col < NMO && col < P.n_mo) {
+                    const double cf = cfr[(((rw >> 2) * NT) + (col >> 3)) * 32 + 4 * (col & 7) + (rw & 3)];
+                    zsum = fma(cf, accz[m][t][j], zsum);
+                    if (dC && beta >= 0 && wo < io.M)
+                      dC[(wo * P.n_ao + beta) * P.n_mo_all + P.mo_orig[col]] = P.ao_nrm[R] * accv[m][t][j];
+                  }
+                }
+              zsum += shfl_xor_d(zsum, 1);
+              zsum += shfl_xor_d(zsum, 2);
+              if (dZ && fk == 0 && beta >= 0 && wo < io.M) dZ[wo * P.n_ao + beta] = zsum;
+            }
+          }
+          __syncwarp();
+          ++chunk;
+          continue;
+        }
         // lane <-> (walker gg, MO column): Gamma's column in registers, the tile rows read as broadcasts;
         // dzeta sums its columns across the NMO lanes of a walker
         constexpr int CW = NMO <= 2 ? 2 : (NMO <= 4 ? 4 : (NMO <= 8 ? 8 : 16));  // aligned power-of-two lane block per walker
