@@ -337,10 +337,13 @@ __global__ void __launch_bounds__(WPB * 32, 1)
           dax[0] = gx[m < 5 ? m : 0];
         }
       }
-      for (int t = 0; t < nf; ++t) {
-        const double phi = gr * ang[t];
-        tl[(row + t) * S] = nuc ? fma(gr, dax[t], phi * radx) : phi;
-        tz[(row + t) * S] = nuc ? fma(gr, dang[t], phi * radc) : phi * zf;
+#pragma unroll
+      for (int t = 0; t < 5; ++t) {  // unrolled: ang / dang / dax stay in registers
+        if (t < nf) {
+          const double phi = gr * ang[t];
+          tl[(row + t) * S] = nuc ? fma(gr, dax[t], phi * radx) : phi;
+          tz[(row + t) * S] = nuc ? fma(gr, dang[t], phi * radc) : phi * zf;
+        }
       }
       const int flush = meta >> 20;
       if (flush) {
@@ -410,68 +413,99 @@ __global__ void __launch_bounds__(WPB * 32, 1)
           ++chunk;
           continue;
         }
-        // lane <-> (walker gg, MO column): Gamma's column in registers, the tile rows read as broadcasts;
-        // dzeta sums its columns across the NMO lanes of a walker
-        constexpr int CW = NMO <= 2 ? 2 : (NMO <= 4 ? 4 : (NMO <= 8 ? 8 : 16));  // aligned power-of-two lane block per walker
-        static_assert(NMO <= CW, "at most 16 MO columns");
-        for (int pi = lane; pi < ((G * CW + 31) & ~31); pi += 32) {
-          const int gq = pi / CW, col = pi & (CW - 1);
-          const bool pv = gq < G && col < NMO;
-          const int gg = pv ? gq : 0;
-          const int64_t wo = grp * G + gg;
-          const bool ok = pv && col < P.n_mo && wo < io.M;
-          double gam[2 * NS];
+        {
+          // Nuclear mode on the FP64 tensor cores: the same contraction on both column sets (pass 0: d/dx in the value
+          // columns, d/dy in the operator columns; pass 1: d/dz in the operator columns), each D row multiplied by its
+          // (N C) row and summed over the MOs, the row sums parked in the (now dead) tile, then one lane per (walker,
+          // column set) adds the rows of each centre in row order and subtracts them from dR: the same lane owns the same
+          // output in every chunk and pass, so its read-modify-writes are ordered.
+          const int fr = lane >> 2, fk = lane & 3;
+          constexpr int KS = (2 * NS + 3) / 4;
+          double rs[2][GE::GMAX][2];  // [column set][walker][M-tile]
 #pragma unroll
-          for (int i = 0; i < 2 * NS; ++i) gam[i] = (pv && i < ne) ? sGam[(gg * ne + i) * NMO + col] : 0.0;
-          const int64_t orow = wo * P.n_ao;
-          const int ocol = P.mo_orig[col < NMO ? col : 0];
-          double racc = 0.0, racx = 0.0;  // nuclear mode: running sums (component comp, x) over the rows of centre cur
-          int cur = -1;
-          for (int rw = 0; rw < kChunk; ++rw) {
-            const int R = chunk * kChunk + rw, beta = P.ao_orig[R];
-            if (beta < 0) continue;
-            const double *trow = tile + rw * S;
-            double t = 0.0, u = 0.0;
+          for (int gg = 0; gg < GE::GMAX; ++gg) {
+            rs[0][gg][0] = rs[0][gg][1] = rs[1][gg][0] = rs[1][gg][1] = 0.0;
+            if (gg < G) {
+              double accv[2][NT][2], accz[2][NT][2];
 #pragma unroll
-            for (int i = 0; i < 2 * NS; ++i)
-              if (i < ne) {
-                if (!nuc || pass == 0) t = fma(trow[gg * ne + i], gam[i], t);
-                u = fma(trow[GE::opCol(gg * ne + i)], gam[i], u);
-              }
-            if (dC && ok) dC[(orow + beta) * P.n_mo_all + ocol] = P.ao_nrm[R] * t;
-            if (dZ || nuc) {
-              // kernel-order (N C)[R][col] from the DMMA B-fragment table
-              const double cf = ok ? cfr[(((rw >> 2) * NT) + (col >> 3)) * 32 + 4 * (col & 7) + (rw & 3)] : 0.0;
-              double a = cf * u;
+              for (int m = 0; m < 2; ++m)
 #pragma unroll
-              for (int m = 1; m < CW; m <<= 1) a += shfl_xor_d(a, m);
-              if (nuc) {
-                double ax = (pass == 0) ? cf * t : 0.0;
-                if (pass == 0) {
+                for (int t = 0; t < NT; ++t) accv[m][t][0] = accv[m][t][1] = accz[m][t][0] = accz[m][t][1] = 0.0;
 #pragma unroll
-                  for (int m = 1; m < CW; m <<= 1) ax += shfl_xor_d(ax, m);
+              for (int ks = 0; ks < KS; ++ks) {
+                const int ie = 4 * ks + fk;
+                const int iec = (ie < ne) ? ie : (ne - 1);
+                double bfr[NT];
+#pragma unroll
+                for (int t = 0; t < NT; ++t) {
+                  const int col = 8 * t + fr;
+                  bfr[t] = (ie < ne && col < NMO) ? sGam[(gg * ne + ie) * NMO + col] : 0.0;
                 }
-                // the same lane owns walker gg in every chunk and pass, so its read-modify-writes are ordered
-                const int at = row_atom[R];
-                if (at != cur) {
-                  if (cur >= 0 && pv && col == 0 && wo < io.M) {
-                    dRo[(wo * P.n_atoms + cur) * 3 + comp] -= racc;
-                    if (pass == 0) dRo[(wo * P.n_atoms + cur) * 3] -= racx;
+#pragma unroll
+                for (int m = 0; m < 2; ++m) {
+                  const double av = tile[(8 * m + fr) * S + gg * ne + iec];
+                  const double az = tile[(8 * m + fr) * S + GE::opCol(gg * ne + iec)];
+#pragma unroll
+                  for (int t = 0; t < NT; ++t) {
+                    if (pass == 0) dmma884(accv[m][t][0], accv[m][t][1], av, bfr[t]);
+                    dmma884(accz[m][t][0], accz[m][t][1], az, bfr[t]);
                   }
-                  cur = at;
-                  racc = 0.0;
-                  racx = 0.0;
                 }
-                racc += a;
-                racx += ax;
-              } else if (pv && col == 0 && wo < io.M) {
-                dZ[orow + beta] = a;
+              }
+#pragma unroll
+              for (int m = 0; m < 2; ++m) {
+                const int rw = 8 * m + fr;
+                double sv = 0.0, sz = 0.0;
+#pragma unroll
+                for (int t = 0; t < NT; ++t)
+#pragma unroll
+                  for (int j2 = 0; j2 < 2; ++j2) {
+                    const int col = 8 * t + 2 * fk + j2;
+                    if (col < NMO && col < P.n_mo) {
+                      const double cf = cfr[(((rw >> 2) * NT) + (col >> 3)) * 32 + 4 * (col & 7) + (rw & 3)];
+                      sv = fma(cf, accv[m][t][j2], sv);
+                      sz = fma(cf, accz[m][t][j2], sz);
+                    }
+                  }
+                sv += shfl_xor_d(sv, 1); sv += shfl_xor_d(sv, 2);
+                sz += shfl_xor_d(sz, 1); sz += shfl_xor_d(sz, 2);
+                rs[0][gg][m] = sv;
+                rs[1][gg][m] = sz;
               }
             }
           }
-          if (nuc && cur >= 0 && pv && col == 0 && wo < io.M) {
-            dRo[(wo * P.n_atoms + cur) * 3 + comp] -= racc;
-            if (pass == 0) dRo[(wo * P.n_atoms + cur) * 3] -= racx;
+          __syncwarp();  // every lane is done reading the tile: park the row sums [column set][walker][16 rows] in it
+          if (fk == 0) {
+#pragma unroll
+            for (int gg = 0; gg < GE::GMAX; ++gg)
+              if (gg < G) {
+#pragma unroll
+                for (int m = 0; m < 2; ++m) {
+                  tile[(0 * G + gg) * kChunk + 8 * m + fr] = rs[0][gg][m];
+                  tile[(1 * G + gg) * kChunk + 8 * m + fr] = rs[1][gg][m];
+                }
+              }
+          }
+          __syncwarp();
+          for (int item = lane; item < 2 * G; item += 32) {
+            const int cset = item / G, gg = item - cset * G;
+            const int64_t wo = grp * G + gg;
+            if ((cset == 0 && pass != 0) || wo >= io.M) continue;
+            const int cidx = (cset == 0) ? 0 : comp;
+            double racc = 0.0;
+            int cur = -1;
+            for (int rw = 0; rw < kChunk; ++rw) {
+              const int R = chunk * kChunk + rw;
+              if (P.ao_orig[R] < 0) continue;
+              const int at = row_atom[R];
+              if (at != cur) {
+                if (cur >= 0) dRo[(wo * P.n_atoms + cur) * 3 + cidx] -= racc;
+                cur = at;
+                racc = 0.0;
+              }
+              racc += tile[(cset * G + gg) * kChunk + rw];
+            }
+            if (cur >= 0) dRo[(wo * P.n_atoms + cur) * 3 + cidx] -= racc;
           }
         }
         __syncwarp();
