@@ -44,6 +44,7 @@ extern "C" {
 #define QMC_EUNSUPPORTED (-2) /* valid problem outside the compiled limits (see qmc_setup) */
 #define QMC_ECUDA (-3)        /* a CUDA runtime call failed */
 #define QMC_ENOMEM (-4)       /* host allocation failed */
+#define QMC_ETOOLARGE (-5)    /* size beyond the fixed scratch of the allocation-free entry point */
 
 typedef struct qmc_system qmc_system_t; /* opaque */
 
@@ -190,6 +191,22 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
  *   d_x device in [M]; h_mean, h_stderr host out (either may be NULL).
  * Deterministic (fixed reduction tree, compensated).  Synchronises cuda_stream. */
 int qmc_batch_stats(const double *d_x, int64_t M, double *h_mean, double *h_stderr, void *cuda_stream);
+
+/* The allocation-free entry point: qmc_batch_stats for callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid allocation).  Same reduction, same kernel, but the scratch (block
+ * partials and the completion counter) is a fixed file-scope device array of 6400 bytes that every GPU that loads the
+ * library holds until the process exits, and the result stays on the device:
+ *   d_x   device in  [M], 1 <= M <= 67 108 864 (2^26); a larger M is rejected with QMC_ETOOLARGE
+ *   d_out device out [2] = {mean, standard error of the mean}
+ * Calls no cudaMalloc / cudaFree / allocating routine; asynchronous on cuda_stream (one 4-byte memset node and one
+ * kernel).  qmc_static_scratch_init(device) resolves the array's device address (cudaGetSymbolAddress, once per
+ * device); the first qmc_batch_stats_static call on a device does it itself, so call it beforehand when that first call
+ * would fall inside a graph capture.  EVERY call on a device shares the one array, which keeps the last call's
+ * contents (the call clears what must start at zero): calls that overlap on the GPU -- two streams, or two replays of
+ * a captured graph in flight -- race; serialise them.  Deterministic; results equal qmc_batch_stats' up to the
+ * rounding order of a different block count. */
+int qmc_static_scratch_init(int device);
+int qmc_batch_stats_static(const double *d_x, int64_t M, double *d_out, void *cuda_stream);
 
 /* ---- the factors of the gradient estimator, eq. 6 ----
  * Variational parameters handled: theta = (jastrow_a_par, jastrow_a_anti, jastrow_b, jastrow_en_w0,

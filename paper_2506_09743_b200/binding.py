@@ -11,13 +11,14 @@ import torch
 
 from . import build as _build
 
-QMC_OK, QMC_EINVAL, QMC_EUNSUPPORTED, QMC_ECUDA, QMC_ENOMEM = 0, -1, -2, -3, -4
+QMC_OK, QMC_EINVAL, QMC_EUNSUPPORTED, QMC_ECUDA, QMC_ENOMEM, QMC_ETOOLARGE = 0, -1, -2, -3, -4, -5
 _lib = None
 
 EXPORTS = ["qmc_setup", "qmc_destroy", "qmc_local_energy", "qmc_log_psi", "qmc_metropolis", "qmc_batch_stats",
            "qmc_fp64_peak", "qmc_model_flops", "qmc_launch_count", "qmc_status_string", "qmc_n_param", "qmc_local_energy_explicit", "qmc_set_kernel_timing", "qmc_kernel_times",
            "qmc_log_derivatives", "qmc_energy_gradient", "qmc_local_energy_host", "qmc_orbital_derivatives",
-           "qmc_nuclear_log_gradient", "qmc_nuclear_energy_gradient", "qmc_force", "qmc_local_energy_gradient"]
+           "qmc_nuclear_log_gradient", "qmc_nuclear_energy_gradient", "qmc_force", "qmc_local_energy_gradient",
+           "qmc_static_scratch_init", "qmc_batch_stats_static"]
 
 
 class QmcError(RuntimeError):
@@ -81,6 +82,10 @@ def lib():
         L.qmc_metropolis.argtypes = [vp, vp, i64, dbl, C.c_int32, C.c_uint64, C.c_uint64, i64, vp, vp, vp, vp, vp, vp]
         L.qmc_batch_stats.restype = C.c_int
         L.qmc_batch_stats.argtypes = [vp, i64, vp, vp, vp]
+        L.qmc_static_scratch_init.restype = C.c_int
+        L.qmc_static_scratch_init.argtypes = [C.c_int]
+        L.qmc_batch_stats_static.restype = C.c_int
+        L.qmc_batch_stats_static.argtypes = [vp, i64, vp, vp]
         L.qmc_fp64_peak.restype = C.c_int
         L.qmc_fp64_peak.argtypes = [C.c_int, C.c_int, C.c_int, vp]
         L.qmc_model_flops.restype = dbl
@@ -303,6 +308,15 @@ def batch_stats(x, stream=None):
     m, s = C.c_double(), C.c_double()
     _check(lib().qmc_batch_stats(_dp(x), x.numel(), C.addressof(m), C.addressof(s), _stream(stream)))
     return m.value, s.value
+
+
+def batch_stats_static(x, out, stream=None):
+    """qmc_batch_stats_static: the allocation-free variant; out = float64 cuda tensor [2] supplied by the caller receives
+    {mean, standard error}.  Asynchronous; at most 2^26 values; calls on one device must not overlap on the GPU."""
+    assert x.is_cuda and x.dtype == torch.float64 and x.is_contiguous()
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == 2
+    _check(lib().qmc_batch_stats_static(_dp(x), x.numel(), _dp(out), _stream(stream)))
+    return out
 
 
 def energy_gradient(eloc, O, stream=None):

@@ -167,6 +167,19 @@ int reduce_scratch(int dev, cudaStream_t st, size_t n_param, size_t gpart, Reduc
   return QMC_OK;
 }
 
+// ---- qmc_batch_stats_static: the allocation-free entry point.  Its scratch (block partials {n, mean, M2} of
+// batch_stats_kernel, then the completion counter) is this file-scope device array: every GPU that loads the library
+// holds these kStaticScratchBytes until the process exits.  In host code the array's NAME is a host-side stand-in, not
+// a device address; the address comes from cudaGetSymbolAddress, once per device, with that device current.
+constexpr int kStaticBlocks = 256;                                   // blocks of the launch = partials held
+constexpr int64_t kStaticMaxM = (int64_t)1 << 26;                    // 67 108 864 values (512 MiB of doubles)
+constexpr size_t kStaticPartialBytes = sizeof(double) * 3 * kStaticBlocks;
+constexpr size_t kStaticScratchBytes = kStaticPartialBytes + 256;    // + the counter, on its own 256-byte line
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+unsigned char *g_static_ptr[kStaticMaxDevices] = {};                 // device address of g_static_scratch, per device
+
 double sto_norm(int n, int l, int m, double zeta) {
   double fact = 1.0;
   for (int i = 2; i <= 2 * n; ++i) fact *= i;
@@ -228,6 +241,7 @@ const char *qmc_status_string(int status) {
     case QMC_EINVAL: return "invalid argument";
     case QMC_EUNSUPPORTED: return "problem outside the compiled limits";
     case QMC_ENOMEM: return "host allocation failed";
+    case QMC_ETOOLARGE: return "size beyond the fixed scratch of the allocation-free entry point (qmc_batch_stats_static: M <= 67108864)";
     case QMC_ECUDA: return g_cuda_err.empty() ? "CUDA error" : g_cuda_err.c_str();
     default: return "unknown status";
   }
@@ -1347,6 +1361,40 @@ int qmc_batch_stats(const double *d_x, int64_t M, double *h_mean, double *h_stde
   CK(cudaStreamSynchronize(st));  // the last block wrote {mean, stderr} into mapped host memory
   if (h_mean) *h_mean = r->h_res[0];
   if (h_stderr) *h_stderr = r->h_res[1];
+  return QMC_OK;
+}
+
+int qmc_static_scratch_init(int device) {
+  if (device < 0 || device >= kStaticMaxDevices) return QMC_EINVAL;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (g_static_ptr[device]) return QMC_OK;
+  CK(cudaSetDevice(device));
+  unsigned char *ptr = nullptr;
+  CK(cudaGetSymbolAddress((void **)&ptr, g_static_scratch));  // with `device` current: this device's copy of the array
+  if (!ptr) return QMC_ECUDA;
+  g_static_ptr[device] = ptr;
+  return QMC_OK;
+}
+
+int qmc_batch_stats_static(const double *d_x, int64_t M, double *d_out, void *cuda_stream) {
+  if (!d_x || !d_out || M <= 0) return QMC_EINVAL;
+  if (M > kStaticMaxM) return QMC_ETOOLARGE;  // beyond the fixed scratch's stated limit
+  int dev = 0;
+  if (int rc = device_of(d_x, &dev)) return rc;
+  if (dev < 0 || dev >= kStaticMaxDevices) return QMC_EINVAL;
+  if (!g_static_ptr[dev])
+    if (int rc = qmc_static_scratch_init(dev)) return rc;
+  CK(cudaSetDevice(dev));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  unsigned char *base = g_static_ptr[dev];
+  double *partial = reinterpret_cast<double *>(base);
+  unsigned int *done = reinterpret_cast<unsigned int *>(base + kStaticPartialBytes);
+  // the array keeps the last call's contents: the counter must start at zero (the partials are overwritten before read)
+  CK(cudaMemsetAsync(done, 0, sizeof(unsigned int), st));
+  const int nblk = (int)std::min<int64_t>(kStaticBlocks, (M + kStatsThreads - 1) / kStatsThreads);
+  batch_stats_kernel<<<nblk, kStatsThreads, 0, st>>>(d_x, M, partial, done, d_out);
+  CK(cudaGetLastError());
+  ++g_launches;
   return QMC_OK;
 }
 
