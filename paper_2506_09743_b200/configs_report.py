@@ -4,7 +4,9 @@
 
 Per configuration: device time of qmc_local_energy (walker*E_L/s) and of qmc_metropolis with the
 configuration's own sweep count and step (walker-steps/s), both as model FP64 TFLOP/s (qmc_model_flops) and as
-a fraction of the DFMA peak measured in the same process.  Configuration 5 (CO dissociation scan) runs its 50
+a fraction of the FP64 peak measured in the same process (the largest of the DFMA and DMMA microbenchmarks of
+qmc_fp64_peak: one pipe); the sampler + E_L pair is also timed as one captured CUDA graph (the way to run the
+launch-bound small systems).  Configuration 5 (CO dissociation scan) runs its 50
 sweeps with E_L after every sweep and reports mean E_L and its standard error per geometry (DESIGN.md reading
 Q16: per-walker sweep average first, then the standard error over walkers; no burn-in is discarded -- this is a
 throughput and parity benchmark, not a physics result).  CUDA events on the current stream around 10 back-to-back calls, 3 warm-ups,
@@ -63,12 +65,35 @@ def measure(name, d, r_host, peak):
     t_O = _time(lambda: s.log_derivatives(rd, O=O))
     t_orb = _time(lambda: s.orbital_derivatives(rd, d.n_ao, d.n_mo))
     t_nuc = _time(lambda: s.nuclear_log_gradient(rd, d.n_atoms))
+    t_frc = _time(lambda: s.nuclear_energy_gradient(rd, d.n_atoms))
+    t_fuse = _time(lambda: s.local_energy_gradient(rd))
+    # sampler + E_L as one CUDA graph (no allocation after the warm-up calls above), replayed back to back
+    st = torch.cuda.Stream()
+    st.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(st):
+        s.metropolis(r, step, sweeps, seed=1, logpsi=lp, sign=sg, stream=st)
+        s.local_energy(r, lp, sg, el, stream=st)
+        st.synchronize()
+        g = torch.cuda.CUDAGraph()
+        g.capture_begin()
+        s.metropolis(r, step, sweeps, seed=1, logpsi=lp, sign=sg, stream=st)
+        s.local_energy(r, lp, sg, el, stream=st)
+        g.capture_end()
+    torch.cuda.current_stream().wait_stream(st)
+    t_graph = _time(lambda: g.replay())
+
+    def eager_pair():
+        s.metropolis(r, step, sweeps, seed=1, logpsi=lp, sign=sg)
+        s.local_energy(r, lp, sg, el)
+
+    t_pair = _time(eager_pair)
     f_el, f_st = s.model_flops(0), s.model_flops(1)
     row = dict(config=name, n_e=d.n_e, n_ao=d.n_ao, n_mo=d.n_mo, n_det=d.n_det, walkers=M, el_ms=1e3 * t_el, el_rate=M / t_el,
                el_tflops=f_el * M / t_el / 1e12, el_frac=f_el * M / t_el / 1e12 / peak, sweeps=sweeps,
                met_ms=1e3 * t_met, met_rate=M * sweeps / t_met, met_tflops=f_st * M * sweeps / t_met / 1e12,
                met_frac=f_st * M * sweeps / t_met / 1e12 / peak, deriv_walkers=Md, n_param=s.n_param(),
-               el_d_ms=1e3 * t_el_d, O_ms=1e3 * t_O, orb_ms=1e3 * t_orb, nuc_ms=1e3 * t_nuc)
+               el_d_ms=1e3 * t_el_d, O_ms=1e3 * t_O, orb_ms=1e3 * t_orb, nuc_ms=1e3 * t_nuc, frc_ms=1e3 * t_frc,
+               fuse_ms=1e3 * t_fuse, graph_ms=1e3 * t_graph, pair_ms=1e3 * t_pair)
     s.close()
     return row
 
@@ -122,23 +147,25 @@ def main():
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("configs_report needs a CUDA device: the product path has no CPU fallback")
-    peak = qb.fp64_peak(0, reps=5)
+    peak = max(qb.fp64_peak(k, reps=5) for k in (0, 1, 3))
     rows = [measure("H2", *wl.h2(), peak), measure("LiH", *wl.lih(), peak), measure("Li2 (30 AOs)", *wl.li2(), peak),
             measure("Li2-28", *wl.li2(variant="28"), peak), measure("CO", *wl.co(), peak)]
-    print(f"DFMA peak measured in this process: {peak:.1f} TFLOP/s")
-    print("| config | N_e | N_AO | N_det | walkers | E_L call ms | M walker*E_L/s | model TFLOP/s | of DFMA peak | sweeps | "
-          "Metropolis ms | M walker-steps/s | model TFLOP/s | of DFMA peak |")
-    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+    print(f"FP64 peak measured in this process (max of DFMA, two-register DFMA, DMMA): {peak:.1f} TFLOP/s")
+    print("| config | N_e | N_AO | N_det | walkers | E_L call ms | M walker*E_L/s | model TFLOP/s | of peak | sweeps | "
+          "Metropolis ms | M walker-steps/s | model TFLOP/s | of peak | sweeps + E_L eager ms | as one CUDA graph ms |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|")
     for x in rows:
         print(f"| {x['config']} | {x['n_e']} | {x['n_ao']} | {x['n_det']} | {x['walkers']} | {x['el_ms']:.3f} | "
               f"{x['el_rate'] / 1e6:.1f} | {x['el_tflops']:.2f} | {100 * x['el_frac']:.1f} % | {x['sweeps']} | "
-              f"{x['met_ms']:.3f} | {x['met_rate'] / 1e6:.1f} | {x['met_tflops']:.2f} | {100 * x['met_frac']:.1f} % |")
+              f"{x['met_ms']:.3f} | {x['met_rate'] / 1e6:.1f} | {x['met_tflops']:.2f} | {100 * x['met_frac']:.1f} % | "
+              f"{x['pair_ms']:.3f} | {x['graph_ms']:.3f} |")
     print("\nParameter derivatives (eq. 6 factors), same sampled walkers, device time per call:")
-    print("| config | walkers | E_L ms | n_param | E_L + O_p ms | orbital parameters (N_AO x N_MO + N_AO) | dC, dzeta ms | grad_R ln Psi ms |")
-    print("|---|---|---|---|---|---|---|---|")
+    print("| config | walkers | E_L ms | n_param | E_L + O_p ms | E_L + fused eq. 6 gradient ms | orbital parameters (N_AO x N_MO + N_AO) | "
+          "dC, dzeta ms | grad_R ln Psi ms | grad_R E_L ms |")
+    print("|---|---|---|---|---|---|---|---|---|---|")
     for x in rows:
-        print(f"| {x['config']} | {x['deriv_walkers']} | {x['el_d_ms']:.3f} | {x['n_param']} | {x['O_ms']:.3f} | "
-              f"{x['n_ao']} x {x['n_mo']} + {x['n_ao']} | {x['orb_ms']:.3f} | {x['nuc_ms']:.3f} |")
+        print(f"| {x['config']} | {x['deriv_walkers']} | {x['el_d_ms']:.3f} | {x['n_param']} | {x['O_ms']:.3f} | {x['fuse_ms']:.3f} | "
+              f"{x['n_ao']} x {x['n_mo']} + {x['n_ao']} | {x['orb_ms']:.3f} | {x['nuc_ms']:.3f} | {x['frc_ms']:.3f} |")
     print("\nAccelerated (excitation tables, F.6/F.7) vs explicit per-determinant E_L (PAPER.md:345-349, Fig. 11), CO shape:")
     print("| N_det | walkers | tables ms | explicit ms | explicit / tables |")
     print("|---|---|---|---|---|")
@@ -148,7 +175,7 @@ def main():
         geo, t_total = scan(args.scan_geometries, peak)
         print(f"\nCO scan (500 determinants, {geo[0]['walkers']} walkers per geometry, {geo[0]['sweeps']} sweeps + E_L on every "
               f"sweep): {len(geo)} geometries in {t_total:.2f} s")
-        print("| R (bohr) | mean E_L (Ha) | std error | seconds | model TFLOP/s | of DFMA peak |")
+        print("| R (bohr) | mean E_L (Ha) | std error | seconds | model TFLOP/s | of peak |")
         print("|---|---|---|---|---|---|")
         for g in geo:
             print(f"| {g['R']:.2f} | {g['mean_E_L']:.5f} | {g['stderr']:.5f} | {g['seconds']:.3f} | {g['tflops']:.2f} | "

@@ -35,6 +35,7 @@ int cuda_fail(cudaError_t e, const char *what) {
 
 struct Variant {
   int NS, NMO, LP, ws_doubles;
+  int wpb_psi_max;       // launch bound of the values-only kernels, in warps
   int psi_ws_doubles;    // the values-only kernels' compact scratch
   int metro_ws_doubles;  // the sampler's per-warp scratch: the evaluator's plus two sweeps of draws
   bool exact;  // compiled for n_up = n_dn = NS
@@ -59,11 +60,12 @@ Variant make_variant() {
   v.LP = Geo<NS, NMO>::LP;
   v.exact = X;
   v.ws_doubles = Geo<NS, NMO>::total;
+  v.wpb_psi_max = kWarpsPsiOf<NS>;
   v.psi_ws_doubles = Geo<NS, NMO>::totalC(true);
   v.metro_ws_doubles = Geo<NS, NMO>::totalC(true) + 2 * kDrawDoubles<NS>;
   v.k_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl>;
-  v.k_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi>;
-  v.k_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi>;
+  v.k_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsiOf<NS>>;
+  v.k_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsiOf<NS>>;
   v.k_expl = (const void *)explicit_energy_kernel<NS, NMO, X, kWarpsEl>;
   v.k_el_deriv = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true>;
   v.k_orb = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrb>;
@@ -76,13 +78,13 @@ Variant make_variant() {
   v.frc_ws_doubles = Geo<NS, NMO>::total + Geo<NS, NMO>::frcExtra;
   v.k_el_fuse = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true, false, false, true>;
   v.e_el_fuse = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true, true, false, true>;
-  v.b_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi, false, false, true>;
-  v.b_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi, false, true>;
+  v.b_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsiOf<NS>, false, false, true>;
+  v.b_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsiOf<NS>, false, true>;
   v.b_el = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBf>;
   v.bf_ws_doubles = BfGeo<NS, NMO>::total;
   v.e_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, false, true>;
-  v.e_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsi, false, true>;
-  v.e_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsi, true>;
+  v.e_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsiOf<NS>, false, true>;
+  v.e_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsiOf<NS>, true>;
   v.e_expl = (const void *)explicit_energy_kernel<NS, NMO, X, kWarpsEl, true>;
   v.e_el_deriv = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true, true>;
   return v;
@@ -199,6 +201,7 @@ struct qmc_system {
   Variant var{};
   int smem_el = 0, smem_psi = 0;  // dynamic shared memory of the E_L kernels (kWarpsEl warps) / values-only kernels
   int smem_metro = 0;             // ... of the sampler
+  int warps_psi = 0, warps_metro = 0;  // warps per block the values-only kernels are launched with
   int blocks_el = 0, blocks_psi = 0, blocks_metro = 0, blocks_expl = 0, blocks_deriv = 0;
   void *d_C = nullptr, *d_dets = nullptr, *d_gen = nullptr, *d_cols = nullptr, *d_orig = nullptr, *d_yrec = nullptr, *d_ytgt = nullptr, *d_rowao = nullptr,
        *d_rownrm = nullptr;
@@ -786,8 +789,19 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   P.n_mo_all = d->n_mo;
   P.smem_const_bytes = (int)((szC + szD + 15) / 16 * 16);
   s->smem_el = P.smem_const_bytes + kWarpsEl * var->ws_doubles * (int)sizeof(double);
-  s->smem_psi = P.smem_const_bytes + kWarpsPsi * var->psi_ws_doubles * (int)sizeof(double);
-  s->smem_metro = P.smem_const_bytes + kWarpsPsi * var->metro_ws_doubles * (int)sizeof(double);
+  // values-only kernels: the most warps per block (up to the launch bound) that keep QMC_MINBLOCKS blocks' shared
+  // memory on an SM -- a long expansion's constants would otherwise cost a whole block of warps
+  int sm_smem = 0;
+  cudaDeviceGetAttribute(&sm_smem, cudaDevAttrMaxSharedMemoryPerMultiprocessor, device);
+  auto fit_warps = [&](int ws_doubles) {
+    int w = var->wpb_psi_max;
+    while (w > 4 && QMC_MINBLOCKS * (P.smem_const_bytes + w * ws_doubles * (int)sizeof(double) + 1024) > sm_smem) --w;
+    return w;
+  };
+  s->warps_psi = fit_warps(var->psi_ws_doubles);
+  s->warps_metro = fit_warps(var->metro_ws_doubles);
+  s->smem_psi = P.smem_const_bytes + s->warps_psi * var->psi_ws_doubles * (int)sizeof(double);
+  s->smem_metro = P.smem_const_bytes + s->warps_metro * var->metro_ws_doubles * (int)sizeof(double);
 
   int dev_smem = 0, n_sm = 0;
   cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
@@ -799,7 +813,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   s->n_sm = n_sm;
   const void *ks[5] = {s->var.k_el, s->var.k_psi, s->var.k_metro, s->var.k_expl, s->var.k_el_deriv};
   int *nb[5] = {&s->blocks_el, &s->blocks_psi, &s->blocks_metro, &s->blocks_expl, &s->blocks_deriv};
-  const int kw[5] = {kWarpsEl, kWarpsPsi, kWarpsPsi, kWarpsEl, kWarpsEl};
+  const int kw[5] = {kWarpsEl, s->warps_psi, s->warps_metro, kWarpsEl, kWarpsEl};
   const int ksm[5] = {s->smem_el, s->smem_psi, s->smem_metro, s->smem_el, s->smem_el};
   for (int i = 0; i < 5; ++i) {
     if ((e = cudaFuncSetAttribute(ks[i], cudaFuncAttributeMaxDynamicSharedMemorySize, ksm[i])) != cudaSuccess) {
@@ -857,7 +871,7 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
     return QMC_OK;
   }
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
-  const int wpb = el ? kWarpsEl : kWarpsPsi, smem = el ? s->smem_el : s->smem_psi;
+  const int wpb = el ? kWarpsEl : s->warps_psi, smem = el ? s->smem_el : s->smem_psi;
   const int64_t need = (groups + wpb - 1) / wpb;
   const int grid = (int)std::min<int64_t>(need, d_O ? s->blocks_deriv : (el ? s->blocks_el : s->blocks_psi));
   double *fb = nullptr;
@@ -1020,12 +1034,12 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
   mp.n_accepted = d_counter;
   if (h_n_accepted) CK(cudaMemsetAsync(d_counter, 0, sizeof(unsigned long long), st));
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
-  const int64_t need = (groups + kWarpsPsi - 1) / kWarpsPsi;
+  const int64_t need = (groups + s->warps_metro - 1) / s->warps_metro;
   const int grid = (int)std::min<int64_t>(need, s->blocks_metro);
   void *args[3] = {(void *)&s->P, (void *)&io, (void *)&mp};
   if (!d_eloc_acc) {
     // one persistent launch for all sweeps: coordinates and log|Psi| stay in registers
-    CK(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_metro, st));
+    CK(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(s->warps_metro * 32), args, s->smem_metro, st));
     ++g_launches;
   } else {
     // E_L after every sweep (BASELINE config 5): one-sweep launches of the sampler alternate with the
@@ -1050,14 +1064,14 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
     mp.n_sweeps = 1;
     if (n_sweeps == 0) {  // nothing to accumulate; still report log|Psi| of the starting positions
       mp.n_sweeps = 0;
-      CKS(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_metro, st));
+      CKS(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(s->warps_metro * 32), args, s->smem_metro, st));
       ++g_launches;
     }
     for (int32_t sw = 0; sw < n_sweeps; ++sw) {
       mp.sweep0 = (uint32_t)(sweep_offset + (uint64_t)sw);
       mp.accept = d_accept ? d_accept + (size_t)sw * (size_t)M : nullptr;
       mp.resume = sw > 0 ? 1 : 0;
-      CKS(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(kWarpsPsi * 32), args, s->smem_metro, st));
+      CKS(cudaLaunchKernel(s->var.k_metro, dim3(grid), dim3(s->warps_metro * 32), args, s->smem_metro, st));
       ++g_launches;
       int rc = launch_eval(s, d_r, M, nullptr, nullptr, scratch, st, true);
       if (rc != QMC_OK) {

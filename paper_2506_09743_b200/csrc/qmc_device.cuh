@@ -40,7 +40,15 @@ constexpr int kMaxEen = 6;    // terms of the electron-electron-nucleus Jastrow 
                              // Measured on CO, 32768 walkers, early / equilibrated: 8 warps 0.82 / 0.63 ms, 10: 0.80 / 0.60, 12: 0.78 / 0.80
                              // (12 x 16.3 KB of scratch leave ~30 KB of L1 for the term lists and the constant tables)
 #endif
+#ifndef QMC_WARPS_PSI_SMALL
+#define QMC_WARPS_PSI_SMALL 10  // ... of the instantiations for fewer than 5 electrons per spin (96 registers: 14 warps cost
+                                // the Li2 sampler 0.32 -> 0.44 ms per 10 sweeps through the 72-register cap)
+#endif
 constexpr int kWarpsEl = QMC_WARPS, kWarpsPsi = QMC_WARPS_PSI, kWarpsOrb = QMC_WARPS_ORB, kWarpsOrbSmall = 8;
+// launch bound (= most warps per block) of the values-only kernels of an instantiation; qmc_setup launches the
+// largest count up to it that still fits two blocks' shared memory on an SM (long expansions: more constants)
+template <int NS>
+constexpr int kWarpsPsiOf = (NS >= 5) ? QMC_WARPS_PSI : QMC_WARPS_PSI_SMALL;
 constexpr int kWarpsBf = 4;  // warps (= walkers in flight) per block of the backflow E_L kernel
 constexpr int kWarpsMax = kWarpsEl > kWarpsPsi ? kWarpsEl : kWarpsPsi;
 

@@ -55,7 +55,8 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
   const int g = lane / ne, e = lane - g * ne;
   const int64_t n_groups = (io.M + G - 1) / G;
-  const int64_t stride = (int64_t)gridDim.x * WPB;
+  const int wpb = (int)(blockDim.x >> 5);  // warps launched per block (<= WPB, the launch bound)
+  const int64_t stride = (int64_t)gridDim.x * wpb;
   const int np = kJastrowParams + 7 * P.n_een + P.n_det_all;
   double *sO = ws + GE::total, *accO = sO + G * np, *accOE = accO + np;  // FUSE only
   double accE = 0.0;
@@ -73,7 +74,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
       dummy_xyz(lane, x, y, z);
     }
   };
-  for (int64_t grp = (int64_t)blockIdx.x * WPB + warp; grp < n_groups; grp += stride) {
+  for (int64_t grp = (int64_t)blockIdx.x * wpb + warp; grp < n_groups; grp += stride) {
     double x, y, z;
     fetch(grp, x, y, z);
     eval_walkers<NS, NMO, EL, X, false, DERIV, EEN, 0, BF, FUSE>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1, DerivOut{io.O, grp * G, io.M});
@@ -133,7 +134,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   }
   if (FUSE) {
     // transposed, [2 n_param + 1][grid warps], so that the final kernel reads each parameter's column contiguously
-    const int64_t nwarps = (int64_t)gridDim.x * WPB, me = (int64_t)blockIdx.x * WPB + warp;
+    const int64_t nwarps = (int64_t)gridDim.x * wpb, me = (int64_t)blockIdx.x * wpb + warp;
     for (int p = lane; p < 2 * np; p += 32) io.fuse_part[p * nwarps + me] = accO[p];
     if (lane == 0) io.fuse_part[(int64_t)2 * np * nwarps + me] = accE;
   }
@@ -896,9 +897,10 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G, nc = 3 * ne, npair = (nc + 1) / 2;
   const int g = lane / ne, e = lane - g * ne;
   const int64_t n_groups = (io.M + G - 1) / G;
-  const int64_t stride = (int64_t)gridDim.x * WPB;
+  const int wpb = (int)(blockDim.x >> 5);  // warps launched per block (<= WPB, the launch bound)
+  const int64_t stride = (int64_t)gridDim.x * wpb;
   unsigned long long acc_count = 0;
-  for (int64_t grp = (int64_t)blockIdx.x * WPB + warp; grp < n_groups; grp += stride) {
+  for (int64_t grp = (int64_t)blockIdx.x * wpb + warp; grp < n_groups; grp += stride) {
     const int64_t w = grp * G + g;
     const bool own = (g < G) && (w < io.M);
     const int rg = (own ? g : 0) * 4;
