@@ -257,6 +257,16 @@ def main():
     for _ in range(args.steps):
         e2e_step()
     t_e2e = time.perf_counter() - t0
+    # the same through one upload: sample AND evaluate from host buffers (qmc_vmc_step_host: H2D of the walkers,
+    # 20 sweeps, E_L, statistics, D2H of walkers and energies) -- what a VMC iteration moves over PCIe
+    el_pin = torch.empty(M, dtype=torch.float64).pin_memory()
+    r_step = r_pin.clone().pin_memory()
+    for k in range(2):
+        sysh.vmc_step_host(r_step, step_size, n_sweeps, seed, sweep_offset=k * n_sweeps, walker_offset=rank * M, eloc_host=el_pin, n_chunks=2)
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        sysh.vmc_step_host(r_step, step_size, n_sweeps, seed, sweep_offset=(2 + k) * n_sweeps, walker_offset=rank * M, eloc_host=el_pin, n_chunks=2)
+    t_vmc = time.perf_counter() - t0
     clocks = sampler.stop()
 
     # ---- E_L + parameter derivatives O (eq. 6 factors) and the gradient estimator,
@@ -406,6 +416,10 @@ def main():
             "cpu_baseline": cpu,
             "e2e": {"value": e2e_rate, "unit": UNIT, "h2d_bytes_per_step": int(r_pin.numel() * 8),
                     "d2h_bytes_per_step": int(out_pin.numel() * 8)},
+            "e2e_vmc_step": {"ms": 1e3 * t_vmc / K, "walker_steps_per_s": world * M * n_sweeps / (t_vmc / K),
+                             "walker_E_L_per_s": world * M / (t_vmc / K),
+                             "h2d_bytes_per_step": int(r_pin.numel() * 8), "d2h_bytes_per_step": int(r_pin.numel() * 8 + M * 8),
+                             "note": "qmc_vmc_step_host: one upload, 20 sweeps + E_L + statistics, walkers and E_L back; wall clock"},
             "log_derivatives": {"n_param": n_par, "ms_local_energy_plus_O": 1e3 * t_d / K_DERIV,
                                 "ms_energy_gradient": 1e3 * t_g / K_DERIV, "O_bytes": int(M) * n_par * 8,
                                 "gradient_hbm_gbs": int(M) * (n_par + 1) * 8 / (t_g / K_DERIV) / 1e9,

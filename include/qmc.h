@@ -141,6 +141,18 @@ int qmc_local_energy(qmc_system_t *s, const double *d_r, int64_t M, double *d_lo
 int qmc_local_energy_host(qmc_system_t *s, const double *h_r, int64_t M, double *h_logpsi, double *h_sign,
                           double *h_eloc, int32_t n_chunks);
 
+/* One sampling-and-evaluation step with HOST buffers (what a VMC iteration does between two parameter updates,
+ * PAPER.md:180-182): upload the walkers once, n_sweeps Metropolis sweeps (as qmc_metropolis, same random-number
+ * stream: the trajectories equal the device call's), E_L of the resulting walkers, batch mean and standard error
+ * (eq. 3), walkers and energies back to the host.
+ *   h_r host in/out [n_e][3][M];  h_eloc host out [M] (may be NULL);  h_mean, h_stderr host out (may be NULL)
+ * The walkers are cut into n_chunks ranges pipelined over the handle's two internal streams (copies of one range
+ * overlap the sweeps of the other; page-locked host memory needed for the overlap).  Shares the scratch of
+ * qmc_local_energy_host: one host-variant call at a time per handle.  Synchronous. */
+int qmc_vmc_step_host(qmc_system_t *s, double *h_r, int64_t M, double step, int32_t n_sweeps, uint64_t seed,
+                      uint64_t sweep_offset, int64_t walker_offset, double *h_eloc, double *h_mean, double *h_stderr,
+                      int32_t n_chunks);
+
 /* qmc_local_energy with EVERY walker on the explicit route: each determinant's Slater matrices are eliminated on
  * their own (G.7 per determinant; what PAPER.md:349 / Fig. 11 calls "explicit"), no excitation tables.
  * Same arguments, same outputs within rounding; N_det eliminations per walker and spin instead of one.  It exists

@@ -18,7 +18,7 @@ EXPORTS = ["qmc_setup", "qmc_destroy", "qmc_local_energy", "qmc_log_psi", "qmc_m
            "qmc_fp64_peak", "qmc_model_flops", "qmc_launch_count", "qmc_status_string", "qmc_n_param", "qmc_local_energy_explicit", "qmc_set_kernel_timing", "qmc_kernel_times",
            "qmc_log_derivatives", "qmc_energy_gradient", "qmc_local_energy_host", "qmc_orbital_derivatives",
            "qmc_nuclear_log_gradient", "qmc_nuclear_energy_gradient", "qmc_force", "qmc_local_energy_gradient",
-           "qmc_static_scratch_init", "qmc_batch_stats_static"]
+           "qmc_static_scratch_init", "qmc_batch_stats_static", "qmc_vmc_step_host"]
 
 
 class QmcError(RuntimeError):
@@ -76,6 +76,8 @@ def lib():
         L.qmc_force.argtypes = [vp, vp, vp, i64, C.c_int32, vp, vp, vp]
         L.qmc_local_energy_host.restype = C.c_int
         L.qmc_local_energy_host.argtypes = [vp, vp, i64, vp, vp, vp, C.c_int32]
+        L.qmc_vmc_step_host.restype = C.c_int
+        L.qmc_vmc_step_host.argtypes = [vp, vp, i64, dbl, C.c_int32, C.c_uint64, C.c_uint64, i64, vp, vp, vp, C.c_int32]
         L.qmc_log_psi.restype = C.c_int
         L.qmc_log_psi.argtypes = [vp, vp, i64, vp, vp, vp]
         L.qmc_metropolis.restype = C.c_int
@@ -217,6 +219,20 @@ class QmcSystem:
         _check(lib().qmc_local_energy_host(self._h, r_host.data_ptr(), M, out_host[0].data_ptr(), out_host[1].data_ptr(),
                                            out_host[2].data_ptr(), int(n_chunks)))
         return out_host
+
+    def vmc_step_host(self, r_host, step, n_sweeps, seed, sweep_offset=0, walker_offset=0, eloc_host=None, n_chunks: int = 2):
+        """qmc_vmc_step_host: r_host float64 CPU tensor [n_e,3,M] is sampled in place (n_sweeps sweeps) and its E_L
+        evaluated; returns (mean, stderr); eloc_host (CPU tensor [M]) receives the per-walker energies.  Synchronous."""
+        assert (not r_host.is_cuda) and r_host.dtype == torch.float64 and r_host.is_contiguous()
+        assert r_host.dim() == 3 and r_host.shape[0] == self.n_e and r_host.shape[1] == 3
+        M = int(r_host.shape[2])
+        if eloc_host is not None:
+            assert (not eloc_host.is_cuda) and eloc_host.dtype == torch.float64 and eloc_host.is_contiguous() and eloc_host.numel() == M
+        m, e = C.c_double(), C.c_double()
+        _check(lib().qmc_vmc_step_host(self._h, r_host.data_ptr(), M, float(step), int(n_sweeps), int(seed), int(sweep_offset),
+                                       int(walker_offset), None if eloc_host is None else eloc_host.data_ptr(),
+                                       C.addressof(m), C.addressof(e), int(n_chunks)))
+        return m.value, e.value
 
     def log_psi(self, r, logpsi=None, sign=None, stream=None):
         M = self._chk_r(r)

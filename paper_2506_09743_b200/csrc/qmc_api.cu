@@ -234,6 +234,8 @@ struct qmc_system {
   cudaStream_t hst[2] = {nullptr, nullptr};
   double *hbuf[2] = {nullptr, nullptr};
   int64_t hbuf_walkers = 0;
+  double *helo = nullptr;  // qmc_vmc_step_host: E_L of the whole batch [helo_walkers]
+  int64_t helo_walkers = 0;
 };
 
 extern "C" {
@@ -280,6 +282,7 @@ void qmc_destroy(qmc_system_t *s) {
     if (s->hst[i]) cudaStreamDestroy(s->hst[i]);
     cudaFree(s->hbuf[i]);
   }
+  cudaFree(s->helo);
   delete s;
 }
 
@@ -995,6 +998,57 @@ int qmc_local_energy_host(qmc_system_t *s, const double *h_r, int64_t M, double 
       cudaError_t e = cudaStreamSynchronize(s->hst[i]);
       if (e != cudaSuccess && rc == QMC_OK) rc = cuda_fail(e, "qmc_local_energy_host");
     }
+  return rc;
+}
+
+int qmc_vmc_step_host(qmc_system_t *s, double *h_r, int64_t M, double step, int32_t n_sweeps, uint64_t seed,
+                      uint64_t sweep_offset, int64_t walker_offset, double *h_eloc, double *h_mean, double *h_stderr,
+                      int32_t n_chunks) {
+  if (!s || !h_r || M <= 0 || n_chunks < 1 || !(step > 0.0) || n_sweeps < 0 || walker_offset < 0) return QMC_EINVAL;
+  CK(cudaSetDevice(s->device));
+  const int ne = s->P.n_e;
+  int64_t Mc = (M + n_chunks - 1) / n_chunks;
+  Mc = (Mc + 31) / 32 * 32;
+  if (Mc > s->hbuf_walkers) {
+    for (int i = 0; i < 2; ++i) {
+      if (!s->hst[i]) CK(cudaStreamCreateWithFlags(&s->hst[i], cudaStreamNonBlocking));
+      CK(cudaStreamSynchronize(s->hst[i]));
+      cudaFree(s->hbuf[i]);
+      s->hbuf[i] = nullptr;
+      CK(cudaMalloc(&s->hbuf[i], (size_t)(3 * ne + 3) * (size_t)Mc * sizeof(double)));
+    }
+    s->hbuf_walkers = Mc;
+  }
+  if (M > s->helo_walkers) {
+    CK(cudaDeviceSynchronize());
+    cudaFree(s->helo);
+    s->helo = nullptr;
+    CK(cudaMalloc(&s->helo, (size_t)M * sizeof(double)));
+    s->helo_walkers = M;
+  }
+  int rc = QMC_OK;
+  int c = 0;
+  for (int64_t a = 0; a < M && rc == QMC_OK; a += Mc, ++c) {
+    const int64_t m = std::min<int64_t>(Mc, M - a);
+    cudaStream_t st = s->hst[c & 1];
+    double *d_r = s->hbuf[c & 1];
+    CK(cudaMemcpy2DAsync(d_r, (size_t)m * sizeof(double), h_r + a, (size_t)M * sizeof(double), (size_t)m * sizeof(double),
+                         (size_t)3 * ne, cudaMemcpyHostToDevice, st));
+    rc = qmc_metropolis(s, d_r, m, step, n_sweeps, seed, sweep_offset, walker_offset + a, nullptr, nullptr, nullptr, nullptr,
+                        nullptr, st);
+    if (rc != QMC_OK) break;
+    rc = launch_eval(s, d_r, m, nullptr, nullptr, s->helo + a, st, true);
+    if (rc != QMC_OK) break;
+    CK(cudaMemcpy2DAsync(h_r + a, (size_t)M * sizeof(double), d_r, (size_t)m * sizeof(double), (size_t)m * sizeof(double),
+                         (size_t)3 * ne, cudaMemcpyDeviceToHost, st));
+    if (h_eloc) CK(cudaMemcpyAsync(h_eloc + a, s->helo + a, (size_t)m * sizeof(double), cudaMemcpyDeviceToHost, st));
+  }
+  for (int i = 0; i < 2; ++i)
+    if (s->hst[i]) {
+      cudaError_t e = cudaStreamSynchronize(s->hst[i]);
+      if (e != cudaSuccess && rc == QMC_OK) rc = cuda_fail(e, "qmc_vmc_step_host");
+    }
+  if (rc == QMC_OK && (h_mean || h_stderr)) rc = qmc_batch_stats(s->helo, M, h_mean, h_stderr, s->hst[0]);
   return rc;
 }
 

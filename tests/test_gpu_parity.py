@@ -1466,3 +1466,28 @@ def test_h2_force_is_along_the_axis_and_antisymmetric(env):
     assert abs(F[0, 2] + F[1, 2]) < 5 * float(both.std() / math.sqrt(both.numel())), (F, sig)
     assert np.all(np.isfinite(F)) and abs(F[0, 2]) < 1.0
     s.close()
+
+
+def test_vmc_step_host_equals_the_device_calls(env):
+    """qmc_vmc_step_host (host buffers, chunked over two streams) against qmc_metropolis + qmc_local_energy +
+    qmc_batch_stats on device buffers: same trajectories bit for bit (Philox is keyed by the global walker index), same
+    E_L and statistics up to rounding order; ragged size, 1 and 3 chunks."""
+    torch, ob, qb = env
+    d, r = wl.li2(M=4099)
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    s.metropolis(rg, 0.3, 7, seed=33, sweep_offset=5, walker_offset=11)
+    el = s.local_energy(rg)[2]
+    m0, e0 = qb.batch_stats(el)
+    for n_chunks in (1, 3):
+        rh = torch.from_numpy(r.copy()).pin_memory()
+        eh = torch.empty(4099, dtype=torch.float64).pin_memory()
+        m, e = s.vmc_step_host(rh, 0.3, 7, 33, sweep_offset=5, walker_offset=11, eloc_host=eh, n_chunks=n_chunks)
+        assert torch.equal(rh, rg.cpu())
+        # E_L: bit for bit except on the few walkers the explicit route re-evaluates, whose determinant slices are dealt
+        # over the grid according to the size of the launch (rounding order of the slice sums)
+        elc = el.cpu()
+        diff = (eh - elc).abs() / elc.abs().clamp(min=1.0)
+        assert float(diff.max()) < 1e-11 and int((diff > 0).sum()) <= 4099 // 50, (float(diff.max()), int((diff > 0).sum()))
+        assert abs(m - m0) <= 1e-11 * abs(m0) and abs(e - e0) <= 1e-10 * e0
+    s.close()
