@@ -431,6 +431,25 @@ __device__ __forceinline__ double exp_neg(double x, const double *__restrict__ t
   return __hiloint2double(__double2hiint(p) + ((n >> 6) << 20), __double2loint(p));
 }
 
+// The same with the table given as a 32-bit shared-memory address held in a register (the hot AO loop: the generic
+// pointer made the compiler rebuild the shared window base -- S2UR + two ULEA -- at every call).
+__device__ __forceinline__ double exp_neg_s32(double x, uint32_t tab32, const MathConsts &K) {
+  constexpr double kMagic = 6755399441055744.0;
+  x = __hiloint2double((int)min((unsigned)__double2hiint(x), 0xC0859000u), __double2loint(x));
+  const double t = fma(x, K.e_scale, kMagic);
+  const int n = __double2loint(t);
+  const double nd = t - kMagic;
+  double f = fma(nd, K.e_ln2hi, x);
+  f = fma(nd, K.e_ln2lo, f);
+  const double f2 = f * f;
+  const double a = fma(f, K.e_c5, K.e_c4), b = fma(f, K.e_c3, 0.5);
+  const double q = fma(f2, fma(f2, a, b), f);
+  double T;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(T) : "r"(tab32 + (uint32_t)((n & (kExpTab - 1)) << 3)));
+  const double p = fma(T, q, T);
+  return __hiloint2double(__double2hiint(p) + ((n >> 6) << 20), __double2loint(p));
+}
+
 // ---------------------------------------------------------------------------------
 // Elementary functions of the Box-Muller transform (reading Q9), table-driven so that one
 // normal pair costs ~40 FP64 instructions.  Tables are built in long double by qmc_setup (kRngTab

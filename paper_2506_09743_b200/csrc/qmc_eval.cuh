@@ -411,6 +411,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
     const uint32_t tl32 = opaque_u32((uint32_t)__cvta_generic_to_shared(tl));
     const uint32_t to32 = EL ? opaque_u32(tl32 + 8u * (uint32_t)oo) : 0u;
     const double *const afrag = tile + fk * S + fr;                // A fragments: + 4 ks S + tile column
+    const uint32_t exp32 = opaque_u32((uint32_t)__cvta_generic_to_shared(sExp));  // exp_neg's table
     int chunk = 0;
     double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1.0, r = 1.0, ri = 1.0, gd = 0.0, pw = 1.0;
     uint32_t tr = tl32, tro = to32;  // this lane's tile cells of the next AO row (rows follow the record stream)
@@ -438,7 +439,7 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
           }
           continue;
         }
-        const double gr = exp_neg(-sh.zeta * r, sExp, P.mc) * pw;  // r^k e^{-zeta r}
+        const double gr = exp_neg_s32(-sh.zeta * r, exp32, P.mc) * pw;  // r^k e^{-zeta r}
         double h = 0.0;
         if (EL) {
           // lap(S r^k e^{-zeta r}) = phi * [zeta^2 - 2 zeta (k+l+1)/r + k (k+2l+1)/r^2]
