@@ -12,9 +12,10 @@ value   = walker*E_L evaluations per second (M / device time of qmc_local_energy
 e2e     = the same metric through the C ABI call that takes HOST buffers (qmc_local_energy_host): pinned
           host walkers -> H2D -> kernels -> D2H of log|Psi|, sign, E_L, all inside the timed region (the
           call pipelines walker ranges over two streams so the copies overlap the kernels).
-roofline= model FP64 flop-equivalents of the E_L kernel / its mean launch time, against the FP64 peak measured in
-          this same process: the largest of the DFMA and DMMA microbenchmarks of qmc_fp64_peak (they run on one
-          pipe); the sampler and the whole call are reported against the same denominator.
+roofline= model FP64 flop-equivalents per launch / mean launch time of the kernel that dominates the timed step (the
+          sampler: one launch = 20 sweeps), against the FP64 peak measured in this same process: the largest of the
+          DFMA and DMMA microbenchmarks of qmc_fp64_peak (they run on one pipe); the fused E_L kernel and the whole
+          E_L call are reported beside it (roofline.local_energy_kernel) against the same denominator.
 cpu_baseline = the CPU oracle, as it stands, on the host cores, on a bounded sample.
 
 N > 1 (torchrun): walkers are sharded, M per GPU fixed (weak scaling), no data-path
@@ -133,10 +134,10 @@ def run_reference(args):
 K_DERIV = 5  # timed repetitions of the NEXT-1 block
 
 
-def profile_traffic():
-    """DRAM bytes (read + written) per launch of the dominant kernel, from the committed ncu summary."""
+def profile_traffic(name):
+    """DRAM bytes (read + written) per launch of a kernel, from its committed ncu summary under profiles/."""
     import re
-    path = os.path.join(ROOT, "profiles", "r02_el_kernel.md")
+    path = os.path.join(ROOT, "profiles", name)
     try:
         m = re.search(r"dram_bytes_per_launch:\s*(\d+)", open(path).read())
         return int(m.group(1)) if m else None
@@ -391,28 +392,36 @@ def main():
                            "frac_of_dfma_peak": achieved_met / peak_dfma,
                            "model_flop_eq_per_walker_step": flops_st},
             "local_energy_ms": 1e3 * t_el / K,
-            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                         "frac": achieved / peak,
-                         "kernel_ms": 1e3 * t_kmain / K, "fallback_kernel_ms": 1e3 * t_kfb / K,
-                         "achieved_call": achieved_call, "frac_call": achieved_call / peak,
-                         "achieved_sampler": achieved_met, "frac_sampler": achieved_met / peak,
-                         "frac_of_dfma_microbenchmark": achieved / peak_dfma,
-                         "timing": "kernel_ms: CUDA events recorded inside qmc_local_energy on the launching stream before and "
-                                   "after the table-path kernel (qmc_set_kernel_timing), mean over a replay of the K steps "
-                                   "(flush, sampler, E_L, statistics) right after the timed ones; *_call: events around the "
-                                   "whole call in the K timed steps, which also runs the explicit fallback kernel",
-                         "traffic": profile_traffic(),
-                         "kernel": "local_energy_kernel<7,14,true>",
+            # the dominant kernel of the timed step BY TIME is the sampler (one launch = 20 sweeps of M walkers, ~90 % of
+            # the step: profiles/r02_launches.md); the fused E_L kernel that north_star's 50 % target names is reported
+            # beside it, against the same peak
+            "roofline": {"bound": "alu", "kernel": "metropolis_kernel<7,14> (one launch = 20 sweeps of 131072 walkers)",
+                         "achieved": achieved_met, "peak": peak, "unit": "TFLOP/s", "frac": achieved_met / peak,
+                         "kernel_ms": 1e3 * t_met / K,
+                         "model_flop_eq_per_launch": flops_st * M * n_sweeps, "model_flop_eq_per_walker_step": flops_st,
+                         "traffic": profile_traffic("r02_metro_kernel.md"),
+                         "algorithmic_bytes_per_launch": int(M) * (2 * 3 * d.n_e * 8 + 16),
+                         "timing": "CUDA events on the launching stream around the single-launch qmc_metropolis call, sum over the "
+                                   "K timed steps",
+                         "local_energy_kernel": {
+                             "kernel": "local_energy_kernel<7,14,true>", "achieved": achieved, "frac": achieved / peak,
+                             "kernel_ms": 1e3 * t_kmain / K, "fallback_kernel_ms": 1e3 * t_kfb / K,
+                             "achieved_call": achieved_call, "frac_call": achieved_call / peak,
+                             "frac_of_dfma_microbenchmark": achieved / peak_dfma,
+                             "model_flop_eq_per_walker": flops_el, "traffic": profile_traffic("r02_el_kernel.md"),
+                             "algorithmic_bytes_per_launch": int(M) * (3 * d.n_e * 8 + 24),
+                             "timing": "kernel_ms: CUDA events recorded inside qmc_local_energy on the launching stream before and "
+                                       "after the table-path kernel (qmc_set_kernel_timing), mean over a replay of the K steps "
+                                       "(flush, sampler, E_L, statistics) right after the timed ones; *_call: events around the "
+                                       "whole call in the K timed steps, which also runs the explicit fallback kernel"},
                          "peak_source": "max of the qmc_fp64_peak DFMA (8 chains), DFMA (two-register form) and DMMA m8n8k4 "
                                         "microbenchmarks measured in this process: one shared FP64 pipe (no FP64 entry in "
                                         "MEASURED_PEAKS.json)",
                          "dfma_peak": peak_dfma, "dfma_two_register_peak": peak_dfma2, "dfma_three_register_rate": peak_dfma3,
                          "dmma_peak": peak_dmma,
                          "dfma_dependent_latency_cycles": 64.0 * 4 * 148 * (clocks.get("sm_mhz") or 1965.0) * 1e6 / (rate_chain * 1e12),
-                         "model_flop_eq_per_walker": flops_el,
                          # 148 SMs x 64 FP64 FMA/clk x 2 x the SM clock seen during the run
-                         "peak_nominal": 148 * 64 * 2 * (clocks.get("sm_mhz") or 1965.0) * 1e-6,
-                         "frac_of_nominal": achieved / (148 * 64 * 2 * (clocks.get("sm_mhz") or 1965.0) * 1e-6)},
+                         "peak_nominal": 148 * 64 * 2 * (clocks.get("sm_mhz") or 1965.0) * 1e-6},
             "cpu_baseline": cpu,
             "e2e": {"value": e2e_rate, "unit": UNIT, "h2d_bytes_per_step": int(r_pin.numel() * 8),
                     "d2h_bytes_per_step": int(out_pin.numel() * 8)},
