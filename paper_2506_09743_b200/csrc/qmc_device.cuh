@@ -23,6 +23,9 @@ constexpr int kMaxEen = 6;    // terms of the electron-electron-nucleus Jastrow 
 #ifndef QMC_MINBLOCKS
 #define QMC_MINBLOCKS 2      // blocks per SM the register allocation must allow
 #endif
+#ifndef QMC_MINBLOCKS_EL
+#define QMC_MINBLOCKS_EL 2   // ... of the E_L kernels (QMC_WARPS warps per block)
+#endif
 #ifndef QMC_PAIR_UNROLL
 #define QMC_PAIR_UNROLL 2    // unroll factor of the electron-pair loop
 #endif

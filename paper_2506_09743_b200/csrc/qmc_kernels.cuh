@@ -40,7 +40,7 @@ __device__ __forceinline__ void dummy_xyz(int lane, double &x, double &y, double
 // each warp keeps sum_w O_p and sum_w O_p E_L over its walkers and writes them once at the end; a group on the explicit
 // work list (its E_L is corrected later) parks its rows in io.fb_O instead; fused_gradient_final_kernel finishes.
 template <int NS, int NMO, bool EL, bool X, int WPB, bool DERIV = false, bool EEN = false, bool BF = false, bool FUSE = false>
-__global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
+__global__ void __launch_bounds__(WPB * 32, EL ? QMC_MINBLOCKS_EL : QMC_MINBLOCKS)
     local_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
   const double *sC;
@@ -146,7 +146,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
 // its partial sums; the warp that finishes a group last adds the partials in slice order (deterministic)
 // and writes the outputs.
 template <int NS, int NMO, bool X, int WPB, bool EEN = false>
-__global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
+__global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS_EL)
     explicit_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
   const int n_list = *io.fb_count;
