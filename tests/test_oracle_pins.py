@@ -1223,3 +1223,95 @@ def test_backflow_limit_antisymmetry_and_sampler_value():
     buf = np.zeros((24, 64))
     assert L.oracle_log_derivatives(ob_.ref, r.ctypes.data, 24, 0, 24, buf.ctypes.data) == -2
     assert L.oracle_nuclear_energy_gradient(ob_.ref, r.ctypes.data, 24, 0, 24, buf.ctypes.data) == -2
+
+
+# ---------------------------------------------------------------- P14b: F.8 / F.9 and the table route of the backflow term
+def test_P14b_second_order_trace_identities_on_random_matrices():
+    # (i) F.8 with F.9 as printed (last line of Appendix H, PAPER.md:542 -- lines 499 and 514-516 of the
+    # derivation are garbled, the result is legible):  Tr((A_X^-1 B_X)^2) = Tr((A_0^-1 B_0)^2) + Tr((T~ M)^2) + 2 Tr(T~ Y),
+    # T~ = (P A_0^-1 A_X P)^-1 inside the substituted subspace, M of F.7, Y = A_0^-1 B_0 M; single and double substitutions
+    rng = np.random.default_rng(140)
+    n = 6
+    A0, B0 = rng.standard_normal((n, n)), rng.standard_normal((n, n))
+    Av, Bv = rng.standard_normal((n, 4)), rng.standard_normal((n, 4))
+    Ai0 = np.linalg.inv(A0)
+    for P, Q in (([1], [2]), ([4], [0]), ([0, 3], [1, 0]), ([2, 5], [3, 2])):
+        AX, BX = A0.copy(), B0.copy()
+        for p, q in zip(P, Q):
+            AX[:, p] = Av[:, q]
+            BX[:, p] = Bv[:, q]
+        Tt = np.zeros((n, n))
+        Tt[np.ix_(P, P)] = np.linalg.inv((Ai0 @ AX)[np.ix_(P, P)])
+        M = Ai0 @ BX - Ai0 @ B0 @ Ai0 @ AX                                   # F.7
+        Y = Ai0 @ B0 @ M                                                       # F.9
+        lhs = np.trace(np.linalg.inv(AX) @ BX @ np.linalg.inv(AX) @ BX)
+        rhs = np.trace(Ai0 @ B0 @ Ai0 @ B0) + np.trace(Tt @ M @ Tt @ M) + 2 * np.trace(Tt @ Y)   # F.8
+        assert abs(lhs - rhs) < 1e-10 * max(1.0, abs(lhs)), (P, Q, lhs, rhs)
+    # (ii) what the CUDA table route of the backflow kernel assembles, against brute force over the
+    # 3 N_e coordinates: B_l = d_l A dense (rows of both spins couple through the Jacobian J of the backflow map),
+    #   E2_X = sum_l (Tr(A^-1 d_l A)^up + Tr(..)^dn)^2 - sum_l Tr((A^-1 d_l A)^2)^up - (..)^dn
+    # from per-spin tables T, E[q][p][l] (= M_l[p][q] of F.7 for B_l), Y2[q][p] (= sum_l Y_l[p][q] of F.9), division-free:
+    #   R^up R^dn E2_X = R^up R^dn E2_0 + 2 R^dn t0.e~^up + 2 R^up t0.e~^dn + 2 e~^up.e~^dn + R^dn b^up + R^up b^dn
+    n_up, n_dn, nv = 4, 3, 3
+    ne = n_up + n_dn
+    nc = 3 * ne
+    J = rng.standard_normal((ne, 3, nc)) * 0.3
+    for i in range(ne):
+        for a in range(3):
+            J[i, a, 3 * i + a] += 1.0
+    spins = [(0, n_up), (n_up, n_dn)]
+    A0s = [rng.standard_normal((m, m)) for _, m in spins]
+    Avs = [rng.standard_normal((m, nv)) for _, m in spins]
+    V0s = [rng.standard_normal((3, m, m)) for _, m in spins]
+    Vvs = [rng.standard_normal((3, m, nv)) for _, m in spins]
+
+    def brute(exc):
+        t1, s2, D = np.zeros((2, nc)), np.zeros(2), np.zeros(2)
+        for sp, (e0, m) in enumerate(spins):
+            A, V = A0s[sp].copy(), V0s[sp].copy()
+            for p, q in zip(*exc[sp]):
+                A[:, p] = Avs[sp][:, q]
+                V[:, :, p] = Vvs[sp][:, :, q]
+            Ai = np.linalg.inv(A)
+            D[sp] = np.linalg.det(A)
+            for l in range(nc):
+                G = Ai @ sum(V[a] * J[e0:e0 + m, a, l][:, None] for a in range(3))
+                t1[sp, l] = np.trace(G)
+                s2[sp] += np.trace(G @ G)
+        return D, np.sum((t1[0] + t1[1]) ** 2) - s2[0] - s2[1]
+
+    tab = []
+    for sp, (e0, m) in enumerate(spins):
+        rho = np.linalg.inv(A0s[sp])
+        T = rho @ Avs[sp]
+        W0 = np.array([V0s[sp][a] @ rho for a in range(3)])
+        mm = np.array([Vvs[sp][a] - V0s[sp][a] @ T for a in range(3)])
+        Js = J[e0:e0 + m]
+        g0 = np.array([[W0[a][i][i] for a in range(3)] for i in range(m)])
+        C = np.einsum('ial,jbl->iajb', Js, Js)
+        tab.append(dict(T=T, t0=np.einsum('ial,ia->l', Js, g0), E=np.einsum('ial,aiq,pi->qpl', Js, mm, rho),
+                        s0=np.einsum('iajb,aij,bji->', C, W0, W0), Y2=np.einsum('iajb,aij,bjq,pi->qp', C, W0, mm, rho),
+                        D0=np.linalg.det(A0s[sp])))
+    t0 = tab[0]['t0'] + tab[1]['t0']
+    E2_0 = t0 @ t0 - tab[0]['s0'] - tab[1]['s0']
+    cases = [(([], []), ([], [])), (([1], [2]), ([], [])), (([], []), ([0], [1])), (([2], [0]), ([1], [2])),
+             (([0, 3], [1, 2]), ([], [])), (([1, 2], [0, 2]), ([0, 2], [0, 1])), (([0], [0]), ([1, 2], [1, 2]))]
+    for exc in cases:
+        R, et, b = [1.0, 1.0], [np.zeros(nc), np.zeros(nc)], [0.0, 0.0]
+        for sp in range(2):
+            P, Q = exc[sp]
+            tb = tab[sp]
+            if len(P) == 1:
+                R[sp], et[sp], b[sp] = tb['T'][P[0], Q[0]], tb['E'][Q[0], P[0]], -2 * tb['Y2'][Q[0], P[0]]
+            elif len(P) == 2:
+                TPQ = tb['T'][np.ix_(P, Q)]
+                R[sp] = np.linalg.det(TPQ)
+                adj = np.array([[TPQ[1, 1], -TPQ[0, 1]], [-TPQ[1, 0], TPQ[0, 0]]])
+                Ml = np.array([[tb['E'][Q[bb], P[aa]] for bb in range(2)] for aa in range(2)])
+                Y2 = np.array([[tb['Y2'][Q[bb], P[aa]] for bb in range(2)] for aa in range(2)])
+                et[sp] = sum(adj[bb, aa] * Ml[aa, bb] for aa in range(2) for bb in range(2))
+                b[sp] = 2 * np.sum(Ml[0, 0] * Ml[1, 1] - Ml[0, 1] * Ml[1, 0]) - 2 * sum(adj[bb, aa] * Y2[aa, bb] for aa in range(2) for bb in range(2))
+        got = R[0] * R[1] * E2_0 + 2 * R[1] * (t0 @ et[0]) + 2 * R[0] * (t0 @ et[1]) + 2 * (et[0] @ et[1]) + R[1] * b[0] + R[0] * b[1]
+        D, E2 = brute(exc)
+        assert np.allclose([D[0] / tab[0]['D0'], D[1] / tab[1]['D0']], R, rtol=1e-10)
+        assert abs(R[0] * R[1] * E2 - got) < 1e-10 * max(1.0, abs(got)), (exc, R[0] * R[1] * E2, got)
