@@ -48,7 +48,8 @@ struct Variant {
   const void *k_frc, *k_frc_small;  // nuclear energy gradient (8 / 4 warps per block)
   const void *k_el_fuse, *e_el_fuse;   // E_L + fused eq. 6 reduction (without / with the e-e-n kernel)
   const void *b_psi, *b_metro, *b_el;  // backflow: values-only kernels, and the E_L kernel (explicit route)
-  int bf_ws_doubles;
+  const void *b_tab;                   // backflow E_L from the reference's tables (F.6-F.9)
+  int bf_ws_doubles, bf_tab_ws_doubles, bf_e_doubles;
   int frc_ws_doubles;
 };
 
@@ -82,6 +83,9 @@ Variant make_variant() {
   v.b_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsiOf<NS>, false, true>;
   v.b_el = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBf>;
   v.bf_ws_doubles = BfGeo<NS, NMO>::total;
+  v.b_tab = (const void *)backflow_tables_kernel<NS, NMO, kWarpsBf>;
+  v.bf_tab_ws_doubles = BfGeo<NS, NMO>::total2;
+  v.bf_e_doubles = BfGeo<NS, NMO>::eDoubles;
   v.e_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, false, true>;
   v.e_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsiOf<NS>, false, true>;
   v.e_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsiOf<NS>, true>;
@@ -214,6 +218,7 @@ struct qmc_system {
   struct Scratch {
     void *p = nullptr; size_t bytes = 0; unsigned long long *counter = nullptr;
     void *fuse = nullptr; size_t fuse_bytes = 0;  // qmc_local_energy_gradient: warp partials, parked O rows, order list
+    void *bf = nullptr; size_t bf_bytes = 0;      // backflow table route: E vectors per resident warp, flagged-walker list
   };
   std::mutex scratch_mu;
   std::unordered_map<cudaStream_t, Scratch> scratch;
@@ -221,8 +226,10 @@ struct qmc_system {
   // qmc_local_energy_host: two internal streams and double-buffered device scratch (grown on demand)
   bool fuse_ready = false; // fused E_L + eq. 6 kernel configured (lazily)
   int blocks_fuse = 0, smem_fuse = 0;
-  bool bf_ready = false;   // backflow E_L kernel configured (lazily)
-  int blocks_bf = 0;
+  bool bf_ready = false;   // backflow E_L kernels configured (lazily)
+  int blocks_bf = 0, blocks_bf_tab = 0, warps_bf_tab = 0;
+  void *d_bfdets = nullptr;  // BfDet records of the table route (null: the expansion has general determinants)
+  int n_bfdets = 0;
   bool frc_ready = false;  // nuclear energy-gradient kernel configured (lazily)
   int frc_warps = 0, blocks_frc = 0;
   bool orb_ready = false;  // orbital-derivative kernel configured (lazily: most users never call it)
@@ -276,6 +283,7 @@ void qmc_destroy(qmc_system_t *s) {
     cudaFree(kv.second.p);
     cudaFree(kv.second.counter);
     cudaFree(kv.second.fuse);
+    cudaFree(kv.second.bf);
   }
   for (void *q : s->retired) cudaFree(q);
   for (int i = 0; i < 2; ++i) {
@@ -283,6 +291,7 @@ void qmc_destroy(qmc_system_t *s) {
     cudaFree(s->hbuf[i]);
   }
   cudaFree(s->helo);
+  cudaFree(s->d_bfdets);
   delete s;
 }
 
@@ -751,6 +760,25 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     }
   }
 
+  // backflow table route: one compact record per determinant (caller order), when no determinant needs more than two
+  // substitutions in a spin
+  std::vector<BfDet> bfdets;
+  if (P.bf_w != 0.0 && gens.empty()) {
+    std::vector<Exc> by_orig(excs);
+    std::sort(by_orig.begin(), by_orig.end(), [](const Exc &a, const Exc &b) { return a.orig < b.orig; });
+    for (const Exc &x : by_orig) {
+      BfDet r{};
+      r.d = x.d;
+      for (int sp = 0; sp < 2; ++sp) {
+        r.k[sp] = (uint8_t)x.k[sp];
+        for (int t = 0; t < x.k[sp] && t < 2; ++t) {
+          r.p[sp][t] = (uint8_t)x.p[sp][t];
+          r.q[sp][t] = (uint8_t)x.q[sp][t];
+        }
+      }
+      bfdets.push_back(r);
+    }
+  }
   // ---- upload
   cudaError_t e = cudaSetDevice(device);
   if (e != cudaSuccess) { delete s; return cuda_fail(e, "cudaSetDevice"); }
@@ -776,6 +804,15 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     int rc = cuda_fail(e, "qmc_setup upload");
     qmc_destroy(s);
     return rc;
+  }
+  if (!bfdets.empty()) {
+    if ((e = cudaMalloc(&s->d_bfdets, bfdets.size() * sizeof(BfDet))) != cudaSuccess ||
+        (e = cudaMemcpy(s->d_bfdets, bfdets.data(), bfdets.size() * sizeof(BfDet), cudaMemcpyHostToDevice)) != cudaSuccess) {
+      int rc = cuda_fail(e, "qmc_setup upload (backflow records)");
+      qmc_destroy(s);
+      return rc;
+    }
+    s->n_bfdets = (int)bfdets.size();
   }
   P.exp_tab = (const double *)s->d_C + P.c_doubles;
   P.rng_tab = P.exp_tab + kExpTab;
@@ -864,11 +901,58 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
         CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, s->var.b_el, kWarpsBf * 32, smem));
         if (per_sm < 1) return QMC_EUNSUPPORTED;
         s->blocks_bf = per_sm * s->n_sm;
+        if (s->n_bfdets > 0) {  // the table route: as many warps per block (up to kWarpsBf) as shared memory holds
+          int wt = kWarpsBf;
+          while (wt > 1 && s->P.smem_const_bytes + wt * s->var.bf_tab_ws_doubles * (int)sizeof(double) > dev_smem) --wt;
+          const int smem_t = s->P.smem_const_bytes + wt * s->var.bf_tab_ws_doubles * (int)sizeof(double);
+          if (smem_t <= dev_smem) {
+            CK(cudaFuncSetAttribute(s->var.b_tab, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t));
+            CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, s->var.b_tab, wt * 32, smem_t));
+            if (per_sm >= 1) {
+              s->warps_bf_tab = wt;
+              s->blocks_bf_tab = per_sm * s->n_sm;
+            }
+          }
+        }
         s->bf_ready = true;
       }
     }
-    const int grid = (int)std::min<int64_t>((M + kWarpsBf - 1) / kWarpsBf, s->blocks_bf);
     void *bargs[2] = {(void *)&s->P, (void *)&io};
+    if (s->warps_bf_tab > 0 && !explicit_only) {
+      // tables first (F.6-F.9), then the explicit kernel over the walkers it listed
+      const int wt = s->warps_bf_tab;
+      const int grid_t = (int)std::min<int64_t>((M + wt - 1) / wt, s->blocks_bf_tab);
+      const size_t e_bytes = (size_t)grid_t * wt * (size_t)s->var.bf_e_doubles * sizeof(double);
+      const size_t need = e_bytes + (size_t)(M + 2) * sizeof(int);
+      unsigned char *base = nullptr;
+      {
+        std::lock_guard<std::mutex> lock(s->scratch_mu);
+        qmc_system::Scratch &sc = s->scratch[st];
+        if (sc.bf_bytes < need) {
+          if (sc.bf) s->retired.push_back(sc.bf);
+          sc.bf = nullptr;
+          sc.bf_bytes = 0;
+          CK(cudaMalloc(&sc.bf, need));
+          sc.bf_bytes = need;
+        }
+        base = static_cast<unsigned char *>(sc.bf);
+      }
+      int *li = reinterpret_cast<int *>(base + e_bytes);
+      CK(cudaMemsetAsync(li, 0, sizeof(int), st));
+      io.fb_count = li;
+      io.fb_list = li + 1;
+      const BfDet *dets = static_cast<const BfDet *>(s->d_bfdets);
+      int n_dets = s->n_bfdets;
+      double *esc = reinterpret_cast<double *>(base);
+      void *targs[5] = {(void *)&s->P, (void *)&io, (void *)&dets, (void *)&n_dets, (void *)&esc};
+      const int smem_t = s->P.smem_const_bytes + wt * s->var.bf_tab_ws_doubles * (int)sizeof(double);
+      CK(cudaLaunchKernel(s->var.b_tab, dim3(grid_t), dim3(wt * 32), targs, smem_t, st));
+      ++g_launches;
+      CK(cudaLaunchKernel(s->var.b_el, dim3(s->blocks_bf), dim3(kWarpsBf * 32), bargs, smem, st));
+      ++g_launches;
+      return QMC_OK;
+    }
+    const int grid = (int)std::min<int64_t>((M + kWarpsBf - 1) / kWarpsBf, s->blocks_bf);
     CK(cudaLaunchKernel(s->var.b_el, dim3(grid), dim3(kWarpsBf * 32), bargs, smem, st));
     ++g_launches;
     return QMC_OK;

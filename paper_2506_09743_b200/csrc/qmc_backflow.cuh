@@ -33,6 +33,9 @@ __device__ __forceinline__ void sym_mul(const Sym3 &a, const Sym3 &b, double o[9
 }
 
 constexpr int kBfLP = 8;  // lanes per (determinant, spin) problem: n_up, n_dn <= 8
+// fallback thresholds of the table route (as kFallbackK / kFallbackKappa of the plain path, tighter: the second-order
+// tables carry one more factor A0^-1)
+constexpr double kBfFallbackK = 1.0e4, kBfFallbackKappa = 1.0e4;
 
 template <int NS, int NMO>
 struct BfGeo {
@@ -43,33 +46,37 @@ struct BfGeo {
   static constexpr int oC = oS + 192;                  // [NE][NE][9] C blocks
   static constexpr int oMO = oC + NE * NE * 9;         // [5][NE][NMO] MO rows: value, operator, d_x, d_y, d_z
   static constexpr int oW = oMO + 5 * NE * NMO;        // [4][3][NS][NS] W^a of the four problems in flight
-  static constexpr int oPr = oW + 4 * 3 * NS * NS;     // [4][2] {det, trace}
+  static constexpr int oPr = oW + cmax(4 * 3 * NS * NS, 2 * 3 * NS * 8);  // [4][2] {det, trace}  (the W region also hosts the
+                                                                          // table route's R [2][3][NS][8])
   static constexpr int oP = oPr + 8;                   // [NE][NE][6] pair matrices
   static constexpr int total = (oP + NE * NE * 6 + 1) & ~1;
+  // table route (backflow_tables_kernel), per spin, with row
+  // stride 8:  T [NS][8], M1 [NS][8] (first-order table of the combined operator), rho = A0^-1 [NS][8], G = A0^-1 B0 [NS][8],
+  // W0 [3][NS][8], m [3][NS][8], Y2 [kMaxVirt(q)][8(p)], then scalars [8]
+  static constexpr int tSpin = 4 * NS * 8 + 2 * 3 * NS * 8 + kMaxVirt * 8;
+  static constexpr int oTab = total;                   // behind the common regions (bf_build fills those)
+  static constexpr int oSc = oTab + 2 * tSpin;
+  static constexpr int total2 = (oSc + 8 + 1) & ~1;
+  static constexpr int NC = 3 * NE;                    // coordinates l = 3 m + b
+  static constexpr int LS = (NC + 3) & ~3;             // stride of an E vector in the global scratch
+  static constexpr int eDoubles = 2 * kMaxVirt * NS * LS;  // E[sp][q][p][l] per warp (global memory, L2-resident)
 };
 
-template <int NS, int NMO, int WPB>
-__global__ void __launch_bounds__(WPB * 32, 1)
-    backflow_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
-  extern __shared__ __align__(16) unsigned char smem[];
+// Phases 1-2 of a backflow evaluation for walker w (one warp; lane = electron): Jastrow, potential, the backflow map and its
+// derivatives (pair matrices P, their sums S, the C blocks) and the five MO planes at the backflow coordinates (value,
+// combined operator B = -1/2 (C_ii : Hess + L_i . grad) - gt_i . grad, d_x, d_y, d_z) into the warp's scratch.
+// Jsh / esh: this lane's share of J and of -1/2 (lap J + |grad J|^2) + V_ee + V_en.
+template <int NS, int NMO>
+__device__ __forceinline__ void bf_build(const SysParams &P, const double *__restrict__ sCf, const double *__restrict__ sExp,
+                                         double *__restrict__ ws, const WalkerIO &io, int64_t w, int lane, double &Jsh, double &esh) {
   using BG = BfGeo<NS, NMO>;
   constexpr int NT = (NMO + 7) / 8;
-  // constants: C fragments and the exp table (the layout of load_constants)
-  double *sCf = reinterpret_cast<double *>(smem);
-  const int nC = P.c_doubles;
-  for (int i = threadIdx.x; i < nC; i += blockDim.x) sCf[i] = P.C[i];
-  double *sExp = sCf + nC;
-  for (int i = threadIdx.x; i < kExpTab + kRngTab; i += blockDim.x) sExp[i] = P.exp_tab[i];
-  __syncthreads();
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  double *ws = reinterpret_cast<double *>(smem + P.smem_const_bytes) + warp * BG::total;
-  double *sXYZ = ws + BG::oXYZ, *sGJ = ws + BG::oGJ, *sS = ws + BG::oS, *sCb = ws + BG::oC, *sMO = ws + BG::oMO,
-         *sW = ws + BG::oW, *sPr = ws + BG::oPr, *sP = ws + BG::oP;
-  const int n_up = P.n_up, n_dn = P.n_dn, ne = P.n_e;
+  double *sXYZ = ws + BG::oXYZ, *sGJ = ws + BG::oGJ, *sS = ws + BG::oS, *sCb = ws + BG::oC, *sMO = ws + BG::oMO, *sP = ws + BG::oP;
+  const int n_up = P.n_up, ne = P.n_e;
   const double bw = P.bf_w;
   const bool act = lane < ne;
   const int i = act ? lane : 0;
-  for (int64_t w = (int64_t)blockIdx.x * WPB + warp; w < io.M; w += (int64_t)gridDim.x * WPB) {
+  {
     double x = 0.37 + 0.11 * lane, y = -0.21 + 0.07 * lane, z = 0.53 - 0.05 * lane;
     if (act) {
       x = io.r_in[((int64_t)lane * 3 + 0) * io.M + w];
@@ -246,6 +253,33 @@ __global__ void __launch_bounds__(WPB * 32, 1)
       }
     }
     __syncwarp();
+    Jsh = act ? Jp : 0.0;
+    esh = act ? fma(-0.5, lapJ + fma(gJx, gJx, fma(gJy, gJy, gJz * gJz)), vee + ven) : 0.0;
+  }
+}
+
+template <int NS, int NMO, int WPB>
+__global__ void __launch_bounds__(WPB * 32, 1)
+    backflow_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  using BG = BfGeo<NS, NMO>;
+  // constants: C fragments and the exp table (the layout of load_constants)
+  double *sCf = reinterpret_cast<double *>(smem);
+  const int nC = P.c_doubles;
+  for (int i = threadIdx.x; i < nC; i += blockDim.x) sCf[i] = P.C[i];
+  double *sExp = sCf + nC;
+  for (int i = threadIdx.x; i < kExpTab + kRngTab; i += blockDim.x) sExp[i] = P.exp_tab[i];
+  __syncthreads();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  double *ws = reinterpret_cast<double *>(smem + P.smem_const_bytes) + warp * BG::total;
+  double *sCb = ws + BG::oC, *sMO = ws + BG::oMO, *sW = ws + BG::oW, *sPr = ws + BG::oPr;
+  const int n_up = P.n_up, n_dn = P.n_dn, ne = P.n_e;
+  // list mode (io.fb_list): only the walkers the table-route kernel flagged (nearly singular reference)
+  const int64_t n_work = io.fb_list ? (int64_t)*io.fb_count : io.M;
+  for (int64_t wk = (int64_t)blockIdx.x * WPB + warp; wk < n_work; wk += (int64_t)gridDim.x * WPB) {
+    const int64_t w = io.fb_list ? (int64_t)io.fb_list[wk] : wk;
+    double Js, es;
+    bf_build<NS, NMO>(P, sCf, sExp, ws, io, w, lane, Js, es);
     // ---- phase 3: every determinant on its own, two at a time (four (determinant, spin) problems of 8 lanes)
     const int c = lane & (kBfLP - 1), slot = lane >> 3, gbase = lane - c;
     const int dsel = slot >> 1, sp = slot & 1;
@@ -372,14 +406,357 @@ __global__ void __launch_bounds__(WPB * 32, 1)
     // ---- assembly (F.1, eq. 1): lanes 0 and 16 hold the sums of the even and odd determinants
     sig += __shfl_xor_sync(0xffffffffu, sig, 16);
     numk += __shfl_xor_sync(0xffffffffu, numk, 16);
-    double Js = act ? Jp : 0.0;
-    double es = act ? fma(-0.5, lapJ + fma(gJx, gJx, fma(gJy, gJy, gJz * gJz)), vee + ven) : 0.0;
 #pragma unroll
     for (int mm = 16; mm > 0; mm >>= 1) { Js += shfl_xor_d(Js, mm); es += shfl_xor_d(es, mm); }
     if (lane == 0) {
       if (io.logpsi) io.logpsi[w] = Js + log(fabs(sig));
       if (io.sign) io.sign[w] = (sig > 0.0) ? 1.0 : ((sig < 0.0) ? -1.0 : 0.0);
       if (io.eloc) io.eloc[w] = es + numk / sig + P.vnn;
+    }
+    __syncwarp();
+  }
+}
+
+// One determinant relative to the reference for the table route: substituted positions p and virtual indices q per spin
+// (k <= 2 per spin; expansions with more take the explicit kernel).  24 bytes.
+struct BfDet {
+  double d;
+  uint8_t k[2];
+  uint8_t p[2][2];
+  uint8_t q[2][2];
+  uint8_t pad[6];
+};
+
+// ---------------------------------------------------------------------------------
+// The accelerated route (F.6-F.9): only the reference determinant of each spin is eliminated; every
+// other determinant comes from tables.  With B_l = d_l A (dense: every row depends on every coordinate l through the
+// Jacobian J of the backflow map) the paper's tables are, per spin,
+//   T = A0^-1 Av,   M_l = A0^-1 B_l,v - A0^-1 B_l,0 T  (F.7),   Y_l = A0^-1 B_l,0 M_l  (F.9),
+// and here (derivation pinned by tests/test_oracle_pins.py::test_P14b...):
+//   rho = A0^-1,  W0^a = V0^a rho,  m^a = Vv^a - V0^a T   (V^a = d_a phi rows),
+//   E[q][p][l] = M_l[p][q] = sum_i rho[p][i] sum_a J_il^a m^a[i][q]     (42-vectors, kept in a per-warp global scratch)
+//   Y2[q][p]   = sum_l Y_l[p][q] = sum_i rho[p][i] sum_{i',a'} (sum_a C_ii'^{aa'} W0^a[i][i']) m^{a'}[i'][q]
+//   t0_l = sum_i sum_a J_il^a W0^a[i][i],   s0 = sum_{ii'} C_ii' : W0[i][i'] (x) W0[i'][i],   E2_0 = |t0|^2 - s0^up - s0^dn
+// and per determinant (substitution blocks T_PQ, k <= 2 per spin), division-free:
+//   R = det T_PQ,  e~_l = Tr(adj(T_PQ) E_PQ,l),  b = 2 sum_l det(E_PQ,l) [k = 2] - 2 Tr(adj(T_PQ) Y2_PQ)
+//   R^up R^dn E2_X = R^up R^dn E2_0 + 2 R^dn t0.e~^up + 2 R^up t0.e~^dn + 2 e~^up.e~^dn + R^dn b^up + R^up b^dn
+// so that  -1/2 lap Psi / Psi = -1/2 (lap J + |grad J|^2) + [ den (t^up + t^dn) + num1 - 1/2 sum_n d_n R R E2_n ] / den
+// with den, num1 the first-order sums of the plain path (combined operator B of bf_build).  One walker per warp; lane l
+// accumulates the l-dependent part over all determinants, one warp reduction at the end.  Walkers whose reference is
+// nearly singular (kappa / (Sigma/D0) criteria of section 5.6) are listed for the explicit kernel.
+// ---------------------------------------------------------------------------------
+template <int NS, int NMO, int WPB>
+__global__ void __launch_bounds__(WPB * 32, 1)
+    backflow_tables_kernel(const __grid_constant__ SysParams P, const WalkerIO io, const BfDet *__restrict__ dets, int n_dets,
+                           double *__restrict__ escratch) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  using BG = BfGeo<NS, NMO>;
+  double *sCf = reinterpret_cast<double *>(smem);
+  const int nC = P.c_doubles;
+  for (int i = threadIdx.x; i < nC; i += blockDim.x) sCf[i] = P.C[i];
+  double *sExp = sCf + nC;
+  for (int i = threadIdx.x; i < kExpTab + kRngTab; i += blockDim.x) sExp[i] = P.exp_tab[i];
+  __syncthreads();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  double *ws = reinterpret_cast<double *>(smem + P.smem_const_bytes) + warp * BG::total2;
+  const double *sCb = ws + BG::oC, *sMO = ws + BG::oMO, *sP = ws + BG::oP, *sS = ws + BG::oS;
+  double *sTab = ws + BG::oTab, *sSc = ws + BG::oSc;
+  const int wpb = (int)(blockDim.x >> 5);  // warps launched per block (<= WPB)
+  double *E = escratch + ((int64_t)blockIdx.x * wpb + warp) * BG::eDoubles;
+  const int n_up = P.n_up, n_dn = P.n_dn, ne = P.n_e, nc = 3 * ne;
+  constexpr int LS = BG::LS;
+  // regions of one spin's tables
+  auto tabT = [&](int sp) { return sTab + sp * BG::tSpin; };
+  auto tabM1 = [&](int sp) { return sTab + sp * BG::tSpin + NS * 8; };
+  auto tabRho = [&](int sp) { return sTab + sp * BG::tSpin + 2 * NS * 8; };
+  auto tabG = [&](int sp) { return sTab + sp * BG::tSpin + 3 * NS * 8; };
+  auto tabW0 = [&](int sp) { return sTab + sp * BG::tSpin + 4 * NS * 8; };
+  auto tabMq = [&](int sp) { return sTab + sp * BG::tSpin + 4 * NS * 8 + 3 * NS * 8; };
+  auto tabY2 = [&](int sp) { return sTab + sp * BG::tSpin + 4 * NS * 8 + 6 * NS * 8; };
+  for (int64_t w = (int64_t)blockIdx.x * wpb + warp; w < io.M; w += (int64_t)gridDim.x * wpb) {
+    double Js, es;
+    bf_build<NS, NMO>(P, sCf, sExp, ws, io, w, lane, Js, es);
+    // ---- reference elimination: [A0 | Av | B0 | Bv | 1], lanes 0-7 spin up, 8-15 spin down (lane c = column c)
+    const int c = lane & 7, sp = (lane >> 3) & 1;
+    const int ns = sp ? n_dn : n_up, nv = P.nv[sp], e0 = sp ? n_up : 0;
+    double detv = 1.0, t0v = 0.0, kap = 0.0;
+    {
+      double a0[NS], av[NS], b0[NS], bv[NS], ai[NS];
+      const bool cA = c < ns, cV = c < nv;
+      const int colA = cA ? P.ref_col[sp][c] : 0, colV = cV ? P.virt_col[sp][c] : 0;
+#pragma unroll
+      for (int q = 0; q < NS; ++q) {
+        const bool rq = q < ns;
+        const int row = e0 + (rq ? q : 0);
+        a0[q] = (rq && cA) ? sMO[(0 * BG::NE + row) * NMO + colA] : ((q == c) ? 1.0 : 0.0);
+        av[q] = (rq && cV) ? sMO[(0 * BG::NE + row) * NMO + colV] : 0.0;
+        b0[q] = (rq && cA) ? sMO[(1 * BG::NE + row) * NMO + colA] : 0.0;
+        bv[q] = (rq && cV) ? sMO[(1 * BG::NE + row) * NMO + colV] : 0.0;
+        ai[q] = (rq && cA && q == c) ? 1.0 : 0.0;
+      }
+      int perm[NS];
+      int myrow = 0;
+      bool used = !(c < NS);
+      const int gbase = lane - c;
+#pragma unroll
+      for (int k = 0; k < NS; ++k) {
+        unsigned key = used ? 0u : (((unsigned)(__double2hiint(a0[k]) & 0x7fffffff) & ~7u) | (unsigned)c);
+#pragma unroll
+        for (int mm = 1; mm < 8; mm <<= 1) key = max(key, __shfl_xor_sync(0xffffffffu, key, mm));
+        const int pl = (int)(key & 7u);
+        perm[k] = pl;
+        if (c == pl) { used = true; myrow = k; }
+        double f[NS];
+#pragma unroll
+        for (int q = 0; q < NS; ++q) f[q] = __shfl_sync(0xffffffffu, a0[q], gbase + pl);
+        const double piv = f[k], inv = 1.0 / piv;
+        detv *= piv;
+#define QMC_BF_ELIM(v)                                                  \
+        {                                                               \
+          const double t = v[k] * inv;                                  \
+          v[k] = t;                                                     \
+          _Pragma("unroll") for (int q = 0; q < NS; ++q) if (q != k) v[q] = fma(-f[q], t, v[q]); \
+        }
+        QMC_BF_ELIM(a0) QMC_BF_ELIM(av) QMC_BF_ELIM(b0) QMC_BF_ELIM(bv) QMC_BF_ELIM(ai)
+#undef QMC_BF_ELIM
+      }
+      int inversions = 0;
+#pragma unroll
+      for (int k = 0; k < NS; ++k)
+#pragma unroll
+        for (int k2 = k + 1; k2 < NS; ++k2) inversions += (perm[k] > perm[k2]) ? 1 : 0;
+      if (inversions & 1) detv = -detv;
+#pragma unroll
+      for (int q = 0; q < NS; ++q) if (q == myrow && c < NS) t0v = b0[q];
+#pragma unroll
+      for (int mm = 1; mm < 8; mm <<= 1) t0v += shfl_xor_d(t0v, mm);
+      unsigned kk = 0u;
+#pragma unroll
+      for (int k = 0; k < NS; ++k) kk = max(kk, (unsigned)(__double2hiint(av[k]) & 0x7fffffff));
+#pragma unroll
+      for (int mm = 1; mm < 8; mm <<= 1) kk = max(kk, __shfl_xor_sync(0xffffffffu, kk, mm));
+      kap = __hiloint2double((int)min(kk, 0x7ff00000u), 0);
+      if (lane < 16) {  // rows in position order: row k of the reduced blocks belongs to position perm[k]
+        double *T = tabT(sp), *H = tabM1(sp), *Rho = tabRho(sp), *G = tabG(sp);
+#pragma unroll
+        for (int k = 0; k < NS; ++k) {
+          T[perm[k] * 8 + c] = av[k];
+          H[perm[k] * 8 + c] = bv[k];    // A0^-1 Bv for now
+          Rho[perm[k] * 8 + c] = ai[k];  // A0^-1[position][electron c]
+          G[perm[k] * 8 + c] = b0[k];    // (A0^-1 B0)[position][position c]
+        }
+      }
+    }
+    __syncwarp();
+    // ---- first-order table M1 = A0^-1 Bv - (A0^-1 B0) T (F.7 for the combined operator), lane c = virtual q
+    if (lane < 16 && c < nv) {
+      double *T = tabT(sp), *M1 = tabM1(sp), *G = tabG(sp);
+      for (int p2 = 0; p2 < ns; ++p2) {
+        double t = M1[p2 * 8 + c];
+        for (int j = 0; j < ns; ++j) t = fma(-G[p2 * 8 + j], T[j * 8 + c], t);
+        M1[p2 * 8 + c] = t;
+      }
+    }
+    // ---- W0^a = V0^a rho (lane c = electron i'), m^a = Vv^a - V0^a T (lane c = virtual q)
+    if (lane < 16) {
+      const double *T = tabT(sp), *Rho = tabRho(sp);
+      double *W0 = tabW0(sp), *Mq = tabMq(sp);
+      for (int a = 0; a < 3; ++a)
+        for (int i = 0; i < ns; ++i) {
+          const double *vrow = sMO + ((2 + a) * BG::NE + e0 + i) * NMO;
+          double tw = 0.0, tm = (c < nv) ? vrow[P.virt_col[sp][c < kMaxVirt ? c : 0]] : 0.0;
+          for (int k = 0; k < ns; ++k) {
+            const double v = vrow[P.ref_col[sp][k]];
+            tw = fma(v, Rho[k * 8 + c], tw);
+            tm = fma(-v, T[k * 8 + c], tm);
+          }
+          W0[(a * NS + i) * 8 + c] = (c < ns) ? tw : 0.0;
+          Mq[(a * NS + i) * 8 + c] = (c < nv) ? tm : 0.0;
+        }
+    }
+    __syncwarp();
+    // column b of the (symmetric) Jacobian block J_im = d rt_i / d r_m:  1 + S_i (m = i),  -P_im (m != i)
+    auto jcol = [&](int i, int m, int b, double &j0, double &j1, double &j2) {
+      double xx, yy, zz, xy, yz, zx;
+      if (i == m) {
+        xx = 1.0 + sS[i]; yy = 1.0 + sS[32 + i]; zz = 1.0 + sS[64 + i]; xy = sS[96 + i]; yz = sS[128 + i]; zx = sS[160 + i];
+      } else {
+        const double *pp = sP + (i * ne + m) * 6;
+        xx = -pp[0]; yy = -pp[1]; zz = -pp[2]; xy = -pp[3]; yz = -pp[4]; zx = -pp[5];
+      }
+      j0 = (b == 0) ? xx : ((b == 1) ? xy : zx);
+      j1 = (b == 0) ? xy : ((b == 1) ? yy : yz);
+      j2 = (b == 0) ? zx : ((b == 1) ? yz : zz);
+    };
+    // ---- t0_l and the E vectors, lane = coordinate l = 3 m + b (two rounds)
+    double t0l[2] = {0.0, 0.0};
+    for (int rd = 0; rd < 2; ++rd) {
+      const int l = lane + 32 * rd;
+      if (l < nc) {
+        const int m = l / 3, b = l - 3 * m;
+        double t = 0.0;
+        for (int s2 = 0; s2 < 2; ++s2) {
+          const int ns2 = s2 ? n_dn : n_up, nv2 = P.nv[s2], f0 = s2 ? n_up : 0;
+          const double *W0 = tabW0(s2), *Mq = tabMq(s2), *Rho = tabRho(s2);
+          double jc[NS][3];
+#pragma unroll
+          for (int i = 0; i < NS; ++i) {
+            jc[i][0] = jc[i][1] = jc[i][2] = 0.0;
+            if (i < ns2) {
+              jcol(f0 + i, m, b, jc[i][0], jc[i][1], jc[i][2]);
+              t = fma(jc[i][0], W0[(0 * NS + i) * 8 + i], fma(jc[i][1], W0[(1 * NS + i) * 8 + i], fma(jc[i][2], W0[(2 * NS + i) * 8 + i], t)));
+            }
+          }
+          for (int q = 0; q < nv2; ++q) {
+            double acc[NS];
+#pragma unroll
+            for (int p2 = 0; p2 < NS; ++p2) acc[p2] = 0.0;
+#pragma unroll
+            for (int i = 0; i < NS; ++i) {
+              if (i < ns2) {
+                const double f = fma(jc[i][0], Mq[(0 * NS + i) * 8 + q], fma(jc[i][1], Mq[(1 * NS + i) * 8 + q], jc[i][2] * Mq[(2 * NS + i) * 8 + q]));
+#pragma unroll
+                for (int p2 = 0; p2 < NS; ++p2) acc[p2] = fma(Rho[p2 * 8 + i], f, acc[p2]);
+              }
+            }
+#pragma unroll
+            for (int p2 = 0; p2 < NS; ++p2)
+              if (p2 < ns2) __stcg(E + ((s2 * kMaxVirt + q) * NS + p2) * LS + l, acc[p2]);
+          }
+        }
+        t0l[rd] = t;
+      }
+    }
+    // ---- R^{a'}[i][i'] = sum_a C_ii'^{aa'} W0^a[i][i'] (lane c = i'), s0, then Y2[q][p] (lane c = q)
+    double *sR = ws + BG::oW;
+    double s0v = 0.0;
+    if (lane < 16) {
+      const double *W0 = tabW0(sp);
+      if (c < ns)
+        for (int i = 0; i < ns; ++i) {
+          const double *cb = sCb + ((e0 + i) * ne + e0 + c) * 9;
+          const double w0 = W0[(0 * NS + i) * 8 + c], w1 = W0[(1 * NS + i) * 8 + c], w2 = W0[(2 * NS + i) * 8 + c];
+#pragma unroll
+          for (int a2 = 0; a2 < 3; ++a2) {
+            const double r = fma(cb[0 + a2], w0, fma(cb[3 + a2], w1, cb[6 + a2] * w2));
+            sR[((sp * 3 + a2) * NS + i) * 8 + c] = r;
+            s0v = fma(r, W0[(a2 * NS + c) * 8 + i], s0v);
+          }
+        }
+    }
+#pragma unroll
+    for (int mm = 1; mm < 8; mm <<= 1) s0v += shfl_xor_d(s0v, mm);
+    __syncwarp();
+    if (lane < 16 && c < nv) {
+      const double *Mq = tabMq(sp), *Rho = tabRho(sp);
+      double *Y2 = tabY2(sp);
+      double S2[NS];
+#pragma unroll
+      for (int i = 0; i < NS; ++i) {
+        S2[i] = 0.0;
+        if (i < ns) {
+          double t = 0.0;
+          for (int i2 = 0; i2 < ns; ++i2)
+#pragma unroll
+            for (int a2 = 0; a2 < 3; ++a2) t = fma(sR[((sp * 3 + a2) * NS + i) * 8 + i2], Mq[(a2 * NS + i2) * 8 + c], t);
+          S2[i] = t;
+        }
+      }
+      for (int p2 = 0; p2 < ns; ++p2) {
+        double t = 0.0;
+#pragma unroll
+        for (int i = 0; i < NS; ++i)
+          if (i < ns) t = fma(Rho[p2 * 8 + i], S2[i], t);
+        Y2[c * 8 + p2] = t;
+      }
+    }
+    if (c == 0 && lane < 16) {
+      sSc[sp * 4 + 0] = detv;
+      sSc[sp * 4 + 1] = t0v;
+      sSc[sp * 4 + 2] = s0v;
+      sSc[sp * 4 + 3] = kap;
+    }
+    __syncwarp();
+    // ---- CI sum over the determinants: uniform scalars in every lane, the l-dependent part per lane
+    {
+      const double *Tu = tabT(0), *Td = tabT(1), *M1u = tabM1(0), *M1d = tabM1(1), *Y2u = tabY2(0), *Y2d = tabY2(1);
+      double den = 0.0, num1 = 0.0, uni = 0.0, accl = 0.0;
+      const int l0 = lane, l1 = lane + 32;
+      const bool has1 = l1 < nc, has0 = l0 < nc;
+      for (int n = 0; n < n_dets; ++n) {
+        const uint2 *raw = reinterpret_cast<const uint2 *>(dets + n);
+        const uint2 w0 = __ldg(raw), w1 = __ldg(raw + 1);
+        const double d = __hiloint2double((int)w0.y, (int)w0.x);
+        const unsigned ku = w1.x & 255u, kd = (w1.x >> 8) & 255u;
+        // bytes: k[0] k[1] | p[0][0] p[0][1] p[1][0] p[1][1] q[0][0] q[0][1] | q[1][0] q[1][1] pad...
+        const unsigned pu0 = (w1.x >> 16) & 255u, pu1 = w1.x >> 24, pd0 = w1.y & 255u, pd1 = (w1.y >> 8) & 255u;
+        const unsigned qu0 = (w1.y >> 16) & 255u, qu1 = w1.y >> 24;
+        const uint2 w2 = __ldg(raw + 2);
+        const unsigned qd0 = w2.x & 255u, qd1 = (w2.x >> 8) & 255u;
+        double R[2], Rd[2], trY[2], e0v[2], e1v[2], dm0[2], dm1[2];
+#pragma unroll
+        for (int s2 = 0; s2 < 2; ++s2) {
+          const unsigned k = s2 ? kd : ku, p0 = s2 ? pd0 : pu0, p1 = s2 ? pd1 : pu1, q0 = s2 ? qd0 : qu0, q1 = s2 ? qd1 : qu1;
+          const double *T = s2 ? Td : Tu, *M1 = s2 ? M1d : M1u, *Y2 = s2 ? Y2d : Y2u;
+          const double *Es = E + (int64_t)s2 * kMaxVirt * NS * LS;
+          R[s2] = 1.0; Rd[s2] = 0.0; trY[s2] = 0.0; e0v[s2] = e1v[s2] = dm0[s2] = dm1[s2] = 0.0;
+          if (k == 1) {
+            R[s2] = T[p0 * 8 + q0];
+            Rd[s2] = M1[p0 * 8 + q0];
+            trY[s2] = Y2[q0 * 8 + p0];
+            const double *e = Es + (q0 * NS + p0) * LS;
+            if (has0) e0v[s2] = __ldcg(e + l0);
+            if (has1) e1v[s2] = __ldcg(e + l1);
+          } else if (k == 2) {
+            const double t11 = T[p0 * 8 + q0], t12 = T[p0 * 8 + q1], t21 = T[p1 * 8 + q0], t22 = T[p1 * 8 + q1];
+            R[s2] = fma(t11, t22, -t12 * t21);
+            Rd[s2] = fma(t22, M1[p0 * 8 + q0], fma(t11, M1[p1 * 8 + q1], -fma(t12, M1[p1 * 8 + q0], t21 * M1[p0 * 8 + q1])));
+            trY[s2] = fma(t22, Y2[q0 * 8 + p0], fma(t11, Y2[q1 * 8 + p1], -fma(t12, Y2[q0 * 8 + p1], t21 * Y2[q1 * 8 + p0])));
+            const double *e11 = Es + (q0 * NS + p0) * LS, *e12 = Es + (q1 * NS + p0) * LS, *e21 = Es + (q0 * NS + p1) * LS,
+                         *e22 = Es + (q1 * NS + p1) * LS;
+            if (has0) {
+              const double a = __ldcg(e11 + l0), b2 = __ldcg(e12 + l0), c2 = __ldcg(e21 + l0), dd = __ldcg(e22 + l0);
+              e0v[s2] = fma(t22, a, fma(t11, dd, -fma(t12, c2, t21 * b2)));
+              dm0[s2] = fma(a, dd, -b2 * c2);
+            }
+            if (has1) {
+              const double a = __ldcg(e11 + l1), b2 = __ldcg(e12 + l1), c2 = __ldcg(e21 + l1), dd = __ldcg(e22 + l1);
+              e1v[s2] = fma(t22, a, fma(t11, dd, -fma(t12, c2, t21 * b2)));
+              dm1[s2] = fma(a, dd, -b2 * c2);
+            }
+          }
+        }
+        den = fma(d * R[0], R[1], den);                                        // eq. 4
+        num1 = fma(d, fma(Rd[0], R[1], R[0] * Rd[1]), num1);                   // F.6 (first order)
+        uni = fma(-2.0 * d, fma(R[1], trY[0], R[0] * trY[1]), uni);            // F.9 (summed over l)
+        const double x0 = fma(t0l[0], fma(R[1], e0v[0], R[0] * e0v[1]), fma(e0v[0], e0v[1], fma(R[1], dm0[0], R[0] * dm0[1])));
+        const double x1 = fma(t0l[1], fma(R[1], e1v[0], R[0] * e1v[1]), fma(e1v[0], e1v[1], fma(R[1], dm1[0], R[0] * dm1[1])));
+        accl = fma(2.0 * d, x0 + x1, accl);
+      }
+      double tt = fma(t0l[0], t0l[0], t0l[1] * t0l[1]);
+#pragma unroll
+      for (int mm = 16; mm > 0; mm >>= 1) {
+        accl += shfl_xor_d(accl, mm);
+        tt += shfl_xor_d(tt, mm);
+        Js += shfl_xor_d(Js, mm);
+        es += shfl_xor_d(es, mm);
+      }
+      if (lane == 0) {
+        const double du = sSc[0], dd = sSc[4];
+        const double second = fma(den, tt - sSc[2] - sSc[6], uni + accl);
+        const double numt = fma(den, sSc[1] + sSc[5], num1) - 0.5 * second;
+        const double sig = du * dd * den;
+        const double eloc = es + numt / den + P.vnn;
+        if (io.logpsi) io.logpsi[w] = Js + log(fabs(du)) + log(fabs(dd)) + log(fabs(den));
+        if (io.sign) io.sign[w] = (sig > 0.0) ? 1.0 : ((sig < 0.0) ? -1.0 : 0.0);
+        if (io.eloc) io.eloc[w] = eloc;
+        // nearly singular reference: the explicit kernel re-evaluates the walker (criteria of DESIGN.md section 5.6; the
+        // second-order tables amplify by one more power of kappa, hence the lower thresholds)
+        const double ku2 = sSc[3], kd2 = sSc[7], scale = fmax(1.0, fabs(eloc));
+        const bool ok = (den * den <= fmin(kBfFallbackK * scale, kFallbackCap)) && (ku2 * ku2 <= kBfFallbackKappa * scale) &&
+                        (kd2 * kd2 <= kBfFallbackKappa * scale);
+        if (!ok && io.fb_list) io.fb_list[atomicAdd(io.fb_count, 1)] = (int)w;
+      }
     }
     __syncwarp();
   }
