@@ -334,7 +334,7 @@ def main():
         if k >= 3:
             t_f += a.elapsed_time(b) * 1e-3
             t_fr += b.elapsed_time(c) * 1e-3
-    # NEXT-3: the same wavefunction with the inverse backflow transformation (w = 0.05): E_L by the explicit-route
+    # NEXT-3: the same wavefunction with the inverse backflow transformation (w = 0.05): E_L by the table-route
     # backflow kernel, log|Psi| and the sampler with the orbitals at the backflow coordinates
     import copy
     d_bf = copy.copy(d)
@@ -453,8 +453,9 @@ def main():
             "backflow": {"w": 0.05, "ms_local_energy": 1e3 * t_b[0] / K_DERIV, "walkers_local_energy": int(M_orb),
                          "ms_log_psi": 1e3 * t_b[1] / K_DERIV, "ms_metropolis": 1e3 * t_b[2] / K_DERIV, "walkers": int(M),
                          "walker_steps_per_s": world * M * n_sweeps / (t_b[2] / K_DERIV),
-                         "note": "SURVEY 8(f) NEXT-3: inverse backflow K_BF = w/r; E_L on the explicit route (every determinant "
-                                 "eliminated on its own), values-only kernels on the excitation tables"},
+                         "note": "SURVEY 8(f) NEXT-3: inverse backflow K_BF = w/r; E_L from the reference's tables (F.6-F.9, "
+                                 "explicit route for walkers with a nearly singular reference), values-only kernels on "
+                                 "the excitation tables"},
             "gpu_launches": int(launches),
             "clocks": clocks,
             "last_step": {"mean_E_L": mean, "stderr": err},

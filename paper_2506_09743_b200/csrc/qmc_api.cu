@@ -83,9 +83,9 @@ Variant make_variant() {
   v.b_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsiOf<NS>, false, true>;
   v.b_el = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBf>;
   v.bf_ws_doubles = BfGeo<NS, NMO>::total;
-  v.b_tab = (const void *)backflow_tables_kernel<NS, NMO, kWarpsBf>;
-  v.bf_tab_ws_doubles = BfGeo<NS, NMO>::total2;
-  v.bf_e_doubles = BfGeo<NS, NMO>::eDoubles;
+  v.b_tab = (const void *)backflow_tables_kernel<NS, NMO, kWarpsBfTab>;
+  v.bf_tab_ws_doubles = BfGeoT<NS, NMO>::total;
+  v.bf_e_doubles = BfGeoT<NS, NMO>::eDoubles;
   v.e_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, false, true>;
   v.e_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsiOf<NS>, false, true>;
   v.e_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsiOf<NS>, true>;
@@ -901,8 +901,8 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
         CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, s->var.b_el, kWarpsBf * 32, smem));
         if (per_sm < 1) return QMC_EUNSUPPORTED;
         s->blocks_bf = per_sm * s->n_sm;
-        if (s->n_bfdets > 0) {  // the table route: as many warps per block (up to kWarpsBf) as shared memory holds
-          int wt = kWarpsBf;
+        if (s->n_bfdets > 0) {  // the table route: as many warps per block (up to kWarpsBfTab) as shared memory holds
+          int wt = kWarpsBfTab;
           while (wt > 1 && s->P.smem_const_bytes + wt * s->var.bf_tab_ws_doubles * (int)sizeof(double) > dev_smem) --wt;
           const int smem_t = s->P.smem_const_bytes + wt * s->var.bf_tab_ws_doubles * (int)sizeof(double);
           if (smem_t <= dev_smem) {

@@ -46,32 +46,49 @@ struct BfGeo {
   static constexpr int oC = oS + 192;                  // [NE][NE][9] C blocks
   static constexpr int oMO = oC + NE * NE * 9;         // [5][NE][NMO] MO rows: value, operator, d_x, d_y, d_z
   static constexpr int oW = oMO + 5 * NE * NMO;        // [4][3][NS][NS] W^a of the four problems in flight
-  static constexpr int oPr = oW + cmax(4 * 3 * NS * NS, 2 * 3 * NS * 8);  // [4][2] {det, trace}  (the W region also hosts the
-                                                                          // table route's R [2][3][NS][8])
+  static constexpr int oPr = oW + 4 * 3 * NS * NS;     // [4][2] {det, trace}
   static constexpr int oP = oPr + 8;                   // [NE][NE][6] pair matrices
   static constexpr int total = (oP + NE * NE * 6 + 1) & ~1;
-  // table route (backflow_tables_kernel), per spin, with row
-  // stride 8:  T [NS][8], M1 [NS][8] (first-order table of the combined operator), rho = A0^-1 [NS][8], G = A0^-1 B0 [NS][8],
-  // W0 [3][NS][8], m [3][NS][8], Y2 [kMaxVirt(q)][8(p)], then scalars [8]
+  static constexpr bool kTab = false;
+  __device__ static __forceinline__ int pofs(int i, int m, int ne) { return (i * ne + m) * 6; }  // P_im, both orders stored
+};
+
+// Scratch of the table route (backflow_tables_kernel): no off-diagonal C blocks (the same-spin ones are formed pair by
+// pair where they are contracted, the cross-spin ones enter only through t0), each pair matrix once (P_im = P_mi).
+// Per spin, with row stride 8:  T [NS][8], M1 [NS][8] (first-order table of the combined operator), rho = A0^-1 [NS][8],
+// G = A0^-1 B0 [NS][8], W0 [3][NS][8], m [3][NS][8], Y2 [kMaxVirt(q)][8(p)]; then scalars [8].
+template <int NS, int NMO>
+struct BfGeoT {
+  static constexpr int NE = 2 * NS;
+  static constexpr int oXYZ = 0;                       // [3][32] electron coordinates
+  static constexpr int oGJ = oXYZ + 96;                // [3][32] grad_i J
+  static constexpr int oS = oGJ + 96;                  // [6][32] S_i = sum_j P_ij
+  static constexpr int oCd = oS + 192;                 // [6][32] diagonal blocks C_ii (symmetric)
+  static constexpr int oMO = oCd + 192;                // [5][NE][NMO] MO rows, later R [2][3][NS][8]
+  static constexpr int oP = oMO + cmax(5 * NE * NMO, 2 * 3 * NS * 8);  // [NE (NE - 1) / 2][6] pair matrices
   static constexpr int tSpin = 4 * NS * 8 + 2 * 3 * NS * 8 + kMaxVirt * 8;
-  static constexpr int oTab = total;                   // behind the common regions (bf_build fills those)
+  static constexpr int oTab = oP + cmax(NE * (NE - 1) / 2, 1) * 6;
   static constexpr int oSc = oTab + 2 * tSpin;
-  static constexpr int total2 = (oSc + 8 + 1) & ~1;
+  static constexpr int total = (oSc + 8 + 1) & ~1;
   static constexpr int NC = 3 * NE;                    // coordinates l = 3 m + b
   static constexpr int LS = (NC + 3) & ~3;             // stride of an E vector in the global scratch
   static constexpr int eDoubles = 2 * kMaxVirt * NS * LS;  // E[sp][q][p][l] per warp (global memory, L2-resident)
+  static constexpr bool kTab = true;
+  __device__ static __forceinline__ int pofs(int i, int m, int ne) {
+    const int a = min(i, m), b = max(i, m);
+    return ((a * (2 * ne - a - 1)) / 2 + (b - a - 1)) * 6;
+  }
 };
 
 // Phases 1-2 of a backflow evaluation for walker w (one warp; lane = electron): Jastrow, potential, the backflow map and its
 // derivatives (pair matrices P, their sums S, the C blocks) and the five MO planes at the backflow coordinates (value,
 // combined operator B = -1/2 (C_ii : Hess + L_i . grad) - gt_i . grad, d_x, d_y, d_z) into the warp's scratch.
 // Jsh / esh: this lane's share of J and of -1/2 (lap J + |grad J|^2) + V_ee + V_en.
-template <int NS, int NMO>
+template <int NS, int NMO, class BG>
 __device__ __forceinline__ void bf_build(const SysParams &P, const double *__restrict__ sCf, const double *__restrict__ sExp,
                                          double *__restrict__ ws, const WalkerIO &io, int64_t w, int lane, double &Jsh, double &esh) {
-  using BG = BfGeo<NS, NMO>;
   constexpr int NT = (NMO + 7) / 8;
-  double *sXYZ = ws + BG::oXYZ, *sGJ = ws + BG::oGJ, *sS = ws + BG::oS, *sCb = ws + BG::oC, *sMO = ws + BG::oMO, *sP = ws + BG::oP;
+  double *sXYZ = ws + BG::oXYZ, *sGJ = ws + BG::oGJ, *sS = ws + BG::oS, *sMO = ws + BG::oMO, *sP = ws + BG::oP;
   const int n_up = P.n_up, ne = P.n_e;
   const double bw = P.bf_w;
   const bool act = lane < ne;
@@ -112,8 +129,8 @@ __device__ __forceinline__ void bf_build(const SysParams &P, const double *__res
       S2.xy = fma(eta, Pm.xy, S2.xy); S2.yz = fma(eta, Pm.yz, S2.yz); S2.zx = fma(eta, Pm.zx, S2.zx);
       const double l3 = -4.0 * bw * ri * ri * ri;
       Lx = fma(l3, dx, Lx); Ly = fma(l3, dy, Ly); Lz = fma(l3, dz, Lz);
-      if (act) {
-        double *pp = sP + (i * ne + j) * 6;
+      if (act && (!BG::kTab || j > i)) {
+        double *pp = sP + BG::pofs(i, j, ne);
         pp[0] = Pm.xx; pp[1] = Pm.yy; pp[2] = Pm.zz; pp[3] = Pm.xy; pp[4] = Pm.yz; pp[5] = Pm.zx;
       }
     }
@@ -132,7 +149,7 @@ __device__ __forceinline__ void bf_build(const SysParams &P, const double *__res
     const Sym3 Ji{1.0 + S.xx, 1.0 + S.yy, 1.0 + S.zz, S.xy, S.yz, S.zx};
     for (int m = 0; m < ne; ++m) {
       if (m == i) continue;
-      const double *pp = sP + (i * ne + m) * 6;
+      const double *pp = sP + BG::pofs(i, m, ne);
       const double ax = sGJ[m], ay = sGJ[32 + m], az = sGJ[64 + m];
       gtx -= fma(pp[0], ax, fma(pp[3], ay, pp[5] * az));
       gty -= fma(pp[3], ax, fma(pp[1], ay, pp[4] * az));
@@ -146,7 +163,11 @@ __device__ __forceinline__ void bf_build(const SysParams &P, const double *__res
       sym_mul(Ji, Ji, q);
       Cd = Sym3{q[0] + S2.xx, q[4] + S2.yy, q[8] + S2.zz, q[1] + S2.xy, q[5] + S2.yz, q[2] + S2.zx};
     }
-    if (act) {
+    if constexpr (BG::kTab) {  // the diagonal blocks only (backflow_tables_kernel forms the others where it contracts them)
+      double *sCd = ws + BG::oCd;
+      sCd[lane] = Cd.xx; sCd[32 + lane] = Cd.yy; sCd[64 + lane] = Cd.zz; sCd[96 + lane] = Cd.xy; sCd[128 + lane] = Cd.yz; sCd[160 + lane] = Cd.zx;
+    } else if (act) {
+      double *sCb = ws + BG::oC;
       double *cb = sCb + (i * ne + i) * 9;
       cb[0] = Cd.xx; cb[1] = Cd.xy; cb[2] = Cd.zx; cb[3] = Cd.xy; cb[4] = Cd.yy; cb[5] = Cd.yz; cb[6] = Cd.zx; cb[7] = Cd.yz; cb[8] = Cd.zz;
       for (int i2 = 0; i2 < ne; ++i2) {
@@ -279,7 +300,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
   for (int64_t wk = (int64_t)blockIdx.x * WPB + warp; wk < n_work; wk += (int64_t)gridDim.x * WPB) {
     const int64_t w = io.fb_list ? (int64_t)io.fb_list[wk] : wk;
     double Js, es;
-    bf_build<NS, NMO>(P, sCf, sExp, ws, io, w, lane, Js, es);
+    bf_build<NS, NMO, BG>(P, sCf, sExp, ws, io, w, lane, Js, es);
     // ---- phase 3: every determinant on its own, two at a time (four (determinant, spin) problems of 8 lanes)
     const int c = lane & (kBfLP - 1), slot = lane >> 3, gbase = lane - c;
     const int dsel = slot >> 1, sp = slot & 1;
@@ -450,7 +471,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
     backflow_tables_kernel(const __grid_constant__ SysParams P, const WalkerIO io, const BfDet *__restrict__ dets, int n_dets,
                            double *__restrict__ escratch) {
   extern __shared__ __align__(16) unsigned char smem[];
-  using BG = BfGeo<NS, NMO>;
+  using BG = BfGeoT<NS, NMO>;
   double *sCf = reinterpret_cast<double *>(smem);
   const int nC = P.c_doubles;
   for (int i = threadIdx.x; i < nC; i += blockDim.x) sCf[i] = P.C[i];
@@ -458,8 +479,8 @@ __global__ void __launch_bounds__(WPB * 32, 1)
   for (int i = threadIdx.x; i < kExpTab + kRngTab; i += blockDim.x) sExp[i] = P.exp_tab[i];
   __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  double *ws = reinterpret_cast<double *>(smem + P.smem_const_bytes) + warp * BG::total2;
-  const double *sCb = ws + BG::oC, *sMO = ws + BG::oMO, *sP = ws + BG::oP, *sS = ws + BG::oS;
+  double *ws = reinterpret_cast<double *>(smem + P.smem_const_bytes) + warp * BG::total;
+  const double *sCd = ws + BG::oCd, *sMO = ws + BG::oMO, *sP = ws + BG::oP, *sS = ws + BG::oS;
   double *sTab = ws + BG::oTab, *sSc = ws + BG::oSc;
   const int wpb = (int)(blockDim.x >> 5);  // warps launched per block (<= WPB)
   double *E = escratch + ((int64_t)blockIdx.x * wpb + warp) * BG::eDoubles;
@@ -475,7 +496,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
   auto tabY2 = [&](int sp) { return sTab + sp * BG::tSpin + 4 * NS * 8 + 6 * NS * 8; };
   for (int64_t w = (int64_t)blockIdx.x * wpb + warp; w < io.M; w += (int64_t)gridDim.x * wpb) {
     double Js, es;
-    bf_build<NS, NMO>(P, sCf, sExp, ws, io, w, lane, Js, es);
+    bf_build<NS, NMO, BG>(P, sCf, sExp, ws, io, w, lane, Js, es);
     // ---- reference elimination: [A0 | Av | B0 | Bv | 1], lanes 0-7 spin up, 8-15 spin down (lane c = column c)
     const int c = lane & 7, sp = (lane >> 3) & 1;
     const int ns = sp ? n_dn : n_up, nv = P.nv[sp], e0 = sp ? n_up : 0;
@@ -581,7 +602,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
       if (i == m) {
         xx = 1.0 + sS[i]; yy = 1.0 + sS[32 + i]; zz = 1.0 + sS[64 + i]; xy = sS[96 + i]; yz = sS[128 + i]; zx = sS[160 + i];
       } else {
-        const double *pp = sP + (i * ne + m) * 6;
+        const double *pp = sP + BG::pofs(i, m, ne);
         xx = -pp[0]; yy = -pp[1]; zz = -pp[2]; xy = -pp[3]; yz = -pp[4]; zx = -pp[5];
       }
       j0 = (b == 0) ? xx : ((b == 1) ? xy : zx);
@@ -627,25 +648,72 @@ __global__ void __launch_bounds__(WPB * 32, 1)
         t0l[rd] = t;
       }
     }
-    // ---- R^{a'}[i][i'] = sum_a C_ii'^{aa'} W0^a[i][i'] (lane c = i'), s0, then Y2[q][p] (lane c = q)
-    double *sR = ws + BG::oW;
-    double s0v = 0.0;
-    if (lane < 16) {
-      const double *W0 = tabW0(sp);
-      if (c < ns)
-        for (int i = 0; i < ns; ++i) {
-          const double *cb = sCb + ((e0 + i) * ne + e0 + c) * 9;
-          const double w0 = W0[(0 * NS + i) * 8 + c], w1 = W0[(1 * NS + i) * 8 + c], w2 = W0[(2 * NS + i) * 8 + c];
+    // ---- R^{a'}[i][i'] = sum_a C_ii'^{aa'} W0^a[i][i'] and s0 = sum R^{a'}[i][i'] W0^{a'}[i'][i], same-spin (i, i') only:
+    // one lane per unordered pair forms C_ii' = -J_ii P_ii' - P_ii' J_i'i' + sum_{m != i, i'} P_im P_i'm once and serves
+    // both orders (C_i'i is its transpose); lanes 0-15 the diagonal (C_ii from bf_build).  Then Y2[q][p] (lane c = q).
+    double *sR = ws + BG::oMO;  // the MO planes are dead
+    double s0u = 0.0, s0d = 0.0;
+    {
+      const int npu = n_up * (n_up - 1) / 2, npd = n_dn * (n_dn - 1) / 2;
+      for (int pi = lane; pi < npu + npd; pi += 32) {
+        const int s2 = pi >= npu ? 1 : 0;
+        int rem = pi - (s2 ? npu : 0);
+        const int ns2 = s2 ? n_dn : n_up, f0 = s2 ? n_up : 0;
+        int i = 0;
+        while (rem >= ns2 - 1 - i) { rem -= ns2 - 1 - i; ++i; }
+        const int i2 = i + 1 + rem;  // i < i2 < ns2 (positions within the spin)
+        const int gi = f0 + i, gi2 = f0 + i2;
+        const double *pq = sP + BG::pofs(gi, gi2, ne);
+        const Sym3 Pq{pq[0], pq[1], pq[2], pq[3], pq[4], pq[5]};
+        const Sym3 J1{1.0 + sS[gi], 1.0 + sS[32 + gi], 1.0 + sS[64 + gi], sS[96 + gi], sS[128 + gi], sS[160 + gi]};
+        const Sym3 J2{1.0 + sS[gi2], 1.0 + sS[32 + gi2], 1.0 + sS[64 + gi2], sS[96 + gi2], sS[128 + gi2], sS[160 + gi2]};
+        double cc[9], t[9];
+        sym_mul(J1, Pq, cc);
+        sym_mul(Pq, J2, t);
 #pragma unroll
-          for (int a2 = 0; a2 < 3; ++a2) {
-            const double r = fma(cb[0 + a2], w0, fma(cb[3 + a2], w1, cb[6 + a2] * w2));
-            sR[((sp * 3 + a2) * NS + i) * 8 + c] = r;
-            s0v = fma(r, W0[(a2 * NS + c) * 8 + i], s0v);
-          }
+        for (int k = 0; k < 9; ++k) cc[k] = -cc[k] - t[k];
+        for (int m = 0; m < ne; ++m) {
+          if (m == gi || m == gi2) continue;
+          const double *p1 = sP + BG::pofs(gi, m, ne), *p2 = sP + BG::pofs(gi2, m, ne);
+          sym_mul(Sym3{p1[0], p1[1], p1[2], p1[3], p1[4], p1[5]}, Sym3{p2[0], p2[1], p2[2], p2[3], p2[4], p2[5]}, t);
+#pragma unroll
+          for (int k = 0; k < 9; ++k) cc[k] += t[k];
         }
+        const double *W0 = tabW0(s2);
+        const double a0 = W0[(0 * NS + i) * 8 + i2], a1 = W0[(1 * NS + i) * 8 + i2], a2v = W0[(2 * NS + i) * 8 + i2];  // W0^a[i][i2]
+        const double b0 = W0[(0 * NS + i2) * 8 + i], b1 = W0[(1 * NS + i2) * 8 + i], b2v = W0[(2 * NS + i2) * 8 + i];  // W0^a[i2][i]
+        double acc = 0.0;
+#pragma unroll
+        for (int a2 = 0; a2 < 3; ++a2) {
+          const double r12 = fma(cc[0 + a2], a0, fma(cc[3 + a2], a1, cc[6 + a2] * a2v));            // R^{a2}[i][i2]
+          const double r21 = fma(cc[3 * a2 + 0], b0, fma(cc[3 * a2 + 1], b1, cc[3 * a2 + 2] * b2v));  // R^{a2}[i2][i]
+          sR[((s2 * 3 + a2) * NS + i) * 8 + i2] = r12;
+          sR[((s2 * 3 + a2) * NS + i2) * 8 + i] = r21;
+          const double wb = (a2 == 0) ? b0 : ((a2 == 1) ? b1 : b2v), wa = (a2 == 0) ? a0 : ((a2 == 1) ? a1 : a2v);
+          acc = fma(r12, wb, fma(r21, wa, acc));
+        }
+        if (s2) s0d += acc; else s0u += acc;
+      }
+      if (lane < 16 && c < ns) {
+        const int gi = e0 + c;
+        const double *W0 = tabW0(sp);
+        const double w0 = W0[(0 * NS + c) * 8 + c], w1 = W0[(1 * NS + c) * 8 + c], w2 = W0[(2 * NS + c) * 8 + c];
+        const double cxx = sCd[gi], cyy = sCd[32 + gi], czz = sCd[64 + gi], cxy = sCd[96 + gi], cyz = sCd[128 + gi], czx = sCd[160 + gi];
+        const double r0 = fma(cxx, w0, fma(cxy, w1, czx * w2)), r1 = fma(cxy, w0, fma(cyy, w1, cyz * w2)),
+                     r2 = fma(czx, w0, fma(cyz, w1, czz * w2));
+        sR[((sp * 3 + 0) * NS + c) * 8 + c] = r0;
+        sR[((sp * 3 + 1) * NS + c) * 8 + c] = r1;
+        sR[((sp * 3 + 2) * NS + c) * 8 + c] = r2;
+        const double acc = fma(r0, w0, fma(r1, w1, r2 * w2));
+        if (sp) s0d += acc; else s0u += acc;
+      }
     }
 #pragma unroll
-    for (int mm = 1; mm < 8; mm <<= 1) s0v += shfl_xor_d(s0v, mm);
+    for (int mm = 16; mm > 0; mm >>= 1) {
+      s0u += shfl_xor_d(s0u, mm);
+      s0d += shfl_xor_d(s0d, mm);
+    }
+    const double s0v = sp ? s0d : s0u;
     __syncwarp();
     if (lane < 16 && c < nv) {
       const double *Mq = tabMq(sp), *Rho = tabRho(sp);
@@ -683,15 +751,18 @@ __global__ void __launch_bounds__(WPB * 32, 1)
       double den = 0.0, num1 = 0.0, uni = 0.0, accl = 0.0;
       const int l0 = lane, l1 = lane + 32;
       const bool has1 = l1 < nc, has0 = l0 < nc;
+      const uint2 *raw = reinterpret_cast<const uint2 *>(dets);
+      uint2 nx0 = __ldg(raw), nx1 = __ldg(raw + 1), nx2 = __ldg(raw + 2);
       for (int n = 0; n < n_dets; ++n) {
-        const uint2 *raw = reinterpret_cast<const uint2 *>(dets + n);
-        const uint2 w0 = __ldg(raw), w1 = __ldg(raw + 1);
+        const uint2 w0 = nx0, w1 = nx1, w2 = nx2;
+        if (n + 1 < n_dets) {  // the next record while this one is processed
+          nx0 = __ldg(raw + 3 * (n + 1)); nx1 = __ldg(raw + 3 * (n + 1) + 1); nx2 = __ldg(raw + 3 * (n + 1) + 2);
+        }
         const double d = __hiloint2double((int)w0.y, (int)w0.x);
         const unsigned ku = w1.x & 255u, kd = (w1.x >> 8) & 255u;
         // bytes: k[0] k[1] | p[0][0] p[0][1] p[1][0] p[1][1] q[0][0] q[0][1] | q[1][0] q[1][1] pad...
         const unsigned pu0 = (w1.x >> 16) & 255u, pu1 = w1.x >> 24, pd0 = w1.y & 255u, pd1 = (w1.y >> 8) & 255u;
         const unsigned qu0 = (w1.y >> 16) & 255u, qu1 = w1.y >> 24;
-        const uint2 w2 = __ldg(raw + 2);
         const unsigned qd0 = w2.x & 255u, qd1 = (w2.x >> 8) & 255u;
         double R[2], Rd[2], trY[2], e0v[2], e1v[2], dm0[2], dm1[2];
 #pragma unroll

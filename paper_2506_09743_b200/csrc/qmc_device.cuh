@@ -53,6 +53,7 @@ constexpr int kWarpsEl = QMC_WARPS, kWarpsPsi = QMC_WARPS_PSI, kWarpsOrb = QMC_W
 template <int NS>
 constexpr int kWarpsPsiOf = (NS >= 5) ? QMC_WARPS_PSI : QMC_WARPS_PSI_SMALL;
 constexpr int kWarpsBf = 4;  // warps (= walkers in flight) per block of the backflow E_L kernel
+constexpr int kWarpsBfTab = 8; // backflow_tables_kernel: at most this many (fewer when the per-warp scratch does not fit)
 constexpr int kWarpsMax = kWarpsEl > kWarpsPsi ? kWarpsEl : kWarpsPsi;
 
 // shell record kinds

@@ -1350,6 +1350,36 @@ def test_backflow_odd_systems_500_determinants_and_the_zero_limit(env):
     s0.close(); s1.close()
 
 
+def test_backflow_full_size_table_route_against_the_explicit_route_and_sampled_oracle(env):
+    """32768 CO walkers (the size bench.py times the backflow E_L on): the table route (F.6-F.9, one elimination per
+    spin) against the explicit route of the same library (every determinant eliminated on its own) on every walker, and
+    against the oracle on a sample."""
+    torch, ob, qb = env
+    d, r = wl.co(M=32768)
+    d = _with_bf(d, 0.05)
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    lp, sg, el = (t.cpu().numpy() for t in s.local_energy(rg))
+    lpe, sge, ele = (t.cpu().numpy() for t in s.local_energy_explicit(rg))
+    s.close()
+    keep = (lpe - lpe.max() > math.log(1e-6)) & np.isfinite(ele)
+    assert keep.sum() > 4000                                       # the seeded batch is not equilibrated
+    assert np.array_equal(sg[keep], sge[keep])
+    assert np.max(np.abs(lp - lpe)[keep]) < 1e-10
+    rel = np.abs(el - ele) / np.maximum(1.0, np.abs(ele))
+    # the two routes share phases 1-2 and differ in the determinant algebra: 1e-8 is the contract, the bulk sits far below
+    assert np.max(rel[keep]) < 1e-8, (int(np.argmax(np.where(keep, rel, 0))), float(np.max(rel[keep])))
+    assert np.median(rel[keep]) < 1e-12
+    idx = np.random.default_rng(5).choice(np.flatnonzero(keep), 192, replace=False)
+    rs = np.ascontiguousarray(r[:, :, idx])
+    o, ox = ob.OracleSystem(d), ob.OracleSystem(d, extended=True)
+    lp0, sg0, el0 = ob.local_energy(o, rs, threads=8)
+    lpx, sgx, elx = ob.local_energy(ox, rs, threads=8)
+    assert np.array_equal(sg[idx], sg0)
+    adjudicate(lp[idx], lp0, lpx, 1e-10, what="backflow log|Psi| at full size")
+    adjudicate(el[idx], el0, elx, 1e-8, scale=np.maximum(1.0, np.abs(elx)), what="backflow E_L at full size")
+
+
 def test_backflow_sampler_unsupported_calls_and_output_bounds(env):
     torch, ob, qb = env
     d, r = wl.li2(M=301)
