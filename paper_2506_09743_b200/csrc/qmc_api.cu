@@ -230,6 +230,7 @@ struct qmc_system {
   int blocks_bf = 0, blocks_bf_tab = 0, warps_bf_tab = 0;
   void *d_bfdets = nullptr;  // BfDet records of the table route (null: the expansion has general determinants)
   int n_bfdets = 0;
+  BfClasses bf_cls{};      // class boundaries of the sorted records
   bool frc_ready = false;  // nuclear energy-gradient kernel configured (lazily)
   int frc_warps = 0, blocks_frc = 0;
   bool orb_ready = false;  // orbital-derivative kernel configured (lazily: most users never call it)
@@ -763,6 +764,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   // backflow table route: one compact record per determinant (caller order), when no determinant needs more than two
   // substitutions in a spin
   std::vector<BfDet> bfdets;
+  BfClasses bf_cls{};
   if (P.bf_w != 0.0 && gens.empty()) {
     std::vector<Exc> by_orig(excs);
     std::sort(by_orig.begin(), by_orig.end(), [](const Exc &a, const Exc &b) { return a.orig < b.orig; });
@@ -778,6 +780,14 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
       }
       bfdets.push_back(r);
     }
+    // one loop per class (k_up, k_dn) in the kernel: records sorted by class, caller order within a class
+    std::stable_sort(bfdets.begin(), bfdets.end(), [](const BfDet &a, const BfDet &b) { return 3 * a.k[0] + a.k[1] < 3 * b.k[0] + b.k[1]; });
+    int at = 0;
+    for (int c = 0; c < 9; ++c) {
+      bf_cls.start[c] = at;
+      while (at < (int)bfdets.size() && 3 * bfdets[at].k[0] + bfdets[at].k[1] == c) ++at;
+    }
+    bf_cls.start[9] = at;
   }
   // ---- upload
   cudaError_t e = cudaSetDevice(device);
@@ -813,6 +823,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
       return rc;
     }
     s->n_bfdets = (int)bfdets.size();
+    s->bf_cls = bf_cls;
   }
   P.exp_tab = (const double *)s->d_C + P.c_doubles;
   P.rng_tab = P.exp_tab + kExpTab;
@@ -942,9 +953,8 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
       io.fb_count = li;
       io.fb_list = li + 1;
       const BfDet *dets = static_cast<const BfDet *>(s->d_bfdets);
-      int n_dets = s->n_bfdets;
       double *esc = reinterpret_cast<double *>(base);
-      void *targs[5] = {(void *)&s->P, (void *)&io, (void *)&dets, (void *)&n_dets, (void *)&esc};
+      void *targs[5] = {(void *)&s->P, (void *)&io, (void *)&dets, (void *)&s->bf_cls, (void *)&esc};
       const int smem_t = s->P.smem_const_bytes + wt * s->var.bf_tab_ws_doubles * (int)sizeof(double);
       CK(cudaLaunchKernel(s->var.b_tab, dim3(grid_t), dim3(wt * 32), targs, smem_t, st));
       ++g_launches;

@@ -1,8 +1,8 @@
 // qmc_backflow.cuh -- local energy of a backflow-transformed Slater-Jastrow wavefunction:
 //   rt_i = r_i + sum_{j != i} K_BF(r_ij) (r_i - r_j),  K_BF(r) = w / r
 // orbitals at rt, Jastrow factor at r.  Every row of a Slater matrix now depends on every electron, so the last two
-// terms of F.5 and the cross term of F.4 no longer vanish.  First cut: the explicit route, every
-// determinant eliminated on its own, one walker per warp.
+// terms of F.5 and the cross term of F.4 no longer vanish.  Two kernels, one walker per warp: the
+// explicit route (every determinant eliminated on its own) and, below it, the route on the reference's tables.
 //
 // Formulation (derived here; the oracle evaluates F.3-F.5 coordinate by coordinate instead).  With the 3x3 blocks of
 // the map's Jacobian  J_im = d rt_i / d r_m  (pair matrices P_ij = (w/r_ij)(1 - u u^T), u = (r_i - r_j)/r_ij:
@@ -17,6 +17,8 @@
 //   -1/2 lap Psi / Psi = -1/2 (lap J + |grad J|^2) + sum_n w_n [ Tr(A_n^-1 B_n)^up + Tr(..)^dn - 1/2 E2_n ] / sum_n w_n.
 // Without backflow C is the identity and E2 = 0 (G.5/G.6).
 #pragma once
+#include <type_traits>
+
 #include "qmc_device.cuh"
 
 namespace qmc {
@@ -448,12 +450,51 @@ struct BfDet {
   uint8_t pad[6];
 };
 
+// Class boundaries of the sorted records: class 3 k_up + k_dn occupies [start[c], start[c + 1]).
+struct BfClasses { int start[10]; };
+
+// One spin's share of a determinant in the table route, substitution order K known at compile time: R = det T_PQ,
+// Rd = Tr(adj(T_PQ) M1_PQ), trY = Tr(adj(T_PQ) Y2_PQ), e = Tr(adj(T_PQ) E_PQ,l) and dm = det E_PQ,l for this lane's two
+// coordinates.
+struct BfSpinTerms { double R, Rd, trY, e0, e1, dm0, dm1; };
+template <int K, int NS, int LS>
+__device__ __forceinline__ void bf_spin_terms(const double *__restrict__ T, const double *__restrict__ M1, const double *__restrict__ Y2,
+                                              const double *__restrict__ Es, unsigned p0, unsigned p1, unsigned q0, unsigned q1,
+                                              bool has0, bool has1, int l0, int l1, BfSpinTerms &o) {
+  o.R = 1.0; o.Rd = 0.0; o.trY = 0.0; o.e0 = o.e1 = o.dm0 = o.dm1 = 0.0;
+  if constexpr (K == 1) {
+    o.R = T[p0 * 8 + q0];
+    o.Rd = M1[p0 * 8 + q0];
+    o.trY = Y2[q0 * 8 + p0];
+    const double *e = Es + (q0 * NS + p0) * LS;
+    if (has0) o.e0 = __ldcg(e + l0);
+    if (has1) o.e1 = __ldcg(e + l1);
+  } else if constexpr (K == 2) {
+    const double t11 = T[p0 * 8 + q0], t12 = T[p0 * 8 + q1], t21 = T[p1 * 8 + q0], t22 = T[p1 * 8 + q1];
+    o.R = fma(t11, t22, -t12 * t21);
+    o.Rd = fma(t22, M1[p0 * 8 + q0], fma(t11, M1[p1 * 8 + q1], -fma(t12, M1[p1 * 8 + q0], t21 * M1[p0 * 8 + q1])));
+    o.trY = fma(t22, Y2[q0 * 8 + p0], fma(t11, Y2[q1 * 8 + p1], -fma(t12, Y2[q0 * 8 + p1], t21 * Y2[q1 * 8 + p0])));
+    const double *e11 = Es + (q0 * NS + p0) * LS, *e12 = Es + (q1 * NS + p0) * LS, *e21 = Es + (q0 * NS + p1) * LS,
+                 *e22 = Es + (q1 * NS + p1) * LS;
+    if (has0) {
+      const double a = __ldcg(e11 + l0), b2 = __ldcg(e12 + l0), c2 = __ldcg(e21 + l0), dd = __ldcg(e22 + l0);
+      o.e0 = fma(t22, a, fma(t11, dd, -fma(t12, c2, t21 * b2)));
+      o.dm0 = fma(a, dd, -b2 * c2);
+    }
+    if (has1) {
+      const double a = __ldcg(e11 + l1), b2 = __ldcg(e12 + l1), c2 = __ldcg(e21 + l1), dd = __ldcg(e22 + l1);
+      o.e1 = fma(t22, a, fma(t11, dd, -fma(t12, c2, t21 * b2)));
+      o.dm1 = fma(a, dd, -b2 * c2);
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------
 // The accelerated route (F.6-F.9): only the reference determinant of each spin is eliminated; every
 // other determinant comes from tables.  With B_l = d_l A (dense: every row depends on every coordinate l through the
 // Jacobian J of the backflow map) the paper's tables are, per spin,
 //   T = A0^-1 Av,   M_l = A0^-1 B_l,v - A0^-1 B_l,0 T  (F.7),   Y_l = A0^-1 B_l,0 M_l  (F.9),
-// and here (derivation pinned by tests/test_oracle_pins.py::test_P14b...):
+// and here (derivation pinned on random matrices by the P14b test of the CPU suite):
 //   rho = A0^-1,  W0^a = V0^a rho,  m^a = Vv^a - V0^a T   (V^a = d_a phi rows),
 //   E[q][p][l] = M_l[p][q] = sum_i rho[p][i] sum_a J_il^a m^a[i][q]     (42-vectors, kept in a per-warp global scratch)
 //   Y2[q][p]   = sum_l Y_l[p][q] = sum_i rho[p][i] sum_{i',a'} (sum_a C_ii'^{aa'} W0^a[i][i']) m^{a'}[i'][q]
@@ -468,8 +509,8 @@ struct BfDet {
 // ---------------------------------------------------------------------------------
 template <int NS, int NMO, int WPB>
 __global__ void __launch_bounds__(WPB * 32, 1)
-    backflow_tables_kernel(const __grid_constant__ SysParams P, const WalkerIO io, const BfDet *__restrict__ dets, int n_dets,
-                           double *__restrict__ escratch) {
+    backflow_tables_kernel(const __grid_constant__ SysParams P, const WalkerIO io, const BfDet *__restrict__ dets,
+                           const BfClasses cls, double *__restrict__ escratch) {
   extern __shared__ __align__(16) unsigned char smem[];
   using BG = BfGeoT<NS, NMO>;
   double *sCf = reinterpret_cast<double *>(smem);
@@ -745,65 +786,49 @@ __global__ void __launch_bounds__(WPB * 32, 1)
       sSc[sp * 4 + 3] = kap;
     }
     __syncwarp();
-    // ---- CI sum over the determinants: uniform scalars in every lane, the l-dependent part per lane
+    // ---- CI sum over the determinants: uniform scalars in every lane, the l-dependent part per lane.  The records are
+    // sorted by class (k_up, k_dn) at setup: one loop per class, the substitution orders known at compile time.
     {
       const double *Tu = tabT(0), *Td = tabT(1), *M1u = tabM1(0), *M1d = tabM1(1), *Y2u = tabY2(0), *Y2d = tabY2(1);
       double den = 0.0, num1 = 0.0, uni = 0.0, accl = 0.0;
       const int l0 = lane, l1 = lane + 32;
       const bool has1 = l1 < nc, has0 = l0 < nc;
       const uint2 *raw = reinterpret_cast<const uint2 *>(dets);
-      uint2 nx0 = __ldg(raw), nx1 = __ldg(raw + 1), nx2 = __ldg(raw + 2);
-      for (int n = 0; n < n_dets; ++n) {
-        const uint2 w0 = nx0, w1 = nx1, w2 = nx2;
-        if (n + 1 < n_dets) {  // the next record while this one is processed
-          nx0 = __ldg(raw + 3 * (n + 1)); nx1 = __ldg(raw + 3 * (n + 1) + 1); nx2 = __ldg(raw + 3 * (n + 1) + 2);
-        }
-        const double d = __hiloint2double((int)w0.y, (int)w0.x);
-        const unsigned ku = w1.x & 255u, kd = (w1.x >> 8) & 255u;
-        // bytes: k[0] k[1] | p[0][0] p[0][1] p[1][0] p[1][1] q[0][0] q[0][1] | q[1][0] q[1][1] pad...
-        const unsigned pu0 = (w1.x >> 16) & 255u, pu1 = w1.x >> 24, pd0 = w1.y & 255u, pd1 = (w1.y >> 8) & 255u;
-        const unsigned qu0 = (w1.y >> 16) & 255u, qu1 = w1.y >> 24;
-        const unsigned qd0 = w2.x & 255u, qd1 = (w2.x >> 8) & 255u;
-        double R[2], Rd[2], trY[2], e0v[2], e1v[2], dm0[2], dm1[2];
-#pragma unroll
-        for (int s2 = 0; s2 < 2; ++s2) {
-          const unsigned k = s2 ? kd : ku, p0 = s2 ? pd0 : pu0, p1 = s2 ? pd1 : pu1, q0 = s2 ? qd0 : qu0, q1 = s2 ? qd1 : qu1;
-          const double *T = s2 ? Td : Tu, *M1 = s2 ? M1d : M1u, *Y2 = s2 ? Y2d : Y2u;
-          const double *Es = E + (int64_t)s2 * kMaxVirt * NS * LS;
-          R[s2] = 1.0; Rd[s2] = 0.0; trY[s2] = 0.0; e0v[s2] = e1v[s2] = dm0[s2] = dm1[s2] = 0.0;
-          if (k == 1) {
-            R[s2] = T[p0 * 8 + q0];
-            Rd[s2] = M1[p0 * 8 + q0];
-            trY[s2] = Y2[q0 * 8 + p0];
-            const double *e = Es + (q0 * NS + p0) * LS;
-            if (has0) e0v[s2] = __ldcg(e + l0);
-            if (has1) e1v[s2] = __ldcg(e + l1);
-          } else if (k == 2) {
-            const double t11 = T[p0 * 8 + q0], t12 = T[p0 * 8 + q1], t21 = T[p1 * 8 + q0], t22 = T[p1 * 8 + q1];
-            R[s2] = fma(t11, t22, -t12 * t21);
-            Rd[s2] = fma(t22, M1[p0 * 8 + q0], fma(t11, M1[p1 * 8 + q1], -fma(t12, M1[p1 * 8 + q0], t21 * M1[p0 * 8 + q1])));
-            trY[s2] = fma(t22, Y2[q0 * 8 + p0], fma(t11, Y2[q1 * 8 + p1], -fma(t12, Y2[q0 * 8 + p1], t21 * Y2[q1 * 8 + p0])));
-            const double *e11 = Es + (q0 * NS + p0) * LS, *e12 = Es + (q1 * NS + p0) * LS, *e21 = Es + (q0 * NS + p1) * LS,
-                         *e22 = Es + (q1 * NS + p1) * LS;
-            if (has0) {
-              const double a = __ldcg(e11 + l0), b2 = __ldcg(e12 + l0), c2 = __ldcg(e21 + l0), dd = __ldcg(e22 + l0);
-              e0v[s2] = fma(t22, a, fma(t11, dd, -fma(t12, c2, t21 * b2)));
-              dm0[s2] = fma(a, dd, -b2 * c2);
-            }
-            if (has1) {
-              const double a = __ldcg(e11 + l1), b2 = __ldcg(e12 + l1), c2 = __ldcg(e21 + l1), dd = __ldcg(e22 + l1);
-              e1v[s2] = fma(t22, a, fma(t11, dd, -fma(t12, c2, t21 * b2)));
-              dm1[s2] = fma(a, dd, -b2 * c2);
-            }
+      const double *Eu = E, *Ed = E + (int64_t)kMaxVirt * NS * LS;
+      auto run_class = [&](auto KU, auto KD, int n_begin, int n_end) {
+        constexpr int ku = decltype(KU)::value, kd = decltype(KD)::value;
+        if (n_begin >= n_end) return;
+        uint2 nx0 = __ldg(raw + 3 * n_begin), nx1 = __ldg(raw + 3 * n_begin + 1), nx2 = __ldg(raw + 3 * n_begin + 2);
+        for (int n = n_begin; n < n_end; ++n) {
+          const uint2 w0 = nx0, w1 = nx1, w2 = nx2;
+          if (n + 1 < n_end) {  // the next record while this one is processed
+            nx0 = __ldg(raw + 3 * (n + 1)); nx1 = __ldg(raw + 3 * (n + 1) + 1); nx2 = __ldg(raw + 3 * (n + 1) + 2);
           }
+          const double d = __hiloint2double((int)w0.y, (int)w0.x);
+          // bytes: k[0] k[1] | p[0][0] p[0][1] p[1][0] p[1][1] q[0][0] q[0][1] | q[1][0] q[1][1] pad...
+          BfSpinTerms up, dn;
+          bf_spin_terms<ku, NS, LS>(Tu, M1u, Y2u, Eu, (w1.x >> 16) & 255u, w1.x >> 24, (w1.y >> 16) & 255u, w1.y >> 24, has0, has1, l0, l1, up);
+          bf_spin_terms<kd, NS, LS>(Td, M1d, Y2d, Ed, w1.y & 255u, (w1.y >> 8) & 255u, w2.x & 255u, (w2.x >> 8) & 255u, has0, has1, l0, l1, dn);
+          den = fma(d * up.R, dn.R, den);                                      // eq. 4
+          num1 = fma(d, fma(up.Rd, dn.R, up.R * dn.Rd), num1);                 // F.6 (first order)
+          uni = fma(-2.0 * d, fma(dn.R, up.trY, up.R * dn.trY), uni);          // F.9 (summed over l)
+          const double x0 = fma(t0l[0], fma(dn.R, up.e0, up.R * dn.e0), fma(up.e0, dn.e0, fma(dn.R, up.dm0, up.R * dn.dm0)));
+          const double x1 = fma(t0l[1], fma(dn.R, up.e1, up.R * dn.e1), fma(up.e1, dn.e1, fma(dn.R, up.dm1, up.R * dn.dm1)));
+          accl = fma(2.0 * d, x0 + x1, accl);
         }
-        den = fma(d * R[0], R[1], den);                                        // eq. 4
-        num1 = fma(d, fma(Rd[0], R[1], R[0] * Rd[1]), num1);                   // F.6 (first order)
-        uni = fma(-2.0 * d, fma(R[1], trY[0], R[0] * trY[1]), uni);            // F.9 (summed over l)
-        const double x0 = fma(t0l[0], fma(R[1], e0v[0], R[0] * e0v[1]), fma(e0v[0], e0v[1], fma(R[1], dm0[0], R[0] * dm0[1])));
-        const double x1 = fma(t0l[1], fma(R[1], e1v[0], R[0] * e1v[1]), fma(e1v[0], e1v[1], fma(R[1], dm1[0], R[0] * dm1[1])));
-        accl = fma(2.0 * d, x0 + x1, accl);
-      }
+      };
+      using I0 = std::integral_constant<int, 0>;
+      using I1 = std::integral_constant<int, 1>;
+      using I2 = std::integral_constant<int, 2>;
+      run_class(I0{}, I0{}, cls.start[0], cls.start[1]);
+      run_class(I0{}, I1{}, cls.start[1], cls.start[2]);
+      run_class(I0{}, I2{}, cls.start[2], cls.start[3]);
+      run_class(I1{}, I0{}, cls.start[3], cls.start[4]);
+      run_class(I1{}, I1{}, cls.start[4], cls.start[5]);
+      run_class(I1{}, I2{}, cls.start[5], cls.start[6]);
+      run_class(I2{}, I0{}, cls.start[6], cls.start[7]);
+      run_class(I2{}, I1{}, cls.start[7], cls.start[8]);
+      run_class(I2{}, I2{}, cls.start[8], cls.start[9]);
       double tt = fma(t0l[0], t0l[0], t0l[1] * t0l[1]);
 #pragma unroll
       for (int mm = 16; mm > 0; mm >>= 1) {
