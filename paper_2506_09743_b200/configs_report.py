@@ -15,6 +15,7 @@ best of 3 batches.  There is no CPU fallback: without a GPU this raises.
 from __future__ import annotations
 
 import argparse
+import copy
 
 import torch
 
@@ -112,8 +113,38 @@ def fig11(walkers=32768, n_dets=(1, 4, 20, 100, 500)):
         sg, el = torch.empty_like(lp), torch.empty_like(lp)
         t_tab = _time(lambda: s.local_energy(r, lp, sg, el))
         t_exp = _time(lambda: s.local_energy_explicit(r, lp, sg, el), reps=3, warm=1)
-        out.append(dict(n_det=nd, walkers=walkers, tab_ms=1e3 * t_tab, exp_ms=1e3 * t_exp))
         s.close()
+        # the same with the inverse backflow transformation (F.8/F.9 tables against every determinant explicit)
+        d_bf = copy.copy(d)
+        d_bf.backflow_w = 0.05
+        s = qb.QmcSystem(d_bf, 0)
+        t_btab = _time(lambda: s.local_energy(r, lp, sg, el), reps=5)
+        t_bexp = _time(lambda: s.local_energy_explicit(r, lp, sg, el), reps=2, warm=1)
+        s.close()
+        out.append(dict(n_det=nd, walkers=walkers, tab_ms=1e3 * t_tab, exp_ms=1e3 * t_exp, btab_ms=1e3 * t_btab,
+                        bexp_ms=1e3 * t_bexp))
+    return out
+
+
+def fig10(points=(1000, 32768)):
+    """The workload of PAPER.md:313-321 (Fig. 10): the kinetic energy by the trace formulas on the four molecules,
+    ground-state determinant only, with and without backflow.  Here: the whole E_L call (kinetic + potential)."""
+    out = []
+    for name in ("H2", "LiH", "Li2", "CO"):
+        for M in points:
+            d, r_host = wl.CONFIGS[name](M=M)
+            d = copy.copy(d)
+            d.det_up, d.det_dn, d.ci_coeff = d.det_up[:1], d.det_dn[:1], d.ci_coeff[:1]
+            r = torch.from_numpy(r_host).cuda()
+            lp = torch.empty(M, dtype=torch.float64, device="cuda")
+            sg, el = torch.empty_like(lp), torch.empty_like(lp)
+            row = dict(config=name, points=M)
+            for key, w in (("plain_ms", 0.0), ("bf_ms", 0.05)):
+                d.backflow_w = w
+                s = qb.QmcSystem(d, 0)
+                row[key] = 1e3 * _time(lambda: s.local_energy(r, lp, sg, el))
+                s.close()
+            out.append(row)
     return out
 
 
@@ -167,10 +198,17 @@ def main():
         print(f"| {x['config']} | {x['deriv_walkers']} | {x['el_d_ms']:.3f} | {x['n_param']} | {x['O_ms']:.3f} | {x['fuse_ms']:.3f} | "
               f"{x['n_ao']} x {x['n_mo']} + {x['n_ao']} | {x['orb_ms']:.3f} | {x['nuc_ms']:.3f} | {x['frc_ms']:.3f} |")
     print("\nAccelerated (excitation tables, F.6/F.7) vs explicit per-determinant E_L (PAPER.md:345-349, Fig. 11), CO shape:")
-    print("| N_det | walkers | tables ms | explicit ms | explicit / tables |")
-    print("|---|---|---|---|---|")
+    print("| N_det | walkers | tables ms | explicit ms | explicit / tables | backflow: tables (F.8/F.9) ms | backflow: explicit ms | explicit / tables |")
+    print("|---|---|---|---|---|---|---|---|")
     for x in fig11():
-        print(f"| {x['n_det']} | {x['walkers']} | {x['tab_ms']:.3f} | {x['exp_ms']:.3f} | {x['exp_ms'] / x['tab_ms']:.1f} |")
+        print(f"| {x['n_det']} | {x['walkers']} | {x['tab_ms']:.3f} | {x['exp_ms']:.3f} | {x['exp_ms'] / x['tab_ms']:.1f} | "
+              f"{x['btab_ms']:.3f} | {x['bexp_ms']:.3f} | {x['bexp_ms'] / x['btab_ms']:.1f} |")
+    print("\nGround-state determinant only, with and without the inverse backflow (workload of PAPER.md:313-321, Fig. 10), "
+          "E_L call, device time:")
+    print("| config | points | E_L ms | E_L with backflow ms |")
+    print("|---|---|---|---|")
+    for x in fig10():
+        print(f"| {x['config']} | {x['points']} | {x['plain_ms']:.4f} | {x['bf_ms']:.4f} |")
     if args.scan_geometries > 0:
         geo, t_total = scan(args.scan_geometries, peak)
         print(f"\nCO scan (500 determinants, {geo[0]['walkers']} walkers per geometry, {geo[0]['sweeps']} sweeps + E_L on every "

@@ -39,7 +39,7 @@ constexpr int kMaxEen = 6;    // terms of the electron-electron-nucleus Jastrow 
                              // 5.52 after the record-stream change, 14: 5.39, 16 (one block per SM): 6.46
 #endif
 #ifndef QMC_WARPS_ORB
-#define QMC_WARPS_ORB 10     // warps per block of the orbital-derivative kernel (one block per SM; 8 when shared memory is short).
+#define QMC_WARPS_ORB 10     // warps per block of the orbital-derivative kernel (one block per SM; 8 when shared memory is short; 12 fits but is 40 % slower on bench.py's walkers).
                              // Measured on CO, 32768 walkers, early / equilibrated: 8 warps 0.82 / 0.63 ms, 10: 0.80 / 0.60, 12: 0.78 / 0.80
                              // (12 x 16.3 KB of scratch leave ~30 KB of L1 for the term lists and the constant tables)
 #endif
