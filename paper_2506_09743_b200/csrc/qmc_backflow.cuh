@@ -36,8 +36,19 @@ __device__ __forceinline__ void sym_mul(const Sym3 &a, const Sym3 &b, double o[9
 
 constexpr int kBfLP = 8;  // lanes per (determinant, spin) problem: n_up, n_dn <= 8
 // fallback thresholds of the table route (as kFallbackK / kFallbackKappa of the plain path, tighter: the second-order
-// tables carry one more factor A0^-1)
-constexpr double kBfFallbackK = 1.0e4, kBfFallbackKappa = 1.0e4;
+// tables carry one more factor A0^-1), not scaled with |E_L|.  Measured (table route against the explicit route, 32768
+// equilibrated CO walkers / worst of 100 random systems against the long-double CPU reference): 1e4 scaled with
+// max(1, |E_L|): 2.3e-8 / 1.8e-8, 2.8 ms; 1e4: 1.4e-9 / 6.4e-10, 3.4 ms; 1e3: 6e-11 / 2e-10, 4.9 ms.
+#ifndef QMC_BF_FALLBACK_K
+#define QMC_BF_FALLBACK_K 1.0e4
+#endif
+#ifndef QMC_BF_FALLBACK_KAPPA
+#define QMC_BF_FALLBACK_KAPPA 1.0e4
+#endif
+#ifndef QMC_BF_FALLBACK_ESCALE
+#define QMC_BF_FALLBACK_ESCALE 0  // 1: thresholds times max(1, |E_L|) as in the plain path -- measured too lenient here
+#endif
+constexpr double kBfFallbackK = QMC_BF_FALLBACK_K, kBfFallbackKappa = QMC_BF_FALLBACK_KAPPA;
 
 template <int NS, int NMO>
 struct BfGeo {
@@ -847,8 +858,8 @@ __global__ void __launch_bounds__(WPB * 32, 1)
         if (io.sign) io.sign[w] = (sig > 0.0) ? 1.0 : ((sig < 0.0) ? -1.0 : 0.0);
         if (io.eloc) io.eloc[w] = eloc;
         // nearly singular reference: the explicit kernel re-evaluates the walker (criteria of DESIGN.md section 5.6; the
-        // second-order tables amplify by one more power of kappa, hence the lower thresholds)
-        const double ku2 = sSc[3], kd2 = sSc[7], scale = fmax(1.0, fabs(eloc));
+        // second-order tables amplify by one more power of kappa, hence the lower, unscaled thresholds)
+        const double ku2 = sSc[3], kd2 = sSc[7], scale = QMC_BF_FALLBACK_ESCALE ? fmax(1.0, fabs(eloc)) : 1.0;
         const bool ok = (den * den <= fmin(kBfFallbackK * scale, kFallbackCap)) && (ku2 * ku2 <= kBfFallbackKappa * scale) &&
                         (kd2 * kd2 <= kBfFallbackKappa * scale);
         if (!ok && io.fb_list) io.fb_list[atomicAdd(io.fb_count, 1)] = (int)w;

@@ -12,7 +12,7 @@ from paper_2506_09743_b200.workloads import SystemDesc
 pytestmark = pytest.mark.gpu
 
 
-def random_system(seed, case):
+def random_system(seed, case, kmax=4):
     """(SystemDesc, walkers) or None when the draw falls outside the library's limits"""
     rng = np.random.default_rng([seed, case])
     n_at = int(rng.integers(1, 5))
@@ -43,7 +43,7 @@ def random_system(seed, case):
 
     def rand_list(ns, ref):
         lst = ref.copy()
-        k = int(rng.integers(0, min(ns, n_mo - ns, 4) + 1)) if ns else 0
+        k = int(rng.integers(0, min(ns, n_mo - ns, kmax) + 1)) if ns else 0
         if k:
             pos = rng.choice(ns, k, replace=False)
             lst[pos] = rng.choice(np.setdiff1d(np.arange(n_mo), ref), k, replace=False)
@@ -132,4 +132,51 @@ def test_random_systems_against_the_oracle(seed):
     assert evaluated >= 30
     # exceptions stay a small minority of the walkers compared (reported by -rA / on failure)
     print(f"fuzz seed {seed}: {evaluated} systems, {walkers} walkers, adjudicated exceptions {exc}")
+    assert max(exc.values()) <= 0.1 * walkers, (exc, walkers)
+
+
+@pytest.mark.parametrize("seed,kmax", [(21, 2), (22, 4)])
+def test_random_backflow_systems_against_the_oracle(seed, kmax):
+    """Inverse backflow on random systems (D.1 Jastrow; substitution orders <= 2: the table route of F.6-F.9 with its
+    list of nearly singular walkers; orders up to 4: every determinant explicit): log|Psi| from the E_L kernel and from the
+    values-only kernel, sign, E_L, and the explicit route on the same walkers, contract tolerances with adjudication."""
+    import torch
+    from oracle import binding as ob
+    from paper_2506_09743_b200 import binding as qb
+    from tests.helpers import adjudicate
+    evaluated = walkers = 0
+    exc = dict(lp=0, lpv=0, el=0, elx=0)
+    for case in range(40):
+        drawn = random_system(seed, case, kmax)
+        if drawn is None:
+            continue
+        d, r = drawn
+        rng = np.random.default_rng([seed, case, 7])
+        d.jastrow_en_w0 = d.jastrow_en_w1 = d.jastrow_en_w2 = 0.0   # backflow is built for the D.1 Jastrow
+        d.jastrow_een = None
+        d.backflow_w = float(rng.uniform(-0.2, 0.2))
+        try:
+            s = qb.QmcSystem(d, 0)
+        except qb.QmcError as e:
+            assert e.status == qb.QMC_EUNSUPPORTED, (case, e)
+            continue
+        evaluated += 1
+        o, ox = ob.OracleSystem(d), ob.OracleSystem(d, extended=True)
+        lp0, sg0, el0 = ob.local_energy(o, r, threads=4)
+        lpX, sgX, elX = ob.local_energy(ox, r, threads=4)
+        rg = torch.from_numpy(r).cuda()
+        lp, sg, el = (t.cpu().numpy() for t in s.local_energy(rg))
+        lpv, sgv = (t.cpu().numpy() for t in s.log_psi(rg))
+        lpe, sge, ele = (t.cpu().numpy() for t in s.local_energy_explicit(rg))
+        s.close()
+        keep = (lpX - lpX.max() > math.log(1e-6)) & np.isfinite(elX)
+        walkers += int(keep.sum())
+        assert np.array_equal(sg[keep], sg0[keep]) and np.array_equal(sgv[keep], sg0[keep]) and np.array_equal(sge[keep], sg0[keep]), case
+        esc = np.maximum(1, np.abs(elX))
+        exc["lp"] += adjudicate(lp, lp0, lpX, 1e-10, mask=keep, what=(case, "backflow log|Psi|"))
+        exc["lpv"] += adjudicate(lpv, lp0, lpX, 1e-10, mask=keep, what=(case, "backflow log|Psi| (values only)"))
+        exc["el"] += adjudicate(el, el0, elX, 1e-8, scale=esc, mask=keep, what=(case, "backflow E_L"))
+        exc["elx"] += adjudicate(ele, el0, elX, 1e-8, scale=esc, mask=keep, what=(case, "backflow E_L explicit"))
+    assert evaluated >= 20
+    print(f"backflow fuzz seed {seed}: {evaluated} systems, {walkers} walkers, adjudicated exceptions {exc}")
     assert max(exc.values()) <= 0.1 * walkers, (exc, walkers)

@@ -1378,6 +1378,22 @@ def test_backflow_full_size_table_route_against_the_explicit_route_and_sampled_o
     assert np.array_equal(sg[idx], sg0)
     adjudicate(lp[idx], lp0, lpx, 1e-10, what="backflow log|Psi| at full size")
     adjudicate(el[idx], el0, elx, 1e-8, scale=np.maximum(1.0, np.abs(elx)), what="backflow E_L at full size")
+    # the same property on equilibrated walkers (the bench's: 260 sweeps of the plain sampler of this library first), where
+    # nearly all walkers sit in the criterion set and nearly singular references are typical rather than rare
+    d0, r0 = wl.co(M=32768)
+    s0 = qb.QmcSystem(d0)
+    rg = _to_gpu(torch, r0)
+    s0.metropolis(rg, 0.2, 260, seed=1234)
+    s0.close()
+    s = qb.QmcSystem(d)
+    lp, sg, el = s.local_energy(rg)
+    lpe, sge, ele = s.local_energy_explicit(rg)
+    s.close()
+    keep = (lpe - lpe.max() > math.log(1e-6)) & torch.isfinite(ele)
+    assert int(keep.sum()) > 16000
+    assert bool((sg == sge)[keep].all()) and float((lp - lpe).abs()[keep].max()) < 1e-10
+    rel = ((el - ele).abs() / ele.abs().clamp(min=1.0))[keep]
+    assert float(rel.max()) < 5e-9, float(rel.max())               # half the contract's bound between the two routes
 
 
 def test_backflow_sampler_unsupported_calls_and_output_bounds(env):
