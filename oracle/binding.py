@@ -232,11 +232,12 @@ def batch_stats(x):
 
 
 def log_derivatives(sysd: OracleSystem, r_soa, threads: int = 1):
-    """O[M, 6 + 7 n_een + n_det] = (dPsi/dtheta)/Psi for theta = (a_par, a_anti, b, en_w0, en_w1, en_w2,
-    the seven parameters of every e-e-n term in een_params order, d_0 .. d_{n_det-1})  (eq. 6)."""
+    """O[M, 6 + 7 n_een + n_det (+ 1)] = (dPsi/dtheta)/Psi for theta = (a_par, a_anti, b, en_w0, en_w1, en_w2,
+    the seven parameters of every e-e-n term in een_params order, d_0 .. d_{n_det-1}, and -- with backflow on -- the
+    backflow weight w)  (eq. 6)."""
     r = np.ascontiguousarray(r_soa, np.float64)
     M = r.shape[2]
-    O = np.empty((M, 6 + 7 * int(sysd.c.n_een) + int(sysd.c.n_det)))
+    O = np.empty((M, 6 + 7 * int(sysd.c.n_een) + int(sysd.c.n_det) + (1 if float(sysd.c.backflow_w) != 0.0 else 0)))
     L = sysd.L
 
     def run(rng):

@@ -731,13 +731,21 @@ void oracle_batch_stats(const double *x, int64_t M, double *mean, double *stderr
 
 int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                            int64_t w1, double *O) {
-  if (s->backflow_w != 0.0) return -2; /* parameter / nuclear derivatives are not derived for backflow wavefunctions */
-  int ne = s->n_up + s->n_dn, nmo = s->n_mo, nj = 6 + 7 * s->n_een, np = nj + s->n_det;
+  /* With the backflow transformation the Jastrow entries are unchanged (the Jastrow factor sits at r),
+   * the orbitals of the CI entries sit at the backflow coordinates, and one more entry follows them: the backflow
+   * weight w of K_BF(r) = w / r,
+   *   d ln Psi / d w = sum_n d_n D_n^up D_n^dn [Tr(A_n^-1 d_w A_n)^up + (..)^dn] / Sigma,
+   *   d_w A[i][j] = grad phi_j(rt_i) . d rt_i / d w,   d rt_i / d w = sum_{j != i} (r_i - r_j) / r_ij. */
+  const int bf = s->backflow_w != 0.0;
+  int ne = s->n_up + s->n_dn, nmo = s->n_mo, nj = 6 + 7 * s->n_een, np = nj + s->n_det + (bf ? 1 : 0);
   real *mo = (real *)malloc(sizeof(real) * (size_t)(ne * nmo + 1));
+  real *dmo = (real *)malloc(sizeof(real) * (size_t)(ne * nmo + 1));
   real *A = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
+  real *Ai = (real *)malloc(sizeof(real) * (size_t)(ne * ne + 1));
   real *pos = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
+  real *post = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
   real *prod = (real *)malloc(sizeof(real) * (size_t)(s->n_det + 1));
-  if (!mo || !A || !pos || !prod) return -1;
+  if (!mo || !dmo || !A || !Ai || !pos || !post || !prod) return -1;
   real ao[5];
   for (int64_t w = w0; w < w1; ++w) {
     gather_walker(r, M, w, ne, pos);
@@ -805,28 +813,46 @@ int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64
       for (int k = 0; k < 7; ++k) out[6 + 7 * mu + k] = dq[k];
     }
     /* CI: Sigma = sum_n d_n D_n^up D_n^dn  (eq. 4):  d ln Sigma / d d_n = D_n^up D_n^dn / Sigma */
-    for (int i = 0; i < ne * nmo; ++i) mo[i] = 0.0;
-    for (int i = 0; i < ne; ++i)
-      for (int beta = 0; beta < s->n_ao; ++beta) {
-        ao_eval_r(s, beta, pos + 3 * i, ao);
-        for (int alpha = 0; alpha < nmo; ++alpha) mo[i * nmo + alpha] += s->mo_coeff[beta * nmo + alpha] * ao[0];
+    for (int q = 0; q < 3 * ne; ++q) post[q] = pos[q];
+    if (bf) backflow_map(s, pos, post, NULL, NULL);
+    for (int i = 0; i < ne * nmo; ++i) mo[i] = dmo[i] = 0.0;
+    for (int i = 0; i < ne; ++i) {
+      real dw[3] = {0.0, 0.0, 0.0};  /* d rt_i / d w */
+      for (int j = 0; j < ne; ++j) {
+        if (j == i) continue;
+        real dx = pos[3 * i] - pos[3 * j], dy = pos[3 * i + 1] - pos[3 * j + 1], dz = pos[3 * i + 2] - pos[3 * j + 2];
+        real rij = sqrt(dx * dx + dy * dy + dz * dz);
+        dw[0] += dx / rij; dw[1] += dy / rij; dw[2] += dz / rij;
       }
-    real sigma = 0.0;
+      for (int beta = 0; beta < s->n_ao; ++beta) {
+        ao_eval_r(s, beta, post + 3 * i, ao);
+        for (int alpha = 0; alpha < nmo; ++alpha) {
+          mo[i * nmo + alpha] += s->mo_coeff[beta * nmo + alpha] * ao[0];
+          dmo[i * nmo + alpha] += s->mo_coeff[beta * nmo + alpha] * (ao[1] * dw[0] + ao[2] * dw[1] + ao[3] * dw[2]);
+        }
+      }
+    }
+    real sigma = 0.0, dsigma = 0.0;
     for (int n = 0; n < s->n_det; ++n) {
-      real D[2];
+      real D[2], tr[2] = {0.0, 0.0};
       for (int sp = 0; sp < 2; ++sp) {
         int ns = sp ? s->n_dn : s->n_up, e0 = sp ? s->n_up : 0;
         const int32_t *lst = sp ? s->det_dn + (size_t)n * s->n_dn : s->det_up + (size_t)n * s->n_up;
         for (int i = 0; i < ns; ++i)
           for (int j = 0; j < ns; ++j) A[i * ns + j] = mo[(e0 + i) * nmo + lst[j]];
-        D[sp] = det_inv_r(ns, A, NULL);
+        D[sp] = det_inv_r(ns, A, bf ? Ai : NULL);
+        if (bf)  /* Tr(A^-1 d_w A) = sum_ij Ai[j][i] d_w A[i][j] */
+          for (int i = 0; i < ns; ++i)
+            for (int j = 0; j < ns; ++j) tr[sp] += Ai[j * ns + i] * dmo[(e0 + i) * nmo + lst[j]];
       }
       prod[n] = D[0] * D[1];
       sigma += s->ci_coeff[n] * prod[n];
+      dsigma += s->ci_coeff[n] * prod[n] * (tr[0] + tr[1]);
     }
     for (int n = 0; n < s->n_det; ++n) out[nj + n] = prod[n] / sigma;
+    if (bf) out[nj + s->n_det] = dsigma / sigma;
   }
-  free(mo); free(A); free(pos); free(prod);
+  free(mo); free(dmo); free(A); free(Ai); free(pos); free(post); free(prod);
   return 0;
 }
 

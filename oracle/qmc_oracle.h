@@ -109,7 +109,10 @@ void oracle_batch_stats(const double *x, int64_t M, double *mean, double *stderr
  * rows w0 <= w < w1 are written.
  * Psi = e^J Sigma (eq. 4), so d ln Psi / d(Jastrow parameter) is the
  * parameter derivative of D.1 summed over pairs, and
- * d ln Psi / d d_n = D_n^up D_n^dn / Sigma, every determinant factored explicitly. */
+ * d ln Psi / d d_n = D_n^up D_n^dn / Sigma, every determinant factored explicitly.
+ * With backflow_w != 0 the determinants sit at the backflow coordinates and ONE MORE entry
+ * follows the CI entries, the backflow weight: d ln Psi / d w = sum_n d_n D_n [Tr(A_n^-1 d_w A_n)^up + (..)^dn] / Sigma
+ * with d_w A[i][j] = grad phi_j(rt_i) . sum_{j' != i} (r_i - r_j') / r_ij'; O is then [M][6 + 7 n_een + n_det + 1]. */
 int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                            int64_t w1, double *O);
 

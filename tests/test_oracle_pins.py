@@ -1218,11 +1218,55 @@ def test_backflow_limit_antisymmetry_and_sampler_value():
     assert np.max((np.abs(elx - el) / np.maximum(1, np.abs(el)))[keep]) < 1e-9
     out = ob.metropolis(ob_, r, 0.2, 0, seed=1)
     assert np.max(np.abs(out["logpsi"] - lp)) < 1e-12
-    # parameter and nuclear derivatives are not derived for backflow wavefunctions: the calls say so
+    # nuclear derivatives are not derived for backflow wavefunctions: the call says so
     L = ob.lib()
     buf = np.zeros((24, 64))
-    assert L.oracle_log_derivatives(ob_.ref, r.ctypes.data, 24, 0, 24, buf.ctypes.data) == -2
     assert L.oracle_nuclear_energy_gradient(ob_.ref, r.ctypes.data, 24, 0, 24, buf.ctypes.data) == -2
+
+
+@pytest.mark.parametrize("name,w", [("H2", 0.2), ("LiH", -0.12), ("Li2", 0.08), ("CO", 0.05)])
+def test_backflow_log_derivatives_vs_finite_differences_of_log_psi(name, w):
+    # eq. 6 factors of a backflow wavefunction: the Jastrow entries (J sits at r), the CI entries (determinants at the
+    # backflow coordinates) and the backflow weight itself (last entry) against Richardson central differences of the
+    # pinned log|Psi| in each parameter
+    import copy
+    d, r = wl.CONFIGS[name](M=6)
+    d = _with_bf(d, w)
+    O = ob.log_derivatives(ob.OracleSystem(d), r)
+    n_det = len(d.ci_coeff)
+    assert O.shape == (6, 6 + n_det + 1)
+
+    def lp_with(**kw):
+        d2 = copy.copy(d)
+        for k, v in kw.items():
+            setattr(d2, k, v)
+        return ob.local_energy(ob.OracleSystem(d2), r)[0]
+
+    def fd(field, value, h, index=None):
+        def at(x):
+            if index is None:
+                return lp_with(**{field: x})
+            arr = np.array(getattr(d, field), dtype=np.float64).copy()
+            arr[index] = x
+            return lp_with(**{field: arr})
+        d1 = (at(value + h) - at(value - h)) / (2 * h)
+        d2 = (at(value + 2 * h) - at(value - 2 * h)) / (4 * h)
+        return (4 * d1 - d2) / 3
+
+    tol = lambda x: 1e-6 * np.maximum(1.0, np.abs(x))
+    want = fd("backflow_w", w, 1e-4)
+    assert np.all(np.abs(O[:, -1] - want) < tol(want)), (O[:, -1], want)
+    assert np.max(np.abs(O[:, -1])) > 1e-3                                    # not a vacuous comparison
+    for col, field in ((0, "jastrow_a_par"), (1, "jastrow_a_anti"), (2, "jastrow_b")):
+        want = fd(field, getattr(d, field), 1e-3)
+        assert np.all(np.abs(O[:, col] - want) < tol(want)), (field, O[:, col], want)
+    for n in range(min(n_det, 4)):
+        want = fd("ci_coeff", float(d.ci_coeff[n]), 1e-3 * max(1.0, abs(float(d.ci_coeff[n]))), index=n)
+        assert np.all(np.abs(O[:, 6 + n] - want) < tol(want)), (n, O[:, 6 + n], want)
+    # the CI entries are the determinant ratios at the BACKFLOW coordinates: with w they differ from the plain ones
+    if n_det > 1:
+        O0 = ob.log_derivatives(ob.OracleSystem(_with_bf(d, 0.0)), r)
+        assert O0.shape == (6, 6 + n_det) and np.max(np.abs(O0[:, 6:] - O[:, 6:6 + n_det])) > 1e-6
 
 
 # ---------------------------------------------------------------- P14b: F.8 / F.9 and the table route of the backflow term
