@@ -341,9 +341,12 @@ def main():
     d_bf.backflow_w = 0.05
     sys_bf = qb.QmcSystem(d_bf, device=local_rank)
     r_bf = r0.clone()
-    t_b = [0.0, 0.0, 0.0]
+    t_b = [0.0, 0.0, 0.0, 0.0]
+    O_bf = torch.empty((r_orb.shape[2], sys_bf.n_param()), dtype=torch.float64, device=dev)
     for k in range(3 + K_DERIV):
-        e0_, e1_, e2_, e3_ = ev(), ev(), ev(), ev()
+        e0_, e1_, e2_, e3_, e4_ = ev(), ev(), ev(), ev(), ev()
+        e4_.record(st)
+        sys_bf.log_derivatives(r_orb, lp_o, sg_o, el_o, O_bf)
         e0_.record(st)
         sys_bf.local_energy(r_orb, lp_o, sg_o, el_o)
         e1_.record(st)
@@ -356,7 +359,9 @@ def main():
             t_b[0] += e0_.elapsed_time(e1_) * 1e-3
             t_b[1] += e1_.elapsed_time(e2_) * 1e-3
             t_b[2] += e2_.elapsed_time(e3_) * 1e-3
+            t_b[3] += e4_.elapsed_time(e0_) * 1e-3
     sys_bf.close()
+    del O_bf
     del dC, dz, dR, dE, r_orb, r_bf
 
     t_met, t_el, t_all, t_e2e, t_kmain, t_kfb = max_over_ranks([t_met, t_el, t_all, t_e2e, t_kmain, t_kfb], device=dev)
@@ -450,12 +455,13 @@ def main():
                                                 "tables, explicit route for groups with a near-singular reference) and the "
                                                 "estimator of eq. 7; the walkers are not equilibrated here, so F is a throughput "
                                                 "figure, not a physical force"},
-            "backflow": {"w": 0.05, "ms_local_energy": 1e3 * t_b[0] / K_DERIV, "walkers_local_energy": int(M_orb),
+            "backflow": {"w": 0.05, "ms_local_energy": 1e3 * t_b[0] / K_DERIV, "ms_log_derivatives": 1e3 * t_b[3] / K_DERIV, "walkers_local_energy": int(M_orb),
                          "ms_log_psi": 1e3 * t_b[1] / K_DERIV, "ms_metropolis": 1e3 * t_b[2] / K_DERIV, "walkers": int(M),
                          "walker_steps_per_s": world * M * n_sweeps / (t_b[2] / K_DERIV),
                          "note": "SURVEY 8(f) NEXT-3: inverse backflow K_BF = w/r; E_L from the reference's tables (F.6-F.9, "
                                  "explicit route for walkers with a nearly singular reference), values-only kernels on "
-                                 "the excitation tables"},
+                                 "the excitation tables; ms_log_derivatives = E_L + the eq. 6 factors with the backflow "
+                                 "weight as a parameter"},
             "gpu_launches": int(launches),
             "clocks": clocks,
             "last_step": {"mean_E_L": mean, "stderr": err},

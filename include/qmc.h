@@ -103,8 +103,9 @@ typedef struct {
    * the reference determinant's tables (F.6-F.9) when no determinant substitutes more than two
    * orbitals in a spin, with walkers whose reference is nearly singular - and every walker otherwise - on the explicit
    * route (every determinant eliminated on its own); qmc_log_psi and qmc_metropolis keep the excitation tables;
-   * the derivative calls (qmc_log_derivatives, qmc_orbital_derivatives, qmc_nuclear_*) return QMC_EUNSUPPORTED, and so
-   * does qmc_setup when backflow is combined with the D.2 / D.3 Jastrow kernels. */
+   * qmc_log_derivatives returns the eq. 6 factors with ONE MORE entry, the backflow weight itself (see qmc_n_param);
+   * qmc_local_energy_gradient, qmc_orbital_derivatives and qmc_nuclear_* return QMC_EUNSUPPORTED, and so does
+   * qmc_setup when backflow is combined with the D.2 / D.3 Jastrow kernels. */
   double backflow_w;
 } qmc_system_desc_t;
 
@@ -226,6 +227,10 @@ int qmc_batch_stats_static(const double *d_x, int64_t M, double *d_out, void *cu
  * Variational parameters handled: theta = (jastrow_a_par, jastrow_a_anti, jastrow_b, jastrow_en_w0,
  * jastrow_en_w1, jastrow_en_w2, then the seven parameters c, a_f, b_f, a_g, b_g, a_h, b_h of every e-e-n term in
  * een_params order (D.3), then d_0 .. d_{n_det-1}); n_param = 6 + 7 n_een + n_det (qmc_n_param).
+ * With backflow_w != 0 one more entry follows the CI entries, the backflow weight w of K_BF(r) = w / r:
+ *   d ln Psi / d w = sum_n d_n D_n [Tr(A_n^-1 d_w A_n)^up + (..)^dn] / Sigma,  d_w A[i][k] = grad phi_k(rt_i) . sum_{j != i} (r_i - r_j) / r_ij
+ * (n_param = 6 + n_det + 1; the Jastrow entries are unchanged, the CI entries are the determinant ratios at the backflow
+ * coordinates; from the reference's tables like E_L, the explicit route for walkers with a nearly singular reference).
  * The MO and AO parameters (mu, zeta of PAPER.md:55-57) have their own call, qmc_orbital_derivatives. */
 int qmc_n_param(const qmc_system_t *s);
 

@@ -287,7 +287,8 @@ class QmcSystem:
 
     def log_derivatives(self, r, logpsi=None, sign=None, eloc=None, O=None, stream=None):
         """qmc_log_derivatives: (logpsi, sign, eloc, O[M, n_param]) with O_p = (dPsi/dtheta_p)/Psi (eq. 6),
-        theta = (a_par, a_anti, b, en_w0, en_w1, en_w2, 7 parameters per e-e-n term, d_0 .. d_{n_det-1})."""
+        theta = (a_par, a_anti, b, en_w0, en_w1, en_w2, 7 parameters per e-e-n term, d_0 .. d_{n_det-1}, and -- for a
+        backflow wavefunction -- the backflow weight w)."""
         M = self._chk_r(r)
         new = lambda: torch.empty(M, dtype=torch.float64, device=r.device)
         logpsi = new() if logpsi is None else logpsi

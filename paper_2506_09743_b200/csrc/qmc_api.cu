@@ -49,6 +49,7 @@ struct Variant {
   const void *k_el_fuse, *e_el_fuse;   // E_L + fused eq. 6 reduction (without / with the e-e-n kernel)
   const void *b_psi, *b_metro, *b_el;  // backflow: values-only kernels, and the E_L kernel (explicit route)
   const void *b_tab;                   // backflow E_L from the reference's tables (F.6-F.9)
+  const void *b_el_d, *b_tab_d;        // the same two with the parameter derivatives (eq. 6 factors, backflow weight last)
   int bf_ws_doubles, bf_tab_ws_doubles, bf_e_doubles;
   int frc_ws_doubles;
 };
@@ -84,6 +85,8 @@ Variant make_variant() {
   v.b_el = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBf>;
   v.bf_ws_doubles = BfGeo<NS, NMO>::total;
   v.b_tab = (const void *)backflow_tables_kernel<NS, NMO, kWarpsBfTab>;
+  v.b_el_d = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBf, true>;
+  v.b_tab_d = (const void *)backflow_tables_kernel<NS, NMO, kWarpsBfTab, true>;
   v.bf_tab_ws_doubles = BfGeoT<NS, NMO>::total;
   v.bf_e_doubles = BfGeoT<NS, NMO>::eDoubles;
   v.e_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, false, true>;
@@ -765,7 +768,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   // substitutions in a spin
   std::vector<BfDet> bfdets;
   BfClasses bf_cls{};
-  if (P.bf_w != 0.0 && gens.empty()) {
+  if (P.bf_w != 0.0 && gens.empty() && d->n_det <= 65535) {  // (the records carry the caller's index in 16 bits)
     std::vector<Exc> by_orig(excs);
     std::sort(by_orig.begin(), by_orig.end(), [](const Exc &a, const Exc &b) { return a.orig < b.orig; });
     for (const Exc &x : by_orig) {
@@ -778,6 +781,7 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
           r.q[sp][t] = (uint8_t)x.q[sp][t];
         }
       }
+      r.orig = (uint16_t)x.orig;
       bfdets.push_back(r);
     }
     // one loop per class (k_up, k_dn) in the kernel: records sorted by class, caller order within a class
@@ -897,9 +901,9 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
   io.O = d_O;
   io.M = M;
   if (s->P.bf_w != 0.0 && el) {
-    // backflow wavefunction: E_L by its own kernel, every determinant explicit (qmc_backflow.cuh);
-    // the parameter derivatives are not derived for it
-    if (d_O) return QMC_EUNSUPPORTED;
+    // backflow wavefunction: E_L by its own kernels (qmc_backflow.cuh); with d_O their instantiations
+    // that also write the parameter derivatives, [M][qmc_n_param] with the backflow weight last
+    const void *k_el = d_O ? s->var.b_el_d : s->var.b_el, *k_tab = d_O ? s->var.b_tab_d : s->var.b_tab;
     const int smem = s->P.smem_const_bytes + kWarpsBf * s->var.bf_ws_doubles * (int)sizeof(double);
     {
       std::lock_guard<std::mutex> lock(s->scratch_mu);
@@ -908,6 +912,7 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
         cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, s->device);
         if (smem > dev_smem) return QMC_EUNSUPPORTED;
         CK(cudaFuncSetAttribute(s->var.b_el, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        CK(cudaFuncSetAttribute(s->var.b_el_d, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         int per_sm = 0;
         CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, s->var.b_el, kWarpsBf * 32, smem));
         if (per_sm < 1) return QMC_EUNSUPPORTED;
@@ -918,6 +923,7 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
           const int smem_t = s->P.smem_const_bytes + wt * s->var.bf_tab_ws_doubles * (int)sizeof(double);
           if (smem_t <= dev_smem) {
             CK(cudaFuncSetAttribute(s->var.b_tab, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t));
+            CK(cudaFuncSetAttribute(s->var.b_tab_d, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t));
             CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, s->var.b_tab, wt * 32, smem_t));
             if (per_sm >= 1) {
               s->warps_bf_tab = wt;
@@ -956,14 +962,14 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
       double *esc = reinterpret_cast<double *>(base);
       void *targs[5] = {(void *)&s->P, (void *)&io, (void *)&dets, (void *)&s->bf_cls, (void *)&esc};
       const int smem_t = s->P.smem_const_bytes + wt * s->var.bf_tab_ws_doubles * (int)sizeof(double);
-      CK(cudaLaunchKernel(s->var.b_tab, dim3(grid_t), dim3(wt * 32), targs, smem_t, st));
+      CK(cudaLaunchKernel(k_tab, dim3(grid_t), dim3(wt * 32), targs, smem_t, st));
       ++g_launches;
-      CK(cudaLaunchKernel(s->var.b_el, dim3(s->blocks_bf), dim3(kWarpsBf * 32), bargs, smem, st));
+      CK(cudaLaunchKernel(k_el, dim3(s->blocks_bf), dim3(kWarpsBf * 32), bargs, smem, st));
       ++g_launches;
       return QMC_OK;
     }
     const int grid = (int)std::min<int64_t>((M + kWarpsBf - 1) / kWarpsBf, s->blocks_bf);
-    CK(cudaLaunchKernel(s->var.b_el, dim3(grid), dim3(kWarpsBf * 32), bargs, smem, st));
+    CK(cudaLaunchKernel(k_el, dim3(grid), dim3(kWarpsBf * 32), bargs, smem, st));
     ++g_launches;
     return QMC_OK;
   }
@@ -1242,7 +1248,9 @@ int qmc_metropolis(qmc_system_t *s, double *d_r, int64_t M, double step, int32_t
   return QMC_OK;
 }
 
-int qmc_n_param(const qmc_system_t *s) { return s ? kJastrowParams + 7 * s->P.n_een + s->P.n_det_all : QMC_EINVAL; }
+int qmc_n_param(const qmc_system_t *s) {
+  return s ? kJastrowParams + 7 * s->P.n_een + s->P.n_det_all + (s->P.bf_w != 0.0 ? 1 : 0) : QMC_EINVAL;  // backflow: + its weight
+}
 
 int qmc_log_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, double *d_eloc,
                         double *d_O, void *cuda_stream) {

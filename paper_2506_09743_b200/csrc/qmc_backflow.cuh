@@ -82,7 +82,7 @@ struct BfGeoT {
   static constexpr int tSpin = 4 * NS * 8 + 2 * 3 * NS * 8 + kMaxVirt * 8;
   static constexpr int oTab = oP + cmax(NE * (NE - 1) / 2, 1) * 6;
   static constexpr int oSc = oTab + 2 * tSpin;
-  static constexpr int total = (oSc + 8 + 1) & ~1;
+  static constexpr int total = (oSc + 16 + 1) & ~1;  // scalars [16]: per spin {det, t0, s0, kappa}, then t_w per spin
   static constexpr int NC = 3 * NE;                    // coordinates l = 3 m + b
   static constexpr int LS = (NC + 3) & ~3;             // stride of an E vector in the global scratch
   static constexpr int eDoubles = 2 * kMaxVirt * NS * LS;  // E[sp][q][p][l] per warp (global memory, L2-resident)
@@ -97,7 +97,7 @@ struct BfGeoT {
 // derivatives (pair matrices P, their sums S, the C blocks) and the five MO planes at the backflow coordinates (value,
 // combined operator B = -1/2 (C_ii : Hess + L_i . grad) - gt_i . grad, d_x, d_y, d_z) into the warp's scratch.
 // Jsh / esh: this lane's share of J and of -1/2 (lap J + |grad J|^2) + V_ee + V_en.
-template <int NS, int NMO, class BG>
+template <int NS, int NMO, class BG, bool DERIV = false>
 __device__ __forceinline__ void bf_build(const SysParams &P, const double *__restrict__ sCf, const double *__restrict__ sExp,
                                          double *__restrict__ ws, const WalkerIO &io, int64_t w, int lane, double &Jsh, double &esh) {
   constexpr int NT = (NMO + 7) / 8;
@@ -119,6 +119,7 @@ __device__ __forceinline__ void bf_build(const SysParams &P, const double *__res
     double Jp = 0.0, gJx = 0.0, gJy = 0.0, gJz = 0.0, lapJ = 0.0, vee = 0.0, ven = 0.0;
     double px = 0.0, py = 0.0, pz = 0.0, Lx = 0.0, Ly = 0.0, Lz = 0.0;
     Sym3 S{0, 0, 0, 0, 0, 0}, S2{0, 0, 0, 0, 0, 0};
+    double dpar = 0.0, danti = 0.0, dbb = 0.0, dw0 = 0.0, dw1 = 0.0, dw2 = 0.0;  // DERIV: parameter derivatives of J
     const bool up = i < n_up;
     for (int o = 1; o < ne; ++o) {
       int j = i + o;
@@ -130,6 +131,11 @@ __device__ __forceinline__ void bf_build(const SysParams &P, const double *__res
       const double di = rcp_fast(fma(P.b, r, 1.0));
       const double u1 = a * di * di, u2 = -2.0 * P.b * u1 * di;
       Jp = fma(0.5 * a * di, r, Jp);
+      if (DERIV) {  // D.1: dK/da = r / (1 + b r), dK/db = -a r^2 / (1 + b r)^2; every pair is met by both of its lanes
+        const double rd = 0.5 * r * di;
+        if ((j < n_up) == up) dpar += rd; else danti += rd;
+        dbb = fma(-a * rd, r * di, dbb);
+      }
       const double sc = u1 * ri;
       gJx = fma(sc, dx, gJx); gJy = fma(sc, dy, gJy); gJz = fma(sc, dz, gJz);
       lapJ += fma(2.0, sc, u2);
@@ -149,7 +155,26 @@ __device__ __forceinline__ void bf_build(const SysParams &P, const double *__res
     }
     for (int at = 0; at < P.n_atoms; ++at) {
       const double dx = x - P.atom[at][0], dy = y - P.atom[at][1], dz = z - P.atom[at][2];
-      ven = fma(-P.atom[at][3], rsqrt_fast(fma(dx, dx, fma(dy, dy, dz * dz))), ven);
+      const double d2 = fma(dx, dx, fma(dy, dy, dz * dz)), rinv = rsqrt_fast(d2);
+      ven = fma(-P.atom[at][3], rinv, ven);
+      if (DERIV) {  // D.2: dK/dw0 = r / D, dK/dw1 = r^2 / D, dK/dw2 = -(w0 r + w1 r^2) r / D^2, D = 1 + w2 r
+        const double ra = d2 * rinv, Di = rcp_fast(fma(P.en_w2, ra, 1.0));
+        dw0 = fma(ra, Di, dw0);
+        dw1 = fma(ra * ra, Di, dw1);
+        dw2 = fma(-(P.en_w0 * ra + P.en_w1 * ra * ra) * ra, Di * Di, dw2);
+      }
+    }
+    if (DERIV) {
+      if (!act) dpar = danti = dbb = dw0 = dw1 = dw2 = 0.0;
+#pragma unroll
+      for (int mm = 16; mm > 0; mm >>= 1) {
+        dpar += shfl_xor_d(dpar, mm); danti += shfl_xor_d(danti, mm); dbb += shfl_xor_d(dbb, mm);
+        dw0 += shfl_xor_d(dw0, mm); dw1 += shfl_xor_d(dw1, mm); dw2 += shfl_xor_d(dw2, mm);
+      }
+      if (lane == 0 && io.O) {
+        double *row = io.O + w * (int64_t)(kJastrowParams + 7 * P.n_een + P.n_det_all + 1);
+        row[0] = dpar; row[1] = danti; row[2] = dbb; row[3] = dw0; row[4] = dw1; row[5] = dw2;
+      }
     }
     const double xt = fma(bw, px, x), yt = fma(bw, py, y), zt = fma(bw, pz, z);
     sGJ[lane] = gJx; sGJ[32 + lane] = gJy; sGJ[64 + lane] = gJz;
@@ -206,6 +231,9 @@ __device__ __forceinline__ void bf_build(const SysParams &P, const double *__res
       }
     }
     __syncwarp();
+    if (DERIV) {  // d rt_i / d w = sum_j (r_i - r_j) / r_ij takes the place of grad J (dead from here on)
+      sGJ[lane] = px; sGJ[32 + lane] = py; sGJ[64 + lane] = pz;
+    }
     // ---- phase 2: STOs at the backflow coordinates and AO -> MO, per electron:
     // value, combined operator b = -1/2 (C_ii : Hess + L_i . grad) - gt_i . grad, and the three gradient components
     {
@@ -292,7 +320,7 @@ __device__ __forceinline__ void bf_build(const SysParams &P, const double *__res
   }
 }
 
-template <int NS, int NMO, int WPB>
+template <int NS, int NMO, int WPB, bool DERIV = false>
 __global__ void __launch_bounds__(WPB * 32, 1)
     backflow_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -313,12 +341,17 @@ __global__ void __launch_bounds__(WPB * 32, 1)
   for (int64_t wk = (int64_t)blockIdx.x * WPB + warp; wk < n_work; wk += (int64_t)gridDim.x * WPB) {
     const int64_t w = io.fb_list ? (int64_t)io.fb_list[wk] : wk;
     double Js, es;
-    bf_build<NS, NMO, BG>(P, sCf, sExp, ws, io, w, lane, Js, es);
+    bf_build<NS, NMO, BG, DERIV>(P, sCf, sExp, ws, io, w, lane, Js, es);
     // ---- phase 3: every determinant on its own, two at a time (four (determinant, spin) problems of 8 lanes)
     const int c = lane & (kBfLP - 1), slot = lane >> 3, gbase = lane - c;
     const int dsel = slot >> 1, sp = slot & 1;
     const int ns = sp ? n_dn : n_up, e0 = sp ? n_up : 0;
-    double sig = 0.0, numk = 0.0;
+    double sig = 0.0, numk = 0.0, numw = 0.0;
+    // DERIV (eq. 6 factors): row of this walker; the Jastrow entries are bf_build's, the CI entries D_n / Sigma
+    // and the backflow weight's sum_n d_n D_n [Tr(A_n^-1 d_w A_n)^up + ^dn] / Sigma with d_w A[i][k] = grad phi_k . d rt_i / d w
+    const int nj = kJastrowParams + 7 * P.n_een;
+    double *orow = (DERIV && io.O) ? io.O + w * (int64_t)(nj + P.n_det_all + 1) : nullptr;
+    const double *sPw = ws + BG::oGJ;
     for (int n0 = 0; n0 < P.n_det_all; n0 += 2) {
       const int n = n0 + dsel;
       const bool nvalid = n < P.n_det_all;
@@ -404,11 +437,12 @@ __global__ void __launch_bounds__(WPB * 32, 1)
       __syncwarp();
       // E2 of this determinant: lane ld of its 16 lanes = electron ld (both spins)
       const int ld = lane & 15, dme = lane >> 4;  // dme = which of the two determinants
-      double e2 = 0.0;
+      double e2 = 0.0, tw = 0.0;
       if (ld < ne) {
         const int spi = (ld < n_up) ? 0 : 1, ii = ld - (spi ? n_up : 0);
         const double *Wi = sW + ((dme * 2 + spi) * 3) * NS * NS;
         const double wi[3] = {Wi[(0 * NS + ii) * NS + ii], Wi[(1 * NS + ii) * NS + ii], Wi[(2 * NS + ii) * NS + ii]};
+        if (DERIV) tw = fma(sPw[ld], wi[0], fma(sPw[32 + ld], wi[1], sPw[64 + ld] * wi[2]));
         for (int j = 0; j < ne; ++j) {
           const int spj = (j < n_up) ? 0 : 1, jj = j - (spj ? n_up : 0);
           const double *Wj = sW + ((dme * 2 + spj) * 3) * NS * NS;
@@ -430,10 +464,19 @@ __global__ void __launch_bounds__(WPB * 32, 1)
       }
 #pragma unroll
       for (int mm = 8; mm > 0; mm >>= 1) e2 += shfl_xor_d(e2, mm);
+      if (DERIV) {
+#pragma unroll
+        for (int mm = 8; mm > 0; mm >>= 1) tw += shfl_xor_d(tw, mm);
+      }
       if (ld == 0 && (n0 + dme) < P.n_det_all) {
-        const double wn = P.det_cols[n0 + dme].d * sPr[(dme * 2) * 2 + 0] * sPr[(dme * 2 + 1) * 2 + 0];
+        const double dd = sPr[(dme * 2) * 2 + 0] * sPr[(dme * 2 + 1) * 2 + 0];
+        const double wn = P.det_cols[n0 + dme].d * dd;
         sig += wn;                                                                            // eq. 4
         numk = fma(wn, sPr[(dme * 2) * 2 + 1] + sPr[(dme * 2 + 1) * 2 + 1] - 0.5 * e2, numk);  // F.2, F.4, F.5
+        if (DERIV) {
+          numw = fma(wn, tw, numw);
+          if (orow) orow[nj + n0 + dme] = dd;  // D_n^up D_n^dn, divided by Sigma below
+        }
       }
       __syncwarp();
     }
@@ -447,6 +490,15 @@ __global__ void __launch_bounds__(WPB * 32, 1)
       if (io.sign) io.sign[w] = (sig > 0.0) ? 1.0 : ((sig < 0.0) ? -1.0 : 0.0);
       if (io.eloc) io.eloc[w] = es + numk / sig + P.vnn;
     }
+    if (DERIV) {
+      numw += __shfl_xor_sync(0xffffffffu, numw, 16);
+      const double isig = 1.0 / __shfl_sync(0xffffffffu, sig, 0);
+      __syncwarp();  // the determinant products of lanes 0 and 16 are visible to the whole warp
+      if (orow) {
+        for (int n = lane; n < P.n_det_all; n += 32) orow[nj + n] *= isig;
+        if (lane == 0) orow[nj + P.n_det_all] = numw * isig;
+      }
+    }
     __syncwarp();
   }
 }
@@ -458,8 +510,10 @@ struct BfDet {
   uint8_t k[2];
   uint8_t p[2][2];
   uint8_t q[2][2];
-  uint8_t pad[6];
+  uint16_t orig;  // caller's index of the determinant (the records are sorted by class)
+  uint8_t pad[4];
 };
+static_assert(sizeof(BfDet) == 24, "BfDet is read as three 8-byte words");
 
 // Class boundaries of the sorted records: class 3 k_up + k_dn occupies [start[c], start[c + 1]).
 struct BfClasses { int start[10]; };
@@ -467,15 +521,17 @@ struct BfClasses { int start[10]; };
 // One spin's share of a determinant in the table route, substitution order K known at compile time: R = det T_PQ,
 // Rd = Tr(adj(T_PQ) M1_PQ), trY = Tr(adj(T_PQ) Y2_PQ), e = Tr(adj(T_PQ) E_PQ,l) and dm = det E_PQ,l for this lane's two
 // coordinates.
-struct BfSpinTerms { double R, Rd, trY, e0, e1, dm0, dm1; };
-template <int K, int NS, int LS>
+struct BfSpinTerms { double R, Rd, trY, e0, e1, dm0, dm1, Rw; };
+template <int K, int NS, int LS, bool DERIV = false>
 __device__ __forceinline__ void bf_spin_terms(const double *__restrict__ T, const double *__restrict__ M1, const double *__restrict__ Y2,
                                               const double *__restrict__ Es, unsigned p0, unsigned p1, unsigned q0, unsigned q1,
-                                              bool has0, bool has1, int l0, int l1, BfSpinTerms &o) {
-  o.R = 1.0; o.Rd = 0.0; o.trY = 0.0; o.e0 = o.e1 = o.dm0 = o.dm1 = 0.0;
+                                              bool has0, bool has1, int l0, int l1, BfSpinTerms &o,
+                                              const double *__restrict__ Mw = nullptr) {
+  o.R = 1.0; o.Rd = 0.0; o.trY = 0.0; o.e0 = o.e1 = o.dm0 = o.dm1 = 0.0; o.Rw = 0.0;
   if constexpr (K == 1) {
     o.R = T[p0 * 8 + q0];
     o.Rd = M1[p0 * 8 + q0];
+    if (DERIV) o.Rw = Mw[p0 * 8 + q0];
     o.trY = Y2[q0 * 8 + p0];
     const double *e = Es + (q0 * NS + p0) * LS;
     if (has0) o.e0 = __ldcg(e + l0);
@@ -484,6 +540,7 @@ __device__ __forceinline__ void bf_spin_terms(const double *__restrict__ T, cons
     const double t11 = T[p0 * 8 + q0], t12 = T[p0 * 8 + q1], t21 = T[p1 * 8 + q0], t22 = T[p1 * 8 + q1];
     o.R = fma(t11, t22, -t12 * t21);
     o.Rd = fma(t22, M1[p0 * 8 + q0], fma(t11, M1[p1 * 8 + q1], -fma(t12, M1[p1 * 8 + q0], t21 * M1[p0 * 8 + q1])));
+    if (DERIV) o.Rw = fma(t22, Mw[p0 * 8 + q0], fma(t11, Mw[p1 * 8 + q1], -fma(t12, Mw[p1 * 8 + q0], t21 * Mw[p0 * 8 + q1])));
     o.trY = fma(t22, Y2[q0 * 8 + p0], fma(t11, Y2[q1 * 8 + p1], -fma(t12, Y2[q0 * 8 + p1], t21 * Y2[q1 * 8 + p0])));
     const double *e11 = Es + (q0 * NS + p0) * LS, *e12 = Es + (q1 * NS + p0) * LS, *e21 = Es + (q0 * NS + p1) * LS,
                  *e22 = Es + (q1 * NS + p1) * LS;
@@ -518,7 +575,7 @@ __device__ __forceinline__ void bf_spin_terms(const double *__restrict__ T, cons
 // accumulates the l-dependent part over all determinants, one warp reduction at the end.  Walkers whose reference is
 // nearly singular (kappa / (Sigma/D0) criteria of section 5.6) are listed for the explicit kernel.
 // ---------------------------------------------------------------------------------
-template <int NS, int NMO, int WPB>
+template <int NS, int NMO, int WPB, bool DERIV = false>
 __global__ void __launch_bounds__(WPB * 32, 1)
     backflow_tables_kernel(const __grid_constant__ SysParams P, const WalkerIO io, const BfDet *__restrict__ dets,
                            const BfClasses cls, double *__restrict__ escratch) {
@@ -548,7 +605,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
   auto tabY2 = [&](int sp) { return sTab + sp * BG::tSpin + 4 * NS * 8 + 6 * NS * 8; };
   for (int64_t w = (int64_t)blockIdx.x * wpb + warp; w < io.M; w += (int64_t)gridDim.x * wpb) {
     double Js, es;
-    bf_build<NS, NMO, BG>(P, sCf, sExp, ws, io, w, lane, Js, es);
+    bf_build<NS, NMO, BG, DERIV>(P, sCf, sExp, ws, io, w, lane, Js, es);
     // ---- reference elimination: [A0 | Av | B0 | Bv | 1], lanes 0-7 spin up, 8-15 spin down (lane c = column c)
     const int c = lane & 7, sp = (lane >> 3) & 1;
     const int ns = sp ? n_dn : n_up, nv = P.nv[sp], e0 = sp ? n_up : 0;
@@ -648,6 +705,34 @@ __global__ void __launch_bounds__(WPB * 32, 1)
         }
     }
     __syncwarp();
+    if (DERIV) {
+      // the backflow weight as a parameter (eq. 6 factor): d_w A[i][k] = grad phi_k(rt_i) . pw_i, pw_i = d rt_i / d w (left in
+      // the grad J region by bf_build) is one more one-body operator: t_w = sum_i pw_i . W0[i][i] and its first-order table
+      // M_w[p][q] = sum_i rho[p][i] pw_i . m[i][q] (F.7), kept where G = A0^-1 B0 was (dead since M1)
+      const double *sPw = ws + BG::oGJ;
+      double twv = 0.0;
+      if (lane < 16) {
+        const double *W0 = tabW0(sp), *Mq = tabMq(sp), *Rho = tabRho(sp);
+        double *Mw = tabG(sp);
+        if (c < ns) twv = fma(sPw[e0 + c], W0[(0 * NS + c) * 8 + c], fma(sPw[32 + e0 + c], W0[(1 * NS + c) * 8 + c], sPw[64 + e0 + c] * W0[(2 * NS + c) * 8 + c]));
+        if (c < nv) {
+          double f[NS];
+#pragma unroll
+          for (int i = 0; i < NS; ++i)
+            f[i] = (i < ns) ? fma(sPw[e0 + i], Mq[(0 * NS + i) * 8 + c], fma(sPw[32 + e0 + i], Mq[(1 * NS + i) * 8 + c], sPw[64 + e0 + i] * Mq[(2 * NS + i) * 8 + c])) : 0.0;
+          for (int p2 = 0; p2 < ns; ++p2) {
+            double t = 0.0;
+#pragma unroll
+            for (int i = 0; i < NS; ++i)
+              if (i < ns) t = fma(Rho[p2 * 8 + i], f[i], t);
+            Mw[p2 * 8 + c] = t;
+          }
+        }
+      }
+#pragma unroll
+      for (int mm = 1; mm < 8; mm <<= 1) twv += shfl_xor_d(twv, mm);
+      if (c == 0 && lane < 16) sSc[8 + sp] = twv;
+    }
     // column b of the (symmetric) Jacobian block J_im = d rt_i / d r_m:  1 + S_i (m = i),  -P_im (m != i)
     auto jcol = [&](int i, int m, int b, double &j0, double &j1, double &j2) {
       double xx, yy, zz, xy, yz, zx;
@@ -801,7 +886,10 @@ __global__ void __launch_bounds__(WPB * 32, 1)
     // sorted by class (k_up, k_dn) at setup: one loop per class, the substitution orders known at compile time.
     {
       const double *Tu = tabT(0), *Td = tabT(1), *M1u = tabM1(0), *M1d = tabM1(1), *Y2u = tabY2(0), *Y2d = tabY2(1);
-      double den = 0.0, num1 = 0.0, uni = 0.0, accl = 0.0;
+      double den = 0.0, num1 = 0.0, uni = 0.0, accl = 0.0, numw = 0.0;
+      const double *Mwu = tabG(0), *Mwd = tabG(1);
+      const int nj = kJastrowParams + 7 * P.n_een;
+      double *orow = (DERIV && io.O) ? io.O + w * (int64_t)(nj + P.n_det_all + 1) : nullptr;
       const int l0 = lane, l1 = lane + 32;
       const bool has1 = l1 < nc, has0 = l0 < nc;
       const uint2 *raw = reinterpret_cast<const uint2 *>(dets);
@@ -818,8 +906,12 @@ __global__ void __launch_bounds__(WPB * 32, 1)
           const double d = __hiloint2double((int)w0.y, (int)w0.x);
           // bytes: k[0] k[1] | p[0][0] p[0][1] p[1][0] p[1][1] q[0][0] q[0][1] | q[1][0] q[1][1] pad...
           BfSpinTerms up, dn;
-          bf_spin_terms<ku, NS, LS>(Tu, M1u, Y2u, Eu, (w1.x >> 16) & 255u, w1.x >> 24, (w1.y >> 16) & 255u, w1.y >> 24, has0, has1, l0, l1, up);
-          bf_spin_terms<kd, NS, LS>(Td, M1d, Y2d, Ed, w1.y & 255u, (w1.y >> 8) & 255u, w2.x & 255u, (w2.x >> 8) & 255u, has0, has1, l0, l1, dn);
+          bf_spin_terms<ku, NS, LS, DERIV>(Tu, M1u, Y2u, Eu, (w1.x >> 16) & 255u, w1.x >> 24, (w1.y >> 16) & 255u, w1.y >> 24, has0, has1, l0, l1, up, Mwu);
+          bf_spin_terms<kd, NS, LS, DERIV>(Td, M1d, Y2d, Ed, w1.y & 255u, (w1.y >> 8) & 255u, w2.x & 255u, (w2.x >> 8) & 255u, has0, has1, l0, l1, dn, Mwd);
+          if (DERIV) {
+            numw = fma(d, fma(up.Rw, dn.R, up.R * dn.Rw), numw);
+            if (orow && lane == 0) orow[nj + (w2.x >> 16)] = up.R * dn.R;  // D_n / D_0, divided by Sigma / D_0 below
+          }
           den = fma(d * up.R, dn.R, den);                                      // eq. 4
           num1 = fma(d, fma(up.Rd, dn.R, up.R * dn.Rd), num1);                 // F.6 (first order)
           uni = fma(-2.0 * d, fma(dn.R, up.trY, up.R * dn.trY), uni);          // F.9 (summed over l)
@@ -863,6 +955,12 @@ __global__ void __launch_bounds__(WPB * 32, 1)
         const bool ok = (den * den <= fmin(kBfFallbackK * scale, kFallbackCap)) && (ku2 * ku2 <= kBfFallbackKappa * scale) &&
                         (kd2 * kd2 <= kBfFallbackKappa * scale);
         if (!ok && io.fb_list) io.fb_list[atomicAdd(io.fb_count, 1)] = (int)w;
+        if (DERIV && orow) orow[nj + P.n_det_all] = sSc[8] + sSc[9] + numw / den;
+      }
+      if (DERIV && orow) {
+        __syncwarp();  // lane 0's ratios are visible to the warp
+        const double iden = 1.0 / den;
+        for (int n = lane; n < P.n_det_all; n += 32) orow[nj + n] *= iden;
       }
     }
     __syncwarp();

@@ -139,13 +139,14 @@ def test_random_systems_against_the_oracle(seed):
 def test_random_backflow_systems_against_the_oracle(seed, kmax):
     """Inverse backflow on random systems (D.1 Jastrow; substitution orders <= 2: the table route of F.6-F.9 with its
     list of nearly singular walkers; orders up to 4: every determinant explicit): log|Psi| from the E_L kernel and from the
-    values-only kernel, sign, E_L, and the explicit route on the same walkers, contract tolerances with adjudication."""
+    values-only kernel, sign, E_L, the eq. 6 factors (backflow weight last), and the explicit route on the same walkers,
+    contract tolerances with adjudication."""
     import torch
     from oracle import binding as ob
     from paper_2506_09743_b200 import binding as qb
     from tests.helpers import adjudicate
     evaluated = walkers = 0
-    exc = dict(lp=0, lpv=0, el=0, elx=0)
+    exc = dict(lp=0, lpv=0, el=0, elx=0, O=0)
     for case in range(40):
         drawn = random_system(seed, case, kmax)
         if drawn is None:
@@ -168,10 +169,13 @@ def test_random_backflow_systems_against_the_oracle(seed, kmax):
         lp, sg, el = (t.cpu().numpy() for t in s.local_energy(rg))
         lpv, sgv = (t.cpu().numpy() for t in s.log_psi(rg))
         lpe, sge, ele = (t.cpu().numpy() for t in s.local_energy_explicit(rg))
+        O = s.log_derivatives(rg)[3].cpu().numpy()
         s.close()
+        O0, OX = ob.log_derivatives(o, r, threads=4), ob.log_derivatives(ox, r, threads=4)
         keep = (lpX - lpX.max() > math.log(1e-6)) & np.isfinite(elX)
         walkers += int(keep.sum())
         assert np.array_equal(sg[keep], sg0[keep]) and np.array_equal(sgv[keep], sg0[keep]) and np.array_equal(sge[keep], sg0[keep]), case
+        exc["O"] += adjudicate(O, O0, OX, 1e-8, scale=np.maximum(1, np.abs(OX)), mask=keep, what=(case, "backflow O_p"))
         esc = np.maximum(1, np.abs(elX))
         exc["lp"] += adjudicate(lp, lp0, lpX, 1e-10, mask=keep, what=(case, "backflow log|Psi|"))
         exc["lpv"] += adjudicate(lpv, lp0, lpX, 1e-10, mask=keep, what=(case, "backflow log|Psi| (values only)"))

@@ -1306,7 +1306,16 @@ def check_backflow(env, d, r, threads=8):
     n1 = adjudicate(lp, lp0, lpx, 1e-10, mask=keep, what="backflow log|Psi| (E_L kernel)")
     n2 = adjudicate(lp2, lp0, lpx, 1e-10, mask=keep, what="backflow log|Psi| (values-only kernel)")
     n3 = adjudicate(el, el0, elx, 1e-8, scale=np.maximum(1.0, np.abs(elx)), mask=keep, what="backflow E_L")
-    return n1, n2, n3, int(keep.sum())
+    # eq. 6 factors of the backflow wavefunction (Jastrow entries, CI entries at the backflow coordinates, the backflow
+    # weight last), with E_L / log|Psi| / sign of the same call bit-identical to qmc_local_energy's
+    O0, Ox = ob.log_derivatives(o, r, threads=threads), ob.log_derivatives(ox, r, threads=threads)
+    s = qb.QmcSystem(d)
+    assert s.n_param() == O0.shape[1] == 6 + len(d.ci_coeff) + 1
+    lpd, sgd, eld, O = (t.cpu().numpy() for t in s.log_derivatives(_to_gpu(torch, r)))
+    s.close()
+    assert np.array_equal(lpd, lp) and np.array_equal(sgd, sg) and np.array_equal(eld, el)
+    n4 = adjudicate(O, O0, Ox, 1e-8, scale=np.maximum(1.0, np.abs(Ox)), mask=keep, what="backflow O_p")
+    return n1, n2, max(n3, n4), int(keep.sum())
 
 
 @pytest.mark.parametrize("name,M,w", [("H2", 515, 0.2), ("LiH", 300, 0.12), ("Li2", 257, 0.08), ("CO", 129, 0.05), ("CO", 3, 0.05)])
@@ -1405,7 +1414,7 @@ def test_backflow_sampler_unsupported_calls_and_output_bounds(env):
     check_metropolis(env, _with_bf(d5, 0.05), r5, 0.2, 4, seed=12, eloc_acc=True)
     s = qb.QmcSystem(d)
     rg = _to_gpu(torch, r)
-    for call in (lambda: s.log_derivatives(rg), lambda: s.orbital_derivatives(rg, d.n_ao, d.n_mo),
+    for call in (lambda: s.local_energy_gradient(rg), lambda: s.orbital_derivatives(rg, d.n_ao, d.n_mo),
                  lambda: s.nuclear_log_gradient(rg, d.n_atoms), lambda: s.nuclear_energy_gradient(rg, d.n_atoms)):
         with pytest.raises(qb.QmcError) as ei:
             call()
@@ -1416,6 +1425,11 @@ def test_backflow_sampler_unsupported_calls_and_output_bounds(env):
     assert qb.lib().qmc_local_energy(s._h, rq.data_ptr(), M, a.ptr, b.ptr, c.ptr, torch.cuda.current_stream().cuda_stream) == 0
     torch.cuda.synchronize()
     a.check("backflow logpsi"); b.check("backflow sign"); c.check("backflow eloc")
+    a, b, c, o = _Guarded(torch, M), _Guarded(torch, M), _Guarded(torch, M), _Guarded(torch, M * s.n_param())
+    assert qb.lib().qmc_log_derivatives(s._h, rq.data_ptr(), M, a.ptr, b.ptr, c.ptr, o.ptr, torch.cuda.current_stream().cuda_stream) == 0
+    torch.cuda.synchronize()
+    a.check("backflow logpsi (derivative call)"); b.check("backflow sign (derivative call)")
+    c.check("backflow eloc (derivative call)"); o.check("backflow O")
     s.close()
     with pytest.raises(qb.QmcError) as ei:     # backflow with the many-body Jastrow kernels is outside what is built
         qb.QmcSystem(_with_en(d, 0.3, -0.05, 0.7))
