@@ -694,6 +694,26 @@ def test_vmc_example_gradient_descent_lowers_the_h2_energy(env):
     assert d_opt.jastrow_en_w1 != 0.0 and -1.20 < e[-1] < -1.10   # exact H2: -1.1745 Ha; HF-like orbital + Jastrow ~ -1.15
 
 
+def test_vmc_example_optimises_the_backflow_weight(env):
+    # eq. 6 for a backflow wavefunction (qmc_log_derivatives with the backflow weight as its last parameter): H2 with a
+    # far too strong inverse backflow, w = 0.3 and w = -0.2; descending along the gradient takes both to the same small
+    # weight and the energy down to the Jastrow-only level (seeded, hence reproducible)
+    import copy
+    from paper_2506_09743_b200 import vmc_example as vx
+    d, r = wl.h2(M=65536)
+    finals = []
+    for w0 in (0.3, -0.2):
+        d1 = copy.copy(d)
+        d1.backflow_w = w0
+        hist, d_opt = vx.optimise(d1, r, iterations=6, lr=0.2, step=0.5, verbose=False)
+        e = [h[0] for h in hist]
+        assert e[-1] < e[0] - 4 * max(hist[0][1], hist[-1][1]), (w0, hist)
+        assert hist[-1][2] < 0.1 * hist[0][2]                      # the gradient norm collapses
+        assert -1.17 < e[-1] < -1.13 and abs(d_opt.backflow_w) < 0.06, (w0, e, d_opt.backflow_w)
+        finals.append(d_opt.backflow_w)
+    assert abs(finals[0] - finals[1]) < 0.03, finals
+
+
 def test_vmc_example_recovers_detuned_exponents_through_the_orbital_derivatives(env):
     # eq. 6 with O = d ln Psi / d zeta, d ln Psi / d C (qmc_orbital_derivatives): H2 with both AO exponents scaled by 1.35;
     # descending along the orbital gradient brings zeta back towards its value and the energy down by ten standard
