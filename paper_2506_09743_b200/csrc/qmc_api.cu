@@ -14,9 +14,18 @@
 #include <unordered_map>
 #include <vector>
 
-#include "qmc_kernels.cuh"
+#include "qmc_variant.cuh"
 
 using namespace qmc;
+
+namespace qmc {  // the instantiations, one translation unit each (qmc_variant_*.cu)
+Variant variant_1_2();
+Variant variant_2_2();
+Variant variant_3_8();
+Variant variant_7_14();
+Variant variant_4_8();
+Variant variant_8_16();
+}  // namespace qmc
 
 namespace {
 
@@ -33,81 +42,17 @@ int cuda_fail(cudaError_t e, const char *what) {
     if (e__ != cudaSuccess) return cuda_fail(e__, #call); \
   } while (0)
 
-struct Variant {
-  int NS, NMO, LP, ws_doubles;
-  int wpb_psi_max;       // launch bound of the values-only kernels, in warps
-  int psi_ws_doubles;    // the values-only kernels' compact scratch
-  int metro_ws_doubles;  // the sampler's per-warp scratch: the evaluator's plus two sweeps of draws
-  bool exact;  // compiled for n_up = n_dn = NS
-  const void *k_el, *k_psi, *k_metro, *k_expl, *k_el_deriv;
-  const void *e_el, *e_psi, *e_metro, *e_expl, *e_el_deriv;
-  const void *k_orb;  // orbital-parameter derivatives, kWarpsOrb warps per block
-  const void *k_orb_small;  // the same with kWarpsOrbSmall warps (less shared memory)
-  const void *k_nuc, *k_nuc_small;  // the same kernel in nuclear mode (qmc_nuclear_log_gradient)
-  int orb_ws_doubles;
-  const void *k_frc, *k_frc_small;  // nuclear energy gradient (8 / 4 warps per block)
-  const void *k_el_fuse, *e_el_fuse;   // E_L + fused eq. 6 reduction (without / with the e-e-n kernel)
-  const void *b_psi, *b_metro, *b_el;  // backflow: values-only kernels, and the E_L kernel (explicit route)
-  const void *b_tab;                   // backflow E_L from the reference's tables (F.6-F.9)
-  const void *b_el_d, *b_tab_d;        // the same two with the parameter derivatives (eq. 6 factors, backflow weight last)
-  int bf_ws_doubles, bf_tab_ws_doubles, bf_e_doubles;
-  int frc_ws_doubles;
-};
-
-template <int NS, int NMO, bool X>
-Variant make_variant() {
-  Variant v;
-  v.NS = NS;
-  v.NMO = NMO;
-  v.LP = Geo<NS, NMO>::LP;
-  v.exact = X;
-  v.ws_doubles = Geo<NS, NMO>::total;
-  v.wpb_psi_max = kWarpsPsiOf<NS>;
-  v.psi_ws_doubles = Geo<NS, NMO>::totalC(true);
-  v.metro_ws_doubles = Geo<NS, NMO>::totalC(true) + 2 * kDrawDoubles<NS>;
-  v.k_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl>;
-  v.k_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsiOf<NS>>;
-  v.k_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsiOf<NS>>;
-  v.k_expl = (const void *)explicit_energy_kernel<NS, NMO, X, kWarpsEl>;
-  v.k_el_deriv = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true>;
-  v.k_orb = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrb>;
-  v.k_orb_small = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrbSmall>;
-  v.k_nuc = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrb, true>;
-  v.k_nuc_small = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrbSmall, true>;
-  v.orb_ws_doubles = Geo<NS, NMO>::total + Geo<NS, NMO>::orbExtra;
-  v.k_frc = (const void *)nuclear_energy_gradient_kernel<NS, NMO, X, 8>;
-  v.k_frc_small = (const void *)nuclear_energy_gradient_kernel<NS, NMO, X, 4>;
-  v.frc_ws_doubles = Geo<NS, NMO>::total + Geo<NS, NMO>::frcExtra;
-  v.k_el_fuse = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true, false, false, true>;
-  v.e_el_fuse = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true, true, false, true>;
-  v.b_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsiOf<NS>, false, false, true>;
-  v.b_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsiOf<NS>, false, true>;
-  v.b_el = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBf>;
-  v.bf_ws_doubles = BfGeo<NS, NMO>::total;
-  v.b_tab = (const void *)backflow_tables_kernel<NS, NMO, kWarpsBfTab>;
-  v.b_el_d = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBf, true>;
-  v.b_tab_d = (const void *)backflow_tables_kernel<NS, NMO, kWarpsBfTab, true>;
-  v.bf_tab_ws_doubles = BfGeoT<NS, NMO>::total;
-  v.bf_e_doubles = BfGeoT<NS, NMO>::eDoubles;
-  v.e_el = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, false, true>;
-  v.e_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsiOf<NS>, false, true>;
-  v.e_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsiOf<NS>, true>;
-  v.e_expl = (const void *)explicit_energy_kernel<NS, NMO, X, kWarpsEl, true>;
-  v.e_el_deriv = (const void *)local_energy_kernel<NS, NMO, true, X, kWarpsEl, true, true>;
-  return v;
-}
-
 const std::vector<Variant> &variants() {
   static const std::vector<Variant> v = {
 #ifndef QMC_ONLY_CO  // (experiments: build the headline instantiation only)
-      make_variant<1, 2, true>(),   // H2-like
-      make_variant<2, 2, true>(),   // LiH-like single determinant
-      make_variant<3, 8, true>(),   // Li2-like
+      variant_1_2(),   // H2-like
+      variant_2_2(),   // LiH-like single determinant
+      variant_3_8(),   // Li2-like
 #endif
-      make_variant<7, 14, true>(),  // CO-like (headline)
+      variant_7_14(),  // CO-like (headline)
 #ifndef QMC_ONLY_CO
-      make_variant<4, 8, false>(),  // generic, runtime electron counts
-      make_variant<8, 16, false>(), // generic upper bound
+      variant_4_8(),   // generic, runtime electron counts
+      variant_8_16(),  // generic upper bound
 #endif
   };
   return v;
@@ -359,10 +304,6 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     delete s;
     return QMC_EINVAL;
   }
-  if (d->backflow_w != 0.0 && (d->n_een > 0 || P.has_en)) {  // backflow is built with the Pade e-e Jastrow only
-    delete s;
-    return QMC_EUNSUPPORTED;
-  }
   if (d->n_een < 0 || (d->n_een > 0 && !d->een_params)) {
     delete s;
     return QMC_EINVAL;
@@ -497,6 +438,10 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     s->var.k_metro = var->e_metro;
     s->var.k_expl = var->e_expl;
     s->var.k_el_deriv = var->e_el_deriv;
+    if (P.bf_w != 0.0) {  // both: the values-only kernels with D.3 at r and the orbitals at the backflow coordinates
+      s->var.k_psi = var->be_psi;
+      s->var.k_metro = var->be_metro;
+    }
   }
   const int NMO = var->NMO;
   std::vector<DetRec> dets(n_packed);
@@ -903,7 +848,9 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
   if (s->P.bf_w != 0.0 && el) {
     // backflow wavefunction: E_L by its own kernels (qmc_backflow.cuh); with d_O their instantiations
     // that also write the parameter derivatives, [M][qmc_n_param] with the backflow weight last
-    const void *k_el = d_O ? s->var.b_el_d : s->var.b_el, *k_tab = d_O ? s->var.b_tab_d : s->var.b_tab;
+    const bool mb = s->P.has_en || s->P.n_een > 0;
+    const void *k_el = mb ? (d_O ? s->var.b_el_dm : s->var.b_el_m) : (d_O ? s->var.b_el_d : s->var.b_el);
+    const void *k_tab = mb ? (d_O ? s->var.b_tab_dm : s->var.b_tab_m) : (d_O ? s->var.b_tab_d : s->var.b_tab);
     const int smem = s->P.smem_const_bytes + kWarpsBf * s->var.bf_ws_doubles * (int)sizeof(double);
     {
       std::lock_guard<std::mutex> lock(s->scratch_mu);
@@ -911,8 +858,8 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
         int dev_smem = 0;
         cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, s->device);
         if (smem > dev_smem) return QMC_EUNSUPPORTED;
-        CK(cudaFuncSetAttribute(s->var.b_el, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        CK(cudaFuncSetAttribute(s->var.b_el_d, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        for (const void *k : {s->var.b_el, s->var.b_el_d, s->var.b_el_m, s->var.b_el_dm})
+          CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         int per_sm = 0;
         CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, s->var.b_el, kWarpsBf * 32, smem));
         if (per_sm < 1) return QMC_EUNSUPPORTED;
@@ -922,8 +869,8 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
           while (wt > 1 && s->P.smem_const_bytes + wt * s->var.bf_tab_ws_doubles * (int)sizeof(double) > dev_smem) --wt;
           const int smem_t = s->P.smem_const_bytes + wt * s->var.bf_tab_ws_doubles * (int)sizeof(double);
           if (smem_t <= dev_smem) {
-            CK(cudaFuncSetAttribute(s->var.b_tab, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t));
-            CK(cudaFuncSetAttribute(s->var.b_tab_d, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t));
+            for (const void *k : {s->var.b_tab, s->var.b_tab_d, s->var.b_tab_m, s->var.b_tab_dm})
+              CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_t));
             CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, s->var.b_tab, wt * 32, smem_t));
             if (per_sm >= 1) {
               s->warps_bf_tab = wt;

@@ -20,6 +20,7 @@
 #include <type_traits>
 
 #include "qmc_device.cuh"
+#include "qmc_eval.cuh"  // een_terms_inl / een_param_terms_inl (D.3)
 
 namespace qmc {
 
@@ -97,7 +98,9 @@ struct BfGeoT {
 // derivatives (pair matrices P, their sums S, the C blocks) and the five MO planes at the backflow coordinates (value,
 // combined operator B = -1/2 (C_ii : Hess + L_i . grad) - gt_i . grad, d_x, d_y, d_z) into the warp's scratch.
 // Jsh / esh: this lane's share of J and of -1/2 (lap J + |grad J|^2) + V_ee + V_en.
-template <int NS, int NMO, class BG, bool DERIV = false>
+// MB: the wavefunction carries the many-body Jastrow kernels D.2 / D.3 (own instantiations: their code costs the plain
+// ones 6 % when it is merely present).  DERIV: also the parameter derivatives of J into io.O and d rt / d w into the grad J region.
+template <int NS, int NMO, class BG, bool DERIV = false, bool MB = false>
 __device__ __forceinline__ void bf_build(const SysParams &P, const double *__restrict__ sCf, const double *__restrict__ sExp,
                                          double *__restrict__ ws, const WalkerIO &io, int64_t w, int lane, double &Jsh, double &esh) {
   constexpr int NT = (NMO + 7) / 8;
@@ -117,6 +120,27 @@ __device__ __forceinline__ void bf_build(const SysParams &P, const double *__res
     __syncwarp();
     // ---- phase 1: Jastrow (D.1), e-e and e-n potential (eq. 1), the backflow map and its derivatives
     double Jp = 0.0, gJx = 0.0, gJy = 0.0, gJz = 0.0, lapJ = 0.0, vee = 0.0, ven = 0.0;
+    if (MB && P.n_een > 0) {
+      // electron-electron-nucleus kernel (D.3): this electron's share, and with DERIV the seven parameters
+      // of every term summed over the walker's electrons.  First, while little is live.
+      double t[5];
+      een_terms_inl<true>(P, sXYZ, 0, ne, i, x, y, z, t);
+      Jp = t[0]; gJx = t[1]; gJy = t[2]; gJz = t[3]; lapJ = t[4];
+      if (DERIV) {
+        double *row = io.O ? io.O + w * (int64_t)(kJastrowParams + 7 * P.n_een + P.n_det_all + 1) : nullptr;
+        for (int mu = 0; mu < P.n_een; ++mu) {
+          double dq[7];
+          een_param_terms_inl(P, sXYZ, 0, ne, i, x, y, z, mu, dq);
+#pragma unroll
+          for (int k = 0; k < 7; ++k) {
+            double tk = act ? dq[k] : 0.0;
+#pragma unroll
+            for (int mm = 16; mm > 0; mm >>= 1) tk += shfl_xor_d(tk, mm);
+            if (lane == 0 && row) row[kJastrowParams + 7 * mu + k] = tk;
+          }
+        }
+      }
+    }
     double px = 0.0, py = 0.0, pz = 0.0, Lx = 0.0, Ly = 0.0, Lz = 0.0;
     Sym3 S{0, 0, 0, 0, 0, 0}, S2{0, 0, 0, 0, 0, 0};
     double dpar = 0.0, danti = 0.0, dbb = 0.0, dw0 = 0.0, dw1 = 0.0, dw2 = 0.0;  // DERIV: parameter derivatives of J
@@ -157,13 +181,28 @@ __device__ __forceinline__ void bf_build(const SysParams &P, const double *__res
       const double dx = x - P.atom[at][0], dy = y - P.atom[at][1], dz = z - P.atom[at][2];
       const double d2 = fma(dx, dx, fma(dy, dy, dz * dz)), rinv = rsqrt_fast(d2);
       ven = fma(-P.atom[at][3], rinv, ven);
-      if (DERIV) {  // D.2: dK/dw0 = r / D, dK/dw1 = r^2 / D, dK/dw2 = -(w0 r + w1 r^2) r / D^2, D = 1 + w2 r
+      if ((MB && P.has_en) || DERIV) {
+        // electron-nucleus Jastrow kernel (D.2): K = N / D, N = w0 r + w1 r^2, D = 1 + w2 r,
+        // K' = (N' - w2 K) / D, K'' = (N'' - 2 w2 K') / D; grad_i J += K' d / r, lap_i J += K'' + 2 K' / r
         const double ra = d2 * rinv, Di = rcp_fast(fma(P.en_w2, ra, 1.0));
-        dw0 = fma(ra, Di, dw0);
-        dw1 = fma(ra * ra, Di, dw1);
-        dw2 = fma(-(P.en_w0 * ra + P.en_w1 * ra * ra) * ra, Di * Di, dw2);
+        const double K = ra * fma(P.en_w1, ra, P.en_w0) * Di;
+        if (MB && P.has_en) {
+          const double K1 = (fma(2.0 * P.en_w1, ra, P.en_w0) - P.en_w2 * K) * Di;
+          const double K2 = 2.0 * fma(-P.en_w2, K1, P.en_w1) * Di;
+          const double sc = K1 * rinv;
+          Jp += K;
+          gJx = fma(sc, dx, gJx); gJy = fma(sc, dy, gJy); gJz = fma(sc, dz, gJz);
+          lapJ += fma(2.0, sc, K2);
+        }
+        if (DERIV) {  // dK/dw0 = r / D, dK/dw1 = r^2 / D, dK/dw2 = -N r / D^2 = -K r / D
+          const double rd = ra * Di;
+          dw0 += rd;
+          dw1 = fma(ra, rd, dw1);
+          dw2 = fma(-K, rd, dw2);
+        }
       }
     }
+
     if (DERIV) {
       if (!act) dpar = danti = dbb = dw0 = dw1 = dw2 = 0.0;
 #pragma unroll
@@ -171,8 +210,8 @@ __device__ __forceinline__ void bf_build(const SysParams &P, const double *__res
         dpar += shfl_xor_d(dpar, mm); danti += shfl_xor_d(danti, mm); dbb += shfl_xor_d(dbb, mm);
         dw0 += shfl_xor_d(dw0, mm); dw1 += shfl_xor_d(dw1, mm); dw2 += shfl_xor_d(dw2, mm);
       }
-      if (lane == 0 && io.O) {
-        double *row = io.O + w * (int64_t)(kJastrowParams + 7 * P.n_een + P.n_det_all + 1);
+      double *row = io.O ? io.O + w * (int64_t)(kJastrowParams + 7 * P.n_een + P.n_det_all + 1) : nullptr;
+      if (lane == 0 && row) {
         row[0] = dpar; row[1] = danti; row[2] = dbb; row[3] = dw0; row[4] = dw1; row[5] = dw2;
       }
     }
@@ -320,7 +359,7 @@ __device__ __forceinline__ void bf_build(const SysParams &P, const double *__res
   }
 }
 
-template <int NS, int NMO, int WPB, bool DERIV = false>
+template <int NS, int NMO, int WPB, bool DERIV = false, bool MB = false>
 __global__ void __launch_bounds__(WPB * 32, 1)
     backflow_energy_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -341,7 +380,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
   for (int64_t wk = (int64_t)blockIdx.x * WPB + warp; wk < n_work; wk += (int64_t)gridDim.x * WPB) {
     const int64_t w = io.fb_list ? (int64_t)io.fb_list[wk] : wk;
     double Js, es;
-    bf_build<NS, NMO, BG, DERIV>(P, sCf, sExp, ws, io, w, lane, Js, es);
+    bf_build<NS, NMO, BG, DERIV, MB>(P, sCf, sExp, ws, io, w, lane, Js, es);
     // ---- phase 3: every determinant on its own, two at a time (four (determinant, spin) problems of 8 lanes)
     const int c = lane & (kBfLP - 1), slot = lane >> 3, gbase = lane - c;
     const int dsel = slot >> 1, sp = slot & 1;
@@ -575,7 +614,7 @@ __device__ __forceinline__ void bf_spin_terms(const double *__restrict__ T, cons
 // accumulates the l-dependent part over all determinants, one warp reduction at the end.  Walkers whose reference is
 // nearly singular (kappa / (Sigma/D0) criteria of section 5.6) are listed for the explicit kernel.
 // ---------------------------------------------------------------------------------
-template <int NS, int NMO, int WPB, bool DERIV = false>
+template <int NS, int NMO, int WPB, bool DERIV = false, bool MB = false>
 __global__ void __launch_bounds__(WPB * 32, 1)
     backflow_tables_kernel(const __grid_constant__ SysParams P, const WalkerIO io, const BfDet *__restrict__ dets,
                            const BfClasses cls, double *__restrict__ escratch) {
@@ -605,7 +644,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
   auto tabY2 = [&](int sp) { return sTab + sp * BG::tSpin + 4 * NS * 8 + 6 * NS * 8; };
   for (int64_t w = (int64_t)blockIdx.x * wpb + warp; w < io.M; w += (int64_t)gridDim.x * wpb) {
     double Js, es;
-    bf_build<NS, NMO, BG, DERIV>(P, sCf, sExp, ws, io, w, lane, Js, es);
+    bf_build<NS, NMO, BG, DERIV, MB>(P, sCf, sExp, ws, io, w, lane, Js, es);
     // ---- reference elimination: [A0 | Av | B0 | Bv | 1], lanes 0-7 spin up, 8-15 spin down (lane c = column c)
     const int c = lane & 7, sp = (lane >> 3) & 1;
     const int ns = sp ? n_dn : n_up, nv = P.nv[sp], e0 = sp ? n_up : 0;

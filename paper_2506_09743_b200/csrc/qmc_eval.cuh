@@ -32,7 +32,7 @@ __device__ __forceinline__ void excite_double(uint32_t idx, const double *__rest
 
 // General substitution order k (> 2): R = det T[p,q]; Rd = Tr(adj(T[p,q]) Mt[p,q]) = sum_j det(T[p,q] with
 // column j taken from Mt[p,q]) -- division-free, valid at R = 0.  Rare path: local-memory k x k LU.
-__device__ __noinline__ double small_det(double *a, int k) {
+static __device__ __noinline__ double small_det(double *a, int k) {
   double det = 1.0;
   for (int c = 0; c < k; ++c) {
     int piv = c;
@@ -86,11 +86,12 @@ __device__ __noinline__ void excite_general(const GenSpin *g, const double *T, i
 // The lane keeps only its own electron's share: of the two ordered pairs (i,j) and (j,i)
 //   u  = c (g_j f_i + f_j g_i),  v' = c (g_j f'_i + f_j g'_i),  vL = c (g_j (f''_i + 2f'_i/r_ai) + f_j (g''_i + 2g'_i/r_ai))
 //   J share 1/2 u h;  grad_i += v' h e_ai + u h' e_ij;  lap_i += vL h + u (h'' + 2h'/r_ij) + 2 v' h' e_ai.e_ij.
-// Out of line (rare option, keeps the hot kernels small).  out = {J share, grad x, y, z, lap}.
+// Out of line in the plain kernels (rare option, keeps the hot kernels small; een_terms), inlined in the backflow
+// kernels (a call there costs more in spills than it saves; een_terms_inl).  out = {J share, grad x, y, z, lap}.
 // ---------------------------------------------------------------------------------
 template <bool EL>
-__device__ __noinline__ void een_terms(const SysParams &P, const double *sXYZ, int base, int ne, int e, double x, double y,
-                                       double z, double *out) {
+__device__ __forceinline__ void een_terms_inl(const SysParams &P, const double *sXYZ, int base, int ne, int e, double x, double y,
+                                              double z, double *out) {
   double Jp = 0.0, gx = 0.0, gy = 0.0, gz = 0.0, lap = 0.0;
   const int n = P.n_een;
   for (int at = 0; at < P.n_atoms; ++at) {
@@ -169,13 +170,18 @@ __device__ __noinline__ void een_terms(const SysParams &P, const double *sXYZ, i
   out[3] = gz;
   out[4] = lap;
 }
+template <bool EL>
+__device__ __noinline__ void een_terms(const SysParams &P, const double *sXYZ, int base, int ne, int e, double x, double y,
+                                       double z, double *out) {
+  een_terms_inl<EL>(P, sXYZ, base, ne, e, x, y, z, out);
+}
 
 // Parameter derivatives of the e-e-n kernel (eq. 6 factors of D.3): for the lane's electron i and term mu the sums over
 // nuclei a and partners j != i (the ordered pairs that start at i) of d(c f(r_ai) g(r_aj) h(r_ij))/d(c, a_f, b_f, a_g,
 // b_g, a_h, b_h), with p = a r/(1 + b r): dp/da = r/(1 + b r) =: P, dp/db = -a r^2/(1 + b r)^2 = -p P.  q0 = c / 2 is the
 // weight of an ordered pair (reading Q22), so d/dc carries the 1/2 explicitly.  Out of line.
-__device__ __noinline__ void een_param_terms(const SysParams &P, const double *sXYZ, int base, int ne, int e, double x,
-                                             double y, double z, int mu, double *dq) {
+__device__ __forceinline__ void een_param_terms_inl(const SysParams &P, const double *sXYZ, int base, int ne, int e, double x,
+                                                    double y, double z, int mu, double *dq) {
   const double q0 = P.een[mu][0], q1 = P.een[mu][1], q2 = P.een[mu][2], q3 = P.een[mu][3], q4 = P.een[mu][4],
                q5 = P.een[mu][5], q6 = P.een[mu][6];
   double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0, s4 = 0.0, s5 = 0.0, s6 = 0.0;
@@ -214,6 +220,10 @@ __device__ __noinline__ void een_param_terms(const SysParams &P, const double *s
   dq[4] = q0 * s4;
   dq[5] = q0 * s5;
   dq[6] = q0 * s6;
+}
+static __device__ __noinline__ void een_param_terms(const SysParams &P, const double *sXYZ, int base, int ne, int e, double x,
+                                             double y, double z, int mu, double *dq) {
+  een_param_terms_inl(P, sXYZ, base, ne, e, x, y, z, mu, dq);
 }
 
 // ---------------------------------------------------------------------------------

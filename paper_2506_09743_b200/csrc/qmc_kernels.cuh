@@ -518,6 +518,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
   }
 }
 
+#ifndef QMC_VARIANT_TU  // (the per-variant translation units hold only the template kernels)
 // ---------------------------------------------------------------------------------
 // Nuclear dependence of the Jastrow factor (eq. 7's grad_alpha ln rho): dR[w][a][c] = d J / d R_a,c
 //   D.2: K(r_ia) = (w0 r + w1 r^2) / (1 + w2 r)              ->  -K' e_ai
@@ -574,6 +575,7 @@ __global__ void __launch_bounds__(128)
   }
 }
 
+#endif  // QMC_VARIANT_TU
 // ---------------------------------------------------------------------------------
 // Nuclear gradient of the local energy, grad_alpha E_L: the first term of the force estimator, eq. 7.
 // The atomic positions are inputs of the AO layer: d phi_beta(r_i) / d R_alpha = -grad phi_beta(r_i)
@@ -788,6 +790,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
   }
 }
 
+#ifndef QMC_VARIANT_TU  // (the per-variant translation units hold only the template kernels)
 // d (V_en + V_nn) / d R_alpha (eq. 1): -Z_alpha sum_i (r_i - R_alpha) / |r_i - R_alpha|^3
 // - Z_alpha sum_beta Z_beta (R_alpha - R_beta) / |R_alpha - R_beta|^3.  One thread per walker; writes every entry of dE.
 __global__ void __launch_bounds__(128)
@@ -870,6 +873,7 @@ __global__ void __launch_bounds__(128) force_final_kernel(const double *__restri
   }
 }
 
+#endif  // QMC_VARIANT_TU
 // ---------------------------------------------------------------------------------
 // Persistent all-electron Metropolis (readings Q9, Q10).
 // Walker coordinates and log|Psi| stay in registers for all sweeps.
@@ -981,6 +985,7 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS)
   }
 }
 
+#ifndef QMC_VARIANT_TU  // (the per-variant translation units hold only the template kernels)
 // every group on the explicit kernel's work list (qmc_local_energy_explicit)
 __global__ void __launch_bounds__(256) list_all_groups_kernel(int *__restrict__ count, int *__restrict__ list,
                                                               int *__restrict__ done, int n_groups) {
@@ -1270,4 +1275,5 @@ __global__ void __launch_bounds__(256) fp64_probe_kernel(double *out, int iters,
   if (s == 123.456) out[0] = s;
 }
 
+#endif  // QMC_VARIANT_TU
 }  // namespace qmc

@@ -137,7 +137,7 @@ def test_random_systems_against_the_oracle(seed):
 
 @pytest.mark.parametrize("seed,kmax", [(21, 2), (22, 4)])
 def test_random_backflow_systems_against_the_oracle(seed, kmax):
-    """Inverse backflow on random systems (D.1 Jastrow; substitution orders <= 2: the table route of F.6-F.9 with its
+    """Inverse backflow on random systems (all Jastrow variants; substitution orders <= 2: the table route of F.6-F.9 with its
     list of nearly singular walkers; orders up to 4: every determinant explicit): log|Psi| from the E_L kernel and from the
     values-only kernel, sign, E_L, the eq. 6 factors (backflow weight last), and the explicit route on the same walkers,
     contract tolerances with adjudication."""
@@ -153,8 +153,6 @@ def test_random_backflow_systems_against_the_oracle(seed, kmax):
             continue
         d, r = drawn
         rng = np.random.default_rng([seed, case, 7])
-        d.jastrow_en_w0 = d.jastrow_en_w1 = d.jastrow_en_w2 = 0.0   # backflow is built for the D.1 Jastrow
-        d.jastrow_een = None
         d.backflow_w = float(rng.uniform(-0.2, 0.2))
         try:
             s = qb.QmcSystem(d, 0)

@@ -1330,7 +1330,8 @@ def check_backflow(env, d, r, threads=8):
     # weight last), with E_L / log|Psi| / sign of the same call bit-identical to qmc_local_energy's
     O0, Ox = ob.log_derivatives(o, r, threads=threads), ob.log_derivatives(ox, r, threads=threads)
     s = qb.QmcSystem(d)
-    assert s.n_param() == O0.shape[1] == 6 + len(d.ci_coeff) + 1
+    n_een = 0 if d.jastrow_een is None else len(d.jastrow_een)
+    assert s.n_param() == O0.shape[1] == 6 + 7 * n_een + len(d.ci_coeff) + 1
     lpd, sgd, eld, O = (t.cpu().numpy() for t in s.log_derivatives(_to_gpu(torch, r)))
     s.close()
     assert np.array_equal(lpd, lp) and np.array_equal(sgd, sg) and np.array_equal(eld, el)
@@ -1425,6 +1426,21 @@ def test_backflow_full_size_table_route_against_the_explicit_route_and_sampled_o
     assert float(rel.max()) < 5e-9, float(rel.max())               # half the contract's bound between the two routes
 
 
+@pytest.mark.parametrize("name,M,w", [("H2", 131, -0.15), ("LiH", 200, 0.1), ("Li2", 131, 0.08), ("CO", 67, 0.05)])
+def test_backflow_with_the_many_body_jastrow(env, name, M, w):
+    """Backflow combined with the electron-nucleus and electron-electron-nucleus Jastrow kernels (D.2, D.3,
+    PAPER.md:245-253; the Jastrow factor and its derivatives sit at r, the orbitals at the backflow coordinates): E_L,
+    log|Psi| from both kernels, the eq. 6 factors of all 6 + 7 n_een + n_det + 1 parameters, and the sampler."""
+    d, r = wl.CONFIGS[name](M=M)
+    d_en = _with_bf(_with_en(d, 0.3, -0.05, 0.7), w)
+    n1, n2, n3, nk = check_backflow(env, d_en, r)
+    assert max(n1, n2, n3) <= max(2, nk // 20), (n1, n2, n3, nk)
+    d_all = _with_bf(_with_een(_with_en(d, 0.2, -0.03, 0.8)), w)
+    n1, n2, n3, nk = check_backflow(env, d_all, r)
+    assert max(n1, n2, n3) <= max(2, nk // 20), (n1, n2, n3, nk)
+    check_metropolis(env, d_all, r[:, :, :64].copy(), 0.3, 3, seed=21, eloc_acc=True)
+
+
 def test_backflow_sampler_unsupported_calls_and_output_bounds(env):
     torch, ob, qb = env
     d, r = wl.li2(M=301)
@@ -1451,9 +1467,6 @@ def test_backflow_sampler_unsupported_calls_and_output_bounds(env):
     a.check("backflow logpsi (derivative call)"); b.check("backflow sign (derivative call)")
     c.check("backflow eloc (derivative call)"); o.check("backflow O")
     s.close()
-    with pytest.raises(qb.QmcError) as ei:     # backflow with the many-body Jastrow kernels is outside what is built
-        qb.QmcSystem(_with_en(d, 0.3, -0.05, 0.7))
-    assert ei.value.status == qb.QMC_EUNSUPPORTED
 
 
 def test_fused_energy_gradient_with_listed_groups_and_at_full_size(env):
