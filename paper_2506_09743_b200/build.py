@@ -42,7 +42,7 @@ def build(force: bool = False, verbose: bool = False, extra_flags: list[str] | N
 
         with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 1)) as ex:
             objs = list(ex.map(compile_one, SOURCES))
-        subprocess.check_call([nvcc, "-shared", "-o", out] + objs)
+        subprocess.check_call([nvcc] + FLAGS[:2] + ["-shared", "-o", out] + objs)
     finally:
         shutil.rmtree(tmp, ignore_errors=True)
     return out
