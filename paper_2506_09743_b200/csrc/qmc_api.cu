@@ -71,6 +71,7 @@ struct ReduceScratch {
   double *d_gpart = nullptr;     // [blocks][n_param] partials of gradient_partial_kernel
   size_t gpart_doubles = 0;
 };
+constexpr int kBfTablesMinDets = 8;  // backflow E_L: expansions up to this size take the explicit kernel alone
 constexpr int kReduceBlocks = 592;  // 4 per SM on 148 SMs; any value gives the same result up to rounding order
 std::mutex g_reduce_mu;
 std::unordered_map<uint64_t, ReduceScratch> g_reduce;
@@ -175,7 +176,7 @@ struct qmc_system {
   bool fuse_ready = false; // fused E_L + eq. 6 kernel configured (lazily)
   int blocks_fuse = 0, smem_fuse = 0;
   bool bf_ready = false;   // backflow E_L kernels configured (lazily)
-  int blocks_bf = 0, blocks_bf_tab = 0, warps_bf_tab = 0;
+  int blocks_bf = 0, blocks_bf_tab = 0, warps_bf_tab = 0, warps_bf = 0;
   void *d_bfdets = nullptr;  // BfDet records of the table route (null: the expansion has general determinants)
   int n_bfdets = 0;
   BfClasses bf_cls{};      // class boundaries of the sorted records
@@ -851,20 +852,27 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
     const bool mb = s->P.has_en || s->P.n_een > 0;
     const void *k_el = mb ? (d_O ? s->var.b_el_dm : s->var.b_el_m) : (d_O ? s->var.b_el_d : s->var.b_el);
     const void *k_tab = mb ? (d_O ? s->var.b_tab_dm : s->var.b_tab_m) : (d_O ? s->var.b_tab_d : s->var.b_tab);
-    const int smem = s->P.smem_const_bytes + kWarpsBf * s->var.bf_ws_doubles * (int)sizeof(double);
+    auto smem_for = [&](int warps) { return s->P.smem_const_bytes + warps * s->var.bf_ws_doubles * (int)sizeof(double); };
     {
       std::lock_guard<std::mutex> lock(s->scratch_mu);
       if (!s->bf_ready) {
         int dev_smem = 0;
         cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, s->device);
-        if (smem > dev_smem) return QMC_EUNSUPPORTED;
+        int we = kWarpsBfTab;  // the explicit kernel: as many warps per block as shared memory holds
+        while (we > 1 && smem_for(we) > dev_smem) --we;
+        if (smem_for(we) > dev_smem) return QMC_EUNSUPPORTED;
+        s->warps_bf = we;
+        const int smem = smem_for(we);
         for (const void *k : {s->var.b_el, s->var.b_el_d, s->var.b_el_m, s->var.b_el_dm})
           CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         int per_sm = 0;
-        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, s->var.b_el, kWarpsBf * 32, smem));
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, s->var.b_el, we * 32, smem));
         if (per_sm < 1) return QMC_EUNSUPPORTED;
         s->blocks_bf = per_sm * s->n_sm;
-        if (s->n_bfdets > 0) {  // the table route: as many warps per block (up to kWarpsBfTab) as shared memory holds
+        // the table route, for expansions of more than kBfTablesMinDets determinants (measured, CO shape, ms per 32768
+        // walkers, tables / explicit: 1 determinant 1.13 / 0.92, 4: 1.43 / 1.11, 20: 1.96 / 2.61, 100: 3.2 / 10.1
+        // finds the same for few determinants): as many warps per block (up to kWarpsBfTab) as shared memory holds
+        if (s->n_bfdets > kBfTablesMinDets) {
           int wt = kWarpsBfTab;
           while (wt > 1 && s->P.smem_const_bytes + wt * s->var.bf_tab_ws_doubles * (int)sizeof(double) > dev_smem) --wt;
           const int smem_t = s->P.smem_const_bytes + wt * s->var.bf_tab_ws_doubles * (int)sizeof(double);
@@ -881,6 +889,7 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
         s->bf_ready = true;
       }
     }
+    const int we = s->warps_bf, smem = smem_for(we);
     void *bargs[2] = {(void *)&s->P, (void *)&io};
     if (s->warps_bf_tab > 0 && !explicit_only) {
       // tables first (F.6-F.9), then the explicit kernel over the walkers it listed
@@ -911,12 +920,12 @@ static int launch_eval(qmc_system_t *s, const double *d_r, int64_t M, double *d_
       const int smem_t = s->P.smem_const_bytes + wt * s->var.bf_tab_ws_doubles * (int)sizeof(double);
       CK(cudaLaunchKernel(k_tab, dim3(grid_t), dim3(wt * 32), targs, smem_t, st));
       ++g_launches;
-      CK(cudaLaunchKernel(k_el, dim3(s->blocks_bf), dim3(kWarpsBf * 32), bargs, smem, st));
+      CK(cudaLaunchKernel(k_el, dim3(s->blocks_bf), dim3(we * 32), bargs, smem, st));
       ++g_launches;
       return QMC_OK;
     }
-    const int grid = (int)std::min<int64_t>((M + kWarpsBf - 1) / kWarpsBf, s->blocks_bf);
-    CK(cudaLaunchKernel(k_el, dim3(grid), dim3(kWarpsBf * 32), bargs, smem, st));
+    const int grid = (int)std::min<int64_t>((M + we - 1) / we, s->blocks_bf);
+    CK(cudaLaunchKernel(k_el, dim3(grid), dim3(we * 32), bargs, smem, st));
     ++g_launches;
     return QMC_OK;
   }

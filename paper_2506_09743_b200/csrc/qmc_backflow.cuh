@@ -57,14 +57,20 @@ struct BfGeo {
   static constexpr int oXYZ = 0;                       // [3][32] electron coordinates
   static constexpr int oGJ = oXYZ + 96;                // [3][32] grad_i J
   static constexpr int oS = oGJ + 96;                  // [6][32] S_i = sum_j P_ij
-  static constexpr int oC = oS + 192;                  // [NE][NE][9] C blocks
-  static constexpr int oMO = oC + NE * NE * 9;         // [5][NE][NMO] MO rows: value, operator, d_x, d_y, d_z
+  static constexpr int oC = oS + 192;                  // [NE (NE + 1) / 2][9] C blocks C_ii', i <= i' (C_i'i is the transpose)
+  static constexpr int oMO = oC + NE * (NE + 1) / 2 * 9;  // [5][NE][NMO] MO rows: value, operator, d_x, d_y, d_z
   static constexpr int oW = oMO + 5 * NE * NMO;        // [4][3][NS][NS] W^a of the four problems in flight
   static constexpr int oPr = oW + 4 * 3 * NS * NS;     // [4][2] {det, trace}
-  static constexpr int oP = oPr + 8;                   // [NE][NE][6] pair matrices
-  static constexpr int total = (oP + NE * NE * 6 + 1) & ~1;
+  static constexpr int oP = oPr + 8;                   // [NE (NE - 1) / 2][6] pair matrices (P_im = P_mi)
+  static constexpr int total = (oP + cmax(NE * (NE - 1) / 2, 1) * 6 + 1) & ~1;
   static constexpr bool kTab = false;
-  __device__ static __forceinline__ int pofs(int i, int m, int ne) { return (i * ne + m) * 6; }  // P_im, both orders stored
+  __device__ static __forceinline__ int pofs(int i, int m, int ne) {
+    const int a = min(i, m), b = max(i, m);
+    return ((a * (2 * ne - a - 1)) / 2 + (b - a - 1)) * 6;
+  }
+  __device__ static __forceinline__ int cofs(int a, int b, int ne) {  // a <= b
+    return (a * ne - (a * (a - 1)) / 2 + (b - a)) * 9;
+  }
 };
 
 // Scratch of the table route (backflow_tables_kernel): no off-diagonal C blocks (the same-spin ones are formed pair by
@@ -93,6 +99,29 @@ struct BfGeoT {
     return ((a * (2 * ne - a - 1)) / 2 + (b - a - 1)) * 6;
   }
 };
+
+// C_ii' = sum_m J_im J_i'm for i != i' (3x3, row-major into cc):  -J_ii P_ii' - P_ii' J_i'i' + sum_{m != i, i'} P_im P_i'm
+// from the pair matrices and their sums in the warp's scratch (J_ii = 1 + S_i, J_im = -P_im).
+template <class BG>
+__device__ __forceinline__ void bf_pair_block(const double *__restrict__ sP, const double *__restrict__ sS, int gi, int gi2, int ne,
+                                              double cc[9]) {
+  const double *pq = sP + BG::pofs(gi, gi2, ne);
+  const Sym3 Pq{pq[0], pq[1], pq[2], pq[3], pq[4], pq[5]};
+  const Sym3 J1{1.0 + sS[gi], 1.0 + sS[32 + gi], 1.0 + sS[64 + gi], sS[96 + gi], sS[128 + gi], sS[160 + gi]};
+  const Sym3 J2{1.0 + sS[gi2], 1.0 + sS[32 + gi2], 1.0 + sS[64 + gi2], sS[96 + gi2], sS[128 + gi2], sS[160 + gi2]};
+  double t[9];
+  sym_mul(J1, Pq, cc);
+  sym_mul(Pq, J2, t);
+#pragma unroll
+  for (int k = 0; k < 9; ++k) cc[k] = -cc[k] - t[k];
+  for (int m = 0; m < ne; ++m) {
+    if (m == gi || m == gi2) continue;
+    const double *p1 = sP + BG::pofs(gi, m, ne), *p2 = sP + BG::pofs(gi2, m, ne);
+    sym_mul(Sym3{p1[0], p1[1], p1[2], p1[3], p1[4], p1[5]}, Sym3{p2[0], p2[1], p2[2], p2[3], p2[4], p2[5]}, t);
+#pragma unroll
+    for (int k = 0; k < 9; ++k) cc[k] += t[k];
+  }
+}
 
 // Phases 1-2 of a backflow evaluation for walker w (one warp; lane = electron): Jastrow, potential, the backflow map and its
 // derivatives (pair matrices P, their sums S, the C blocks) and the five MO planes at the backflow coordinates (value,
@@ -172,7 +201,7 @@ __device__ __forceinline__ void bf_build(const SysParams &P, const double *__res
       S2.xy = fma(eta, Pm.xy, S2.xy); S2.yz = fma(eta, Pm.yz, S2.yz); S2.zx = fma(eta, Pm.zx, S2.zx);
       const double l3 = -4.0 * bw * ri * ri * ri;
       Lx = fma(l3, dx, Lx); Ly = fma(l3, dy, Ly); Lz = fma(l3, dz, Lz);
-      if (act && (!BG::kTab || j > i)) {
+      if (act && j > i) {  // each pair matrix once (P_ij = P_ji)
         double *pp = sP + BG::pofs(i, j, ne);
         pp[0] = Pm.xx; pp[1] = Pm.yy; pp[2] = Pm.zz; pp[3] = Pm.xy; pp[4] = Pm.yz; pp[5] = Pm.zx;
       }
@@ -243,30 +272,23 @@ __device__ __forceinline__ void bf_build(const SysParams &P, const double *__res
     if constexpr (BG::kTab) {  // the diagonal blocks only (backflow_tables_kernel forms the others where it contracts them)
       double *sCd = ws + BG::oCd;
       sCd[lane] = Cd.xx; sCd[32 + lane] = Cd.yy; sCd[64 + lane] = Cd.zz; sCd[96 + lane] = Cd.xy; sCd[128 + lane] = Cd.yz; sCd[160 + lane] = Cd.zx;
-    } else if (act) {
+    } else {
+      // every block C_ii', i <= i' (the explicit kernel's E2 runs over all pairs of both spins): the diagonal by its lane, the
+      // others one lane per unordered pair
       double *sCb = ws + BG::oC;
-      double *cb = sCb + (i * ne + i) * 9;
-      cb[0] = Cd.xx; cb[1] = Cd.xy; cb[2] = Cd.zx; cb[3] = Cd.xy; cb[4] = Cd.yy; cb[5] = Cd.yz; cb[6] = Cd.zx; cb[7] = Cd.yz; cb[8] = Cd.zz;
-      for (int i2 = 0; i2 < ne; ++i2) {
-        if (i2 == i) continue;
-        const double *pq = sP + (i * ne + i2) * 6;
-        const Sym3 Pq{pq[0], pq[1], pq[2], pq[3], pq[4], pq[5]};
-        const Sym3 J2{1.0 + sS[i2], 1.0 + sS[32 + i2], 1.0 + sS[64 + i2], sS[96 + i2], sS[128 + i2], sS[160 + i2]};
-        double acc[9], t[9];
-        sym_mul(Ji, Pq, acc);
-        sym_mul(Pq, J2, t);
+      if (act) {
+        double *cb = sCb + BG::cofs(i, i, ne);
+        cb[0] = Cd.xx; cb[1] = Cd.xy; cb[2] = Cd.zx; cb[3] = Cd.xy; cb[4] = Cd.yy; cb[5] = Cd.yz; cb[6] = Cd.zx; cb[7] = Cd.yz; cb[8] = Cd.zz;
+      }
+      for (int pi = lane; pi < ne * (ne - 1) / 2; pi += 32) {
+        int rem = pi, a = 0;
+        while (rem >= ne - 1 - a) { rem -= ne - 1 - a; ++a; }
+        const int b = a + 1 + rem;  // a < b < ne
+        double cc[9];
+        bf_pair_block<BG>(sP, sS, a, b, ne, cc);
+        double *co = sCb + BG::cofs(a, b, ne);
 #pragma unroll
-        for (int k = 0; k < 9; ++k) acc[k] = -acc[k] - t[k];
-        for (int m = 0; m < ne; ++m) {
-          if (m == i || m == i2) continue;
-          const double *p1 = sP + (i * ne + m) * 6, *p2 = sP + (i2 * ne + m) * 6;
-          sym_mul(Sym3{p1[0], p1[1], p1[2], p1[3], p1[4], p1[5]}, Sym3{p2[0], p2[1], p2[2], p2[3], p2[4], p2[5]}, t);
-#pragma unroll
-          for (int k = 0; k < 9; ++k) acc[k] += t[k];
-        }
-        double *co = sCb + (i * ne + i2) * 9;
-#pragma unroll
-        for (int k = 0; k < 9; ++k) co[k] = acc[k];
+        for (int k = 0; k < 9; ++k) co[k] = cc[k];
       }
     }
     __syncwarp();
@@ -377,7 +399,8 @@ __global__ void __launch_bounds__(WPB * 32, 1)
   const int n_up = P.n_up, n_dn = P.n_dn, ne = P.n_e;
   // list mode (io.fb_list): only the walkers the table-route kernel flagged (nearly singular reference)
   const int64_t n_work = io.fb_list ? (int64_t)*io.fb_count : io.M;
-  for (int64_t wk = (int64_t)blockIdx.x * WPB + warp; wk < n_work; wk += (int64_t)gridDim.x * WPB) {
+  const int wpb = (int)(blockDim.x >> 5);  // warps launched per block (<= WPB: as many as shared memory holds)
+  for (int64_t wk = (int64_t)blockIdx.x * wpb + warp; wk < n_work; wk += (int64_t)gridDim.x * wpb) {
     const int64_t w = io.fb_list ? (int64_t)io.fb_list[wk] : wk;
     double Js, es;
     bf_build<NS, NMO, BG, DERIV, MB>(P, sCf, sExp, ws, io, w, lane, Js, es);
@@ -485,18 +508,19 @@ __global__ void __launch_bounds__(WPB * 32, 1)
         for (int j = 0; j < ne; ++j) {
           const int spj = (j < n_up) ? 0 : 1, jj = j - (spj ? n_up : 0);
           const double *Wj = sW + ((dme * 2 + spj) * 3) * NS * NS;
-          const double *cb = sCb + (ld * ne + j) * 9;
+          const bool lo = ld <= j;  // stored block C_ab, a <= b; C_ba is its transpose
+          const double *cb = sCb + BG::cofs(lo ? ld : j, lo ? j : ld, ne);
           const double wj[3] = {Wj[(0 * NS + jj) * NS + jj], Wj[(1 * NS + jj) * NS + jj], Wj[(2 * NS + jj) * NS + jj]};
           double t = 0.0;
 #pragma unroll
           for (int a = 0; a < 3; ++a)
 #pragma unroll
-            for (int b = 0; b < 3; ++b) t = fma(cb[3 * a + b] * wi[a], wj[b], t);
+            for (int b = 0; b < 3; ++b) t = fma(cb[lo ? 3 * a + b : 3 * b + a] * wi[a], wj[b], t);
           if (spi == spj) {
 #pragma unroll
             for (int a = 0; a < 3; ++a)
 #pragma unroll
-              for (int b = 0; b < 3; ++b) t = fma(-cb[3 * a + b] * Wi[(a * NS + ii) * NS + jj], Wj[(b * NS + jj) * NS + ii], t);
+              for (int b = 0; b < 3; ++b) t = fma(-cb[lo ? 3 * a + b : 3 * b + a] * Wi[(a * NS + ii) * NS + jj], Wj[(b * NS + jj) * NS + ii], t);
           }
           e2 += t;
         }
@@ -839,22 +863,8 @@ __global__ void __launch_bounds__(WPB * 32, 1)
         while (rem >= ns2 - 1 - i) { rem -= ns2 - 1 - i; ++i; }
         const int i2 = i + 1 + rem;  // i < i2 < ns2 (positions within the spin)
         const int gi = f0 + i, gi2 = f0 + i2;
-        const double *pq = sP + BG::pofs(gi, gi2, ne);
-        const Sym3 Pq{pq[0], pq[1], pq[2], pq[3], pq[4], pq[5]};
-        const Sym3 J1{1.0 + sS[gi], 1.0 + sS[32 + gi], 1.0 + sS[64 + gi], sS[96 + gi], sS[128 + gi], sS[160 + gi]};
-        const Sym3 J2{1.0 + sS[gi2], 1.0 + sS[32 + gi2], 1.0 + sS[64 + gi2], sS[96 + gi2], sS[128 + gi2], sS[160 + gi2]};
-        double cc[9], t[9];
-        sym_mul(J1, Pq, cc);
-        sym_mul(Pq, J2, t);
-#pragma unroll
-        for (int k = 0; k < 9; ++k) cc[k] = -cc[k] - t[k];
-        for (int m = 0; m < ne; ++m) {
-          if (m == gi || m == gi2) continue;
-          const double *p1 = sP + BG::pofs(gi, m, ne), *p2 = sP + BG::pofs(gi2, m, ne);
-          sym_mul(Sym3{p1[0], p1[1], p1[2], p1[3], p1[4], p1[5]}, Sym3{p2[0], p2[1], p2[2], p2[3], p2[4], p2[5]}, t);
-#pragma unroll
-          for (int k = 0; k < 9; ++k) cc[k] += t[k];
-        }
+        double cc[9];
+        bf_pair_block<BG>(sP, sS, gi, gi2, ne, cc);
         const double *W0 = tabW0(s2);
         const double a0 = W0[(0 * NS + i) * 8 + i2], a1 = W0[(1 * NS + i) * 8 + i2], a2v = W0[(2 * NS + i) * 8 + i2];  // W0^a[i][i2]
         const double b0 = W0[(0 * NS + i2) * 8 + i], b1 = W0[(1 * NS + i2) * 8 + i], b2v = W0[(2 * NS + i2) * 8 + i];  // W0^a[i2][i]

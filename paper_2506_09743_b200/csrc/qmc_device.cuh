@@ -52,8 +52,8 @@ constexpr int kWarpsEl = QMC_WARPS, kWarpsPsi = QMC_WARPS_PSI, kWarpsOrb = QMC_W
 // largest count up to it that still fits two blocks' shared memory on an SM (long expansions: more constants)
 template <int NS>
 constexpr int kWarpsPsiOf = (NS >= 5) ? QMC_WARPS_PSI : QMC_WARPS_PSI_SMALL;
-constexpr int kWarpsBf = 4;  // warps (= walkers in flight) per block of the backflow E_L kernel
-constexpr int kWarpsBfTab = 8; // backflow_tables_kernel: at most this many (fewer when the per-warp scratch does not fit)
+constexpr int kWarpsBfTab = 8; // warps (= walkers in flight) per block of the backflow E_L kernels: at most this many (fewer
+                               // when the per-warp scratch does not fit)
 constexpr int kWarpsMax = kWarpsEl > kWarpsPsi ? kWarpsEl : kWarpsPsi;
 
 // shell record kinds

@@ -59,14 +59,14 @@ Variant make_variant() {
   v.b_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsiOf<NS>, false, true>;
   v.be_psi = (const void *)local_energy_kernel<NS, NMO, false, X, kWarpsPsiOf<NS>, false, true, true>;
   v.be_metro = (const void *)metropolis_kernel<NS, NMO, X, kWarpsPsiOf<NS>, true, true>;
-  v.b_el = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBf>;
+  v.b_el = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBfTab>;
   v.bf_ws_doubles = BfGeo<NS, NMO>::total;
   v.b_tab = (const void *)backflow_tables_kernel<NS, NMO, kWarpsBfTab>;
-  v.b_el_d = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBf, true>;
+  v.b_el_d = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBfTab, true>;
   v.b_tab_d = (const void *)backflow_tables_kernel<NS, NMO, kWarpsBfTab, true>;
-  v.b_el_m = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBf, false, true>;
+  v.b_el_m = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBfTab, false, true>;
   v.b_tab_m = (const void *)backflow_tables_kernel<NS, NMO, kWarpsBfTab, false, true>;
-  v.b_el_dm = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBf, true, true>;
+  v.b_el_dm = (const void *)backflow_energy_kernel<NS, NMO, kWarpsBfTab, true, true>;
   v.b_tab_dm = (const void *)backflow_tables_kernel<NS, NMO, kWarpsBfTab, true, true>;
   v.bf_tab_ws_doubles = BfGeoT<NS, NMO>::total;
   v.bf_e_doubles = BfGeoT<NS, NMO>::eDoubles;
