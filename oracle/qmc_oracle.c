@@ -888,7 +888,8 @@ void oracle_energy_gradient(const double *eloc, const double *O, int64_t M, int3
 
 int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                                int64_t w1, double *dC, double *dzeta) {
-  if (s->backflow_w != 0.0) return -2; /* parameter / nuclear derivatives are not derived for backflow wavefunctions */
+  /* With the backflow transformation the orbitals sit at the backflow coordinates rt, which depend on
+   * neither C nor zeta: the same formulas with phi and d phi / d zeta evaluated at rt_i. */
   int ne = s->n_up + s->n_dn, nmo = s->n_mo, nao = s->n_ao;
   real *aov = (real *)malloc(sizeof(real) * (size_t)(ne * nao + 1));      /* ao_beta(r_i) */
   real *aoz = (real *)malloc(sizeof(real) * (size_t)(ne * nao + 1));      /* d ao_beta / d zeta (r_i) */
@@ -897,10 +898,13 @@ int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, i
   real *Ai = (real *)malloc(sizeof(real) * (size_t)(2 * ne * ne + 2));    /* both spins' inverses of one determinant */
   real *gam = (real *)malloc(sizeof(real) * (size_t)(ne * nmo + 1));      /* Gamma[i][alpha], not yet / Sigma */
   real *pos = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
-  if (!aov || !aoz || !mo || !A || !Ai || !gam || !pos) return -1;
+  real *pos0 = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
+  if (!aov || !aoz || !mo || !A || !Ai || !gam || !pos || !pos0) return -1;
   real ao[5];
   for (int64_t w = w0; w < w1; ++w) {
-    gather_walker(r, M, w, ne, pos);
+    gather_walker(r, M, w, ne, pos0);
+    for (int q = 0; q < 3 * ne; ++q) pos[q] = pos0[q];
+    if (s->backflow_w != 0.0) backflow_map(s, pos0, pos, NULL, NULL);  /* pos: where the orbitals are evaluated */
     for (int i = 0; i < ne; ++i)
       for (int beta = 0; beta < nao; ++beta) {
         ao_eval_r(s, beta, pos + 3 * i, ao);
@@ -956,7 +960,7 @@ int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, i
         dzeta[(size_t)w * nao + beta] = t / sigma;
       }
   }
-  free(aov); free(aoz); free(mo); free(A); free(Ai); free(gam); free(pos);
+  free(aov); free(aoz); free(mo); free(A); free(Ai); free(gam); free(pos); free(pos0);
   return 0;
 }
 
@@ -976,7 +980,8 @@ int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, i
 
 int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                                 int64_t w1, double *dR) {
-  if (s->backflow_w != 0.0) return -2; /* parameter / nuclear derivatives are not derived for backflow wavefunctions */
+  /* With the backflow transformation the orbitals sit at the backflow coordinates rt, which do not depend
+   * on the nuclei: the Slater part with phi and grad phi at rt_i, the Jastrow parts (at r) unchanged. */
   int ne = s->n_up + s->n_dn, nmo = s->n_mo, nao = s->n_ao, na = s->n_atoms;
   real *aov = (real *)malloc(sizeof(real) * (size_t)(ne * nao + 1));       /* ao_beta(r_i) */
   real *aog = (real *)malloc(sizeof(real) * (size_t)(3 * ne * nao + 1));   /* grad ao_beta(r_i) */
@@ -985,13 +990,16 @@ int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, 
   real *Ai = (real *)malloc(sizeof(real) * (size_t)(2 * ne * ne + 2));
   real *gam = (real *)malloc(sizeof(real) * (size_t)(ne * nmo + 1));
   real *pos = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
-  if (!aov || !aog || !mo || !A || !Ai || !gam || !pos) return -1;
+  real *post = (real *)malloc(sizeof(real) * (size_t)(3 * ne + 1));
+  if (!aov || !aog || !mo || !A || !Ai || !gam || !pos || !post) return -1;
   real ao[5];
   for (int64_t w = w0; w < w1; ++w) {
     gather_walker(r, M, w, ne, pos);
+    for (int q = 0; q < 3 * ne; ++q) post[q] = pos[q];
+    if (s->backflow_w != 0.0) backflow_map(s, pos, post, NULL, NULL);  /* post: where the orbitals are evaluated */
     for (int i = 0; i < ne; ++i)
       for (int beta = 0; beta < nao; ++beta) {
-        ao_eval_r(s, beta, pos + 3 * i, ao);
+        ao_eval_r(s, beta, post + 3 * i, ao);
         aov[i * nao + beta] = ao[0];
         for (int c = 0; c < 3; ++c) aog[(i * nao + beta) * 3 + c] = ao[1 + c];
       }
@@ -1071,7 +1079,7 @@ int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, 
           }
         }
   }
-  free(aov); free(aog); free(mo); free(A); free(Ai); free(gam); free(pos);
+  free(aov); free(aog); free(mo); free(A); free(Ai); free(gam); free(pos); free(post);
   return 0;
 }
 

@@ -124,7 +124,9 @@ int oracle_log_derivatives(const oracle_system_desc_t *s, const double *r, int64
  *   d ln Sigma / d A_n[i][j] = A_n^-1[j][i]  =>  Gamma[i][alpha] = sum_n w_n A_n^-1[pos_n(alpha)][i],
  *   w_n = d_n D_n^up D_n^dn / Sigma;  dC[beta][alpha] = sum_i ao_beta(r_i) Gamma[i][alpha];
  *   dzeta[beta] = sum_alpha C[beta][alpha] sum_i (d ao_beta / d zeta)(r_i) Gamma[i][alpha].
- * Either output may be NULL.  Rows w0 <= w < w1. */
+ * Either output may be NULL.  Rows w0 <= w < w1. 
+ * With backflow_w != 0 the orbitals (and their derivatives) are evaluated at the backflow coordinates, which depend on
+ * none of these parameters; the Jastrow factor stays at r. */
 int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                                int64_t w1, double *dC, double *dzeta);
 
@@ -132,7 +134,9 @@ int oracle_orbital_derivatives(const oracle_system_desc_t *s, const double *r, i
  * estimator (eq. 7), with the atomic positions as parameters of the AO layer:
  * dR [M][n_atoms][3].  d ao_beta(r_i) / d R_a = -grad_r ao_beta(r_i) for the AOs of centre a; chain rule through
  * every determinant inverted explicitly (Gamma as in oracle_orbital_derivatives), plus the nuclear dependence of
- * the Jastrow kernels D.2 and D.3.  Rows w0 <= w < w1. */
+ * the Jastrow kernels D.2 and D.3.  Rows w0 <= w < w1. 
+ * With backflow_w != 0 the orbitals (and their derivatives) are evaluated at the backflow coordinates, which depend on
+ * none of these parameters; the Jastrow factor stays at r. */
 int oracle_nuclear_log_gradient(const oracle_system_desc_t *s, const double *r, int64_t M, int64_t w0,
                                 int64_t w1, double *dR);
 

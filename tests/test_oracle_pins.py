@@ -887,8 +887,12 @@ def test_orbital_derivatives_vs_central_differences_of_log_psi(name, M):
     # d ln Psi / d zeta_beta and d ln Psi / d C[beta][alpha] against Richardson central differences of the
     # oracle's own log|Psi| (rebuilt with one AO exponent / one MO coefficient perturbed): pins the inverse
     # transposition, the column bookkeeping over determinants, the CI weights and d(norm)/d zeta
-    import copy
     d, r = wl.CONFIGS[name](M=M)
+    _check_orbital_derivatives_fd(d, r, name)
+
+
+def _check_orbital_derivatives_fd(d, r, name):
+    import copy
     o = ob.OracleSystem(d)
     dC, dz = ob.orbital_derivatives(o, r)
     rng = np.random.default_rng(3)
@@ -950,11 +954,14 @@ def test_nuclear_log_gradient_vs_central_differences_of_log_psi(name, M):
     # grad_alpha ln|Psi| against Richardson central differences of the oracle's own (pinned) log|Psi| with one
     # nuclear coordinate displaced, D.2 and D.3 switched on: pins the sign of d ao / d R, the AO -> atom
     # bookkeeping, the CI weights, and both Jastrow chain rules
-    import copy
     d, r = wl.CONFIGS[name](M=M)
-    d = _with_een(_with_en(d, 0.3, -0.05, 0.7))
+    _check_nuclear_log_gradient_fd(_with_een(_with_en(d, 0.3, -0.05, 0.7)), r, name)
+
+
+def _check_nuclear_log_gradient_fd(d, r, name):
+    import copy
     dR = ob.nuclear_log_gradient(ob.OracleSystem(d), r)
-    assert dR.shape == (M, d.n_atoms, 3)
+    assert dR.shape == (r.shape[2], d.n_atoms, 3)
 
     def lp(a, c, t):
         d2 = copy.copy(d)
@@ -1267,6 +1274,19 @@ def test_backflow_log_derivatives_vs_finite_differences_of_log_psi(name, w):
     if n_det > 1:
         O0 = ob.log_derivatives(ob.OracleSystem(_with_bf(d, 0.0)), r)
         assert O0.shape == (6, 6 + n_det) and np.max(np.abs(O0[:, 6:] - O[:, 6:6 + n_det])) > 1e-6
+
+
+@pytest.mark.parametrize("name,M,w", [("H2", 5, 0.2), ("LiH", 4, -0.12), ("Li2", 3, 0.08), ("CO", 2, 0.05)])
+def test_backflow_orbital_and_nuclear_derivatives_vs_central_differences_of_log_psi(name, M, w):
+    # orbitals at the backflow coordinates (which depend on neither C, zeta nor the nuclei), Jastrow factor (D.1, D.2, D.3)
+    # at r: the same Richardson differences of the pinned log|Psi| as for the plain wavefunction
+    d, r = wl.CONFIGS[name](M=M)
+    _check_orbital_derivatives_fd(_with_bf(d, w), r, name)
+    _check_nuclear_log_gradient_fd(_with_bf(_with_een(_with_en(d, 0.3, -0.05, 0.7)), w), r, name)
+    # and they differ from the plain ones
+    dC0, _ = ob.orbital_derivatives(ob.OracleSystem(d), r)
+    dC1, _ = ob.orbital_derivatives(ob.OracleSystem(_with_bf(d, w)), r)
+    assert np.max(np.abs(dC1 - dC0)) > 1e-4
 
 
 # ---------------------------------------------------------------- P14b: F.8 / F.9 and the table route of the backflow term
