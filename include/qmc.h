@@ -104,8 +104,10 @@ typedef struct {
    * orbitals in a spin, with walkers whose reference is nearly singular - and every walker otherwise - on the explicit
    * route (every determinant eliminated on its own); qmc_log_psi and qmc_metropolis keep the excitation tables;
    * qmc_log_derivatives returns the eq. 6 factors with ONE MORE entry, the backflow weight itself (see qmc_n_param);
-   * qmc_local_energy_gradient, qmc_orbital_derivatives and qmc_nuclear_* return QMC_EUNSUPPORTED.  Every Jastrow
-   * kernel (D.1, D.2, D.3) combines with backflow: the Jastrow factor and its derivatives sit at r. */
+   * qmc_orbital_derivatives and qmc_nuclear_log_gradient evaluate their AOs at the backflow coordinates (which depend
+   * on neither the orbital parameters nor the nuclei); qmc_local_energy_gradient and qmc_nuclear_energy_gradient return
+   * QMC_EUNSUPPORTED.  Every Jastrow kernel (D.1, D.2, D.3) combines with backflow: the Jastrow factor and its
+   * derivatives sit at r. */
   double backflow_w;
 } qmc_system_desc_t;
 

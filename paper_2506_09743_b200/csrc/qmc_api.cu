@@ -432,6 +432,10 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
   if (P.bf_w != 0.0) {  // the values-only instantiations that evaluate the orbitals at the backflow coordinates
     s->var.k_psi = var->b_psi;
     s->var.k_metro = var->b_metro;
+    s->var.k_orb = var->k_orb_b;  // and the orbital-parameter / nuclear log-gradient kernels with the AOs there
+    s->var.k_orb_small = var->k_orb_small_b;
+    s->var.k_nuc = var->k_nuc_b;
+    s->var.k_nuc_small = var->k_nuc_small_b;
   }
   if (P.n_een > 0) {  // the instantiations that carry the e-e-n Jastrow kernel
     s->var.k_el = var->e_el;
@@ -1281,13 +1285,11 @@ static int orbital_launch(qmc_system_t *s, const double *d_r, int64_t M, double 
 
 int qmc_orbital_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d_dC, double *d_dzeta, void *cuda_stream) {
   if (!s || !d_r || M <= 0 || (!d_dC && !d_dzeta)) return QMC_EINVAL;
-  if (s->P.bf_w != 0.0) return QMC_EUNSUPPORTED;  // not derived for backflow wavefunctions
   return orbital_launch(s, d_r, M, d_dC, d_dzeta, nullptr, cuda_stream);
 }
 
 int qmc_nuclear_log_gradient(qmc_system_t *s, const double *d_r, int64_t M, double *d_dR, void *cuda_stream) {
   if (!s || !d_r || M <= 0 || !d_dR) return QMC_EINVAL;
-  if (s->P.bf_w != 0.0) return QMC_EUNSUPPORTED;  // not derived for backflow wavefunctions
   CK(cudaSetDevice(s->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
   // Jastrow part (D.2, D.3) initialises dR, one thread per walker; the AO part is subtracted by the second launch

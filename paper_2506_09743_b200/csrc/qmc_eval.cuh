@@ -269,7 +269,8 @@ __device__ void eval_walkers(const SysParams &P, const double *__restrict__ sExp
   double *sG = ws + GE::oG, *sT = ws + GE::oT, *sProb = ws + GE::oProbC(CP);
   double *sRes = ws + GE::oResC(CP);
 
-  static_assert(!BF || (!EL && !EXPL && !DERIV && ORB == 0), "backflow: values-only evaluation here");
+  // backflow here only where orbital VALUES suffice: log|Psi| and Gamma = d ln Sigma / d Phi (ORB 1, 2: orbital_derivatives_kernel)
+  static_assert(!BF || (!EL && !DERIV && (ORB == 0 ? !EXPL : (ORB == 1 || ORB == 2))), "backflow: values-only evaluation here");
   // ---- publish coordinates for the pair loop
   sXYZ[lane] = x;  // [xyz][lane]: the pair loop reads consecutive lanes
   sXYZ[32 + lane] = y;

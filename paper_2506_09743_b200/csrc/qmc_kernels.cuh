@@ -228,7 +228,9 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS_EL)
 // a second pass over the shells that rebuilds phi and d phi / d zeta = phi (d ln N / d zeta - r) in the AO tile and
 // contracts them with Gamma.  Outputs travel in io.logpsi (dC) and io.eloc (dzeta); either may be null.
 // ---------------------------------------------------------------------------------
-template <int NS, int NMO, bool X, int WPB, bool NUC = false>
+// BF: backflow wavefunction: phi, d phi / d zeta and d phi / d R are evaluated at the backflow coordinates, which
+// depend on none of these parameters; Gamma from the values-only evaluator at the same coordinates.
+template <int NS, int NMO, bool X, int WPB, bool NUC = false, bool BF = false>
 __global__ void __launch_bounds__(WPB * 32, 1)
     orbital_derivatives_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -267,9 +269,25 @@ __global__ void __launch_bounds__(WPB * 32, 1)
     // Gamma = d ln Sigma / d Phi from the reference's tables (one elimination per spin); when a walker of the group
     // has (Sigma/D_0)^2 > kFallbackOrb (reference near-singular) or the expansion has general determinants, from every
     // determinant's inverse instead: unnormalised Gamma and Sigma (sRes[4 g])
+    double xo = x, yo = y, zo = z;  // where this lane's orbitals sit
+    if (BF) {  // rt_i = r_i + w sum_{j != i} (r_i - r_j) / r_ij over the walker's other electrons (the scratch is free here)
+      ws[lane] = x; ws[32 + lane] = y; ws[64 + lane] = z;
+      __syncwarp();
+      const int base = ((lane < G * ne) ? g : 0) * ne;
+      double px = 0.0, py = 0.0, pz = 0.0;
+      for (int o = 1; o < ne; ++o) {
+        int j = e + o;
+        j -= (j >= ne) ? ne : 0;
+        const double ddx = x - ws[base + j], ddy = y - ws[32 + base + j], ddz = z - ws[64 + base + j];
+        const double ri = rsqrt_fast(fma(ddx, ddx, fma(ddy, ddy, ddz * ddz)));
+        px = fma(ddx, ri, px); py = fma(ddy, ri, py); pz = fma(ddz, ri, pz);
+      }
+      xo = fma(P.bf_w, px, x); yo = fma(P.bf_w, py, y); zo = fma(P.bf_w, pz, z);
+      __syncwarp();
+    }
     bool expl = P.n_gen > 0;
     if (!expl) {
-      eval_walkers<NS, NMO, false, X, false, false, false, 2>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
+      eval_walkers<NS, NMO, false, X, false, false, false, 2, BF>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
       for (int gg = 0; gg < G; ++gg) {
         const double den = (ws + GE::oProb)[gg * 8 + 3];  // Sigma / D_0 of walker gg (NaN for a singular reference)
         const double kap = (ws + GE::oProb)[gg * 8 + 7];  // max |T| over both spins
@@ -278,7 +296,7 @@ __global__ void __launch_bounds__(WPB * 32, 1)
       __syncwarp();
     }
     if (expl) {
-      eval_walkers<NS, NMO, false, X, true, false, false, 1>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
+      eval_walkers<NS, NMO, false, X, true, false, false, 1, BF>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
       for (int i = lane; i < G * ne * NMO; i += 32) sGam[i] /= sRes[(i / (ne * NMO)) * 4 + 0];
       __syncwarp();
     }
@@ -294,9 +312,9 @@ __global__ void __launch_bounds__(WPB * 32, 1)
       const int meta = sh.meta, kind = meta & 15;
       if (kind == SH_POW) continue;  // the radial power is in the shell records' own meta word
       if (kind == SH_ATOM) {
-        dx = x - sh.zeta;
-        dy = y - sh.c1;
-        dz = z - sh.c2;
+        dx = xo - sh.zeta;
+        dy = yo - sh.c1;
+        dz = zo - sh.c2;
         r2 = fma(dx, dx, fma(dy, dy, dz * dz));
         r = r2 * rsqrt_fast(r2);
         continue;

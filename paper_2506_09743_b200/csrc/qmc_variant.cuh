@@ -17,6 +17,7 @@ struct Variant {
   const void *k_orb;  // orbital-parameter derivatives, kWarpsOrb warps per block
   const void *k_orb_small;  // the same with kWarpsOrbSmall warps (less shared memory)
   const void *k_nuc, *k_nuc_small;  // the same kernel in nuclear mode (qmc_nuclear_log_gradient)
+  const void *k_orb_b, *k_orb_small_b, *k_nuc_b, *k_nuc_small_b;  // the four for a backflow wavefunction
   int orb_ws_doubles;
   const void *k_frc, *k_frc_small;  // nuclear energy gradient (8 / 4 warps per block)
   const void *k_el_fuse, *e_el_fuse;   // E_L + fused eq. 6 reduction (without / with the e-e-n kernel)
@@ -49,6 +50,10 @@ Variant make_variant() {
   v.k_orb_small = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrbSmall>;
   v.k_nuc = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrb, true>;
   v.k_nuc_small = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrbSmall, true>;
+  v.k_orb_b = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrb, false, true>;
+  v.k_orb_small_b = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrbSmall, false, true>;
+  v.k_nuc_b = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrb, true, true>;
+  v.k_nuc_small_b = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrbSmall, true, true>;
   v.orb_ws_doubles = Geo<NS, NMO>::total + Geo<NS, NMO>::orbExtra;
   v.k_frc = (const void *)nuclear_energy_gradient_kernel<NS, NMO, X, 8>;
   v.k_frc_small = (const void *)nuclear_energy_gradient_kernel<NS, NMO, X, 4>;

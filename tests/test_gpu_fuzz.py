@@ -146,7 +146,7 @@ def test_random_backflow_systems_against_the_oracle(seed, kmax):
     from paper_2506_09743_b200 import binding as qb
     from tests.helpers import adjudicate
     evaluated = walkers = 0
-    exc = dict(lp=0, lpv=0, el=0, elx=0, O=0)
+    exc = dict(lp=0, lpv=0, el=0, elx=0, O=0, dC=0, dz=0)
     for case in range(40):
         # (expansions of up to 8 determinants take the explicit kernel alone: longer ones for the table route)
         drawn = random_system(seed, case, kmax, n_det_max=40 if kmax == 2 else 12)
@@ -169,12 +169,17 @@ def test_random_backflow_systems_against_the_oracle(seed, kmax):
         lpv, sgv = (t.cpu().numpy() for t in s.log_psi(rg))
         lpe, sge, ele = (t.cpu().numpy() for t in s.local_energy_explicit(rg))
         O = s.log_derivatives(rg)[3].cpu().numpy()
+        dC, dz = (t.cpu().numpy() for t in s.orbital_derivatives(rg, d.n_ao, d.n_mo))
         s.close()
         O0, OX = ob.log_derivatives(o, r, threads=4), ob.log_derivatives(ox, r, threads=4)
+        dC0, dz0 = ob.orbital_derivatives(o, r, threads=4)
+        dCX, dzX = ob.orbital_derivatives(ox, r, threads=4)
         keep = (lpX - lpX.max() > math.log(1e-6)) & np.isfinite(elX)
         walkers += int(keep.sum())
         assert np.array_equal(sg[keep], sg0[keep]) and np.array_equal(sgv[keep], sg0[keep]) and np.array_equal(sge[keep], sg0[keep]), case
         exc["O"] += adjudicate(O, O0, OX, 1e-8, scale=np.maximum(1, np.abs(OX)), mask=keep, what=(case, "backflow O_p"))
+        exc["dC"] += adjudicate(dC, dC0, dCX, 1e-8, scale=np.maximum(1, np.abs(dCX)), mask=keep, what=(case, "backflow dC"))
+        exc["dz"] += adjudicate(dz, dz0, dzX, 1e-8, scale=np.maximum(1, np.abs(dzX)), mask=keep, what=(case, "backflow dzeta"))
         esc = np.maximum(1, np.abs(elX))
         exc["lp"] += adjudicate(lp, lp0, lpX, 1e-10, mask=keep, what=(case, "backflow log|Psi|"))
         exc["lpv"] += adjudicate(lpv, lp0, lpX, 1e-10, mask=keep, what=(case, "backflow log|Psi| (values only)"))

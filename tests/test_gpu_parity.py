@@ -1441,6 +1441,15 @@ def test_backflow_with_the_many_body_jastrow(env, name, M, w):
     check_metropolis(env, d_all, r[:, :, :64].copy(), 0.3, 3, seed=21, eloc_acc=True)
 
 
+@pytest.mark.parametrize("name,M,w", [("H2", 131, -0.15), ("LiH", 200, 0.1), ("Li2", 257, 0.08), ("CO", 129, 0.05)])
+def test_backflow_orbital_derivatives_and_nuclear_log_gradient(env, name, M, w):
+    """d ln Psi / d C, d ln Psi / d zeta and grad_alpha ln|Psi| of a backflow wavefunction (AOs at the backflow
+    coordinates; the nuclear gradient with the D.2 / D.3 Jastrow parts at r), both routes of the kernel."""
+    d, r = wl.CONFIGS[name](M=M)
+    check_orbital_derivatives(env, _with_bf(d, w), r)
+    check_nuclear_log_gradient(env, _with_bf(_with_een(_with_en(d, 0.2, -0.03, 0.8)), w), r)
+
+
 def test_backflow_sampler_unsupported_calls_and_output_bounds(env):
     torch, ob, qb = env
     d, r = wl.li2(M=301)
@@ -1450,8 +1459,7 @@ def test_backflow_sampler_unsupported_calls_and_output_bounds(env):
     check_metropolis(env, _with_bf(d5, 0.05), r5, 0.2, 4, seed=12, eloc_acc=True)
     s = qb.QmcSystem(d)
     rg = _to_gpu(torch, r)
-    for call in (lambda: s.local_energy_gradient(rg), lambda: s.orbital_derivatives(rg, d.n_ao, d.n_mo),
-                 lambda: s.nuclear_log_gradient(rg, d.n_atoms), lambda: s.nuclear_energy_gradient(rg, d.n_atoms)):
+    for call in (lambda: s.local_energy_gradient(rg), lambda: s.nuclear_energy_gradient(rg, d.n_atoms)):
         with pytest.raises(qb.QmcError) as ei:
             call()
         assert ei.value.status == qb.QMC_EUNSUPPORTED
