@@ -105,9 +105,9 @@ typedef struct {
    * route (every determinant eliminated on its own); qmc_log_psi and qmc_metropolis keep the excitation tables;
    * qmc_log_derivatives returns the eq. 6 factors with ONE MORE entry, the backflow weight itself (see qmc_n_param);
    * qmc_orbital_derivatives and qmc_nuclear_log_gradient evaluate their AOs at the backflow coordinates (which depend
-   * on neither the orbital parameters nor the nuclei); qmc_local_energy_gradient and qmc_nuclear_energy_gradient return
-   * QMC_EUNSUPPORTED.  Every Jastrow kernel (D.1, D.2, D.3) combines with backflow: the Jastrow factor and its
-   * derivatives sit at r. */
+   * on neither the orbital parameters nor the nuclei); qmc_local_energy_gradient gives the same estimator, not fused
+   * (the rows pass through a scratch of the handle); qmc_nuclear_energy_gradient returns QMC_EUNSUPPORTED.  Every
+   * Jastrow kernel (D.1, D.2, D.3) combines with backflow: the Jastrow factor and its derivatives sit at r. */
   double backflow_w;
 } qmc_system_desc_t;
 
@@ -255,7 +255,8 @@ int qmc_log_derivatives(qmc_system_t *s, const double *d_r, int64_t M, double *d
  *   d_logpsi, d_sign device out [M] (may be NULL);  d_eloc device out [M] (required);
  *   h_Ev host out (may be NULL);  h_grad host out [n_param].
  * Synchronises cuda_stream.  QMC_EUNSUPPORTED when the rows of a warp's walkers do not fit shared memory (very long
- * expansions: use qmc_log_derivatives + qmc_energy_gradient) or for a backflow wavefunction. */
+ * expansions: use qmc_log_derivatives + qmc_energy_gradient).  For a backflow wavefunction the call runs those two steps
+ * itself (n_param includes the backflow weight). */
 int qmc_local_energy_gradient(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, double *d_eloc,
                               double *h_Ev, double *h_grad, void *cuda_stream);
 

@@ -1302,9 +1302,29 @@ int qmc_nuclear_log_gradient(qmc_system_t *s, const double *d_r, int64_t M, doub
 int qmc_local_energy_gradient(qmc_system_t *s, const double *d_r, int64_t M, double *d_logpsi, double *d_sign, double *d_eloc,
                               double *h_Ev, double *h_grad, void *cuda_stream) {
   if (!s || !d_r || M <= 0 || !d_eloc || !h_grad) return QMC_EINVAL;
-  if (s->P.bf_w != 0.0) return QMC_EUNSUPPORTED;
   CK(cudaSetDevice(s->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (s->P.bf_w != 0.0) {
+    // backflow wavefunction: the same estimator from qmc_log_derivatives and qmc_energy_gradient, the rows [M][n_param]
+    // in a per-stream scratch of the handle (not fused: the backflow kernels hold one walker per warp and no row buffer)
+    const int npb = qmc_n_param(s);
+    const size_t need = (size_t)M * (size_t)npb * sizeof(double);
+    double *rows = nullptr;
+    {
+      std::lock_guard<std::mutex> lock(s->scratch_mu);
+      qmc_system::Scratch &sc = s->scratch[st];
+      if (sc.fuse_bytes < need) {
+        if (sc.fuse) s->retired.push_back(sc.fuse);
+        sc.fuse = nullptr;
+        sc.fuse_bytes = 0;
+        CK(cudaMalloc(&sc.fuse, need));
+        sc.fuse_bytes = need;
+      }
+      rows = static_cast<double *>(sc.fuse);
+    }
+    if (int rc = launch_eval(s, d_r, M, d_logpsi, d_sign, d_eloc, cuda_stream, true, rows)) return rc;
+    return qmc_energy_gradient(d_eloc, rows, M, npb, h_Ev, h_grad, cuda_stream);
+  }
   const int np = kJastrowParams + 7 * s->P.n_een + s->P.n_det_all, G = s->P.G;
   const int fuse_stride = ((G + 2) * np + G + 1) & ~1;  // G rows, two accumulator rows, 1 / (Sigma / D_0) per walker
   const void *kern = s->P.n_een > 0 ? s->var.e_el_fuse : s->var.k_el_fuse;

@@ -57,8 +57,8 @@ def optimise(d, r_host, iterations=12, lr=0.2, sweeps=20, step=0.4, seed=1, opti
     mask[2:N_JASTROW] = True                      # b and the electron-nucleus kernel
     if optimise_ci and len(d.ci_coeff) > 1:
         mask[N_JASTROW + 1:N_JASTROW + len(d.ci_coeff)] = True   # d_0 fixes the normalisation
-    if bf:                                        # backflow wavefunction: its weight is a parameter; the
-        mask[3:N_JASTROW] = False                 # library does not combine backflow with the e-n kernel
+    if bf:                                        # backflow wavefunction: its weight is a parameter; this
+        mask[3:N_JASTROW] = False                 # example then leaves the e-n kernel alone (b, CI and w move)
         mask[-1] = True
     history = []
     for it in range(iterations):

@@ -1332,7 +1332,12 @@ def check_backflow(env, d, r, threads=8):
     s = qb.QmcSystem(d)
     n_een = 0 if d.jastrow_een is None else len(d.jastrow_een)
     assert s.n_param() == O0.shape[1] == 6 + 7 * n_een + len(d.ci_coeff) + 1
-    lpd, sgd, eld, O = (t.cpu().numpy() for t in s.log_derivatives(_to_gpu(torch, r)))
+    lpd_t, sgd_t, eld_t, O_t = s.log_derivatives(_to_gpu(torch, r))
+    lpd, sgd, eld, O = (t.cpu().numpy() for t in (lpd_t, sgd_t, eld_t, O_t))
+    # the estimator call (for backflow: the same two steps inside the library) against the two calls made here
+    ev_u, g_u = qb.energy_gradient(eld_t, O_t)
+    _, _, _, ev_f, g_f = s.local_energy_gradient(_to_gpu(torch, r))
+    assert ev_f == ev_u and np.array_equal(g_f, g_u)
     s.close()
     assert np.array_equal(lpd, lp) and np.array_equal(sgd, sg) and np.array_equal(eld, el)
     n4 = adjudicate(O, O0, Ox, 1e-8, scale=np.maximum(1.0, np.abs(Ox)), mask=keep, what="backflow O_p")
@@ -1459,7 +1464,7 @@ def test_backflow_sampler_unsupported_calls_and_output_bounds(env):
     check_metropolis(env, _with_bf(d5, 0.05), r5, 0.2, 4, seed=12, eloc_acc=True)
     s = qb.QmcSystem(d)
     rg = _to_gpu(torch, r)
-    for call in (lambda: s.local_energy_gradient(rg), lambda: s.nuclear_energy_gradient(rg, d.n_atoms)):
+    for call in (lambda: s.nuclear_energy_gradient(rg, d.n_atoms),):
         with pytest.raises(qb.QmcError) as ei:
             call()
         assert ei.value.status == qb.QMC_EUNSUPPORTED
