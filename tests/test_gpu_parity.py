@@ -575,12 +575,22 @@ def test_local_energy_host_matches_device_call(env, M, chunks, pinned):
 
 
 # ----------------------------------------------------------------------------- CUDA graphs
-@pytest.mark.parametrize("name", ["H2", "Li2"])
-def test_calls_can_be_captured_in_a_cuda_graph(env, name):
+def _with_bf_early(d, w):
+    import copy
+    d2 = copy.copy(d)
+    d2.backflow_w = w
+    return d2
+
+
+@pytest.mark.parametrize("name,bf", [("H2", False), ("Li2", False), ("Li2", True), ("CO", True)])
+def test_calls_can_be_captured_in_a_cuda_graph(env, name, bf):
     # after one warm-up call (which sizes the handle's per-stream fallback scratch) qmc_metropolis and
     # qmc_local_energy contain nothing that breaks stream capture; a replay reproduces the eager run bit for bit
+    # (bf: the backflow kernels, table route + listed walkers on the explicit kernel)
     torch, ob, qb = env
     d, r = wl.CONFIGS[name](M=777)
+    if bf:
+        d = _with_bf_early(d, 0.07)
     s = qb.QmcSystem(d)
     r0 = _to_gpu(torch, r)
     rg = r0.clone()
