@@ -168,6 +168,7 @@ struct qmc_system {
     void *p = nullptr; size_t bytes = 0; unsigned long long *counter = nullptr;
     void *fuse = nullptr; size_t fuse_bytes = 0;  // qmc_local_energy_gradient: warp partials, parked O rows, order list
     void *bf = nullptr; size_t bf_bytes = 0;      // backflow table route: E vectors per resident warp, flagged-walker list
+    int *work = nullptr;                          // work counter of the kernels that deal their groups dynamically
   };
   std::mutex scratch_mu;
   std::unordered_map<cudaStream_t, Scratch> scratch;
@@ -232,6 +233,7 @@ void qmc_destroy(qmc_system_t *s) {
   for (auto &kv : s->scratch) {
     cudaFree(kv.second.p);
     cudaFree(kv.second.counter);
+    cudaFree(kv.second.work);
     cudaFree(kv.second.fuse);
     cudaFree(kv.second.bf);
   }
@@ -1275,6 +1277,12 @@ static int orbital_launch(qmc_system_t *s, const double *d_r, int64_t M, double 
   io.logpsi = d_dC;    // this kernel's outputs travel in the two output slots: dC [M][n_ao][n_mo], dzeta [M][n_ao]
   io.eloc = d_dzeta;
   io.O = d_dR;         // nuclear mode: dR [M][n_atoms][3], decremented by the AO part
+  {
+    qmc_system::Scratch &sc = s->scratch[st];  // (scratch_mu is held)
+    if (!sc.work) CK(cudaMalloc(&sc.work, sizeof(int)));
+    io.fb_count = sc.work;
+  }
+  CK(cudaMemsetAsync(io.fb_count, 0, sizeof(int), st));
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
   const int grid = (int)std::min<int64_t>((groups + warps - 1) / warps, s->blocks_orb);
   void *args[2] = {(void *)&s->P, (void *)&io};
@@ -1457,6 +1465,13 @@ int qmc_nuclear_energy_gradient(qmc_system_t *s, const double *d_r, int64_t M, d
   io.r_in = d_r;
   io.M = M;
   io.O = d_dE;
+  {
+    std::lock_guard<std::mutex> lock(s->scratch_mu);
+    qmc_system::Scratch &sc = s->scratch[st];
+    if (!sc.work) CK(cudaMalloc(&sc.work, sizeof(int)));
+    io.fb_count = sc.work;
+  }
+  CK(cudaMemsetAsync(io.fb_count, 0, sizeof(int), st));
   const int warps = s->frc_warps;
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
   const int grid = (int)std::min<int64_t>((groups + warps - 1) / warps, s->blocks_frc);
