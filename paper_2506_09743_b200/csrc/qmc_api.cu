@@ -168,7 +168,8 @@ struct qmc_system {
     void *p = nullptr; size_t bytes = 0; unsigned long long *counter = nullptr;
     void *fuse = nullptr; size_t fuse_bytes = 0;  // qmc_local_energy_gradient: warp partials, parked O rows, order list
     void *bf = nullptr; size_t bf_bytes = 0;      // backflow table route: E vectors per resident warp, flagged-walker list
-    int *work = nullptr;                          // work counter of the kernels that deal their groups dynamically
+    int *work = nullptr;                          // {work counter, list counter} of the kernels that deal their groups dynamically
+    void *orb = nullptr; size_t orb_bytes = 0;    // orbital_explicit_kernel: partial Gamma per work item, group list, slice counters
   };
   std::mutex scratch_mu;
   std::unordered_map<cudaStream_t, Scratch> scratch;
@@ -234,6 +235,7 @@ void qmc_destroy(qmc_system_t *s) {
     cudaFree(kv.second.p);
     cudaFree(kv.second.counter);
     cudaFree(kv.second.work);
+    cudaFree(kv.second.orb);
     cudaFree(kv.second.fuse);
     cudaFree(kv.second.bf);
   }
@@ -438,6 +440,10 @@ int qmc_setup(const qmc_system_desc_t *d, int device, qmc_system_t **out) {
     s->var.k_orb_small = var->k_orb_small_b;
     s->var.k_nuc = var->k_nuc_b;
     s->var.k_nuc_small = var->k_nuc_small_b;
+    s->var.x_orb = var->x_orb_b;
+    s->var.x_orb_small = var->x_orb_small_b;
+    s->var.x_nuc = var->x_nuc_b;
+    s->var.x_nuc_small = var->x_nuc_small_b;
   }
   if (P.n_een > 0) {  // the instantiations that carry the e-e-n Jastrow kernel
     s->var.k_el = var->e_el;
@@ -1260,6 +1266,10 @@ static int orbital_launch(qmc_system_t *s, const double *d_r, int64_t M, double 
     CK(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_for(s->orb_warps)));
     CK(cudaFuncSetAttribute(s->orb_warps == kWarpsOrb ? s->var.k_nuc : s->var.k_nuc_small,
                             cudaFuncAttributeMaxDynamicSharedMemorySize, smem_for(s->orb_warps)));
+    CK(cudaFuncSetAttribute(s->orb_warps == kWarpsOrb ? s->var.x_orb : s->var.x_orb_small,
+                            cudaFuncAttributeMaxDynamicSharedMemorySize, smem_for(s->orb_warps)));
+    CK(cudaFuncSetAttribute(s->orb_warps == kWarpsOrb ? s->var.x_nuc : s->var.x_nuc_small,
+                            cudaFuncAttributeMaxDynamicSharedMemorySize, smem_for(s->orb_warps)));
     int per_sm = 0;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, s->orb_warps * 32, smem_for(s->orb_warps)));
     if (per_sm < 1) return QMC_EUNSUPPORTED;
@@ -1277,17 +1287,35 @@ static int orbital_launch(qmc_system_t *s, const double *d_r, int64_t M, double 
   io.logpsi = d_dC;    // this kernel's outputs travel in the two output slots: dC [M][n_ao][n_mo], dzeta [M][n_ao]
   io.eloc = d_dzeta;
   io.O = d_dR;         // nuclear mode: dR [M][n_atoms][3], decremented by the AO part
-  {
-    qmc_system::Scratch &sc = s->scratch[st];  // (scratch_mu is held)
-    if (!sc.work) CK(cudaMalloc(&sc.work, sizeof(int)));
-    io.fb_count = sc.work;
-  }
-  CK(cudaMemsetAsync(io.fb_count, 0, sizeof(int), st));
   const int64_t groups = (M + s->P.G - 1) / s->P.G;
   const int grid = (int)std::min<int64_t>((groups + warps - 1) / warps, s->blocks_orb);
+  {
+    // scratch of the pair of launches: {work counter, list counter}; the listed groups' partial Gamma per work item of the
+    // explicit kernel (at most one item per warp of its grid when a group is sliced), the group list and slice counters
+    qmc_system::Scratch &sc = s->scratch[st];  // (scratch_mu is held)
+    if (!sc.work) CK(cudaMalloc(&sc.work, 2 * sizeof(int)));
+    io.fb_count = sc.work;
+    const size_t ps = (size_t)s->P.G * (size_t)s->P.n_e * (size_t)s->var.NMO + (size_t)s->P.G;
+    const size_t n_part = (size_t)s->blocks_orb * (size_t)warps * ps;
+    const size_t need = n_part * sizeof(double) + (size_t)(2 * groups) * sizeof(int);
+    if (sc.orb_bytes < need) {
+      if (sc.orb) s->retired.push_back(sc.orb);
+      sc.orb = nullptr;
+      sc.orb_bytes = 0;
+      CK(cudaMalloc(&sc.orb, need));
+      sc.orb_bytes = need;
+    }
+    io.fb_part = static_cast<double *>(sc.orb);
+    io.fb_list = reinterpret_cast<int *>(io.fb_part + n_part);
+    io.fb_done = io.fb_list + groups;
+  }
+  CK(cudaMemsetAsync(io.fb_count, 0, 2 * sizeof(int), st));
   void *args[2] = {(void *)&s->P, (void *)&io};
   CK(cudaLaunchKernel(kern, dim3(grid), dim3(warps * 32), args, smem, st));
-  ++g_launches;
+  const void *kx = d_dR ? (warps == kWarpsOrb ? s->var.x_nuc : s->var.x_nuc_small)
+                        : (warps == kWarpsOrb ? s->var.x_orb : s->var.x_orb_small);
+  CK(cudaLaunchKernel(kx, dim3(s->blocks_orb), dim3(warps * 32), args, smem, st));
+  g_launches += 2;
   return QMC_OK;
 }
 
@@ -1468,7 +1496,7 @@ int qmc_nuclear_energy_gradient(qmc_system_t *s, const double *d_r, int64_t M, d
   {
     std::lock_guard<std::mutex> lock(s->scratch_mu);
     qmc_system::Scratch &sc = s->scratch[st];
-    if (!sc.work) CK(cudaMalloc(&sc.work, sizeof(int)));
+    if (!sc.work) CK(cudaMalloc(&sc.work, 2 * sizeof(int)));
     io.fb_count = sc.work;
   }
   CK(cudaMemsetAsync(io.fb_count, 0, sizeof(int), st));

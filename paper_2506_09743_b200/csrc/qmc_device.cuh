@@ -152,8 +152,14 @@ constexpr double kFallbackKappa = QMC_FALLBACK_KAPPA;
 constexpr double kFallbackKappaCap = (QMC_FALLBACK_KAPPA > 1.0e100) ? QMC_FALLBACK_KAPPA : 1.0e10;
 // Orbital-parameter derivatives: the table-path error of Gamma is ~1.2e-15 (Sigma/D_0)^2 of the walker's largest
 // derivative (measured); beyond (Sigma/D_0)^2 = 1e4 the group takes the explicit route.
-constexpr double kFallbackOrb = 1.0e4;
-constexpr double kFallbackOrbKappa = 1.0e6;  // ... or kappa^2 beyond 1e6 (same conditioning estimate as E_L's)
+#ifndef QMC_FALLBACK_ORB
+#define QMC_FALLBACK_ORB 1.0e4
+#endif
+#ifndef QMC_FALLBACK_ORB_KAPPA
+#define QMC_FALLBACK_ORB_KAPPA 1.0e6
+#endif
+constexpr double kFallbackOrb = QMC_FALLBACK_ORB;
+constexpr double kFallbackOrbKappa = QMC_FALLBACK_ORB_KAPPA;  // ... or kappa^2 beyond 1e6 (same conditioning estimate as E_L's)
 
 // One term of Y[spin][p][q] = d(Sigma/D_0)/dT[p][q]: w * R_other * T_spin[cof]  (w = d_n times the cofactor's sign;
 // oth = the other spin's 2x2 code {i11, i12, i21, i22} as in class-4 DetRec, constant slots for k < 2;

@@ -228,87 +228,40 @@ __global__ void __launch_bounds__(WPB * 32, QMC_MINBLOCKS_EL)
 // a second pass over the shells that rebuilds phi and d phi / d zeta = phi (d ln N / d zeta - r) in the AO tile and
 // contracts them with Gamma.  Outputs travel in io.logpsi (dC) and io.eloc (dzeta); either may be null.
 // ---------------------------------------------------------------------------------
-// BF: backflow wavefunction (PAPER.md:53): phi, d phi / d zeta and d phi / d R are evaluated at the backflow coordinates, which
-// depend on none of these parameters; Gamma from the values-only evaluator at the same coordinates.
-template <int NS, int NMO, bool X, int WPB, bool NUC = false, bool BF = false>
-__global__ void __launch_bounds__(WPB * 32, 1)
-    orbital_derivatives_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
-  extern __shared__ __align__(16) unsigned char smem[];
-  const double *sC;
-  const double *sExp;
-  const DetRec *sDet;
-  double *wsBase;
-  load_constants<NMO>(P, smem, sC, sExp, sDet, wsBase);
+// Backflow coordinates of the lane's electron: rt_i = r_i + w sum_{j != i} (r_i - r_j) / r_ij over the other
+// electrons of its walker (walker g of the warp, electron e); the first 96 doubles of the warp's scratch must be free.
+__device__ __forceinline__ void backflow_lane_coords(double w, double *__restrict__ ws, int lane, int g, int e, int ne, double x,
+                                                     double y, double z, double &xo, double &yo, double &zo) {
+  ws[lane] = x; ws[32 + lane] = y; ws[64 + lane] = z;
+  __syncwarp();
+  const int base = g * ne;
+  double px = 0.0, py = 0.0, pz = 0.0;
+  for (int o = 1; o < ne; ++o) {
+    int j = e + o;
+    j -= (j >= ne) ? ne : 0;
+    const double ddx = x - ws[base + j], ddy = y - ws[32 + base + j], ddz = z - ws[64 + base + j];
+    const double ri = rsqrt_fast(fma(ddx, ddx, fma(ddy, ddy, ddz * ddz)));
+    px = fma(ddx, ri, px); py = fma(ddy, ri, py); pz = fma(ddz, ri, pz);
+  }
+  xo = fma(w, px, x); yo = fma(w, py, y); zo = fma(w, pz, z);
+  __syncwarp();
+}
+
+// The second pass of the orbital-derivative kernels for group grp, with the normalised Gamma [G][ne][NMO] of its walkers in
+// the warp's scratch (ws + oGam) and the lane's orbital position (xo, yo, zo): rebuilds phi and d phi / d zeta (nuclear mode:
+// d phi / d R) in the AO tile and contracts them with Gamma on the FP64 tensor cores.
+template <int NS, int NMO, bool X, bool NUC>
+__device__ __forceinline__ void orbital_second_pass(const SysParams &P, const WalkerIO &io, double *__restrict__ ws,
+                                                    const double *__restrict__ sC, const double *__restrict__ sExp, int lane,
+                                                    int64_t grp, double xo, double yo, double zo) {
   using GE = Geo<NS, NMO>;
   constexpr int S = GE::S2, NT = GE::NT;
-  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
-  double *ws = wsBase + warp * (GE::total + GE::orbExtra);
+  constexpr bool nuc = NUC;
   const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
-  const int g = lane / ne, e = lane - g * ne;
-  const int64_t n_groups = (io.M + G - 1) / G;
-  const int64_t stride = (int64_t)gridDim.x * WPB;
-  double *dC = io.logpsi, *dZ = io.eloc;
-  // nuclear mode (qmc_nuclear_log_gradient): io.O = dR [M][n_atoms][3]; d phi / d R_c = -d phi / d r_c takes the place of
-  // phi and d phi / d zeta in the two column sets of the tile: the second pass runs twice, (x, y) then z, and the
-  // contraction is summed over the rows of each centre
-  double *dRo = io.O;
-  constexpr bool nuc = NUC;  // its own instantiation: the parameter-derivative kernel keeps its code and registers
+  double *dC = io.logpsi, *dZ = io.eloc, *dRo = io.O;
   const int *row_atom = P.ao_orig + P.n_chunks * kChunk;
   double *sGam = ws + GE::oGam;
-  const double *sRes = ws + GE::oRes;
-  // The groups are dealt by an atomic counter (io.fb_count, zeroed by the host): a group on the explicit route costs tens of
-  // ordinary ones, and where such groups sit at regular distances a fixed assignment piles them onto the same warps
-  // (measured: 0.53 ms with 10 warps per block, 0.74 ms with 9 or 12 on the same walkers).
-  auto next_group = [&]() {
-    int v = 0;
-    if (lane == 0) v = atomicAdd(io.fb_count, 1);
-    return (int64_t)__shfl_sync(0xffffffffu, v, 0);
-  };
-  (void)stride;
-  for (int64_t grp = next_group(); grp < n_groups; grp = next_group()) {
-    const int64_t w = grp * G + g;
-    double x, y, z;
-    if ((g < G) && (w < io.M)) {
-      x = io.r_in[((int64_t)e * 3 + 0) * io.M + w];
-      y = io.r_in[((int64_t)e * 3 + 1) * io.M + w];
-      z = io.r_in[((int64_t)e * 3 + 2) * io.M + w];
-    } else {
-      dummy_xyz(lane, x, y, z);
-    }
-    // Gamma = d ln Sigma / d Phi from the reference's tables (one elimination per spin); when a walker of the group
-    // has (Sigma/D_0)^2 > kFallbackOrb (reference near-singular) or the expansion has general determinants, from every
-    // determinant's inverse instead: unnormalised Gamma and Sigma (sRes[4 g])
-    double xo = x, yo = y, zo = z;  // where this lane's orbitals sit
-    if (BF) {  // rt_i = r_i + w sum_{j != i} (r_i - r_j) / r_ij over the walker's other electrons (the scratch is free here)
-      ws[lane] = x; ws[32 + lane] = y; ws[64 + lane] = z;
-      __syncwarp();
-      const int base = ((lane < G * ne) ? g : 0) * ne;
-      double px = 0.0, py = 0.0, pz = 0.0;
-      for (int o = 1; o < ne; ++o) {
-        int j = e + o;
-        j -= (j >= ne) ? ne : 0;
-        const double ddx = x - ws[base + j], ddy = y - ws[32 + base + j], ddz = z - ws[64 + base + j];
-        const double ri = rsqrt_fast(fma(ddx, ddx, fma(ddy, ddy, ddz * ddz)));
-        px = fma(ddx, ri, px); py = fma(ddy, ri, py); pz = fma(ddz, ri, pz);
-      }
-      xo = fma(P.bf_w, px, x); yo = fma(P.bf_w, py, y); zo = fma(P.bf_w, pz, z);
-      __syncwarp();
-    }
-    bool expl = P.n_gen > 0;
-    if (!expl) {
-      eval_walkers<NS, NMO, false, X, false, false, false, 2, BF>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
-      for (int gg = 0; gg < G; ++gg) {
-        const double den = (ws + GE::oProb)[gg * 8 + 3];  // Sigma / D_0 of walker gg (NaN for a singular reference)
-        const double kap = (ws + GE::oProb)[gg * 8 + 7];  // max |T| over both spins
-        expl |= !(den * den <= kFallbackOrb) || !(kap * kap <= kFallbackOrbKappa);
-      }
-      __syncwarp();
-    }
-    if (expl) {
-      eval_walkers<NS, NMO, false, X, true, false, false, 1, BF>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
-      for (int i = lane; i < G * ne * NMO; i += 32) sGam[i] /= sRes[(i / (ne * NMO)) * 4 + 0];
-      __syncwarp();
-    }
+  {
     // second pass over the shells: phi into column lane, d phi / d zeta into column opCol(lane) of the tile
     double *const tile = ws;
     double *const tl = tile + lane, *const tz = tile + GE::opCol(lane);
@@ -542,6 +495,152 @@ __global__ void __launch_bounds__(WPB * 32, 1)
     }
     __syncwarp();
     }
+  }
+}
+
+// BF: backflow wavefunction (PAPER.md:53): phi, d phi / d zeta and d phi / d R are evaluated at the backflow coordinates, which
+// depend on none of these parameters; Gamma from the values-only evaluator at the same coordinates.
+template <int NS, int NMO, bool X, int WPB, bool NUC = false, bool BF = false>
+__global__ void __launch_bounds__(WPB * 32, 1)
+    orbital_derivatives_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const double *sC;
+  const double *sExp;
+  const DetRec *sDet;
+  double *wsBase;
+  load_constants<NMO>(P, smem, sC, sExp, sDet, wsBase);
+  using GE = Geo<NS, NMO>;
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
+  double *ws = wsBase + warp * (GE::total + GE::orbExtra);
+  const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
+  const int g = lane / ne, e = lane - g * ne;
+  const int64_t n_groups = (io.M + G - 1) / G;
+  // nuclear mode (qmc_nuclear_log_gradient): io.O = dR [M][n_atoms][3]; d phi / d R_c = -d phi / d r_c takes the place of
+  // phi and d phi / d zeta in the two column sets of the tile: the second pass runs twice, (x, y) then z, and the
+  // contraction is summed over the rows of each centre
+  // The groups are dealt by an atomic counter (io.fb_count, zeroed by the host): a group on the explicit route costs tens of
+  // ordinary ones, and where such groups sit at regular distances a fixed assignment piles them onto the same warps
+  // (measured: 0.53 ms with 10 warps per block, 0.74 ms with 9 or 12 on the same walkers).
+  auto next_group = [&]() {
+    int v = 0;
+    if (lane == 0) v = atomicAdd(io.fb_count, 1);
+    return (int64_t)__shfl_sync(0xffffffffu, v, 0);
+  };
+  for (int64_t grp = next_group(); grp < n_groups; grp = next_group()) {
+    const int64_t w = grp * G + g;
+    double x, y, z;
+    if ((g < G) && (w < io.M)) {
+      x = io.r_in[((int64_t)e * 3 + 0) * io.M + w];
+      y = io.r_in[((int64_t)e * 3 + 1) * io.M + w];
+      z = io.r_in[((int64_t)e * 3 + 2) * io.M + w];
+    } else {
+      dummy_xyz(lane, x, y, z);
+    }
+    // Gamma = d ln Sigma / d Phi from the reference's tables (one elimination per spin); when a walker of the group
+    // has (Sigma/D_0)^2 > kFallbackOrb (reference near-singular) or the expansion has general determinants, from every
+    // determinant's inverse instead: unnormalised Gamma and Sigma (sRes[4 g])
+    double xo = x, yo = y, zo = z;  // where this lane's orbitals sit
+    if (BF) backflow_lane_coords(P.bf_w, ws, lane, (lane < G * ne) ? g : 0, e, ne, x, y, z, xo, yo, zo);
+    bool expl = P.n_gen > 0;
+    if (!expl) {
+      eval_walkers<NS, NMO, false, X, false, false, false, 2, BF>(P, sExp, sC, sDet, ws, x, y, z, lane, 0, 1);
+      for (int gg = 0; gg < G; ++gg) {
+        const double den = (ws + GE::oProb)[gg * 8 + 3];  // Sigma / D_0 of walker gg (NaN for a singular reference)
+        const double kap = (ws + GE::oProb)[gg * 8 + 7];  // max |T| over both spins
+        expl |= !(den * den <= kFallbackOrb) || !(kap * kap <= kFallbackOrbKappa);
+      }
+      __syncwarp();
+    }
+    if (expl) {  // listed for orbital_explicit_kernel, which deals the determinants of such a group over several warps
+      if (lane == 0) {
+        const int idx = atomicAdd(io.fb_count + 1, 1);
+        io.fb_list[idx] = (int)grp;
+        io.fb_done[idx] = 0;
+      }
+      __syncwarp();
+      continue;
+    }
+    orbital_second_pass<NS, NMO, X, NUC>(P, io, ws, sC, sExp, lane, grp, xo, yo, zo);
+  }
+}
+
+// The groups orbital_derivatives_kernel listed (a walker with a nearly singular reference, or an expansion with general
+// determinants): Gamma from every determinant's own inverse.  Work item = (listed group, determinant slice), dealt over the
+// whole grid as in explicit_energy_kernel: every warp rebuilds the MO rows of its group and accumulates the unnormalised
+// Gamma and Sigma of its determinants; the warp that finishes a group last adds the partials in slice order
+// (deterministic), normalises and runs the second pass.  (One warp per group took 100 determinants in a row while the rest
+// of the grid waited: 0.19 of 0.53 ms for 32768 CO walkers.)
+template <int NS, int NMO, bool X, int WPB, bool NUC = false, bool BF = false>
+__global__ void __launch_bounds__(WPB * 32, 1)
+    orbital_explicit_kernel(const __grid_constant__ SysParams P, const WalkerIO io) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  const int n_list = io.fb_count[1];
+  if (n_list == 0) return;
+  const int total_warps = (int)gridDim.x * WPB;
+  int SL = total_warps / n_list;                       // slices per group
+  SL = min(SL, (P.n_det_all + 3) / 4);                 // at least ~4 determinants per slice
+  SL = max(SL, 1);
+  const int64_t n_items = (int64_t)n_list * SL;
+  if ((int64_t)blockIdx.x >= n_items) return;          // items are dealt block-first: nothing for this block
+  const double *sC;
+  const double *sExp;
+  const DetRec *sDet;
+  double *wsBase;
+  load_constants<NMO>(P, smem, sC, sExp, sDet, wsBase);
+  using GE = Geo<NS, NMO>;
+  const int warp = __shfl_sync(0xffffffffu, threadIdx.x >> 5, 0), lane = threadIdx.x & 31;
+  double *ws = wsBase + warp * (GE::total + GE::orbExtra);
+  const int ne = X ? 2 * NS : P.n_e, G = X ? GE::GMAX : P.G;
+  const int g = lane / ne, e = lane - g * ne;
+  double *sGam = ws + GE::oGam, *sRes = ws + GE::oRes;
+  const int nG = G * ne * NMO, PS = nG + G;            // a partial record: Gamma [G][ne][NMO], then Sigma per walker
+  for (int64_t item = (int64_t)warp * gridDim.x + blockIdx.x; item < n_items; item += total_warps) {
+    const int entry = (int)(item / SL), slice = (int)(item - (int64_t)entry * SL);
+    const int64_t grp = io.fb_list[entry];
+    const int64_t w = grp * G + g;
+    double x, y, z;
+    if ((g < G) && (w < io.M)) {
+      x = io.r_in[((int64_t)e * 3 + 0) * io.M + w];
+      y = io.r_in[((int64_t)e * 3 + 1) * io.M + w];
+      z = io.r_in[((int64_t)e * 3 + 2) * io.M + w];
+    } else {
+      dummy_xyz(lane, x, y, z);
+    }
+    double xo = x, yo = y, zo = z;
+    if (BF) backflow_lane_coords(P.bf_w, ws, lane, (lane < G * ne) ? g : 0, e, ne, x, y, z, xo, yo, zo);
+    eval_walkers<NS, NMO, false, X, true, false, false, 1, BF>(P, sExp, sC, sDet, ws, x, y, z, lane, slice, SL);
+    int last = 1;
+    if (SL > 1) {
+      double *part = io.fb_part + item * PS;
+      for (int i = lane; i < nG; i += 32) part[i] = sGam[i];
+      if (lane < G) part[nG + lane] = sRes[lane * 4 + 0];
+      __threadfence();
+      __syncwarp();  // every lane's partial is stored and fenced before lane 0 publishes the slice as done
+      int l = 0;
+      if (lane == 0) l = (atomicAdd(io.fb_done + entry, 1) == SL - 1) ? 1 : 0;
+      last = __shfl_sync(0xffffffffu, l, 0);
+      if (last) {
+        __threadfence();
+        const double *p0 = io.fb_part + (int64_t)entry * SL * PS;
+        for (int i = lane; i < nG; i += 32) {
+          double a = 0.0;
+          for (int sl = 0; sl < SL; ++sl) a += __ldcg(p0 + (int64_t)sl * PS + i);
+          sGam[i] = a;
+        }
+        if (lane < G) {
+          double a = 0.0;
+          for (int sl = 0; sl < SL; ++sl) a += __ldcg(p0 + (int64_t)sl * PS + nG + lane);
+          sRes[lane * 4 + 0] = a;
+        }
+        __syncwarp();
+      }
+    }
+    if (last) {
+      for (int i = lane; i < nG; i += 32) sGam[i] /= sRes[(i / (ne * NMO)) * 4 + 0];
+      __syncwarp();
+      orbital_second_pass<NS, NMO, X, NUC>(P, io, ws, sC, sExp, lane, grp, xo, yo, zo);
+    }
+    __syncwarp();
   }
 }
 

@@ -18,6 +18,8 @@ struct Variant {
   const void *k_orb_small;  // the same with kWarpsOrbSmall warps (less shared memory)
   const void *k_nuc, *k_nuc_small;  // the same kernel in nuclear mode (qmc_nuclear_log_gradient)
   const void *k_orb_b, *k_orb_small_b, *k_nuc_b, *k_nuc_small_b;  // the four for a backflow wavefunction
+  const void *x_orb, *x_orb_small, *x_nuc, *x_nuc_small;          // orbital_explicit_kernel for the groups those list
+  const void *x_orb_b, *x_orb_small_b, *x_nuc_b, *x_nuc_small_b;
   int orb_ws_doubles;
   const void *k_frc, *k_frc_small;  // nuclear energy gradient (8 / 4 warps per block)
   const void *k_el_fuse, *e_el_fuse;   // E_L + fused eq. 6 reduction (without / with the e-e-n kernel)
@@ -54,6 +56,14 @@ Variant make_variant() {
   v.k_orb_small_b = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrbSmall, false, true>;
   v.k_nuc_b = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrb, true, true>;
   v.k_nuc_small_b = (const void *)orbital_derivatives_kernel<NS, NMO, X, kWarpsOrbSmall, true, true>;
+  v.x_orb = (const void *)orbital_explicit_kernel<NS, NMO, X, kWarpsOrb>;
+  v.x_orb_small = (const void *)orbital_explicit_kernel<NS, NMO, X, kWarpsOrbSmall>;
+  v.x_nuc = (const void *)orbital_explicit_kernel<NS, NMO, X, kWarpsOrb, true>;
+  v.x_nuc_small = (const void *)orbital_explicit_kernel<NS, NMO, X, kWarpsOrbSmall, true>;
+  v.x_orb_b = (const void *)orbital_explicit_kernel<NS, NMO, X, kWarpsOrb, false, true>;
+  v.x_orb_small_b = (const void *)orbital_explicit_kernel<NS, NMO, X, kWarpsOrbSmall, false, true>;
+  v.x_nuc_b = (const void *)orbital_explicit_kernel<NS, NMO, X, kWarpsOrb, true, true>;
+  v.x_nuc_small_b = (const void *)orbital_explicit_kernel<NS, NMO, X, kWarpsOrbSmall, true, true>;
   v.orb_ws_doubles = Geo<NS, NMO>::total + Geo<NS, NMO>::orbExtra;
   v.k_frc = (const void *)nuclear_energy_gradient_kernel<NS, NMO, X, 8>;
   v.k_frc_small = (const void *)nuclear_energy_gradient_kernel<NS, NMO, X, 4>;
