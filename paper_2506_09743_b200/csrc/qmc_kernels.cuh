@@ -250,6 +250,10 @@ __device__ __forceinline__ void backflow_lane_coords(double w, double *__restric
 #ifndef QMC_NUC_DIRECT
 #define QMC_NUC_DIRECT 1
 #endif
+#ifndef QMC_FRC_DIRECT
+#define QMC_FRC_DIRECT 1
+#endif
+constexpr bool kFrcDirect = QMC_FRC_DIRECT != 0;  // nuclear energy gradient: the direct form of the second pass (0: the tile form)
 constexpr bool kNucDirect = QMC_NUC_DIRECT != 0;  // nuclear log-gradient: the direct form of orbital_second_pass (0: the tile form)
 
 // The second pass of the orbital-derivative kernels for group grp, with the normalised Gamma [G][ne][NMO] of its walkers in
@@ -901,6 +905,123 @@ __global__ void __launch_bounds__(WPB * 32, 1)
     }
     const double gJx = sGJ[lane], gJy = sGJ[32 + lane], gJz = sGJ[64 + lane];
     __syncwarp();
+    if (kFrcDirect) {
+      // Direct form (as the nuclear log-gradient's): lane = electron with its rows of G1 and G2 in registers, ONE pass over
+      // the shell records (exp once) with the value and operator tangents of all three components, the (N C) row read as
+      // broadcasts: dE[a][c] += sum_{beta on a} (w2 val_c + w1 op_c), w1,2 = sum_alpha G1,2[i][alpha] (N C)[beta][alpha],
+      // summed over the walker's electrons by shuffles where the centre changes.
+      const bool act = lane < G * ne;
+      double g1[NMO], g2[NMO];
+#pragma unroll
+      for (int c = 0; c < NMO; ++c) {
+        g1[c] = (act && c < P.n_mo) ? sGam[lane * NMO + c] : 0.0;
+        g2[c] = (act && c < P.n_mo) ? sGam2[lane * NMO + c] : 0.0;
+      }
+      int chunk = 0, cur = -1;
+      double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1.0, r = 1.0, ri = 1.0, q = 0.0;
+      double ax = 0.0, ay = 0.0, az = 0.0;
+      auto flush_centre = [&]() {
+        const int base = (act ? g : 0) * ne;
+        double tx = 0.0, ty = 0.0, tz2 = 0.0;
+        for (int j = 0; j < ne; ++j) {
+          tx += shfl_d(ax, base + j, 32);
+          ty += shfl_d(ay, base + j, 32);
+          tz2 += shfl_d(az, base + j, 32);
+        }
+        const int64_t wo = grp * G + g;
+        if (act && lane == base && wo < io.M && cur >= 0) {
+          double *o = dEo + (wo * P.n_atoms + cur) * 3;
+          o[0] += tx; o[1] += ty; o[2] += tz2;
+        }
+        ax = ay = az = 0.0;
+      };
+      for (int s = 0; s < P.n_shell; ++s) {
+        const ShellRec &sh = P.shells[s];
+        const int meta = sh.meta, kind = meta & 15;
+        if (kind == SH_POW) continue;
+        if (kind == SH_ATOM) {
+          dx = x - sh.zeta;
+          dy = y - sh.c1;
+          dz = z - sh.c2;
+          r2 = fma(dx, dx, fma(dy, dy, dz * dz));
+          ri = rsqrt_fast(r2);
+          r = r2 * ri;
+          q = fma(gJx, dx, fma(gJy, dy, gJz * dz)) * ri;
+          continue;
+        }
+        double f = exp_neg(-sh.zeta * r, sExp, P.mc);
+        if (meta & kMetaK1) f *= r;
+        if (meta & kMetaK2) f *= r2;
+        const double ux = dx * ri, uy = dy * ri, uz = dz * ri;
+        const double rho = fma(sh.kd, ri, -sh.zeta);
+        const double F2 = fma(rho, rho, -sh.kd * ri * ri);
+        const double lam = fma(fma(sh.c2, ri, -sh.c1), ri, sh.zeta * sh.zeta);
+        const double dlam = fma(-2.0 * sh.c2, ri, sh.c1) * ri * ri;
+        const int row = (meta >> 12) & 15, m = (meta >> 8) & 15;
+        double Sv[5], Sx[5], Sy[5], Sz[5], wx[5], wy[5], wz[5];
+        int nf = 1;
+        Sv[0] = 1.0; Sx[0] = Sy[0] = Sz[0] = 0.0; wx[0] = wy[0] = wz[0] = 0.0;
+        if (kind == SH_P || kind == SH_P1) {
+          const double pv[3] = {dx, dy, dz};
+          if (kind == SH_P) {
+            nf = 3;
+#pragma unroll
+            for (int t = 0; t < 3; ++t) { Sv[t] = pv[t]; Sx[t] = (t == 0); Sy[t] = (t == 1); Sz[t] = (t == 2); wx[t] = wy[t] = wz[t] = 0.0; }
+          } else {
+            Sv[0] = (m == 0) ? dx : ((m == 1) ? dy : dz);
+            Sx[0] = (m == 0); Sy[0] = (m == 1); Sz[0] = (m == 2);
+          }
+        } else if (kind == SH_D || kind == SH_D1) {
+          const double dS[5] = {dx * dy, dy * dz, dz * dx, fma(dx, dx, -dy * dy), fma(2.0 * dz, dz, -fma(dx, dx, dy * dy))};
+          const double dSx[5] = {dy, 0.0, dz, 2.0 * dx, -2.0 * dx};
+          const double dSy[5] = {dx, dz, 0.0, -2.0 * dy, -2.0 * dy};
+          const double dSz[5] = {0.0, dy, dx, 0.0, 4.0 * dz};
+          const double dwx[5] = {gJy, 0.0, gJz, 2.0 * gJx, -2.0 * gJx};
+          const double dwy[5] = {gJx, gJz, 0.0, -2.0 * gJy, -2.0 * gJy};
+          const double dwz[5] = {0.0, gJy, gJx, 0.0, 4.0 * gJz};
+          if (kind == SH_D) {
+            nf = 5;
+#pragma unroll
+            for (int t = 0; t < 5; ++t) { Sv[t] = dS[t]; Sx[t] = dSx[t]; Sy[t] = dSy[t]; Sz[t] = dSz[t]; wx[t] = dwx[t]; wy[t] = dwy[t]; wz[t] = dwz[t]; }
+          } else {
+#pragma unroll
+            for (int t = 0; t < 5; ++t)
+              if (t == m) { Sv[0] = dS[t]; Sx[0] = dSx[t]; Sy[0] = dSy[t]; Sz[0] = dSz[t]; wx[0] = dwx[t]; wy[0] = dwy[t]; wz[0] = dwz[t]; }
+          }
+        }
+        const double *cfr = sC + chunk * ((kChunk / 4) * NT * 32);
+#pragma unroll
+        for (int t = 0; t < 5; ++t) {
+          if (t < nf) {
+            const int rw = row + t, R = chunk * kChunk + rw;
+            const int at = row_atom[R];
+            if (at != cur) {  // uniform: every lane walks the same records
+              if (cur >= 0) flush_centre();
+              cur = at;
+            }
+            double w1 = 0.0, w2 = 0.0;
+#pragma unroll
+            for (int c = 0; c < NMO; ++c) {
+              const double cf = cfr[(((rw >> 2) * NT) + (c >> 3)) * 32 + 4 * (c & 7) + (rw & 3)];
+              w1 = fma(g1[c], cf, w1);
+              w2 = fma(g2[c], cf, w2);
+            }
+            const double gs = fma(gJx, Sx[t], fma(gJy, Sy[t], gJz * Sz[t]));
+            double val, op;
+            force_ao_pair<0>(f, Sv[t], Sx[t], Sy[t], Sz[t], wx[t], gs, ux, uy, uz, gJx, gJy, gJz, ri, rho, q, lam, dlam, F2, val, op);
+            ax = fma(w2, val, fma(w1, op, ax));
+            force_ao_pair<1>(f, Sv[t], Sx[t], Sy[t], Sz[t], wy[t], gs, ux, uy, uz, gJx, gJy, gJz, ri, rho, q, lam, dlam, F2, val, op);
+            ay = fma(w2, val, fma(w1, op, ay));
+            force_ao_pair<2>(f, Sv[t], Sx[t], Sy[t], Sz[t], wz[t], gs, ux, uy, uz, gJx, gJy, gJz, ri, rho, q, lam, dlam, F2, val, op);
+            az = fma(w2, val, fma(w1, op, az));
+          }
+        }
+        if (meta >> 20) ++chunk;
+      }
+      if (cur >= 0) flush_centre();
+      __syncwarp();
+      continue;
+    }
     double *const tile = ws;
     double *const tl = tile + lane, *const tz = tile + GE::opCol(lane);
 #pragma unroll 1
