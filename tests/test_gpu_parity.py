@@ -918,6 +918,40 @@ def test_orbital_derivatives_are_repeatable_bit_for_bit(env):
     s.close()
 
 
+def test_orbital_derivatives_full_size_sampled_euler_identity_and_repeatability(env):
+    """32768 CO walkers (the size bench.py times the call on), the seeded batch and the same walkers after 60 sweeps of this
+    library's sampler (where nearly all walkers sit in the criterion set and the groups with a nearly singular reference go
+    through orbital_explicit_kernel in determinant slices): a sample of the seeded batch against the oracle (dC and dzeta),
+    Euler's identity sum C d ln Psi / d C = N_e on every walker of both batches, bit-repeatability at this size."""
+    torch, ob, qb = env
+    from tests.helpers import adjudicate
+    d, r = wl.co(M=32768)
+    s = qb.QmcSystem(d)
+    rg = _to_gpu(torch, r)
+    Ct = torch.from_numpy(np.asarray(d.mo_coeff, np.float64)).cuda()
+    for stage in range(2):
+        if stage == 1:
+            s.metropolis(rg, 0.2, 60, seed=77)
+        dC, dz = s.orbital_derivatives(rg, d.n_ao, d.n_mo)
+        dC2, dz2 = s.orbital_derivatives(rg, d.n_ao, d.n_mo)
+        assert torch.equal(dC, dC2) and torch.equal(dz, dz2)
+        lp = s.log_psi(rg)[0]
+        keep = lp - lp.max() > math.log(1e-6)
+        euler = (dC * Ct[None]).sum(dim=(1, 2))
+        scale = (dC * Ct[None]).abs().amax(dim=(1, 2)).clamp(min=1.0)
+        assert float(((euler - d.n_e).abs() / scale)[keep].max()) < 1e-8, stage
+        if stage == 0:
+            idx = np.random.default_rng(9).choice(np.flatnonzero(keep.cpu().numpy()), 192, replace=False)
+            rs = np.ascontiguousarray(r[:, :, idx])
+            o, ox = ob.OracleSystem(d), ob.OracleSystem(d, extended=True)
+            dC0, dz0 = ob.orbital_derivatives(o, rs, threads=8)
+            dCx, dzx = ob.orbital_derivatives(ox, rs, threads=8)
+            it = torch.from_numpy(idx).cuda()
+            adjudicate(dC[it].cpu().numpy(), dC0, dCx, 1e-8, scale=np.maximum(1.0, np.abs(dCx)), what="dC at full size")
+            adjudicate(dz[it].cpu().numpy(), dz0, dzx, 1e-8, scale=np.maximum(1.0, np.abs(dzx)), what="dzeta at full size")
+    s.close()
+
+
 # ----------------------------------------------------------------------------- nuclear log-gradient (eq. 7, PAPER.md:84-89)
 def check_nuclear_log_gradient(env, d, r, threads=8):
     torch, ob, qb = env
